@@ -1,0 +1,182 @@
+"""ctypes wrapper around the C++ oracle (hlb_oracle.cpp, hlb_oracle_dense.cpp).
+
+TEST INFRASTRUCTURE ONLY -- see the package docstring. Argument marshalling and the g++
+build; no arithmetic of the method lives here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liboracle.so")
+_SOURCES = [os.path.join(_HERE, "hlb_oracle.cpp"), os.path.join(_HERE, "hlb_oracle_dense.cpp")]
+_lock = threading.Lock()
+_lib = None
+
+VARIANT_SHIFTED, VARIANT_RAW, VARIANT_SHIFTED_LD, VARIANT_RAW_LD = 0, 1, 2, 3
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ -O2 (no -ffast-math, no -march: plain IEEE double,
+    no FMA contraction) into oracle/liboracle.so."""
+    newest = max(os.path.getmtime(s) for s in _SOURCES)
+    if not force and os.path.exists(_LIB_PATH) and os.path.getmtime(_LIB_PATH) >= newest:
+        return _LIB_PATH
+    tmp = _LIB_PATH + f".tmp{os.getpid()}"
+    cmd = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+           "-Wall", "-Wextra", "-o", tmp] + _SOURCES
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _LIB_PATH)
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    with _lock:
+        if _lib is not None:
+            return _lib
+        build()
+        lib = ctypes.CDLL(_LIB_PATH)
+        c_dp = ctypes.POINTER(ctypes.c_double)
+        lib.hlbo_create.restype = ctypes.c_void_p
+        lib.hlbo_create.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                    ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
+                                    ctypes.c_int]
+        lib.hlbo_destroy.argtypes = [ctypes.c_void_p]
+        lib.hlbo_destroy.restype = None
+        for name in ("hlbo_num_sites", "hlbo_steps_done"):
+            getattr(lib, name).restype = ctypes.c_int64
+            getattr(lib, name).argtypes = [ctypes.c_void_p]
+        lib.hlbo_site_voxels.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_set_state.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_set_populations.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_get_populations.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_step.argtypes = [ctypes.c_void_p, ctypes.c_int64]
+        lib.hlbo_get_macroscopic.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_velocity_set.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_set_threads.argtypes = [ctypes.c_int]
+        lib.hlbo_get_threads.restype = ctypes.c_int
+        lib.hlbd_run.restype = ctypes.c_int
+        lib.hlbd_run.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                 ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
+                                 ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                                 ctypes.c_void_p, ctypes.c_void_p]
+        for name in ("hlbo_site_voxels", "hlbo_set_state", "hlbo_set_populations",
+                     "hlbo_get_populations", "hlbo_step", "hlbo_get_macroscopic",
+                     "hlbo_velocity_set", "hlbo_set_threads"):
+            getattr(lib, name).restype = None
+        del c_dp
+        _lib = lib
+        return lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def velocity_set():
+    """(c[15,3] int32, w[15] float64, opp[15] int32) in the oracle's own q order."""
+    lib = _load()
+    c = np.zeros((15, 3), dtype=np.int32)
+    w = np.zeros(15, dtype=np.float64)
+    opp = np.zeros(15, dtype=np.int32)
+    lib.hlbo_velocity_set(_ptr(c), _ptr(w), _ptr(opp))
+    return c, w, opp
+
+
+class Oracle:
+    """One oracle simulation. Per-site arrays are in canonical order (ascending voxel)."""
+
+    def __init__(self, site_type, periodic=0, tau=1.0, iolet_rho=(), variant=VARIANT_SHIFTED,
+                 threads=1):
+        lib = _load()
+        st = np.ascontiguousarray(site_type, dtype=np.uint8)
+        assert st.ndim == 3
+        nz, ny, nx = st.shape
+        io = np.ascontiguousarray(np.asarray(iolet_rho, dtype=np.float64))
+        lib.hlbo_set_threads(int(threads))
+        self._lib = lib
+        self._h = lib.hlbo_create(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
+                                  _ptr(io), int(variant))
+        if not self._h:
+            raise ValueError("hlbo_create rejected its arguments")
+        self.n_sites = int(lib.hlbo_num_sites(self._h))
+        self.threads = int(lib.hlbo_get_threads())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.hlbo_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def site_voxels(self):
+        v = np.zeros(self.n_sites, dtype=np.int64)
+        self._lib.hlbo_site_voxels(self._h, _ptr(v))
+        return v
+
+    def set_state(self, rho=None, u=None):
+        rho = None if rho is None else np.ascontiguousarray(rho, dtype=np.float64)
+        u = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
+        if rho is not None:
+            assert rho.shape == (self.n_sites,)
+        if u is not None:
+            assert u.shape == (self.n_sites, 3)
+        self._lib.hlbo_set_state(self._h, _ptr(rho), _ptr(u))
+
+    def set_populations(self, f):
+        f = np.ascontiguousarray(f, dtype=np.float64)
+        assert f.shape == (self.n_sites, 15)
+        self._lib.hlbo_set_populations(self._h, _ptr(f))
+
+    def get_populations(self):
+        f = np.zeros((self.n_sites, 15), dtype=np.float64)
+        self._lib.hlbo_get_populations(self._h, _ptr(f))
+        return f
+
+    def step(self, n=1):
+        self._lib.hlbo_set_threads(self.threads)
+        self._lib.hlbo_step(self._h, int(n))
+
+    def steps_done(self):
+        return int(self._lib.hlbo_steps_done(self._h))
+
+    def get_macroscopic(self):
+        rho = np.zeros(self.n_sites, dtype=np.float64)
+        u = np.zeros((self.n_sites, 3), dtype=np.float64)
+        self._lib.hlbo_get_macroscopic(self._h, _ptr(rho), _ptr(u))
+        return rho, u
+
+
+def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1):
+    """Run a workloads.Workload for ``steps`` (default: its own count); returns rho, u."""
+    o = Oracle(workload.site_type, workload.periodic, workload.tau, workload.iolet_rho,
+               variant=variant, threads=threads)
+    if workload.rho0 is not None or workload.u0 is not None:
+        o.set_state(workload.rho0, workload.u0)
+    o.step(workload.steps if steps is None else steps)
+    out = o.get_macroscopic()
+    o.close()
+    return out
+
+
+def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None):
+    """Dense-grid twin: per-VOXEL rho [nz,ny,nx] and u [nz,ny,nx,3]."""
+    lib = _load()
+    st = np.ascontiguousarray(site_type, dtype=np.uint8)
+    nz, ny, nx = st.shape
+    io = np.ascontiguousarray(np.asarray(iolet_rho, dtype=np.float64))
+    r0 = None if rho0_vox is None else np.ascontiguousarray(rho0_vox, dtype=np.float64)
+    u0 = None if u0_vox is None else np.ascontiguousarray(u0_vox, dtype=np.float64)
+    rho = np.zeros((nz, ny, nx), dtype=np.float64)
+    u = np.zeros((nz, ny, nx, 3), dtype=np.float64)
+    rc = lib.hlbd_run(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]), _ptr(io),
+                      _ptr(r0), _ptr(u0), int(steps), _ptr(rho), _ptr(u))
+    if rc != 0:
+        raise ValueError("hlbd_run rejected its arguments")
+    return rho, u

@@ -1,0 +1,405 @@
+"""Pins for the oracle (oracle/hlb_oracle.cpp): things the mathematics fixes.
+
+The paper (arxiv 1906.11925) prints no flow values, so none of these is a paper number;
+each is a closed form, an invariant, a brute-force twin or a special case, chosen so that
+a dropped term, a wrong sign/index or a transposed direction fails at least one.
+Numbering P1..P12 follows SURVEY.md §8(c) "What pins the oracle".
+"""
+import itertools
+import math
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+
+C, WT, OPP = oracle.velocity_set()
+
+
+def canon_coords(st):
+    nz, ny, nx = st.shape
+    v = np.flatnonzero(st.reshape(-1) == 1)
+    return v % nx, (v // nx) % ny, v // (nx * ny)
+
+
+# ------------------------------------------------------------------ P1 lattice identities
+def test_p1_velocity_set_is_d3q15():
+    vecs = {tuple(int(a) for a in c) for c in C}
+    assert len(vecs) == 15
+    assert (0, 0, 0) in vecs
+    axis = {v for v in vecs if sum(abs(a) for a in v) == 1}
+    diag = {v for v in vecs if all(abs(a) == 1 for a in v)}
+    assert len(axis) == 6 and len(diag) == 8
+    w = [Fraction(float(x)).limit_denominator(1000) for x in WT]
+    for c, wq in zip(C, w):
+        n2 = int(np.dot(c, c))
+        assert wq == {0: Fraction(2, 9), 1: Fraction(1, 9), 3: Fraction(1, 72)}[n2]
+    assert sum(w) == 1
+
+
+def test_p1_moment_identities():
+    w = [Fraction(float(x)).limit_denominator(1000) for x in WT]
+    c = [[int(a) for a in q] for q in C]
+    d = lambda a, b: 1 if a == b else 0
+    for a in range(3):
+        assert sum(w[q] * c[q][a] for q in range(15)) == 0
+        for b in range(3):
+            assert sum(w[q] * c[q][a] * c[q][b] for q in range(15)) == Fraction(d(a, b), 3)
+            for e in range(3):
+                assert sum(w[q] * c[q][a] * c[q][b] * c[q][e] for q in range(15)) == 0
+                for g in range(3):
+                    iso = Fraction(d(a, b) * d(e, g) + d(a, e) * d(b, g) + d(a, g) * d(b, e), 9)
+                    assert sum(w[q] * c[q][a] * c[q][b] * c[q][e] * c[q][g]
+                               for q in range(15)) == iso
+
+
+def test_p1_opposites():
+    for q in range(15):
+        assert OPP[OPP[q]] == q
+        assert np.array_equal(C[OPP[q]], -C[q])
+        assert WT[OPP[q]] == WT[q]
+
+
+# ------------------------------------------------------------------ P2 rest state
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_p2_rest_state_is_bitwise_invariant(seed):
+    wl = W.random_mask((9, 8, 7), p_fluid=0.55, n_iolets=2, seed=seed)
+    o = oracle.Oracle(wl.site_type, 0, 0.7, [1.0, 1.0])     # iolets at rho = 1: still at rest
+    o.step(40)
+    rho, u = o.get_macroscopic()
+    assert np.all(rho == 1.0)
+    assert np.all(u == 0.0)
+
+
+# ------------------------------------------------------------------ P3 uniform flow
+def test_p3_uniform_flow_is_a_fixed_point():
+    st = np.ones((5, 6, 7), dtype=np.uint8)
+    o = oracle.Oracle(st, 7, 0.83, [])
+    n = o.n_sites
+    rho0 = np.full(n, 1.03)
+    u0 = np.tile(np.array([0.02, -0.01, 0.03]), (n, 1))
+    o.set_state(rho0, u0)
+    o.step(25)
+    rho, u = o.get_macroscopic()
+    assert np.max(np.abs(rho - 1.03)) < 1e-15
+    assert np.max(np.abs(u - u0)) < 1e-16
+
+
+# ------------------------------------------------------------------ P4/P5 conservation
+def test_p4_p5_mass_and_momentum_conserved_periodic():
+    wl = W.random_mask((8, 7, 6), p_fluid=1.1, n_iolets=0, periodic=7, seed=5)
+    o = oracle.Oracle(wl.site_type, 7, 0.62, [])
+    o.set_state(wl.rho0, wl.u0)
+    r0, u0 = o.get_macroscopic()
+    m0, j0 = r0.sum(), (r0[:, None] * u0).sum(axis=0)
+    o.step(200)
+    r1, u1 = o.get_macroscopic()
+    assert abs(r1.sum() - m0) / o.n_sites < 1e-15
+    assert np.max(np.abs((r1[:, None] * u1).sum(axis=0) - j0)) / o.n_sites < 1e-16
+    assert np.max(np.abs(u1 - u0)) > 1e-4        # something did happen
+
+
+def test_p4_mass_conserved_with_walls():
+    wl = W.random_mask((9, 8, 7), p_fluid=0.6, n_iolets=0, periodic=2, seed=11)
+    o = oracle.Oracle(wl.site_type, 2, 0.9, [])
+    o.set_state(wl.rho0, wl.u0)
+    m0 = o.get_macroscopic()[0].sum()
+    o.step(150)
+    assert abs(o.get_macroscopic()[0].sum() - m0) / o.n_sites < 1e-15
+
+
+# ------------------------------------------------------------------ pure streaming
+@pytest.mark.parametrize("q", range(15))
+def test_streaming_moves_a_marked_population_along_c(q):
+    """tau = 1e30 switches collision off (f* = f exactly in fp64); a marked population in
+    slot q at x0 must be found in slot q at x0 + n c_q (periodic wrap) and nowhere else."""
+    nx, ny, nz = 5, 4, 3
+    st = np.ones((nz, ny, nx), dtype=np.uint8)
+    o = oracle.Oracle(st, 7, 1e30, [])
+    f = np.tile(WT, (o.n_sites, 1))
+    x0 = (1, 2, 0)
+    i0 = (x0[2] * ny + x0[1]) * nx + x0[0]
+    f[i0, q] += 0.125
+    o.set_populations(f)
+    n = 7
+    o.step(n)
+    g = o.get_populations()
+    x1 = ((x0[0] + n * C[q][0]) % nx, (x0[1] + n * C[q][1]) % ny, (x0[2] + n * C[q][2]) % nz)
+    i1 = (x1[2] * ny + x1[1]) * nx + x1[0]
+    expect = np.tile(WT, (o.n_sites, 1))
+    expect[i1, q] += 0.125
+    assert np.array_equal(g, expect)
+
+
+def test_streaming_bounces_back_half_way():
+    """1-D channel x = 0..3, outside solid: a population moving +x from x = 1 is at x = 2,
+    x = 3 after 1, 2 steps, then reversed in the opposite slot at x = 3 (the wall sits
+    half a link beyond x = 3), then at x = 2 moving -x."""
+    st = np.ones((1, 1, 4), dtype=np.uint8)
+    o = oracle.Oracle(st, 0, 1e30, [])
+    qp = [q for q in range(15) if tuple(C[q]) == (1, 0, 0)][0]
+    qm = OPP[qp]
+    base = np.tile(WT, (4, 1))
+    # y/z links all bounce back onto the same site, so the base state is stationary
+    f = base.copy()
+    f[1, qp] += 0.25
+    o.set_populations(f)
+    where = []
+    for _ in range(5):
+        o.step(1)
+        d = o.get_populations() - base
+        (i,), (q,) = np.nonzero(d)[0], np.nonzero(d)[1]
+        assert d[i, q] == 0.25
+        where.append((int(i), int(q)))
+    assert where == [(2, qp), (3, qp), (3, qm), (2, qm), (1, qm)]
+
+
+# ------------------------------------------------------------------ relaxation rate
+@pytest.mark.parametrize("tau", [0.6, 1.0, 1.7])
+def test_non_equilibrium_part_decays_by_one_minus_one_over_tau(tau):
+    """1x1x1 periodic box: every neighbour is the site itself, so streaming is the identity
+    and a mass- and momentum-free perturbation decays exactly as (1 - 1/tau)^n."""
+    st = np.ones((1, 1, 1), dtype=np.uint8)
+    o = oracle.Oracle(st, 7, tau, [])
+    qx = [q for q in range(15) if tuple(C[q]) == (1, 0, 0)][0]
+    q0 = [q for q in range(15) if tuple(C[q]) == (0, 0, 0)][0]
+    pert = np.zeros(15)
+    pert[qx] = pert[OPP[qx]] = 1e-3
+    pert[q0] = -2e-3
+    o.set_populations((WT + pert)[None, :])
+    n = 9
+    o.step(n)
+    got = o.get_populations()[0] - WT
+    assert np.max(np.abs(got - (1.0 - 1.0 / tau) ** n * pert)) < 1e-16   # ulp(w_0) = 2.8e-17
+
+
+# ------------------------------------------------------------------ P6 shear wave
+@pytest.mark.parametrize("tau", [0.6, 0.8, 1.2])
+def test_p6_shear_wave_decays_at_nu(tau):
+    ny = 64
+    st = np.ones((1, ny, 1), dtype=np.uint8)
+    o = oracle.Oracle(st, 7, tau, [])
+    k = 2 * math.pi / ny
+    u0 = np.zeros((ny, 3))
+    u0[:, 0] = 1e-3 * np.sin(k * np.arange(ny))
+    o.set_state(np.ones(ny), u0)
+    T = 300
+    o.step(T)
+    _, u = o.get_macroscopic()
+    amp = 2.0 / ny * np.dot(u[:, 0], np.sin(k * np.arange(ny)))
+    nu = (tau - 0.5) / 3.0
+    assert amp / 1e-3 == pytest.approx(math.exp(-nu * k * k * T), rel=4e-3)
+    assert np.max(np.abs(u[:, 1:])) < 1e-15
+
+
+# ------------------------------------------------------------------ P7 Taylor-Green
+def test_p7_taylor_green_kinetic_energy_decay():
+    wl = W.periodic_cube(n=32, tau=0.6, u0=0.01, nz=1)
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, [])
+    o.set_state(wl.rho0, wl.u0)
+    ke = []
+    for _ in range(4):
+        r, u = o.get_macroscopic()
+        ke.append(0.5 * np.sum(r[:, None] * u * u))
+        o.step(100)
+    nu, k = (0.6 - 0.5) / 3.0, wl.info["k"]
+    expect = math.exp(-4.0 * nu * k * k * 100)          # KE ~ exp(-4 nu k^2 t)
+    for a, b in zip(ke[1:-1], ke[2:]):                   # skip the first (acoustic transient)
+        assert b / a == pytest.approx(expect, rel=1e-3)
+    assert ke[1] / ke[0] == pytest.approx(expect, rel=2e-2)   # start-up transient (rho = 1, f = feq)
+
+
+# ------------------------------------------------------------------ P8 Poiseuille
+@pytest.mark.parametrize("tau", [0.5 + math.sqrt(3.0 / 16.0), 0.9, 0.6])
+def test_p8_plane_poiseuille_between_bounce_back_walls(tau):
+    """Channel of H fluid rows between solid rows, periodic in x, density iolets in z.
+    LBGK with halfway bounce-back has a closed-form steady solution (He, Zou, Luo & Dembo
+    1997): the walls sit at y = 1/2 and y = H + 1/2 and the parabola carries a uniform
+    numerical slip,
+        u_z(y) = G/(2 nu) [ (y - 1/2)(H + 1/2 - y) + (16 (tau - 1/2)^2 - 3) / 12 ],
+    which vanishes at tau = 1/2 + sqrt(3/16). G = -(1/3) d rho/dz is measured on the
+    developed mid-section (the iolet rule A6 has an entrance layer, so the nominal
+    (rho_in - rho_out)/(3L) is only approached to 7-25 %)."""
+    H, L = 11, 24
+    st = np.zeros((L + 2, H + 2, 1), dtype=np.uint8)
+    st[1:L + 1, 1:H + 1, 0] = 1
+    st[0, 1:H + 1, 0] = 2
+    st[L + 1, 1:H + 1, 0] = 3
+    o = oracle.Oracle(st, 1, tau, [1.0005, 0.9995], threads=4)
+    o.step(8000)
+    rho, u = o.get_macroscopic()
+    x, y, z = canon_coords(st)
+    za, zb = 9, 16
+    G = (rho[z == za].mean() - rho[z == zb].mean()) / (3.0 * (zb - za))
+    nu = (tau - 0.5) / 3.0
+    assert G == pytest.approx(0.001 / (3.0 * L), rel=0.30) and G > 0      # flows inlet -> outlet
+    mid = z == (L // 2)
+    yy = y[mid].astype(float)
+    slip = (16.0 * (tau - 0.5) ** 2 - 3.0) / 12.0
+    expect = G / (2.0 * nu) * ((yy - 0.5) * (H + 0.5 - yy) + slip)
+    got = (rho * u[:, 2])[mid]
+    assert np.max(np.abs(got / expect - 1.0)) < 2.5e-3
+    assert np.max(np.abs(u[mid, 0])) < 1e-12 and np.max(np.abs(u[mid, 1])) < 1e-5
+
+
+def test_p8_pipe_poiseuille_config0():
+    """BASELINE configs[0] geometry run to steady state (200 steps is not
+    steady). u_max = G R^2 / (4 nu) = 1.6667e-3; staircase wall => loose tolerances."""
+    wl = W.pipe()
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, threads=4)
+    o.step(2500)
+    rho, u = o.get_macroscopic()
+    x, y, z = canon_coords(wl.site_type)
+    R, L, nu = 8.0, 64.0, (wl.tau - 0.5) / 3.0
+    G = (wl.iolet_rho[0] - wl.iolet_rho[1]) / (3.0 * L)
+    umax = G * R * R / (4.0 * nu)
+    centre = (z == 32) & (x == 8) & (y == 8)
+    assert u[centre, 2][0] == pytest.approx(umax, rel=0.02)
+    line = (z == 32) & (y == 8)
+    r = np.abs(x[line] - 8.0)
+    expect = G * (R * R - r * r) / (4.0 * nu)
+    got = u[line, 2]
+    assert np.linalg.norm(got - expect) / np.linalg.norm(expect) < 0.10
+    assert np.max(np.abs(got - got[::-1])) < 1e-12                  # mirror symmetric
+    assert np.all(got > 0)
+
+
+# ------------------------------------------------------------------ P9 dense twin
+@pytest.mark.parametrize("seed,periodic,shape", [
+    (0, 0, (7, 6, 5)), (1, 7, (6, 6, 6)), (2, 1, (12, 5, 4)), (3, 2, (4, 9, 5)),
+    (4, 4, (5, 4, 11)), (5, 5, (8, 3, 7)), (6, 0, (12, 12, 12)), (7, 7, (1, 1, 3)),
+    (8, 3, (2, 2, 2)),
+])
+def test_p9_dense_push_twin_equals_sparse_pull(seed, periodic, shape):
+    wl = W.random_mask(shape, p_fluid=0.6, n_iolets=3, p_iolet=0.08, periodic=periodic,
+                       tau=0.5 + 0.1 * (1 + seed), seed=100 + seed)
+    steps = 12
+    st = wl.site_type
+    vox = wl.fluid_voxels()
+    nvox = st.size
+    rho0v = np.ones(nvox)
+    u0v = np.zeros((nvox, 3))
+    rho0v[vox] = wl.rho0
+    u0v[vox] = wl.u0
+    rd, ud = oracle.dense_run(st, periodic, wl.tau, wl.iolet_rho, steps, rho0v, u0v)
+    rd, ud = rd.reshape(-1)[vox], ud.reshape(-1, 3)[vox]
+    for variant, tol in ((oracle.VARIANT_RAW, 2e-15), (oracle.VARIANT_SHIFTED, 2e-14)):
+        o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, variant=variant)
+        assert np.array_equal(o.site_voxels(), vox)
+        o.set_state(wl.rho0, wl.u0)
+        o.step(steps)
+        r, u = o.get_macroscopic()
+        assert np.max(np.abs(r - rd)) < tol
+        assert np.max(np.abs(u - ud)) < tol
+
+
+# ------------------------------------------------------------------ P11 symmetry
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_p11_mirror_symmetry(axis):
+    wl = W.random_mask((7, 6, 5), p_fluid=0.65, n_iolets=2, seed=42)
+    st = wl.site_type
+    np_axis = 2 - axis                     # array is [z, y, x]
+    st_m = np.ascontiguousarray(np.flip(st, axis=np_axis))
+    nz, ny, nx = st.shape
+    # scatter canonical fields to voxel grids, flip, gather back in the mirrored canonical order
+    vox = wl.fluid_voxels()
+    rho_v = np.zeros(st.size)
+    u_v = np.zeros((st.size, 3))
+    rho_v[vox] = wl.rho0
+    u_v[vox] = wl.u0
+    rho_m = np.flip(rho_v.reshape(nz, ny, nx), axis=np_axis).reshape(-1)
+    u_m = np.flip(u_v.reshape(nz, ny, nx, 3), axis=np_axis).reshape(-1, 3).copy()
+    u_m[:, axis] *= -1.0
+    vox_m = np.flatnonzero(st_m.reshape(-1) == 1)
+    a = oracle.Oracle(st, 0, wl.tau, wl.iolet_rho)
+    a.set_state(wl.rho0, wl.u0)
+    b = oracle.Oracle(st_m, 0, wl.tau, wl.iolet_rho)
+    b.set_state(rho_m[vox_m], u_m[vox_m])
+    a.step(15)
+    b.step(15)
+    ra, ua = a.get_macroscopic()
+    rb, ub = b.get_macroscopic()
+    ra_v = np.zeros(st.size)
+    ua_v = np.zeros((st.size, 3))
+    ra_v[vox] = ra
+    ua_v[vox] = ua
+    ra_m = np.flip(ra_v.reshape(nz, ny, nx), axis=np_axis).reshape(-1)[vox_m]
+    ua_m = np.flip(ua_v.reshape(nz, ny, nx, 3), axis=np_axis).reshape(-1, 3)[vox_m].copy()
+    ua_m[:, axis] *= -1.0
+    assert np.max(np.abs(rb - ra_m)) < 1e-15
+    assert np.max(np.abs(ub - ua_m)) < 1e-16
+
+
+def test_p11_axis_permutation_symmetry():
+    """Swapping the x and z axes of geometry and state swaps them in the result."""
+    wl = W.random_mask((6, 5, 4), p_fluid=0.7, n_iolets=1, seed=9)
+    st = wl.site_type
+    st_p = np.ascontiguousarray(st.transpose(2, 1, 0))          # [x, y, z] as new [z, y, x]
+    vox = wl.fluid_voxels()
+    nz, ny, nx = st.shape
+    rho_v = np.zeros(st.size)
+    u_v = np.zeros((st.size, 3))
+    rho_v[vox] = wl.rho0
+    u_v[vox] = wl.u0
+    rho_p = rho_v.reshape(nz, ny, nx).transpose(2, 1, 0).reshape(-1)
+    u_p = u_v.reshape(nz, ny, nx, 3).transpose(2, 1, 0, 3).reshape(-1, 3)[:, ::-1]
+    vox_p = np.flatnonzero(st_p.reshape(-1) == 1)
+    a = oracle.Oracle(st, 0, wl.tau, wl.iolet_rho)
+    a.set_state(wl.rho0, wl.u0)
+    b = oracle.Oracle(st_p, 0, wl.tau, wl.iolet_rho)
+    b.set_state(rho_p[vox_p], np.ascontiguousarray(u_p[vox_p]))
+    a.step(10)
+    b.step(10)
+    ra, ua = a.get_macroscopic()
+    rb, ub = b.get_macroscopic()
+    ra_v = np.zeros(st.size)
+    ua_v = np.zeros((st.size, 3))
+    ra_v[vox] = ra
+    ua_v[vox] = ua
+    ra_p = ra_v.reshape(nz, ny, nx).transpose(2, 1, 0).reshape(-1)[vox_p]
+    ua_p = ua_v.reshape(nz, ny, nx, 3).transpose(2, 1, 0, 3).reshape(-1, 3)[vox_p][:, ::-1]
+    assert np.max(np.abs(rb - ra_p)) < 1e-15
+    assert np.max(np.abs(ub - ua_p)) < 1e-16
+
+
+# ------------------------------------------------------------------ P12 roundoff yardstick
+def test_p12_long_double_twin_bounds_the_oracles_roundoff():
+    wl = W.periodic_cube(n=16, tau=0.6, u0=0.01, nz=2)
+    res = {}
+    for v in (oracle.VARIANT_SHIFTED, oracle.VARIANT_RAW, oracle.VARIANT_SHIFTED_LD,
+              oracle.VARIANT_RAW_LD):
+        o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, [], variant=v)
+        o.set_state(wl.rho0, wl.u0)
+        o.step(300)
+        res[v] = o.get_macroscopic()
+    ref_r, ref_u = res[oracle.VARIANT_SHIFTED_LD]
+    umax = np.max(np.linalg.norm(ref_u, axis=1))
+
+    def err(v):
+        r, u = res[v]
+        return np.max(np.abs(r - ref_r)), np.max(np.abs(u - ref_u)) / umax
+
+    e_rho, e_u = err(oracle.VARIANT_SHIFTED)
+    assert e_rho < 1e-15 and e_u < 5e-14          # the oracle: orders below the 1e-12 budget
+    e_rho, e_u = err(oracle.VARIANT_RAW)
+    assert e_rho < 1e-13 and e_u < 1e-11          # raw f: same iteration, roundoff near 1e-12
+    e_rho, e_u = err(oracle.VARIANT_RAW_LD)
+    assert e_rho < 1e-15 and e_u < 1e-13
+
+
+# ------------------------------------------------------------------ degenerate cases
+def test_isolated_site_and_argument_checks():
+    st = np.zeros((3, 3, 3), dtype=np.uint8)
+    st[1, 1, 1] = 1
+    o = oracle.Oracle(st, 0, 0.8, [])
+    o.set_state(np.array([1.01]), np.array([[0.01, 0.0, 0.0]]))
+    o.step(5)
+    rho, u = o.get_macroscopic()
+    assert rho[0] == pytest.approx(1.01, abs=1e-15)          # mass stays on the site
+    with pytest.raises(ValueError):
+        oracle.Oracle(st, 0, 0.5, [])                         # tau must exceed 1/2
+    st[0, 0, 0] = 4
+    with pytest.raises(ValueError):
+        oracle.Oracle(st, 0, 0.8, [1.0])                      # type 4 needs 3 iolets
