@@ -1,0 +1,161 @@
+/* hlb.h -- C-ABI boundary of the B200-native sparse lattice-Boltzmann site update.
+ *
+ * One thing lives behind this header: the per-timestep site update of a HemeLB-style
+ * solver -- "a lattice of fluid sites, each equipped with a single-particle distribution
+ * ... evolution of these particle distributions over consecutive propagation and collision
+ * steps" (section II), with "simple bounce-back boundary condition"
+ * (section IV) -- in the concrete form BASELINE.json `north_star` fixes:
+ * fused D3Q15 LBGK collide-and-stream over a sparse, indirectly addressed list of fluid
+ * sites, halfway bounce-back walls, constant-density inlets/outlets. The formulas and the
+ * readings of every point the paper leaves open are in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - Plain C ABI: no C++ or torch types. Every function returns HLB_OK (0) or a negative
+ *     hlb_status and never throws; hlb_last_error() gives a thread-local message.
+ *   - Voxel box nx*ny*nz, linear voxel index v = (z*ny + y)*nx + x.
+ *   - CANONICAL SITE ORDER = ascending v over the fluid voxels. Every per-site array that
+ *     crosses this boundary (rho, u, populations, site voxels) is in canonical order; the
+ *     library's internal (Morton / blocked) order never leaks.
+ *   - "host" / "device" is stated per pointer. Inputs are caller-owned and only read during
+ *     the call. Outputs go to caller-allocated buffers.
+ *   - Device memory comes from the caller's allocator callback (PyTorch in the Python
+ *     binding) and is released by the caller after hlb_geometry_destroy(); with a NULL
+ *     callback the library uses cudaMalloc / cudaFree itself.
+ *   - All device work is enqueued on hlb_params.stream. The library never calls
+ *     cudaSetDevice and creates no streams. hlb_step() is asynchronous; the calls that
+ *     return data to the host synchronise that stream.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point fails
+ *     with HLB_ECUDA. hlb_preprocess_* are host-only by design (the geometry preprocessor
+ *     is host code) and work anywhere.
+ */
+#ifndef HLB_H_
+#define HLB_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  HLB_OK = 0,
+  HLB_EINVAL = -1,    /* NULL pointer, non-positive extent, tau <= 0.5, site type >=
+                         2 + n_iolets, n < 0, unknown flag combination                    */
+  HLB_ENOFLUID = -2,  /* no voxel of type 1                                               */
+  HLB_ETOOLARGE = -3, /* N >= 2^31 - 128 (site indices are int32)                         */
+  HLB_ENOMEM = -4,    /* allocator returned NULL                                          */
+  HLB_ECUDA = -5      /* a CUDA call failed (text in hlb_last_error())                    */
+} hlb_status;
+
+/* hlb_params.flags: one value from each group, OR-ed together. */
+enum {
+  HLB_STORE_F64 = 0x0,     /* populations stored as IEEE binary64                          */
+  HLB_STORE_F32 = 0x1,     /* stored as binary32 (round-to-nearest-even on store, exact
+                              widening on load); ALL arithmetic stays fp64; what is stored
+                              is h_q = f_q - w_q (reading R-shift)               */
+  HLB_TWO_LATTICE = 0x0,   /* two population arrays, pull (gather) form                    */
+  HLB_AA = 0x2,            /* one array updated in place, A-A pattern (even/odd steps)     */
+  HLB_ORDER_MORTON = 0x0,  /* internal site order: Morton (Z) curve over voxel coordinates */
+  HLB_ORDER_RASTER = 0x4,  /* internal order = canonical order                             */
+  HLB_ORDER_TILED = 0x8,   /* Morton over 8x8x8 blocks, x-fastest raster inside a block    */
+  HLB_ORDER_MASK = 0xC,
+  HLB_NO_GRAPH = 0x10      /* launch every step directly instead of replaying a captured
+                              CUDA graph of steps (debugging / profiling)                  */
+};
+
+typedef struct hlb_geometry hlb_geometry; /* opaque handle */
+
+/* Returns a DEVICE pointer to `bytes` bytes, at least 256-byte aligned, or NULL. The
+ * memory must stay valid until after hlb_geometry_destroy(). */
+typedef void* (*hlb_alloc_fn)(size_t bytes, void* user);
+
+typedef struct {
+  int32_t nx, ny, nz;      /* voxel box, each >= 1                                         */
+  uint32_t periodic;       /* bit0 = x, bit1 = y, bit2 = z wrap; a non-periodic axis has
+                              solid outside the box                                        */
+  double tau;              /* LBGK relaxation time, must be > 0.5; nu = (tau - 1/2)/3      */
+  int32_t n_iolets;        /* 0..253                                                       */
+  const double* iolet_rho; /* HOST, n_iolets densities in lattice units (may be NULL when
+                              n_iolets == 0)                                               */
+  uint32_t flags;          /* HLB_STORE_* | HLB_TWO_LATTICE/HLB_AA | HLB_ORDER_* | ...     */
+  hlb_alloc_fn alloc;      /* device allocator or NULL (=> cudaMalloc)                     */
+  void* alloc_user;
+  void* stream;            /* cudaStream_t as void*; NULL = the legacy default stream      */
+} hlb_params;
+
+/* Build the geometry: extract the fluid sites, order them, build the int32 pull-neighbour
+ * table (wall and iolet links encoded as bounce-back targets), upload, and initialise the
+ * state to rho = 1, u = 0 (f = f_eq, step counter 0).
+ *   site_type: HOST array of nx*ny*nz bytes. 0 = solid, 1 = fluid, 2+k = ghost voxel of
+ *              iolet k (never simulated; it marks the links that cross iolet k).
+ * Errors: HLB_EINVAL, HLB_ENOFLUID, HLB_ETOOLARGE, HLB_ENOMEM, HLB_ECUDA. On error *out
+ * is set to NULL. */
+int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geometry** out);
+
+/* Set f_q(x, 0) = f_eq_q(rho(x), u(x)) and the step counter to 0.
+ *   rho: HOST [N] or NULL (=> 1);  u: HOST [N][3] or NULL (=> 0); canonical order. */
+int hlb_set_state(hlb_geometry* g, const double* rho, const double* u);
+
+/* Replace the n_iolets iolet densities (HOST array). Takes effect from the next step. */
+int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho);
+
+/* Advance n >= 0 time steps: n launches of ONE fused collide-and-stream kernel (A-A:
+ * alternating even/odd kernels), asynchronously on the stream. n == 0 is a no-op. A
+ * kernel fault surfaces at the next synchronising call. */
+int hlb_step(hlb_geometry* g, int64_t n);
+
+/* rho(x) = sum_q f_q, u(x) = sum_q c_q f_q / rho of the PRE-collision populations after
+ * hlb_steps_done() steps (reading R-readout), canonical order.
+ *   rho: HOST [N];  u: HOST [N][3]. Either may be NULL. Synchronises the stream. */
+int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u);
+
+/* Same, into DEVICE buffers (rho [N], u [N][3]); enqueued on the stream, no sync. */
+int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);
+
+/* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][15], canonical site
+ * order, q in the order of hlb_velocity_set(). For population-level parity checks. */
+int hlb_get_populations(hlb_geometry* g, double* f);
+
+/* Set pre-collision populations f_q(x, 0) directly (HOST [N][15], layout as above) and
+ * the step counter to 0. */
+int hlb_set_populations(hlb_geometry* g, const double* f);
+
+int64_t hlb_num_sites(const hlb_geometry* g);  /* N, or HLB_EINVAL for NULL                */
+int64_t hlb_steps_done(const hlb_geometry* g);
+/* Linear voxel index of every site, HOST [N], canonical order (ascending). */
+int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v);
+/* Bytes of device memory the geometry holds (populations + tables + scratch). */
+int64_t hlb_device_bytes(const hlb_geometry* g);
+/* Kernel launches enqueued by hlb_step() so far (graph replays count their nodes). */
+int64_t hlb_launch_count(const hlb_geometry* g);
+
+void hlb_geometry_destroy(hlb_geometry* g); /* NULL is a no-op                            */
+const char* hlb_last_error(void);           /* thread-local, never NULL                   */
+
+/* The library's D3Q15 set: c HOST [15][3], w HOST [15], opp HOST [15]. */
+void hlb_velocity_set(int32_t* c, double* w, int32_t* opp);
+
+/* ---- geometry preprocessor, host only (subsystem (b) of BASELINE.json north_star) ----
+ * Two calls: hlb_preprocess_count() gives N and the plane stride Ns (N rounded up to a
+ * multiple of 128); hlb_preprocess_tables() fills caller-allocated HOST arrays:
+ *   voxel_of_site [N]      linear voxel index of internal site i
+ *   canon_of_site [N]      canonical rank of internal site i
+ *   nbr           [14][Ns] entry (q-1)*Ns + i describes the pull source x - c_q of link q
+ *                          (q = 1..14) of internal site i:
+ *                            >= 0            internal index of the fluid source site
+ *                            0x80000000      solid (or outside a non-periodic box): the
+ *                                            bounce-back target is slot opp(q) of site i
+ *                            0x80000000 | (k+1)  ghost voxel of iolet k (also a bounce-back
+ *                                            target; the kernel substitutes f_eq(rho_k, u))
+ *                          entries i >= N of each plane are 0x80000000.
+ * Only nx, ny, nz, periodic, n_iolets and the HLB_ORDER_* bits of p are read. */
+int hlb_preprocess_count(const uint8_t* site_type, const hlb_params* p, int64_t* n_sites,
+                         int64_t* stride);
+int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t* voxel_of_site,
+                          int32_t* canon_of_site, int32_t* nbr);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HLB_H_ */

@@ -1,0 +1,252 @@
+"""Thin Python binding of include/hlb.h: argument marshalling only.
+
+Same names as the C-ABI entry points. PyTorch supplies device memory (the allocator
+callback hands out ``torch.empty`` buffers that live as long as the Geometry object) and
+the CUDA stream; every step of the path runs in the kernels of libhlb.so. There is no CPU
+fallback: if libhlb.so cannot be built or loaded, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+HLB_OK, HLB_EINVAL, HLB_ENOFLUID, HLB_ETOOLARGE, HLB_ENOMEM, HLB_ECUDA = 0, -1, -2, -3, -4, -5
+HLB_STORE_F64, HLB_STORE_F32 = 0x0, 0x1
+HLB_TWO_LATTICE, HLB_AA = 0x0, 0x2
+HLB_ORDER_MORTON, HLB_ORDER_RASTER, HLB_ORDER_TILED = 0x0, 0x4, 0x8
+HLB_NO_GRAPH = 0x10
+
+_ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+
+
+class hlb_params(ctypes.Structure):
+    _fields_ = [
+        ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
+        ("periodic", ctypes.c_uint32),
+        ("tau", ctypes.c_double),
+        ("n_iolets", ctypes.c_int32),
+        ("iolet_rho", ctypes.c_void_p),
+        ("flags", ctypes.c_uint32),
+        ("alloc", _ALLOC_FN),
+        ("alloc_user", ctypes.c_void_p),
+        ("stream", ctypes.c_void_p),
+    ]
+
+
+class HlbError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"hlb error {code}: {msg}")
+        self.code = code
+
+
+def _load() -> ctypes.CDLL:
+    path = _build.build()
+    lib = ctypes.CDLL(path)
+    vp, i64, c_int = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+    sigs = {
+        "hlb_geometry_create": (c_int, [vp, ctypes.POINTER(hlb_params), ctypes.POINTER(vp)]),
+        "hlb_set_state": (c_int, [vp, vp, vp]),
+        "hlb_set_iolet_density": (c_int, [vp, vp]),
+        "hlb_step": (c_int, [vp, i64]),
+        "hlb_get_macroscopic": (c_int, [vp, vp, vp]),
+        "hlb_get_macroscopic_device": (c_int, [vp, vp, vp]),
+        "hlb_get_populations": (c_int, [vp, vp]),
+        "hlb_set_populations": (c_int, [vp, vp]),
+        "hlb_num_sites": (i64, [vp]),
+        "hlb_steps_done": (i64, [vp]),
+        "hlb_get_site_voxels": (c_int, [vp, vp]),
+        "hlb_device_bytes": (i64, [vp]),
+        "hlb_launch_count": (i64, [vp]),
+        "hlb_geometry_destroy": (None, [vp]),
+        "hlb_last_error": (ctypes.c_char_p, []),
+        "hlb_velocity_set": (None, [vp, vp, vp]),
+        "hlb_preprocess_count": (c_int, [vp, ctypes.POINTER(hlb_params), ctypes.POINTER(i64),
+                                         ctypes.POINTER(i64)]),
+        "hlb_preprocess_tables": (c_int, [vp, ctypes.POINTER(hlb_params), vp, vp, vp]),
+    }
+    for name, (res, args) in sigs.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    return lib
+
+
+LIB_PATH = _build.LIB_PATH
+_lib = _load()
+EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density", "hlb_step",
+            "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
+            "hlb_set_populations", "hlb_num_sites", "hlb_steps_done", "hlb_get_site_voxels",
+            "hlb_device_bytes", "hlb_launch_count", "hlb_geometry_destroy", "hlb_last_error",
+            "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables")
+
+
+def hlb_last_error() -> str:
+    return _lib.hlb_last_error().decode()
+
+
+def _check(rc: int):
+    if rc != HLB_OK:
+        raise HlbError(rc, hlb_last_error())
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _host(a, dtype, shape=None):
+    if a is None:
+        return None
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if shape is not None and a.shape != shape:
+        raise ValueError(f"expected shape {shape}, got {a.shape}")
+    return a
+
+
+def hlb_velocity_set():
+    c = np.zeros((15, 3), dtype=np.int32)
+    w = np.zeros(15, dtype=np.float64)
+    opp = np.zeros(15, dtype=np.int32)
+    _lib.hlb_velocity_set(_ptr(c), _ptr(w), _ptr(opp))
+    return c, w, opp
+
+
+def _params(site_type, periodic, tau, iolet_rho, flags):
+    st = np.ascontiguousarray(site_type, dtype=np.uint8)
+    if st.ndim != 3:
+        raise ValueError("site_type must be a (nz, ny, nx) array")
+    nz, ny, nx = st.shape
+    io = np.ascontiguousarray(np.asarray(iolet_rho, dtype=np.float64).reshape(-1))
+    p = hlb_params()
+    p.nx, p.ny, p.nz = nx, ny, nz
+    p.periodic = int(periodic)
+    p.tau = float(tau)
+    p.n_iolets = int(io.shape[0])
+    p.iolet_rho = io.ctypes.data if io.shape[0] else None
+    p.flags = int(flags)
+    return st, io, p
+
+
+def hlb_preprocess(site_type, periodic=0, n_iolets=0, flags=0):
+    """Host-only preprocessor: returns dict(N, Ns, voxel_of_site, canon_of_site, nbr[14, Ns])."""
+    st, io, p = _params(site_type, periodic, 1.0, np.ones(n_iolets), flags)
+    n, ns = ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(_lib.hlb_preprocess_count(_ptr(st), ctypes.byref(p), ctypes.byref(n), ctypes.byref(ns)))
+    N, Ns = n.value, ns.value
+    vox = np.zeros(N, dtype=np.int64)
+    canon = np.zeros(N, dtype=np.int32)
+    nbr = np.zeros((14, Ns), dtype=np.int32)
+    _check(_lib.hlb_preprocess_tables(_ptr(st), ctypes.byref(p), _ptr(vox), _ptr(canon), _ptr(nbr)))
+    return {"N": N, "Ns": Ns, "voxel_of_site": vox, "canon_of_site": canon, "nbr": nbr}
+
+
+class Geometry:
+    """Owner of one hlb_geometry handle and of the torch buffers behind it."""
+
+    def __init__(self, site_type, periodic=0, tau=1.0, iolet_rho=(), flags=0, device=None,
+                 stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise HlbError(HLB_ECUDA, "no CUDA device: the site update has no CPU fallback")
+        self._torch = torch
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None \
+            else torch.device(device)
+        self._buffers = []
+        self._h = ctypes.c_void_p(None)
+        st, io, p = _params(site_type, periodic, tau, iolet_rho, flags)
+
+        def _alloc(nbytes, _user):
+            try:
+                t = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device=self.device)
+            except Exception:  # OOM -> NULL -> HLB_ENOMEM
+                return None
+            self._buffers.append(t)
+            return t.data_ptr()
+
+        self._alloc_cb = _ALLOC_FN(_alloc)     # keep the callback object alive
+        p.alloc = self._alloc_cb
+        p.alloc_user = None
+        with torch.cuda.device(self.device):
+            self.stream = torch.cuda.current_stream() if stream is None else stream
+            p.stream = self.stream.cuda_stream
+            _check(_lib.hlb_geometry_create(_ptr(st), ctypes.byref(p), ctypes.byref(self._h)))
+        self.n_sites = int(_lib.hlb_num_sites(self._h))
+        self.flags = int(flags)
+
+    # -- the C-ABI calls, same names -------------------------------------------------
+    def hlb_set_state(self, rho=None, u=None):
+        n = self.n_sites
+        rho, u = _host(rho, np.float64, (n,)), _host(u, np.float64, (n, 3))
+        _check(_lib.hlb_set_state(self._h, _ptr(rho), _ptr(u)))
+
+    def hlb_set_iolet_density(self, iolet_rho):
+        io = _host(np.asarray(iolet_rho).reshape(-1), np.float64)
+        _check(_lib.hlb_set_iolet_density(self._h, _ptr(io)))
+
+    def hlb_step(self, n: int = 1):
+        _check(_lib.hlb_step(self._h, int(n)))
+
+    def hlb_get_macroscopic(self, rho_out=None, u_out=None):
+        """Host results (numpy); pass preallocated (e.g. pinned) arrays to reuse them."""
+        n = self.n_sites
+        rho = np.empty(n, dtype=np.float64) if rho_out is None else rho_out
+        u = np.empty((n, 3), dtype=np.float64) if u_out is None else u_out
+        _check(_lib.hlb_get_macroscopic(self._h, _ptr(rho), _ptr(u)))
+        return rho, u
+
+    def hlb_get_macroscopic_device(self):
+        """rho [N], u [N,3] as torch cuda tensors (canonical order), stream-ordered."""
+        torch = self._torch
+        rho = torch.empty(self.n_sites, dtype=torch.float64, device=self.device)
+        u = torch.empty((self.n_sites, 3), dtype=torch.float64, device=self.device)
+        _check(_lib.hlb_get_macroscopic_device(self._h, rho.data_ptr(), u.data_ptr()))
+        return rho, u
+
+    def hlb_get_populations(self):
+        f = np.empty((self.n_sites, 15), dtype=np.float64)
+        _check(_lib.hlb_get_populations(self._h, _ptr(f)))
+        return f
+
+    def hlb_set_populations(self, f):
+        f = _host(f, np.float64, (self.n_sites, 15))
+        _check(_lib.hlb_set_populations(self._h, _ptr(f)))
+
+    def hlb_num_sites(self) -> int:
+        return int(_lib.hlb_num_sites(self._h))
+
+    def hlb_steps_done(self) -> int:
+        return int(_lib.hlb_steps_done(self._h))
+
+    def hlb_get_site_voxels(self):
+        v = np.empty(self.n_sites, dtype=np.int64)
+        _check(_lib.hlb_get_site_voxels(self._h, _ptr(v)))
+        return v
+
+    def hlb_device_bytes(self) -> int:
+        return int(_lib.hlb_device_bytes(self._h))
+
+    def hlb_launch_count(self) -> int:
+        return int(_lib.hlb_launch_count(self._h))
+
+    def hlb_geometry_destroy(self):
+        if self._h:
+            self._torch.cuda.synchronize(self.device)
+            _lib.hlb_geometry_destroy(self._h)
+            self._h = ctypes.c_void_p(None)
+            self._buffers.clear()
+
+    close = hlb_geometry_destroy
+
+    def __del__(self):
+        try:
+            self.hlb_geometry_destroy()
+        except Exception:
+            pass
+
+
+def hlb_geometry_create(site_type, periodic=0, tau=1.0, iolet_rho=(), flags=0, **kw) -> Geometry:
+    return Geometry(site_type, periodic, tau, iolet_rho, flags, **kw)

@@ -1,0 +1,318 @@
+// api.cu -- the C-ABI entry points declared in include/hlb.h (argument checking, device
+// buffers through the caller's allocator, stream-ordered kernel launches). Every step of
+// the hot path runs in the kernels of kernels.cu; nothing here computes on the host.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/hlb.h"
+#include "d3q15.h"
+#include "kernels.cuh"
+#include "preprocess.h"
+
+using namespace hlb;
+
+namespace {
+thread_local std::string g_err = "";
+
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return HLB_ECUDA;
+}
+#define HLB_CUDA(call)                                   \
+  do {                                                   \
+    cudaError_t e__ = (call);                            \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+  } while (0)
+
+SiteOrder order_of(uint32_t flags, bool& ok) {
+  ok = true;
+  switch (flags & HLB_ORDER_MASK) {
+    case HLB_ORDER_MORTON: return ORDER_MORTON;
+    case HLB_ORDER_RASTER: return ORDER_RASTER;
+    case HLB_ORDER_TILED: return ORDER_TILED;
+  }
+  ok = false;
+  return ORDER_MORTON;
+}
+}  // namespace
+
+struct hlb_geometry {
+  hlb_params p{};
+  cudaStream_t stream = nullptr;
+  bool aa = false, f32 = false;
+  int64_t N = 0, Ns = 0;
+  std::vector<int64_t> canon_voxels;  // [N] ascending
+  std::vector<double> iolet_rho;
+  DeviceGeometry dg;
+  void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
+  int cur = 0;                        // two-lattice: buffer the next step reads
+  double* scratch = nullptr;          // [N][15] doubles: staging for host<->device transfers
+  int64_t steps = 0, launches = 0, device_bytes = 0;
+  std::vector<void*> owned;           // cudaMalloc'ed (no allocator callback)
+
+  int alloc(size_t bytes, void** out) {
+    void* ptr = nullptr;
+    if (p.alloc) {
+      ptr = p.alloc(bytes, p.alloc_user);
+      if (!ptr) return fail(HLB_ENOMEM, "allocator callback returned NULL");
+    } else {
+      cudaError_t e = cudaMalloc(&ptr, bytes);
+      if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? fail(HLB_ENOMEM, "cudaMalloc: out of memory")
+                                              : cuda_fail(e, "cudaMalloc");
+      }
+      owned.push_back(ptr);
+    }
+    device_bytes += (int64_t)bytes;
+    *out = ptr;
+    return HLB_OK;
+  }
+  size_t store_bytes() const { return f32 ? 4 : 8; }
+  GatherMode gather_mode() const {
+    if (!aa) return GATHER_PULL;
+    return (steps & 1) ? GATHER_AA_ODD : GATHER_OWN;
+  }
+  const void* state_buf() const { return aa ? buf[0] : buf[cur]; }
+};
+
+extern "C" {
+
+const char* hlb_last_error(void) { return g_err.c_str(); }
+
+void hlb_velocity_set(int32_t* c, double* w, int32_t* o) {
+  for (int q = 0; q < Q; ++q) {
+    if (c) { c[3 * q + 0] = cx(q); c[3 * q + 1] = cy(q); c[3 * q + 2] = cz(q); }
+    if (w) w[q] = weight(q);
+    if (o) o[q] = opp(q);
+  }
+}
+
+static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder& order) {
+  if (!site_type || !p) return fail(HLB_EINVAL, "NULL argument");
+  if (p->nx <= 0 || p->ny <= 0 || p->nz <= 0) return fail(HLB_EINVAL, "non-positive box extent");
+  if (p->n_iolets < 0 || p->n_iolets > 253) return fail(HLB_EINVAL, "n_iolets must be in 0..253");
+  if (p->n_iolets > 0 && !p->iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
+  if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
+  if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH))
+    return fail(HLB_EINVAL, "unknown flag bits");
+  bool ok;
+  order = order_of(p->flags, ok);
+  if (!ok) return fail(HLB_EINVAL, "unknown HLB_ORDER_* value");
+  return HLB_OK;
+}
+
+int hlb_preprocess_count(const uint8_t* site_type, const hlb_params* p, int64_t* n_sites,
+                         int64_t* stride) {
+  SiteOrder order;
+  int rc = check_params(site_type, p, order);
+  if (rc) return rc;
+  GeometryTables t;
+  std::string err;
+  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order, true, t, err);
+  if (rc) return fail(rc, err);
+  if (n_sites) *n_sites = t.N;
+  if (stride) *stride = t.Ns;
+  return HLB_OK;
+}
+
+int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t* voxel_of_site,
+                          int32_t* canon_of_site, int32_t* nbr) {
+  SiteOrder order;
+  int rc = check_params(site_type, p, order);
+  if (rc) return rc;
+  GeometryTables t;
+  std::string err;
+  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order, false, t, err);
+  if (rc) return fail(rc, err);
+  if (voxel_of_site) std::memcpy(voxel_of_site, t.voxel_of_site.data(), sizeof(int64_t) * (size_t)t.N);
+  if (canon_of_site) std::memcpy(canon_of_site, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N);
+  if (nbr) std::memcpy(nbr, t.nbr.data(), sizeof(int32_t) * t.nbr.size());
+  return HLB_OK;
+}
+
+int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geometry** out) {
+  if (out) *out = nullptr;
+  if (!out) return fail(HLB_EINVAL, "out is NULL");
+  SiteOrder order;
+  int rc = check_params(site_type, p, order);
+  if (rc) return rc;
+  if (!(p->tau > 0.5)) return fail(HLB_EINVAL, "tau must be > 0.5");
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev == 0) {
+    (void)cudaGetLastError();
+    return fail(HLB_ECUDA, "no CUDA device: the site update has no CPU fallback");
+  }
+  GeometryTables t;
+  std::string err;
+  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order, false, t, err);
+  if (rc) return fail(rc, err);
+
+  hlb_geometry* g = new hlb_geometry();
+  g->p = *p;
+  g->p.iolet_rho = nullptr;
+  g->stream = (cudaStream_t)p->stream;
+  g->aa = (p->flags & HLB_AA) != 0;
+  g->f32 = (p->flags & HLB_STORE_F32) != 0;
+  g->N = t.N;
+  g->Ns = t.Ns;
+  g->iolet_rho.assign(p->iolet_rho, p->iolet_rho + p->n_iolets);
+  g->canon_voxels.resize((size_t)t.N);
+  for (int64_t i = 0; i < t.N; ++i) g->canon_voxels[(size_t)t.canon_of_site[(size_t)i]] = t.voxel_of_site[(size_t)i];
+
+  void *d_nbr = nullptr, *d_bits = nullptr, *d_canon = nullptr, *d_rho = nullptr, *d_scratch = nullptr;
+  const size_t pop_bytes = (size_t)Q * (size_t)t.Ns * g->store_bytes();
+  auto bail = [&](int code) { hlb_geometry_destroy(g); return code; };
+  if ((rc = g->alloc(sizeof(int32_t) * t.nbr.size(), &d_nbr))) return bail(rc);
+  if ((rc = g->alloc(sizeof(uint32_t) * t.iolet_bits.size(), &d_bits))) return bail(rc);
+  if ((rc = g->alloc(sizeof(int32_t) * (size_t)t.N, &d_canon))) return bail(rc);
+  if ((rc = g->alloc(sizeof(double) * (size_t)(p->n_iolets > 0 ? p->n_iolets : 1), &d_rho))) return bail(rc);
+  if ((rc = g->alloc(pop_bytes, &g->buf[0]))) return bail(rc);
+  if (!g->aa && (rc = g->alloc(pop_bytes, &g->buf[1]))) return bail(rc);
+  if ((rc = g->alloc(sizeof(double) * (size_t)Q * (size_t)t.N, &d_scratch))) return bail(rc);
+  g->scratch = (double*)d_scratch;
+
+#define HLB_CUDA_G(call)                                                   \
+  do {                                                                     \
+    cudaError_t e__ = (call);                                              \
+    if (e__ != cudaSuccess) { cuda_fail(e__, #call); return bail(HLB_ECUDA); } \
+  } while (0)
+  HLB_CUDA_G(cudaMemcpyAsync(d_nbr, t.nbr.data(), sizeof(int32_t) * t.nbr.size(), cudaMemcpyHostToDevice, g->stream));
+  HLB_CUDA_G(cudaMemcpyAsync(d_bits, t.iolet_bits.data(), sizeof(uint32_t) * t.iolet_bits.size(), cudaMemcpyHostToDevice, g->stream));
+  HLB_CUDA_G(cudaMemcpyAsync(d_canon, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N, cudaMemcpyHostToDevice, g->stream));
+  if (p->n_iolets > 0)
+    HLB_CUDA_G(cudaMemcpyAsync(d_rho, g->iolet_rho.data(), sizeof(double) * (size_t)p->n_iolets, cudaMemcpyHostToDevice, g->stream));
+  g->dg.N = t.N;
+  g->dg.Ns = t.Ns;
+  g->dg.nbr = (const int32_t*)d_nbr;
+  g->dg.iolet_bits = (const uint32_t*)d_bits;
+  g->dg.canon = (const int32_t*)d_canon;
+  g->dg.iolet_rho = (const double*)d_rho;
+  g->dg.omega = 1.0 / p->tau;
+  g->dg.f32 = g->f32;
+  // the host tables die at the end of this call: finish the uploads first
+  HLB_CUDA_G(cudaStreamSynchronize(g->stream));
+  rc = hlb_set_state(g, nullptr, nullptr);
+  if (rc) return bail(rc);
+  HLB_CUDA_G(cudaStreamSynchronize(g->stream));
+#undef HLB_CUDA_G
+  *out = g;
+  return HLB_OK;
+}
+
+void hlb_geometry_destroy(hlb_geometry* g) {
+  if (!g) return;
+  if (!g->owned.empty()) {
+    cudaStreamSynchronize(g->stream);
+    for (void* ptr : g->owned) cudaFree(ptr);
+  }
+  delete g;
+}
+
+static int init_from(hlb_geometry* g, const double* d_rho, const double* d_u, const double* d_f) {
+  const GatherMode mode = g->aa ? GATHER_OWN : GATHER_PULL;
+  g->cur = 0;
+  g->steps = 0;
+  launch_init(g->dg, g->buf[0], mode, d_rho, d_u, d_f, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  return HLB_OK;
+}
+
+int hlb_set_state(hlb_geometry* g, const double* rho, const double* u) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  double *d_rho = nullptr, *d_u = nullptr;
+  const size_t n = (size_t)g->N;
+  if (rho) {
+    d_rho = g->scratch;
+    HLB_CUDA(cudaMemcpyAsync(d_rho, rho, sizeof(double) * n, cudaMemcpyHostToDevice, g->stream));
+  }
+  if (u) {
+    d_u = g->scratch + n;
+    HLB_CUDA(cudaMemcpyAsync(d_u, u, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, g->stream));
+  }
+  return init_from(g, d_rho, d_u, nullptr);
+}
+
+int hlb_set_populations(hlb_geometry* g, const double* f) {
+  if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
+  HLB_CUDA(cudaMemcpyAsync(g->scratch, f, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyHostToDevice, g->stream));
+  return init_from(g, nullptr, nullptr, g->scratch);
+}
+
+int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (g->p.n_iolets == 0) return HLB_OK;
+  if (!iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
+  g->iolet_rho.assign(iolet_rho, iolet_rho + g->p.n_iolets);
+  HLB_CUDA(cudaMemcpyAsync((void*)g->dg.iolet_rho, g->iolet_rho.data(), sizeof(double) * (size_t)g->p.n_iolets, cudaMemcpyHostToDevice, g->stream));
+  HLB_CUDA(cudaStreamSynchronize(g->stream));  // g->iolet_rho may be reassigned by the next call
+  return HLB_OK;
+}
+
+int hlb_step(hlb_geometry* g, int64_t n) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (n < 0) return fail(HLB_EINVAL, "n < 0");
+  for (int64_t s = 0; s < n; ++s) {
+    if (g->aa) {
+      launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
+    } else {
+      launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->stream);
+      g->cur ^= 1;
+    }
+    ++g->steps;
+    ++g->launches;
+  }
+  if (n > 0) HLB_CUDA(cudaGetLastError());
+  return HLB_OK;
+}
+
+int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (!rho_dev && !u_dev) return HLB_OK;
+  launch_macroscopic(g->dg, g->state_buf(), g->gather_mode(), rho_dev, u_dev, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  return HLB_OK;
+}
+
+int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  const size_t n = (size_t)g->N;
+  double* d_rho = g->scratch;
+  double* d_u = g->scratch + n;
+  int rc = hlb_get_macroscopic_device(g, rho ? d_rho : nullptr, u ? d_u : nullptr);
+  if (rc) return rc;
+  if (rho) HLB_CUDA(cudaMemcpyAsync(rho, d_rho, sizeof(double) * n, cudaMemcpyDeviceToHost, g->stream));
+  if (u) HLB_CUDA(cudaMemcpyAsync(u, d_u, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
+int hlb_get_populations(hlb_geometry* g, double* f) {
+  if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
+  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->scratch, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  HLB_CUDA(cudaMemcpyAsync(f, g->scratch, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
+int64_t hlb_num_sites(const hlb_geometry* g) { return g ? g->N : (int64_t)HLB_EINVAL; }
+int64_t hlb_steps_done(const hlb_geometry* g) { return g ? g->steps : (int64_t)HLB_EINVAL; }
+int64_t hlb_device_bytes(const hlb_geometry* g) { return g ? g->device_bytes : (int64_t)HLB_EINVAL; }
+int64_t hlb_launch_count(const hlb_geometry* g) { return g ? g->launches : (int64_t)HLB_EINVAL; }
+int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v) {
+  if (!g || !v) return fail(HLB_EINVAL, "NULL argument");
+  std::memcpy(v, g->canon_voxels.data(), sizeof(int64_t) * (size_t)g->N);
+  return HLB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,43 @@
+// kernels.cuh -- launchers of the CUDA kernels (sm_100a). Host-callable, defined in kernels.cu.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+namespace hlb {
+
+struct DeviceGeometry {
+  int64_t N = 0;                        // fluid sites
+  int64_t Ns = 0;                       // plane stride (multiple of 128), arrays are [15][Ns]
+  const int32_t* nbr = nullptr;         // [14][Ns] pull-neighbour table (include/hlb.h)
+  const uint32_t* iolet_bits = nullptr; // [Ns/32]
+  const int32_t* canon = nullptr;       // [N] internal -> canonical rank
+  const double* iolet_rho = nullptr;    // [n_iolets]
+  double omega = 1.0;                   // 1 / tau
+  bool f32 = false;                     // HLB_STORE_F32
+};
+
+// One time step, two-lattice pull: dst <- collide(gather(src)).
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);
+// One time step, A-A in place; `odd` selects the phase.
+void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s);
+
+// How the pre-collision populations f(., n) are found in a buffer.
+enum GatherMode {
+  GATHER_PULL = 0,   // two-lattice buffer holding post-collision values: pull through the table
+  GATHER_OWN = 1,    // A-A after an even number of steps: slot q of the site itself
+  GATHER_AA_ODD = 2  // A-A after an odd number of steps: slot opp(q) of x - c_q (slot q at walls)
+};
+// rho [N] / u [N][3] (device, canonical order; either may be NULL)
+void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
+                        double* u, cudaStream_t s);
+// f [N][15] raw populations (device, canonical order)
+void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
+                            cudaStream_t s);
+// Initialise a buffer so that gathering in `mode` (GATHER_PULL or GATHER_OWN) yields
+//   f_q(x) = f_in[canon(x)][q]                       if f_in != NULL, else
+//   f_q(x) = f_eq_q(rho_in[canon(x)], u_in[canon(x)])  (NULL rho => 1, NULL u => 0).
+void launch_init(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
+                 const double* u_in, const double* f_in, cudaStream_t s);
+
+}  // namespace hlb

@@ -1,0 +1,318 @@
+// preprocess.cpp -- geometry preprocessor (host, multi-threaded).
+//
+// voxel mask -> fluid-site list in the internal order (Morton by default) -> int32
+// pull-neighbour table with wall / iolet links encoded as bounce-back targets
+// (BASELINE.json north_star (b); "sparse geometries common in
+// vascular systems"; the paper's own domains are lists of sites grouped
+// in blocks, Table II).
+//
+// Data structure: the box is cut into 8x8x8 blocks. Every non-empty block keeps a 512-bit
+// occupancy map whose bit position is the voxel's rank along the intra-block curve, and
+// the index of its first site. Blocks are numbered along a Morton curve over block
+// coordinates. With the Morton intra-block curve this is exactly the Morton order of the
+// voxel coordinates (the curve is hierarchical), and "which site is voxel (x,y,z)" is
+// start[block] + popcount(bits below) -- no dense voxel->site map (17 GB at config 4) and
+// no 40-million-key sort.
+#include "preprocess.h"
+
+#include <algorithm>
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <thread>
+
+#include "../../include/hlb.h"
+#include "d3q15.h"
+
+namespace hlb {
+namespace {
+
+int thread_count() {
+  static int n = [] {
+    if (const char* e = std::getenv("HLB_THREADS")) {
+      int v = std::atoi(e);
+      if (v > 0) return v;
+    }
+    unsigned hc = std::thread::hardware_concurrency();
+    return (int)std::min<unsigned>(hc ? hc : 1u, 64u);
+  }();
+  return n;
+}
+
+// fn(begin, end) over [0, n) in chunks of `grain`, dynamically scheduled.
+template <class F>
+void parallel_for(int64_t n, int64_t grain, F&& fn) {
+  if (n <= 0) return;
+  const int64_t chunks = (n + grain - 1) / grain;
+  const int T = (int)std::min<int64_t>(thread_count(), chunks);
+  if (T <= 1) { fn((int64_t)0, n); return; }
+  std::atomic<int64_t> next{0};
+  auto worker = [&]() {
+    for (;;) {
+      const int64_t b = next.fetch_add(grain);
+      if (b >= n) break;
+      fn(b, std::min(n, b + grain));
+    }
+  };
+  std::vector<std::thread> pool;
+  pool.reserve(T - 1);
+  for (int t = 1; t < T; ++t) pool.emplace_back(worker);
+  worker();
+  for (auto& th : pool) th.join();
+}
+
+inline uint64_t spread3(uint64_t v) {  // 21 bits -> every third bit
+  v &= 0x1fffffull;
+  v = (v | v << 32) & 0x1f00000000ffffull;
+  v = (v | v << 16) & 0x1f0000ff0000ffull;
+  v = (v | v << 8) & 0x100f00f00f00f00full;
+  v = (v | v << 4) & 0x10c30c30c30c30c3ull;
+  v = (v | v << 2) & 0x1249249249249249ull;
+  return v;
+}
+inline uint64_t morton3(uint32_t x, uint32_t y, uint32_t z) {
+  return spread3(x) | (spread3(y) << 1) | (spread3(z) << 2);
+}
+
+struct Slot {          // one non-empty 8x8x8 block
+  uint64_t bits[8];    // occupancy by intra-block curve position
+  int64_t start;       // internal (base-order) index of its first site
+  uint16_t cum[8];     // sites in words below word w
+  int64_t block;       // raster block id
+  uint64_t key;        // Morton key of the block coordinates
+};
+
+struct BlockIndex {
+  int nx, ny, nz, nbx, nby, nbz;
+  uint16_t pos_of[512];   // ((dz*8+dy)*8+dx) -> curve position
+  uint16_t cell_of[512];  // curve position -> ((dz*8+dy)*8+dx)
+  std::vector<int32_t> slot_of_block;
+  std::vector<Slot> slots;
+
+  inline int64_t lookup(int x, int y, int z) const {
+    const int64_t b = ((int64_t)(z >> 3) * nby + (y >> 3)) * nbx + (x >> 3);
+    const Slot& s = slots[(size_t)slot_of_block[(size_t)b]];
+    const int p = pos_of[((z & 7) << 6) | ((y & 7) << 3) | (x & 7)];
+    const int w = p >> 6;
+    const uint64_t below = s.bits[w] & ((1ull << (p & 63)) - 1ull);
+    return s.start + s.cum[w] + __builtin_popcountll(below);
+  }
+};
+
+}  // namespace
+
+int preprocess_threads() { return thread_count(); }
+
+int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, int n_iolets,
+               SiteOrder order, bool count_only, GeometryTables& out, std::string& err) {
+  if (!type) { err = "site_type is NULL"; return HLB_EINVAL; }
+  if (nx <= 0 || ny <= 0 || nz <= 0) { err = "non-positive box extent"; return HLB_EINVAL; }
+  if (n_iolets < 0 || n_iolets > 253) { err = "n_iolets must be in 0..253"; return HLB_EINVAL; }
+  if (order != ORDER_MORTON && order != ORDER_RASTER && order != ORDER_TILED) {
+    err = "unknown site order"; return HLB_EINVAL;
+  }
+  BlockIndex bi;
+  bi.nx = nx; bi.ny = ny; bi.nz = nz;
+  bi.nbx = (nx + 7) >> 3; bi.nby = (ny + 7) >> 3; bi.nbz = (nz + 7) >> 3;
+  for (int dz = 0; dz < 8; ++dz)
+    for (int dy = 0; dy < 8; ++dy)
+      for (int dx = 0; dx < 8; ++dx) {
+        const int cell = (dz << 6) | (dy << 3) | dx;
+        const int pos = (order == ORDER_TILED) ? cell : (int)morton3(dx, dy, dz);
+        bi.pos_of[cell] = (uint16_t)pos;
+        bi.cell_of[pos] = (uint16_t)cell;
+      }
+  const int64_t nblocks = (int64_t)bi.nbx * bi.nby * bi.nbz;
+  const int64_t nrows = (int64_t)ny * nz;
+  const int max_type = 1 + n_iolets;
+
+  // ---- pass A: occupancy maps per block, fluid count per voxel row, type validation
+  const int64_t nbrows = (int64_t)bi.nby * bi.nbz;
+  std::vector<std::vector<Slot>> row_slots((size_t)nbrows);
+  std::vector<int32_t> row_count((size_t)nrows, 0);
+  std::atomic<int> bad_type{0};
+  parallel_for(nbrows, 4, [&](int64_t rb, int64_t re) {
+    std::vector<uint64_t> acc((size_t)bi.nbx * 8);
+    std::vector<uint8_t> touched((size_t)bi.nbx);
+    for (int64_t r = rb; r < re; ++r) {
+      const int by = (int)(r % bi.nby), bz = (int)(r / bi.nby);
+      std::fill(acc.begin(), acc.end(), 0ull);
+      std::fill(touched.begin(), touched.end(), (uint8_t)0);
+      bool any = false;
+      for (int dz = 0; dz < 8; ++dz) {
+        const int z = bz * 8 + dz;
+        if (z >= nz) break;
+        for (int dy = 0; dy < 8; ++dy) {
+          const int y = by * 8 + dy;
+          if (y >= ny) break;
+          const uint8_t* row = type + ((int64_t)z * ny + y) * nx;
+          int32_t cnt = 0;
+          int x = 0;
+          while (x < nx) {
+            if (x + 8 <= nx) {  // skip 8 solid voxels at a time
+              uint64_t w8;
+              std::memcpy(&w8, row + x, 8);
+              if (w8 == 0) { x += 8; continue; }
+            }
+            const int xe = std::min(nx, x + 8);
+            for (; x < xe; ++x) {
+              const uint8_t t = row[x];
+              if (t == 1) {
+                const int p = bi.pos_of[(dz << 6) | (dy << 3) | (x & 7)];
+                acc[(size_t)(x >> 3) * 8 + (p >> 6)] |= 1ull << (p & 63);
+                touched[(size_t)(x >> 3)] = 1;
+                any = true;
+                ++cnt;
+              } else if (t > max_type) {
+                bad_type.store(1, std::memory_order_relaxed);
+              }
+            }
+          }
+          row_count[(size_t)((int64_t)z * ny + y)] = cnt;
+        }
+      }
+      if (!any) continue;
+      auto& dst = row_slots[(size_t)r];
+      for (int bx = 0; bx < bi.nbx; ++bx) {
+        if (!touched[(size_t)bx]) continue;
+        Slot s;
+        int c = 0;
+        for (int w = 0; w < 8; ++w) {
+          s.bits[w] = acc[(size_t)bx * 8 + w];
+          s.cum[w] = (uint16_t)c;
+          c += __builtin_popcountll(s.bits[w]);
+        }
+        s.start = c;  // count for now
+        s.block = ((int64_t)bz * bi.nby + by) * bi.nbx + bx;
+        s.key = morton3((uint32_t)bx, (uint32_t)by, (uint32_t)bz);
+        dst.push_back(s);
+      }
+    }
+  });
+  if (bad_type.load()) { err = "site type >= 2 + n_iolets"; return HLB_EINVAL; }
+
+  size_t nslots = 0;
+  for (auto& v : row_slots) nslots += v.size();
+  if (nslots == 0) { err = "no fluid voxel (type 1)"; return HLB_ENOFLUID; }
+  bi.slots.reserve(nslots);
+  for (auto& v : row_slots) {
+    bi.slots.insert(bi.slots.end(), v.begin(), v.end());
+    std::vector<Slot>().swap(v);
+  }
+  std::sort(bi.slots.begin(), bi.slots.end(),
+            [](const Slot& a, const Slot& b) { return a.key < b.key; });
+  int64_t N = 0;
+  for (auto& s : bi.slots) { const int64_t c = s.start; s.start = N; N += c; }
+  if (N >= (int64_t)0x7fffffff - 128) { err = "too many fluid sites for int32 indices"; return HLB_ETOOLARGE; }
+  out = GeometryTables();
+  out.N = N;
+  out.Ns = (N + 127) / 128 * 128;
+  if (count_only) return HLB_OK;
+
+  bi.slot_of_block.assign((size_t)nblocks, -1);
+  for (size_t s = 0; s < bi.slots.size(); ++s) bi.slot_of_block[(size_t)bi.slots[s].block] = (int32_t)s;
+
+  // ---- pass B: voxel of every site in the base (block-curve) order
+  std::vector<int64_t> voxel_base((size_t)N);
+  parallel_for((int64_t)bi.slots.size(), 64, [&](int64_t sb, int64_t se) {
+    for (int64_t si = sb; si < se; ++si) {
+      const Slot& s = bi.slots[(size_t)si];
+      const int bx = (int)(s.block % bi.nbx), by = (int)((s.block / bi.nbx) % bi.nby),
+                bz = (int)(s.block / ((int64_t)bi.nbx * bi.nby));
+      int64_t i = s.start;
+      for (int w = 0; w < 8; ++w) {
+        uint64_t m = s.bits[w];
+        while (m) {
+          const int p = (w << 6) | __builtin_ctzll(m);
+          m &= m - 1;
+          const int cell = bi.cell_of[p];
+          const int x = bx * 8 + (cell & 7), y = by * 8 + ((cell >> 3) & 7), z = bz * 8 + (cell >> 6);
+          voxel_base[(size_t)i++] = ((int64_t)z * ny + y) * nx + x;
+        }
+      }
+    }
+  });
+
+  // ---- pass C: canonical rank (ascending voxel index) of every base-order site
+  std::vector<int64_t> row_start((size_t)nrows + 1);
+  row_start[0] = 0;
+  for (int64_t r = 0; r < nrows; ++r) row_start[(size_t)r + 1] = row_start[(size_t)r] + row_count[(size_t)r];
+  std::vector<int32_t> canon_base((size_t)N);
+  parallel_for(nrows, 256, [&](int64_t rb, int64_t re) {
+    for (int64_t r = rb; r < re; ++r) {
+      if (row_count[(size_t)r] == 0) continue;
+      const int y = (int)(r % ny), z = (int)(r / ny);
+      const uint8_t* row = type + r * nx;
+      int64_t c = row_start[(size_t)r];
+      for (int x = 0; x < nx; ++x)
+        if (row[x] == 1) canon_base[(size_t)bi.lookup(x, y, z)] = (int32_t)c++;
+    }
+  });
+  std::vector<int32_t>().swap(row_count);
+  std::vector<int64_t>().swap(row_start);
+
+  const bool raster = (order == ORDER_RASTER);
+  out.voxel_of_site.resize((size_t)N);
+  out.canon_of_site.resize((size_t)N);
+  if (raster) {
+    parallel_for(N, 1 << 16, [&](int64_t b, int64_t e) {
+      for (int64_t i = b; i < e; ++i) {
+        const int32_t c = canon_base[(size_t)i];
+        out.voxel_of_site[(size_t)c] = voxel_base[(size_t)i];
+        out.canon_of_site[(size_t)c] = c;
+      }
+    });
+  } else {
+    out.voxel_of_site.swap(voxel_base);
+    out.canon_of_site = canon_base;
+  }
+
+  // ---- pass D: pull-neighbour table
+  const int64_t Ns = out.Ns;
+  out.nbr.assign((size_t)(14 * Ns), (int32_t)NBR_WALL_BIT);
+  out.iolet_bits.assign((size_t)(Ns / 32), 0u);
+  std::atomic<int64_t> n_io_sites{0}, n_wall_links{0};
+  const bool px = periodic & 1u, py = periodic & 2u, pz = periodic & 4u;
+  parallel_for(N, 1 << 14, [&](int64_t b, int64_t e) {  // grain is a multiple of 32
+    int64_t io_sites = 0, wall_links = 0;
+    for (int64_t i = b; i < e; ++i) {
+      const int64_t v = out.voxel_of_site[(size_t)i];
+      const int x = (int)(v % nx), y = (int)((v / nx) % ny), z = (int)(v / ((int64_t)nx * ny));
+      bool has_io = false;
+      for (int q = 1; q < Q; ++q) {
+        int sx = x - cx(q), sy = y - cy(q), sz = z - cz(q);
+        bool outside = false;
+        if (sx < 0) { if (px) sx += nx; else outside = true; }
+        else if (sx >= nx) { if (px) sx -= nx; else outside = true; }
+        if (sy < 0) { if (py) sy += ny; else outside = true; }
+        else if (sy >= ny) { if (py) sy -= ny; else outside = true; }
+        if (sz < 0) { if (pz) sz += nz; else outside = true; }
+        else if (sz >= nz) { if (pz) sz -= nz; else outside = true; }
+        int32_t entry;
+        const uint8_t t = outside ? (uint8_t)0 : type[((int64_t)sz * ny + sy) * nx + sx];
+        if (t == 1) {
+          const int64_t sb = bi.lookup(sx, sy, sz);
+          entry = raster ? canon_base[(size_t)sb] : (int32_t)sb;
+        } else if (t == 0) {
+          entry = (int32_t)NBR_WALL_BIT;
+          ++wall_links;
+        } else {
+          entry = (int32_t)(NBR_WALL_BIT | (uint32_t)(t - 1));  // iolet k = t-2 -> k+1
+          has_io = true;
+        }
+        out.nbr[(size_t)((q - 1) * Ns + i)] = entry;
+      }
+      if (has_io) {
+        out.iolet_bits[(size_t)(i >> 5)] |= 1u << (i & 31);
+        ++io_sites;
+      }
+    }
+    n_io_sites += io_sites;
+    n_wall_links += wall_links;
+  });
+  out.n_iolet_sites = n_io_sites.load();
+  out.n_wall_links = n_wall_links.load();
+  return HLB_OK;
+}
+
+}  // namespace hlb

@@ -1,0 +1,30 @@
+// preprocess.h -- geometry preprocessor (host): voxel mask -> ordered site list + int32
+// pull-neighbour table. Subsystem (b) of BASELINE.json north_star; SURVEY.md §8(a) row S0.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace hlb {
+
+enum SiteOrder { ORDER_MORTON = 0, ORDER_RASTER = 1, ORDER_TILED = 2 };
+
+struct GeometryTables {
+  int64_t N = 0;    // fluid sites
+  int64_t Ns = 0;   // plane stride of every [slot][site] array: N rounded up to 128
+  std::vector<int64_t> voxel_of_site;  // [N]  internal order -> linear voxel index
+  std::vector<int32_t> canon_of_site;  // [N]  internal order -> canonical rank
+  std::vector<int32_t> nbr;            // [14][Ns], encoding: include/hlb.h
+  std::vector<uint32_t> iolet_bits;    // [Ns/32] bit (i & 31) of word i >> 5: site i has an iolet link
+  int64_t n_iolet_sites = 0;
+  int64_t n_wall_links = 0;
+};
+
+// Returns 0 or a negative hlb_status; `err` gets the message. With count_only the tables
+// are left empty and only N / Ns are set.
+int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, int n_iolets,
+               SiteOrder order, bool count_only, GeometryTables& out, std::string& err);
+
+int preprocess_threads();
+
+}  // namespace hlb

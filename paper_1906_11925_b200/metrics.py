@@ -1,0 +1,28 @@
+"""The metric of the paper and the bytes-per-site model of the roofline.
+
+SUPS ("Site Updates Per Second") = fluid sites x time steps / wall seconds; this
+reproduces Table III of the paper from Table II to the integer (
+tests/golden/paper_tables_II_III.txt).
+"""
+
+
+def sups(n_sites: int, steps: int, seconds: float) -> float:
+    return float(n_sites) * float(steps) / float(seconds)
+
+
+def msups(n_sites: int, steps: int, seconds: float) -> float:
+    return sups(n_sites, steps, seconds) / 1.0e6
+
+
+# Algorithmic bytes per site update: 15
+# populations read + 15 written + 14 int32 table entries; A-A reads the table on odd steps only.
+BYTES_PER_SITE = {
+    ("two_lattice", "f64"): 296.0,
+    ("aa", "f64"): 268.0,
+    ("two_lattice", "f32"): 176.0,
+    ("aa", "f32"): 148.0,
+}
+
+
+def algorithmic_bytes_per_site(scheme: str, store: str) -> float:
+    return BYTES_PER_SITE[(scheme, store)]

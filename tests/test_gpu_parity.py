@@ -1,0 +1,274 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the oracle, element by
+element, on the same seeded inputs.
+
+Bar (BASELINE.json north_star): fp64 rho and u within 1e-12 relative max error, the
+fp32-storage variant within 1e-5. Norm (reading R-norm):
+E_rho = max|rho - rho_ref| / max|rho_ref|,  E_u = max_{x,a}|u_a - u_ref,a| / max_x |u_ref|_2.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def hlb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1906_11925_b200 as m
+    return m
+
+
+def flags_of(hlb, scheme, store, order="morton"):
+    f = hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE
+    f |= hlb.HLB_STORE_F32 if store == "f32" else hlb.HLB_STORE_F64
+    f |= {"morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER, "tiled": hlb.HLB_ORDER_TILED}[order]
+    return f
+
+
+def errors(rho, u, rho_ref, u_ref):
+    e_rho = np.max(np.abs(rho - rho_ref)) / np.max(np.abs(rho_ref))
+    un = np.max(np.linalg.norm(u_ref, axis=1))
+    e_u = np.max(np.abs(u - u_ref)) / (un if un > 0 else 1.0)
+    return e_rho, e_u
+
+
+def run_gpu(hlb, wl, steps, scheme, store, order="morton"):
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, scheme, store, order))
+    if wl.rho0 is not None or wl.u0 is not None:
+        g.hlb_set_state(wl.rho0, wl.u0)
+    g.hlb_step(steps)
+    assert g.hlb_steps_done() == steps
+    out = g.hlb_get_macroscopic()
+    g.close()
+    return out
+
+
+def run_oracle(wl, steps, threads=0):
+    return oracle.run(wl, steps=steps, threads=threads)
+
+
+_oracle_cache = {}
+
+
+def oracle_cached(name, steps):
+    key = (name, steps)
+    if key not in _oracle_cache:
+        _oracle_cache[key] = run_oracle(W.by_name(name, small=True), steps)
+    return _oracle_cache[key]
+
+
+# ------------------------------------------------------------- the five configs, scaled down
+@pytest.mark.parametrize("store", ["f64", "f32"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+@pytest.mark.parametrize("name", W.CONFIG_NAMES)
+def test_small_configs_match_oracle(hlb, name, scheme, store):
+    wl = W.by_name(name, small=True)
+    for steps in (wl.steps, wl.steps + 1):            # even and odd (A-A read-out parity)
+        rho_ref, u_ref = oracle_cached(name, steps)
+        rho, u = run_gpu(hlb, wl, steps, scheme, store)
+        e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+        assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
+
+
+@pytest.mark.parametrize("order", ["raster", "tiled"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_result_is_independent_of_site_order(hlb, scheme, order):
+    """P10: the internal order never leaks -- bitwise identical canonical results."""
+    wl = W.by_name("aneurysm", small=True)
+    a = run_gpu(hlb, wl, 41, scheme, "f64", "morton")
+    b = run_gpu(hlb, wl, 41, scheme, "f64", order)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+@pytest.mark.parametrize("store", ["f64", "f32"])
+def test_aa_equals_two_lattice_bitwise(hlb, store):
+    """P14: same per-site arithmetic, so the two schemes agree bit for bit."""
+    wl = W.by_name("tree", small=True)
+    for steps in (6, 7):
+        a = run_gpu(hlb, wl, steps, "two_lattice", store)
+        b = run_gpu(hlb, wl, steps, "aa", store)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+# ------------------------------------------------------------- random masks, every BC at once
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+@pytest.mark.parametrize("seed,periodic,shape", [
+    (0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (33, 5, 4)), (3, 2, (4, 19, 5)),
+    (4, 4, (5, 4, 17)), (5, 7, (1, 1, 3)), (6, 3, (2, 2, 2)), (7, 0, (24, 20, 18)),
+    (8, 5, (40, 9, 23)),
+])
+def test_random_masks_match_oracle(hlb, scheme, seed, periodic, shape):
+    wl = W.random_mask(shape, p_fluid=0.6, n_iolets=3, p_iolet=0.06, periodic=periodic,
+                       tau=0.55 + 0.07 * seed, seed=200 + seed)
+    for steps in (0, 1, 2, 9, 10):
+        rho_ref, u_ref = run_oracle(wl, steps, threads=1)
+        rho, u = run_gpu(hlb, wl, steps, scheme, "f64")
+        e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+        assert e_rho < 1e-13 and e_u < 1e-12, (steps, e_rho, e_u)
+
+
+def _match_directions(hlb):
+    c_o, _, _ = oracle.velocity_set()
+    c_g, _, _ = hlb.hlb_velocity_set()
+    return [int(np.flatnonzero((c_g == c).all(axis=1))[0]) for c in c_o]   # oracle q -> library q
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_populations_match_oracle(hlb, scheme):
+    """Population-level parity (stronger than moments), including set/get of populations."""
+    wl = W.random_mask((12, 11, 10), p_fluid=0.65, n_iolets=2, periodic=1, tau=0.7, seed=77)
+    perm = _match_directions(hlb)
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho)
+    o.set_state(wl.rho0, wl.u0)
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, scheme, "f64"))
+    g.hlb_set_state(wl.rho0, wl.u0)
+    assert np.array_equal(g.hlb_get_site_voxels(), o.site_voxels())
+    for steps in (0, 1, 4, 3):
+        o.step(steps)
+        g.hlb_step(steps)
+        fo, fg = o.get_populations(), g.hlb_get_populations()
+        assert np.max(np.abs(fg[:, perm] - fo)) < 1e-15
+    # round trip: the oracle's populations pushed into the library, then stepped
+    fo = o.get_populations()
+    fg = np.empty_like(fo)
+    fg[:, perm] = fo
+    g.hlb_set_populations(fg)
+    assert g.hlb_steps_done() == 0
+    assert np.max(np.abs(g.hlb_get_populations() - fg)) < 1e-16
+    o.step(5)
+    g.hlb_step(5)
+    assert np.max(np.abs(g.hlb_get_populations()[:, perm] - o.get_populations())) < 1e-15
+    g.close()
+
+
+# ------------------------------------------------------------- invariants on the GPU itself
+@pytest.mark.parametrize("store", ["f64", "f32"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_rest_state_is_bitwise_invariant(hlb, scheme, store):
+    wl = W.by_name("tree", small=True)
+    g = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, np.ones(wl.n_iolets),
+                                flags_of(hlb, scheme, store))
+    g.hlb_step(51)
+    rho, u = g.hlb_get_macroscopic()
+    assert np.all(rho == 1.0) and np.all(u == 0.0)
+    g.close()
+
+
+def test_state_round_trip_and_iolet_update(hlb):
+    wl = W.by_name("pipe", small=True)
+    n = wl.n_sites
+    rng = np.random.default_rng(3)
+    rho0 = 1.0 + 0.01 * rng.standard_normal(n)
+    u0 = 0.01 * rng.standard_normal((n, 3))
+    for scheme in ("two_lattice", "aa"):
+        g = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, scheme, "f64"))
+        g.hlb_set_state(rho0, u0)
+        rho, u = g.hlb_get_macroscopic()
+        assert np.max(np.abs(rho - rho0)) < 1e-15 and np.max(np.abs(u - u0)) < 1e-16
+        rd, ud = g.hlb_get_macroscopic_device()
+        assert np.array_equal(rd.cpu().numpy(), rho) and np.array_equal(ud.cpu().numpy(), u)
+        # new iolet densities take effect: compare with an oracle built with them
+        g.hlb_set_state(None, None)
+        g.hlb_set_iolet_density([1.002, 0.997])
+        g.hlb_step(20)
+        o = oracle.Oracle(wl.site_type, 0, wl.tau, [1.002, 0.997])
+        o.step(20)
+        e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())
+        assert e_rho < 1e-12 and e_u < 1e-12
+        g.close()
+
+
+def test_degenerate_geometries(hlb):
+    st = np.zeros((3, 3, 3), dtype=np.uint8)
+    st[1, 1, 1] = 1                                   # one site, every link bounces back
+    for scheme in ("two_lattice", "aa"):
+        g = hlb.hlb_geometry_create(st, 0, 0.8, [], flags_of(hlb, scheme, "f64"))
+        g.hlb_set_state(np.array([1.01]), np.array([[0.01, -0.02, 0.005]]))
+        g.hlb_step(0)
+        g.hlb_step(7)
+        o = oracle.Oracle(st, 0, 0.8, [])
+        o.set_state(np.array([1.01]), np.array([[0.01, -0.02, 0.005]]))
+        o.step(7)
+        (r, u), (ro, uo) = g.hlb_get_macroscopic(), o.get_macroscopic()
+        assert abs(r[0] - ro[0]) < 1e-15 and np.max(np.abs(u - uo)) < 1e-15
+        g.close()
+    with pytest.raises(hlb.HlbError) as e:
+        hlb.hlb_geometry_create(np.zeros((2, 2, 2), dtype=np.uint8), 0, 0.8, [])
+    assert e.value.code == hlb.HLB_ENOFLUID
+    with pytest.raises(hlb.HlbError) as e:
+        hlb.hlb_geometry_create(st, 0, 0.5, [])
+    assert e.value.code == hlb.HLB_EINVAL
+    g = hlb.hlb_geometry_create(st, 0, 0.8, [])
+    with pytest.raises(hlb.HlbError):
+        g.hlb_step(-1)
+    g.close()
+
+
+# ------------------------------------------------------------- full-size configs
+def test_config0_pipe_full(hlb):
+    """BASELINE configs[0] exactly: 12,608 sites, tau 0.8, 200 steps."""
+    wl = W.pipe()
+    assert wl.n_sites == 12608
+    rho_ref, u_ref = run_oracle(wl, wl.steps)
+    for scheme in ("two_lattice", "aa"):
+        e_rho, e_u = errors(*run_gpu(hlb, wl, wl.steps, scheme, "f64"), rho_ref, u_ref)
+        assert e_rho < 1e-12 and e_u < 1e-12, (scheme, e_rho, e_u)
+
+
+def test_config1_cube_full_size(hlb):
+    """BASELINE configs[1] at full size (128^3, tau 0.6, Taylor-Green): parity with the
+    oracle after 60 steps (every site), then the full 1000 steps checked through properties
+    that hold at any size: exact mass conservation and the closed-form decay."""
+    wl = W.periodic_cube()
+    n = wl.n_sites
+    assert n == 128 ** 3
+    rho_ref, u_ref = run_oracle(wl, 60)
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, [], flags_of(hlb, "two_lattice", "f64"))
+    g.hlb_set_state(wl.rho0, wl.u0)
+    g.hlb_step(60)
+    e_rho, e_u = errors(*g.hlb_get_macroscopic(), rho_ref, u_ref)
+    assert e_rho < 1e-12 and e_u < 1e-12, (e_rho, e_u)
+    ke = {}
+    for t in (200, 600, 1000):
+        g.hlb_step(t - g.hlb_steps_done())
+        rho, u = g.hlb_get_macroscopic()
+        ke[t] = 0.5 * np.sum(rho[:, None] * u * u)
+        assert abs(rho.sum() - n) / n < 1e-14           # mass: exactly conserved up to rounding
+    nu, k = (wl.tau - 0.5) / 3.0, wl.info["k"]
+    for a, b in ((200, 600), (600, 1000)):
+        assert ke[b] / ke[a] == pytest.approx(np.exp(-4.0 * nu * k * k * (b - a)), rel=2e-3)
+    g.close()
+
+
+def test_config2_aneurysm_full_size(hlb):
+    """BASELINE configs[2] at full size (739,223 sites): all sites against the oracle after
+    150 steps; the 2000-step run is the slow record test below."""
+    wl = W.aneurysm()
+    assert wl.n_sites == 739223
+    rho_ref, u_ref = run_oracle(wl, 150)
+    for scheme in ("two_lattice", "aa"):
+        e_rho, e_u = errors(*run_gpu(hlb, wl, 150, scheme, "f64"), rho_ref, u_ref)
+        assert e_rho < 1e-12 and e_u < 1e-12, (scheme, e_rho, e_u)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name", ["cube", "aneurysm", "tree", "bigtree"])
+def test_full_configs_full_steps_record(hlb, name):
+    """Record runs (HLB_RUN_SLOW=1): full size AND full step count against the oracle."""
+    wl = W.by_name(name)
+    rho_ref, u_ref = run_oracle(wl, wl.steps)
+    stores = ("f64", "f32") if name == "tree" else ("f64",)
+    for store in stores:
+        e_rho, e_u = errors(*run_gpu(hlb, wl, wl.steps, wl.scheme, store), rho_ref, u_ref)
+        print(f"RECORD {name} N={wl.n_sites} steps={wl.steps} {wl.scheme}/{store} E_rho={e_rho:.3e} E_u={e_u:.3e}")
+        assert e_rho < TOL[store] and e_u < TOL[store]

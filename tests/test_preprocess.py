@@ -1,0 +1,119 @@
+"""Host logic of the geometry preprocessor (no GPU): brute-force checks of the site
+ordering and of the int32 pull-neighbour table on random small masks."""
+import numpy as np
+import pytest
+
+import paper_1906_11925_b200 as hlb
+import workloads as W
+
+C, WT, OPP = hlb.hlb_velocity_set()
+WALL = np.int32(-2 ** 31)
+
+
+def morton_key(x, y, z):
+    k = 0
+    for b in range(21):
+        k |= ((x >> b) & 1) << (3 * b) | ((y >> b) & 1) << (3 * b + 1) | ((z >> b) & 1) << (3 * b + 2)
+    return k
+
+
+def brute_table(st, periodic, vox_of_site):
+    nz, ny, nx = st.shape
+    site_of_vox = {int(v): i for i, v in enumerate(vox_of_site)}
+    n = len(vox_of_site)
+    out = np.zeros((14, n), dtype=np.int64)
+    for i, v in enumerate(vox_of_site):
+        x, y, z = int(v % nx), int((v // nx) % ny), int(v // (nx * ny))
+        for q in range(1, 15):
+            s = [x - int(C[q][0]), y - int(C[q][1]), z - int(C[q][2])]
+            outside = False
+            for a, ext in enumerate((nx, ny, nz)):
+                if s[a] < 0 or s[a] >= ext:
+                    if periodic & (1 << a):
+                        s[a] %= ext
+                    else:
+                        outside = True
+            t = 0 if outside else int(st[s[2], s[1], s[0]])
+            if t == 1:
+                out[q - 1, i] = site_of_vox[(s[2] * ny + s[1]) * nx + s[0]]
+            elif t == 0:
+                out[q - 1, i] = -2 ** 31
+            else:
+                out[q - 1, i] = -2 ** 31 + (t - 2) + 1
+    return out
+
+
+def test_library_velocity_set_is_d3q15():
+    assert {tuple(c) for c in C.tolist()} == {
+        (0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1),
+        (1, 1, 1), (-1, -1, -1), (1, 1, -1), (-1, -1, 1), (1, -1, 1), (-1, 1, -1),
+        (1, -1, -1), (-1, 1, 1)}
+    for q in range(15):
+        assert np.array_equal(C[OPP[q]], -C[q]) and OPP[OPP[q]] == q
+        assert WT[q] == {0: 2 / 9, 1: 1 / 9, 3: 1 / 72}[int(C[q] @ C[q])]
+
+
+@pytest.mark.parametrize("order", [hlb.HLB_ORDER_MORTON, hlb.HLB_ORDER_RASTER, hlb.HLB_ORDER_TILED])
+@pytest.mark.parametrize("seed,periodic,shape", [
+    (0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (20, 5, 4)), (3, 2, (4, 19, 5)),
+    (4, 4, (5, 4, 17)), (5, 7, (1, 1, 3)), (6, 3, (2, 2, 2)), (7, 0, (16, 16, 16)),
+    (8, 5, (17, 9, 23)),
+])
+def test_table_matches_brute_force(order, seed, periodic, shape):
+    wl = W.random_mask(shape, p_fluid=0.55, n_iolets=3, p_iolet=0.08, periodic=periodic, seed=seed)
+    st = wl.site_type
+    t = hlb.hlb_preprocess(st, periodic, 3, order)
+    canon = wl.fluid_voxels()
+    N = len(canon)
+    assert t["N"] == N and t["Ns"] % 128 == 0 and N <= t["Ns"] < N + 128
+    vox = t["voxel_of_site"]
+    assert np.array_equal(np.sort(vox), canon)                       # a permutation of the sites
+    assert np.array_equal(canon[t["canon_of_site"]], vox)            # canonical rank is right
+    nz, ny, nx = st.shape
+    x, y, z = vox % nx, (vox // nx) % ny, vox // (nx * ny)
+    if order == hlb.HLB_ORDER_RASTER:
+        assert np.array_equal(vox, canon)
+    elif order == hlb.HLB_ORDER_MORTON:
+        keys = [morton_key(int(a), int(b), int(c)) for a, b, c in zip(x, y, z)]
+        assert keys == sorted(keys)
+    else:  # Morton over 8^3 blocks, raster inside
+        keys = [(morton_key(int(a) >> 3, int(b) >> 3, int(c) >> 3), int(c) & 7, int(b) & 7, int(a) & 7)
+                for a, b, c in zip(x, y, z)]
+        assert keys == sorted(keys)
+    nbr = t["nbr"]
+    assert np.array_equal(nbr[:, :N].astype(np.int64), brute_table(st, periodic, vox))
+    assert np.all(nbr[:, N:] == WALL)                                 # padding sites: all wall
+
+
+def test_orders_describe_the_same_links():
+    wl = W.by_name("tree", small=True)
+    a = hlb.hlb_preprocess(wl.site_type, 0, wl.n_iolets, hlb.HLB_ORDER_MORTON)
+    b = hlb.hlb_preprocess(wl.site_type, 0, wl.n_iolets, hlb.HLB_ORDER_RASTER)
+    assert a["N"] == wl.n_sites == b["N"]
+    # same links, different numbering: map both tables to voxel space and compare
+    def links(t):
+        N = t["N"]
+        nb = t["nbr"][:, :N].astype(np.int64)
+        v = t["voxel_of_site"]
+        src = np.where(nb >= 0, v[np.clip(nb, 0, N - 1)], nb)
+        order = np.argsort(v)
+        return src[:, order]
+    assert np.array_equal(links(a), links(b))
+
+
+def test_argument_errors():
+    st = np.zeros((3, 3, 3), dtype=np.uint8)
+    with pytest.raises(hlb.HlbError) as e:
+        hlb.hlb_preprocess(st, 0, 0, 0)
+    assert e.value.code == hlb.HLB_ENOFLUID
+    st[1, 1, 1] = 1
+    st[0, 0, 0] = 5
+    with pytest.raises(hlb.HlbError) as e:
+        hlb.hlb_preprocess(st, 0, 2, 0)                                # type 5 needs 4 iolets
+    assert e.value.code == hlb.HLB_EINVAL
+    st[0, 0, 0] = 0
+    with pytest.raises(hlb.HlbError) as e:
+        hlb.hlb_preprocess(st, 0, 0, 0xC)                              # unknown order
+    assert e.value.code == hlb.HLB_EINVAL
+    t = hlb.hlb_preprocess(st, 0, 0, 0)                                # isolated site: all walls
+    assert t["N"] == 1 and np.all(t["nbr"] == WALL)
