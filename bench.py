@@ -1,0 +1,432 @@
+#!/usr/bin/env python
+"""bench.py -- MSUPS and fraction of the HBM roofline of the fused D3Q15 site update.
+
+Contract (one JSON line on stdout, printed by rank 0):
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload bigtree|tree|aneurysm|cube|pipe]
+                  [--scheme aa|two_lattice] [--store f64|f32] [--order morton|raster|tiled]
+                  [--inner S] [--impl ours|reference]
+
+* metric/unit: BASELINE.json's metric -- fluid site updates per second, in MSUPS
+  (= fluid sites x LB time steps / seconds / 1e6; the paper's SUPS definition, PAPER.md
+  Tables II/III, lines 115-133).
+* A bench "step" is one hlb_step(S) call: S (= --inner) consecutive LB time steps, each ONE
+  launch of the fused collide-and-stream kernel over every fluid site of the workload (all
+  rows S1..S8 of SURVEY.md section 8(a)). The default workload is BASELINE configs[4]
+  ("the largest geometry", the one north_star's roofline target is stated on).
+* value: device-timed (CUDA events on the launching stream, populations resident in HBM).
+* e2e: the same metric through the C-ABI with HOST buffers: every step uploads the initial
+  rho/u from pinned host memory (hlb_set_state), runs hlb_step(S), and reads rho/u back to
+  pinned host memory (hlb_get_macroscopic); the copies are inside the timed region.
+* roofline: algorithmic bytes per launch / average launch duration of the dominant kernel,
+  against MEASURED_PEAKS.json's hbm_gbs (fallback 6650 GB/s, B200_PROFILING.md).
+* cpu_baseline: the oracle (oracle/, as it stands, 1 thread) timed on a bounded crop of the
+  same geometry on this box's host cores. `--impl reference` times only that.
+* Multi-GPU (--gpus N under torchrun): REPLICAS ONLY: every rank
+  runs the same workload on its own GPU, no data-path collective; value = total site updates
+  of all ranks / max-over-ranks time; "scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fluid site updates/sec (MSUPS), D3Q15 LBGK sparse site update"
+UNIT = "MSUPS"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
+DEFAULT_SCHEME = {"pipe": "two_lattice", "cube": "two_lattice", "aneurysm": "two_lattice",
+                  "tree": "two_lattice", "bigtree": "aa"}
+WORKLOAD_DESC = {
+    "pipe": "BASELINE configs[0]: pipe R=8 L=64",
+    "cube": "BASELINE configs[1]: periodic 128^3 Taylor-Green",
+    "aneurysm": "BASELINE configs[2]: sine vessel + sac, 480x160x160",
+    "tree": "BASELINE configs[3]: 5-level tree, 1024^3 box, r0=32",
+    "bigtree": "BASELINE configs[4]: 5-level tree, 2048x2048x1024 box, r0=64",
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="bigtree", choices=list(WORKLOAD_DESC))
+    ap.add_argument("--scheme", default=None, choices=["aa", "two_lattice"])
+    ap.add_argument("--store", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--order", default="morton", choices=["morton", "raster", "tiled"])
+    ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--small", action="store_true", help="scaled-down geometry (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0,
+                    help="CPU work budget of the cpu_baseline leg")
+    ap.add_argument("--ref-seconds", type=float, default=120.0,
+                    help="total budget of an --impl reference run")
+    return ap.parse_args()
+
+
+# --------------------------------------------------------------------------- helpers
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            v = float(json.load(fh)["hbm_gbs"])
+        return v, "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(workload, scheme, store, kernel):
+    """dram bytes per launch from the committed ncu --set full capture (profiles/traffic.csv:
+    workload,scheme,store,kernel,n_sites,dram_bytes_per_launch,source), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        parts = [p.strip() for p in line.split(",")]
+        if parts[:4] == [workload, scheme, store, kernel]:
+            try:
+                return float(parts[5])
+            except (ValueError, IndexError):
+                return None
+    return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with nvidia-smi while the timed region runs."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, power = [], None, set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.lines if t0 - 0.05 <= t <= t1 + 0.15] or [l for _, l in self.lines]
+        for l in rows:
+            p = [x.strip() for x in l.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0]))
+                smax = float(p[1])
+                power.append(float(p[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "reasons": sorted(reasons), "samples": len(sm),
+                "power_w_max": max(power) if power else None}
+
+
+def crop_sample(wl, max_sites=1_200_000):
+    """A bounded sample of the workload for the CPU legs: the sub-box of the voxel array,
+    starting at the low-x end of the fluid's bounding box (the inlet side), that holds about
+    max_sites fluid sites. Outside the crop counts as solid, like outside the full box."""
+    st = wl.site_type
+    if wl.n_sites <= max_sites:
+        return st, wl.periodic, "whole geometry"
+    per_x = np.count_nonzero(st == 1, axis=(0, 1)).astype(np.int64)     # fluid per x-slab
+    cum = np.cumsum(per_x)
+    x1 = int(np.searchsorted(cum, max_sites)) + 1
+    x0 = int(np.argmax(per_x > 0))
+    x0 = max(0, x0 - 2)                                               # keep the inlet ghost slab
+    sub = st[:, :, x0:x1]
+    zs = np.flatnonzero(np.any(sub != 0, axis=(1, 2)))
+    ys = np.flatnonzero(np.any(sub != 0, axis=(0, 2)))
+    sub = np.ascontiguousarray(sub[zs[0]:zs[-1] + 1, ys[0]:ys[-1] + 1, :])
+    return sub, 0, f"crop x in [{x0},{x1}) of the same voxel array (outside = solid)"
+
+
+def time_oracle(wl, budget_s, threads=1):
+    """Oracle MSUPS on the bounded sample: 1 calibration step, then as many steps as fit
+    the budget. Returns (msups, n_sites, steps, seconds, sample description)."""
+    import oracle
+    st, periodic, what = crop_sample(wl)
+    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, threads=threads)
+    n = o.n_sites
+    t0 = time.perf_counter()
+    o.step(1)
+    t1 = time.perf_counter() - t0
+    steps = int(max(2, min(200, budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    o.close()
+    return n * steps / dt / 1e6, n, steps, dt, what, o.threads
+
+
+def host_cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+# --------------------------------------------------------------------------- reference arm
+def run_reference(args, rank, world):
+    if rank != 0:
+        return 0
+    import workloads as W
+    import oracle
+    wl = W.by_name(args.workload, small=args.small)
+    scheme = args.scheme or DEFAULT_SCHEME[args.workload]
+    st, periodic, what = crop_sample(wl)
+    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, threads=1)
+    n = o.n_sites
+    t0 = time.perf_counter()
+    o.step(1)
+    t1 = time.perf_counter() - t0
+    total = args.steps + args.warmup
+    lb_per_step = int(max(1, min(args.inner, args.ref_seconds / total / max(t1, 1e-6))))
+    for _ in range(args.warmup):
+        o.step(lb_per_step)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(lb_per_step)
+    dt = time.perf_counter() - t0
+    o.close()
+    value = n * lb_per_step * args.steps / dt / 1e6
+    sample = f"{what}: {n} sites x {lb_per_step} LB steps per bench step"
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
+                   "scheme": scheme, "store": args.store, "n_sites_full": wl.n_sites,
+                   "n_sites_sample": n, "lb_steps_per_step": lb_per_step, "tau": wl.tau,
+                   "host_cpu": host_cpu_model(), "host_cores": os.cpu_count()},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------- our arm
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+    if args.inner < 2 or args.inner % 2:
+        raise SystemExit("--inner must be even and >= 2 (A-A alternates two kernels)")
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the site update has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    import paper_1906_11925_b200 as hlb
+    import workloads as W
+
+    scheme = args.scheme or DEFAULT_SCHEME[args.workload]
+    t_gen = time.perf_counter()
+    wl = W.by_name(args.workload, small=args.small)
+    t_gen = time.perf_counter() - t_gen
+    flags = (hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE) | \
+            (hlb.HLB_STORE_F32 if args.store == "f32" else hlb.HLB_STORE_F64) | \
+            {"morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
+             "tiled": hlb.HLB_ORDER_TILED}[args.order]
+    t_create = time.perf_counter()
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t_create
+    N = g.n_sites
+    S = args.inner
+    if wl.rho0 is not None or wl.u0 is not None:
+        g.hlb_set_state(wl.rho0, wl.u0)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident timing: K x hlb_step(S)
+    for _ in range(args.warmup):
+        g.hlb_step(S)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    l0 = g.hlb_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    w0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        g.hlb_step(S)
+    ev1.record(stream)
+    barrier()
+    w1 = time.time()
+    clocks = sampler.stop(w0, w1)
+    ms = ev0.elapsed_time(ev1)
+    launches = g.hlb_launch_count() - l0
+
+    # ---------------- per-kernel durations (events around single launches, same stream)
+    reps = max(6, min(40, 2 * args.steps))
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(2 * reps)]
+    torch.cuda.synchronize()
+    parity0 = g.hlb_steps_done() & 1
+    for a, b in evs:
+        a.record(stream)
+        g.hlb_step(1)
+        b.record(stream)
+    torch.cuda.synchronize()
+    per = np.array([a.elapsed_time(b) for a, b in evs])
+    if scheme == "aa":
+        phase = (parity0 + np.arange(per.size)) & 1          # 0: even-phase kernel, 1: odd-phase
+        k_ms = {"k_aa<even>": float(np.mean(per[phase == 0])),
+                "k_aa<odd>": float(np.mean(per[phase == 1]))}
+        k_bytes = {"k_aa<even>": 15 * 2 * (4 if args.store == "f32" else 8),
+                   "k_aa<odd>": 15 * 2 * (4 if args.store == "f32" else 8) + 56}
+    else:
+        k_ms = {"k_pull": float(np.mean(per))}
+        k_bytes = {"k_pull": 15 * 2 * (4 if args.store == "f32" else 8) + 56}
+    dominant = max(k_ms, key=lambda k: k_ms[k])
+
+    # ---------------- end to end through the C-ABI with host buffers
+    e2e = None
+    if not args.no_e2e:
+        rho_h = torch.empty(N, dtype=torch.float64).pin_memory()
+        u_h = torch.empty((N, 3), dtype=torch.float64).pin_memory()
+        rho_in = torch.ones(N, dtype=torch.float64).pin_memory()
+        u_in = torch.zeros((N, 3), dtype=torch.float64).pin_memory()
+        if wl.rho0 is not None:
+            rho_in.numpy()[:] = wl.rho0
+        if wl.u0 is not None:
+            u_in.numpy()[:] = wl.u0
+        rho_np, u_np, rin_np, uin_np = rho_h.numpy(), u_h.numpy(), rho_in.numpy(), u_in.numpy()
+
+        def e2e_step():
+            g.hlb_set_state(rin_np, uin_np)             # H2D: rho [N], u [N][3]
+            g.hlb_step(S)
+            g.hlb_get_macroscopic(rho_np, u_np)        # D2H: rho [N], u [N][3] (synchronises)
+
+        e2e_steps = max(2, min(args.steps, 5))
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        barrier()
+        t_e2e = time.perf_counter() - t0
+        e2e = (t_e2e, e2e_steps)
+
+    # ---------------- aggregate over ranks (max time; total work)
+    ms_all, e2e_all = ms, (e2e[0] if e2e else 0.0)
+    if world > 1:
+        t = torch.tensor([ms, e2e_all], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_all, e2e_all = float(t[0]), float(t[1])
+    value = world * N * S * args.steps / (ms_all * 1e-3) / 1e6
+
+    peak, peak_src = measured_peak()
+    dom_ms = k_ms[dominant]
+    achieved = k_bytes[dominant] * N / (dom_ms * 1e-3) / 1e9
+    traffic = committed_traffic(args.workload, scheme, args.store, dominant)
+    step_bytes = hlb.algorithmic_bytes_per_site(scheme, args.store)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {
+            "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
+            "n_sites": N, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
+            "order": args.order, "tau": wl.tau, "n_iolets": wl.n_iolets,
+            "box": list(wl.shape), "seed": wl.info.get("seed"),
+            "device_bytes": g.hlb_device_bytes(),
+            "l2": "no flush: the populations + table (device_bytes) exceed the 126 MB L2"
+                  if g.hlb_device_bytes() > 4 * 126e6 else "working set is L2-sized: not an HBM measurement",
+            "parallelism": "replicas" if world > 1 else "single GPU",
+            "geometry_seconds": {"generate": round(t_gen, 2), "create": round(t_create, 2)},
+        },
+        "algorithmic_gbs": value * 1e6 * step_bytes / 1e9 / world,
+        "frac_of_measured_hbm": value * 1e6 * step_bytes / 1e9 / world / peak,
+        "frac_of_nominal_8000": value * 1e6 * step_bytes / 1e9 / world / 8000.0,
+        "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak,
+                     "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "bytes_per_site": k_bytes[dominant],
+                     "sites_per_launch": N, "ms_per_launch": dom_ms,
+                     "kernels": {k: {"ms": k_ms[k], "bytes_per_site": k_bytes[k],
+                                     "gbs": k_bytes[k] * N / (k_ms[k] * 1e-3) / 1e9} for k in k_ms}},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if e2e:
+        out["e2e"] = {"value": world * N * S * e2e[1] / e2e_all / 1e6, "unit": UNIT,
+                      "h2d_bytes_per_step": 32 * N, "d2h_bytes_per_step": 32 * N,
+                      "steps": e2e[1], "ms_per_step": e2e_all / e2e[1] * 1e3,
+                      "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}
+    g.close()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, n, st, dt, what, thr = time_oracle(wl, args.cpu_seconds, threads=1)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
+                               "sample": f"{what}: {n} sites x {st} LB steps in {dt:.1f} s",
+                               "host_cpu": host_cpu_model(), "host_cores": os.cpu_count()}
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
