@@ -64,6 +64,7 @@ def parse_args():
     ap.add_argument("--scheme", default=None, choices=["aa", "two_lattice"])
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--order", default="morton", choices=["morton", "raster", "tiled"])
+    ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="scaled-down geometry (debugging only)")
@@ -282,7 +283,9 @@ def main():
     flags = (hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE) | \
             (hlb.HLB_STORE_F32 if args.store == "f32" else hlb.HLB_STORE_F64) | \
             {"morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
-             "tiled": hlb.HLB_ORDER_TILED}[args.order]
+             "tiled": hlb.HLB_ORDER_TILED}[args.order] | \
+            {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
+             "records": hlb.HLB_LINKS_RECORDS}[args.links]
     t_create = time.perf_counter()
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
     torch.cuda.synchronize()
@@ -390,7 +393,8 @@ def main():
         "config": {
             "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
             "n_sites": N, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
-            "order": args.order, "tau": wl.tau, "n_iolets": wl.n_iolets,
+            "order": args.order, "links": "records" if g.hlb_uses_records() else "table",
+            "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
             "box": list(wl.shape), "seed": wl.info.get("seed"),
             "device_bytes": g.hlb_device_bytes(),
             "l2": "no flush: the populations + table (device_bytes) exceed the 126 MB L2"

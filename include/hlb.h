@@ -60,8 +60,12 @@ enum {
   HLB_ORDER_RASTER = 0x4,  /* internal order = canonical order                             */
   HLB_ORDER_TILED = 0x8,   /* Morton over 8x8x8 blocks, x-fastest raster inside a block    */
   HLB_ORDER_MASK = 0xC,
-  HLB_NO_GRAPH = 0x10      /* launch every step directly instead of replaying a captured
+  HLB_NO_GRAPH = 0x10,     /* launch every step directly instead of replaying a captured
                               CUDA graph of steps (debugging / profiling)                  */
+  HLB_LINKS_AUTO = 0x0,    /* the step kernels read the run-length link records when at
+                              least half of them are not sentinels, else the table         */
+  HLB_LINKS_TABLE = 0x20,  /* always read the int32 table (ablation / profiling)           */
+  HLB_LINKS_RECORDS = 0x40 /* always read the records                                     */
 };
 
 typedef struct hlb_geometry hlb_geometry; /* opaque handle */
@@ -129,6 +133,10 @@ int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v);
 int64_t hlb_device_bytes(const hlb_geometry* g);
 /* Kernel launches enqueued by hlb_step() so far (graph replays count their nodes). */
 int64_t hlb_launch_count(const hlb_geometry* g);
+/* 1 if the step kernels of this geometry read the link records, 0 if they read the table. */
+int hlb_uses_records(const hlb_geometry* g);
+/* Fraction of (group, q) link records that are sentinels (see hlb_preprocess_records). */
+double hlb_record_sentinel_fraction(const hlb_geometry* g);
 
 void hlb_geometry_destroy(hlb_geometry* g); /* NULL is a no-op                            */
 const char* hlb_last_error(void);           /* thread-local, never NULL                   */
@@ -154,6 +162,21 @@ int hlb_preprocess_count(const uint8_t* site_type, const hlb_params* p, int64_t*
                          int64_t* stride);
 int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t* voxel_of_site,
                           int32_t* canon_of_site, int32_t* nbr);
+
+/* Run-length link records of a table (host only): the compressed form of nbr that the step
+ * kernels read. A group is 32 consecutive internal sites (one warp). For group g and link q
+ * the record rec[(g*14 + (q-1))*4 .. +4] = { wall, start, base0, base1 }:
+ *   wall   bit l set: the entry of lane l is negative (solid or iolet: bounce-back target)
+ *   start  bit l set: lane l is not a wall lane and begins a run, i.e. lane l-1 is a wall
+ *          lane or nbr[lane l] != nbr[lane l-1] + 1
+ *   base0, base1: the table entries of the first lanes of run 0 and run 1
+ * so that the entry of a non-wall lane l in run r, which started at lane s, is
+ * base_r + (l - s). A (g, q) with more than two runs gets the sentinel {0, 0, 0, 0} (a real
+ * record never has wall == 0 and start == 0) and the kernels read nbr for it instead.
+ *   nbr: HOST [14][stride] as filled by hlb_preprocess_tables; stride a multiple of 32
+ *   rec: HOST [stride/32][14][4] uint32, filled
+ *   n_sentinel: number of (g, q) that got the sentinel (may be NULL) */
+int hlb_preprocess_records(const int32_t* nbr, int64_t stride, uint32_t* rec, int64_t* n_sentinel);
 
 #ifdef __cplusplus
 }

@@ -20,6 +20,7 @@ HLB_STORE_F64, HLB_STORE_F32 = 0x0, 0x1
 HLB_TWO_LATTICE, HLB_AA = 0x0, 0x2
 HLB_ORDER_MORTON, HLB_ORDER_RASTER, HLB_ORDER_TILED = 0x0, 0x4, 0x8
 HLB_NO_GRAPH = 0x10
+HLB_LINKS_AUTO, HLB_LINKS_TABLE, HLB_LINKS_RECORDS = 0x0, 0x20, 0x40
 
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 
@@ -62,6 +63,9 @@ def _load() -> ctypes.CDLL:
         "hlb_get_site_voxels": (c_int, [vp, vp]),
         "hlb_device_bytes": (i64, [vp]),
         "hlb_launch_count": (i64, [vp]),
+        "hlb_uses_records": (c_int, [vp]),
+        "hlb_record_sentinel_fraction": (ctypes.c_double, [vp]),
+        "hlb_preprocess_records": (c_int, [vp, i64, vp, ctypes.POINTER(i64)]),
         "hlb_geometry_destroy": (None, [vp]),
         "hlb_last_error": (ctypes.c_char_p, []),
         "hlb_velocity_set": (None, [vp, vp, vp]),
@@ -81,8 +85,10 @@ _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
             "hlb_set_populations", "hlb_num_sites", "hlb_steps_done", "hlb_get_site_voxels",
-            "hlb_device_bytes", "hlb_launch_count", "hlb_geometry_destroy", "hlb_last_error",
-            "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables")
+            "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
+            "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
+            "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables",
+            "hlb_preprocess_records")
 
 
 def hlb_last_error() -> str:
@@ -142,6 +148,18 @@ def hlb_preprocess(site_type, periodic=0, n_iolets=0, flags=0):
     nbr = np.zeros((14, Ns), dtype=np.int32)
     _check(_lib.hlb_preprocess_tables(_ptr(st), ctypes.byref(p), _ptr(vox), _ptr(canon), _ptr(nbr)))
     return {"N": N, "Ns": Ns, "voxel_of_site": vox, "canon_of_site": canon, "nbr": nbr}
+
+
+def hlb_preprocess_records(nbr):
+    """Run-length link records of a [14, Ns] table: (rec [Ns/32, 14, 4] uint32, n_sentinel)."""
+    nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+    if nbr.ndim != 2 or nbr.shape[0] != 14:
+        raise ValueError("nbr must be [14, Ns]")
+    ns = nbr.shape[1]
+    rec = np.zeros((max(ns // 32, 0), 14, 4), dtype=np.uint32)
+    n = ctypes.c_int64(0)
+    _check(_lib.hlb_preprocess_records(_ptr(nbr), ns, _ptr(rec), ctypes.byref(n)))
+    return rec, n.value
 
 
 class Geometry:
@@ -231,6 +249,12 @@ class Geometry:
 
     def hlb_launch_count(self) -> int:
         return int(_lib.hlb_launch_count(self._h))
+
+    def hlb_uses_records(self) -> bool:
+        return bool(_lib.hlb_uses_records(self._h))
+
+    def hlb_record_sentinel_fraction(self) -> float:
+        return float(_lib.hlb_record_sentinel_fraction(self._h))
 
     def hlb_geometry_destroy(self):
         if self._h:

@@ -56,6 +56,7 @@ struct hlb_geometry {
   int cur = 0;                        // two-lattice: buffer the next step reads
   double* scratch = nullptr;          // [N][15] doubles: staging for host<->device transfers
   int64_t steps = 0, launches = 0, device_bytes = 0;
+  double sentinel_fraction = 0.0;     // of the (group, q) link records
   std::vector<void*> owned;           // cudaMalloc'ed (no allocator callback)
 
   int alloc(size_t bytes, void** out) {
@@ -102,8 +103,11 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->n_iolets < 0 || p->n_iolets > 253) return fail(HLB_EINVAL, "n_iolets must be in 0..253");
   if (p->n_iolets > 0 && !p->iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
-  if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH))
+  if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
+                             HLB_LINKS_TABLE | HLB_LINKS_RECORDS))
     return fail(HLB_EINVAL, "unknown flag bits");
+  if ((p->flags & HLB_LINKS_TABLE) && (p->flags & HLB_LINKS_RECORDS))
+    return fail(HLB_EINVAL, "HLB_LINKS_TABLE and HLB_LINKS_RECORDS are exclusive");
   bool ok;
   order = order_of(p->flags, ok);
   if (!ok) return fail(HLB_EINVAL, "unknown HLB_ORDER_* value");
@@ -139,6 +143,14 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
   return HLB_OK;
 }
 
+int hlb_preprocess_records(const int32_t* nbr, int64_t stride, uint32_t* rec, int64_t* n_sentinel) {
+  if (!nbr || !rec) return fail(HLB_EINVAL, "NULL argument");
+  if (stride <= 0 || stride % 32) return fail(HLB_EINVAL, "stride must be a positive multiple of 32");
+  const int64_t n = build_link_records(nbr, stride, rec);
+  if (n_sentinel) *n_sentinel = n;
+  return HLB_OK;
+}
+
 int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geometry** out) {
   if (out) *out = nullptr;
   if (!out) return fail(HLB_EINVAL, "out is NULL");
@@ -170,10 +182,16 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   for (int64_t i = 0; i < t.N; ++i) g->canon_voxels[(size_t)t.canon_of_site[(size_t)i]] = t.voxel_of_site[(size_t)i];
 
   void *d_nbr = nullptr, *d_bits = nullptr, *d_canon = nullptr, *d_rho = nullptr, *d_scratch = nullptr;
+  void* d_rec = nullptr;
+  g->sentinel_fraction = (double)t.n_rec_fallback / (double)((t.Ns / 32) * (Q - 1));
+  const bool use_rec = (p->flags & HLB_LINKS_RECORDS) ? true
+                       : (p->flags & HLB_LINKS_TABLE) ? false
+                                                      : g->sentinel_fraction <= 0.5;
   const size_t pop_bytes = (size_t)Q * (size_t)t.Ns * g->store_bytes();
   auto bail = [&](int code) { hlb_geometry_destroy(g); return code; };
   if ((rc = g->alloc(sizeof(int32_t) * t.nbr.size(), &d_nbr))) return bail(rc);
   if ((rc = g->alloc(sizeof(uint32_t) * t.iolet_bits.size(), &d_bits))) return bail(rc);
+  if (use_rec && (rc = g->alloc(sizeof(uint32_t) * t.rec.size(), &d_rec))) return bail(rc);
   if ((rc = g->alloc(sizeof(int32_t) * (size_t)t.N, &d_canon))) return bail(rc);
   if ((rc = g->alloc(sizeof(double) * (size_t)(p->n_iolets > 0 ? p->n_iolets : 1), &d_rho))) return bail(rc);
   if ((rc = g->alloc(pop_bytes, &g->buf[0]))) return bail(rc);
@@ -188,6 +206,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   } while (0)
   HLB_CUDA_G(cudaMemcpyAsync(d_nbr, t.nbr.data(), sizeof(int32_t) * t.nbr.size(), cudaMemcpyHostToDevice, g->stream));
   HLB_CUDA_G(cudaMemcpyAsync(d_bits, t.iolet_bits.data(), sizeof(uint32_t) * t.iolet_bits.size(), cudaMemcpyHostToDevice, g->stream));
+  if (use_rec)
+    HLB_CUDA_G(cudaMemcpyAsync(d_rec, t.rec.data(), sizeof(uint32_t) * t.rec.size(), cudaMemcpyHostToDevice, g->stream));
   HLB_CUDA_G(cudaMemcpyAsync(d_canon, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N, cudaMemcpyHostToDevice, g->stream));
   if (p->n_iolets > 0)
     HLB_CUDA_G(cudaMemcpyAsync(d_rho, g->iolet_rho.data(), sizeof(double) * (size_t)p->n_iolets, cudaMemcpyHostToDevice, g->stream));
@@ -195,6 +215,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.Ns = t.Ns;
   g->dg.nbr = (const int32_t*)d_nbr;
   g->dg.iolet_bits = (const uint32_t*)d_bits;
+  g->dg.rec = d_rec;
+  g->dg.use_rec = use_rec;
   g->dg.canon = (const int32_t*)d_canon;
   g->dg.iolet_rho = (const double*)d_rho;
   g->dg.omega = 1.0 / p->tau;
@@ -309,6 +331,8 @@ int64_t hlb_num_sites(const hlb_geometry* g) { return g ? g->N : (int64_t)HLB_EI
 int64_t hlb_steps_done(const hlb_geometry* g) { return g ? g->steps : (int64_t)HLB_EINVAL; }
 int64_t hlb_device_bytes(const hlb_geometry* g) { return g ? g->device_bytes : (int64_t)HLB_EINVAL; }
 int64_t hlb_launch_count(const hlb_geometry* g) { return g ? g->launches : (int64_t)HLB_EINVAL; }
+int hlb_uses_records(const hlb_geometry* g) { return g ? (g->dg.use_rec ? 1 : 0) : (int)HLB_EINVAL; }
+double hlb_record_sentinel_fraction(const hlb_geometry* g) { return g ? g->sentinel_fraction : -1.0; }
 int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v) {
   if (!g || !v) return fail(HLB_EINVAL, "NULL argument");
   std::memcpy(v, g->canon_voxels.data(), sizeof(int64_t) * (size_t)g->N);

@@ -20,7 +20,15 @@
 namespace hlb {
 namespace {
 
-constexpr int BLOCK = 256;
+constexpr int BLOCK = 256;   // read-out / init kernels
+
+#ifndef HLB_STEP_BLOCK
+#define HLB_STEP_BLOCK 128   // Ns is a multiple of 128: the step kernels need no bounds test
+#endif
+#ifndef HLB_STEP_MINB
+#define HLB_STEP_MINB 6      // resident blocks per SM the register budget is tuned for
+#endif
+constexpr int SBLOCK = HLB_STEP_BLOCK;
 
 __device__ __forceinline__ int iolet_of(int32_t e) {  // -1: not an iolet link
   return e < 0 ? (int)(e & 0x7fffffff) - 1 : -1;
@@ -31,6 +39,39 @@ __device__ __forceinline__ void load_entries(const int32_t* __restrict__ nbr, lo
                                              long long i, int32_t (&e)[Q - 1]) {
 #pragma unroll
   for (int q = 1; q < Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+}
+
+// Link entries of site i for the step kernels: >= 0 source site, < 0 bounce-back target
+// (the iolet id is NOT decoded here; the rare iolet path reloads the table). With REC the
+// warp reads one 16-byte record per link instead of 32 table entries (include/hlb.h,
+// hlb_preprocess_records); a sentinel record sends the whole warp to the table.
+template <bool REC>
+__device__ __forceinline__ void load_links(const int32_t* __restrict__ nbr,
+                                           const uint4* __restrict__ rec, long long Ns,
+                                           long long i, int32_t (&e)[Q - 1]) {
+  if (!REC) {
+#pragma unroll
+    for (int q = 1; q < Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+    return;
+  }
+  const int lane = threadIdx.x & 31;
+  const uint4* r = rec + (i >> 5) * (Q - 1);
+  uint4 v[Q - 1];
+#pragma unroll
+  for (int q = 1; q < Q; ++q) v[q - 1] = __ldg(r + (q - 1));
+  const uint32_t le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
+#pragma unroll
+  for (int q = 1; q < Q; ++q) {
+    const uint4 t = v[q - 1];
+    if ((t.x | t.y) == 0u) {  // sentinel (warp-uniform): more than two runs
+      e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+    } else {
+      const uint32_t le = t.y & le_mask;           // run starts at or below this lane
+      const int s = 31 - __clz((int)le);           // lane the run started at
+      const int base = (le & (le - 1)) ? (int)t.w : (int)t.z;  // second run iff two starts
+      e[q - 1] = ((t.x >> lane) & 1u) ? (int32_t)0x80000000 : base + (lane - s);
+    }
+  }
 }
 
 // Address (element offset) where the pre-collision f_q(x) of link q lives.
@@ -44,55 +85,74 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
   return wall ? (long long)q * Ns + i : (long long)opp(q) * Ns + e;
 }
 
-// Replace, for every iolet link p of this site, the value that will be read back as
-// f_p(x, t+1) by the constant-density equilibrium f_eq_p(rho_k, u(x, t)) (reading A6).
-// out[p] is that value; for non-iolet links it keeps the bounced post-collision value.
-__device__ __forceinline__ void iolet_substitute(const int32_t (&e)[Q - 1], const Moments& m,
-                                                 const double* __restrict__ iolet_rho,
-                                                 double (&out)[Q]) {
-#pragma unroll
+// Rare path (sites on an inlet/outlet cap): for every iolet link p of site i replace
+// out[p] -- the value that will be read back as f_p(x, t+1) -- by the constant-density
+// equilibrium f_eq_p(rho_k, u(x, t)) (reading A6). The table entries are re-read here so
+// that the common path does not keep them in registers.
+__device__ __noinline__ void iolet_substitute_slow(const int32_t* __restrict__ nbr, long long Ns,
+                                                   long long i, double ux, double uy, double uz,
+                                                   const double* __restrict__ iolet_rho,
+                                                   double* __restrict__ out) {
+#pragma unroll 1
   for (int p = 1; p < Q; ++p) {
-    const int k = iolet_of(e[p - 1]);
+    const int k = iolet_of(__ldg(nbr + (long long)(p - 1) * Ns + i));
     if (k >= 0) {
       const double rk = __ldg(iolet_rho + k);
-      out[p] = heq_of(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+      const double cu = (double)cx_rt(p) * ux + (double)cy_rt(p) * uy + (double)cz_rt(p) * uz;
+      const double uu = ux * ux + uy * uy + uz * uz;
+      out[p] = weight_rt(p) * ((rk - 1.0) + rk * (3.0 * cu + 4.5 * cu * cu - 1.5 * uu));
     }
   }
+}
+
+// out[] stays in registers on the common path: only the rare path copies it through the
+// stack for the out-of-line call.
+__device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
+                                                 long long i, const Moments& m,
+                                                 const double* __restrict__ iolet_rho,
+                                                 double (&out)[Q]) {
+  double tmp[Q];
+#pragma unroll
+  for (int p = 1; p < Q; ++p) tmp[p] = out[p];
+  iolet_substitute_slow(nbr, Ns, i, m.ux, m.uy, m.uz, iolet_rho, tmp);
+#pragma unroll
+  for (int p = 1; p < Q; ++p) out[p] = tmp[p];
+}
+
+__device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iolet_bits, long long i) {
+  return (__ldg(iolet_bits + (i >> 5)) >> (threadIdx.x & 31)) & 1u;
 }
 
 // ------------------------------------------------------------------ two-lattice pull
 // src holds post-collision values h*(., t-1) (iolet slots substituted); one launch does
 // gather -> moments -> BGK -> store of h*(., t) into dst (rows S1..S6 fused).
-template <typename ST>
-__global__ void __launch_bounds__(BLOCK)
+template <typename ST, bool REC>
+__global__ void __launch_bounds__(SBLOCK, HLB_STEP_MINB)
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
+       const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
        const double* __restrict__ iolet_rho, long long Ns, double omega) {
-  const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
-  if (i >= Ns) return;
-  int32_t e[Q - 1];
-  load_entries<ST>(nbr, Ns, i, e);
+  const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[Q];
-  h[0] = to_real(src[i]);
-  int io = 0;
+  {
+    int32_t e[Q - 1];
+    load_links<REC>(nbr, rec, Ns, i, e);
+    h[0] = to_real(src[i]);
 #pragma unroll
-  for (int q = 1; q < Q; ++q) {
-    h[q] = to_real(src[slot_of<GATHER_PULL>(q, e[q - 1], Ns, i)]);
-    io |= e[q - 1] < 0 ? (e[q - 1] & 0x7fffffff) : 0;
+    for (int q = 1; q < Q; ++q) h[q] = to_real(src[slot_of<GATHER_PULL>(q, e[q - 1], Ns, i)]);
   }
   const Moments m = moments_of(h);
-  double hs[Q];
-  collide(h, m, omega, hs);
-  if (io) {  // rare: sites on an inlet/outlet cap
+  collide(h, m, omega, h);
+  if (has_iolet_link(iolet_bits, i)) {  // rare: sites on an inlet/outlet cap
     // slot opp(p) of this site is read back by link p next step
     double back[Q];
 #pragma unroll
-    for (int p = 1; p < Q; ++p) back[p] = hs[opp(p)];
-    iolet_substitute(e, m, iolet_rho, back);
+    for (int p = 1; p < Q; ++p) back[p] = h[opp(p)];
+    iolet_substitute(nbr, Ns, i, m, iolet_rho, back);
 #pragma unroll
-    for (int p = 1; p < Q; ++p) hs[opp(p)] = back[p];
+    for (int p = 1; p < Q; ++p) h[opp(p)] = back[p];
   }
 #pragma unroll
-  for (int q = 0; q < Q; ++q) dst[(long long)q * Ns + i] = to_store<ST>(hs[q]);
+  for (int q = 0; q < Q; ++q) dst[(long long)q * Ns + i] = to_store<ST>(h[q]);
 }
 
 // ------------------------------------------------------------------ A-A in place
@@ -100,42 +160,46 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // Odd phase: read f_q from slot opp(q) of x - c_q (slot q of x at a wall), write h*_q to
 // the address f_opp(q) was read from. Read set = write set per site in both phases, so one
 // array and no inter-thread hazards.
-template <typename ST, bool ODD>
-__global__ void __launch_bounds__(BLOCK)
-k_aa(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint32_t* __restrict__ iolet_bits,
-     const double* __restrict__ iolet_rho, long long Ns, double omega) {
-  const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
-  if (i >= Ns) return;
-  int32_t e[Q - 1];
-  bool io;
-  if (ODD) {
-    load_entries<ST>(nbr, Ns, i, e);
-    int any = 0;
-#pragma unroll
-    for (int q = 1; q < Q; ++q) any |= e[q - 1] < 0 ? (e[q - 1] & 0x7fffffff) : 0;
-    io = any != 0;
-  } else {
-    io = (__ldg(iolet_bits + (i >> 5)) >> (i & 31)) & 1u;
-    if (io) load_entries<ST>(nbr, Ns, i, e);
-  }
-  long long addr[Q];
+template <typename ST>
+__global__ void __launch_bounds__(SBLOCK, HLB_STEP_MINB)
+k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
+          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
+          long long Ns, double omega) {
+  const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[Q];
-  addr[0] = i;
 #pragma unroll
-  for (int q = 1; q < Q; ++q)
-    addr[q] = ODD ? slot_of<GATHER_AA_ODD>(q, e[q - 1], Ns, i) : slot_of<GATHER_OWN>(q, 0, Ns, i);
-#pragma unroll
-  for (int q = 0; q < Q; ++q) h[q] = to_real(a[addr[q]]);
+  for (int q = 0; q < Q; ++q) h[q] = to_real(a[(long long)q * Ns + i]);
   const Moments m = moments_of(h);
-  double hs[Q];
-  collide(h, m, omega, hs);
+  collide(h, m, omega, h);
   double out[Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
-  out[0] = hs[0];
 #pragma unroll
-  for (int p = 1; p < Q; ++p) out[p] = hs[opp(p)];
-  if (io) iolet_substitute(e, m, iolet_rho, out);
+  for (int p = 0; p < Q; ++p) out[p] = h[opp(p)];
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute(nbr, Ns, i, m, iolet_rho, out);
 #pragma unroll
-  for (int p = 0; p < Q; ++p) a[addr[p]] = to_store<ST>(out[p]);
+  for (int p = 0; p < Q; ++p) a[(long long)p * Ns + i] = to_store<ST>(out[p]);
+}
+
+template <typename ST, bool REC>
+__global__ void __launch_bounds__(SBLOCK, HLB_STEP_MINB)
+k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
+         const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
+         long long Ns, double omega) {
+  const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
+  int32_t e[Q - 1];
+  load_links<REC>(nbr, rec, Ns, i, e);
+  double h[Q];
+  h[0] = to_real(a[i]);
+#pragma unroll
+  for (int q = 1; q < Q; ++q) h[q] = to_real(a[slot_of<GATHER_AA_ODD>(q, e[q - 1], Ns, i)]);
+  const Moments m = moments_of(h);
+  collide(h, m, omega, h);
+  double out[Q];
+#pragma unroll
+  for (int p = 0; p < Q; ++p) out[p] = h[opp(p)];
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute(nbr, Ns, i, m, iolet_rho, out);
+  a[i] = to_store<ST>(out[0]);
+#pragma unroll
+  for (int p = 1; p < Q; ++p) a[slot_of<GATHER_AA_ODD>(p, e[p - 1], Ns, i)] = to_store<ST>(out[p]);
 }
 
 // ------------------------------------------------------------------ read-out / init
@@ -232,24 +296,36 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + BLOCK - 1) / BLOC
 
 }  // namespace
 
-void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  if (g.f32)
-    k_pull<float><<<grid_for(g.Ns), BLOCK, 0, s>>>((const float*)src, (float*)dst, g.nbr,
-                                                   g.iolet_rho, g.Ns, g.omega);
+template <typename ST>
+static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+  const unsigned grid = (unsigned)(g.Ns / SBLOCK);
+  if (g.use_rec)
+    k_pull<ST, true><<<grid, SBLOCK, 0, s>>>((const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec,
+                                             g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
   else
-    k_pull<double><<<grid_for(g.Ns), BLOCK, 0, s>>>((const double*)src, (double*)dst, g.nbr,
-                                                    g.iolet_rho, g.Ns, g.omega);
+    k_pull<ST, false><<<grid, SBLOCK, 0, s>>>((const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec,
+                                              g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
+}
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+  if (g.f32) pull_t<float>(g, src, dst, s);
+  else pull_t<double>(g, src, dst, s);
 }
 
+template <typename ST>
+static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
+  const unsigned grid = (unsigned)(g.Ns / SBLOCK);
+  if (!odd)
+    k_aa_even<ST><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
+  else if (g.use_rec)
+    k_aa_odd<ST, true><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
+                                               g.iolet_rho, g.Ns, g.omega);
+  else
+    k_aa_odd<ST, false><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
+                                                g.iolet_rho, g.Ns, g.omega);
+}
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
-  const unsigned grid = grid_for(g.Ns);
-  if (g.f32) {
-    if (odd) k_aa<float, true><<<grid, BLOCK, 0, s>>>((float*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
-    else k_aa<float, false><<<grid, BLOCK, 0, s>>>((float*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
-  } else {
-    if (odd) k_aa<double, true><<<grid, BLOCK, 0, s>>>((double*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
-    else k_aa<double, false><<<grid, BLOCK, 0, s>>>((double*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
-  }
+  if (g.f32) aa_t<float>(g, a, odd, s);
+  else aa_t<double>(g, a, odd, s);
 }
 
 template <typename ST>

@@ -11,6 +11,8 @@ struct DeviceGeometry {
   int64_t Ns = 0;                       // plane stride (multiple of 128), arrays are [15][Ns]
   const int32_t* nbr = nullptr;         // [14][Ns] pull-neighbour table (include/hlb.h)
   const uint32_t* iolet_bits = nullptr; // [Ns/32]
+  const void* rec = nullptr;            // [Ns/32][14] 16-byte link records (include/hlb.h)
+  bool use_rec = false;                 // step kernels read rec instead of nbr
   const int32_t* canon = nullptr;       // [N] internal -> canonical rank
   const double* iolet_rho = nullptr;    // [n_iolets]
   double omega = 1.0;                   // 1 / tau

@@ -103,6 +103,44 @@ struct BlockIndex {
 
 int preprocess_threads() { return thread_count(); }
 
+// A group is 32 consecutive sites (one warp). For link q of a group, the lanes whose pull
+// source is a fluid site split into runs of lanes with consecutive source indices; with an
+// x-fastest site order almost every (group, q) has one or two runs, and 16 bytes then
+// replace the 128 bytes of table entries the warp would load.
+int64_t build_link_records(const int32_t* nbr, int64_t Ns, uint32_t* rec) {
+  const int64_t G = Ns / 32;
+  std::atomic<int64_t> fallback{0};
+  parallel_for(G, 1 << 10, [&](int64_t gb, int64_t ge) {
+    int64_t fb = 0;
+    for (int64_t g = gb; g < ge; ++g) {
+      for (int q = 1; q < Q; ++q) {
+        const int32_t* e = nbr + (int64_t)(q - 1) * Ns + g * 32;
+        uint32_t wall = 0, start = 0;
+        int32_t base[2] = {0, 0};
+        int runs = 0;
+        for (int l = 0; l < 32; ++l) {
+          if (e[l] < 0) { wall |= 1u << l; continue; }
+          const bool cont = l > 0 && e[l - 1] >= 0 && e[l] == e[l - 1] + 1;
+          if (!cont) {
+            if (runs < 2) base[runs] = e[l];
+            ++runs;
+            start |= 1u << l;
+          }
+        }
+        uint32_t* r = rec + ((size_t)g * (Q - 1) + (size_t)(q - 1)) * 4;
+        if (runs > 2) {
+          r[0] = r[1] = r[2] = r[3] = 0u;  // sentinel: read the table itself
+          ++fb;
+        } else {
+          r[0] = wall; r[1] = start; r[2] = (uint32_t)base[0]; r[3] = (uint32_t)base[1];
+        }
+      }
+    }
+    fallback += fb;
+  });
+  return fallback.load();
+}
+
 int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, int n_iolets,
                SiteOrder order, bool count_only, GeometryTables& out, std::string& err) {
   if (!type) { err = "site_type is NULL"; return HLB_EINVAL; }
@@ -312,6 +350,10 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
   });
   out.n_iolet_sites = n_io_sites.load();
   out.n_wall_links = n_wall_links.load();
+
+  // ---- pass E: run-length link records
+  out.rec.assign((size_t)(Ns / 32) * (Q - 1) * 4, 0u);
+  out.n_rec_fallback = build_link_records(out.nbr.data(), Ns, out.rec.data());
   return HLB_OK;
 }
 

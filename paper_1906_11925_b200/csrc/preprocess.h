@@ -16,6 +16,8 @@ struct GeometryTables {
   std::vector<int32_t> canon_of_site;  // [N]  internal order -> canonical rank
   std::vector<int32_t> nbr;            // [14][Ns], encoding: include/hlb.h
   std::vector<uint32_t> iolet_bits;    // [Ns/32] bit (i & 31) of word i >> 5: site i has an iolet link
+  std::vector<uint32_t> rec;           // [Ns/32][14][4] run-length link records (include/hlb.h)
+  int64_t n_rec_fallback = 0;          // (group, q) pairs with more than 2 runs (record = sentinel)
   int64_t n_iolet_sites = 0;
   int64_t n_wall_links = 0;
 };
@@ -24,6 +26,10 @@ struct GeometryTables {
 // are left empty and only N / Ns are set.
 int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, int n_iolets,
                SiteOrder order, bool count_only, GeometryTables& out, std::string& err);
+
+// Run-length link records of a finished table: rec [Ns/32][14][4] (encoding: include/hlb.h,
+// hlb_preprocess_records). Returns the number of (group, q) pairs that got the sentinel.
+int64_t build_link_records(const int32_t* nbr, int64_t Ns, uint32_t* rec);
 
 int preprocess_threads();
 

@@ -26,10 +26,11 @@ def hlb():
     return m
 
 
-def flags_of(hlb, scheme, store, order="morton"):
+def flags_of(hlb, scheme, store, order="morton", links="auto"):
     f = hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE
     f |= hlb.HLB_STORE_F32 if store == "f32" else hlb.HLB_STORE_F64
     f |= {"morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER, "tiled": hlb.HLB_ORDER_TILED}[order]
+    f |= {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE, "records": hlb.HLB_LINKS_RECORDS}[links]
     return f
 
 
@@ -40,9 +41,11 @@ def errors(rho, u, rho_ref, u_ref):
     return e_rho, e_u
 
 
-def run_gpu(hlb, wl, steps, scheme, store, order="morton"):
+def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto"):
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
-                                flags_of(hlb, scheme, store, order))
+                                flags_of(hlb, scheme, store, order, links))
+    if links != "auto":
+        assert g.hlb_uses_records() == (links == "records")
     if wl.rho0 is not None or wl.u0 is not None:
         g.hlb_set_state(wl.rho0, wl.u0)
     g.hlb_step(steps)
@@ -79,6 +82,32 @@ def test_small_configs_match_oracle(hlb, name, scheme, store):
         assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
 
 
+@pytest.mark.parametrize("store", ["f64", "f32"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+@pytest.mark.parametrize("name", W.CONFIG_NAMES)
+def test_small_configs_match_oracle_through_link_records(hlb, name, scheme, store):
+    """The run-length link records (the form the step kernels read on x-fastest orders)
+    against the oracle, raster order, records forced."""
+    wl = W.by_name(name, small=True)
+    steps = wl.steps + 1
+    rho_ref, u_ref = oracle_cached(name, steps)
+    rho, u = run_gpu(hlb, wl, steps, scheme, store, "raster", "records")
+    e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+    assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
+
+
+@pytest.mark.parametrize("order", ["morton", "raster", "tiled"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_link_records_and_table_agree_bitwise(hlb, scheme, order):
+    """Records and table describe the same links: bitwise identical results, whatever the
+    share of sentinel records (morton: nearly all; raster: few)."""
+    for name, steps in (("aneurysm", 33), ("cube", 12)):
+        wl = W.by_name(name, small=True)
+        a = run_gpu(hlb, wl, steps, scheme, "f64", order, "table")
+        b = run_gpu(hlb, wl, steps, scheme, "f64", order, "records")
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
 @pytest.mark.parametrize("order", ["raster", "tiled"])
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
 def test_result_is_independent_of_site_order(hlb, scheme, order):
@@ -109,9 +138,10 @@ def test_aa_equals_two_lattice_bitwise(hlb, store):
 def test_random_masks_match_oracle(hlb, scheme, seed, periodic, shape):
     wl = W.random_mask(shape, p_fluid=0.6, n_iolets=3, p_iolet=0.06, periodic=periodic,
                        tau=0.55 + 0.07 * seed, seed=200 + seed)
+    links, order = ("records", "raster") if seed % 2 else ("table", "morton")
     for steps in (0, 1, 2, 9, 10):
         rho_ref, u_ref = run_oracle(wl, steps, threads=1)
-        rho, u = run_gpu(hlb, wl, steps, scheme, "f64")
+        rho, u = run_gpu(hlb, wl, steps, scheme, "f64", order, links)
         e_rho, e_u = errors(rho, u, rho_ref, u_ref)
         assert e_rho < 1e-13 and e_u < 1e-12, (steps, e_rho, e_u)
 

@@ -117,3 +117,72 @@ def test_argument_errors():
     assert e.value.code == hlb.HLB_EINVAL
     t = hlb.hlb_preprocess(st, 0, 0, 0)                                # isolated site: all walls
     assert t["N"] == 1 and np.all(t["nbr"] == WALL)
+
+
+# ------------------------------------------------------------------ run-length link records
+def decode_records(rec, nbr):
+    """Pure-numpy reading of include/hlb.h's record encoding: returns (entries, sentinel)
+    with entries[q-1, i] = decoded source index, -1 at wall lanes, and sentinel[g, q-1]."""
+    G = rec.shape[0]
+    out = np.full((14, G * 32), -1, dtype=np.int64)
+    sentinel = np.zeros((G, 14), dtype=bool)
+    for g in range(G):
+        for k in range(14):
+            wall, start, b0, b1 = (int(v) for v in rec[g, k])
+            if wall == 0 and start == 0:
+                sentinel[g, k] = True
+                continue
+            for l in range(32):
+                if (wall >> l) & 1:
+                    continue
+                le = start & ((2 << l) - 1)
+                assert le != 0, "a non-wall lane must belong to a run"
+                s = le.bit_length() - 1
+                r = bin(le).count("1") - 1
+                assert r in (0, 1)
+                out[k, g * 32 + l] = np.int32(np.uint32(b1 if r else b0)) + (l - s)
+    return out, sentinel
+
+
+@pytest.mark.parametrize("order", [hlb.HLB_ORDER_MORTON, hlb.HLB_ORDER_RASTER, hlb.HLB_ORDER_TILED])
+@pytest.mark.parametrize("case", ["random", "random_periodic", "pipe", "tree"])
+def test_link_records_decode_to_the_table(order, case):
+    if case == "random":
+        wl = W.random_mask((24, 9, 7), p_fluid=0.8, n_iolets=2, p_iolet=0.05, seed=4)
+    elif case == "random_periodic":
+        wl = W.random_mask((64, 6, 5), p_fluid=1.1, n_iolets=0, periodic=7, seed=5)
+    else:
+        wl = W.by_name(case, small=True)
+    t = hlb.hlb_preprocess(wl.site_type, wl.periodic, wl.n_iolets, order)
+    nbr = t["nbr"].astype(np.int64)
+    rec, n_sentinel = hlb.hlb_preprocess_records(t["nbr"])
+    assert rec.shape == (t["Ns"] // 32, 14, 4)
+    dec, sentinel = decode_records(rec, nbr)
+    assert n_sentinel == int(sentinel.sum())
+    # brute-force run count per (group, q): sentinel <=> more than two runs
+    G = t["Ns"] // 32
+    nb = nbr.reshape(14, G, 32)
+    for g in range(G):
+        for k in range(14):
+            runs, prev = 0, None
+            for l in range(32):
+                e = nb[k, g, l]
+                if e < 0:
+                    prev = None
+                    continue
+                if prev is None or e != prev + 1:
+                    runs += 1
+                prev = e
+            assert sentinel[g, k] == (runs > 2)
+    keep = ~np.repeat(sentinel.T, 32, axis=1)              # [14, Ns]
+    expect = np.where(nbr >= 0, nbr, -1)
+    assert np.array_equal(dec[keep], expect[keep])
+    if order == hlb.HLB_ORDER_RASTER and case == "random_periodic":
+        assert n_sentinel < 0.6 * G * 14                    # x-runs make most records real
+
+
+def test_link_records_argument_errors():
+    with pytest.raises(hlb.HlbError):
+        hlb.hlb_preprocess_records(np.zeros((14, 33), dtype=np.int32))
+    with pytest.raises(ValueError):
+        hlb.hlb_preprocess_records(np.zeros((13, 32), dtype=np.int32))
