@@ -63,7 +63,7 @@ def parse_args():
     ap.add_argument("--workload", default="bigtree", choices=list(WORKLOAD_DESC))
     ap.add_argument("--scheme", default=None, choices=["aa", "two_lattice"])
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--order", default="morton", choices=["morton", "raster", "tiled"])
+    ap.add_argument("--order", default="auto", choices=["auto", "morton", "raster", "tiled"])
     ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -282,7 +282,7 @@ def main():
     t_gen = time.perf_counter() - t_gen
     flags = (hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE) | \
             (hlb.HLB_STORE_F32 if args.store == "f32" else hlb.HLB_STORE_F64) | \
-            {"morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
+            {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
              "tiled": hlb.HLB_ORDER_TILED}[args.order] | \
             {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
              "records": hlb.HLB_LINKS_RECORDS}[args.links]

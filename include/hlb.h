@@ -56,9 +56,11 @@ enum {
                               is h_q = f_q - w_q (reading R-shift)               */
   HLB_TWO_LATTICE = 0x0,   /* two population arrays, pull (gather) form                    */
   HLB_AA = 0x2,            /* one array updated in place, A-A pattern (even/odd steps)     */
-  HLB_ORDER_MORTON = 0x0,  /* internal site order: Morton (Z) curve over voxel coordinates */
-  HLB_ORDER_RASTER = 0x4,  /* internal order = canonical order                             */
-  HLB_ORDER_TILED = 0x8,   /* Morton over 8x8x8 blocks, x-fastest raster inside a block    */
+  HLB_ORDER_AUTO = 0x0,    /* internal site order: the library's choice -- currently raster,
+                              the fastest measured on B200       */
+  HLB_ORDER_MORTON = 0x4,  /* Morton (Z) curve over voxel coordinates                      */
+  HLB_ORDER_RASTER = 0x8,  /* internal order = canonical order (x fastest)                 */
+  HLB_ORDER_TILED = 0xC,   /* Morton over 8x8x8 blocks, x-fastest raster inside a block    */
   HLB_ORDER_MASK = 0xC,
   HLB_NO_GRAPH = 0x10,     /* launch every step directly instead of replaying a captured
                               CUDA graph of steps (debugging / profiling)                  */
@@ -106,7 +108,9 @@ int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho);
 
 /* Advance n >= 0 time steps: n launches of ONE fused collide-and-stream kernel (A-A:
  * alternating even/odd kernels), asynchronously on the stream. n == 0 is a no-op. A
- * kernel fault surfaces at the next synchronising call. */
+ * kernel fault surfaces at the next synchronising call. For geometries of up to 2^22
+ * sites on a non-NULL stream the launches are replayed from a captured CUDA graph in
+ * chunks of 32 steps (same kernels, same order; HLB_NO_GRAPH switches it off). */
 int hlb_step(hlb_geometry* g, int64_t n);
 
 /* rho(x) = sum_q f_q, u(x) = sum_q c_q f_q / rho of the PRE-collision populations after

@@ -18,7 +18,7 @@ from . import build as _build
 HLB_OK, HLB_EINVAL, HLB_ENOFLUID, HLB_ETOOLARGE, HLB_ENOMEM, HLB_ECUDA = 0, -1, -2, -3, -4, -5
 HLB_STORE_F64, HLB_STORE_F32 = 0x0, 0x1
 HLB_TWO_LATTICE, HLB_AA = 0x0, 0x2
-HLB_ORDER_MORTON, HLB_ORDER_RASTER, HLB_ORDER_TILED = 0x0, 0x4, 0x8
+HLB_ORDER_AUTO, HLB_ORDER_MORTON, HLB_ORDER_RASTER, HLB_ORDER_TILED = 0x0, 0x4, 0x8, 0xC
 HLB_NO_GRAPH = 0x10
 HLB_LINKS_AUTO, HLB_LINKS_TABLE, HLB_LINKS_RECORDS = 0x0, 0x20, 0x40
 

@@ -3,6 +3,7 @@
 // the hot path runs in the kernels of kernels.cu; nothing here computes on the host.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -35,6 +36,7 @@ int cuda_fail(cudaError_t e, const char* what) {
 SiteOrder order_of(uint32_t flags, bool& ok) {
   ok = true;
   switch (flags & HLB_ORDER_MASK) {
+    case HLB_ORDER_AUTO: return ORDER_RASTER;
     case HLB_ORDER_MORTON: return ORDER_MORTON;
     case HLB_ORDER_RASTER: return ORDER_RASTER;
     case HLB_ORDER_TILED: return ORDER_TILED;
@@ -57,6 +59,10 @@ struct hlb_geometry {
   double* scratch = nullptr;          // [N][15] doubles: staging for host<->device transfers
   int64_t steps = 0, launches = 0, device_bytes = 0;
   double sentinel_fraction = 0.0;     // of the (group, q) link records
+  // hlb_step(n) replays a captured CUDA graph of GRAPH_STEPS steps while n allows: removes
+  // the per-launch host cost that dominates small geometries (BASELINE configs[0], [2])
+  cudaGraphExec_t graph_exec = nullptr;
+  bool graph_failed = false;
   std::vector<void*> owned;           // cudaMalloc'ed (no allocator callback)
 
   int alloc(size_t bytes, void** out) {
@@ -233,6 +239,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
 
 void hlb_geometry_destroy(hlb_geometry* g) {
   if (!g) return;
+  if (g->graph_exec) cudaGraphExecDestroy(g->graph_exec);
   if (!g->owned.empty()) {
     cudaStreamSynchronize(g->stream);
     for (void* ptr : g->owned) cudaFree(ptr);
@@ -280,18 +287,65 @@ int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho) {
   return HLB_OK;
 }
 
+constexpr int64_t GRAPH_STEPS = 32;  // even: the buffer / phase parity is back where it started
+
+static void enqueue_one_step(hlb_geometry* g) {
+  if (g->aa) {
+    launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
+  } else {
+    launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->stream);
+    g->cur ^= 1;
+  }
+  ++g->steps;
+  ++g->launches;
+}
+
+// Capture GRAPH_STEPS steps starting at even parity (two-lattice: cur == 0; A-A: even
+// phase). Any failure just disables the graph path: the direct launches are equivalent.
+static void build_step_graph(hlb_geometry* g) {
+  cudaGraph_t graph = nullptr;
+  const int64_t steps0 = g->steps, launches0 = g->launches;
+  const int cur0 = g->cur;
+  if (cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    (void)cudaGetLastError();
+    g->graph_failed = true;
+    return;
+  }
+  for (int64_t s = 0; s < GRAPH_STEPS; ++s) enqueue_one_step(g);
+  const cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
+  g->steps = steps0;
+  g->launches = launches0;
+  g->cur = cur0;
+  if (e != cudaSuccess || !graph ||
+      cudaGraphInstantiate(&g->graph_exec, graph, 0) != cudaSuccess) {
+    (void)cudaGetLastError();
+    g->graph_exec = nullptr;
+    g->graph_failed = true;
+  }
+  if (graph) cudaGraphDestroy(graph);
+}
+
 int hlb_step(hlb_geometry* g, int64_t n) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   if (n < 0) return fail(HLB_EINVAL, "n < 0");
-  for (int64_t s = 0; s < n; ++s) {
-    if (g->aa) {
-      launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
-    } else {
-      launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->stream);
-      g->cur ^= 1;
+  // graphs pay off only when a step is short next to the launch cost
+  const bool want_graph = !(g->p.flags & HLB_NO_GRAPH) && !g->graph_failed && g->stream != nullptr &&
+                          g->N <= (int64_t)4 << 20;
+  int64_t left = n;
+  while (left > 0) {
+    const bool even = g->aa ? (g->steps & 1) == 0 : g->cur == 0;
+    if (want_graph && even && left >= GRAPH_STEPS && !g->graph_failed) {
+      if (!g->graph_exec) build_step_graph(g);
+      if (g->graph_exec) {
+        HLB_CUDA(cudaGraphLaunch(g->graph_exec, g->stream));
+        g->steps += GRAPH_STEPS;
+        g->launches += GRAPH_STEPS;
+        left -= GRAPH_STEPS;
+        continue;
+      }
     }
-    ++g->steps;
-    ++g->launches;
+    enqueue_one_step(g);
+    --left;
   }
   if (n > 0) HLB_CUDA(cudaGetLastError());
   return HLB_OK;

@@ -24,20 +24,6 @@ HLB_HD constexpr int cz(int q) { constexpr int t[Q] = {0, 0, 0, 0, 0, 1, -1, 1, 
 HLB_HD constexpr int opp(int q) { return q == 0 ? 0 : (((q - 1) ^ 1) + 1); }
 HLB_HD constexpr double weight(int q) { return q == 0 ? 2.0 / 9.0 : (q <= 6 ? 1.0 / 9.0 : 1.0 / 72.0); }
 
-// run-time q (loops that are deliberately not unrolled): sign patterns of the table above
-HLB_HD int cx_rt(int q) { return q == 0 || (q >= 3 && q <= 6) ? 0 : ((q & 1) ? 1 : -1); }
-HLB_HD int cy_rt(int q) {
-  if (q < 3 || q == 5 || q == 6) return 0;
-  const int s = (q & 1) ? 1 : -1;
-  return q >= 11 ? -s : s;
-}
-HLB_HD int cz_rt(int q) {
-  if (q < 5) return 0;
-  const int s = (q & 1) ? 1 : -1;
-  return (q == 9 || q == 10 || q == 13 || q == 14) ? -s : s;
-}
-HLB_HD double weight_rt(int q) { return q == 0 ? 2.0 / 9.0 : (q <= 6 ? 1.0 / 9.0 : 1.0 / 72.0); }
-
 // neighbour-table entry encoding (include/hlb.h, hlb_preprocess_tables)
 constexpr uint32_t NBR_WALL_BIT = 0x80000000u;
 HLB_HD constexpr bool nbr_is_wall(int32_t e) { return e < 0; }                 // solid or iolet

@@ -25,8 +25,19 @@ constexpr int BLOCK = 256;   // read-out / init kernels
 #ifndef HLB_STEP_BLOCK
 #define HLB_STEP_BLOCK 128   // Ns is a multiple of 128: the step kernels need no bounds test
 #endif
-#ifndef HLB_STEP_MINB
-#define HLB_STEP_MINB 6      // resident blocks per SM the register budget is tuned for
+// Resident blocks per SM each step kernel's register budget is tuned for (measured on
+// B200, profiles/r01_tuning.md): 7 x 128 threads at <= 72 registers for the pull kernel,
+// 6 x 128 at <= 80 for the two A-A kernels. Fewer registers spill the 15 populations,
+// more cut the loads in flight. The table-reading variants (REC = false) hold 14 more
+// live values and get one block less.
+#ifndef HLB_PULL_MINB
+#define HLB_PULL_MINB 7
+#endif
+#ifndef HLB_AA_EVEN_MINB
+#define HLB_AA_EVEN_MINB 6
+#endif
+#ifndef HLB_AA_ODD_MINB
+#define HLB_AA_ODD_MINB 6
 #endif
 constexpr int SBLOCK = HLB_STEP_BLOCK;
 
@@ -88,35 +99,20 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 // Rare path (sites on an inlet/outlet cap): for every iolet link p of site i replace
 // out[p] -- the value that will be read back as f_p(x, t+1) -- by the constant-density
 // equilibrium f_eq_p(rho_k, u(x, t)) (reading A6). The table entries are re-read here so
-// that the common path does not keep them in registers.
-__device__ __noinline__ void iolet_substitute_slow(const int32_t* __restrict__ nbr, long long Ns,
-                                                   long long i, double ux, double uy, double uz,
-                                                   const double* __restrict__ iolet_rho,
-                                                   double* __restrict__ out) {
-#pragma unroll 1
-  for (int p = 1; p < Q; ++p) {
-    const int k = iolet_of(__ldg(nbr + (long long)(p - 1) * Ns + i));
-    if (k >= 0) {
-      const double rk = __ldg(iolet_rho + k);
-      const double cu = (double)cx_rt(p) * ux + (double)cy_rt(p) * uy + (double)cz_rt(p) * uz;
-      const double uu = ux * ux + uy * uy + uz * uz;
-      out[p] = weight_rt(p) * ((rk - 1.0) + rk * (3.0 * cu + 4.5 * cu * cu - 1.5 * uu));
-    }
-  }
-}
-
-// out[] stays in registers on the common path: only the rare path copies it through the
-// stack for the out-of-line call.
+// that the common path does not keep them in registers; fully unrolled so that out[] stays
+// in registers (no call, no stack).
 __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
                                                  long long i, const Moments& m,
                                                  const double* __restrict__ iolet_rho,
                                                  double (&out)[Q]) {
-  double tmp[Q];
 #pragma unroll
-  for (int p = 1; p < Q; ++p) tmp[p] = out[p];
-  iolet_substitute_slow(nbr, Ns, i, m.ux, m.uy, m.uz, iolet_rho, tmp);
-#pragma unroll
-  for (int p = 1; p < Q; ++p) out[p] = tmp[p];
+  for (int p = 1; p < Q; ++p) {
+    const int k = iolet_of(__ldg(nbr + (long long)(p - 1) * Ns + i));
+    if (k >= 0) {
+      const double rk = __ldg(iolet_rho + k);
+      out[p] = heq_of(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+    }
+  }
 }
 
 __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iolet_bits, long long i) {
@@ -127,7 +123,7 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
 // src holds post-collision values h*(., t-1) (iolet slots substituted); one launch does
 // gather -> moments -> BGK -> store of h*(., t) into dst (rows S1..S6 fused).
 template <typename ST, bool REC>
-__global__ void __launch_bounds__(SBLOCK, HLB_STEP_MINB)
+__global__ void __launch_bounds__(SBLOCK, REC ? HLB_PULL_MINB : HLB_PULL_MINB - 1)
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
        const double* __restrict__ iolet_rho, long long Ns, double omega) {
@@ -161,7 +157,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // the address f_opp(q) was read from. Read set = write set per site in both phases, so one
 // array and no inter-thread hazards.
 template <typename ST>
-__global__ void __launch_bounds__(SBLOCK, HLB_STEP_MINB)
+__global__ void __launch_bounds__(SBLOCK, HLB_AA_EVEN_MINB)
 k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
           const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
           long long Ns, double omega) {
@@ -180,7 +176,7 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
 }
 
 template <typename ST, bool REC>
-__global__ void __launch_bounds__(SBLOCK, HLB_STEP_MINB)
+__global__ void __launch_bounds__(SBLOCK, REC ? HLB_AA_ODD_MINB : HLB_AA_ODD_MINB - 1)
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
          long long Ns, double omega) {

@@ -181,6 +181,31 @@ def test_populations_match_oracle(hlb, scheme):
     g.close()
 
 
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_graph_replay_equals_direct_launches(hlb, scheme):
+    """hlb_step replays captured graphs of 32 steps; same kernels, so bitwise the same as
+    HLB_NO_GRAPH, whatever the split of the steps into calls (odd starts included)."""
+    wl = W.by_name("aneurysm", small=True)
+    f = flags_of(hlb, scheme, "f64", "raster")
+    a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f)
+    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | hlb.HLB_NO_GRAPH)
+    for n in (1, 70, 33, 32, 100):
+        a.hlb_step(n)
+        b.hlb_step(n)
+        assert a.hlb_steps_done() == b.hlb_steps_done()
+        assert a.hlb_launch_count() == b.hlb_launch_count() == a.hlb_steps_done()
+        ra, ua = a.hlb_get_macroscopic()
+        rb, ub = b.hlb_get_macroscopic()
+        assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
+    a.hlb_set_state(None, None)                      # reset, then straight into a graph
+    b.hlb_set_state(None, None)
+    a.hlb_step(64)
+    b.hlb_step(64)
+    assert np.array_equal(a.hlb_get_macroscopic()[1], b.hlb_get_macroscopic()[1])
+    a.close()
+    b.close()
+
+
 # ------------------------------------------------------------- invariants on the GPU itself
 @pytest.mark.parametrize("store", ["f64", "f32"])
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])

@@ -53,7 +53,8 @@ def test_library_velocity_set_is_d3q15():
         assert WT[q] == {0: 2 / 9, 1: 1 / 9, 3: 1 / 72}[int(C[q] @ C[q])]
 
 
-@pytest.mark.parametrize("order", [hlb.HLB_ORDER_MORTON, hlb.HLB_ORDER_RASTER, hlb.HLB_ORDER_TILED])
+@pytest.mark.parametrize("order", [hlb.HLB_ORDER_AUTO, hlb.HLB_ORDER_MORTON, hlb.HLB_ORDER_RASTER,
+                                   hlb.HLB_ORDER_TILED])
 @pytest.mark.parametrize("seed,periodic,shape", [
     (0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (20, 5, 4)), (3, 2, (4, 19, 5)),
     (4, 4, (5, 4, 17)), (5, 7, (1, 1, 3)), (6, 3, (2, 2, 2)), (7, 0, (16, 16, 16)),
@@ -71,7 +72,7 @@ def test_table_matches_brute_force(order, seed, periodic, shape):
     assert np.array_equal(canon[t["canon_of_site"]], vox)            # canonical rank is right
     nz, ny, nx = st.shape
     x, y, z = vox % nx, (vox // nx) % ny, vox // (nx * ny)
-    if order == hlb.HLB_ORDER_RASTER:
+    if order in (hlb.HLB_ORDER_RASTER, hlb.HLB_ORDER_AUTO):
         assert np.array_equal(vox, canon)
     elif order == hlb.HLB_ORDER_MORTON:
         keys = [morton_key(int(a), int(b), int(c)) for a, b, c in zip(x, y, z)]
@@ -113,7 +114,7 @@ def test_argument_errors():
     assert e.value.code == hlb.HLB_EINVAL
     st[0, 0, 0] = 0
     with pytest.raises(hlb.HlbError) as e:
-        hlb.hlb_preprocess(st, 0, 0, 0xC)                              # unknown order
+        hlb.hlb_preprocess(st, 0, 0, 0x1000)                           # unknown flag bit
     assert e.value.code == hlb.HLB_EINVAL
     t = hlb.hlb_preprocess(st, 0, 0, 0)                                # isolated site: all walls
     assert t["N"] == 1 and np.all(t["nbr"] == WALL)
