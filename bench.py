@@ -65,6 +65,7 @@ def parse_args():
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--order", default="auto", choices=["auto", "morton", "raster", "tiled"])
     ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
+    ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="scaled-down geometry (debugging only)")
@@ -285,7 +286,8 @@ def main():
             {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
              "tiled": hlb.HLB_ORDER_TILED}[args.order] | \
             {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
-             "records": hlb.HLB_LINKS_RECORDS}[args.links]
+             "records": hlb.HLB_LINKS_RECORDS}[args.links] | \
+            (hlb.HLB_NO_PREFETCH if args.no_prefetch else 0)
     t_create = time.perf_counter()
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
     torch.cuda.synchronize()
@@ -394,6 +396,7 @@ def main():
             "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
             "n_sites": N, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
             "order": args.order, "links": "records" if g.hlb_uses_records() else "table",
+            "l2_prefetch": not args.no_prefetch,
             "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
             "box": list(wl.shape), "seed": wl.info.get("seed"),
             "device_bytes": g.hlb_device_bytes(),

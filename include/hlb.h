@@ -67,7 +67,8 @@ enum {
   HLB_LINKS_AUTO = 0x0,    /* the step kernels read the run-length link records when at
                               least half of them are not sentinels, else the table         */
   HLB_LINKS_TABLE = 0x20,  /* always read the int32 table (ablation / profiling)           */
-  HLB_LINKS_RECORDS = 0x40 /* always read the records                                     */
+  HLB_LINKS_RECORDS = 0x40,/* always read the records                                     */
+  HLB_NO_PREFETCH = 0x80   /* step kernels issue no L2 prefetches (ablation / profiling)   */
 };
 
 typedef struct hlb_geometry hlb_geometry; /* opaque handle */

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -110,7 +111,7 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->n_iolets > 0 && !p->iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
   if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
-                             HLB_LINKS_TABLE | HLB_LINKS_RECORDS))
+                             HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH))
     return fail(HLB_EINVAL, "unknown flag bits");
   if ((p->flags & HLB_LINKS_TABLE) && (p->flags & HLB_LINKS_RECORDS))
     return fail(HLB_EINVAL, "HLB_LINKS_TABLE and HLB_LINKS_RECORDS are exclusive");
@@ -223,6 +224,17 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.iolet_bits = (const uint32_t*)d_bits;
   g->dg.rec = d_rec;
   g->dg.use_rec = use_rec;
+  if (!(p->flags & HLB_NO_PREFETCH)) {
+    // L2 prefetch distance: 3/4 of the sites resident on the chip (measured optimum on
+    // B200: 0.6 .. 0.9, profiles/r01_tuning.md). HLB_PREFETCH_SITES overrides it (tuning).
+    int dev = 0, sms = 0;
+    HLB_CUDA_G(cudaGetDevice(&dev));
+    HLB_CUDA_G(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull() * 3 / 4 / 128 * 128;
+    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa() * 3 / 4 / 128 * 128;
+    if (const char* e = std::getenv("HLB_PREFETCH_SITES"))
+      g->dg.prefetch_pull = g->dg.prefetch_aa = std::atoll(e);
+  }
   g->dg.canon = (const int32_t*)d_canon;
   g->dg.iolet_rho = (const double*)d_rho;
   g->dg.omega = 1.0 / p->tau;

@@ -115,6 +115,12 @@ __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr
   }
 }
 
+// L2 prefetch of data that a block scheduled roughly one wave later will load: brings the
+// DRAM fetch forward without holding registers or a scoreboard slot.
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
 __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iolet_bits, long long i) {
   return (__ldg(iolet_bits + (i >> 5)) >> (threadIdx.x & 31)) & 1u;
 }
@@ -126,7 +132,7 @@ template <typename ST, bool REC>
 __global__ void __launch_bounds__(SBLOCK, REC ? HLB_PULL_MINB : HLB_PULL_MINB - 1)
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
-       const double* __restrict__ iolet_rho, long long Ns, double omega) {
+       const double* __restrict__ iolet_rho, long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[Q];
   {
@@ -135,6 +141,16 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
     h[0] = to_real(src[i]);
 #pragma unroll
     for (int q = 1; q < Q; ++q) h[q] = to_real(src[slot_of<GATHER_PULL>(q, e[q - 1], Ns, i)]);
+    if (pf > 0 && i + pf < Ns) {
+      // the links of site i + pf are, to first order, those of site i shifted by pf
+      if (REC) { if ((threadIdx.x & 31) < 7) prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31)); }
+      prefetch_l2(src + i + pf);
+#pragma unroll
+      for (int q = 1; q < Q; ++q) {
+        const long long o = slot_of<GATHER_PULL>(q, e[q - 1], Ns, i) + pf;
+        prefetch_l2(src + (o < (long long)Q * Ns ? o : i));
+      }
+    }
   }
   const Moments m = moments_of(h);
   collide(h, m, omega, h);
@@ -160,11 +176,15 @@ template <typename ST>
 __global__ void __launch_bounds__(SBLOCK, HLB_AA_EVEN_MINB)
 k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
           const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
-          long long Ns, double omega) {
+          long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[Q];
 #pragma unroll
   for (int q = 0; q < Q; ++q) h[q] = to_real(a[(long long)q * Ns + i]);
+  if (pf > 0 && i + pf < Ns) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) prefetch_l2(a + (long long)q * Ns + i + pf);
+  }
   const Moments m = moments_of(h);
   collide(h, m, omega, h);
   double out[Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
@@ -179,7 +199,7 @@ template <typename ST, bool REC>
 __global__ void __launch_bounds__(SBLOCK, REC ? HLB_AA_ODD_MINB : HLB_AA_ODD_MINB - 1)
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
-         long long Ns, double omega) {
+         long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   int32_t e[Q - 1];
   load_links<REC>(nbr, rec, Ns, i, e);
@@ -187,6 +207,15 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   h[0] = to_real(a[i]);
 #pragma unroll
   for (int q = 1; q < Q; ++q) h[q] = to_real(a[slot_of<GATHER_AA_ODD>(q, e[q - 1], Ns, i)]);
+  if (pf > 0 && i + pf < Ns) {
+    if (REC) { if ((threadIdx.x & 31) < 7) prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31)); }
+    prefetch_l2(a + i + pf);
+#pragma unroll
+    for (int q = 1; q < Q; ++q) {
+      const long long o = slot_of<GATHER_AA_ODD>(q, e[q - 1], Ns, i) + pf;
+      prefetch_l2(a + (o < (long long)Q * Ns ? o : i));
+    }
+  }
   const Moments m = moments_of(h);
   collide(h, m, omega, h);
   double out[Q];
@@ -292,15 +321,18 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + BLOCK - 1) / BLOC
 
 }  // namespace
 
+int resident_sites_per_sm_pull() { return SBLOCK * HLB_PULL_MINB; }
+int resident_sites_per_sm_aa() { return SBLOCK * HLB_AA_ODD_MINB; }
+
 template <typename ST>
 static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   const unsigned grid = (unsigned)(g.Ns / SBLOCK);
   if (g.use_rec)
     k_pull<ST, true><<<grid, SBLOCK, 0, s>>>((const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec,
-                                             g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
+                                             g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_pull);
   else
     k_pull<ST, false><<<grid, SBLOCK, 0, s>>>((const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec,
-                                              g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
+                                              g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_pull);
 }
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   if (g.f32) pull_t<float>(g, src, dst, s);
@@ -311,13 +343,13 @@ template <typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const unsigned grid = (unsigned)(g.Ns / SBLOCK);
   if (!odd)
-    k_aa_even<ST><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega);
+    k_aa_even<ST><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_pull);
   else if (g.use_rec)
     k_aa_odd<ST, true><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-                                               g.iolet_rho, g.Ns, g.omega);
+                                               g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
   else
     k_aa_odd<ST, false><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-                                                g.iolet_rho, g.Ns, g.omega);
+                                                g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
 }
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   if (g.f32) aa_t<float>(g, a, odd, s);

@@ -13,11 +13,18 @@ struct DeviceGeometry {
   const uint32_t* iolet_bits = nullptr; // [Ns/32]
   const void* rec = nullptr;            // [Ns/32][14] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
+  // > 0: every thread L2-prefetches what site i + prefetch_* will load (about 3/4 of the
+  // sites resident on the chip at once, i.e. the blocks scheduled just under a wave later)
+  int64_t prefetch_pull = 0, prefetch_aa = 0;
   const int32_t* canon = nullptr;       // [N] internal -> canonical rank
   const double* iolet_rho = nullptr;    // [n_iolets]
   double omega = 1.0;                   // 1 / tau
   bool f32 = false;                     // HLB_STORE_F32
 };
+
+// Sites resident on an SM at once (threads per block x resident blocks) per step kernel.
+int resident_sites_per_sm_pull();
+int resident_sites_per_sm_aa();
 
 // One time step, two-lattice pull: dst <- collide(gather(src)).
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);

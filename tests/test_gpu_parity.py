@@ -206,6 +206,24 @@ def test_graph_replay_equals_direct_launches(hlb, scheme):
     b.close()
 
 
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_l2_prefetch_changes_nothing(hlb, scheme, monkeypatch):
+    """The L2 prefetches are hints: bitwise the same results with a distance that really
+    fires on a small geometry (HLB_PREFETCH_SITES) and with HLB_NO_PREFETCH."""
+    wl = W.by_name("tree", small=True)
+    f = flags_of(hlb, scheme, "f64", "raster", "records")
+    monkeypatch.setenv("HLB_PREFETCH_SITES", "1024")
+    a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f)
+    monkeypatch.delenv("HLB_PREFETCH_SITES")
+    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | hlb.HLB_NO_PREFETCH)
+    a.hlb_step(37)
+    b.hlb_step(37)
+    (ra, ua), (rb, ub) = a.hlb_get_macroscopic(), b.hlb_get_macroscopic()
+    assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
+    a.close()
+    b.close()
+
+
 # ------------------------------------------------------------- invariants on the GPU itself
 @pytest.mark.parametrize("store", ["f64", "f32"])
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
