@@ -170,14 +170,15 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
 
 /* Run-length link records of a table (host only): the compressed form of nbr that the step
  * kernels read. A group is 32 consecutive internal sites (one warp). For group g and link q
- * the record rec[(g*14 + (q-1))*4 .. +4] = { wall, start, base0, base1 }:
- *   wall   bit l set: the entry of lane l is negative (solid or iolet: bounce-back target)
- *   start  bit l set: lane l is not a wall lane and begins a run, i.e. lane l-1 is a wall
- *          lane or nbr[lane l] != nbr[lane l-1] + 1
- *   base0, base1: the table entries of the first lanes of run 0 and run 1
- * so that the entry of a non-wall lane l in run r, which started at lane s, is
- * base_r + (l - s). A (g, q) with more than two runs gets the sentinel {0, 0, 0, 0} (a real
- * record never has wall == 0 and start == 0) and the kernels read nbr for it instead.
+ * the record rec[(g*14 + (q-1))*4 .. +4] = { wall, second, off0, off1 }:
+ *   wall    bit l set: the entry of lane l is negative (solid or iolet: bounce-back target)
+ *   second  the non-wall lanes split into runs of lanes with consecutive entries (a wall
+ *           lane or a jump in the entries ends a run); second = the lane at which run 1
+ *           starts, 32 if there is only one run (or none)
+ *   off0, off1: (entry of the run's first lane) - (that lane), as int32, for run 0 and 1
+ * so that the entry of a non-wall lane l is (l >= second ? off1 : off0) + l. A (g, q) with
+ * more than two runs gets the sentinel { 0, 0xffffffff, 0, 0 } and the kernels read nbr for
+ * it instead.
  *   nbr: HOST [14][stride] as filled by hlb_preprocess_tables; stride a multiple of 32
  *   rec: HOST [stride/32][14][4] uint32, filled
  *   n_sentinel: number of (g, q) that got the sentinel (may be NULL) */

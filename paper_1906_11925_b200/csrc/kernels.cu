@@ -52,36 +52,52 @@ __device__ __forceinline__ void load_entries(const int32_t* __restrict__ nbr, lo
   for (int q = 1; q < Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
 }
 
-// Link entries of site i for the step kernels: >= 0 source site, < 0 bounce-back target
-// (the iolet id is NOT decoded here; the rare iolet path reloads the table). With REC the
-// warp reads one 16-byte record per link instead of 32 table entries (include/hlb.h,
-// hlb_preprocess_records); a sentinel record sends the whole warp to the table.
-template <bool REC>
-__device__ __forceinline__ void load_links(const int32_t* __restrict__ nbr,
-                                           const uint4* __restrict__ rec, long long Ns,
-                                           long long i, int32_t (&e)[Q - 1]) {
+// Flat element offsets (slot * Ns + site) of the 14 link populations of site i, for the step
+// kernels. IT is the offset type: uint32_t when 15 * Ns < 2^32 (one IMAD.WIDE per access
+// instead of 64-bit index arithmetic -- the integer work matters: these kernels run at the
+// chip's power cap), long long otherwise.
+//   MODE GATHER_PULL  : fluid source e -> q * Ns + e       ; wall -> opp(q) * Ns + i
+//   MODE GATHER_AA_ODD: fluid source e -> opp(q) * Ns + e  ; wall -> q * Ns + i
+// With REC the warp reads one 16-byte record per link instead of 32 table entries
+// (include/hlb.h, hlb_preprocess_records): entry = (lane >= second ? off1 : off0) + lane;
+// a sentinel record (warp-uniform) sends the warp to the table for that link. The iolet id
+// is NOT decoded here; the rare iolet path re-reads the table.
+template <int MODE, bool REC, typename IT>
+__device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
+                                             const uint4* __restrict__ rec, long long Ns,
+                                             long long i, IT (&off)[Q - 1]) {
+  const IT n = (IT)Ns, self = (IT)i;
   if (!REC) {
+    int32_t e[Q - 1];
 #pragma unroll
     for (int q = 1; q < Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+#pragma unroll
+    for (int q = 1; q < Q; ++q) {
+      const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
+      off[q - 1] = e[q - 1] < 0 ? (IT)qw * n + self : (IT)qf * n + (IT)e[q - 1];
+    }
     return;
   }
-  const int lane = threadIdx.x & 31;
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t lane_bit = 1u << lane;
   const uint4* r = rec + (i >> 5) * (Q - 1);
   uint4 v[Q - 1];
 #pragma unroll
   for (int q = 1; q < Q; ++q) v[q - 1] = __ldg(r + (q - 1));
-  const uint32_t le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
 #pragma unroll
   for (int q = 1; q < Q; ++q) {
+    const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
     const uint4 t = v[q - 1];
-    if ((t.x | t.y) == 0u) {  // sentinel (warp-uniform): more than two runs
-      e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+    int32_t e;
+    bool wall;
+    if (t.y == 0xffffffffu) {  // sentinel: more than two runs
+      e = __ldg(nbr + (long long)(q - 1) * Ns + i);
+      wall = e < 0;
     } else {
-      const uint32_t le = t.y & le_mask;           // run starts at or below this lane
-      const int s = 31 - __clz((int)le);           // lane the run started at
-      const int base = (le & (le - 1)) ? (int)t.w : (int)t.z;  // second run iff two starts
-      e[q - 1] = ((t.x >> lane) & 1u) ? (int32_t)0x80000000 : base + (lane - s);
+      e = (int32_t)(lane >= t.y ? t.w : t.z) + (int32_t)lane;
+      wall = (t.x & lane_bit) != 0u;
     }
+    off[q - 1] = wall ? (IT)qw * n + self : (IT)qf * n + (IT)e;
   }
 }
 
@@ -128,7 +144,10 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
 // ------------------------------------------------------------------ two-lattice pull
 // src holds post-collision values h*(., t-1) (iolet slots substituted); one launch does
 // gather -> moments -> BGK -> store of h*(., t) into dst (rows S1..S6 fused).
-template <typename ST, bool REC>
+// pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
+// of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
+// padding, so only the one warp-uniform test is needed.
+template <typename ST, bool REC, typename IT>
 __global__ void __launch_bounds__(SBLOCK, REC ? HLB_PULL_MINB : HLB_PULL_MINB - 1)
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
@@ -136,20 +155,18 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[Q];
   {
-    int32_t e[Q - 1];
-    load_links<REC>(nbr, rec, Ns, i, e);
+    IT off[Q - 1];
+    link_offsets<GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
     h[0] = to_real(src[i]);
 #pragma unroll
-    for (int q = 1; q < Q; ++q) h[q] = to_real(src[slot_of<GATHER_PULL>(q, e[q - 1], Ns, i)]);
+    for (int q = 1; q < Q; ++q) h[q] = to_real(src[off[q - 1]]);
     if (pf > 0 && i + pf < Ns) {
-      // the links of site i + pf are, to first order, those of site i shifted by pf
-      if (REC) { if ((threadIdx.x & 31) < 7) prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31)); }
-      prefetch_l2(src + i + pf);
+      const ST* ahead = src + pf;
+      if (REC && (threadIdx.x & 31) < 7)
+        prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31));
+      prefetch_l2(ahead + i);
 #pragma unroll
-      for (int q = 1; q < Q; ++q) {
-        const long long o = slot_of<GATHER_PULL>(q, e[q - 1], Ns, i) + pf;
-        prefetch_l2(src + (o < (long long)Q * Ns ? o : i));
-      }
+      for (int q = 1; q < Q; ++q) prefetch_l2(ahead + off[q - 1]);
     }
   }
   const Moments m = moments_of(h);
@@ -163,8 +180,9 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 #pragma unroll
     for (int p = 1; p < Q; ++p) h[opp(p)] = back[p];
   }
+  ST* d = dst + i;
 #pragma unroll
-  for (int q = 0; q < Q; ++q) dst[(long long)q * Ns + i] = to_store<ST>(h[q]);
+  for (int q = 0; q < Q; ++q) d[(long long)q * Ns] = to_store<ST>(h[q]);
 }
 
 // ------------------------------------------------------------------ A-A in place
@@ -178,12 +196,13 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
           const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
           long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
+  ST* p0 = a + i;
   double h[Q];
 #pragma unroll
-  for (int q = 0; q < Q; ++q) h[q] = to_real(a[(long long)q * Ns + i]);
+  for (int q = 0; q < Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
   if (pf > 0 && i + pf < Ns) {
 #pragma unroll
-    for (int q = 0; q < Q; ++q) prefetch_l2(a + (long long)q * Ns + i + pf);
+    for (int q = 0; q < Q; ++q) prefetch_l2(p0 + (long long)q * Ns + pf);
   }
   const Moments m = moments_of(h);
   collide(h, m, omega, h);
@@ -192,29 +211,28 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
   for (int p = 0; p < Q; ++p) out[p] = h[opp(p)];
   if (has_iolet_link(iolet_bits, i)) iolet_substitute(nbr, Ns, i, m, iolet_rho, out);
 #pragma unroll
-  for (int p = 0; p < Q; ++p) a[(long long)p * Ns + i] = to_store<ST>(out[p]);
+  for (int p = 0; p < Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
 
-template <typename ST, bool REC>
+template <typename ST, bool REC, typename IT>
 __global__ void __launch_bounds__(SBLOCK, REC ? HLB_AA_ODD_MINB : HLB_AA_ODD_MINB - 1)
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
          long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
-  int32_t e[Q - 1];
-  load_links<REC>(nbr, rec, Ns, i, e);
+  IT off[Q - 1];
+  link_offsets<GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
   double h[Q];
   h[0] = to_real(a[i]);
 #pragma unroll
-  for (int q = 1; q < Q; ++q) h[q] = to_real(a[slot_of<GATHER_AA_ODD>(q, e[q - 1], Ns, i)]);
+  for (int q = 1; q < Q; ++q) h[q] = to_real(a[off[q - 1]]);
   if (pf > 0 && i + pf < Ns) {
-    if (REC) { if ((threadIdx.x & 31) < 7) prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31)); }
-    prefetch_l2(a + i + pf);
+    const ST* ahead = a + pf;
+    if (REC && (threadIdx.x & 31) < 7)
+      prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31));
+    prefetch_l2(ahead + i);
 #pragma unroll
-    for (int q = 1; q < Q; ++q) {
-      const long long o = slot_of<GATHER_AA_ODD>(q, e[q - 1], Ns, i) + pf;
-      prefetch_l2(a + (o < (long long)Q * Ns ? o : i));
-    }
+    for (int q = 1; q < Q; ++q) prefetch_l2(ahead + off[q - 1]);
   }
   const Moments m = moments_of(h);
   collide(h, m, omega, h);
@@ -224,7 +242,7 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   if (has_iolet_link(iolet_bits, i)) iolet_substitute(nbr, Ns, i, m, iolet_rho, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
-  for (int p = 1; p < Q; ++p) a[slot_of<GATHER_AA_ODD>(p, e[p - 1], Ns, i)] = to_store<ST>(out[p]);
+  for (int p = 1; p < Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
 }
 
 // ------------------------------------------------------------------ read-out / init
@@ -324,32 +342,46 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + BLOCK - 1) / BLOC
 int resident_sites_per_sm_pull() { return SBLOCK * HLB_PULL_MINB; }
 int resident_sites_per_sm_aa() { return SBLOCK * HLB_AA_ODD_MINB; }
 
+template <typename ST, bool REC, typename IT>
+static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+  k_pull<ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
+      (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_rho, g.Ns,
+      g.omega, g.prefetch_pull);
+}
 template <typename ST>
 static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  const unsigned grid = (unsigned)(g.Ns / SBLOCK);
-  if (g.use_rec)
-    k_pull<ST, true><<<grid, SBLOCK, 0, s>>>((const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec,
-                                             g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_pull);
-  else
-    k_pull<ST, false><<<grid, SBLOCK, 0, s>>>((const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec,
-                                              g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_pull);
+  const bool idx32 = (long long)Q * g.Ns < (1ll << 32);
+  if (g.use_rec) {
+    if (idx32) pull_launch<ST, true, uint32_t>(g, src, dst, s);
+    else pull_launch<ST, true, long long>(g, src, dst, s);
+  } else {
+    if (idx32) pull_launch<ST, false, uint32_t>(g, src, dst, s);
+    else pull_launch<ST, false, long long>(g, src, dst, s);
+  }
 }
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   if (g.f32) pull_t<float>(g, src, dst, s);
   else pull_t<double>(g, src, dst, s);
 }
 
+template <typename ST, bool REC, typename IT>
+static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
+  k_aa_odd<ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
+      (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
+}
 template <typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
-  const unsigned grid = (unsigned)(g.Ns / SBLOCK);
-  if (!odd)
-    k_aa_even<ST><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_pull);
-  else if (g.use_rec)
-    k_aa_odd<ST, true><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-                                               g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
-  else
-    k_aa_odd<ST, false><<<grid, SBLOCK, 0, s>>>((ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-                                                g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
+  const bool idx32 = (long long)Q * g.Ns < (1ll << 32);
+  if (!odd) {
+    k_aa_even<ST><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits,
+                                                               g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
+  } else if (g.use_rec) {
+    if (idx32) aa_odd_launch<ST, true, uint32_t>(g, a, s);
+    else aa_odd_launch<ST, true, long long>(g, a, s);
+  } else {
+    if (idx32) aa_odd_launch<ST, false, uint32_t>(g, a, s);
+    else aa_odd_launch<ST, false, long long>(g, a, s);
+  }
 }
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   if (g.f32) aa_t<float>(g, a, odd, s);

@@ -17,44 +17,87 @@ struct Moments {
   double drho, rho, ux, uy, uz;
 };
 
+// Every floating-point operation below is an explicit round-to-nearest intrinsic
+// (__dadd_rn / __dmul_rn / __fma_rn): the compiler may neither contract nor split them, so
+// all kernel instantiations (two-lattice, A-A even / odd, table or records, fp64 or fp32
+// storage) evaluate bit-identical arithmetic whatever their register allocation or inlining
+// context (SURVEY.md §8(c) pin P14).
+__device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double sub(double a, double b) { return __dadd_rn(a, -b); }
+__device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+
+// c_q . u with the +-1 / 0 components folded at compile time (exact: only additions)
+__device__ __forceinline__ double c_dot_u(int q, double ux, double uy, double uz) {
+  double r = 0.0;
+  bool first = true;
+  const int c[3] = {cx(q), cy(q), cz(q)};
+  const double u[3] = {ux, uy, uz};
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (c[a] == 0) continue;
+    const double t = c[a] > 0 ? u[a] : -u[a];
+    r = first ? t : add(r, t);
+    first = false;
+  }
+  return r;
+}
+
 // Opposite pairs (2k-1, 2k), k = 1..7, first member has c = (1,0,0) (0,1,0) (0,0,1)
 // (1,1,1) (1,1,-1) (1,-1,1) (1,-1,-1): sums and differences of pairs give all moments.
 __device__ __forceinline__ Moments moments_of(const double (&h)[Q]) {
-  const double d1 = h[1] - h[2], d2 = h[3] - h[4], d3 = h[5] - h[6];
-  const double d4 = h[7] - h[8], d5 = h[9] - h[10], d6 = h[11] - h[12], d7 = h[13] - h[14];
-  const double s_axis = ((h[1] + h[2]) + (h[3] + h[4])) + (h[5] + h[6]);
-  const double s_diag = ((h[7] + h[8]) + (h[9] + h[10])) + ((h[11] + h[12]) + (h[13] + h[14]));
+  const double d1 = sub(h[1], h[2]), d2 = sub(h[3], h[4]), d3 = sub(h[5], h[6]);
+  const double d4 = sub(h[7], h[8]), d5 = sub(h[9], h[10]), d6 = sub(h[11], h[12]),
+               d7 = sub(h[13], h[14]);
+  const double s_axis = add(add(add(h[1], h[2]), add(h[3], h[4])), add(h[5], h[6]));
+  const double s_diag = add(add(add(h[7], h[8]), add(h[9], h[10])),
+                            add(add(h[11], h[12]), add(h[13], h[14])));
   Moments m;
-  m.drho = h[0] + (s_axis + s_diag);
-  m.rho = 1.0 + m.drho;
-  const double jx = d1 + ((d4 + d5) + (d6 + d7));
-  const double jy = d2 + ((d4 + d5) - (d6 + d7));
-  const double jz = d3 + ((d4 - d5) + (d6 - d7));
-  const double inv = 1.0 / m.rho;
-  m.ux = jx * inv;
-  m.uy = jy * inv;
-  m.uz = jz * inv;
+  m.drho = add(h[0], add(s_axis, s_diag));
+  m.rho = add(1.0, m.drho);
+  const double jx = add(d1, add(add(d4, d5), add(d6, d7)));
+  const double jy = add(d2, sub(add(d4, d5), add(d6, d7)));
+  const double jz = add(d3, add(sub(d4, d5), sub(d6, d7)));
+  const double inv = __drcp_rn(m.rho);
+  m.ux = mul(jx, inv);
+  m.uy = mul(jy, inv);
+  m.uz = mul(jz, inv);
   return m;
 }
 
-// Shifted equilibrium of direction q (compile-time q after unrolling) for density
-// 1 + drho and velocity (ux, uy, uz).
-__device__ __forceinline__ double heq_of(int q, double drho, double rho, double ux, double uy,
-                                         double uz) {
-  const double cu = (double)cx(q) * ux + (double)cy(q) * uy + (double)cz(q) * uz;
-  const double uu = ux * ux + uy * uy + uz * uz;
-  return weight(q) * (drho + rho * (3.0 * cu + 4.5 * cu * cu - 1.5 * uu));
+__device__ __forceinline__ double u_dot_u(double ux, double uy, double uz) {
+  return fma_(ux, ux, fma_(uy, uy, mul(uz, uz)));
 }
 
-// hs_q = h_q + omega (heq_q(m) - h_q)
+// Shifted equilibrium of direction q (compile-time q after unrolling) for density
+// 1 + drho and velocity (ux, uy, uz): w_q [drho + rho (3 c.u + 4.5 (c.u)^2 - 1.5 u.u)].
+__device__ __forceinline__ double heq_of(int q, double drho, double rho, double ux, double uy,
+                                         double uz) {
+  const double cu = c_dot_u(q, ux, uy, uz);
+  const double uu15 = mul(1.5, u_dot_u(ux, uy, uz));
+  const double poly = add(mul(3.0, cu), fma_(mul(4.5, cu), cu, -uu15));
+  return mul(weight(q), fma_(rho, poly, drho));
+}
+
+// hs_q = h_q + omega (heq_q(m) - h_q), evaluated per opposite pair (a, b = opp(a)), c = c_a:
+//   heq_a = S + A, heq_b = S - A,  S = w (drho + rho (4.5 (c.u)^2 - 1.5 u.u)),  A = 3 w rho (c.u)
+// -- the same equilibrium as heq_of(), with the part even in c computed once per pair (a
+// third fewer fp64 operations; the kernels run into the 1 kW power cap otherwise).
 __device__ __forceinline__ void collide(const double (&h)[Q], const Moments& m, double omega,
                                         double (&hs)[Q]) {
-  const double uu15 = 1.5 * (m.ux * m.ux + m.uy * m.uy + m.uz * m.uz);
+  const double uu15 = mul(1.5, u_dot_u(m.ux, m.uy, m.uz));
+  const double heq0 = mul(weight(0), fma_(-m.rho, uu15, m.drho));
+  hs[0] = fma_(omega, sub(heq0, h[0]), h[0]);
+  const double r3_axis = mul(3.0 * weight(1), m.rho), r3_diag = mul(3.0 * weight(7), m.rho);
 #pragma unroll
-  for (int q = 0; q < Q; ++q) {
-    const double cu = (double)cx(q) * m.ux + (double)cy(q) * m.uy + (double)cz(q) * m.uz;
-    const double heq = weight(q) * (m.drho + m.rho * ((3.0 * cu + 4.5 * cu * cu) - uu15));
-    hs[q] = h[q] + omega * (heq - h[q]);
+  for (int a = 1; a < Q; a += 2) {
+    const int b = a + 1;  // opp(a)
+    const double cu = c_dot_u(a, m.ux, m.uy, m.uz);
+    const double S = mul(weight(a), fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
+    const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
+    const double ha = h[a], hb = h[b];
+    hs[a] = fma_(omega, sub(add(S, A), ha), ha);
+    hs[b] = fma_(omega, sub(sub(S, A), hb), hb);
   }
 }
 

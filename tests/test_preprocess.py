@@ -129,19 +129,17 @@ def decode_records(rec, nbr):
     sentinel = np.zeros((G, 14), dtype=bool)
     for g in range(G):
         for k in range(14):
-            wall, start, b0, b1 = (int(v) for v in rec[g, k])
-            if wall == 0 and start == 0:
+            wall, second, o0, o1 = (int(v) for v in rec[g, k])
+            if second == 0xFFFFFFFF:
+                assert wall == 0 and o0 == 0 and o1 == 0
                 sentinel[g, k] = True
                 continue
+            assert 1 <= second <= 32
             for l in range(32):
                 if (wall >> l) & 1:
                     continue
-                le = start & ((2 << l) - 1)
-                assert le != 0, "a non-wall lane must belong to a run"
-                s = le.bit_length() - 1
-                r = bin(le).count("1") - 1
-                assert r in (0, 1)
-                out[k, g * 32 + l] = np.int32(np.uint32(b1 if r else b0)) + (l - s)
+                off = o1 if l >= second else o0
+                out[k, g * 32 + l] = int(np.int32(np.uint32(off))) + l
     return out, sentinel
 
 
