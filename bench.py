@@ -200,6 +200,24 @@ def time_oracle(wl, budget_s, threads=1):
     return n * steps / dt / 1e6, n, steps, dt, what, o.threads
 
 
+def max_over_ranks(values, world, device):
+    """Element-wise maximum of a list of floats over all ranks (replicas: no data-path
+    collective, only this reduction of the timings)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def replicas_value(n_sites, lb_steps, world, seconds):
+    """Whole-job MSUPS of `world` replicas that each did n_sites x lb_steps site updates in
+    at most `seconds` (the max over ranks)."""
+    return world * n_sites * lb_steps / seconds / 1e6
+
+
 def host_cpu_model():
     try:
         for line in open("/proc/cpuinfo"):
@@ -376,12 +394,8 @@ def main():
         e2e = (t_e2e, e2e_steps)
 
     # ---------------- aggregate over ranks (max time; total work)
-    ms_all, e2e_all = ms, (e2e[0] if e2e else 0.0)
-    if world > 1:
-        t = torch.tensor([ms, e2e_all], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_all, e2e_all = float(t[0]), float(t[1])
-    value = world * N * S * args.steps / (ms_all * 1e-3) / 1e6
+    ms_all, e2e_all = max_over_ranks([ms, e2e[0] if e2e else 0.0], world, dev)
+    value = replicas_value(N, S * args.steps, world, ms_all * 1e-3)
 
     peak, peak_src = measured_peak()
     dom_ms = k_ms[dominant]
@@ -418,7 +432,7 @@ def main():
         "clocks": clocks,
     }
     if e2e:
-        out["e2e"] = {"value": world * N * S * e2e[1] / e2e_all / 1e6, "unit": UNIT,
+        out["e2e"] = {"value": replicas_value(N, S * e2e[1], world, e2e_all), "unit": UNIT,
                       "h2d_bytes_per_step": 32 * N, "d2h_bytes_per_step": 32 * N,
                       "steps": e2e[1], "ms_per_step": e2e_all / e2e[1] * 1e3,
                       "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}

@@ -123,7 +123,9 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u);
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);
 
 /* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][15], canonical site
- * order, q in the order of hlb_velocity_set(). For population-level parity checks. */
+ * order, q in the order of hlb_velocity_set(). For population-level parity checks. The
+ * first call of this or of hlb_set_populations allocates a [N][15] fp64 staging buffer
+ * through the allocator (HLB_ENOMEM if that fails). */
 int hlb_get_populations(hlb_geometry* g, double* f);
 
 /* Set pre-collision populations f_q(x, 0) directly (HOST [N][15], layout as above) and

@@ -57,7 +57,9 @@ struct hlb_geometry {
   DeviceGeometry dg;
   void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
   int cur = 0;                        // two-lattice: buffer the next step reads
-  double* scratch = nullptr;          // [N][15] doubles: staging for host<->device transfers
+  double* scratch = nullptr;          // [4 N] doubles: staging of rho [N], u [N][3] transfers
+  double* scratch_pop = nullptr;      // [N][15] doubles, allocated by the first
+                                      // hlb_get_populations / hlb_set_populations call
   int64_t steps = 0, launches = 0, device_bytes = 0;
   double sentinel_fraction = 0.0;     // of the (group, q) link records
   // hlb_step(n) replays a captured CUDA graph of GRAPH_STEPS steps while n allows: removes
@@ -194,6 +196,26 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   const bool use_rec = (p->flags & HLB_LINKS_RECORDS) ? true
                        : (p->flags & HLB_LINKS_TABLE) ? false
                                                       : g->sentinel_fraction <= 0.5;
+  if (!(p->flags & HLB_NO_PREFETCH)) {
+    // L2 prefetch distance: 3/4 of the sites resident on the chip (measured optimum on
+    // B200: 0.6 .. 0.9, profiles/r01_tuning.md). HLB_PREFETCH_SITES overrides it (tuning).
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+      cuda_fail(cudaGetLastError(), "cudaDeviceGetAttribute");
+      delete g;
+      return HLB_ECUDA;
+    }
+    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull() * 3 / 4 / 128 * 128;
+    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa() * 3 / 4 / 128 * 128;
+    if (const char* e = std::getenv("HLB_PREFETCH_SITES")) {
+      const long long v = std::atoll(e);
+      g->dg.prefetch_pull = g->dg.prefetch_aa = v > 0 ? (v < (1ll << 24) ? v : (1ll << 24)) : 0;
+    }
+  }
+  // tail padding: a prefetch reaches at most `distance` elements past the last plane
+  const size_t pad_bytes =
+      (size_t)std::max(g->dg.prefetch_pull, g->dg.prefetch_aa) * g->store_bytes();
   const size_t pop_bytes = (size_t)Q * (size_t)t.Ns * g->store_bytes();
   auto bail = [&](int code) { hlb_geometry_destroy(g); return code; };
   if ((rc = g->alloc(sizeof(int32_t) * t.nbr.size(), &d_nbr))) return bail(rc);
@@ -201,9 +223,9 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   if (use_rec && (rc = g->alloc(sizeof(uint32_t) * t.rec.size(), &d_rec))) return bail(rc);
   if ((rc = g->alloc(sizeof(int32_t) * (size_t)t.N, &d_canon))) return bail(rc);
   if ((rc = g->alloc(sizeof(double) * (size_t)(p->n_iolets > 0 ? p->n_iolets : 1), &d_rho))) return bail(rc);
-  if ((rc = g->alloc(pop_bytes, &g->buf[0]))) return bail(rc);
-  if (!g->aa && (rc = g->alloc(pop_bytes, &g->buf[1]))) return bail(rc);
-  if ((rc = g->alloc(sizeof(double) * (size_t)Q * (size_t)t.N, &d_scratch))) return bail(rc);
+  if ((rc = g->alloc(pop_bytes + pad_bytes, &g->buf[0]))) return bail(rc);
+  if (!g->aa && (rc = g->alloc(pop_bytes + pad_bytes, &g->buf[1]))) return bail(rc);
+  if ((rc = g->alloc(sizeof(double) * 4 * (size_t)t.N, &d_scratch))) return bail(rc);
   g->scratch = (double*)d_scratch;
 
 #define HLB_CUDA_G(call)                                                   \
@@ -224,17 +246,6 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.iolet_bits = (const uint32_t*)d_bits;
   g->dg.rec = d_rec;
   g->dg.use_rec = use_rec;
-  if (!(p->flags & HLB_NO_PREFETCH)) {
-    // L2 prefetch distance: 3/4 of the sites resident on the chip (measured optimum on
-    // B200: 0.6 .. 0.9, profiles/r01_tuning.md). HLB_PREFETCH_SITES overrides it (tuning).
-    int dev = 0, sms = 0;
-    HLB_CUDA_G(cudaGetDevice(&dev));
-    HLB_CUDA_G(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull() * 3 / 4 / 128 * 128;
-    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa() * 3 / 4 / 128 * 128;
-    if (const char* e = std::getenv("HLB_PREFETCH_SITES"))
-      g->dg.prefetch_pull = g->dg.prefetch_aa = std::atoll(e);
-  }
   g->dg.canon = (const int32_t*)d_canon;
   g->dg.iolet_rho = (const double*)d_rho;
   g->dg.omega = 1.0 / p->tau;
@@ -268,6 +279,15 @@ static int init_from(hlb_geometry* g, const double* d_rho, const double* d_u, co
   return HLB_OK;
 }
 
+static int ensure_scratch_pop(hlb_geometry* g) {
+  if (g->scratch_pop) return HLB_OK;
+  void* ptr = nullptr;
+  const int rc = g->alloc(sizeof(double) * (size_t)Q * (size_t)g->N, &ptr);
+  if (rc) return rc;
+  g->scratch_pop = (double*)ptr;
+  return HLB_OK;
+}
+
 int hlb_set_state(hlb_geometry* g, const double* rho, const double* u) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   double *d_rho = nullptr, *d_u = nullptr;
@@ -285,8 +305,10 @@ int hlb_set_state(hlb_geometry* g, const double* rho, const double* u) {
 
 int hlb_set_populations(hlb_geometry* g, const double* f) {
   if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
-  HLB_CUDA(cudaMemcpyAsync(g->scratch, f, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyHostToDevice, g->stream));
-  return init_from(g, nullptr, nullptr, g->scratch);
+  int rc = ensure_scratch_pop(g);
+  if (rc) return rc;
+  HLB_CUDA(cudaMemcpyAsync(g->scratch_pop, f, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyHostToDevice, g->stream));
+  return init_from(g, nullptr, nullptr, g->scratch_pop);
 }
 
 int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho) {
@@ -386,9 +408,11 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u) {
 
 int hlb_get_populations(hlb_geometry* g, double* f) {
   if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
-  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->scratch, g->stream);
+  int rc = ensure_scratch_pop(g);
+  if (rc) return rc;
+  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->scratch_pop, g->stream);
   HLB_CUDA(cudaGetLastError());
-  HLB_CUDA(cudaMemcpyAsync(f, g->scratch, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaMemcpyAsync(f, g->scratch_pop, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));
   return HLB_OK;
 }
