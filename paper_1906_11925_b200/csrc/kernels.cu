@@ -84,20 +84,35 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
   uint4 v[Q - 1];
 #pragma unroll
   for (int q = 1; q < Q; ++q) v[q - 1] = __ldg(r + (q - 1));
+  // second <= 32 in a real record, 0xffffffff in a sentinel: one warp-uniform test decides
+  // whether this warp needs the table at all, so the common path carries no sentinel code
+  uint32_t any = 0u;
 #pragma unroll
-  for (int q = 1; q < Q; ++q) {
-    const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
-    const uint4 t = v[q - 1];
-    int32_t e;
-    bool wall;
-    if (t.y == 0xffffffffu) {  // sentinel: more than two runs
-      e = __ldg(nbr + (long long)(q - 1) * Ns + i);
-      wall = e < 0;
-    } else {
-      e = (int32_t)(lane >= t.y ? t.w : t.z) + (int32_t)lane;
-      wall = (t.x & lane_bit) != 0u;
+  for (int q = 1; q < Q; ++q) any |= v[q - 1].y;
+  if ((int32_t)any >= 0) {
+#pragma unroll
+    for (int q = 1; q < Q; ++q) {
+      const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
+      const uint4 t = v[q - 1];
+      const IT e = (IT)((lane >= t.y ? t.w : t.z) + lane);
+      off[q - 1] = (t.x & lane_bit) ? (IT)qw * n + self : (IT)qf * n + e;
     }
-    off[q - 1] = wall ? (IT)qw * n + self : (IT)qf * n + (IT)e;
+  } else {
+#pragma unroll
+    for (int q = 1; q < Q; ++q) {
+      const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
+      const uint4 t = v[q - 1];
+      int32_t e;
+      bool wall;
+      if (t.y == 0xffffffffu) {  // sentinel: more than two runs
+        e = __ldg(nbr + (long long)(q - 1) * Ns + i);
+        wall = e < 0;
+      } else {
+        e = (int32_t)((lane >= t.y ? t.w : t.z) + lane);
+        wall = (t.x & lane_bit) != 0u;
+      }
+      off[q - 1] = wall ? (IT)qw * n + self : (IT)qf * n + (IT)e;
+    }
   }
 }
 
@@ -162,6 +177,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
     for (int q = 1; q < Q; ++q) h[q] = to_real(src[off[q - 1]]);
     if (pf > 0 && i + pf < Ns) {
       const ST* ahead = src + pf;
+      asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
       if (REC && (threadIdx.x & 31) < 7)
         prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31));
       prefetch_l2(ahead + i);
@@ -228,6 +244,7 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   for (int q = 1; q < Q; ++q) h[q] = to_real(a[off[q - 1]]);
   if (pf > 0 && i + pf < Ns) {
     const ST* ahead = a + pf;
+    asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
     if (REC && (threadIdx.x & 31) < 7)
       prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31));
     prefetch_l2(ahead + i);
