@@ -22,6 +22,7 @@ HLB_ORDER_AUTO, HLB_ORDER_MORTON, HLB_ORDER_RASTER, HLB_ORDER_TILED = 0x0, 0x4, 
 HLB_NO_GRAPH = 0x10
 HLB_LINKS_AUTO, HLB_LINKS_TABLE, HLB_LINKS_RECORDS = 0x0, 0x20, 0x40
 HLB_NO_PREFETCH = 0x80
+HLB_INDEX64 = 0x100
 
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 

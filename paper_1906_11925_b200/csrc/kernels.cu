@@ -367,7 +367,7 @@ static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cud
 }
 template <typename ST>
 static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  const bool idx32 = (long long)Q * g.Ns < (1ll << 32);
+  const bool idx32 = !g.index64;
   if (g.use_rec) {
     if (idx32) pull_launch<ST, true, uint32_t>(g, src, dst, s);
     else pull_launch<ST, true, long long>(g, src, dst, s);
@@ -388,7 +388,7 @@ static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
 }
 template <typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
-  const bool idx32 = (long long)Q * g.Ns < (1ll << 32);
+  const bool idx32 = !g.index64;
   if (!odd) {
     k_aa_even<ST><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits,
                                                                g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);

@@ -13,6 +13,7 @@ struct DeviceGeometry {
   const uint32_t* iolet_bits = nullptr; // [Ns/32]
   const void* rec = nullptr;            // [Ns/32][14] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
+  bool index64 = false;                 // flat offsets need (or are forced to) 64 bits
   // > 0: every thread L2-prefetches what site i + prefetch_* will load (about 3/4 of the
   // sites resident on the chip at once, i.e. the blocks scheduled just under a wave later)
   int64_t prefetch_pull = 0, prefetch_aa = 0;

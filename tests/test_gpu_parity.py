@@ -206,6 +206,22 @@ def test_graph_replay_equals_direct_launches(hlb, scheme):
     b.close()
 
 
+@pytest.mark.parametrize("links", ["table", "records"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_64_bit_offset_kernels_equal_32_bit(hlb, scheme, links):
+    """Above 2^32 / 15 sites the kernels index with 64-bit offsets; HLB_INDEX64 forces that
+    instantiation on a small geometry: bitwise the same as the 32-bit one."""
+    wl = W.by_name("bigtree", small=True)
+    f = flags_of(hlb, scheme, "f64", "raster", links)
+    out = []
+    for extra in (0, hlb.HLB_INDEX64):
+        g = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | extra)
+        g.hlb_step(23)
+        out.append(g.hlb_get_macroscopic())
+        g.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+
+
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
 def test_l2_prefetch_changes_nothing(hlb, scheme, monkeypatch):
     """The L2 prefetches are hints: bitwise the same results with a distance that really
