@@ -29,7 +29,8 @@ def hlb():
 def flags_of(hlb, scheme, store, order="morton", links="auto"):
     f = hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE
     f |= hlb.HLB_STORE_F32 if store == "f32" else hlb.HLB_STORE_F64
-    f |= {"morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER, "tiled": hlb.HLB_ORDER_TILED}[order]
+    f |= {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
+          "tiled": hlb.HLB_ORDER_TILED}[order]
     f |= {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE, "records": hlb.HLB_LINKS_RECORDS}[links]
     return f
 
@@ -348,6 +349,86 @@ def test_config2_aneurysm_full_size(hlb):
     for scheme in ("two_lattice", "aa"):
         e_rho, e_u = errors(*run_gpu(hlb, wl, 150, scheme, "f64"), rho_ref, u_ref)
         assert e_rho < 1e-12 and e_u < 1e-12, (scheme, e_rho, e_u)
+
+
+def _smooth_state(x, y, z):
+    """A smooth, non-trivial initial field as a function of ABSOLUTE voxel coordinates, so
+    that a crop and the full geometry start from the same state."""
+    x, y, z = (np.asarray(a, dtype=np.float64) for a in (x, y, z))
+    rho = 1.0 + 0.01 * np.sin(0.07 * x + 0.05 * y) * np.cos(0.06 * z)
+    u = 0.02 * np.stack([np.sin(0.05 * y + 0.03 * z), np.cos(0.04 * x - 0.06 * z),
+                         np.sin(0.03 * x + 0.07 * y)], axis=1)
+    return rho, u
+
+
+def _crop_check(hlb, wl, rho, u, steps, centre, half, tol):
+    """Exact check of a full-size run on a sample: a site update is local (information moves
+    one voxel per step), so the oracle run on the sub-box [centre - half, centre + half] of
+    the same voxel array (outside the crop = solid) reproduces, after `steps` steps, every
+    site that is more than `steps` voxels away from the crop faces lying inside the box."""
+    st = wl.site_type
+    nz, ny, nx = st.shape
+    lo = [max(0, c - half) for c in centre]
+    hi = [min(n, c + half + 1) for c, n in zip(centre, (nx, ny, nz))]
+    sub = np.ascontiguousarray(st[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]])
+    o = oracle.Oracle(sub, 0, wl.tau, wl.iolet_rho, threads=0)
+    v = o.site_voxels()
+    sx, sy, sz = hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]
+    x, y, z = v % sx + lo[0], (v // sx) % sy + lo[1], v // (sx * sy) + lo[2]
+    o.set_state(*_smooth_state(x, y, z))
+    o.step(steps)
+    rho_c, u_c = o.get_macroscopic()
+    o.close()
+    keep = np.ones(v.shape, dtype=bool)
+    for c, l, h, n in ((x, lo[0], hi[0], nx), (y, lo[1], hi[1], ny), (z, lo[2], hi[2], nz)):
+        if l > 0:
+            keep &= c - l > steps
+        if h < n:
+            keep &= (h - 1) - c > steps
+    assert keep.sum() > 1000, "sample too small to mean anything"
+    full_voxel = (z * ny + y) * nx + x
+    canon = np.searchsorted(wl.fluid_voxels(), full_voxel[keep])
+    e_rho = np.max(np.abs(rho[canon] - rho_c[keep])) / np.max(np.abs(rho_c[keep]))
+    un = np.max(np.linalg.norm(u_c[keep], axis=1))
+    e_u = np.max(np.abs(u[canon] - u_c[keep])) / (un if un > 0 else 1.0)
+    assert e_rho < tol and e_u < tol, (centre, e_rho, e_u)
+    return int(keep.sum()), un
+
+
+def _sample_centres(wl, n):
+    """The inlet end, the outlet-most end and evenly spaced fluid voxels in between."""
+    v = wl.fluid_voxels()
+    nz, ny, nx = wl.site_type.shape
+    picks = v[np.linspace(0, len(v) - 1, n).astype(np.int64)]
+    x = picks % nx
+    return [(int(a), int(b), int(c)) for a, b, c in zip(x, (picks // nx) % ny, picks // (nx * ny))]
+
+
+@pytest.mark.parametrize("name,scheme,store", [
+    ("tree", "two_lattice", "f64"), ("tree", "two_lattice", "f32"), ("bigtree", "aa", "f64"),
+])
+def test_configs_3_4_full_size_sampled_against_oracle(hlb, name, scheme, store):
+    """BASELINE configs[3] / [4] at full size in the launch configuration bench.py times
+    (default order, link records, L2 prefetch): 25 steps (odd: A-A read-out through the
+    table), then sub-boxes compared site by site with the oracle (see _crop_check)."""
+    wl = W.by_name(name)
+    steps, half = 25, 56
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, scheme, store, "auto", "auto"))
+    assert g.hlb_uses_records()
+    nz, ny, nx = wl.site_type.shape
+    v = wl.fluid_voxels()
+    g.hlb_set_state(*_smooth_state(v % nx, (v // nx) % ny, v // (nx * ny)))
+    g.hlb_step(steps)
+    rho, u = g.hlb_get_macroscopic()
+    g.close()
+    assert np.all(np.isfinite(rho)) and np.all(np.isfinite(u))
+    checked = 0
+    for centre in _sample_centres(wl, 5):
+        n, un = _crop_check(hlb, wl, rho, u, steps, centre, half, TOL[store])
+        assert un > 1e-3                                  # the sample is not at rest
+        checked += n
+    assert checked > 20000
 
 
 @pytest.mark.slow
