@@ -14,4 +14,5 @@ from .hlb_oracle import (  # noqa: F401
     VARIANT_RAW,
     VARIANT_SHIFTED_LD,
     VARIANT_RAW_LD,
+    LATTICE_Q,
 )

@@ -47,6 +47,13 @@ def _load():
         lib.hlbo_create.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                     ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
                                     ctypes.c_int]
+        lib.hlbo_create_lattice.restype = ctypes.c_void_p
+        lib.hlbo_create_lattice.argtypes = lib.hlbo_create.argtypes + [ctypes.c_int]
+        lib.hlbo_velocity_set_lattice.restype = ctypes.c_int
+        lib.hlbo_velocity_set_lattice.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                                                  ctypes.c_void_p]
+        lib.hlbo_num_q.restype = ctypes.c_int
+        lib.hlbo_num_q.argtypes = [ctypes.c_void_p]
         lib.hlbo_destroy.argtypes = [ctypes.c_void_p]
         lib.hlbo_destroy.restype = None
         for name in ("hlbo_num_sites", "hlbo_steps_done"):
@@ -66,6 +73,8 @@ def _load():
                                  ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                  ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbd_run_lattice.restype = ctypes.c_int
+        lib.hlbd_run_lattice.argtypes = lib.hlbd_run.argtypes + [ctypes.c_int]
         for name in ("hlbo_site_voxels", "hlbo_set_state", "hlbo_set_populations",
                      "hlbo_get_populations", "hlbo_step", "hlbo_get_macroscopic",
                      "hlbo_velocity_set", "hlbo_set_threads"):
@@ -79,13 +88,17 @@ def _ptr(a):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
-def velocity_set():
-    """(c[15,3] int32, w[15] float64, opp[15] int32) in the oracle's own q order."""
+LATTICE_Q = {"d3q15": 15, "d3q19": 19}
+
+
+def velocity_set(lattice="d3q15"):
+    """(c[Q,3] int32, w[Q] float64, opp[Q] int32) in the oracle's own q order."""
     lib = _load()
-    c = np.zeros((15, 3), dtype=np.int32)
-    w = np.zeros(15, dtype=np.float64)
-    opp = np.zeros(15, dtype=np.int32)
-    lib.hlbo_velocity_set(_ptr(c), _ptr(w), _ptr(opp))
+    nq = LATTICE_Q[lattice]
+    c = np.zeros((nq, 3), dtype=np.int32)
+    w = np.zeros(nq, dtype=np.float64)
+    opp = np.zeros(nq, dtype=np.int32)
+    assert lib.hlbo_velocity_set_lattice(nq, _ptr(c), _ptr(w), _ptr(opp)) == nq
     return c, w, opp
 
 
@@ -93,7 +106,7 @@ class Oracle:
     """One oracle simulation. Per-site arrays are in canonical order (ascending voxel)."""
 
     def __init__(self, site_type, periodic=0, tau=1.0, iolet_rho=(), variant=VARIANT_SHIFTED,
-                 threads=1):
+                 threads=1, lattice="d3q15"):
         lib = _load()
         st = np.ascontiguousarray(site_type, dtype=np.uint8)
         assert st.ndim == 3
@@ -101,8 +114,9 @@ class Oracle:
         io = np.ascontiguousarray(np.asarray(iolet_rho, dtype=np.float64))
         lib.hlbo_set_threads(int(threads))
         self._lib = lib
-        self._h = lib.hlbo_create(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
-                                  _ptr(io), int(variant))
+        self.n_q = LATTICE_Q[lattice]
+        self._h = lib.hlbo_create_lattice(_ptr(st), nx, ny, nz, int(periodic), float(tau),
+                                          int(io.shape[0]), _ptr(io), int(variant), self.n_q)
         if not self._h:
             raise ValueError("hlbo_create rejected its arguments")
         self.n_sites = int(lib.hlbo_num_sites(self._h))
@@ -131,11 +145,11 @@ class Oracle:
 
     def set_populations(self, f):
         f = np.ascontiguousarray(f, dtype=np.float64)
-        assert f.shape == (self.n_sites, 15)
+        assert f.shape == (self.n_sites, self.n_q)
         self._lib.hlbo_set_populations(self._h, _ptr(f))
 
     def get_populations(self):
-        f = np.zeros((self.n_sites, 15), dtype=np.float64)
+        f = np.zeros((self.n_sites, self.n_q), dtype=np.float64)
         self._lib.hlbo_get_populations(self._h, _ptr(f))
         return f
 
@@ -153,10 +167,10 @@ class Oracle:
         return rho, u
 
 
-def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1):
+def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15"):
     """Run a workloads.Workload for ``steps`` (default: its own count); returns rho, u."""
     o = Oracle(workload.site_type, workload.periodic, workload.tau, workload.iolet_rho,
-               variant=variant, threads=threads)
+               variant=variant, threads=threads, lattice=lattice)
     if workload.rho0 is not None or workload.u0 is not None:
         o.set_state(workload.rho0, workload.u0)
     o.step(workload.steps if steps is None else steps)
@@ -165,7 +179,8 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1):
     return out
 
 
-def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None):
+def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None,
+              lattice="d3q15"):
     """Dense-grid twin: per-VOXEL rho [nz,ny,nx] and u [nz,ny,nx,3]."""
     lib = _load()
     st = np.ascontiguousarray(site_type, dtype=np.uint8)
@@ -175,8 +190,9 @@ def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=
     u0 = None if u0_vox is None else np.ascontiguousarray(u0_vox, dtype=np.float64)
     rho = np.zeros((nz, ny, nx), dtype=np.float64)
     u = np.zeros((nz, ny, nx, 3), dtype=np.float64)
-    rc = lib.hlbd_run(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]), _ptr(io),
-                      _ptr(r0), _ptr(u0), int(steps), _ptr(rho), _ptr(u))
+    rc = lib.hlbd_run_lattice(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
+                              _ptr(io), _ptr(r0), _ptr(u0), int(steps), _ptr(rho), _ptr(u),
+                              LATTICE_Q[lattice])
     if rc != 0:
         raise ValueError("hlbd_run rejected its arguments")
     return rho, u

@@ -5,7 +5,7 @@
 // up as a disagreement on random small masks:
 //   * arrays over the WHOLE box (every voxel, fluid or not), no site list, no table;
 //   * PUSH form: each fluid voxel collides, then sends f*_q to x + c_q;
-//   * its own hand-typed D3Q15 table in a different order from hlb_oracle.cpp;
+//   * its own hand-typed D3Q15 and D3Q19 tables in a different order from hlb_oracle.cpp;
 //   * raw populations f_q (the textbook formula verbatim), moments as explicit sums.
 //
 // Same method: D3Q15 LBGK ("propagation and collision steps"), halfway bounce-back
@@ -21,19 +21,39 @@
 
 namespace {
 
-// rest, 6 axis vectors, 8 cube diagonals (hand typed)
-const int CX[15] = {0, 1, -1, 0, 0, 0, 0, 1, 1, 1, 1, -1, -1, -1, -1};
-const int CY[15] = {0, 0, 0, 1, -1, 0, 0, 1, 1, -1, -1, 1, 1, -1, -1};
-const int CZ[15] = {0, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 1, -1};
-const int OPP[15] = {0, 2, 1, 4, 3, 6, 5, 14, 13, 12, 11, 10, 9, 8, 7};
-const double WT[15] = {2.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0,
-                       1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0,
-                       1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0};
+struct Lattice {
+  int Q;
+  const int *CX, *CY, *CZ, *OPP;
+  const double* WT;
+};
 
-double feq(int q, double rho, double ux, double uy, double uz) {
-  double cu = CX[q] * ux + CY[q] * uy + CZ[q] * uz;
+// D3Q15: rest, 6 axis vectors, 8 cube diagonals (hand typed)
+const int CX15[15] = {0, 1, -1, 0, 0, 0, 0, 1, 1, 1, 1, -1, -1, -1, -1};
+const int CY15[15] = {0, 0, 0, 1, -1, 0, 0, 1, 1, -1, -1, 1, 1, -1, -1};
+const int CZ15[15] = {0, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 1, -1};
+const int OPP15[15] = {0, 2, 1, 4, 3, 6, 5, 14, 13, 12, 11, 10, 9, 8, 7};
+const double WT15[15] = {2.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0, 1.0 / 9.0,
+                         1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0,
+                         1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0, 1.0 / 72.0};
+
+// D3Q19: rest, 6 axis vectors, then the 12 face diagonals plane by plane: xy, xz, yz
+// (hand typed; weights 1/3, 1/18, 1/36)
+const int CX19[19] = {0, 1, -1, 0, 0, 0, 0, 1, 1, -1, -1, 1, 1, -1, -1, 0, 0, 0, 0};
+const int CY19[19] = {0, 0, 0, 1, -1, 0, 0, 1, -1, 1, -1, 0, 0, 0, 0, 1, 1, -1, -1};
+const int CZ19[19] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1};
+const int OPP19[19] = {0, 2, 1, 4, 3, 6, 5, 10, 9, 8, 7, 14, 13, 12, 11, 18, 17, 16, 15};
+const double WT19[19] = {1.0 / 3.0, 1.0 / 18.0, 1.0 / 18.0, 1.0 / 18.0, 1.0 / 18.0, 1.0 / 18.0,
+                         1.0 / 18.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0,
+                         1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0,
+                         1.0 / 36.0};
+
+const Lattice L15 = {15, CX15, CY15, CZ15, OPP15, WT15};
+const Lattice L19 = {19, CX19, CY19, CZ19, OPP19, WT19};
+
+double feq(const Lattice& L, int q, double rho, double ux, double uy, double uz) {
+  double cu = L.CX[q] * ux + L.CY[q] * uy + L.CZ[q] * uz;
   double uu = ux * ux + uy * uy + uz * uz;
-  return WT[q] * rho * (1.0 + 3.0 * cu + 4.5 * cu * cu - 1.5 * uu);
+  return L.WT[q] * rho * (1.0 + 3.0 * cu + 4.5 * cu * cu - 1.5 * uu);
 }
 
 }  // namespace
@@ -43,12 +63,16 @@ extern "C" {
 // rho0 / u0: per VOXEL ([nvox], [nvox][3]), read only at fluid voxels; NULL => 1 / 0.
 // rho_out / u_out: per voxel, written at fluid voxels, 0 elsewhere.
 // Returns 0, or -1 on a bad argument.
-int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
-             int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
-             int64_t steps, double* rho_out, double* u_out) {
+int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                     int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
+                     int64_t steps, double* rho_out, double* u_out, int lattice_q) {
+  if (lattice_q != 15 && lattice_q != 19) return -1;
+  const Lattice& L = lattice_q == 15 ? L15 : L19;
+  const int Q = L.Q;
+  const int *CX = L.CX, *CY = L.CY, *CZ = L.CZ, *OPP = L.OPP;
   if (!type || nx <= 0 || ny <= 0 || nz <= 0 || !(tau > 0.5) || steps < 0) return -1;
   const int64_t nvox = (int64_t)nx * ny * nz;
-  std::vector<double> f((size_t)nvox * 15, 0.0), g((size_t)nvox * 15, 0.0);
+  std::vector<double> f((size_t)nvox * Q, 0.0), g((size_t)nvox * Q, 0.0);
   for (int z = 0; z < nz; ++z)
     for (int y = 0; y < ny; ++y)
       for (int x = 0; x < nx; ++x) {
@@ -57,7 +81,7 @@ int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, dou
         const double r = rho0 ? rho0[v] : 1.0;
         const double ux = u0 ? u0[v * 3 + 0] : 0.0, uy = u0 ? u0[v * 3 + 1] : 0.0,
                      uz = u0 ? u0[v * 3 + 2] : 0.0;
-        for (int q = 0; q < 15; ++q) f[v * 15 + q] = feq(q, r, ux, uy, uz);
+        for (int q = 0; q < Q; ++q) f[v * Q + q] = feq(L, q, r, ux, uy, uz);
       }
   for (int64_t s = 0; s < steps; ++s) {
     for (int z = 0; z < nz; ++z)
@@ -65,14 +89,14 @@ int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, dou
         for (int x = 0; x < nx; ++x) {
           const int64_t v = ((int64_t)z * ny + y) * nx + x;
           if (type[v] != 1) continue;
-          const double* fv = &f[v * 15];
+          const double* fv = &f[v * Q];
           double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
-          for (int q = 0; q < 15; ++q) {
+          for (int q = 0; q < Q; ++q) {
             rho += fv[q]; jx += CX[q] * fv[q]; jy += CY[q] * fv[q]; jz += CZ[q] * fv[q];
           }
           const double ux = jx / rho, uy = jy / rho, uz = jz / rho;
-          for (int q = 0; q < 15; ++q) {
-            const double fstar = fv[q] - (fv[q] - feq(q, rho, ux, uy, uz)) / tau;
+          for (int q = 0; q < Q; ++q) {
+            const double fstar = fv[q] - (fv[q] - feq(L, q, rho, ux, uy, uz)) / tau;
             int dx = x + CX[q], dy = y + CY[q], dz = z + CZ[q];
             bool outside = false;
             if (dx < 0) { if (periodic & 1u) dx += nx; else outside = true; }
@@ -83,11 +107,11 @@ int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, dou
             if (dz >= nz) { if (periodic & 4u) dz -= nz; else outside = true; }
             const int64_t d = outside ? -1 : ((int64_t)dz * ny + dy) * nx + dx;
             const int t = outside ? 0 : (int)type[d];
-            if (t == 1) g[d * 15 + q] = fstar;
-            else if (t == 0) g[v * 15 + OPP[q]] = fstar;
+            if (t == 1) g[d * Q + q] = fstar;
+            else if (t == 0) g[v * Q + OPP[q]] = fstar;
             else {
               if (t - 2 >= n_iolets) return -1;
-              g[v * 15 + OPP[q]] = feq(OPP[q], iolet_rho[t - 2], ux, uy, uz);
+              g[v * Q + OPP[q]] = feq(L, OPP[q], iolet_rho[t - 2], ux, uy, uz);
             }
           }
         }
@@ -96,8 +120,8 @@ int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, dou
   for (int64_t v = 0; v < nvox; ++v) {
     double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
     if (type[v] == 1) {
-      for (int q = 0; q < 15; ++q) {
-        const double fq = f[v * 15 + q];
+      for (int q = 0; q < Q; ++q) {
+        const double fq = f[v * Q + q];
         rho += fq; jx += CX[q] * fq; jy += CY[q] * fq; jz += CZ[q] * fq;
       }
       rho_out[v] = rho; u_out[v * 3 + 0] = jx / rho; u_out[v * 3 + 1] = jy / rho; u_out[v * 3 + 2] = jz / rho;
@@ -106,6 +130,13 @@ int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, dou
     }
   }
   return 0;
+}
+
+int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+             int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
+             int64_t steps, double* rho_out, double* u_out) {
+  return hlbd_run_lattice(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, rho0, u0, steps,
+                          rho_out, u_out, 15);
 }
 
 }  // extern "C"

@@ -16,6 +16,35 @@ import oracle
 import workloads as W
 
 C, WT, OPP = oracle.velocity_set()
+NQ = 15
+
+
+@pytest.fixture(autouse=True, params=["d3q15", "d3q19"])
+def lattice(request, monkeypatch):
+    """Every pin runs for both lattices of the oracle: D3Q15 (BASELINE.json) and D3Q19 (the
+    lattice the paper names). The fixture makes `lattice=...` the
+    default of oracle.Oracle / oracle.dense_run and points C, WT, OPP, NQ at that lattice."""
+    import sys
+    lat = request.param
+    orig_init, orig_dense = oracle.Oracle.__init__, oracle.dense_run
+
+    def init(self, *a, **k):
+        k.setdefault("lattice", lat)
+        orig_init(self, *a, **k)
+
+    def dense(*a, **k):
+        k.setdefault("lattice", lat)
+        return orig_dense(*a, **k)
+
+    monkeypatch.setattr(oracle.Oracle, "__init__", init)
+    monkeypatch.setattr(oracle, "dense_run", dense)
+    me = sys.modules[__name__]
+    c, w, o = oracle.velocity_set(lat)
+    monkeypatch.setattr(me, "C", c)
+    monkeypatch.setattr(me, "WT", w)
+    monkeypatch.setattr(me, "OPP", o)
+    monkeypatch.setattr(me, "NQ", len(w))
+    return lat
 
 
 def canon_coords(st):
@@ -25,17 +54,23 @@ def canon_coords(st):
 
 
 # ------------------------------------------------------------------ P1 lattice identities
-def test_p1_velocity_set_is_d3q15():
+def test_p1_velocity_set_is_d3q15_or_d3q19(lattice):
     vecs = {tuple(int(a) for a in c) for c in C}
-    assert len(vecs) == 15
+    assert len(vecs) == NQ == {"d3q15": 15, "d3q19": 19}[lattice]
     assert (0, 0, 0) in vecs
     axis = {v for v in vecs if sum(abs(a) for a in v) == 1}
-    diag = {v for v in vecs if all(abs(a) == 1 for a in v)}
-    assert len(axis) == 6 and len(diag) == 8
+    cube = {v for v in vecs if all(abs(a) == 1 for a in v)}
+    face = {v for v in vecs if sum(abs(a) for a in v) == 2}
+    assert len(axis) == 6
+    if lattice == "d3q15":
+        assert len(cube) == 8 and len(face) == 0
+        table = {0: Fraction(2, 9), 1: Fraction(1, 9), 3: Fraction(1, 72)}
+    else:
+        assert len(cube) == 0 and len(face) == 12
+        table = {0: Fraction(1, 3), 1: Fraction(1, 18), 2: Fraction(1, 36)}
     w = [Fraction(float(x)).limit_denominator(1000) for x in WT]
     for c, wq in zip(C, w):
-        n2 = int(np.dot(c, c))
-        assert wq == {0: Fraction(2, 9), 1: Fraction(1, 9), 3: Fraction(1, 72)}[n2]
+        assert wq == table[int(np.dot(c, c))]
     assert sum(w) == 1
 
 
@@ -44,19 +79,19 @@ def test_p1_moment_identities():
     c = [[int(a) for a in q] for q in C]
     d = lambda a, b: 1 if a == b else 0
     for a in range(3):
-        assert sum(w[q] * c[q][a] for q in range(15)) == 0
+        assert sum(w[q] * c[q][a] for q in range(NQ)) == 0
         for b in range(3):
-            assert sum(w[q] * c[q][a] * c[q][b] for q in range(15)) == Fraction(d(a, b), 3)
+            assert sum(w[q] * c[q][a] * c[q][b] for q in range(NQ)) == Fraction(d(a, b), 3)
             for e in range(3):
-                assert sum(w[q] * c[q][a] * c[q][b] * c[q][e] for q in range(15)) == 0
+                assert sum(w[q] * c[q][a] * c[q][b] * c[q][e] for q in range(NQ)) == 0
                 for g in range(3):
                     iso = Fraction(d(a, b) * d(e, g) + d(a, e) * d(b, g) + d(a, g) * d(b, e), 9)
                     assert sum(w[q] * c[q][a] * c[q][b] * c[q][e] * c[q][g]
-                               for q in range(15)) == iso
+                               for q in range(NQ)) == iso
 
 
 def test_p1_opposites():
-    for q in range(15):
+    for q in range(NQ):
         assert OPP[OPP[q]] == q
         assert np.array_equal(C[OPP[q]], -C[q])
         assert WT[OPP[q]] == WT[q]
@@ -111,8 +146,10 @@ def test_p4_mass_conserved_with_walls():
 
 
 # ------------------------------------------------------------------ pure streaming
-@pytest.mark.parametrize("q", range(15))
+@pytest.mark.parametrize("q", range(19))
 def test_streaming_moves_a_marked_population_along_c(q):
+    if q >= NQ:
+        pytest.skip("D3Q15 has 15 directions")
     """tau = 1e30 switches collision off (f* = f exactly in fp64); a marked population in
     slot q at x0 must be found in slot q at x0 + n c_q (periodic wrap) and nowhere else."""
     nx, ny, nz = 5, 4, 3
@@ -139,7 +176,7 @@ def test_streaming_bounces_back_half_way():
     half a link beyond x = 3), then at x = 2 moving -x."""
     st = np.ones((1, 1, 4), dtype=np.uint8)
     o = oracle.Oracle(st, 0, 1e30, [])
-    qp = [q for q in range(15) if tuple(C[q]) == (1, 0, 0)][0]
+    qp = [q for q in range(NQ) if tuple(C[q]) == (1, 0, 0)][0]
     qm = OPP[qp]
     base = np.tile(WT, (4, 1))
     # y/z links all bounce back onto the same site, so the base state is stationary
@@ -163,9 +200,9 @@ def test_non_equilibrium_part_decays_by_one_minus_one_over_tau(tau):
     and a mass- and momentum-free perturbation decays exactly as (1 - 1/tau)^n."""
     st = np.ones((1, 1, 1), dtype=np.uint8)
     o = oracle.Oracle(st, 7, tau, [])
-    qx = [q for q in range(15) if tuple(C[q]) == (1, 0, 0)][0]
-    q0 = [q for q in range(15) if tuple(C[q]) == (0, 0, 0)][0]
-    pert = np.zeros(15)
+    qx = [q for q in range(NQ) if tuple(C[q]) == (1, 0, 0)][0]
+    q0 = [q for q in range(NQ) if tuple(C[q]) == (0, 0, 0)][0]
+    pert = np.zeros(NQ)
     pert[qx] = pert[OPP[qx]] = 1e-3
     pert[q0] = -2e-3
     o.set_populations((WT + pert)[None, :])
