@@ -69,9 +69,14 @@ enum {
   HLB_LINKS_TABLE = 0x20,  /* always read the int32 table (ablation / profiling)           */
   HLB_LINKS_RECORDS = 0x40,/* always read the records                                     */
   HLB_NO_PREFETCH = 0x80,  /* step kernels issue no L2 prefetches (ablation / profiling)   */
-  HLB_INDEX64 = 0x100      /* use the 64-bit flat-offset kernels even when 15 * stride fits
+  HLB_INDEX64 = 0x100,     /* use the 64-bit flat-offset kernels even when Q * stride fits
                               32 bits (they are otherwise only taken above 286 M sites;
                               this flag lets small tests cover them)                       */
+  HLB_LATTICE_D3Q15 = 0x0, /* 15 velocities: rest, 6 axis, 8 cube diagonals (BASELINE.json) */
+  HLB_LATTICE_D3Q19 = 0x200 /* 19 velocities: rest, 6 axis, 12 face diagonals -- the lattice
+                              the paper names. Everywhere below
+                              Q = 15 or 19 is the lattice's population count and Q - 1 its
+                              link count                                                   */
 };
 
 typedef struct hlb_geometry hlb_geometry; /* opaque handle */
@@ -125,17 +130,18 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u);
 /* Same, into DEVICE buffers (rho [N], u [N][3]); enqueued on the stream, no sync. */
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);
 
-/* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][15], canonical site
- * order, q in the order of hlb_velocity_set(). For population-level parity checks. The
- * first call of this or of hlb_set_populations allocates a [N][15] fp64 staging buffer
+/* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][Q], canonical site
+ * order, q in the order of hlb_lattice(). For population-level parity checks. The
+ * first call of this or of hlb_set_populations allocates a [N][Q] fp64 staging buffer
  * through the allocator (HLB_ENOMEM if that fails). */
 int hlb_get_populations(hlb_geometry* g, double* f);
 
-/* Set pre-collision populations f_q(x, 0) directly (HOST [N][15], layout as above) and
+/* Set pre-collision populations f_q(x, 0) directly (HOST [N][Q], layout as above) and
  * the step counter to 0. */
 int hlb_set_populations(hlb_geometry* g, const double* f);
 
 int64_t hlb_num_sites(const hlb_geometry* g);  /* N, or HLB_EINVAL for NULL                */
+int hlb_num_q(const hlb_geometry* g);          /* Q of the geometry's lattice (15 or 19)   */
 int64_t hlb_steps_done(const hlb_geometry* g);
 /* Linear voxel index of every site, HOST [N], canonical order (ascending). */
 int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v);
@@ -153,21 +159,24 @@ const char* hlb_last_error(void);           /* thread-local, never NULL         
 
 /* The library's D3Q15 set: c HOST [15][3], w HOST [15], opp HOST [15]. */
 void hlb_velocity_set(int32_t* c, double* w, int32_t* opp);
+/* The velocity set selected by the HLB_LATTICE_* bits of flags: c HOST [Q][3], w HOST [Q],
+ * opp HOST [Q] (arrays of 19 entries always suffice; any may be NULL). Returns Q. */
+int hlb_lattice(uint32_t flags, int32_t* c, double* w, int32_t* opp);
 
 /* ---- geometry preprocessor, host only (subsystem (b) of BASELINE.json north_star) ----
  * Two calls: hlb_preprocess_count() gives N and the plane stride Ns (N rounded up to a
  * multiple of 128); hlb_preprocess_tables() fills caller-allocated HOST arrays:
  *   voxel_of_site [N]      linear voxel index of internal site i
  *   canon_of_site [N]      canonical rank of internal site i
- *   nbr           [14][Ns] entry (q-1)*Ns + i describes the pull source x - c_q of link q
- *                          (q = 1..14) of internal site i:
+ *   nbr           [Q-1][Ns] entry (q-1)*Ns + i describes the pull source x - c_q of link q
+ *                          (q = 1..Q-1) of internal site i:
  *                            >= 0            internal index of the fluid source site
  *                            0x80000000      solid (or outside a non-periodic box): the
  *                                            bounce-back target is slot opp(q) of site i
  *                            0x80000000 | (k+1)  ghost voxel of iolet k (also a bounce-back
  *                                            target; the kernel substitutes f_eq(rho_k, u))
  *                          entries i >= N of each plane are 0x80000000.
- * Only nx, ny, nz, periodic, n_iolets and the HLB_ORDER_* bits of p are read. */
+ * Only nx, ny, nz, periodic, n_iolets and the HLB_ORDER_* / HLB_LATTICE_* bits of p are read. */
 int hlb_preprocess_count(const uint8_t* site_type, const hlb_params* p, int64_t* n_sites,
                          int64_t* stride);
 int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t* voxel_of_site,
@@ -175,7 +184,7 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
 
 /* Run-length link records of a table (host only): the compressed form of nbr that the step
  * kernels read. A group is 32 consecutive internal sites (one warp). For group g and link q
- * the record rec[(g*14 + (q-1))*4 .. +4] = { wall, second, off0, off1 }:
+ * the record rec[(g*n_links + (q-1))*4 .. +4] = { wall, second, off0, off1 }:
  *   wall    bit l set: the entry of lane l is negative (solid or iolet: bounce-back target)
  *   second  the non-wall lanes split into runs of lanes with consecutive entries (a wall
  *           lane or a jump in the entries ends a run); second = the lane at which run 1
@@ -184,10 +193,12 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
  * so that the entry of a non-wall lane l is (l >= second ? off1 : off0) + l. A (g, q) with
  * more than two runs gets the sentinel { 0, 0xffffffff, 0, 0 } and the kernels read nbr for
  * it instead.
- *   nbr: HOST [14][stride] as filled by hlb_preprocess_tables; stride a multiple of 32
- *   rec: HOST [stride/32][14][4] uint32, filled
+ *   nbr: HOST [n_links][stride] as filled by hlb_preprocess_tables; stride a multiple of 32;
+ *        n_links = Q - 1 = 14 or 18
+ *   rec: HOST [stride/32][n_links][4] uint32, filled
  *   n_sentinel: number of (g, q) that got the sentinel (may be NULL) */
-int hlb_preprocess_records(const int32_t* nbr, int64_t stride, uint32_t* rec, int64_t* n_sentinel);
+int hlb_preprocess_records(const int32_t* nbr, int32_t n_links, int64_t stride, uint32_t* rec,
+                           int64_t* n_sentinel);
 
 #ifdef __cplusplus
 }

@@ -23,6 +23,7 @@ HLB_NO_GRAPH = 0x10
 HLB_LINKS_AUTO, HLB_LINKS_TABLE, HLB_LINKS_RECORDS = 0x0, 0x20, 0x40
 HLB_NO_PREFETCH = 0x80
 HLB_INDEX64 = 0x100
+HLB_LATTICE_D3Q15, HLB_LATTICE_D3Q19 = 0x0, 0x200
 
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 
@@ -61,13 +62,15 @@ def _load() -> ctypes.CDLL:
         "hlb_get_populations": (c_int, [vp, vp]),
         "hlb_set_populations": (c_int, [vp, vp]),
         "hlb_num_sites": (i64, [vp]),
+        "hlb_num_q": (c_int, [vp]),
+        "hlb_lattice": (c_int, [ctypes.c_uint32, vp, vp, vp]),
         "hlb_steps_done": (i64, [vp]),
         "hlb_get_site_voxels": (c_int, [vp, vp]),
         "hlb_device_bytes": (i64, [vp]),
         "hlb_launch_count": (i64, [vp]),
         "hlb_uses_records": (c_int, [vp]),
         "hlb_record_sentinel_fraction": (ctypes.c_double, [vp]),
-        "hlb_preprocess_records": (c_int, [vp, i64, vp, ctypes.POINTER(i64)]),
+        "hlb_preprocess_records": (c_int, [vp, ctypes.c_int32, i64, vp, ctypes.POINTER(i64)]),
         "hlb_geometry_destroy": (None, [vp]),
         "hlb_last_error": (ctypes.c_char_p, []),
         "hlb_velocity_set": (None, [vp, vp, vp]),
@@ -86,7 +89,7 @@ LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
-            "hlb_set_populations", "hlb_num_sites", "hlb_steps_done", "hlb_get_site_voxels",
+            "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
             "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
             "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables",
@@ -123,6 +126,15 @@ def hlb_velocity_set():
     return c, w, opp
 
 
+def hlb_lattice(flags=0):
+    """(c[Q,3], w[Q], opp[Q]) of the lattice selected by the HLB_LATTICE_* bits of flags."""
+    c = np.zeros((19, 3), dtype=np.int32)
+    w = np.zeros(19, dtype=np.float64)
+    opp = np.zeros(19, dtype=np.int32)
+    q = _lib.hlb_lattice(int(flags), _ptr(c), _ptr(w), _ptr(opp))
+    return c[:q].copy(), w[:q].copy(), opp[:q].copy()
+
+
 def _params(site_type, periodic, tau, iolet_rho, flags):
     st = np.ascontiguousarray(site_type, dtype=np.uint8)
     if st.ndim != 3:
@@ -140,27 +152,27 @@ def _params(site_type, periodic, tau, iolet_rho, flags):
 
 
 def hlb_preprocess(site_type, periodic=0, n_iolets=0, flags=0):
-    """Host-only preprocessor: returns dict(N, Ns, voxel_of_site, canon_of_site, nbr[14, Ns])."""
+    """Host-only preprocessor: returns dict(N, Ns, voxel_of_site, canon_of_site, nbr[Q-1, Ns])."""
     st, io, p = _params(site_type, periodic, 1.0, np.ones(n_iolets), flags)
     n, ns = ctypes.c_int64(0), ctypes.c_int64(0)
     _check(_lib.hlb_preprocess_count(_ptr(st), ctypes.byref(p), ctypes.byref(n), ctypes.byref(ns)))
     N, Ns = n.value, ns.value
     vox = np.zeros(N, dtype=np.int64)
     canon = np.zeros(N, dtype=np.int32)
-    nbr = np.zeros((14, Ns), dtype=np.int32)
+    nbr = np.zeros((18 if int(flags) & HLB_LATTICE_D3Q19 else 14, Ns), dtype=np.int32)
     _check(_lib.hlb_preprocess_tables(_ptr(st), ctypes.byref(p), _ptr(vox), _ptr(canon), _ptr(nbr)))
     return {"N": N, "Ns": Ns, "voxel_of_site": vox, "canon_of_site": canon, "nbr": nbr}
 
 
 def hlb_preprocess_records(nbr):
-    """Run-length link records of a [14, Ns] table: (rec [Ns/32, 14, 4] uint32, n_sentinel)."""
+    """Run-length link records of a [Q-1, Ns] table: (rec [Ns/32, Q-1, 4] uint32, n_sentinel)."""
     nbr = np.ascontiguousarray(nbr, dtype=np.int32)
-    if nbr.ndim != 2 or nbr.shape[0] != 14:
-        raise ValueError("nbr must be [14, Ns]")
-    ns = nbr.shape[1]
-    rec = np.zeros((max(ns // 32, 0), 14, 4), dtype=np.uint32)
+    if nbr.ndim != 2 or nbr.shape[0] not in (14, 18):
+        raise ValueError("nbr must be [14, Ns] or [18, Ns]")
+    nl, ns = nbr.shape
+    rec = np.zeros((max(ns // 32, 0), nl, 4), dtype=np.uint32)
     n = ctypes.c_int64(0)
-    _check(_lib.hlb_preprocess_records(_ptr(nbr), ns, _ptr(rec), ctypes.byref(n)))
+    _check(_lib.hlb_preprocess_records(_ptr(nbr), nl, ns, _ptr(rec), ctypes.byref(n)))
     return rec, n.value
 
 
@@ -195,6 +207,7 @@ class Geometry:
             p.stream = self.stream.cuda_stream
             _check(_lib.hlb_geometry_create(_ptr(st), ctypes.byref(p), ctypes.byref(self._h)))
         self.n_sites = int(_lib.hlb_num_sites(self._h))
+        self.n_q = int(_lib.hlb_num_q(self._h))
         self.flags = int(flags)
 
     # -- the C-ABI calls, same names -------------------------------------------------
@@ -227,13 +240,16 @@ class Geometry:
         return rho, u
 
     def hlb_get_populations(self):
-        f = np.empty((self.n_sites, 15), dtype=np.float64)
+        f = np.empty((self.n_sites, self.n_q), dtype=np.float64)
         _check(_lib.hlb_get_populations(self._h, _ptr(f)))
         return f
 
     def hlb_set_populations(self, f):
-        f = _host(f, np.float64, (self.n_sites, 15))
+        f = _host(f, np.float64, (self.n_sites, self.n_q))
         _check(_lib.hlb_set_populations(self._h, _ptr(f)))
+
+    def hlb_num_q(self) -> int:
+        return int(_lib.hlb_num_q(self._h))
 
     def hlb_num_sites(self) -> int:
         return int(_lib.hlb_num_sites(self._h))

@@ -11,7 +11,7 @@
 #include <vector>
 
 #include "../../include/hlb.h"
-#include "d3q15.h"
+#include "lattice.h"
 #include "kernels.cuh"
 #include "preprocess.h"
 
@@ -51,6 +51,7 @@ struct hlb_geometry {
   hlb_params p{};
   cudaStream_t stream = nullptr;
   bool aa = false, f32 = false;
+  int Q = 15;                         // populations per site (15 or 19)
   int64_t N = 0, Ns = 0;
   std::vector<int64_t> canon_voxels;  // [N] ascending
   std::vector<double> iolet_rho;
@@ -98,13 +99,16 @@ extern "C" {
 
 const char* hlb_last_error(void) { return g_err.c_str(); }
 
-void hlb_velocity_set(int32_t* c, double* w, int32_t* o) {
-  for (int q = 0; q < Q; ++q) {
-    if (c) { c[3 * q + 0] = cx(q); c[3 * q + 1] = cy(q); c[3 * q + 2] = cz(q); }
-    if (w) w[q] = weight(q);
+int hlb_lattice(uint32_t flags, int32_t* c, double* w, int32_t* o) {
+  const LatticeDesc& lat = lattice_desc((flags & HLB_LATTICE_D3Q19) != 0);
+  for (int q = 0; q < lat.Q; ++q) {
+    if (c) { c[3 * q + 0] = lat.c[q][0]; c[3 * q + 1] = lat.c[q][1]; c[3 * q + 2] = lat.c[q][2]; }
+    if (w) w[q] = lat.w[q];
     if (o) o[q] = opp(q);
   }
+  return lat.Q;
 }
+void hlb_velocity_set(int32_t* c, double* w, int32_t* o) { (void)hlb_lattice(0, c, w, o); }
 
 static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder& order) {
   if (!site_type || !p) return fail(HLB_EINVAL, "NULL argument");
@@ -113,7 +117,8 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->n_iolets > 0 && !p->iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
   if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
-                             HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH | HLB_INDEX64))
+                             HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH | HLB_INDEX64 |
+                             HLB_LATTICE_D3Q19))
     return fail(HLB_EINVAL, "unknown flag bits");
   if ((p->flags & HLB_LINKS_TABLE) && (p->flags & HLB_LINKS_RECORDS))
     return fail(HLB_EINVAL, "HLB_LINKS_TABLE and HLB_LINKS_RECORDS are exclusive");
@@ -130,7 +135,8 @@ int hlb_preprocess_count(const uint8_t* site_type, const hlb_params* p, int64_t*
   if (rc) return rc;
   GeometryTables t;
   std::string err;
-  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order, true, t, err);
+  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order,
+                  lattice_desc((p->flags & HLB_LATTICE_D3Q19) != 0), true, t, err);
   if (rc) return fail(rc, err);
   if (n_sites) *n_sites = t.N;
   if (stride) *stride = t.Ns;
@@ -144,7 +150,8 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
   if (rc) return rc;
   GeometryTables t;
   std::string err;
-  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order, false, t, err);
+  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order,
+                  lattice_desc((p->flags & HLB_LATTICE_D3Q19) != 0), false, t, err);
   if (rc) return fail(rc, err);
   if (voxel_of_site) std::memcpy(voxel_of_site, t.voxel_of_site.data(), sizeof(int64_t) * (size_t)t.N);
   if (canon_of_site) std::memcpy(canon_of_site, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N);
@@ -152,10 +159,12 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
   return HLB_OK;
 }
 
-int hlb_preprocess_records(const int32_t* nbr, int64_t stride, uint32_t* rec, int64_t* n_sentinel) {
+int hlb_preprocess_records(const int32_t* nbr, int32_t n_links, int64_t stride, uint32_t* rec,
+                           int64_t* n_sentinel) {
   if (!nbr || !rec) return fail(HLB_EINVAL, "NULL argument");
+  if (n_links != 14 && n_links != 18) return fail(HLB_EINVAL, "n_links must be 14 (D3Q15) or 18 (D3Q19)");
   if (stride <= 0 || stride % 32) return fail(HLB_EINVAL, "stride must be a positive multiple of 32");
-  const int64_t n = build_link_records(nbr, stride, rec);
+  const int64_t n = build_link_records(nbr, n_links, stride, rec);
   if (n_sentinel) *n_sentinel = n;
   return HLB_OK;
 }
@@ -175,7 +184,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   }
   GeometryTables t;
   std::string err;
-  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order, false, t, err);
+  rc = preprocess(site_type, p->nx, p->ny, p->nz, p->periodic, p->n_iolets, order,
+                  lattice_desc((p->flags & HLB_LATTICE_D3Q19) != 0), false, t, err);
   if (rc) return fail(rc, err);
 
   hlb_geometry* g = new hlb_geometry();
@@ -184,6 +194,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->stream = (cudaStream_t)p->stream;
   g->aa = (p->flags & HLB_AA) != 0;
   g->f32 = (p->flags & HLB_STORE_F32) != 0;
+  g->Q = (p->flags & HLB_LATTICE_D3Q19) ? 19 : 15;
+  const int Q = g->Q;
   g->N = t.N;
   g->Ns = t.Ns;
   g->iolet_rho.assign(p->iolet_rho, p->iolet_rho + p->n_iolets);
@@ -206,8 +218,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
       delete g;
       return HLB_ECUDA;
     }
-    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull() * 3 / 4 / 128 * 128;
-    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa() * 3 / 4 / 128 * 128;
+    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull(Q == 19) * 3 / 4 / 128 * 128;
+    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa(Q == 19) * 3 / 4 / 128 * 128;
     if (const char* e = std::getenv("HLB_PREFETCH_SITES")) {
       const long long v = std::atoll(e);
       g->dg.prefetch_pull = g->dg.prefetch_aa = v > 0 ? (v < (1ll << 24) ? v : (1ll << 24)) : 0;
@@ -251,6 +263,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.iolet_rho = (const double*)d_rho;
   g->dg.omega = 1.0 / p->tau;
   g->dg.f32 = g->f32;
+  g->dg.d3q19 = Q == 19;
   // the host tables die at the end of this call: finish the uploads first
   HLB_CUDA_G(cudaStreamSynchronize(g->stream));
   rc = hlb_set_state(g, nullptr, nullptr);
@@ -283,7 +296,7 @@ static int init_from(hlb_geometry* g, const double* d_rho, const double* d_u, co
 static int ensure_scratch_pop(hlb_geometry* g) {
   if (g->scratch_pop) return HLB_OK;
   void* ptr = nullptr;
-  const int rc = g->alloc(sizeof(double) * (size_t)Q * (size_t)g->N, &ptr);
+  const int rc = g->alloc(sizeof(double) * (size_t)g->Q * (size_t)g->N, &ptr);
   if (rc) return rc;
   g->scratch_pop = (double*)ptr;
   return HLB_OK;
@@ -308,7 +321,7 @@ int hlb_set_populations(hlb_geometry* g, const double* f) {
   if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
   int rc = ensure_scratch_pop(g);
   if (rc) return rc;
-  HLB_CUDA(cudaMemcpyAsync(g->scratch_pop, f, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyHostToDevice, g->stream));
+  HLB_CUDA(cudaMemcpyAsync(g->scratch_pop, f, sizeof(double) * (size_t)g->Q * (size_t)g->N, cudaMemcpyHostToDevice, g->stream));
   return init_from(g, nullptr, nullptr, g->scratch_pop);
 }
 
@@ -413,11 +426,12 @@ int hlb_get_populations(hlb_geometry* g, double* f) {
   if (rc) return rc;
   launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->scratch_pop, g->stream);
   HLB_CUDA(cudaGetLastError());
-  HLB_CUDA(cudaMemcpyAsync(f, g->scratch_pop, sizeof(double) * (size_t)Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaMemcpyAsync(f, g->scratch_pop, sizeof(double) * (size_t)g->Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));
   return HLB_OK;
 }
 
+int hlb_num_q(const hlb_geometry* g) { return g ? g->Q : (int)HLB_EINVAL; }
 int64_t hlb_num_sites(const hlb_geometry* g) { return g ? g->N : (int64_t)HLB_EINVAL; }
 int64_t hlb_steps_done(const hlb_geometry* g) { return g ? g->steps : (int64_t)HLB_EINVAL; }
 int64_t hlb_device_bytes(const hlb_geometry* g) { return g ? g->device_bytes : (int64_t)HLB_EINVAL; }

@@ -40,16 +40,29 @@ constexpr int BLOCK = 256;   // read-out / init kernels
 #define HLB_AA_ODD_MINB 6
 #endif
 constexpr int SBLOCK = HLB_STEP_BLOCK;
+// D3Q19 keeps 4 more populations (8 registers) and 4 more offsets alive: one block less.
+#ifndef HLB_Q19_MINB_DROP
+#define HLB_Q19_MINB_DROP 1
+#endif
+template <typename L, bool REC> constexpr int pull_minb() {
+  return HLB_PULL_MINB - (REC ? 0 : 1) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
+}
+template <typename L, bool REC> constexpr int aa_odd_minb() {
+  return HLB_AA_ODD_MINB - (REC ? 0 : 1) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
+}
+template <typename L> constexpr int aa_even_minb() {
+  return HLB_AA_EVEN_MINB - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
+}
 
 __device__ __forceinline__ int iolet_of(int32_t e) {  // -1: not an iolet link
   return e < 0 ? (int)(e & 0x7fffffff) - 1 : -1;
 }
 
-template <typename ST>
+template <typename L>
 __device__ __forceinline__ void load_entries(const int32_t* __restrict__ nbr, long long Ns,
-                                             long long i, int32_t (&e)[Q - 1]) {
+                                             long long i, int32_t (&e)[L::Q - 1]) {
 #pragma unroll
-  for (int q = 1; q < Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+  for (int q = 1; q < L::Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
 }
 
 // Flat element offsets (slot * Ns + site) of the 14 link populations of site i, for the step
@@ -62,17 +75,17 @@ __device__ __forceinline__ void load_entries(const int32_t* __restrict__ nbr, lo
 // (include/hlb.h, hlb_preprocess_records): entry = (lane >= second ? off1 : off0) + lane;
 // a sentinel record (warp-uniform) sends the warp to the table for that link. The iolet id
 // is NOT decoded here; the rare iolet path re-reads the table.
-template <int MODE, bool REC, typename IT>
+template <typename L, int MODE, bool REC, typename IT>
 __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
                                              const uint4* __restrict__ rec, long long Ns,
-                                             long long i, IT (&off)[Q - 1]) {
+                                             long long i, IT (&off)[L::Q - 1]) {
   const IT n = (IT)Ns, self = (IT)i;
   if (!REC) {
-    int32_t e[Q - 1];
+    int32_t e[L::Q - 1];
 #pragma unroll
-    for (int q = 1; q < Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
+    for (int q = 1; q < L::Q; ++q) e[q - 1] = __ldg(nbr + (long long)(q - 1) * Ns + i);
 #pragma unroll
-    for (int q = 1; q < Q; ++q) {
+    for (int q = 1; q < L::Q; ++q) {
       const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
       off[q - 1] = e[q - 1] < 0 ? (IT)qw * n + self : (IT)qf * n + (IT)e[q - 1];
     }
@@ -80,18 +93,18 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
   }
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t lane_bit = 1u << lane;
-  const uint4* r = rec + (i >> 5) * (Q - 1);
-  uint4 v[Q - 1];
+  const uint4* r = rec + (i >> 5) * (L::Q - 1);
+  uint4 v[L::Q - 1];
 #pragma unroll
-  for (int q = 1; q < Q; ++q) v[q - 1] = __ldg(r + (q - 1));
+  for (int q = 1; q < L::Q; ++q) v[q - 1] = __ldg(r + (q - 1));
   // second <= 32 in a real record, 0xffffffff in a sentinel: one warp-uniform test decides
   // whether this warp needs the table at all, so the common path carries no sentinel code
   uint32_t any = 0u;
 #pragma unroll
-  for (int q = 1; q < Q; ++q) any |= v[q - 1].y;
+  for (int q = 1; q < L::Q; ++q) any |= v[q - 1].y;
   if ((int32_t)any >= 0) {
 #pragma unroll
-    for (int q = 1; q < Q; ++q) {
+    for (int q = 1; q < L::Q; ++q) {
       const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
       const uint4 t = v[q - 1];
       const IT e = (IT)((lane >= t.y ? t.w : t.z) + lane);
@@ -99,7 +112,7 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
     }
   } else {
 #pragma unroll
-    for (int q = 1; q < Q; ++q) {
+    for (int q = 1; q < L::Q; ++q) {
       const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
       const uint4 t = v[q - 1];
       int32_t e;
@@ -132,16 +145,17 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 // equilibrium f_eq_p(rho_k, u(x, t)) (reading A6). The table entries are re-read here so
 // that the common path does not keep them in registers; fully unrolled so that out[] stays
 // in registers (no call, no stack).
+template <typename L>
 __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
                                                  long long i, const Moments& m,
                                                  const double* __restrict__ iolet_rho,
-                                                 double (&out)[Q]) {
+                                                 double (&out)[L::Q]) {
 #pragma unroll
-  for (int p = 1; p < Q; ++p) {
+  for (int p = 1; p < L::Q; ++p) {
     const int k = iolet_of(__ldg(nbr + (long long)(p - 1) * Ns + i));
     if (k >= 0) {
       const double rk = __ldg(iolet_rho + k);
-      out[p] = heq_of(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+      out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
     }
   }
 }
@@ -162,43 +176,43 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
 // pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
 // of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
 // padding, so only the one warp-uniform test is needed.
-template <typename ST, bool REC, typename IT>
-__global__ void __launch_bounds__(SBLOCK, REC ? HLB_PULL_MINB : HLB_PULL_MINB - 1)
+template <typename L, typename ST, bool REC, typename IT>
+__global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
        const double* __restrict__ iolet_rho, long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
-  double h[Q];
+  double h[L::Q];
   {
-    IT off[Q - 1];
-    link_offsets<GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
+    IT off[L::Q - 1];
+    link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
     h[0] = to_real(src[i]);
 #pragma unroll
-    for (int q = 1; q < Q; ++q) h[q] = to_real(src[off[q - 1]]);
+    for (int q = 1; q < L::Q; ++q) h[q] = to_real(src[off[q - 1]]);
     if (pf > 0 && i + pf < Ns) {
       const ST* ahead = src + pf;
       asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
-      if (REC && (threadIdx.x & 31) < 7)
-        prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31));
+      if (REC && (threadIdx.x & 31) < ((L::Q - 1) * 16 + 31) / 32)
+        prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (L::Q - 1)) + 32 * (threadIdx.x & 31));
       prefetch_l2(ahead + i);
 #pragma unroll
-      for (int q = 1; q < Q; ++q) prefetch_l2(ahead + off[q - 1]);
+      for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
     }
   }
-  const Moments m = moments_of(h);
-  collide(h, m, omega, h);
+  const Moments m = moments_of<L>(h);
+  collide<L>(h, m, omega, h);
   if (has_iolet_link(iolet_bits, i)) {  // rare: sites on an inlet/outlet cap
     // slot opp(p) of this site is read back by link p next step
-    double back[Q];
+    double back[L::Q];
 #pragma unroll
-    for (int p = 1; p < Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute(nbr, Ns, i, m, iolet_rho, back);
+    for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
+    iolet_substitute<L>(nbr, Ns, i, m, iolet_rho, back);
 #pragma unroll
-    for (int p = 1; p < Q; ++p) h[opp(p)] = back[p];
+    for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
   ST* d = dst + i;
 #pragma unroll
-  for (int q = 0; q < Q; ++q) d[(long long)q * Ns] = to_store<ST>(h[q]);
+  for (int q = 0; q < L::Q; ++q) d[(long long)q * Ns] = to_store<ST>(h[q]);
 }
 
 // ------------------------------------------------------------------ A-A in place
@@ -206,85 +220,85 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // Odd phase: read f_q from slot opp(q) of x - c_q (slot q of x at a wall), write h*_q to
 // the address f_opp(q) was read from. Read set = write set per site in both phases, so one
 // array and no inter-thread hazards.
-template <typename ST>
-__global__ void __launch_bounds__(SBLOCK, HLB_AA_EVEN_MINB)
+template <typename L, typename ST>
+__global__ void __launch_bounds__(SBLOCK, aa_even_minb<L>())
 k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
           const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
           long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   ST* p0 = a + i;
-  double h[Q];
+  double h[L::Q];
 #pragma unroll
-  for (int q = 0; q < Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
+  for (int q = 0; q < L::Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
   if (pf > 0 && i + pf < Ns) {
 #pragma unroll
-    for (int q = 0; q < Q; ++q) prefetch_l2(p0 + (long long)q * Ns + pf);
+    for (int q = 0; q < L::Q; ++q) prefetch_l2(p0 + (long long)q * Ns + pf);
   }
-  const Moments m = moments_of(h);
-  collide(h, m, omega, h);
-  double out[Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
+  const Moments m = moments_of<L>(h);
+  collide<L>(h, m, omega, h);
+  double out[L::Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
 #pragma unroll
-  for (int p = 0; p < Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute(nbr, Ns, i, m, iolet_rho, out);
+  for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_rho, out);
 #pragma unroll
-  for (int p = 0; p < Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
+  for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
 
-template <typename ST, bool REC, typename IT>
-__global__ void __launch_bounds__(SBLOCK, REC ? HLB_AA_ODD_MINB : HLB_AA_ODD_MINB - 1)
+template <typename L, typename ST, bool REC, typename IT>
+__global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
          long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
-  IT off[Q - 1];
-  link_offsets<GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
-  double h[Q];
+  IT off[L::Q - 1];
+  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
+  double h[L::Q];
   h[0] = to_real(a[i]);
 #pragma unroll
-  for (int q = 1; q < Q; ++q) h[q] = to_real(a[off[q - 1]]);
+  for (int q = 1; q < L::Q; ++q) h[q] = to_real(a[off[q - 1]]);
   if (pf > 0 && i + pf < Ns) {
     const ST* ahead = a + pf;
     asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
-    if (REC && (threadIdx.x & 31) < 7)
-      prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (Q - 1)) + 32 * (threadIdx.x & 31));
+    if (REC && (threadIdx.x & 31) < ((L::Q - 1) * 16 + 31) / 32)
+      prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (L::Q - 1)) + 32 * (threadIdx.x & 31));
     prefetch_l2(ahead + i);
 #pragma unroll
-    for (int q = 1; q < Q; ++q) prefetch_l2(ahead + off[q - 1]);
+    for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
   }
-  const Moments m = moments_of(h);
-  collide(h, m, omega, h);
-  double out[Q];
+  const Moments m = moments_of<L>(h);
+  collide<L>(h, m, omega, h);
+  double out[L::Q];
 #pragma unroll
-  for (int p = 0; p < Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute(nbr, Ns, i, m, iolet_rho, out);
+  for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_rho, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
-  for (int p = 1; p < Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
+  for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
 }
 
 // ------------------------------------------------------------------ read-out / init
-template <typename ST, int MODE>
+template <typename L, typename ST, int MODE>
 __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
                                                     const int32_t* __restrict__ nbr, long long Ns,
-                                                    long long i, double (&h)[Q]) {
-  int32_t e[Q - 1];
-  if (MODE != GATHER_OWN) load_entries<ST>(nbr, Ns, i, e);
+                                                    long long i, double (&h)[L::Q]) {
+  int32_t e[L::Q - 1];
+  if (MODE != GATHER_OWN) load_entries<L>(nbr, Ns, i, e);
   h[0] = to_real(buf[i]);
 #pragma unroll
-  for (int q = 1; q < Q; ++q)
+  for (int q = 1; q < L::Q; ++q)
     h[q] = to_real(buf[slot_of<MODE>(q, MODE != GATHER_OWN ? e[q - 1] : 0, Ns, i)]);
 }
 
-template <typename ST, int MODE>
+template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
               const int32_t* __restrict__ canon, long long N, long long Ns,
               double* __restrict__ rho, double* __restrict__ u) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
-  double h[Q];
-  gather_precollision<ST, MODE>(buf, nbr, Ns, i, h);
-  const Moments m = moments_of(h);
+  double h[L::Q];
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  const Moments m = moments_of<L>(h);
   const long long c = canon[i];
   if (rho) rho[c] = m.rho;
   if (u) {
@@ -294,38 +308,39 @@ k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
   }
 }
 
-template <typename ST, int MODE>
+template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
                   const int32_t* __restrict__ canon, long long N, long long Ns,
                   double* __restrict__ f) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
-  double h[Q];
-  gather_precollision<ST, MODE>(buf, nbr, Ns, i, h);
+  double h[L::Q];
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
   const long long c = canon[i];
 #pragma unroll
-  for (int q = 0; q < Q; ++q) f[c * Q + q] = h[q] + weight(q);
+  for (int q = 0; q < L::Q; ++q) f[c * L::Q + q] = h[q] + L::weight(q);
 }
 
 // shifted initial population of direction q at internal site `site`
+template <typename L>
 __device__ __forceinline__ double initial_h(int q, long long site, const int32_t* __restrict__ canon,
                                             const double* __restrict__ rho_in,
                                             const double* __restrict__ u_in,
                                             const double* __restrict__ f_in) {
   const long long c = canon[site];
-  if (f_in) return f_in[c * Q + q] - weight(q);
+  if (f_in) return f_in[c * L::Q + q] - L::weight(q);
   const double r = rho_in ? rho_in[c] : 1.0;
   const double ux = u_in ? u_in[3 * c + 0] : 0.0, uy = u_in ? u_in[3 * c + 1] : 0.0,
                uz = u_in ? u_in[3 * c + 2] : 0.0;
-  return heq_of(q, r - 1.0, r, ux, uy, uz);
+  return heq_of<L>(q, r - 1.0, r, ux, uy, uz);
 }
 
 // MODE GATHER_OWN: buf[q][x] = h_q(x). MODE GATHER_PULL: slot (p, y) is read either by the
 // fluid site y + c_p as its direction p, or (wall / iolet link) by y itself as direction
 // opp(p); store the reader's initial population there, so that the first gather yields
 // exactly f(., 0) = f_eq(rho0, u0) at every site and link.
-template <typename ST, int MODE>
+template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_init(ST* __restrict__ buf, const int32_t* __restrict__ nbr, const int32_t* __restrict__ canon,
        long long N, long long Ns, const double* __restrict__ rho_in,
@@ -334,19 +349,19 @@ k_init(ST* __restrict__ buf, const int32_t* __restrict__ nbr, const int32_t* __r
   if (i >= Ns) return;
   if (i >= N) {
 #pragma unroll
-    for (int q = 0; q < Q; ++q) buf[(long long)q * Ns + i] = to_store<ST>(0.0);
+    for (int q = 0; q < L::Q; ++q) buf[(long long)q * Ns + i] = to_store<ST>(0.0);
     return;
   }
-  buf[i] = to_store<ST>(initial_h(0, i, canon, rho_in, u_in, f_in));
+  buf[i] = to_store<ST>(initial_h<L>(0, i, canon, rho_in, u_in, f_in));
 #pragma unroll
-  for (int p = 1; p < Q; ++p) {
+  for (int p = 1; p < L::Q; ++p) {
     double v;
     if (MODE == GATHER_OWN) {
-      v = initial_h(p, i, canon, rho_in, u_in, f_in);
+      v = initial_h<L>(p, i, canon, rho_in, u_in, f_in);
     } else {
       const int32_t e = __ldg(nbr + (long long)(opp(p) - 1) * Ns + i);  // pull source of opp(p) = y + c_p
-      v = e >= 0 ? initial_h(p, e, canon, rho_in, u_in, f_in)
-                 : initial_h(opp(p), i, canon, rho_in, u_in, f_in);
+      v = e >= 0 ? initial_h<L>(p, e, canon, rho_in, u_in, f_in)
+                 : initial_h<L>(opp(p), i, canon, rho_in, u_in, f_in);
     }
     buf[(long long)p * Ns + i] = to_store<ST>(v);
   }
@@ -356,102 +371,111 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + BLOCK - 1) / BLOC
 
 }  // namespace
 
-int resident_sites_per_sm_pull() { return SBLOCK * HLB_PULL_MINB; }
-int resident_sites_per_sm_aa() { return SBLOCK * HLB_AA_ODD_MINB; }
+int resident_sites_per_sm_pull(bool d3q19) {
+  return SBLOCK * (d3q19 ? pull_minb<D3Q19, true>() : pull_minb<D3Q15, true>());
+}
+int resident_sites_per_sm_aa(bool d3q19) {
+  return SBLOCK * (d3q19 ? aa_odd_minb<D3Q19, true>() : aa_odd_minb<D3Q15, true>());
+}
 
-template <typename ST, bool REC, typename IT>
+// ------------------------------------------------------------------ launchers
+template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  k_pull<ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
+  k_pull<L, ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
       (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_rho, g.Ns,
       g.omega, g.prefetch_pull);
 }
-template <typename ST>
+template <typename L, typename ST>
 static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (g.use_rec) {
-    if (idx32) pull_launch<ST, true, uint32_t>(g, src, dst, s);
-    else pull_launch<ST, true, long long>(g, src, dst, s);
+    if (idx32) pull_launch<L, ST, true, uint32_t>(g, src, dst, s);
+    else pull_launch<L, ST, true, long long>(g, src, dst, s);
   } else {
-    if (idx32) pull_launch<ST, false, uint32_t>(g, src, dst, s);
-    else pull_launch<ST, false, long long>(g, src, dst, s);
+    if (idx32) pull_launch<L, ST, false, uint32_t>(g, src, dst, s);
+    else pull_launch<L, ST, false, long long>(g, src, dst, s);
   }
 }
-void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  if (g.f32) pull_t<float>(g, src, dst, s);
-  else pull_t<double>(g, src, dst, s);
-}
-
-template <typename ST, bool REC, typename IT>
+template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
-  k_aa_odd<ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
+  k_aa_odd<L, ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
       (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
 }
-template <typename ST>
+template <typename L, typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (!odd) {
-    k_aa_even<ST><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>((ST*)a, g.nbr, g.iolet_bits,
-                                                               g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
+    k_aa_even<L, ST><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
+        (ST*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
   } else if (g.use_rec) {
-    if (idx32) aa_odd_launch<ST, true, uint32_t>(g, a, s);
-    else aa_odd_launch<ST, true, long long>(g, a, s);
+    if (idx32) aa_odd_launch<L, ST, true, uint32_t>(g, a, s);
+    else aa_odd_launch<L, ST, true, long long>(g, a, s);
   } else {
-    if (idx32) aa_odd_launch<ST, false, uint32_t>(g, a, s);
-    else aa_odd_launch<ST, false, long long>(g, a, s);
+    if (idx32) aa_odd_launch<L, ST, false, uint32_t>(g, a, s);
+    else aa_odd_launch<L, ST, false, long long>(g, a, s);
   }
 }
-void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
-  if (g.f32) aa_t<float>(g, a, odd, s);
-  else aa_t<double>(g, a, odd, s);
-}
-
-template <typename ST>
+template <typename L, typename ST>
 static void macroscopic_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
                           double* u, cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_macroscopic<ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
-    case GATHER_OWN: k_macroscopic<ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
-    case GATHER_AA_ODD: k_macroscopic<ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_PULL: k_macroscopic<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_AA_ODD: k_macroscopic<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
   }
 }
-void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
-                        double* u, cudaStream_t s) {
-  if (g.f32) macroscopic_t<float>(g, buf, mode, rho, u, s);
-  else macroscopic_t<double>(g, buf, mode, rho, u, s);
-}
-
-template <typename ST>
+template <typename L, typename ST>
 static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
                               cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_get_populations<ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
-    case GATHER_OWN: k_get_populations<ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
-    case GATHER_AA_ODD: k_get_populations<ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_PULL: k_get_populations<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_AA_ODD: k_get_populations<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
   }
 }
-void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
-                            cudaStream_t s) {
-  if (g.f32) get_populations_t<float>(g, buf, mode, f, s);
-  else get_populations_t<double>(g, buf, mode, f, s);
-}
-
-template <typename ST>
+template <typename L, typename ST>
 static void init_t(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
                    const double* u_in, const double* f_in, cudaStream_t s) {
   const unsigned grid = grid_for(g.Ns);
   if (mode == GATHER_PULL)
-    k_init<ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>((ST*)buf, g.nbr, g.canon, g.N, g.Ns, rho_in, u_in, f_in);
+    k_init<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>((ST*)buf, g.nbr, g.canon, g.N, g.Ns, rho_in, u_in, f_in);
   else
-    k_init<ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>((ST*)buf, g.nbr, g.canon, g.N, g.Ns, rho_in, u_in, f_in);
+    k_init<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>((ST*)buf, g.nbr, g.canon, g.N, g.Ns, rho_in, u_in, f_in);
+}
+
+// lattice x storage dispatch: F is a generic lambda called with (L{}, ST{})
+template <typename F>
+static void dispatch(const DeviceGeometry& g, F&& f) {
+  if (g.d3q19) {
+    if (g.f32) f(D3Q19{}, float{});
+    else f(D3Q19{}, double{});
+  } else {
+    if (g.f32) f(D3Q15{}, float{});
+    else f(D3Q15{}, double{});
+  }
+}
+
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { pull_t<decltype(l), decltype(st)>(g, src, dst, s); });
+}
+void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { aa_t<decltype(l), decltype(st)>(g, a, odd, s); });
+}
+void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
+                        double* u, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { macroscopic_t<decltype(l), decltype(st)>(g, buf, mode, rho, u, s); });
+}
+void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
+                            cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { get_populations_t<decltype(l), decltype(st)>(g, buf, mode, f, s); });
 }
 void launch_init(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
                  const double* u_in, const double* f_in, cudaStream_t s) {
-  if (g.f32) init_t<float>(g, buf, mode, rho_in, u_in, f_in, s);
-  else init_t<double>(g, buf, mode, rho_in, u_in, f_in, s);
+  dispatch(g, [&](auto l, auto st) { init_t<decltype(l), decltype(st)>(g, buf, mode, rho_in, u_in, f_in, s); });
 }
 
 }  // namespace hlb

@@ -8,10 +8,10 @@ namespace hlb {
 
 struct DeviceGeometry {
   int64_t N = 0;                        // fluid sites
-  int64_t Ns = 0;                       // plane stride (multiple of 128), arrays are [15][Ns]
-  const int32_t* nbr = nullptr;         // [14][Ns] pull-neighbour table (include/hlb.h)
+  int64_t Ns = 0;                       // plane stride (multiple of 128), arrays are [Q][Ns]
+  const int32_t* nbr = nullptr;         // [Q-1][Ns] pull-neighbour table (include/hlb.h)
   const uint32_t* iolet_bits = nullptr; // [Ns/32]
-  const void* rec = nullptr;            // [Ns/32][14] 16-byte link records (include/hlb.h)
+  const void* rec = nullptr;            // [Ns/32][Q-1] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
   bool index64 = false;                 // flat offsets need (or are forced to) 64 bits
   // > 0: every thread L2-prefetches what site i + prefetch_* will load (about 3/4 of the
@@ -21,11 +21,12 @@ struct DeviceGeometry {
   const double* iolet_rho = nullptr;    // [n_iolets]
   double omega = 1.0;                   // 1 / tau
   bool f32 = false;                     // HLB_STORE_F32
+  bool d3q19 = false;                   // HLB_LATTICE_D3Q19 (else D3Q15)
 };
 
 // Sites resident on an SM at once (threads per block x resident blocks) per step kernel.
-int resident_sites_per_sm_pull();
-int resident_sites_per_sm_aa();
+int resident_sites_per_sm_pull(bool d3q19);
+int resident_sites_per_sm_aa(bool d3q19);
 
 // One time step, two-lattice pull: dst <- collide(gather(src)).
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);
@@ -41,7 +42,7 @@ enum GatherMode {
 // rho [N] / u [N][3] (device, canonical order; either may be NULL)
 void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
                         double* u, cudaStream_t s);
-// f [N][15] raw populations (device, canonical order)
+// f [N][Q] raw populations (device, canonical order)
 void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
                             cudaStream_t s);
 // Initialise a buffer so that gathering in `mode` (GATHER_PULL or GATHER_OWN) yields

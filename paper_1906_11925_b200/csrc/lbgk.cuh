@@ -1,4 +1,4 @@
-// lbgk.cuh -- per-site D3Q15 LBGK arithmetic (device), shared by every kernel variant so
+// lbgk.cuh -- per-site LBGK arithmetic (device), for either lattice of lattice.h, shared by every kernel variant so
 // that the two-lattice and A-A schemes, fp64 and fp32 storage, are bitwise identical in
 // their arithmetic (SURVEY.md §8(c) pin P14).
 //
@@ -9,7 +9,7 @@
 // ("collision"; LBGK and the equilibrium: BASELINE.json north_star and
 // the paper gives no formula).
 #pragma once
-#include "d3q15.h"
+#include "lattice.h"
 
 namespace hlb {
 
@@ -28,10 +28,11 @@ __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, 
 __device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
 
 // c_q . u with the +-1 / 0 components folded at compile time (exact: only additions)
+template <typename L>
 __device__ __forceinline__ double c_dot_u(int q, double ux, double uy, double uz) {
   double r = 0.0;
   bool first = true;
-  const int c[3] = {cx(q), cy(q), cz(q)};
+  const int c[3] = {L::cx(q), L::cy(q), L::cz(q)};
   const double u[3] = {ux, uy, uz};
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
@@ -43,25 +44,46 @@ __device__ __forceinline__ double c_dot_u(int q, double ux, double uy, double uz
   return r;
 }
 
-// Opposite pairs (2k-1, 2k), k = 1..7, first member has c = (1,0,0) (0,1,0) (0,0,1)
-// (1,1,1) (1,1,-1) (1,-1,1) (1,-1,-1): sums and differences of pairs give all moments.
-__device__ __forceinline__ Moments moments_of(const double (&h)[Q]) {
-  const double d1 = sub(h[1], h[2]), d2 = sub(h[3], h[4]), d3 = sub(h[5], h[6]);
-  const double d4 = sub(h[7], h[8]), d5 = sub(h[9], h[10]), d6 = sub(h[11], h[12]),
-               d7 = sub(h[13], h[14]);
-  const double s_axis = add(add(add(h[1], h[2]), add(h[3], h[4])), add(h[5], h[6]));
-  const double s_diag = add(add(add(h[7], h[8]), add(h[9], h[10])),
-                            add(add(h[11], h[12]), add(h[13], h[14])));
+// Moments from the opposite pairs (a, b) = (2k-1, 2k), c_b = -c_a: with s_k = h_a + h_b and
+// d_k = h_a - h_b,  drho = h_0 + sum_k s_k  and  j = sum_k c_a d_k.
+template <typename L>
+__device__ __forceinline__ Moments moments_of(const double (&h)[L::Q]) {
+  constexpr int P = (L::Q - 1) / 2;
+  double s[P], d[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    s[k] = add(h[2 * k + 1], h[2 * k + 2]);
+    d[k] = sub(h[2 * k + 1], h[2 * k + 2]);
+  }
+  // axis pairs first, then the diagonals, each summed pairwise
+  double s_axis = add(add(s[0], s[1]), s[2]);
+  double s_diag = add(s[3], s[4]);
+#pragma unroll
+  for (int k = 5; k + 1 < P; k += 2) s_diag = add(s_diag, add(s[k], s[k + 1]));
+  if ((P - 5) % 2) s_diag = add(s_diag, s[P - 1]);
   Moments m;
   m.drho = add(h[0], add(s_axis, s_diag));
   m.rho = add(1.0, m.drho);
-  const double jx = add(d1, add(add(d4, d5), add(d6, d7)));
-  const double jy = add(d2, sub(add(d4, d5), add(d6, d7)));
-  const double jz = add(d3, add(sub(d4, d5), sub(d6, d7)));
+  double j[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    double acc = 0.0;
+    bool first = true;
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+      const int q = 2 * k + 1;
+      const int c = a == 0 ? L::cx(q) : (a == 1 ? L::cy(q) : L::cz(q));
+      if (c == 0) continue;
+      const double t = c > 0 ? d[k] : -d[k];
+      acc = first ? t : add(acc, t);
+      first = false;
+    }
+    j[a] = acc;
+  }
   const double inv = __drcp_rn(m.rho);
-  m.ux = mul(jx, inv);
-  m.uy = mul(jy, inv);
-  m.uz = mul(jz, inv);
+  m.ux = mul(j[0], inv);
+  m.uy = mul(j[1], inv);
+  m.uz = mul(j[2], inv);
   return m;
 }
 
@@ -71,29 +93,32 @@ __device__ __forceinline__ double u_dot_u(double ux, double uy, double uz) {
 
 // Shifted equilibrium of direction q (compile-time q after unrolling) for density
 // 1 + drho and velocity (ux, uy, uz): w_q [drho + rho (3 c.u + 4.5 (c.u)^2 - 1.5 u.u)].
+template <typename L>
 __device__ __forceinline__ double heq_of(int q, double drho, double rho, double ux, double uy,
                                          double uz) {
-  const double cu = c_dot_u(q, ux, uy, uz);
+  const double cu = c_dot_u<L>(q, ux, uy, uz);
   const double uu15 = mul(1.5, u_dot_u(ux, uy, uz));
   const double poly = add(mul(3.0, cu), fma_(mul(4.5, cu), cu, -uu15));
-  return mul(weight(q), fma_(rho, poly, drho));
+  return mul(L::weight(q), fma_(rho, poly, drho));
 }
 
 // hs_q = h_q + omega (heq_q(m) - h_q), evaluated per opposite pair (a, b = opp(a)), c = c_a:
 //   heq_a = S + A, heq_b = S - A,  S = w (drho + rho (4.5 (c.u)^2 - 1.5 u.u)),  A = 3 w rho (c.u)
 // -- the same equilibrium as heq_of(), with the part even in c computed once per pair (a
 // third fewer fp64 operations; the kernels run into the 1 kW power cap otherwise).
-__device__ __forceinline__ void collide(const double (&h)[Q], const Moments& m, double omega,
-                                        double (&hs)[Q]) {
+template <typename L>
+__device__ __forceinline__ void collide(const double (&h)[L::Q], const Moments& m, double omega,
+                                        double (&hs)[L::Q]) {
   const double uu15 = mul(1.5, u_dot_u(m.ux, m.uy, m.uz));
-  const double heq0 = mul(weight(0), fma_(-m.rho, uu15, m.drho));
+  const double heq0 = mul(L::weight(0), fma_(-m.rho, uu15, m.drho));
   hs[0] = fma_(omega, sub(heq0, h[0]), h[0]);
-  const double r3_axis = mul(3.0 * weight(1), m.rho), r3_diag = mul(3.0 * weight(7), m.rho);
+  // two weight classes: axis (q = 1..6) and diagonal (q >= 7)
+  const double r3_axis = mul(3.0 * L::weight(1), m.rho), r3_diag = mul(3.0 * L::weight(7), m.rho);
 #pragma unroll
-  for (int a = 1; a < Q; a += 2) {
+  for (int a = 1; a < L::Q; a += 2) {
     const int b = a + 1;  // opp(a)
-    const double cu = c_dot_u(a, m.ux, m.uy, m.uz);
-    const double S = mul(weight(a), fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
+    const double cu = c_dot_u<L>(a, m.ux, m.uy, m.uz);
+    const double S = mul(L::weight(a), fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
     const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
     const double ha = h[a], hb = h[b];
     hs[a] = fma_(omega, sub(add(S, A), ha), ha);

@@ -22,7 +22,7 @@
 #include <thread>
 
 #include "../../include/hlb.h"
-#include "d3q15.h"
+#include "lattice.h"
 
 namespace hlb {
 namespace {
@@ -107,7 +107,8 @@ int preprocess_threads() { return thread_count(); }
 // source is a fluid site split into runs of lanes with consecutive source indices; with an
 // x-fastest site order almost every (group, q) has one or two runs, and 16 bytes then
 // replace the 128 bytes of table entries the warp would load.
-int64_t build_link_records(const int32_t* nbr, int64_t Ns, uint32_t* rec) {
+int64_t build_link_records(const int32_t* nbr, int n_links, int64_t Ns, uint32_t* rec) {
+  const int Q = n_links + 1;
   const int64_t G = Ns / 32;
   std::atomic<int64_t> fallback{0};
   parallel_for(G, 1 << 10, [&](int64_t gb, int64_t ge) {
@@ -142,7 +143,9 @@ int64_t build_link_records(const int32_t* nbr, int64_t Ns, uint32_t* rec) {
 }
 
 int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, int n_iolets,
-               SiteOrder order, bool count_only, GeometryTables& out, std::string& err) {
+               SiteOrder order, const LatticeDesc& lat, bool count_only, GeometryTables& out,
+               std::string& err) {
+  const int Q = lat.Q;
   if (!type) { err = "site_type is NULL"; return HLB_EINVAL; }
   if (nx <= 0 || ny <= 0 || nz <= 0) { err = "non-positive box extent"; return HLB_EINVAL; }
   if (n_iolets < 0 || n_iolets > 253) { err = "n_iolets must be in 0..253"; return HLB_EINVAL; }
@@ -307,7 +310,7 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
 
   // ---- pass D: pull-neighbour table
   const int64_t Ns = out.Ns;
-  out.nbr.assign((size_t)(14 * Ns), (int32_t)NBR_WALL_BIT);
+  out.nbr.assign((size_t)(Q - 1) * (size_t)Ns, (int32_t)NBR_WALL_BIT);
   out.iolet_bits.assign((size_t)(Ns / 32), 0u);
   std::atomic<int64_t> n_io_sites{0}, n_wall_links{0};
   const bool px = periodic & 1u, py = periodic & 2u, pz = periodic & 4u;
@@ -318,7 +321,7 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
       const int x = (int)(v % nx), y = (int)((v / nx) % ny), z = (int)(v / ((int64_t)nx * ny));
       bool has_io = false;
       for (int q = 1; q < Q; ++q) {
-        int sx = x - cx(q), sy = y - cy(q), sz = z - cz(q);
+        int sx = x - lat.c[q][0], sy = y - lat.c[q][1], sz = z - lat.c[q][2];
         bool outside = false;
         if (sx < 0) { if (px) sx += nx; else outside = true; }
         else if (sx >= nx) { if (px) sx -= nx; else outside = true; }
@@ -353,7 +356,7 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
 
   // ---- pass E: run-length link records
   out.rec.assign((size_t)(Ns / 32) * (Q - 1) * 4, 0u);
-  out.n_rec_fallback = build_link_records(out.nbr.data(), Ns, out.rec.data());
+  out.n_rec_fallback = build_link_records(out.nbr.data(), Q - 1, Ns, out.rec.data());
   return HLB_OK;
 }
 

@@ -5,6 +5,8 @@
 #include <string>
 #include <vector>
 
+#include "lattice.h"
+
 namespace hlb {
 
 enum SiteOrder { ORDER_MORTON = 0, ORDER_RASTER = 1, ORDER_TILED = 2 };
@@ -14,9 +16,9 @@ struct GeometryTables {
   int64_t Ns = 0;   // plane stride of every [slot][site] array: N rounded up to 128
   std::vector<int64_t> voxel_of_site;  // [N]  internal order -> linear voxel index
   std::vector<int32_t> canon_of_site;  // [N]  internal order -> canonical rank
-  std::vector<int32_t> nbr;            // [14][Ns], encoding: include/hlb.h
+  std::vector<int32_t> nbr;            // [Q-1][Ns], encoding: include/hlb.h
   std::vector<uint32_t> iolet_bits;    // [Ns/32] bit (i & 31) of word i >> 5: site i has an iolet link
-  std::vector<uint32_t> rec;           // [Ns/32][14][4] run-length link records (include/hlb.h)
+  std::vector<uint32_t> rec;           // [Ns/32][Q-1][4] run-length link records (include/hlb.h)
   int64_t n_rec_fallback = 0;          // (group, q) pairs with more than 2 runs (record = sentinel)
   int64_t n_iolet_sites = 0;
   int64_t n_wall_links = 0;
@@ -25,11 +27,12 @@ struct GeometryTables {
 // Returns 0 or a negative hlb_status; `err` gets the message. With count_only the tables
 // are left empty and only N / Ns are set.
 int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, int n_iolets,
-               SiteOrder order, bool count_only, GeometryTables& out, std::string& err);
+               SiteOrder order, const LatticeDesc& lat, bool count_only, GeometryTables& out,
+               std::string& err);
 
-// Run-length link records of a finished table: rec [Ns/32][14][4] (encoding: include/hlb.h,
+// Run-length link records of a finished table: rec [Ns/32][Q-1][4] (encoding: include/hlb.h,
 // hlb_preprocess_records). Returns the number of (group, q) pairs that got the sentinel.
-int64_t build_link_records(const int32_t* nbr, int64_t Ns, uint32_t* rec);
+int64_t build_link_records(const int32_t* nbr, int n_links, int64_t Ns, uint32_t* rec);
 
 int preprocess_threads();
 

@@ -24,5 +24,10 @@ BYTES_PER_SITE = {
 }
 
 
-def algorithmic_bytes_per_site(scheme: str, store: str) -> float:
-    return BYTES_PER_SITE[(scheme, store)]
+def algorithmic_bytes_per_site(scheme: str, store: str, n_q: int = 15) -> float:
+    """Q populations read + Q written + (Q - 1) int32 table entries (A-A: on odd steps only)."""
+    if n_q == 15:
+        return BYTES_PER_SITE[(scheme, store)]
+    pop = 8.0 if store == "f64" else 4.0
+    table = 4.0 * (n_q - 1)
+    return 2.0 * n_q * pop + (table if scheme == "two_lattice" else table / 2.0)

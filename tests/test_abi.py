@@ -78,3 +78,6 @@ def test_bytes_per_site_model():
     assert hlb.algorithmic_bytes_per_site("aa", "f64") == 15 * 8 * 2 + 14 * 4 / 2
     assert hlb.algorithmic_bytes_per_site("two_lattice", "f32") == 15 * 4 * 2 + 14 * 4
     assert hlb.algorithmic_bytes_per_site("aa", "f32") == 15 * 4 * 2 + 14 * 4 / 2
+    assert hlb.algorithmic_bytes_per_site("two_lattice", "f64", 19) == 19 * 8 * 2 + 18 * 4   # 376
+    assert hlb.algorithmic_bytes_per_site("aa", "f64", 19) == 19 * 8 * 2 + 18 * 4 / 2
+    assert hlb.algorithmic_bytes_per_site("two_lattice", "f32", 19) == 19 * 4 * 2 + 18 * 4

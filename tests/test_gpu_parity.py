@@ -26,12 +26,13 @@ def hlb():
     return m
 
 
-def flags_of(hlb, scheme, store, order="morton", links="auto"):
+def flags_of(hlb, scheme, store, order="morton", links="auto", lattice="d3q15"):
     f = hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE
     f |= hlb.HLB_STORE_F32 if store == "f32" else hlb.HLB_STORE_F64
     f |= {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
           "tiled": hlb.HLB_ORDER_TILED}[order]
     f |= {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE, "records": hlb.HLB_LINKS_RECORDS}[links]
+    f |= {"d3q15": hlb.HLB_LATTICE_D3Q15, "d3q19": hlb.HLB_LATTICE_D3Q19}[lattice]
     return f
 
 
@@ -42,9 +43,10 @@ def errors(rho, u, rho_ref, u_ref):
     return e_rho, e_u
 
 
-def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto"):
+def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto", lattice="d3q15", extra=0):
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
-                                flags_of(hlb, scheme, store, order, links))
+                                flags_of(hlb, scheme, store, order, links, lattice) | extra)
+    assert g.hlb_num_q() == {"d3q15": 15, "d3q19": 19}[lattice]
     if links != "auto":
         assert g.hlb_uses_records() == (links == "records")
     if wl.rho0 is not None or wl.u0 is not None:
@@ -56,17 +58,17 @@ def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto"):
     return out
 
 
-def run_oracle(wl, steps, threads=0):
-    return oracle.run(wl, steps=steps, threads=threads)
+def run_oracle(wl, steps, threads=0, lattice="d3q15"):
+    return oracle.run(wl, steps=steps, threads=threads, lattice=lattice)
 
 
 _oracle_cache = {}
 
 
-def oracle_cached(name, steps):
-    key = (name, steps)
+def oracle_cached(name, steps, lattice="d3q15"):
+    key = (name, steps, lattice)
     if key not in _oracle_cache:
-        _oracle_cache[key] = run_oracle(W.by_name(name, small=True), steps)
+        _oracle_cache[key] = run_oracle(W.by_name(name, small=True), steps, lattice=lattice)
     return _oracle_cache[key]
 
 
@@ -127,6 +129,89 @@ def test_aa_equals_two_lattice_bitwise(hlb, store):
         a = run_gpu(hlb, wl, steps, "two_lattice", store)
         b = run_gpu(hlb, wl, steps, "aa", store)
         assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+# ------------------------------------------------------------- D3Q19
+@pytest.mark.parametrize("store", ["f64", "f32"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+@pytest.mark.parametrize("name", W.CONFIG_NAMES)
+def test_d3q19_small_configs_match_oracle(hlb, name, scheme, store):
+    """The lattice the paper names: same five geometries, same
+    tolerances, table links at an even and record links at an odd step count."""
+    wl = W.by_name(name, small=True)
+    for steps, order, links in ((wl.steps, "morton", "table"), (wl.steps + 1, "raster", "records")):
+        rho_ref, u_ref = oracle_cached(name, steps, "d3q19")
+        rho, u = run_gpu(hlb, wl, steps, scheme, store, order, links, "d3q19")
+        e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+        assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
+
+
+def test_d3q19_differs_from_d3q15(hlb):
+    """Guard against a lattice flag that is silently ignored."""
+    wl = W.by_name("aneurysm", small=True)
+    a = run_gpu(hlb, wl, 30, "two_lattice", "f64", "raster", "auto", "d3q15")
+    b = run_gpu(hlb, wl, 30, "two_lattice", "f64", "raster", "auto", "d3q19")
+    assert np.max(np.abs(a[1] - b[1])) > 1e-8
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_d3q19_variants_agree_bitwise(hlb, scheme):
+    """D3Q19: records = table, every site order, 64-bit offsets, no prefetch, no graph, and
+    A-A = two-lattice -- all bitwise."""
+    wl = W.by_name("tree", small=True)
+    steps = 35
+    ref = run_gpu(hlb, wl, steps, scheme, "f64", "raster", "table", "d3q19")
+    for order, links, extra in (("raster", "records", 0), ("morton", "records", 0),
+                                ("tiled", "table", 0), ("raster", "records", hlb.HLB_INDEX64),
+                                ("raster", "records", hlb.HLB_NO_PREFETCH | hlb.HLB_NO_GRAPH)):
+        got = run_gpu(hlb, wl, steps, scheme, "f64", order, links, "d3q19", extra)
+        assert np.array_equal(ref[0], got[0]) and np.array_equal(ref[1], got[1]), (order, links, extra)
+    other = run_gpu(hlb, wl, steps, "aa" if scheme == "two_lattice" else "two_lattice", "f64",
+                    "raster", "records", "d3q19")
+    assert np.array_equal(ref[0], other[0]) and np.array_equal(ref[1], other[1])
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+@pytest.mark.parametrize("seed,periodic,shape", [
+    (0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (33, 5, 4)), (5, 7, (1, 1, 3)), (7, 0, (24, 20, 18)),
+    (8, 5, (40, 9, 23)),
+])
+def test_d3q19_random_masks_match_oracle(hlb, scheme, seed, periodic, shape):
+    wl = W.random_mask(shape, p_fluid=0.6, n_iolets=3, p_iolet=0.06, periodic=periodic,
+                       tau=0.55 + 0.07 * seed, seed=300 + seed)
+    links, order = ("records", "raster") if seed % 2 else ("table", "morton")
+    for steps in (0, 1, 2, 9, 10):
+        rho_ref, u_ref = run_oracle(wl, steps, threads=1, lattice="d3q19")
+        rho, u = run_gpu(hlb, wl, steps, scheme, "f64", order, links, "d3q19")
+        e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+        assert e_rho < 1e-13 and e_u < 1e-12, (steps, e_rho, e_u)
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_d3q19_populations_match_oracle(hlb, scheme):
+    wl = W.random_mask((12, 11, 10), p_fluid=0.65, n_iolets=2, periodic=1, tau=0.7, seed=78)
+    c_o = oracle.velocity_set("d3q19")[0]
+    c_g = hlb.hlb_lattice(hlb.HLB_LATTICE_D3Q19)[0]
+    perm = [int(np.flatnonzero((c_g == c).all(axis=1))[0]) for c in c_o]     # oracle q -> library q
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, lattice="d3q19")
+    o.set_state(wl.rho0, wl.u0)
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, scheme, "f64", "raster", "auto", "d3q19"))
+    g.hlb_set_state(wl.rho0, wl.u0)
+    for steps in (0, 1, 4, 3):
+        o.step(steps)
+        g.hlb_step(steps)
+        fo, fg = o.get_populations(), g.hlb_get_populations()
+        assert fg.shape == fo.shape == (wl.n_sites, 19)
+        assert np.max(np.abs(fg[:, perm] - fo)) < 1e-15
+    fo = o.get_populations()
+    fg = np.empty_like(fo)
+    fg[:, perm] = fo
+    g.hlb_set_populations(fg)
+    o.step(5)
+    g.hlb_step(5)
+    assert np.max(np.abs(g.hlb_get_populations()[:, perm] - o.get_populations())) < 1e-15
+    g.close()
 
 
 # ------------------------------------------------------------- random masks, every BC at once

@@ -17,14 +17,18 @@ def morton_key(x, y, z):
     return k
 
 
-def brute_table(st, periodic, vox_of_site):
+LATTICES = {"d3q15": hlb.HLB_LATTICE_D3Q15, "d3q19": hlb.HLB_LATTICE_D3Q19}
+
+
+def brute_table(st, periodic, vox_of_site, C=C):
     nz, ny, nx = st.shape
+    nq = len(C)
     site_of_vox = {int(v): i for i, v in enumerate(vox_of_site)}
     n = len(vox_of_site)
-    out = np.zeros((14, n), dtype=np.int64)
+    out = np.zeros((nq - 1, n), dtype=np.int64)
     for i, v in enumerate(vox_of_site):
         x, y, z = int(v % nx), int((v // nx) % ny), int(v // (nx * ny))
-        for q in range(1, 15):
+        for q in range(1, nq):
             s = [x - int(C[q][0]), y - int(C[q][1]), z - int(C[q][2])]
             outside = False
             for a, ext in enumerate((nx, ny, nz)):
@@ -43,6 +47,21 @@ def brute_table(st, periodic, vox_of_site):
     return out
 
 
+def test_library_d3q19_set():
+    c, w, o = hlb.hlb_lattice(hlb.HLB_LATTICE_D3Q19)
+    assert c.shape == (19, 3)
+    vecs = {tuple(v) for v in c.tolist()}
+    assert len(vecs) == 19 and (0, 0, 0) in vecs
+    assert sum(1 for v in vecs if sum(abs(a) for a in v) == 1) == 6
+    assert sum(1 for v in vecs if sum(abs(a) for a in v) == 2 and max(abs(a) for a in v) == 1) == 12
+    for q in range(19):
+        assert np.array_equal(c[o[q]], -c[q]) and o[o[q]] == q
+        assert w[q] == {0: 1 / 3, 1: 1 / 18, 2: 1 / 36}[int(c[q] @ c[q])]
+    assert abs(w.sum() - 1.0) < 1e-15
+    c15, w15, o15 = hlb.hlb_lattice(0)
+    assert np.array_equal(c15, C) and np.array_equal(w15, WT) and np.array_equal(o15, OPP)
+
+
 def test_library_velocity_set_is_d3q15():
     assert {tuple(c) for c in C.tolist()} == {
         (0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1),
@@ -53,6 +72,7 @@ def test_library_velocity_set_is_d3q15():
         assert WT[q] == {0: 2 / 9, 1: 1 / 9, 3: 1 / 72}[int(C[q] @ C[q])]
 
 
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
 @pytest.mark.parametrize("order", [hlb.HLB_ORDER_AUTO, hlb.HLB_ORDER_MORTON, hlb.HLB_ORDER_RASTER,
                                    hlb.HLB_ORDER_TILED])
 @pytest.mark.parametrize("seed,periodic,shape", [
@@ -60,10 +80,12 @@ def test_library_velocity_set_is_d3q15():
     (4, 4, (5, 4, 17)), (5, 7, (1, 1, 3)), (6, 3, (2, 2, 2)), (7, 0, (16, 16, 16)),
     (8, 5, (17, 9, 23)),
 ])
-def test_table_matches_brute_force(order, seed, periodic, shape):
+def test_table_matches_brute_force(order, seed, periodic, shape, lattice):
     wl = W.random_mask(shape, p_fluid=0.55, n_iolets=3, p_iolet=0.08, periodic=periodic, seed=seed)
     st = wl.site_type
-    t = hlb.hlb_preprocess(st, periodic, 3, order)
+    t = hlb.hlb_preprocess(st, periodic, 3, order | LATTICES[lattice])
+    c_lat = hlb.hlb_lattice(LATTICES[lattice])[0]
+    assert t["nbr"].shape[0] == len(c_lat) - 1
     canon = wl.fluid_voxels()
     N = len(canon)
     assert t["N"] == N and t["Ns"] % 128 == 0 and N <= t["Ns"] < N + 128
@@ -82,7 +104,7 @@ def test_table_matches_brute_force(order, seed, periodic, shape):
                 for a, b, c in zip(x, y, z)]
         assert keys == sorted(keys)
     nbr = t["nbr"]
-    assert np.array_equal(nbr[:, :N].astype(np.int64), brute_table(st, periodic, vox))
+    assert np.array_equal(nbr[:, :N].astype(np.int64), brute_table(st, periodic, vox, c_lat))
     assert np.all(nbr[:, N:] == WALL)                                 # padding sites: all wall
 
 
@@ -124,11 +146,11 @@ def test_argument_errors():
 def decode_records(rec, nbr):
     """Pure-numpy reading of include/hlb.h's record encoding: returns (entries, sentinel)
     with entries[q-1, i] = decoded source index, -1 at wall lanes, and sentinel[g, q-1]."""
-    G = rec.shape[0]
-    out = np.full((14, G * 32), -1, dtype=np.int64)
-    sentinel = np.zeros((G, 14), dtype=bool)
+    G, NL = rec.shape[0], rec.shape[1]
+    out = np.full((NL, G * 32), -1, dtype=np.int64)
+    sentinel = np.zeros((G, NL), dtype=bool)
     for g in range(G):
-        for k in range(14):
+        for k in range(NL):
             wall, second, o0, o1 = (int(v) for v in rec[g, k])
             if second == 0xFFFFFFFF:
                 assert wall == 0 and o0 == 0 and o1 == 0
@@ -143,26 +165,29 @@ def decode_records(rec, nbr):
     return out, sentinel
 
 
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
 @pytest.mark.parametrize("order", [hlb.HLB_ORDER_MORTON, hlb.HLB_ORDER_RASTER, hlb.HLB_ORDER_TILED])
 @pytest.mark.parametrize("case", ["random", "random_periodic", "pipe", "tree"])
-def test_link_records_decode_to_the_table(order, case):
+def test_link_records_decode_to_the_table(order, case, lattice):
     if case == "random":
         wl = W.random_mask((24, 9, 7), p_fluid=0.8, n_iolets=2, p_iolet=0.05, seed=4)
     elif case == "random_periodic":
         wl = W.random_mask((64, 6, 5), p_fluid=1.1, n_iolets=0, periodic=7, seed=5)
     else:
         wl = W.by_name(case, small=True)
-    t = hlb.hlb_preprocess(wl.site_type, wl.periodic, wl.n_iolets, order)
+    t = hlb.hlb_preprocess(wl.site_type, wl.periodic, wl.n_iolets, order | LATTICES[lattice])
     nbr = t["nbr"].astype(np.int64)
+    NL = nbr.shape[0]
+    assert NL == {"d3q15": 14, "d3q19": 18}[lattice]
     rec, n_sentinel = hlb.hlb_preprocess_records(t["nbr"])
-    assert rec.shape == (t["Ns"] // 32, 14, 4)
+    assert rec.shape == (t["Ns"] // 32, NL, 4)
     dec, sentinel = decode_records(rec, nbr)
     assert n_sentinel == int(sentinel.sum())
     # brute-force run count per (group, q): sentinel <=> more than two runs
     G = t["Ns"] // 32
-    nb = nbr.reshape(14, G, 32)
+    nb = nbr.reshape(NL, G, 32)
     for g in range(G):
-        for k in range(14):
+        for k in range(NL):
             runs, prev = 0, None
             for l in range(32):
                 e = nb[k, g, l]
@@ -173,11 +198,11 @@ def test_link_records_decode_to_the_table(order, case):
                     runs += 1
                 prev = e
             assert sentinel[g, k] == (runs > 2)
-    keep = ~np.repeat(sentinel.T, 32, axis=1)              # [14, Ns]
+    keep = ~np.repeat(sentinel.T, 32, axis=1)              # [NL, Ns]
     expect = np.where(nbr >= 0, nbr, -1)
     assert np.array_equal(dec[keep], expect[keep])
     if order == hlb.HLB_ORDER_RASTER and case == "random_periodic":
-        assert n_sentinel < 0.6 * G * 14                    # x-runs make most records real
+        assert n_sentinel < 0.6 * G * NL                    # x-runs make most records real
 
 
 def test_link_records_argument_errors():
