@@ -42,6 +42,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "fluid site updates/sec (MSUPS), D3Q15 LBGK sparse site update"
+METRIC_Q19 = "fluid site updates/sec (MSUPS), D3Q19 LBGK sparse site update"
 UNIT = "MSUPS"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 DEFAULT_SCHEME = {"pipe": "two_lattice", "cube": "two_lattice", "aneurysm": "two_lattice",
@@ -65,6 +66,8 @@ def parse_args():
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--order", default="auto", choices=["auto", "morton", "raster", "tiled"])
     ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
+    ap.add_argument("--lattice", default="d3q15", choices=["d3q15", "d3q19"],
+                    help="d3q15 = BASELINE.json's metric; d3q19 = the lattice the paper ran (NEXT-1)")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -182,12 +185,12 @@ def crop_sample(wl, max_sites=1_200_000):
     return sub, 0, f"crop x in [{x0},{x1}) of the same voxel array (outside = solid)"
 
 
-def time_oracle(wl, budget_s, threads=1):
+def time_oracle(wl, budget_s, threads=1, lattice="d3q15"):
     """Oracle MSUPS on the bounded sample: 1 calibration step, then as many steps as fit
     the budget. Returns (msups, n_sites, steps, seconds, sample description)."""
     import oracle
     st, periodic, what = crop_sample(wl)
-    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, threads=threads)
+    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, threads=threads, lattice=lattice)
     n = o.n_sites
     t0 = time.perf_counter()
     o.step(1)
@@ -237,7 +240,7 @@ def run_reference(args, rank, world):
     wl = W.by_name(args.workload, small=args.small)
     scheme = args.scheme or DEFAULT_SCHEME[args.workload]
     st, periodic, what = crop_sample(wl)
-    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, threads=1)
+    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, threads=1, lattice=args.lattice)
     n = o.n_sites
     t0 = time.perf_counter()
     o.step(1)
@@ -254,12 +257,13 @@ def run_reference(args, rank, world):
     value = n * lb_per_step * args.steps / dt / 1e6
     sample = f"{what}: {n} sites x {lb_per_step} LB steps per bench step"
     out = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": METRIC if args.lattice == "d3q15" else METRIC_Q19, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
-                   "scheme": scheme, "store": args.store, "n_sites_full": wl.n_sites,
+                   "scheme": scheme, "store": args.store, "lattice": args.lattice,
+                   "n_sites_full": wl.n_sites,
                    "n_sites_sample": n, "lb_steps_per_step": lb_per_step, "tau": wl.tau,
                    "host_cpu": host_cpu_model(), "host_cores": os.cpu_count()},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
@@ -305,7 +309,8 @@ def main():
              "tiled": hlb.HLB_ORDER_TILED}[args.order] | \
             {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
              "records": hlb.HLB_LINKS_RECORDS}[args.links] | \
-            (hlb.HLB_NO_PREFETCH if args.no_prefetch else 0)
+            (hlb.HLB_NO_PREFETCH if args.no_prefetch else 0) | \
+            (hlb.HLB_LATTICE_D3Q19 if args.lattice == "d3q19" else hlb.HLB_LATTICE_D3Q15)
     t_create = time.perf_counter()
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
     torch.cuda.synchronize()
@@ -354,15 +359,16 @@ def main():
         b.record(stream)
     torch.cuda.synchronize()
     per = np.array([a.elapsed_time(b) for a, b in evs])
+    nq = g.hlb_num_q()
+    pop_bytes = nq * 2 * (4 if args.store == "f32" else 8)
     if scheme == "aa":
         phase = (parity0 + np.arange(per.size)) & 1          # 0: even-phase kernel, 1: odd-phase
         k_ms = {"k_aa<even>": float(np.mean(per[phase == 0])),
                 "k_aa<odd>": float(np.mean(per[phase == 1]))}
-        k_bytes = {"k_aa<even>": 15 * 2 * (4 if args.store == "f32" else 8),
-                   "k_aa<odd>": 15 * 2 * (4 if args.store == "f32" else 8) + 56}
+        k_bytes = {"k_aa<even>": pop_bytes, "k_aa<odd>": pop_bytes + 4 * (nq - 1)}
     else:
         k_ms = {"k_pull": float(np.mean(per))}
-        k_bytes = {"k_pull": 15 * 2 * (4 if args.store == "f32" else 8) + 56}
+        k_bytes = {"k_pull": pop_bytes + 4 * (nq - 1)}
     dominant = max(k_ms, key=lambda k: k_ms[k])
 
     # ---------------- end to end through the C-ABI with host buffers
@@ -400,15 +406,16 @@ def main():
     peak, peak_src = measured_peak()
     dom_ms = k_ms[dominant]
     achieved = k_bytes[dominant] * N / (dom_ms * 1e-3) / 1e9
-    traffic = committed_traffic(args.workload, scheme, args.store, dominant)
-    step_bytes = hlb.algorithmic_bytes_per_site(scheme, args.store)
+    traffic = committed_traffic(args.workload, scheme, args.store, dominant) if nq == 15 else \
+        committed_traffic(args.workload + "_d3q19", scheme, args.store, dominant)
+    step_bytes = hlb.algorithmic_bytes_per_site(scheme, args.store, nq)
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRIC if nq == 15 else METRIC_Q19, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {
             "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
-            "n_sites": N, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
+            "n_sites": N, "lattice": args.lattice, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
             "order": args.order, "links": "records" if g.hlb_uses_records() else "table",
             "l2_prefetch": not args.no_prefetch,
             "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
@@ -438,7 +445,7 @@ def main():
                       "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}
     g.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, n, st, dt, what, thr = time_oracle(wl, args.cpu_seconds, threads=1)
+        v, n, st, dt, what, thr = time_oracle(wl, args.cpu_seconds, threads=1, lattice=args.lattice)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
                                "sample": f"{what}: {n} sites x {st} LB steps in {dt:.1f} s",
                                "host_cpu": host_cpu_model(), "host_cores": os.cpu_count()}

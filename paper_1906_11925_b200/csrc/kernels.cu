@@ -40,9 +40,10 @@ constexpr int BLOCK = 256;   // read-out / init kernels
 #define HLB_AA_ODD_MINB 6
 #endif
 constexpr int SBLOCK = HLB_STEP_BLOCK;
-// D3Q19 keeps 4 more populations (8 registers) and 4 more offsets alive: one block less.
+// D3Q19 keeps 4 more populations (8 registers) and 4 more offsets alive: two blocks less
+// (measured: 20.8k vs 20.5k MSUPS A-A, 20.1k vs 19.5k pull on configs[4]).
 #ifndef HLB_Q19_MINB_DROP
-#define HLB_Q19_MINB_DROP 1
+#define HLB_Q19_MINB_DROP 2
 #endif
 template <typename L, bool REC> constexpr int pull_minb() {
   return HLB_PULL_MINB - (REC ? 0 : 1) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);

@@ -446,7 +446,7 @@ def _smooth_state(x, y, z):
     return rho, u
 
 
-def _crop_check(hlb, wl, rho, u, steps, centre, half, tol):
+def _crop_check(hlb, wl, rho, u, steps, centre, half, tol, lattice="d3q15"):
     """Exact check of a full-size run on a sample: a site update is local (information moves
     one voxel per step), so the oracle run on the sub-box [centre - half, centre + half] of
     the same voxel array (outside the crop = solid) reproduces, after `steps` steps, every
@@ -456,7 +456,7 @@ def _crop_check(hlb, wl, rho, u, steps, centre, half, tol):
     lo = [max(0, c - half) for c in centre]
     hi = [min(n, c + half + 1) for c, n in zip(centre, (nx, ny, nz))]
     sub = np.ascontiguousarray(st[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]])
-    o = oracle.Oracle(sub, 0, wl.tau, wl.iolet_rho, threads=0)
+    o = oracle.Oracle(sub, 0, wl.tau, wl.iolet_rho, threads=0, lattice=lattice)
     v = o.site_voxels()
     sx, sy, sz = hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]
     x, y, z = v % sx + lo[0], (v // sx) % sy + lo[1], v // (sx * sy) + lo[2]
@@ -489,17 +489,18 @@ def _sample_centres(wl, n):
     return [(int(a), int(b), int(c)) for a, b, c in zip(x, (picks // nx) % ny, picks // (nx * ny))]
 
 
-@pytest.mark.parametrize("name,scheme,store", [
-    ("tree", "two_lattice", "f64"), ("tree", "two_lattice", "f32"), ("bigtree", "aa", "f64"),
+@pytest.mark.parametrize("name,scheme,store,lattice", [
+    ("tree", "two_lattice", "f64", "d3q15"), ("tree", "two_lattice", "f32", "d3q15"),
+    ("bigtree", "aa", "f64", "d3q15"), ("tree", "aa", "f64", "d3q19"),
 ])
-def test_configs_3_4_full_size_sampled_against_oracle(hlb, name, scheme, store):
+def test_configs_3_4_full_size_sampled_against_oracle(hlb, name, scheme, store, lattice):
     """BASELINE configs[3] / [4] at full size in the launch configuration bench.py times
     (default order, link records, L2 prefetch): 25 steps (odd: A-A read-out through the
     table), then sub-boxes compared site by site with the oracle (see _crop_check)."""
     wl = W.by_name(name)
     steps, half = 25, 56
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
-                                flags_of(hlb, scheme, store, "auto", "auto"))
+                                flags_of(hlb, scheme, store, "auto", "auto", lattice))
     assert g.hlb_uses_records()
     nz, ny, nx = wl.site_type.shape
     v = wl.fluid_voxels()
@@ -510,7 +511,7 @@ def test_configs_3_4_full_size_sampled_against_oracle(hlb, name, scheme, store):
     assert np.all(np.isfinite(rho)) and np.all(np.isfinite(u))
     checked = 0
     for centre in _sample_centres(wl, 5):
-        n, un = _crop_check(hlb, wl, rho, u, steps, centre, half, TOL[store])
+        n, un = _crop_check(hlb, wl, rho, u, steps, centre, half, TOL[store], lattice)
         assert un > 1e-3                                  # the sample is not at rest
         checked += n
     assert checked > 20000

@@ -55,6 +55,6 @@ def test_reference_arm_idles_on_other_ranks(monkeypatch):
     """Under torchrun only rank 0 runs the oracle; the others exit 0 without work."""
     import argparse
     import bench
-    args = argparse.Namespace(workload="pipe", small=True, scheme=None, store="f64", steps=1,
+    args = argparse.Namespace(workload="pipe", small=True, scheme=None, store="f64", steps=1, lattice="d3q15",
                               warmup=1, inner=2, ref_seconds=1.0, gpus=2)
     assert bench.run_reference(args, rank=1, world=2) == 0
