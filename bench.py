@@ -4,7 +4,7 @@
 Contract (one JSON line on stdout, printed by rank 0):
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload bigtree|tree|aneurysm|cube|pipe]
                   [--scheme aa|two_lattice] [--store f64|f32] [--order morton|raster|tiled]
-                  [--inner S] [--impl ours|reference]
+                  [--lattice d3q15|d3q19] [--inner S] [--impl ours|reference]
 
 * metric/unit: BASELINE.json's metric -- fluid site updates per second, in MSUPS
   (= fluid sites x LB time steps / seconds / 1e6; the paper's SUPS definition, PAPER.md

@@ -6,8 +6,10 @@
  * steps" (section II), with "simple bounce-back boundary condition"
  * (section IV) -- in the concrete form BASELINE.json `north_star` fixes:
  * fused D3Q15 LBGK collide-and-stream over a sparse, indirectly addressed list of fluid
- * sites, halfway bounce-back walls, constant-density inlets/outlets. The formulas and the
- * readings of every point the paper leaves open are in DESIGN.md ("Readings").
+ * sites, halfway bounce-back walls, constant-density inlets/outlets. The paper's own lattice,
+ * D3Q19, is selected with HLB_LATTICE_D3Q19; Q below is the
+ * lattice's population count (15 or 19). The formulas and the readings of every point the
+ * paper leaves open are in DESIGN.md ("Readings").
  *
  * Conventions
  *   - Plain C ABI: no C++ or torch types. Every function returns HLB_OK (0) or a negative
