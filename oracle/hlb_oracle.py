@@ -73,6 +73,11 @@ def _load():
                                  ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                  ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_set_iolet_velocity.restype = None
+        lib.hlbo_set_iolet_velocity.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbd_run_ladd.restype = ctypes.c_int
+        lib.hlbd_run_ladd.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p, ctypes.c_void_p] + \
+            lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
         lib.hlbd_run_lattice.restype = ctypes.c_int
         lib.hlbd_run_lattice.argtypes = lib.hlbd_run.argtypes + [ctypes.c_int]
         for name in ("hlbo_site_voxels", "hlbo_set_state", "hlbo_set_populations",
@@ -120,6 +125,7 @@ class Oracle:
         if not self._h:
             raise ValueError("hlbo_create rejected its arguments")
         self.n_sites = int(lib.hlbo_num_sites(self._h))
+        self.n_iolets = int(io.shape[0])
         self.threads = int(lib.hlbo_get_threads())
 
     def close(self):
@@ -142,6 +148,14 @@ class Oracle:
         if u is not None:
             assert u.shape == (self.n_sites, 3)
         self._lib.hlbo_set_state(self._h, _ptr(rho), _ptr(u))
+
+    def set_iolet_velocity(self, kind, u):
+        """kind [n_iolets]: 0 constant density, 1 Ladd velocity; u [n_iolets, 3]. Takes effect
+        from the next step."""
+        kind = np.ascontiguousarray(np.asarray(kind, dtype=np.uint8).reshape(-1))
+        u = np.ascontiguousarray(np.asarray(u, dtype=np.float64).reshape(-1, 3))
+        assert kind.shape == (self.n_iolets,) and u.shape == (self.n_iolets, 3)
+        self._lib.hlbo_set_iolet_velocity(self._h, _ptr(kind), _ptr(u))
 
     def set_populations(self, f):
         f = np.ascontiguousarray(f, dtype=np.float64)
@@ -173,6 +187,8 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
                variant=variant, threads=threads, lattice=lattice)
     if workload.rho0 is not None or workload.u0 is not None:
         o.set_state(workload.rho0, workload.u0)
+    if getattr(workload, "iolet_kind", None) is not None:
+        o.set_iolet_velocity(workload.iolet_kind, workload.iolet_u)
     o.step(workload.steps if steps is None else steps)
     out = o.get_macroscopic()
     o.close()
@@ -180,7 +196,7 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
 
 
 def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None,
-              lattice="d3q15"):
+              lattice="d3q15", iolet_kind=None, iolet_u=None):
     """Dense-grid twin: per-VOXEL rho [nz,ny,nx] and u [nz,ny,nx,3]."""
     lib = _load()
     st = np.ascontiguousarray(site_type, dtype=np.uint8)
@@ -190,9 +206,13 @@ def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=
     u0 = None if u0_vox is None else np.ascontiguousarray(u0_vox, dtype=np.float64)
     rho = np.zeros((nz, ny, nx), dtype=np.float64)
     u = np.zeros((nz, ny, nx, 3), dtype=np.float64)
-    rc = lib.hlbd_run_lattice(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
-                              _ptr(io), _ptr(r0), _ptr(u0), int(steps), _ptr(rho), _ptr(u),
-                              LATTICE_Q[lattice])
+    kind = None if iolet_kind is None else \
+        np.ascontiguousarray(np.asarray(iolet_kind, dtype=np.uint8).reshape(-1))
+    uio = None if iolet_u is None else \
+        np.ascontiguousarray(np.asarray(iolet_u, dtype=np.float64).reshape(-1, 3))
+    rc = lib.hlbd_run_ladd(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
+                           _ptr(io), _ptr(kind), _ptr(uio), _ptr(r0), _ptr(u0), int(steps),
+                           _ptr(rho), _ptr(u), LATTICE_Q[lattice])
     if rc != 0:
         raise ValueError("hlbd_run rejected its arguments")
     return rho, u

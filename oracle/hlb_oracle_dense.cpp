@@ -14,6 +14,7 @@
 //     d fluid   : f_q(d, t+1)      = f*_q(x, t)
 //     d solid   : f_opp(q)(x, t+1) = f*_q(x, t)
 //     d iolet k : f_opp(q)(x, t+1) = feq_opp(q)(rho_k, u(x, t))
+//     d velocity iolet k (Ladd): f_opp(q)(x, t+1) = f*_q(x, t) - 6 w_q rho(x, t) c_q.u_k
 // which is the pull rule of hlb_oracle.cpp read from the other end of the link.
 
 #include <cstdint>
@@ -63,9 +64,10 @@ extern "C" {
 // rho0 / u0: per VOXEL ([nvox], [nvox][3]), read only at fluid voxels; NULL => 1 / 0.
 // rho_out / u_out: per voxel, written at fluid voxels, 0 elsewhere.
 // Returns 0, or -1 on a bad argument.
-int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
-                     int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
-                     int64_t steps, double* rho_out, double* u_out, int lattice_q) {
+static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                         int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
+                         const double* iolet_u, const double* rho0, const double* u0,
+                         int64_t steps, double* rho_out, double* u_out, int lattice_q) {
   if (lattice_q != 15 && lattice_q != 19) return -1;
   const Lattice& L = lattice_q == 15 ? L15 : L19;
   const int Q = L.Q;
@@ -111,7 +113,16 @@ int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned perio
             else if (t == 0) g[v * Q + OPP[q]] = fstar;
             else {
               if (t - 2 >= n_iolets) return -1;
-              g[v * Q + OPP[q]] = feq(L, OPP[q], iolet_rho[t - 2], ux, uy, uz);
+              const int k = t - 2;
+              if (iolet_kind && iolet_kind[k] == 1) {
+                // the population leaves along c_q and comes back reversed; seen from the
+                // returning direction opp(q) the gain is +6 w rho c_opp(q).u = -6 w rho c_q.u
+                const double cu = CX[q] * iolet_u[k * 3 + 0] + CY[q] * iolet_u[k * 3 + 1] +
+                                  CZ[q] * iolet_u[k * 3 + 2];
+                g[v * Q + OPP[q]] = fstar - 6.0 * L.WT[q] * rho * cu;
+              } else {
+                g[v * Q + OPP[q]] = feq(L, OPP[q], iolet_rho[k], ux, uy, uz);
+              }
             }
           }
         }
@@ -130,6 +141,22 @@ int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned perio
     }
   }
   return 0;
+}
+
+int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                     int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
+                     int64_t steps, double* rho_out, double* u_out, int lattice_q) {
+  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, nullptr, nullptr, rho0,
+                       u0, steps, rho_out, u_out, lattice_q);
+}
+
+// iolet_kind [n_iolets]: 0 constant density, 1 Ladd velocity with iolet_u [n_iolets][3]
+int hlbd_run_ladd(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                  int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
+                  const double* iolet_u, const double* rho0, const double* u0, int64_t steps,
+                  double* rho_out, double* u_out, int lattice_q) {
+  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
+                       rho0, u0, steps, rho_out, u_out, lattice_q);
 }
 
 int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,

@@ -303,6 +303,61 @@ def test_p8_pipe_poiseuille_config0():
     assert np.all(got > 0)
 
 
+# ------------------------------------------------------------------ Ladd velocity iolets
+@pytest.mark.parametrize("tau", [0.6, 1.0, 1.4])
+def test_ladd_moving_boundary_gives_exact_couette_flow(tau):
+    """A velocity iolet is Ladd's bounce-back off a boundary moving with u_k (PAPER.md lines
+    43, 59: "LADDIOLET"). Tangential motion above a channel of H rows whose lower wall is at
+    rest: the steady state is plane Couette flow, which LBGK with halfway bounce-back
+    represents exactly, u_x(y) = U (y - 1/2) / H with the walls at y = 1/2 and y = H + 1/2.
+    A wrong factor (2 w rho c.u / c_s^2 = 6 w rho c.u) or sign changes the slope."""
+    H, U = 8, 0.01
+    st = np.zeros((1, H + 2, 1), dtype=np.uint8)
+    st[0, 1:H + 1, 0] = 1
+    st[0, H + 1, 0] = 2
+    o = oracle.Oracle(st, 5, tau, [1.0])
+    o.set_iolet_velocity([1], [[U, 0.0, 0.0]])
+    o.step(int(40 * H * H / ((tau - 0.5) / 3.0) / 10))
+    rho, u = o.get_macroscopic()
+    y = np.arange(1, H + 1)
+    assert np.max(np.abs(u[:, 0] - U * (y - 0.5) / H)) < 1e-13
+    assert np.max(np.abs(u[:, 1:])) < 1e-16 and np.max(np.abs(rho - 1.0)) < 1e-15
+
+
+def test_ladd_normal_inflow_injects_mass_flux_rho_times_u():
+    """Normal motion: per step the boundary injects sum_q 6 w_q rho (c_q.u) over the links
+    that cross it = rho u_n exactly (sum over c_qn = +1 of w_q c_qn^2 = 1/6). In a duct that is
+    periodic sideways with a velocity inlet at one end and a constant-density outlet at the
+    other, the steady mass flux is therefore rho(first site) * W everywhere."""
+    L, Wn = 16, 0.005
+    st = np.zeros((L + 2, 1, 1), dtype=np.uint8)
+    st[1:L + 1, 0, 0] = 1
+    st[0, 0, 0] = 2
+    st[L + 1, 0, 0] = 3
+    o = oracle.Oracle(st, 3, 0.8, [1.0, 1.0])
+    o.set_iolet_velocity([1, 0], [[0.0, 0.0, Wn], [0.0, 0.0, 0.0]])
+    o.step(40000)
+    rho, u = o.get_macroscopic()
+    j = rho * u[:, 2]
+    assert np.max(np.abs(j - rho[0] * Wn)) < 1e-13
+    assert np.max(np.abs(u[:, :2])) < 1e-16
+
+
+def test_ladd_velocity_at_rest_is_plain_bounce_back():
+    """u_k = 0 must reproduce a solid wall bit for bit."""
+    wl = W.random_mask((8, 7, 6), p_fluid=0.6, n_iolets=2, p_iolet=0.1, seed=21)
+    as_wall = wl.site_type.copy()
+    as_wall[as_wall >= 2] = 0
+    a = oracle.Oracle(wl.site_type, 0, wl.tau, wl.iolet_rho)
+    a.set_iolet_velocity([1, 1], np.zeros((2, 3)))
+    b = oracle.Oracle(as_wall, 0, wl.tau, [])
+    for o in (a, b):
+        o.set_state(wl.rho0, wl.u0)
+        o.step(12)
+    (ra, ua), (rb, ub) = a.get_macroscopic(), b.get_macroscopic()
+    assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
+
+
 # ------------------------------------------------------------------ P9 dense twin
 @pytest.mark.parametrize("seed,periodic,shape", [
     (0, 0, (7, 6, 5)), (1, 7, (6, 6, 6)), (2, 1, (12, 5, 4)), (3, 2, (4, 9, 5)),
@@ -320,16 +375,22 @@ def test_p9_dense_push_twin_equals_sparse_pull(seed, periodic, shape):
     u0v = np.zeros((nvox, 3))
     rho0v[vox] = wl.rho0
     u0v[vox] = wl.u0
-    rd, ud = oracle.dense_run(st, periodic, wl.tau, wl.iolet_rho, steps, rho0v, u0v)
-    rd, ud = rd.reshape(-1)[vox], ud.reshape(-1, 3)[vox]
-    for variant, tol in ((oracle.VARIANT_RAW, 2e-15), (oracle.VARIANT_SHIFTED, 2e-14)):
-        o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, variant=variant)
-        assert np.array_equal(o.site_voxels(), vox)
-        o.set_state(wl.rho0, wl.u0)
-        o.step(steps)
-        r, u = o.get_macroscopic()
-        assert np.max(np.abs(r - rd)) < tol
-        assert np.max(np.abs(u - ud)) < tol
+    rng = np.random.default_rng(seed)
+    for kind, uio in ((None, None),
+                      (np.array([1, 0, 1], dtype=np.uint8), 0.02 * (rng.random((3, 3)) - 0.5))):
+        rd, ud = oracle.dense_run(st, periodic, wl.tau, wl.iolet_rho, steps, rho0v, u0v,
+                                  iolet_kind=kind, iolet_u=uio)
+        rd, ud = rd.reshape(-1)[vox], ud.reshape(-1, 3)[vox]
+        for variant, tol in ((oracle.VARIANT_RAW, 2e-15), (oracle.VARIANT_SHIFTED, 2e-14)):
+            o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, variant=variant)
+            assert np.array_equal(o.site_voxels(), vox)
+            o.set_state(wl.rho0, wl.u0)
+            if kind is not None:
+                o.set_iolet_velocity(kind, uio)
+            o.step(steps)
+            r, u = o.get_macroscopic()
+            assert np.max(np.abs(r - rd)) < tol
+            assert np.max(np.abs(u - ud)) < tol
 
 
 # ------------------------------------------------------------------ P11 symmetry

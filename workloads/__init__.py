@@ -13,5 +13,6 @@ from .geometries import (  # noqa: F401
     tree,
     random_mask,
     by_name,
+    with_velocity_inlet,
     CONFIG_NAMES,
 )

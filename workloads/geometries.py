@@ -39,6 +39,8 @@ class Workload:
     steps: int                       # step count the config asks for
     rho0: Optional[np.ndarray] = None  # float64 (N,) canonical order, None => 1
     u0: Optional[np.ndarray] = None    # float64 (N, 3) canonical order, None => 0
+    iolet_kind: Optional[np.ndarray] = None  # uint8 (n_iolets,): 0 density, 1 Ladd velocity; None => all 0
+    iolet_u: Optional[np.ndarray] = None     # float64 (n_iolets, 3) velocities of the velocity iolets
     scheme: str = "two_lattice"      # "two_lattice" | "aa"  (what the config asks for)
     store: str = "f64"               # "f64" | "f32"
     info: dict = dataclasses.field(default_factory=dict)
@@ -335,6 +337,18 @@ def random_mask(shape=(8, 7, 6), p_fluid: float = 0.6, n_iolets: int = 2, p_iole
     return Workload("random", st, periodic, tau,
                     rng.uniform(0.98, 1.02, size=n_iolets).astype(np.float64), steps,
                     rho0=rho0, u0=u0, info={"seed": seed})
+
+
+def with_velocity_inlet(wl: Workload, u_in: float = 0.004) -> Workload:
+    """The same geometry with iolet 0 turned into a Ladd velocity inlet (the paper's
+    "LADDIOLET" configuration) blowing u_in along +x for the vessel
+    geometries (their inlet caps face -x) and along +z for the pipe; the other iolets stay
+    constant-density outlets."""
+    kind = np.zeros(wl.n_iolets, dtype=np.uint8)
+    u = np.zeros((wl.n_iolets, 3), dtype=np.float64)
+    kind[0] = 1
+    u[0, 2 if wl.name == "pipe" else 0] = u_in
+    return dataclasses.replace(wl, iolet_kind=kind, iolet_u=u, name=wl.name)
 
 
 def by_name(name: str, small: bool = False) -> Workload:
