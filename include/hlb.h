@@ -114,8 +114,20 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
  *   rho: HOST [N] or NULL (=> 1);  u: HOST [N][3] or NULL (=> 0); canonical order. */
 int hlb_set_state(hlb_geometry* g, const double* rho, const double* u);
 
-/* Replace the n_iolets iolet densities (HOST array). Takes effect from the next step. */
+/* Replace the n_iolets iolet densities (HOST array, each > 0). Takes effect from the next
+ * step; the density of an iolet that is currently a velocity iolet is kept for later. */
 int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho);
+
+/* Choose, per iolet, between the constant-density rule (kind 0, the default:
+ * f_q(x,t+1) = f_eq_q(rho_k, u(x,t))) and Ladd's velocity rule (kind 1, the paper's
+ * "LADDIOLET" boundary, ref. [15]): a link whose source voxel is a
+ * ghost voxel of velocity iolet k bounces back off a boundary moving with u_k,
+ *     f_q(x,t+1) = f*_opp(q)(x,t) + 6 w_q rho(x,t) c_q.u_k      (reading R-ladd).
+ *   kind: HOST [n_iolets] bytes 0 / 1, or NULL (all 0);  u: HOST [n_iolets][3] lattice
+ *   velocities (read for kind 1; may be NULL when no kind is 1).
+ * Takes effect from the next step, so a time-varying inlet (the paper's Fig. 8 waveform) is
+ * hlb_step(n) / hlb_set_iolet_velocity(...) in turn. Errors: HLB_EINVAL. */
+int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u);
 
 /* Advance n >= 0 time steps: n launches of ONE fused collide-and-stream kernel (A-A:
  * alternating even/odd kernels), asynchronously on the stream. n == 0 is a no-op. A

@@ -56,6 +56,7 @@ def _load() -> ctypes.CDLL:
         "hlb_geometry_create": (c_int, [vp, ctypes.POINTER(hlb_params), ctypes.POINTER(vp)]),
         "hlb_set_state": (c_int, [vp, vp, vp]),
         "hlb_set_iolet_density": (c_int, [vp, vp]),
+        "hlb_set_iolet_velocity": (c_int, [vp, vp, vp]),
         "hlb_step": (c_int, [vp, i64]),
         "hlb_get_macroscopic": (c_int, [vp, vp, vp]),
         "hlb_get_macroscopic_device": (c_int, [vp, vp, vp]),
@@ -87,7 +88,8 @@ def _load() -> ctypes.CDLL:
 
 LIB_PATH = _build.LIB_PATH
 _lib = _load()
-EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density", "hlb_step",
+EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
+            "hlb_set_iolet_velocity", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
@@ -219,6 +221,11 @@ class Geometry:
     def hlb_set_iolet_density(self, iolet_rho):
         io = _host(np.asarray(iolet_rho).reshape(-1), np.float64)
         _check(_lib.hlb_set_iolet_density(self._h, _ptr(io)))
+
+    def hlb_set_iolet_velocity(self, kind, u=None):
+        kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8)
+        u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64)
+        _check(_lib.hlb_set_iolet_velocity(self._h, _ptr(kind), _ptr(u)))
 
     def hlb_step(self, n: int = 1):
         _check(_lib.hlb_step(self._h, int(n)))

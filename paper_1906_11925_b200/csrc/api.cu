@@ -55,6 +55,9 @@ struct hlb_geometry {
   int64_t N = 0, Ns = 0;
   std::vector<int64_t> canon_voxels;  // [N] ascending
   std::vector<double> iolet_rho;
+  std::vector<uint8_t> iolet_kind;    // 0 constant density, 1 Ladd velocity
+  std::vector<double> iolet_u;        // [n_iolets][3]
+  std::vector<double> iolet_par;      // [n_iolets][4] as uploaded: {rho or -1, ux, uy, uz}
   DeviceGeometry dg;
   void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
   int cur = 0;                        // two-lattice: buffer the next step reads
@@ -159,6 +162,25 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
   return HLB_OK;
 }
 
+// {rho_k, 0, 0, 0} for a constant-density iolet, {-1, ux, uy, uz} for a velocity iolet
+static int upload_iolets(hlb_geometry* g) {
+  const int n = g->p.n_iolets;
+  if (n == 0) return HLB_OK;
+  HLB_CUDA(cudaStreamSynchronize(g->stream));  // the previous upload may still read iolet_par
+  g->iolet_par.assign((size_t)n * 4, 0.0);
+  for (int k = 0; k < n; ++k) {
+    if (g->iolet_kind[(size_t)k] == 1) {
+      g->iolet_par[(size_t)k * 4] = -1.0;
+      for (int a = 0; a < 3; ++a) g->iolet_par[(size_t)k * 4 + 1 + a] = g->iolet_u[(size_t)k * 3 + a];
+    } else {
+      g->iolet_par[(size_t)k * 4] = g->iolet_rho[(size_t)k];
+    }
+  }
+  HLB_CUDA(cudaMemcpyAsync((void*)g->dg.iolet_par, g->iolet_par.data(), sizeof(double) * 4 * (size_t)n,
+                           cudaMemcpyHostToDevice, g->stream));
+  return HLB_OK;
+}
+
 int hlb_preprocess_records(const int32_t* nbr, int32_t n_links, int64_t stride, uint32_t* rec,
                            int64_t* n_sentinel) {
   if (!nbr || !rec) return fail(HLB_EINVAL, "NULL argument");
@@ -199,6 +221,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->N = t.N;
   g->Ns = t.Ns;
   g->iolet_rho.assign(p->iolet_rho, p->iolet_rho + p->n_iolets);
+  g->iolet_kind.assign((size_t)p->n_iolets, 0);
+  g->iolet_u.assign((size_t)p->n_iolets * 3, 0.0);
   g->canon_voxels.resize((size_t)t.N);
   for (int64_t i = 0; i < t.N; ++i) g->canon_voxels[(size_t)t.canon_of_site[(size_t)i]] = t.voxel_of_site[(size_t)i];
 
@@ -234,7 +258,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   if ((rc = g->alloc(sizeof(uint32_t) * t.iolet_bits.size(), &d_bits))) return bail(rc);
   if (use_rec && (rc = g->alloc(sizeof(uint32_t) * t.rec.size(), &d_rec))) return bail(rc);
   if ((rc = g->alloc(sizeof(int32_t) * (size_t)t.N, &d_canon))) return bail(rc);
-  if ((rc = g->alloc(sizeof(double) * (size_t)(p->n_iolets > 0 ? p->n_iolets : 1), &d_rho))) return bail(rc);
+  if ((rc = g->alloc(sizeof(double) * 4 * (size_t)(p->n_iolets > 0 ? p->n_iolets : 1), &d_rho))) return bail(rc);
   if ((rc = g->alloc(pop_bytes + pad_bytes, &g->buf[0]))) return bail(rc);
   if (!g->aa && (rc = g->alloc(pop_bytes + pad_bytes, &g->buf[1]))) return bail(rc);
   if ((rc = g->alloc(sizeof(double) * 4 * (size_t)t.N, &d_scratch))) return bail(rc);
@@ -250,8 +274,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   if (use_rec)
     HLB_CUDA_G(cudaMemcpyAsync(d_rec, t.rec.data(), sizeof(uint32_t) * t.rec.size(), cudaMemcpyHostToDevice, g->stream));
   HLB_CUDA_G(cudaMemcpyAsync(d_canon, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N, cudaMemcpyHostToDevice, g->stream));
-  if (p->n_iolets > 0)
-    HLB_CUDA_G(cudaMemcpyAsync(d_rho, g->iolet_rho.data(), sizeof(double) * (size_t)p->n_iolets, cudaMemcpyHostToDevice, g->stream));
+  g->dg.iolet_par = (const double*)d_rho;
+  if ((rc = upload_iolets(g))) return bail(rc);
   g->dg.N = t.N;
   g->dg.Ns = t.Ns;
   g->dg.nbr = (const int32_t*)d_nbr;
@@ -260,7 +284,6 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.use_rec = use_rec;
   g->dg.index64 = (p->flags & HLB_INDEX64) != 0 || (int64_t)Q * t.Ns >= ((int64_t)1 << 32);
   g->dg.canon = (const int32_t*)d_canon;
-  g->dg.iolet_rho = (const double*)d_rho;
   g->dg.omega = 1.0 / p->tau;
   g->dg.f32 = g->f32;
   g->dg.d3q19 = Q == 19;
@@ -329,10 +352,25 @@ int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   if (g->p.n_iolets == 0) return HLB_OK;
   if (!iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
+  for (int k = 0; k < g->p.n_iolets; ++k)
+    if (!(iolet_rho[k] > 0.0)) return fail(HLB_EINVAL, "iolet densities must be positive");
   g->iolet_rho.assign(iolet_rho, iolet_rho + g->p.n_iolets);
-  HLB_CUDA(cudaMemcpyAsync((void*)g->dg.iolet_rho, g->iolet_rho.data(), sizeof(double) * (size_t)g->p.n_iolets, cudaMemcpyHostToDevice, g->stream));
-  HLB_CUDA(cudaStreamSynchronize(g->stream));  // g->iolet_rho may be reassigned by the next call
-  return HLB_OK;
+  return upload_iolets(g);
+}
+
+int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  const int n = g->p.n_iolets;
+  if (n == 0) return HLB_OK;
+  for (int k = 0; k < n; ++k) {
+    if (kind && kind[k] > 1) return fail(HLB_EINVAL, "iolet kind must be 0 (density) or 1 (velocity)");
+    if (kind && kind[k] == 1 && !u) return fail(HLB_EINVAL, "u is NULL but a velocity iolet is requested");
+  }
+  for (int k = 0; k < n; ++k) {
+    g->iolet_kind[(size_t)k] = kind ? kind[k] : 0;
+    for (int a = 0; a < 3; ++a) g->iolet_u[(size_t)k * 3 + a] = u ? u[k * 3 + a] : 0.0;
+  }
+  return upload_iolets(g);
 }
 
 constexpr int64_t GRAPH_STEPS = 32;  // even: the buffer / phase parity is back where it started

@@ -142,21 +142,28 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 }
 
 // Rare path (sites on an inlet/outlet cap): for every iolet link p of site i replace
-// out[p] -- the value that will be read back as f_p(x, t+1) -- by the constant-density
-// equilibrium f_eq_p(rho_k, u(x, t)) (reading A6). The table entries are re-read here so
-// that the common path does not keep them in registers; fully unrolled so that out[] stays
-// in registers (no call, no stack).
+// out[p] -- the value that will be read back as f_p(x, t+1), on entry the bounced h*_opp(p) --
+//   constant-density iolet k: by the equilibrium f_eq_p(rho_k, u(x, t))           (reading A6)
+//   velocity iolet k (Ladd):  by h*_opp(p) + 6 w_p rho(x, t) c_p.u_k             (reading R-ladd)
+// The table entries are re-read here so that the common path does not keep them in
+// registers; fully unrolled so that out[] stays in registers (no call, no stack).
 template <typename L>
 __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
                                                  long long i, const Moments& m,
-                                                 const double* __restrict__ iolet_rho,
+                                                 const double* __restrict__ iolet_par,
                                                  double (&out)[L::Q]) {
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) {
     const int k = iolet_of(__ldg(nbr + (long long)(p - 1) * Ns + i));
     if (k >= 0) {
-      const double rk = __ldg(iolet_rho + k);
-      out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+      const double* par = iolet_par + 4 * k;
+      const double rk = __ldg(par);
+      if (rk > 0.0) {
+        out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+      } else {
+        const double cu = c_dot_u<L>(p, __ldg(par + 1), __ldg(par + 2), __ldg(par + 3));
+        out[p] = fma_(mul(6.0 * L::weight(p), m.rho), cu, out[p]);
+      }
     }
   }
 }
@@ -181,7 +188,7 @@ template <typename L, typename ST, bool REC, typename IT>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
-       const double* __restrict__ iolet_rho, long long Ns, double omega, long long pf) {
+       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[L::Q];
   {
@@ -207,7 +214,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L>(nbr, Ns, i, m, iolet_rho, back);
+    iolet_substitute<L>(nbr, Ns, i, m, iolet_par, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
@@ -224,7 +231,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 template <typename L, typename ST>
 __global__ void __launch_bounds__(SBLOCK, aa_even_minb<L>())
 k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
-          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
+          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
           long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   ST* p0 = a + i;
@@ -240,7 +247,7 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
   double out[L::Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_rho, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_par, out);
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
@@ -248,7 +255,7 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
 template <typename L, typename ST, bool REC, typename IT>
 __global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
-         const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_rho,
+         const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
          long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
@@ -271,7 +278,7 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_rho, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_par, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
@@ -383,7 +390,7 @@ int resident_sites_per_sm_aa(bool d3q19) {
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   k_pull<L, ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
-      (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_rho, g.Ns,
+      (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns,
       g.omega, g.prefetch_pull);
 }
 template <typename L, typename ST>
@@ -400,14 +407,14 @@ static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStre
 template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
   k_aa_odd<L, ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
-      (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
+      (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns, g.omega, g.prefetch_aa);
 }
 template <typename L, typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (!odd) {
     k_aa_even<L, ST><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
-        (ST*)a, g.nbr, g.iolet_bits, g.iolet_rho, g.Ns, g.omega, g.prefetch_aa);
+        (ST*)a, g.nbr, g.iolet_bits, g.iolet_par, g.Ns, g.omega, g.prefetch_aa);
   } else if (g.use_rec) {
     if (idx32) aa_odd_launch<L, ST, true, uint32_t>(g, a, s);
     else aa_odd_launch<L, ST, true, long long>(g, a, s);

@@ -5,6 +5,7 @@ Bar (BASELINE.json north_star): fp64 rho and u within 1e-12 relative max error, 
 fp32-storage variant within 1e-5. Norm (reading R-norm):
 E_rho = max|rho - rho_ref| / max|rho_ref|,  E_u = max_{x,a}|u_a - u_ref,a| / max_x |u_ref|_2.
 """
+import math
 import os
 
 import numpy as np
@@ -51,6 +52,8 @@ def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto", lattice
         assert g.hlb_uses_records() == (links == "records")
     if wl.rho0 is not None or wl.u0 is not None:
         g.hlb_set_state(wl.rho0, wl.u0)
+    if wl.iolet_kind is not None:
+        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
     g.hlb_step(steps)
     assert g.hlb_steps_done() == steps
     out = g.hlb_get_macroscopic()
@@ -211,6 +214,60 @@ def test_d3q19_populations_match_oracle(hlb, scheme):
     o.step(5)
     g.hlb_step(5)
     assert np.max(np.abs(g.hlb_get_populations()[:, perm] - o.get_populations())) < 1e-15
+    g.close()
+
+
+# ------------------------------------------------------------- Ladd velocity iolets (NEXT-2)
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+@pytest.mark.parametrize("name", ["pipe", "aneurysm", "tree"])
+def test_velocity_inlet_matches_oracle(hlb, name, scheme, lattice):
+    """The paper's boundary set: Ladd velocity inlet + constant-density
+    outlets, both storage types, even and odd step counts."""
+    wl = W.with_velocity_inlet(W.by_name(name, small=True))
+    for steps, store, order, links in ((wl.steps, "f64", "raster", "records"),
+                                       (wl.steps + 1, "f64", "morton", "table"),
+                                       (wl.steps + 1, "f32", "raster", "auto")):
+        rho_ref, u_ref = run_oracle(wl, steps, lattice=lattice)
+        rho, u = run_gpu(hlb, wl, steps, scheme, store, order, links, lattice)
+        e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+        assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
+    assert np.max(np.abs(u_ref)) > 1e-4                     # the inlet does drive a flow
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_time_varying_velocity_inlet_and_mixed_kinds(hlb, scheme):
+    """A pulsatile inlet (the paper drives its inlet with a velocity waveform, Fig. 8): the
+    velocity changes between hlb_step calls; random masks mix walls, density and velocity
+    iolets on one site. Also switching an iolet back to the density rule."""
+    wl = W.random_mask((14, 12, 10), p_fluid=0.65, n_iolets=3, p_iolet=0.07, periodic=2, tau=0.62,
+                       seed=91)
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho)
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, scheme, "f64", "raster", "auto"))
+    o.set_state(wl.rho0, wl.u0)
+    g.hlb_set_state(wl.rho0, wl.u0)
+    rng = np.random.default_rng(4)
+    for it in range(6):
+        kind = np.array([1, it % 2, 1 - it % 2], dtype=np.uint8)
+        u = 0.02 * math.sin(0.9 * it + 0.3) * (rng.random((3, 3)) - 0.5)
+        o.set_iolet_velocity(kind, u)
+        g.hlb_set_iolet_velocity(kind, u)
+        n = 3 + it
+        o.step(n)
+        g.hlb_step(n)
+        e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())
+        assert e_rho < 1e-13 and e_u < 1e-12, (it, e_rho, e_u)
+    g.hlb_set_iolet_velocity(None, None)                    # all back to constant density
+    g.hlb_set_iolet_density([1.01, 0.99, 1.0])
+    o2 = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, [1.01, 0.99, 1.0])
+    o2.set_populations(o.get_populations())
+    o2.step(7)
+    g.hlb_step(7)
+    e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o2.get_macroscopic())
+    assert e_rho < 1e-13 and e_u < 1e-12
+    with pytest.raises(hlb.HlbError):
+        g.hlb_set_iolet_velocity([2, 0, 0], np.zeros((3, 3)))
     g.close()
 
 
