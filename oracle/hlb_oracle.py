@@ -73,6 +73,8 @@ def _load():
                                  ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                  ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_get_stress.restype = None
+        lib.hlbo_get_stress.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbo_set_iolet_velocity.restype = None
         lib.hlbo_set_iolet_velocity.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbd_run_ladd.restype = ctypes.c_int
@@ -173,6 +175,12 @@ class Oracle:
 
     def steps_done(self):
         return int(self._lib.hlbo_steps_done(self._h))
+
+    def get_stress(self):
+        """Deviatoric stress [N, 6] (xx, yy, zz, xy, xz, yz) of the pre-collision state."""
+        sg = np.zeros((self.n_sites, 6), dtype=np.float64)
+        self._lib.hlbo_get_stress(self._h, _ptr(sg))
+        return sg
 
     def get_macroscopic(self):
         rho = np.zeros(self.n_sites, dtype=np.float64)

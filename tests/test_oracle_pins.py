@@ -358,6 +358,59 @@ def test_ladd_velocity_at_rest_is_plain_bounce_back():
     assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
 
 
+# ------------------------------------------------------------------ viscous stress read-out
+@pytest.mark.parametrize("tau", [0.6, 0.8, 1.4])
+def test_stress_of_couette_flow_is_rho_nu_shear_rate(tau):
+    """sigma_ab = -(1 - 1/(2 tau)) sum_q c_a c_b (f_q - f_eq_q). In steady plane Couette flow
+    (exact in LBGK, see the Ladd pin) the shear stress is rho nu dU/dy at every site: pins the
+    prefactor, the sign and the component order (xy is component 3)."""
+    H, U = 8, 0.01
+    st = np.zeros((1, H + 2, 1), dtype=np.uint8)
+    st[0, 1:H + 1, 0] = 1
+    st[0, H + 1, 0] = 2
+    o = oracle.Oracle(st, 5, tau, [1.0])
+    o.set_iolet_velocity([1], [[U, 0.0, 0.0]])
+    o.step(int(60 * H * H / ((tau - 0.5) / 3.0) / 10))
+    sg = o.get_stress()
+    nu = (tau - 0.5) / 3.0
+    assert sg.shape == (H, 6)
+    assert np.max(np.abs(sg[:, 3] / (nu * U / H) - 1.0)) < 1e-11
+    assert np.max(np.abs(sg[:, [4, 5]])) < 1e-18                     # no xz, yz shear
+    assert np.max(np.abs(sg[:, :3])) < 10.0 * (U / H) ** 2           # normal stresses: O(shear^2)
+
+
+def test_stress_of_poiseuille_flow_is_linear_and_balances_the_pressure_gradient():
+    tau, H, L = 0.9, 11, 24
+    st = np.zeros((L + 2, H + 2, 1), dtype=np.uint8)
+    st[1:L + 1, 1:H + 1, 0] = 1
+    st[0, 1:H + 1, 0] = 2
+    st[L + 1, 1:H + 1, 0] = 3
+    o = oracle.Oracle(st, 1, tau, [1.0005, 0.9995], threads=4)
+    o.step(8000)
+    rho, _ = o.get_macroscopic()
+    sg = o.get_stress()
+    x, y, z = canon_coords(st)
+    G = (rho[z == 9].mean() - rho[z == 16].mean()) / (3.0 * 7)     # -dp/dz on the mid-section
+    mid = z == 12
+    yy = y[mid].astype(float)
+    expect = -G * (yy - (H + 1) / 2.0)                             # momentum balance d sigma_yz/dy = -G
+    got = sg[mid, 5]
+    off = yy != (H + 1) / 2.0
+    assert np.max(np.abs(got[off] / expect[off] - 1.0)) < 5e-3
+    assert abs(got[~off][0]) < 1e-3 * np.max(np.abs(expect))         # zero on the centre line
+    assert np.max(np.abs(got + got[::-1])) < 1e-12 * np.max(np.abs(got))   # antisymmetric
+
+
+def test_stress_vanishes_at_equilibrium():
+    st = np.ones((4, 5, 6), dtype=np.uint8)
+    o = oracle.Oracle(st, 7, 0.7, [])
+    n = o.n_sites
+    o.set_state(np.full(n, 1.02), np.tile(np.array([0.03, -0.02, 0.01]), (n, 1)))
+    assert np.max(np.abs(o.get_stress())) < 1e-17
+    o.step(9)
+    assert np.max(np.abs(o.get_stress())) < 1e-17
+
+
 # ------------------------------------------------------------------ P9 dense twin
 @pytest.mark.parametrize("seed,periodic,shape", [
     (0, 0, (7, 6, 5)), (1, 7, (6, 6, 6)), (2, 1, (12, 5, 4)), (3, 2, (4, 9, 5)),
