@@ -144,6 +144,15 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u);
 /* Same, into DEVICE buffers (rho [N], u [N][3]); enqueued on the stream, no sync. */
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);
 
+/* Deviatoric (viscous) stress tensor of the same pre-collision state,
+ *     sigma_ab(x) = -(1 - 1/(2 tau)) sum_q c_qa c_qb (f_q - f_eq_q(rho, u)),
+ * the quantity wall shear stress is derived from ("pressure and velocity", PAPER.md line 27;
+ * the pressure itself is rho / 3), canonical order, HOST [N][6] in the order xx, yy, zz, xy,
+ * xz, yz. Synchronises the stream. The first call allocates a staging buffer through the
+ * allocator (as hlb_get_populations). hlb_get_stress_device: DEVICE [N][6], no sync. */
+int hlb_get_stress(hlb_geometry* g, double* sigma);
+int hlb_get_stress_device(hlb_geometry* g, double* sigma_dev);
+
 /* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][Q], canonical site
  * order, q in the order of hlb_lattice(). For population-level parity checks. The
  * first call of this or of hlb_set_populations allocates a [N][Q] fp64 staging buffer

@@ -61,6 +61,8 @@ def _load() -> ctypes.CDLL:
         "hlb_get_macroscopic": (c_int, [vp, vp, vp]),
         "hlb_get_macroscopic_device": (c_int, [vp, vp, vp]),
         "hlb_get_populations": (c_int, [vp, vp]),
+        "hlb_get_stress": (c_int, [vp, vp]),
+        "hlb_get_stress_device": (c_int, [vp, vp]),
         "hlb_set_populations": (c_int, [vp, vp]),
         "hlb_num_sites": (i64, [vp]),
         "hlb_num_q": (c_int, [vp]),
@@ -91,6 +93,7 @@ _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_set_iolet_velocity", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
+            "hlb_get_stress", "hlb_get_stress_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
             "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
@@ -245,6 +248,18 @@ class Geometry:
         u = torch.empty((self.n_sites, 3), dtype=torch.float64, device=self.device)
         _check(_lib.hlb_get_macroscopic_device(self._h, rho.data_ptr(), u.data_ptr()))
         return rho, u
+
+    def hlb_get_stress(self):
+        """Deviatoric stress [N, 6] (xx, yy, zz, xy, xz, yz), host."""
+        sg = np.empty((self.n_sites, 6), dtype=np.float64)
+        _check(_lib.hlb_get_stress(self._h, _ptr(sg)))
+        return sg
+
+    def hlb_get_stress_device(self):
+        torch = self._torch
+        sg = torch.empty((self.n_sites, 6), dtype=torch.float64, device=self.device)
+        _check(_lib.hlb_get_stress_device(self._h, sg.data_ptr()))
+        return sg
 
     def hlb_get_populations(self):
         f = np.empty((self.n_sites, self.n_q), dtype=np.float64)

@@ -458,6 +458,24 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u) {
   return HLB_OK;
 }
 
+int hlb_get_stress_device(hlb_geometry* g, double* sigma_dev) {
+  if (!g || !sigma_dev) return fail(HLB_EINVAL, "NULL argument");
+  launch_stress(g->dg, g->state_buf(), g->gather_mode(), sigma_dev, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  return HLB_OK;
+}
+
+int hlb_get_stress(hlb_geometry* g, double* sigma) {
+  if (!g || !sigma) return fail(HLB_EINVAL, "NULL argument");
+  int rc = ensure_scratch_pop(g);  // [N][Q >= 15] doubles hold [N][6]
+  if (rc) return rc;
+  rc = hlb_get_stress_device(g, g->scratch_pop);
+  if (rc) return rc;
+  HLB_CUDA(cudaMemcpyAsync(sigma, g->scratch_pop, sizeof(double) * 6 * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
 int hlb_get_populations(hlb_geometry* g, double* f) {
   if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
   int rc = ensure_scratch_pop(g);

@@ -316,6 +316,37 @@ k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
   }
 }
 
+// Deviatoric (viscous) stress of the pre-collision state, canonical order, [N][6] in the
+// order xx, yy, zz, xy, xz, yz:  sigma_ab = -(1 - omega / 2) sum_q c_qa c_qb (h_q - heq_q)
+// (the shift w_q cancels in h - heq).
+template <typename L, typename ST, int MODE>
+__global__ void __launch_bounds__(BLOCK)
+k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
+         const int32_t* __restrict__ canon, long long N, long long Ns, double omega,
+         double* __restrict__ sigma) {
+  const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
+  if (i >= N) return;
+  double h[L::Q];
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  const Moments m = moments_of<L>(h);
+  double pi[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int q = 1; q < L::Q; ++q) {  // c_0 = 0 contributes nothing
+    const double neq = h[q] - heq_of<L>(q, m.drho, m.rho, m.ux, m.uy, m.uz);
+    const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
+    if (cx * cx) pi[0] += neq;
+    if (cy * cy) pi[1] += neq;
+    if (cz * cz) pi[2] += neq;
+    if (cx * cy) pi[3] += (cx * cy > 0 ? neq : -neq);
+    if (cx * cz) pi[4] += (cx * cz > 0 ? neq : -neq);
+    if (cy * cz) pi[5] += (cy * cz > 0 ? neq : -neq);
+  }
+  const double pref = -(1.0 - 0.5 * omega);
+  const long long c = canon[i];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) sigma[c * 6 + k] = pref * pi[k];
+}
+
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
@@ -446,6 +477,17 @@ static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMo
   }
 }
 template <typename L, typename ST>
+static void stress_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
+                     cudaStream_t s) {
+  const unsigned grid = grid_for(g.N);
+  const ST* b = (const ST*)buf;
+  switch (mode) {
+    case GATHER_PULL: k_stress<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_OWN: k_stress<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_AA_ODD: k_stress<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+  }
+}
+template <typename L, typename ST>
 static void init_t(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
                    const double* u_in, const double* f_in, cudaStream_t s) {
   const unsigned grid = grid_for(g.Ns);
@@ -480,6 +522,10 @@ void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mod
 void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
                             cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { get_populations_t<decltype(l), decltype(st)>(g, buf, mode, f, s); });
+}
+void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
+                   cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, sigma, s); });
 }
 void launch_init(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
                  const double* u_in, const double* f_in, cudaStream_t s) {

@@ -43,6 +43,9 @@ enum GatherMode {
 // rho [N] / u [N][3] (device, canonical order; either may be NULL)
 void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
                         double* u, cudaStream_t s);
+// sigma [N][6] deviatoric stress xx, yy, zz, xy, xz, yz (device, canonical order)
+void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
+                   cudaStream_t s);
 // f [N][Q] raw populations (device, canonical order)
 void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
                             cudaStream_t s);

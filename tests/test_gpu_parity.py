@@ -271,6 +271,45 @@ def test_time_varying_velocity_inlet_and_mixed_kinds(hlb, scheme):
     g.close()
 
 
+# ------------------------------------------------------------- stress read-out (NEXT-3)
+STRESS_TOL = {"f64": 1e-9, "f32": 1e-3}   # f_neq is ~1e-3 of h, so the
+                                          # population-level 1e-15 / 1e-7 is amplified ~1e3 x
+
+
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_stress_matches_oracle(hlb, scheme, lattice):
+    """Deviatoric stress tensor of the pre-collision state, every site and component, after
+    even and odd step counts (A-A reads it through the table after odd counts)."""
+    wl = W.with_velocity_inlet(W.by_name("aneurysm", small=True), u_in=0.01)
+    for store in ("f64", "f32"):
+        o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, lattice=lattice, threads=0)
+        o.set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+        g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                    flags_of(hlb, scheme, store, "raster", "auto", lattice))
+        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+        for n in (60, 41):
+            o.step(n)
+            g.hlb_step(n)
+            ref, got = o.get_stress(), g.hlb_get_stress()
+            scale = np.max(np.abs(ref))
+            assert scale > 1e-7
+            assert np.max(np.abs(got - ref)) / scale < STRESS_TOL[store], (store, n)
+            assert np.array_equal(g.hlb_get_stress_device().cpu().numpy(), got)
+        g.close()
+
+
+def test_stress_is_zero_at_rest_and_uniform_flow(hlb):
+    st = np.ones((6, 5, 4), dtype=np.uint8)
+    g = hlb.hlb_geometry_create(st, 7, 0.7, [])
+    assert np.all(g.hlb_get_stress() == 0.0)
+    n = g.n_sites
+    g.hlb_set_state(np.full(n, 1.02), np.tile(np.array([0.03, -0.02, 0.01]), (n, 1)))
+    g.hlb_step(5)
+    assert np.max(np.abs(g.hlb_get_stress())) < 1e-17
+    g.close()
+
+
 # ------------------------------------------------------------- random masks, every BC at once
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
 @pytest.mark.parametrize("seed,periodic,shape", [
