@@ -73,12 +73,17 @@ def _load():
                                  ctypes.c_uint, ctypes.c_double, ctypes.c_int, ctypes.c_void_p,
                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                  ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_set_wall_distance.restype = None
+        lib.hlbo_set_wall_distance.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbo_get_stress.restype = None
         lib.hlbo_get_stress.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbo_set_iolet_velocity.restype = None
         lib.hlbo_set_iolet_velocity.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbd_run_ladd.restype = ctypes.c_int
         lib.hlbd_run_ladd.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p, ctypes.c_void_p] + \
+            lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
+        lib.hlbd_run_bfl.restype = ctypes.c_int
+        lib.hlbd_run_bfl.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 3 + \
             lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
         lib.hlbd_run_lattice.restype = ctypes.c_int
         lib.hlbd_run_lattice.argtypes = lib.hlbd_run.argtypes + [ctypes.c_int]
@@ -176,6 +181,14 @@ class Oracle:
     def steps_done(self):
         return int(self._lib.hlbo_steps_done(self._h))
 
+    def set_wall_distance(self, d27):
+        """BFL wall distances [N, 27] (canonical order; entry (dz+1)*9+(dy+1)*3+(dx+1) = fraction
+        of the link along (dx,dy,dz) at which the wall sits, <= 0: none) or None (off)."""
+        if d27 is not None:
+            d27 = np.ascontiguousarray(d27, dtype=np.float64)
+            assert d27.shape == (self.n_sites, 27)
+        self._lib.hlbo_set_wall_distance(self._h, _ptr(d27))
+
     def get_stress(self):
         """Deviatoric stress [N, 6] (xx, yy, zz, xy, xz, yz) of the pre-collision state."""
         sg = np.zeros((self.n_sites, 6), dtype=np.float64)
@@ -197,6 +210,8 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
         o.set_state(workload.rho0, workload.u0)
     if getattr(workload, "iolet_kind", None) is not None:
         o.set_iolet_velocity(workload.iolet_kind, workload.iolet_u)
+    if getattr(workload, "wall_distance", None) is not None:
+        o.set_wall_distance(workload.wall_distance)
     o.step(workload.steps if steps is None else steps)
     out = o.get_macroscopic()
     o.close()
@@ -204,7 +219,7 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
 
 
 def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None,
-              lattice="d3q15", iolet_kind=None, iolet_u=None):
+              lattice="d3q15", iolet_kind=None, iolet_u=None, wall_d27_vox=None):
     """Dense-grid twin: per-VOXEL rho [nz,ny,nx] and u [nz,ny,nx,3]."""
     lib = _load()
     st = np.ascontiguousarray(site_type, dtype=np.uint8)
@@ -218,9 +233,12 @@ def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=
         np.ascontiguousarray(np.asarray(iolet_kind, dtype=np.uint8).reshape(-1))
     uio = None if iolet_u is None else \
         np.ascontiguousarray(np.asarray(iolet_u, dtype=np.float64).reshape(-1, 3))
-    rc = lib.hlbd_run_ladd(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
-                           _ptr(io), _ptr(kind), _ptr(uio), _ptr(r0), _ptr(u0), int(steps),
-                           _ptr(rho), _ptr(u), LATTICE_Q[lattice])
+    wd = None if wall_d27_vox is None else np.ascontiguousarray(wall_d27_vox, dtype=np.float64)
+    if wd is not None:
+        assert wd.shape == (nz * ny * nx, 27)
+    rc = lib.hlbd_run_bfl(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
+                          _ptr(io), _ptr(kind), _ptr(uio), _ptr(wd), _ptr(r0), _ptr(u0), int(steps),
+                          _ptr(rho), _ptr(u), LATTICE_Q[lattice])
     if rc != 0:
         raise ValueError("hlbd_run rejected its arguments")
     return rho, u

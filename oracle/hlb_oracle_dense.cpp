@@ -15,6 +15,9 @@
 //     d solid   : f_opp(q)(x, t+1) = f*_q(x, t)
 //     d iolet k : f_opp(q)(x, t+1) = feq_opp(q)(rho_k, u(x, t))
 //     d velocity iolet k (Ladd): f_opp(q)(x, t+1) = f*_q(x, t) - 6 w_q rho(x, t) c_q.u_k
+//     d solid with a BFL wall distance wd along c_q and b = x - c_q fluid:
+//         wd < 1/2 : f_opp(q)(x, t+1) = 2 wd f*_q(x,t) + (1 - 2 wd) f*_q(b,t)
+//         wd >= 1/2: f_opp(q)(x, t+1) = f*_q(x,t)/(2 wd) + (1 - 1/(2 wd)) f*_opp(q)(x,t)
 // which is the pull rule of hlb_oracle.cpp read from the other end of the link.
 
 #include <cstdint>
@@ -66,8 +69,9 @@ extern "C" {
 // Returns 0, or -1 on a bad argument.
 static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
                          int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
-                         const double* iolet_u, const double* rho0, const double* u0,
-                         int64_t steps, double* rho_out, double* u_out, int lattice_q) {
+                         const double* iolet_u, const double* wall_d27, const double* rho0,
+                         const double* u0, int64_t steps, double* rho_out, double* u_out,
+                         int lattice_q) {
   if (lattice_q != 15 && lattice_q != 19) return -1;
   const Lattice& L = lattice_q == 15 ? L15 : L19;
   const int Q = L.Q;
@@ -85,33 +89,62 @@ static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned p
                      uz = u0 ? u0[v * 3 + 2] : 0.0;
         for (int q = 0; q < Q; ++q) f[v * Q + q] = feq(L, q, r, ux, uy, uz);
       }
+  auto wrap = [&](int& cx_, int& cy_, int& cz_) {  // returns true if outside a non-periodic box
+    bool outside = false;
+    if (cx_ < 0) { if (periodic & 1u) cx_ += nx; else outside = true; }
+    if (cx_ >= nx) { if (periodic & 1u) cx_ -= nx; else outside = true; }
+    if (cy_ < 0) { if (periodic & 2u) cy_ += ny; else outside = true; }
+    if (cy_ >= ny) { if (periodic & 2u) cy_ -= ny; else outside = true; }
+    if (cz_ < 0) { if (periodic & 4u) cz_ += nz; else outside = true; }
+    if (cz_ >= nz) { if (periodic & 4u) cz_ -= nz; else outside = true; }
+    return outside;
+  };
+  std::vector<double> fs((size_t)nvox * Q, 0.0), rho_v((size_t)nvox, 0.0), u_v((size_t)nvox * 3, 0.0);
   for (int64_t s = 0; s < steps; ++s) {
+    // collision of every fluid voxel
+    for (int64_t v = 0; v < nvox; ++v) {
+      if (type[v] != 1) continue;
+      const double* fv = &f[v * Q];
+      double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
+      for (int q = 0; q < Q; ++q) {
+        rho += fv[q]; jx += CX[q] * fv[q]; jy += CY[q] * fv[q]; jz += CZ[q] * fv[q];
+      }
+      const double ux = jx / rho, uy = jy / rho, uz = jz / rho;
+      rho_v[v] = rho; u_v[v * 3 + 0] = ux; u_v[v * 3 + 1] = uy; u_v[v * 3 + 2] = uz;
+      for (int q = 0; q < Q; ++q) fs[v * Q + q] = fv[q] - (fv[q] - feq(L, q, rho, ux, uy, uz)) / tau;
+    }
+    // push
     for (int z = 0; z < nz; ++z)
       for (int y = 0; y < ny; ++y)
         for (int x = 0; x < nx; ++x) {
           const int64_t v = ((int64_t)z * ny + y) * nx + x;
           if (type[v] != 1) continue;
-          const double* fv = &f[v * Q];
-          double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
+          const double rho = rho_v[v], ux = u_v[v * 3 + 0], uy = u_v[v * 3 + 1], uz = u_v[v * 3 + 2];
           for (int q = 0; q < Q; ++q) {
-            rho += fv[q]; jx += CX[q] * fv[q]; jy += CY[q] * fv[q]; jz += CZ[q] * fv[q];
-          }
-          const double ux = jx / rho, uy = jy / rho, uz = jz / rho;
-          for (int q = 0; q < Q; ++q) {
-            const double fstar = fv[q] - (fv[q] - feq(L, q, rho, ux, uy, uz)) / tau;
+            const double fstar = fs[v * Q + q];
             int dx = x + CX[q], dy = y + CY[q], dz = z + CZ[q];
-            bool outside = false;
-            if (dx < 0) { if (periodic & 1u) dx += nx; else outside = true; }
-            if (dx >= nx) { if (periodic & 1u) dx -= nx; else outside = true; }
-            if (dy < 0) { if (periodic & 2u) dy += ny; else outside = true; }
-            if (dy >= ny) { if (periodic & 2u) dy -= ny; else outside = true; }
-            if (dz < 0) { if (periodic & 4u) dz += nz; else outside = true; }
-            if (dz >= nz) { if (periodic & 4u) dz -= nz; else outside = true; }
+            const bool outside = wrap(dx, dy, dz);
             const int64_t d = outside ? -1 : ((int64_t)dz * ny + dy) * nx + dx;
             const int t = outside ? 0 : (int)type[d];
             if (t == 1) g[d * Q + q] = fstar;
-            else if (t == 0) g[v * Q + OPP[q]] = fstar;
-            else {
+            else if (t == 0) {
+              // wall along c_q. BFL (linear) if a distance is given and the voxel behind,
+              // x - c_q, is fluid; halfway bounce-back otherwise.
+              double wd = 0.0;
+              if (wall_d27) {
+                const double w27 = wall_d27[v * 27 + (CZ[q] + 1) * 9 + (CY[q] + 1) * 3 + (CX[q] + 1)];
+                if (w27 > 0.0 && w27 <= 1.0) wd = w27;
+              }
+              int bx = x - CX[q], by = y - CY[q], bz = z - CZ[q];
+              const bool b_out = wrap(bx, by, bz);
+              const int64_t b = b_out ? -1 : ((int64_t)bz * ny + by) * nx + bx;
+              if (wd > 0.0 && b >= 0 && type[b] == 1) {
+                if (wd < 0.5) g[v * Q + OPP[q]] = 2.0 * wd * fstar + (1.0 - 2.0 * wd) * fs[b * Q + q];
+                else g[v * Q + OPP[q]] = fstar / (2.0 * wd) + (1.0 - 1.0 / (2.0 * wd)) * fs[v * Q + OPP[q]];
+              } else {
+                g[v * Q + OPP[q]] = fstar;
+              }
+            } else {
               if (t - 2 >= n_iolets) return -1;
               const int k = t - 2;
               if (iolet_kind && iolet_kind[k] == 1) {
@@ -146,17 +179,26 @@ static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned p
 int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
                      int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
                      int64_t steps, double* rho_out, double* u_out, int lattice_q) {
-  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, nullptr, nullptr, rho0,
-                       u0, steps, rho_out, u_out, lattice_q);
+  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, nullptr, nullptr, nullptr,
+                       rho0, u0, steps, rho_out, u_out, lattice_q);
 }
 
-// iolet_kind [n_iolets]: 0 constant density, 1 Ladd velocity with iolet_u [n_iolets][3]
+// iolet_kind [n_iolets]: 0 constant density, 1 Ladd velocity with iolet_u [n_iolets][3];
+// wall_d27 per VOXEL [nvox][27]: BFL wall distance along (dx,dy,dz) at (dz+1)*9+(dy+1)*3+(dx+1),
+// <= 0 none; NULL: plain bounce-back everywhere.
 int hlbd_run_ladd(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
                   int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
                   const double* iolet_u, const double* rho0, const double* u0, int64_t steps,
                   double* rho_out, double* u_out, int lattice_q) {
   return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
-                       rho0, u0, steps, rho_out, u_out, lattice_q);
+                       nullptr, rho0, u0, steps, rho_out, u_out, lattice_q);
+}
+int hlbd_run_bfl(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                 int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
+                 const double* iolet_u, const double* wall_d27, const double* rho0,
+                 const double* u0, int64_t steps, double* rho_out, double* u_out, int lattice_q) {
+  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
+                       wall_d27, rho0, u0, steps, rho_out, u_out, lattice_q);
 }
 
 int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,

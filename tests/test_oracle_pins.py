@@ -358,6 +358,88 @@ def test_ladd_velocity_at_rest_is_plain_bounce_back():
     assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
 
 
+# ------------------------------------------------------------------ BFL interpolated walls
+def _d27_index(dx, dy, dz):
+    return (dz + 1) * 9 + (dy + 1) * 3 + (dx + 1)
+
+
+@pytest.mark.parametrize("tau", [0.6, 1.0])
+@pytest.mark.parametrize("d", [0.15, 0.5, 0.8, 1.0])
+def test_bfl_wall_off_the_lattice_gives_exact_couette_flow(d, tau):
+    """Interpolated bounce-back ("BFL", ref [16]): the lower wall sits
+    the fraction d of a link below the first fluid row (at y = 1 - d, for every link that
+    crosses it, axis or diagonal), the upper boundary is a Ladd wall moving with U at
+    y = H + 1/2. Linear interpolation represents the linear Couette profile exactly:
+    u_x(y) = U (y - y_w) / (H + 1/2 - y_w). Plain bounce-back would put the wall at y = 1/2."""
+    H, U = 8, 0.01
+    st = np.zeros((1, H + 2, 1), dtype=np.uint8)
+    st[0, 1:H + 1, 0] = 1
+    st[0, H + 1, 0] = 2
+    o = oracle.Oracle(st, 5, tau, [1.0])
+    o.set_iolet_velocity([1], [[U, 0.0, 0.0]])
+    d27 = np.zeros((H, 27))
+    for dz in (-1, 0, 1):
+        for dx in (-1, 0, 1):
+            d27[0, _d27_index(dx, -1, dz)] = d          # links of row y = 1 that point down
+    o.set_wall_distance(d27)
+    o.step(int(80 * H * H / ((tau - 0.5) / 3.0) / 10))
+    _, u = o.get_macroscopic()
+    y = np.arange(1, H + 1)
+    yw = 1.0 - d
+    assert np.max(np.abs(u[:, 0] - U * (y - yw) / (H + 0.5 - yw))) < 2e-12 * U / 0.01
+    if d != 0.5:                                           # and it is not the halfway answer
+        assert np.max(np.abs(u[:, 0] - U * (y - 0.5) / H)) > 1e-5
+
+
+def test_bfl_at_half_a_link_is_plain_bounce_back_bitwise():
+    wl = W.random_mask((9, 8, 7), p_fluid=0.6, n_iolets=2, p_iolet=0.06, periodic=1, seed=31)
+    a = oracle.Oracle(wl.site_type, 1, wl.tau, wl.iolet_rho)
+    b = oracle.Oracle(wl.site_type, 1, wl.tau, wl.iolet_rho)
+    b.set_wall_distance(np.full((b.n_sites, 27), 0.5))
+    for o in (a, b):
+        o.set_state(wl.rho0, wl.u0)
+        o.step(15)
+    assert np.array_equal(a.get_populations(), b.get_populations())
+    b.set_wall_distance(None)                               # switching it off again
+    a.step(3)
+    b.step(3)
+    assert np.array_equal(a.get_populations(), b.get_populations())
+
+
+@pytest.mark.parametrize("seed,periodic,shape", [(0, 0, (7, 6, 5)), (1, 7, (6, 6, 6)), (2, 1, (12, 5, 4)),
+                                                 (3, 4, (5, 4, 11)), (4, 0, (12, 12, 12))])
+def test_bfl_dense_push_twin_equals_sparse_pull(seed, periodic, shape):
+    """The independently written dense push implementation, with random wall distances on
+    every link (used only where the link is a wall link), velocity iolets mixed in."""
+    wl = W.random_mask(shape, p_fluid=0.65, n_iolets=2, p_iolet=0.06, periodic=periodic,
+                       tau=0.6 + 0.1 * seed, seed=400 + seed)
+    st, vox = wl.site_type, wl.fluid_voxels()
+    rng = np.random.default_rng(seed)
+    d27 = rng.uniform(0.02, 1.0, size=(len(vox), 27))
+    d27[rng.random(d27.shape) < 0.2] = 0.0                   # some links without a distance
+    d27_vox = np.zeros((st.size, 27))
+    d27_vox[vox] = d27
+    rho0v, u0v = np.ones(st.size), np.zeros((st.size, 3))
+    rho0v[vox], u0v[vox] = wl.rho0, wl.u0
+    kind, uio = np.array([1, 0], dtype=np.uint8), 0.02 * (rng.random((2, 3)) - 0.5)
+    steps = 10
+    rd, ud = oracle.dense_run(st, periodic, wl.tau, wl.iolet_rho, steps, rho0v, u0v,
+                              iolet_kind=kind, iolet_u=uio, wall_d27_vox=d27_vox)
+    rd, ud = rd.reshape(-1)[vox], ud.reshape(-1, 3)[vox]
+    o = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho, variant=oracle.VARIANT_RAW)
+    o.set_state(wl.rho0, wl.u0)
+    o.set_iolet_velocity(kind, uio)
+    o.set_wall_distance(d27)
+    o.step(steps)
+    r, u = o.get_macroscopic()
+    assert np.max(np.abs(r - rd)) < 5e-15 and np.max(np.abs(u - ud)) < 5e-15
+    o2 = oracle.Oracle(st, periodic, wl.tau, wl.iolet_rho)    # without BFL it is another flow
+    o2.set_state(wl.rho0, wl.u0)
+    o2.set_iolet_velocity(kind, uio)
+    o2.step(steps)
+    assert np.max(np.abs(o2.get_macroscopic()[1] - u)) > 1e-6
+
+
 # ------------------------------------------------------------------ viscous stress read-out
 @pytest.mark.parametrize("tau", [0.6, 0.8, 1.4])
 def test_stress_of_couette_flow_is_rho_nu_shear_rate(tau):
