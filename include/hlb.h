@@ -118,6 +118,23 @@ int hlb_set_state(hlb_geometry* g, const double* rho, const double* u);
  * step; the density of an iolet that is currently a velocity iolet is kept for later. */
 int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho);
 
+/* Interpolated ("BFL") walls -- the paper's wall option (ref. [16]:
+ * Bouzidi, Firdaouss & Lallemand), linear form. d27: HOST [N][27] in canonical site order;
+ * entry (dz+1)*9 + (dy+1)*3 + (dx+1) is the fraction d in (0, 1] of the link from the site
+ * along the lattice vector (dx, dy, dz) at which the wall cuts it (1/2 = the halfway
+ * bounce-back default); <= 0 or > 1: no distance for that link. With i = opp(q) the direction
+ * from x to the wall and y = x + c_q the site behind x, a solid-wall link q becomes
+ *     d <  1/2:  f_q(x,t+1) = 2d f*_i(x,t) + (1 - 2d) f*_i(y,t)
+ *     d >= 1/2:  f_q(x,t+1) = f*_i(x,t) / (2d) + (1 - 1/(2d)) f*_q(x,t)
+ * where y is a fluid site; otherwise (y solid or iolet, or no distance) the link stays a
+ * halfway bounce-back (reading R-bfl). Iolet links are not affected. NULL switches
+ * the interpolation off. Only with HLB_TWO_LATTICE, and only while hlb_steps_done() == 0
+ * (after create / hlb_set_state / hlb_set_populations; it survives later hlb_set_state
+ * calls). Allocates its tables through the allocator. Errors: HLB_EINVAL, HLB_ENOMEM,
+ * HLB_ECUDA. hlb_num_bfl_sites: sites with at least one interpolated link (0 when off). */
+int hlb_set_wall_distance(hlb_geometry* g, const double* d27);
+int64_t hlb_num_bfl_sites(const hlb_geometry* g);
+
 /* Choose, per iolet, between the constant-density rule (kind 0, the default:
  * f_q(x,t+1) = f_eq_q(rho_k, u(x,t))) and Ladd's velocity rule (kind 1, the paper's
  * "LADDIOLET" boundary, ref. [15]): a link whose source voxel is a

@@ -57,6 +57,8 @@ def _load() -> ctypes.CDLL:
         "hlb_set_state": (c_int, [vp, vp, vp]),
         "hlb_set_iolet_density": (c_int, [vp, vp]),
         "hlb_set_iolet_velocity": (c_int, [vp, vp, vp]),
+        "hlb_set_wall_distance": (c_int, [vp, vp]),
+        "hlb_num_bfl_sites": (i64, [vp]),
         "hlb_step": (c_int, [vp, i64]),
         "hlb_get_macroscopic": (c_int, [vp, vp, vp]),
         "hlb_get_macroscopic_device": (c_int, [vp, vp, vp]),
@@ -91,7 +93,7 @@ def _load() -> ctypes.CDLL:
 LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
-            "hlb_set_iolet_velocity", "hlb_step",
+            "hlb_set_iolet_velocity", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
             "hlb_get_stress", "hlb_get_stress_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
@@ -229,6 +231,13 @@ class Geometry:
         kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8)
         u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64)
         _check(_lib.hlb_set_iolet_velocity(self._h, _ptr(kind), _ptr(u)))
+
+    def hlb_set_wall_distance(self, d27):
+        d27 = None if d27 is None else _host(d27, np.float64, (self.n_sites, 27))
+        _check(_lib.hlb_set_wall_distance(self._h, _ptr(d27)))
+
+    def hlb_num_bfl_sites(self) -> int:
+        return int(_lib.hlb_num_bfl_sites(self._h))
 
     def hlb_step(self, n: int = 1):
         _check(_lib.hlb_step(self._h, int(n)))

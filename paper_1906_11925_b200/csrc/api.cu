@@ -68,6 +68,8 @@ struct hlb_geometry {
   double sentinel_fraction = 0.0;     // of the (group, q) link records
   // hlb_step(n) replays a captured CUDA graph of GRAPH_STEPS steps while n allows: removes
   // the per-launch host cost that dominates small geometries (BASELINE configs[0], [2])
+  bool bfl_set = false;               // wall distances given (hlb_set_wall_distance)
+  int64_t bfl_sites = 0;              // sites with at least one interpolated link
   cudaGraphExec_t graph_exec = nullptr;
   bool graph_failed = false;
   std::vector<void*> owned;           // cudaMalloc'ed (no allocator callback)
@@ -96,6 +98,9 @@ struct hlb_geometry {
     return (steps & 1) ? GATHER_AA_ODD : GATHER_OWN;
   }
   const void* state_buf() const { return aa ? buf[0] : buf[cur]; }
+  // The BFL interpolation belongs to the propagation: it applies to every gather except the
+  // one of the freshly initialised state f(., 0), which is given, not propagated.
+  BflView bfl_view() const { return (bfl_set && steps > 0) ? dg.bfl : BflView(); }
 };
 
 extern "C" {
@@ -358,6 +363,66 @@ int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho) {
   return upload_iolets(g);
 }
 
+int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (g->aa) return fail(HLB_EINVAL, "interpolated walls need the two-lattice scheme (HLB_TWO_LATTICE)");
+  if (g->steps != 0) return fail(HLB_EINVAL, "set the wall distances before the first step (steps_done == 0)");
+  if (!d27) {
+    g->bfl_set = false;
+    return HLB_OK;
+  }
+  const int Q = g->Q;
+  const int64_t N = g->N, Ns = g->Ns;
+  const LatticeDesc& lat = lattice_desc(Q == 19);
+  // the link table and the canonical ranks live on the device only: fetch them
+  std::vector<int32_t> nbr((size_t)(Q - 1) * (size_t)Ns), canon((size_t)N);
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  HLB_CUDA(cudaMemcpy(nbr.data(), g->dg.nbr, sizeof(int32_t) * nbr.size(), cudaMemcpyDeviceToHost));
+  HLB_CUDA(cudaMemcpy(canon.data(), g->dg.canon, sizeof(int32_t) * canon.size(), cudaMemcpyDeviceToHost));
+  std::vector<uint32_t> bits((size_t)(Ns / 32), 0u);
+  std::vector<int32_t> base((size_t)(Ns / 32), 0);
+  std::vector<double> d;
+  std::vector<double> row((size_t)(Q - 1));
+  int32_t rows = 0;
+  for (int64_t i = 0; i < N; ++i) {
+    if ((i & 31) == 0) base[(size_t)(i >> 5)] = rows;
+    bool any = false;
+    for (int p = 1; p < Q; ++p) {
+      row[(size_t)(p - 1)] = 0.0;
+      const int32_t e = nbr[(size_t)(p - 1) * (size_t)Ns + (size_t)i];
+      const int32_t behind = nbr[(size_t)(opp(p) - 1) * (size_t)Ns + (size_t)i];
+      if (e != (int32_t)NBR_WALL_BIT || behind < 0) continue;  // not a solid-wall link, or no fluid site behind
+      // the wall lies along -c_p
+      const int idx = (-lat.c[p][2] + 1) * 9 + (-lat.c[p][1] + 1) * 3 + (-lat.c[p][0] + 1);
+      const double dd = d27[(size_t)canon[(size_t)i] * 27 + (size_t)idx];
+      if (dd > 0.0 && dd <= 1.0) { row[(size_t)(p - 1)] = dd; any = true; }
+    }
+    if (any) {
+      bits[(size_t)(i >> 5)] |= 1u << (i & 31);
+      d.insert(d.end(), row.begin(), row.end());
+      ++rows;
+    }
+  }
+  for (int64_t gi = (N + 31) / 32; gi < Ns / 32; ++gi) base[(size_t)gi] = rows;
+  if (d.empty()) d.assign((size_t)(Q - 1), 0.0);
+  void *d_bits = nullptr, *d_base = nullptr, *d_d = nullptr;
+  int rc;
+  if ((rc = g->alloc(sizeof(uint32_t) * bits.size(), &d_bits))) return rc;
+  if ((rc = g->alloc(sizeof(int32_t) * base.size(), &d_base))) return rc;
+  if ((rc = g->alloc(sizeof(double) * d.size(), &d_d))) return rc;
+  HLB_CUDA(cudaMemcpy(d_bits, bits.data(), sizeof(uint32_t) * bits.size(), cudaMemcpyHostToDevice));
+  HLB_CUDA(cudaMemcpy(d_base, base.data(), sizeof(int32_t) * base.size(), cudaMemcpyHostToDevice));
+  HLB_CUDA(cudaMemcpy(d_d, d.data(), sizeof(double) * d.size(), cudaMemcpyHostToDevice));
+  g->dg.bfl.bits = (const uint32_t*)d_bits;
+  g->dg.bfl.base = (const int32_t*)d_base;
+  g->dg.bfl.d = (const double*)d_d;
+  g->bfl_set = true;
+  g->bfl_sites = rows;
+  return HLB_OK;
+}
+
+int64_t hlb_num_bfl_sites(const hlb_geometry* g) { return g ? (g->bfl_set ? g->bfl_sites : 0) : (int64_t)HLB_EINVAL; }
+
 int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   const int n = g->p.n_iolets;
@@ -379,7 +444,7 @@ static void enqueue_one_step(hlb_geometry* g) {
   if (g->aa) {
     launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
   } else {
-    launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->stream);
+    launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->bfl_view(), g->stream);
     g->cur ^= 1;
   }
   ++g->steps;
@@ -416,7 +481,7 @@ int hlb_step(hlb_geometry* g, int64_t n) {
   if (n < 0) return fail(HLB_EINVAL, "n < 0");
   // graphs pay off only when a step is short next to the launch cost
   const bool want_graph = !(g->p.flags & HLB_NO_GRAPH) && !g->graph_failed && g->stream != nullptr &&
-                          g->N <= (int64_t)4 << 20;
+                          g->N <= (int64_t)4 << 20 && !g->bfl_set;  // BFL: step 0 differs
   int64_t left = n;
   while (left > 0) {
     const bool even = g->aa ? (g->steps & 1) == 0 : g->cur == 0;
@@ -440,7 +505,7 @@ int hlb_step(hlb_geometry* g, int64_t n) {
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   if (!rho_dev && !u_dev) return HLB_OK;
-  launch_macroscopic(g->dg, g->state_buf(), g->gather_mode(), rho_dev, u_dev, g->stream);
+  launch_macroscopic(g->dg, g->state_buf(), g->gather_mode(), g->bfl_view(), rho_dev, u_dev, g->stream);
   HLB_CUDA(cudaGetLastError());
   return HLB_OK;
 }
@@ -460,7 +525,7 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u) {
 
 int hlb_get_stress_device(hlb_geometry* g, double* sigma_dev) {
   if (!g || !sigma_dev) return fail(HLB_EINVAL, "NULL argument");
-  launch_stress(g->dg, g->state_buf(), g->gather_mode(), sigma_dev, g->stream);
+  launch_stress(g->dg, g->state_buf(), g->gather_mode(), g->bfl_view(), sigma_dev, g->stream);
   HLB_CUDA(cudaGetLastError());
   return HLB_OK;
 }
@@ -480,7 +545,7 @@ int hlb_get_populations(hlb_geometry* g, double* f) {
   if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
   int rc = ensure_scratch_pop(g);
   if (rc) return rc;
-  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->scratch_pop, g->stream);
+  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->bfl_view(), g->scratch_pop, g->stream);
   HLB_CUDA(cudaGetLastError());
   HLB_CUDA(cudaMemcpyAsync(f, g->scratch_pop, sizeof(double) * (size_t)g->Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));

@@ -178,17 +178,49 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
   return (__ldg(iolet_bits + (i >> 5)) >> (threadIdx.x & 31)) & 1u;
 }
 
+// BFL interpolated walls (linear Bouzidi-Firdaouss-Lallemand rule; the paper's "BFL" wall
+// option, ref [16]), applied to the gathered pre-collision values of
+// the two-lattice scheme. On entry h[p] of a wall link p holds the halfway bounce-back value
+// f*_opp(p)(x, t-1) (own slot opp(p) of src); with the wall at the fraction d of the link,
+//   d <  1/2:  h[p] = 2d h[p] + (1 - 2d) f*_opp(p)(x + c_p, t-1)   = ... h[opp(p)], gathered anyway
+//   d >= 1/2:  h[p] = h[p] / (2d) + (1 - 1/(2d)) f*_p(x, t-1)      = own slot p of src
+// d[p-1] > 0 only for wall links whose site behind, x + c_p, is fluid (the host builds it so),
+// hence h[opp(p)] is a plain fluid gather and is never itself rewritten here.
+template <typename L, typename ST>
+__device__ __forceinline__ void bfl_apply(const BflView& b, const ST* __restrict__ src, long long Ns,
+                                          long long i, double (&h)[L::Q]) {
+  const uint32_t word = __ldg(b.bits + (i >> 5));
+  const uint32_t lane = (uint32_t)(i & 31);
+  if (!((word >> lane) & 1u)) return;
+  const long long row = (long long)__ldg(b.base + (i >> 5)) + __popc(word & ((1u << lane) - 1u));
+  const double* d = b.d + row * (L::Q - 1);
+#pragma unroll
+  for (int p = 1; p < L::Q; ++p) {
+    const double dd = __ldg(d + (p - 1));
+    if (dd > 0.0) {
+      const double two_d = mul(2.0, dd);
+      if (dd < 0.5) {
+        h[p] = fma_(two_d, h[p], mul(sub(1.0, two_d), h[opp(p)]));
+      } else {
+        const double inv = __ddiv_rn(1.0, two_d);
+        h[p] = fma_(inv, h[p], mul(sub(1.0, inv), to_real(src[(long long)p * Ns + i])));
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------ two-lattice pull
 // src holds post-collision values h*(., t-1) (iolet slots substituted); one launch does
 // gather -> moments -> BGK -> store of h*(., t) into dst (rows S1..S6 fused).
 // pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
 // of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
 // padding, so only the one warp-uniform test is needed.
-template <typename L, typename ST, bool REC, typename IT>
+template <typename L, typename ST, bool REC, typename IT, bool BFL>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
-       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf) {
+       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf,
+       BflView bfl) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[L::Q];
   {
@@ -207,6 +239,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
       for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
     }
   }
+  if (BFL) bfl_apply<L, ST>(bfl, src, Ns, i, h);
   const Moments m = moments_of<L>(h);
   collide<L>(h, m, omega, h);
   if (has_iolet_link(iolet_bits, i)) {  // rare: sites on an inlet/outlet cap
@@ -288,24 +321,26 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 template <typename L, typename ST, int MODE>
 __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
                                                     const int32_t* __restrict__ nbr, long long Ns,
-                                                    long long i, double (&h)[L::Q]) {
+                                                    long long i, const BflView& bfl,
+                                                    double (&h)[L::Q]) {
   int32_t e[L::Q - 1];
   if (MODE != GATHER_OWN) load_entries<L>(nbr, Ns, i, e);
   h[0] = to_real(buf[i]);
 #pragma unroll
   for (int q = 1; q < L::Q; ++q)
     h[q] = to_real(buf[slot_of<MODE>(q, MODE != GATHER_OWN ? e[q - 1] : 0, Ns, i)]);
+  if (MODE == GATHER_PULL && bfl.bits) bfl_apply<L, ST>(bfl, buf, Ns, i, h);
 }
 
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
-              const int32_t* __restrict__ canon, long long N, long long Ns,
+              const int32_t* __restrict__ canon, long long N, long long Ns, BflView bfl,
               double* __restrict__ rho, double* __restrict__ u) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, bfl, h);
   const Moments m = moments_of<L>(h);
   const long long c = canon[i];
   if (rho) rho[c] = m.rho;
@@ -322,12 +357,12 @@ k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
-         const int32_t* __restrict__ canon, long long N, long long Ns, double omega,
+         const int32_t* __restrict__ canon, long long N, long long Ns, double omega, BflView bfl,
          double* __restrict__ sigma) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, bfl, h);
   const Moments m = moments_of<L>(h);
   double pi[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
@@ -350,12 +385,12 @@ k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
-                  const int32_t* __restrict__ canon, long long N, long long Ns,
+                  const int32_t* __restrict__ canon, long long N, long long Ns, BflView bfl,
                   double* __restrict__ f) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, bfl, h);
   const long long c = canon[i];
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) f[c * L::Q + q] = h[q] + L::weight(q);
@@ -419,20 +454,28 @@ int resident_sites_per_sm_aa(bool d3q19) {
 
 // ------------------------------------------------------------------ launchers
 template <typename L, typename ST, bool REC, typename IT>
-static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  k_pull<L, ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
-      (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns,
-      g.omega, g.prefetch_pull);
+static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
+                        cudaStream_t s) {
+  const unsigned grid = (unsigned)(g.Ns / SBLOCK);
+  if (bfl.bits)
+    k_pull<L, ST, REC, IT, true><<<grid, SBLOCK, 0, s>>>(
+        (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns,
+        g.omega, g.prefetch_pull, bfl);
+  else
+    k_pull<L, ST, REC, IT, false><<<grid, SBLOCK, 0, s>>>(
+        (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns,
+        g.omega, g.prefetch_pull, bfl);
 }
 template <typename L, typename ST>
-static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+static void pull_t(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
+                   cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (g.use_rec) {
-    if (idx32) pull_launch<L, ST, true, uint32_t>(g, src, dst, s);
-    else pull_launch<L, ST, true, long long>(g, src, dst, s);
+    if (idx32) pull_launch<L, ST, true, uint32_t>(g, src, dst, bfl, s);
+    else pull_launch<L, ST, true, long long>(g, src, dst, bfl, s);
   } else {
-    if (idx32) pull_launch<L, ST, false, uint32_t>(g, src, dst, s);
-    else pull_launch<L, ST, false, long long>(g, src, dst, s);
+    if (idx32) pull_launch<L, ST, false, uint32_t>(g, src, dst, bfl, s);
+    else pull_launch<L, ST, false, long long>(g, src, dst, bfl, s);
   }
 }
 template <typename L, typename ST, bool REC, typename IT>
@@ -455,36 +498,36 @@ static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   }
 }
 template <typename L, typename ST>
-static void macroscopic_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
-                          double* u, cudaStream_t s) {
+static void macroscopic_t(const DeviceGeometry& g, const void* buf, GatherMode mode,
+                          const BflView& bfl, double* rho, double* u, cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_macroscopic<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
-    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
-    case GATHER_AA_ODD: k_macroscopic<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_PULL: k_macroscopic<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, rho, u); break;
+    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, rho, u); break;
+    case GATHER_AA_ODD: k_macroscopic<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, rho, u); break;
   }
 }
 template <typename L, typename ST>
-static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
-                              cudaStream_t s) {
+static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMode mode,
+                              const BflView& bfl, double* f, cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_get_populations<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
-    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
-    case GATHER_AA_ODD: k_get_populations<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_PULL: k_get_populations<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, f); break;
+    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, f); break;
+    case GATHER_AA_ODD: k_get_populations<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, f); break;
   }
 }
 template <typename L, typename ST>
-static void stress_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
-                     cudaStream_t s) {
+static void stress_t(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
+                     double* sigma, cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_stress<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
-    case GATHER_OWN: k_stress<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
-    case GATHER_AA_ODD: k_stress<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_PULL: k_stress<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, bfl, sigma); break;
+    case GATHER_OWN: k_stress<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, bfl, sigma); break;
+    case GATHER_AA_ODD: k_stress<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, bfl, sigma); break;
   }
 }
 template <typename L, typename ST>
@@ -509,23 +552,24 @@ static void dispatch(const DeviceGeometry& g, F&& f) {
   }
 }
 
-void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { pull_t<decltype(l), decltype(st)>(g, src, dst, s); });
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
+                 cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { pull_t<decltype(l), decltype(st)>(g, src, dst, bfl, s); });
 }
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { aa_t<decltype(l), decltype(st)>(g, a, odd, s); });
 }
-void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
-                        double* u, cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { macroscopic_t<decltype(l), decltype(st)>(g, buf, mode, rho, u, s); });
+void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
+                        double* rho, double* u, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { macroscopic_t<decltype(l), decltype(st)>(g, buf, mode, bfl, rho, u, s); });
 }
-void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
-                            cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { get_populations_t<decltype(l), decltype(st)>(g, buf, mode, f, s); });
+void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode,
+                            const BflView& bfl, double* f, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { get_populations_t<decltype(l), decltype(st)>(g, buf, mode, bfl, f, s); });
 }
-void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
-                   cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, sigma, s); });
+void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
+                   double* sigma, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, bfl, sigma, s); });
 }
 void launch_init(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
                  const double* u_in, const double* f_in, cudaStream_t s) {

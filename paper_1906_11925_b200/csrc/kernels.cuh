@@ -6,6 +6,15 @@
 
 namespace hlb {
 
+// BFL interpolated walls (two-lattice scheme): sites with at least one interpolated link are
+// flagged in bits [Ns/32]; their distances live in d [n_flagged][Q-1] (0 = plain bounce-back
+// for that link), row = base[group] + number of flagged lanes below. bits == nullptr: off.
+struct BflView {
+  const uint32_t* bits = nullptr;
+  const int32_t* base = nullptr;
+  const double* d = nullptr;
+};
+
 struct DeviceGeometry {
   int64_t N = 0;                        // fluid sites
   int64_t Ns = 0;                       // plane stride (multiple of 128), arrays are [Q][Ns]
@@ -13,6 +22,7 @@ struct DeviceGeometry {
   const uint32_t* iolet_bits = nullptr; // [Ns/32]
   const void* rec = nullptr;            // [Ns/32][Q-1] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
+  BflView bfl;                          // as stored; the API passes it to a launch only when due
   bool index64 = false;                 // flat offsets need (or are forced to) 64 bits
   // > 0: every thread L2-prefetches what site i + prefetch_* will load (about 3/4 of the
   // sites resident on the chip at once, i.e. the blocks scheduled just under a wave later)
@@ -30,7 +40,8 @@ int resident_sites_per_sm_pull(bool d3q19);
 int resident_sites_per_sm_aa(bool d3q19);
 
 // One time step, two-lattice pull: dst <- collide(gather(src)).
-void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
+                 cudaStream_t s);
 // One time step, A-A in place; `odd` selects the phase.
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s);
 
@@ -41,14 +52,16 @@ enum GatherMode {
   GATHER_AA_ODD = 2  // A-A after an odd number of steps: slot opp(q) of x - c_q (slot q at walls)
 };
 // rho [N] / u [N][3] (device, canonical order; either may be NULL)
-void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
-                        double* u, cudaStream_t s);
+// The read-out launchers take the BFL view that applies to the state in `buf` (only used in
+// GATHER_PULL mode; pass BflView() otherwise).
+void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
+                        double* rho, double* u, cudaStream_t s);
 // sigma [N][6] deviatoric stress xx, yy, zz, xy, xz, yz (device, canonical order)
-void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
-                   cudaStream_t s);
+void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
+                   double* sigma, cudaStream_t s);
 // f [N][Q] raw populations (device, canonical order)
-void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
-                            cudaStream_t s);
+void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode,
+                            const BflView& bfl, double* f, cudaStream_t s);
 // Initialise a buffer so that gathering in `mode` (GATHER_PULL or GATHER_OWN) yields
 //   f_q(x) = f_in[canon(x)][q]                       if f_in != NULL, else
 //   f_q(x) = f_eq_q(rho_in[canon(x)], u_in[canon(x)])  (NULL rho => 1, NULL u => 0).

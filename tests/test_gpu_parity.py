@@ -54,6 +54,9 @@ def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto", lattice
         g.hlb_set_state(wl.rho0, wl.u0)
     if wl.iolet_kind is not None:
         g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+    if wl.wall_distance is not None:
+        g.hlb_set_wall_distance(wl.wall_distance)
+        assert g.hlb_num_bfl_sites() > 0
     g.hlb_step(steps)
     assert g.hlb_steps_done() == steps
     out = g.hlb_get_macroscopic()
@@ -269,6 +272,84 @@ def test_time_varying_velocity_inlet_and_mixed_kinds(hlb, scheme):
     with pytest.raises(hlb.HlbError):
         g.hlb_set_iolet_velocity([2, 0, 0], np.zeros((3, 3)))
     g.close()
+
+
+# ------------------------------------------------------------- BFL interpolated walls (NEXT-2)
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("name", ["pipe", "aneurysm"])
+def test_bfl_walls_match_oracle(hlb, name, lattice):
+    """The paper's wall option: sub-voxel wall distances from the
+    analytic surfaces of the pipe and the aneurysm, with a Ladd velocity inlet; two-lattice
+    scheme, both storage types, records and table, even / odd / zero step counts."""
+    wl = W.with_bfl_walls(W.with_velocity_inlet(W.by_name(name, small=True)))
+    plain = W.with_velocity_inlet(W.by_name(name, small=True))
+    for steps, store, order, links in ((wl.steps, "f64", "raster", "records"),
+                                       (wl.steps + 1, "f64", "morton", "table"),
+                                       (0, "f64", "raster", "auto"), (1, "f64", "raster", "auto"),
+                                       (wl.steps, "f32", "raster", "auto")):
+        rho_ref, u_ref = run_oracle(wl, steps, lattice=lattice)
+        rho, u = run_gpu(hlb, wl, steps, "two_lattice", store, order, links, lattice)
+        e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+        assert e_rho < TOL[store] and e_u < TOL[store], (name, store, steps, e_rho, e_u)
+    # and the interpolation does change the flow (the test above is not vacuous)
+    rho_p, u_p = run_oracle(plain, wl.steps, lattice=lattice)
+    rho_b, u_b = run_oracle(wl, wl.steps, lattice=lattice)
+    assert np.max(np.abs(u_p - u_b)) > 1e-6
+
+
+@pytest.mark.parametrize("seed,periodic,shape", [(0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (33, 5, 4)),
+                                                 (3, 0, (24, 20, 18)), (4, 5, (40, 9, 23))])
+def test_bfl_random_masks_and_distances_match_oracle(hlb, seed, periodic, shape):
+    wl = W.random_mask(shape, p_fluid=0.65, n_iolets=3, p_iolet=0.05, periodic=periodic,
+                       tau=0.56 + 0.08 * seed, seed=500 + seed)
+    rng = np.random.default_rng(seed)
+    d27 = rng.uniform(0.01, 1.0, size=(wl.n_sites, 27))
+    d27[rng.random(d27.shape) < 0.25] = 0.0
+    perm = _match_directions(hlb)
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho)
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, "two_lattice", "f64", "raster" if seed % 2 else "morton"))
+    for x in (o, ):
+        x.set_state(wl.rho0, wl.u0)
+        x.set_wall_distance(d27)
+    g.hlb_set_state(wl.rho0, wl.u0)
+    g.hlb_set_wall_distance(d27)
+    for n in (0, 1, 1, 7, 12):
+        o.step(n)
+        g.hlb_step(n)
+        assert np.max(np.abs(g.hlb_get_populations()[:, perm] - o.get_populations())) < 1e-14
+    g.hlb_set_state(wl.rho0, wl.u0)                      # distances survive a re-initialisation
+    o.set_state(wl.rho0, wl.u0)
+    o.step(5)
+    g.hlb_step(5)
+    e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())
+    assert e_rho < 1e-13 and e_u < 1e-12
+    g.close()
+
+
+def test_bfl_at_half_a_link_is_bounce_back_bitwise_and_argument_errors(hlb):
+    wl = W.by_name("tree", small=True)
+    a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, "two_lattice", "f64", "raster"))
+    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, "two_lattice", "f64", "raster"))
+    b.hlb_set_wall_distance(np.full((wl.n_sites, 27), 0.5))
+    assert b.hlb_num_bfl_sites() > 100 and a.hlb_num_bfl_sites() == 0
+    a.hlb_step(40)
+    b.hlb_step(40)
+    (ra, ua), (rb, ub) = a.hlb_get_macroscopic(), b.hlb_get_macroscopic()
+    assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
+    with pytest.raises(hlb.HlbError) as e:
+        b.hlb_set_wall_distance(None)                    # not after the first step
+    assert e.value.code == hlb.HLB_EINVAL
+    b.hlb_set_state(None, None)
+    b.hlb_set_wall_distance(None)                        # allowed again at step 0
+    assert b.hlb_num_bfl_sites() == 0
+    a.close()
+    b.close()
+    c = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, "aa", "f64"))
+    with pytest.raises(hlb.HlbError) as e:
+        c.hlb_set_wall_distance(np.full((wl.n_sites, 27), 0.3))
+    assert e.value.code == hlb.HLB_EINVAL
+    c.close()
 
 
 # ------------------------------------------------------------- stress read-out (NEXT-3)
