@@ -68,6 +68,11 @@ def parse_args():
     ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
     ap.add_argument("--lattice", default="d3q15", choices=["d3q15", "d3q19"],
                     help="d3q15 = BASELINE.json's metric; d3q19 = the lattice the paper ran (NEXT-1)")
+    ap.add_argument("--inlet", default="pressure", choices=["pressure", "velocity"],
+                    help="velocity: iolet 0 becomes a Ladd velocity inlet (the paper's LADDIOLET)")
+    ap.add_argument("--walls", default="bounce_back", choices=["bounce_back", "bfl_random"],
+                    help="bfl_random: interpolated (BFL) walls with seeded random distances on every "
+                         "wall link -- the kernel work of the paper's BFL option (two_lattice only)")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -319,6 +324,13 @@ def main():
     S = args.inner
     if wl.rho0 is not None or wl.u0 is not None:
         g.hlb_set_state(wl.rho0, wl.u0)
+    if args.inlet == "velocity" and wl.n_iolets > 0:
+        wl = W.with_velocity_inlet(wl)
+        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+    if args.walls == "bfl_random":
+        d27 = np.random.default_rng(1906).uniform(0.05, 1.0, size=(N, 27))
+        g.hlb_set_wall_distance(d27)
+        del d27
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -417,7 +429,8 @@ def main():
             "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
             "n_sites": N, "lattice": args.lattice, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
             "order": args.order, "links": "records" if g.hlb_uses_records() else "table",
-            "l2_prefetch": not args.no_prefetch,
+            "l2_prefetch": not args.no_prefetch, "inlet": args.inlet, "walls": args.walls,
+            "bfl_sites": g.hlb_num_bfl_sites(),
             "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
             "box": list(wl.shape), "seed": wl.info.get("seed"),
             "device_bytes": g.hlb_device_bytes(),
