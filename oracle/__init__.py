@@ -15,4 +15,6 @@ from .hlb_oracle import (  # noqa: F401
     VARIANT_SHIFTED_LD,
     VARIANT_RAW_LD,
     LATTICE_Q,
+    render,
+    render_sample,
 )

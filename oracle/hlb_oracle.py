@@ -14,7 +14,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle.so")
-_SOURCES = [os.path.join(_HERE, "hlb_oracle.cpp"), os.path.join(_HERE, "hlb_oracle_dense.cpp")]
+_SOURCES = [os.path.join(_HERE, "hlb_oracle.cpp"), os.path.join(_HERE, "hlb_oracle_dense.cpp"),
+            os.path.join(_HERE, "render_oracle.cpp")]
 _lock = threading.Lock()
 _lib = None
 
@@ -82,6 +83,12 @@ def _load():
         lib.hlbd_run_ladd.restype = ctypes.c_int
         lib.hlbd_run_ladd.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p, ctypes.c_void_p] + \
             lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
+        lib.rendo_sample.restype = ctypes.c_float
+        lib.rendo_sample.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_float, ctypes.c_float, ctypes.c_float]
+        lib.rendo_render.restype = ctypes.c_int64
+        lib.rendo_render.argtypes = [ctypes.c_void_p] + [ctypes.c_int] * 5 + [ctypes.c_void_p] + \
+            [ctypes.c_float] * 5 + [ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbd_run_bfl.restype = ctypes.c_int
         lib.hlbd_run_bfl.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 3 + \
             lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
@@ -242,3 +249,29 @@ def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=
     if rc != 0:
         raise ValueError("hlbd_run rejected its arguments")
     return rho, u
+
+
+# ----------------------------------------------------------------------------- renderer oracle
+def render_sample(volume, p):
+    """One trilinear sample of a float32 volume [nz, ny, nx] at p = (x, y, z)."""
+    lib = _load()
+    vol = np.ascontiguousarray(volume, dtype=np.float32)
+    nz, ny, nx = vol.shape
+    return float(lib.rendo_sample(_ptr(vol), nx, ny, nz, float(p[0]), float(p[1]), float(p[2])))
+
+
+def render(volume, width, height, rot, zoom, step, tf_scale, tf_offset, opacity, lut):
+    """Ray-marched image [height, width, 4] float32 of a float32 volume [nz, ny, nx] (see
+    render_oracle.cpp for the definition). Returns (image, samples_inside_the_box)."""
+    lib = _load()
+    vol = np.ascontiguousarray(volume, dtype=np.float32)
+    nz, ny, nx = vol.shape
+    r = np.ascontiguousarray(np.asarray(rot, dtype=np.float32).reshape(9))
+    l = np.ascontiguousarray(np.asarray(lut, dtype=np.float32).reshape(256, 4))
+    img = np.zeros((height, width, 4), dtype=np.float32)
+    n = lib.rendo_render(_ptr(vol), nx, ny, nz, int(width), int(height), _ptr(r), float(zoom),
+                         float(step), float(tf_scale), float(tf_offset), float(opacity), _ptr(l),
+                         _ptr(img))
+    if n < 0:
+        raise ValueError("rendo_render rejected its arguments")
+    return img, int(n)
