@@ -203,6 +203,43 @@ void hlb_velocity_set(int32_t* c, double* w, int32_t* opp);
  * opp HOST [Q] (arrays of 19 entries always suffice; any may be NULL). Returns Q. */
 int hlb_lattice(uint32_t flags, int32_t* c, double* w, int32_t* opp);
 
+/* ---- volume rendering to a headless buffer -----------------------
+ * The paper's own GPU kernel: "the volume rendering kernel based on the ray marching
+ * algorithm", the look-up table and viewing parameters in constant memory, steering by zoom,
+ * rotation and scale / offset of the transfer function. No window,
+ * no OpenGL: the image is a float RGBA buffer. Definition (reading R-render):
+ *   volume v[z][y][x] of nx*ny*nz floats, voxel centres at integer coordinates;
+ *   orthographic camera along view +z; rot (row-major 3x3) maps view to volume space about
+ *   the box centre; pixel (px, py) -> X = (px + 0.5 - width/2) / zoom, same for Y; samples
+ *   k = 0 .. floor(2T/step) at view z = -T + k step, T = half the box diagonal; samples
+ *   outside [0, n-1]^3 are skipped; trilinear interpolation; t = clamp(value * tf_scale +
+ *   tf_offset, 0, 1); entry (int)(255 t + 0.5) of the 256-entry RGBA table; sample opacity
+ *   a = clamp(lut.a * opacity, 0, 1); front-to-back: C += (1-A) a rgb, A += (1-A) a; stop at
+ *   A >= 0.995. All arithmetic binary32. */
+typedef struct {
+  int32_t width, height;  /* image size in pixels, each >= 1                               */
+  float rot[9];           /* row-major rotation, view -> volume                            */
+  float zoom;             /* pixels per voxel, > 0                                         */
+  float step;             /* distance between samples in voxels, > 0                       */
+  float tf_scale, tf_offset; /* transfer function                                          */
+  float opacity;          /* multiplies the table's alpha                                  */
+  int32_t field;          /* hlb_render only: 0 = speed |u|, 1 = rho - 1                   */
+} hlb_view;
+
+/* Render a HOST volume [nz][ny][nx] with the HOST table lut [256][4] into the HOST image
+ * [height][width][4]. Uses cudaMalloc for its scratch; work goes to `stream` (cudaStream_t as
+ * void*, NULL = default) and is complete on return. Errors: HLB_EINVAL, HLB_ENOMEM, HLB_ECUDA. */
+int hlb_render_volume(const float* volume, int32_t nx, int32_t ny, int32_t nz, const hlb_view* view,
+                      const float* lut, float* image, void* stream);
+
+/* Render the geometry's current state: the scalar field view->field of the pre-collision
+ * state is written into a dense nx*ny*nz float volume on the device (0 outside the fluid;
+ * allocated through the allocator on first use and kept), then ray-marched.
+ *   hlb_render: image HOST [height][width][4], synchronises the stream.
+ *   hlb_render_device: image DEVICE [height][width][4] (16-byte aligned), no sync. */
+int hlb_render(hlb_geometry* g, const hlb_view* view, const float* lut, float* image);
+int hlb_render_device(hlb_geometry* g, const hlb_view* view, const float* lut, float* image_dev);
+
 /* ---- geometry preprocessor, host only (subsystem (b) of BASELINE.json north_star) ----
  * Two calls: hlb_preprocess_count() gives N and the plane stride Ns (N rounded up to a
  * multiple of 128); hlb_preprocess_tables() fills caller-allocated HOST arrays:

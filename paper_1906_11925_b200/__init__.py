@@ -5,5 +5,5 @@ in-tree build plus a thin ctypes binding with the same names. Importing the pack
 and loads the library and fails loudly if that is impossible -- there is no CPU fallback.
 """
 from .binding import *  # noqa: F401,F403
-from .binding import Geometry, HlbError, LIB_PATH, EXPORTED, hlb_params  # noqa: F401
+from .binding import Geometry, HlbError, LIB_PATH, EXPORTED, hlb_params, hlb_view, make_view  # noqa: F401
 from .metrics import msups, sups, BYTES_PER_SITE, algorithmic_bytes_per_site  # noqa: F401

@@ -42,6 +42,28 @@ class hlb_params(ctypes.Structure):
     ]
 
 
+class hlb_view(ctypes.Structure):
+    _fields_ = [
+        ("width", ctypes.c_int32), ("height", ctypes.c_int32),
+        ("rot", ctypes.c_float * 9),
+        ("zoom", ctypes.c_float), ("step", ctypes.c_float),
+        ("tf_scale", ctypes.c_float), ("tf_offset", ctypes.c_float),
+        ("opacity", ctypes.c_float),
+        ("field", ctypes.c_int32),
+    ]
+
+
+def make_view(width, height, rot=None, zoom=1.0, step=1.0, tf_scale=1.0, tf_offset=0.0, opacity=1.0,
+              field=0) -> "hlb_view":
+    v = hlb_view()
+    v.width, v.height = int(width), int(height)
+    r = np.eye(3, dtype=np.float32) if rot is None else np.asarray(rot, dtype=np.float32).reshape(3, 3)
+    v.rot = (ctypes.c_float * 9)(*[float(x) for x in r.reshape(-1)])
+    v.zoom, v.step = float(zoom), float(step)
+    v.tf_scale, v.tf_offset, v.opacity, v.field = float(tf_scale), float(tf_offset), float(opacity), int(field)
+    return v
+
+
 class HlbError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"hlb error {code}: {msg}")
@@ -65,6 +87,10 @@ def _load() -> ctypes.CDLL:
         "hlb_get_populations": (c_int, [vp, vp]),
         "hlb_get_stress": (c_int, [vp, vp]),
         "hlb_get_stress_device": (c_int, [vp, vp]),
+        "hlb_render_volume": (c_int, [vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                      ctypes.POINTER(hlb_view), vp, vp, vp]),
+        "hlb_render": (c_int, [vp, ctypes.POINTER(hlb_view), vp, vp]),
+        "hlb_render_device": (c_int, [vp, ctypes.POINTER(hlb_view), vp, vp]),
         "hlb_set_populations": (c_int, [vp, vp]),
         "hlb_num_sites": (i64, [vp]),
         "hlb_num_q": (c_int, [vp]),
@@ -95,7 +121,8 @@ _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_set_iolet_velocity", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
-            "hlb_get_stress", "hlb_get_stress_device",
+            "hlb_get_stress", "hlb_get_stress_device", "hlb_render_volume", "hlb_render",
+            "hlb_render_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
             "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
@@ -131,6 +158,20 @@ def hlb_velocity_set():
     opp = np.zeros(15, dtype=np.int32)
     _lib.hlb_velocity_set(_ptr(c), _ptr(w), _ptr(opp))
     return c, w, opp
+
+
+def hlb_render_volume(volume, view: "hlb_view", lut):
+    """Ray-march a host float32 volume [nz, ny, nx]; returns the image [height, width, 4]."""
+    import torch
+    if not torch.cuda.is_available():
+        raise HlbError(HLB_ECUDA, "no CUDA device: the renderer has no CPU fallback")
+    vol = np.ascontiguousarray(volume, dtype=np.float32)
+    nz, ny, nx = vol.shape
+    lut = np.ascontiguousarray(np.asarray(lut, dtype=np.float32).reshape(256, 4))
+    img = np.empty((view.height, view.width, 4), dtype=np.float32)
+    stream = torch.cuda.current_stream().cuda_stream
+    _check(_lib.hlb_render_volume(_ptr(vol), nx, ny, nz, ctypes.byref(view), _ptr(lut), _ptr(img), stream))
+    return img
 
 
 def hlb_lattice(flags=0):
@@ -269,6 +310,20 @@ class Geometry:
         sg = torch.empty((self.n_sites, 6), dtype=torch.float64, device=self.device)
         _check(_lib.hlb_get_stress_device(self._h, sg.data_ptr()))
         return sg
+
+    def hlb_render(self, view: "hlb_view", lut):
+        """Image [height, width, 4] float32 (host) of the current state."""
+        lut = np.ascontiguousarray(np.asarray(lut, dtype=np.float32).reshape(256, 4))
+        img = np.empty((view.height, view.width, 4), dtype=np.float32)
+        _check(_lib.hlb_render(self._h, ctypes.byref(view), _ptr(lut), _ptr(img)))
+        return img
+
+    def hlb_render_device(self, view: "hlb_view", lut):
+        torch = self._torch
+        lut = np.ascontiguousarray(np.asarray(lut, dtype=np.float32).reshape(256, 4))
+        img = torch.empty((view.height, view.width, 4), dtype=torch.float32, device=self.device)
+        _check(_lib.hlb_render_device(self._h, ctypes.byref(view), _ptr(lut), img.data_ptr()))
+        return img
 
     def hlb_get_populations(self):
         f = np.empty((self.n_sites, self.n_q), dtype=np.float64)

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB_PATH = os.path.join(HERE, "libhlb.so")
-SOURCES = ["api.cu", "kernels.cu", "preprocess.cpp"]
+SOURCES = ["api.cu", "kernels.cu", "render.cu", "preprocess.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "--shared", "-Xcompiler", "-fPIC,-O3,-Wall,-pthread", "-cudart", "static",

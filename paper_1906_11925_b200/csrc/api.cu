@@ -14,6 +14,7 @@
 #include "lattice.h"
 #include "kernels.cuh"
 #include "preprocess.h"
+#include "render.cuh"
 
 using namespace hlb;
 
@@ -68,6 +69,10 @@ struct hlb_geometry {
   double sentinel_fraction = 0.0;     // of the (group, q) link records
   // hlb_step(n) replays a captured CUDA graph of GRAPH_STEPS steps while n allows: removes
   // the per-launch host cost that dominates small geometries (BASELINE configs[0], [2])
+  float* volume = nullptr;            // [nz][ny][nx] floats for hlb_render (lazy)
+  long long* d_voxels = nullptr;      // [N] canonical voxel index on the device (lazy)
+  float* d_image = nullptr;           // staging image for hlb_render
+  size_t d_image_floats = 0;
   bool bfl_set = false;               // wall distances given (hlb_set_wall_distance)
   int64_t bfl_sites = 0;              // sites with at least one interpolated link
   cudaGraphExec_t graph_exec = nullptr;
@@ -537,6 +542,93 @@ int hlb_get_stress(hlb_geometry* g, double* sigma) {
   rc = hlb_get_stress_device(g, g->scratch_pop);
   if (rc) return rc;
   HLB_CUDA(cudaMemcpyAsync(sigma, g->scratch_pop, sizeof(double) * 6 * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
+static int check_view(const hlb_view* v, const float* lut, RenderSetup& r) {
+  if (!v || !lut) return fail(HLB_EINVAL, "NULL argument");
+  if (v->width <= 0 || v->height <= 0) return fail(HLB_EINVAL, "image size must be positive");
+  if (!(v->zoom > 0.0f) || !(v->step > 0.0f)) return fail(HLB_EINVAL, "zoom and step must be > 0");
+  r.width = v->width; r.height = v->height;
+  for (int k = 0; k < 9; ++k) r.rot[k] = v->rot[k];
+  r.zoom = v->zoom; r.step = v->step; r.tf_scale = v->tf_scale; r.tf_offset = v->tf_offset;
+  r.opacity = v->opacity;
+  return HLB_OK;
+}
+
+int hlb_render_volume(const float* volume, int32_t nx, int32_t ny, int32_t nz, const hlb_view* view,
+                      const float* lut, float* image, void* stream) {
+  if (!volume || !image) return fail(HLB_EINVAL, "NULL argument");
+  if (nx <= 0 || ny <= 0 || nz <= 0) return fail(HLB_EINVAL, "non-positive volume extent");
+  RenderSetup r;
+  int rc = check_view(view, lut, r);
+  if (rc) return rc;
+  r.nx = nx; r.ny = ny; r.nz = nz;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t vbytes = sizeof(float) * (size_t)nx * (size_t)ny * (size_t)nz;
+  const size_t ibytes = sizeof(float) * 4 * (size_t)view->width * (size_t)view->height;
+  float *d_vol = nullptr, *d_img = nullptr;
+  auto done = [&](int code) { cudaFree(d_vol); cudaFree(d_img); return code; };
+  if (cudaMalloc((void**)&d_vol, vbytes) != cudaSuccess || cudaMalloc((void**)&d_img, ibytes) != cudaSuccess) {
+    const cudaError_t e = cudaGetLastError();
+    return done(e == cudaErrorMemoryAllocation ? fail(HLB_ENOMEM, "cudaMalloc: out of memory")
+                                               : cuda_fail(e, "cudaMalloc"));
+  }
+  cudaError_t e = cudaMemcpyAsync(d_vol, volume, vbytes, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = render_upload(r, lut, s);
+  if (e == cudaSuccess) { launch_raymarch(r, d_vol, d_img, s); e = cudaGetLastError(); }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(image, d_img, ibytes, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return done(cuda_fail(e, "hlb_render_volume"));
+  return done(HLB_OK);
+}
+
+int hlb_render_device(hlb_geometry* g, const hlb_view* view, const float* lut, float* image_dev) {
+  if (!g || !image_dev) return fail(HLB_EINVAL, "NULL argument");
+  RenderSetup r;
+  int rc = check_view(view, lut, r);
+  if (rc) return rc;
+  if (view->field != 0 && view->field != 1) return fail(HLB_EINVAL, "field must be 0 (speed) or 1 (rho - 1)");
+  r.nx = g->p.nx; r.ny = g->p.ny; r.nz = g->p.nz;
+  const size_t nvox = (size_t)r.nx * (size_t)r.ny * (size_t)r.nz;
+  if (!g->volume) {
+    void* ptr = nullptr;
+    if ((rc = g->alloc(sizeof(float) * nvox, &ptr))) return rc;
+    g->volume = (float*)ptr;
+    if ((rc = g->alloc(sizeof(long long) * (size_t)g->N, &ptr))) return rc;
+    g->d_voxels = (long long*)ptr;
+    static_assert(sizeof(long long) == sizeof(int64_t), "voxel index width");
+    HLB_CUDA(cudaMemcpyAsync(g->d_voxels, g->canon_voxels.data(), sizeof(int64_t) * (size_t)g->N,
+                             cudaMemcpyHostToDevice, g->stream));
+    HLB_CUDA(cudaMemsetAsync(g->volume, 0, sizeof(float) * nvox, g->stream));  // solid voxels stay 0
+  }
+  double* d_rho = g->scratch;
+  double* d_u = g->scratch + g->N;
+  rc = hlb_get_macroscopic_device(g, d_rho, d_u);
+  if (rc) return rc;
+  launch_scatter_field(d_rho, d_u, g->d_voxels, g->N, view->field, g->volume, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  HLB_CUDA(render_upload(r, lut, g->stream));
+  launch_raymarch(r, g->volume, image_dev, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  return HLB_OK;
+}
+
+int hlb_render(hlb_geometry* g, const hlb_view* view, const float* lut, float* image) {
+  if (!g || !image || !view) return fail(HLB_EINVAL, "NULL argument");
+  if (view->width <= 0 || view->height <= 0) return fail(HLB_EINVAL, "image size must be positive");
+  const size_t nfl = 4 * (size_t)view->width * (size_t)view->height;
+  if (g->d_image_floats < nfl) {
+    void* ptr = nullptr;
+    int rc = g->alloc(sizeof(float) * nfl, &ptr);
+    if (rc) return rc;
+    g->d_image = (float*)ptr;
+    g->d_image_floats = nfl;
+  }
+  int rc = hlb_render_device(g, view, lut, g->d_image);
+  if (rc) return rc;
+  HLB_CUDA(cudaMemcpyAsync(image, g->d_image, sizeof(float) * nfl, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));
   return HLB_OK;
 }

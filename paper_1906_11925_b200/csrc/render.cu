@@ -1,0 +1,138 @@
+// render.cu -- direct volume rendering by ray marching to a headless device buffer
+// (SURVEY.md §8(f) NEXT-4). This is the one GPU kernel the paper itself describes: "The CUDA
+// cores in the rendering layer perform the volume rendering kernel based on the ray marching
+// algorithm", with "the viewing parameters and the look-up table" in "GPU
+// constant memory buffers" and steering by "zooming, model rotation and adjustment of scaling
+// and offset of the transfer functions" (lines 97-99). The OpenGL / Qt display tiers are
+// unavailable on this box; the image stays in a device buffer (or is copied to the host).
+//
+// Definition of the image: DESIGN.md reading R-render (orthographic camera, trilinear
+// sampling, 256-entry RGBA look-up table, front-to-back compositing, early ray termination at
+// A >= 0.995). Arithmetic: binary32, one explicit round-to-nearest intrinsic per operation,
+// in the order the definition states, so that the result does not depend on compiler
+// contraction. The paper keeps the volume in a 3-D texture; here it is a plain float array
+// read through the read-only cache with the interpolation done in the kernel: the texture
+// unit filters with 8-bit weights, which would make the image a property of the hardware
+// filter rather than of the definition (and break exact comparison with the oracle).
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "render.cuh"
+
+namespace hlb {
+namespace {
+
+struct ViewParams {
+  int nx, ny, nz, width, height;
+  float rot[9];
+  float zoom, step, tf_scale, tf_offset, opacity;
+};
+
+// "GPU constant memory buffers" for the look-up table and the viewing parameters
+__constant__ float c_lut[256 * 4];
+__constant__ ViewParams c_view;
+
+__device__ __forceinline__ float clamp01(float x) { return x < 0.0f ? 0.0f : (x > 1.0f ? 1.0f : x); }
+
+__device__ __forceinline__ float lerp_rn(float f, float a, float b) {  // a + f (b - a)
+  return __fmaf_rn(f, __fsub_rn(b, a), a);
+}
+
+__device__ __forceinline__ float trilinear(const float* __restrict__ vol, int nx, int ny, int nz,
+                                           float px, float py, float pz) {
+  int ix = (int)floorf(px), iy = (int)floorf(py), iz = (int)floorf(pz);
+  ix = min(ix, nx - 2); iy = min(iy, ny - 2); iz = min(iz, nz - 2);
+  ix = max(ix, 0); iy = max(iy, 0); iz = max(iz, 0);
+  const float fx = __fsub_rn(px, (float)ix), fy = __fsub_rn(py, (float)iy), fz = __fsub_rn(pz, (float)iz);
+  const int x1 = ix + 1 < nx ? ix + 1 : ix, y1 = iy + 1 < ny ? iy + 1 : iy, z1 = iz + 1 < nz ? iz + 1 : iz;
+  const long long r00 = ((long long)iz * ny + iy) * nx, r10 = ((long long)iz * ny + y1) * nx,
+                  r01 = ((long long)z1 * ny + iy) * nx, r11 = ((long long)z1 * ny + y1) * nx;
+  const float c00 = lerp_rn(fx, __ldg(vol + r00 + ix), __ldg(vol + r00 + x1));
+  const float c10 = lerp_rn(fx, __ldg(vol + r10 + ix), __ldg(vol + r10 + x1));
+  const float c01 = lerp_rn(fx, __ldg(vol + r01 + ix), __ldg(vol + r01 + x1));
+  const float c11 = lerp_rn(fx, __ldg(vol + r11 + ix), __ldg(vol + r11 + x1));
+  return lerp_rn(fz, lerp_rn(fy, c00, c10), lerp_rn(fy, c01, c11));
+}
+
+constexpr int TILE = 16;
+
+__global__ void __launch_bounds__(TILE * TILE)
+k_raymarch(const float* __restrict__ vol, float* __restrict__ image) {
+  const int px = blockIdx.x * TILE + threadIdx.x, py = blockIdx.y * TILE + threadIdx.y;
+  const ViewParams& v = c_view;
+  if (px >= v.width || py >= v.height) return;
+  const float fnx = (float)v.nx, fny = (float)v.ny, fnz = (float)v.nz;
+  const float cx = __fmul_rn(0.5f, (float)(v.nx - 1)), cy = __fmul_rn(0.5f, (float)(v.ny - 1)),
+              cz = __fmul_rn(0.5f, (float)(v.nz - 1));
+  const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(fnx, fnx), __fmul_rn(fny, fny)), __fmul_rn(fnz, fnz));
+  const float T = __fmul_rn(0.5f, __fsqrt_rn(d2));
+  const int K = (int)floorf(__fdiv_rn(__fmul_rn(2.0f, T), v.step)) + 1;
+  const float hx = (float)(v.nx - 1), hy = (float)(v.ny - 1), hz = (float)(v.nz - 1);
+  const float X = __fdiv_rn(__fsub_rn(__fadd_rn((float)px, 0.5f), __fmul_rn(0.5f, (float)v.width)), v.zoom);
+  const float Y = __fdiv_rn(__fsub_rn(__fadd_rn((float)py, 0.5f), __fmul_rn(0.5f, (float)v.height)), v.zoom);
+  // the part of the position that does not depend on the sample index
+  const float bx = __fmaf_rn(v.rot[1], Y, __fmaf_rn(v.rot[0], X, cx));
+  const float by = __fmaf_rn(v.rot[4], Y, __fmaf_rn(v.rot[3], X, cy));
+  const float bz = __fmaf_rn(v.rot[7], Y, __fmaf_rn(v.rot[6], X, cz));
+  float Cr = 0.0f, Cg = 0.0f, Cb = 0.0f, A = 0.0f;
+  for (int k = 0; k < K; ++k) {
+    const float Z = __fmaf_rn((float)k, v.step, -T);
+    const float qx = __fmaf_rn(v.rot[2], Z, bx), qy = __fmaf_rn(v.rot[5], Z, by), qz = __fmaf_rn(v.rot[8], Z, bz);
+    if (qx < 0.0f || qx > hx || qy < 0.0f || qy > hy || qz < 0.0f || qz > hz) continue;
+    const float val = trilinear(vol, v.nx, v.ny, v.nz, qx, qy, qz);
+    const float t = clamp01(__fmaf_rn(val, v.tf_scale, v.tf_offset));
+    const int i = (int)__fmaf_rn(t, 255.0f, 0.5f);
+    const float* e = c_lut + 4 * i;
+    const float a = clamp01(__fmul_rn(e[3], v.opacity));
+    const float wgt = __fmul_rn(__fsub_rn(1.0f, A), a);
+    Cr = __fmaf_rn(wgt, e[0], Cr);
+    Cg = __fmaf_rn(wgt, e[1], Cg);
+    Cb = __fmaf_rn(wgt, e[2], Cb);
+    A = __fadd_rn(A, wgt);
+    if (A >= 0.995f) break;
+  }
+  reinterpret_cast<float4*>(image)[(long long)py * v.width + px] = make_float4(Cr, Cg, Cb, A);
+}
+
+// volume[voxel of site c] = scalar field of site c (canonical order); the rest stays 0
+__global__ void __launch_bounds__(256)
+k_scatter_field(const double* __restrict__ rho, const double* __restrict__ u,
+                const long long* __restrict__ voxel, long long N, int field, float* __restrict__ vol) {
+  const long long c = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (c >= N) return;
+  double s;
+  if (field == 1) {
+    s = rho[c] - 1.0;
+  } else {
+    const double ux = u[3 * c], uy = u[3 * c + 1], uz = u[3 * c + 2];
+    s = sqrt(ux * ux + uy * uy + uz * uz);
+  }
+  vol[voxel[c]] = (float)s;
+}
+
+}  // namespace
+
+cudaError_t render_upload(const RenderSetup& r, const float* lut_host, cudaStream_t s) {
+  ViewParams v;
+  v.nx = r.nx; v.ny = r.ny; v.nz = r.nz; v.width = r.width; v.height = r.height;
+  for (int k = 0; k < 9; ++k) v.rot[k] = r.rot[k];
+  v.zoom = r.zoom; v.step = r.step; v.tf_scale = r.tf_scale; v.tf_offset = r.tf_offset; v.opacity = r.opacity;
+  cudaError_t e = cudaMemcpyToSymbolAsync(c_view, &v, sizeof(v), 0, cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpyToSymbolAsync(c_lut, lut_host, sizeof(float) * 1024, 0, cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) return e;
+  return cudaStreamSynchronize(s);  // v is a stack object; lut_host is the caller's
+}
+
+void launch_raymarch(const RenderSetup& r, const float* vol, float* image, cudaStream_t s) {
+  const dim3 grid((unsigned)((r.width + TILE - 1) / TILE), (unsigned)((r.height + TILE - 1) / TILE));
+  k_raymarch<<<grid, dim3(TILE, TILE), 0, s>>>(vol, image);
+}
+
+void launch_scatter_field(const double* rho, const double* u, const long long* voxel, long long N,
+                          int field, float* vol, cudaStream_t s) {
+  k_scatter_field<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(rho, u, voxel, N, field, vol);
+}
+
+}  // namespace hlb
