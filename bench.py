@@ -73,6 +73,9 @@ def parse_args():
     ap.add_argument("--walls", default="bounce_back", choices=["bounce_back", "bfl_random"],
                     help="bfl_random: interpolated (BFL) walls with seeded random distances on every "
                          "wall link -- the kernel work of the paper's BFL option (two_lattice only)")
+    ap.add_argument("--render", type=int, default=0, metavar="PIXELS",
+                    help="also time the ray-marching renderer (NEXT-4) on the final state: PIXELS x "
+                         "PIXELS frames of the speed field, rotating view; adds a \"render\" object")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -224,6 +227,42 @@ def replicas_value(n_sites, lb_steps, world, seconds):
     """Whole-job MSUPS of `world` replicas that each did n_sites x lb_steps site updates in
     at most `seconds` (the max over ranks)."""
     return world * n_sites * lb_steps / seconds / 1e6
+
+
+def time_renderer(hlb, g, wl, pixels, frames=12):
+    """Frames per second of hlb_render_device on the geometry's current state (speed field,
+    orthographic view turning about the y axis, sample step 0.5 voxel, image kept on the
+    device). The first frame also builds the dense voxel volume."""
+    import math
+    import torch
+    nx, ny, nz = wl.shape
+    lut = np.stack([np.linspace(0, 1, 256)] * 3 + [np.full(256, 0.02)], axis=1).astype(np.float32)
+    rho, u = g.hlb_get_macroscopic()
+    umax = float(np.max(np.linalg.norm(u, axis=1))) or 1.0
+    zoom = pixels / float(max(nx, ny, nz))
+
+    def view(k):
+        a = 2.0 * math.pi * k / frames
+        rot = [[math.cos(a), 0, math.sin(a)], [0, 1, 0], [-math.sin(a), 0, math.cos(a)]]
+        return hlb.make_view(pixels, pixels, rot=rot, zoom=zoom, step=0.5, tf_scale=1.0 / umax,
+                             tf_offset=0.0, opacity=1.0, field=0)
+
+    g.hlb_render_device(view(0), lut)                       # builds the volume
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(torch.cuda.current_stream())
+    for k in range(frames):
+        img = g.hlb_render_device(view(k), lut)
+    ev1.record(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / frames
+    diag = math.sqrt(nx * nx + ny * ny + nz * nz)
+    rays = pixels * pixels
+    return {"pixels": [pixels, pixels], "frames": frames, "ms_per_frame": ms, "fps": 1e3 / ms,
+            "volume_voxels": nx * ny * nz, "sample_step": 0.5,
+            "ray_samples_per_frame_upper_bound": int(rays * (diag / 0.5 + 1)),
+            "includes": "macroscopic read-out + scatter into the voxel volume + ray march, per frame",
+            "max_alpha": float(img[..., 3].max())}
 
 
 def host_cpu_model():
@@ -456,6 +495,8 @@ def main():
                       "h2d_bytes_per_step": 32 * N, "d2h_bytes_per_step": 32 * N,
                       "steps": e2e[1], "ms_per_step": e2e_all / e2e[1] * 1e3,
                       "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}
+    if args.render > 0:
+        out["render"] = time_renderer(hlb, g, wl, args.render)
     g.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, n, st, dt, what, thr = time_oracle(wl, args.cpu_seconds, threads=1, lattice=args.lattice)
