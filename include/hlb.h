@@ -43,7 +43,7 @@ extern "C" {
 typedef enum {
   HLB_OK = 0,
   HLB_EINVAL = -1,    /* NULL pointer, non-positive extent, tau <= 0.5, site type >=
-                         2 + n_iolets, n < 0, unknown flag combination                    */
+                         2 + n_iolets, iolet density <= 0, n < 0, unknown flag combination */
   HLB_ENOFLUID = -2,  /* no voxel of type 1                                               */
   HLB_ETOOLARGE = -3, /* N >= 2^31 - 128 (site indices are int32)                         */
   HLB_ENOMEM = -4,    /* allocator returned NULL                                          */

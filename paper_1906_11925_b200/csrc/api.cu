@@ -128,6 +128,8 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->nx <= 0 || p->ny <= 0 || p->nz <= 0) return fail(HLB_EINVAL, "non-positive box extent");
   if (p->n_iolets < 0 || p->n_iolets > 253) return fail(HLB_EINVAL, "n_iolets must be in 0..253");
   if (p->n_iolets > 0 && !p->iolet_rho) return fail(HLB_EINVAL, "iolet_rho is NULL");
+  for (int k = 0; k < p->n_iolets; ++k)
+    if (!(p->iolet_rho[k] > 0.0)) return fail(HLB_EINVAL, "iolet densities must be positive");
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
   if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
                              HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH | HLB_INDEX64 |

@@ -48,6 +48,12 @@ def test_errors_without_a_device_or_with_bad_arguments():
     assert rc == hlb.HLB_EINVAL and out.value is None
     assert b"tau" in lib.hlb_last_error()
     assert lib.hlb_geometry_create(None, ctypes.byref(p), ctypes.byref(out)) == hlb.HLB_EINVAL
+    p.tau = 0.8
+    p.n_iolets = 1
+    bad_rho = (ctypes.c_double * 1)(-1.0)                 # a density must be positive
+    p.iolet_rho = ctypes.cast(bad_rho, ctypes.c_void_p)
+    assert lib.hlb_geometry_create(st.ctypes.data_as(ctypes.c_void_p), ctypes.byref(p), ctypes.byref(out)) == hlb.HLB_EINVAL
+    assert b"positive" in lib.hlb_last_error()
     lib.hlb_num_sites.restype = ctypes.c_int64
     assert lib.hlb_num_sites(None) == hlb.HLB_EINVAL
     lib.hlb_geometry_destroy(None)                  # NULL is a no-op
