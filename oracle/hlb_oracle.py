@@ -76,6 +76,8 @@ def _load():
                                  ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbo_set_wall_distance.restype = None
         lib.hlbo_set_wall_distance.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_get_wall_shear_stress.restype = None
+        lib.hlbo_get_wall_shear_stress.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbo_get_stress.restype = None
         lib.hlbo_get_stress.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
         lib.hlbo_set_iolet_velocity.restype = None
@@ -201,6 +203,14 @@ class Oracle:
         sg = np.zeros((self.n_sites, 6), dtype=np.float64)
         self._lib.hlbo_get_stress(self._h, _ptr(sg))
         return sg
+
+    def get_wall_shear_stress(self, normals):
+        """|tangential part of sigma n| per site for wall normals [N, 3] (zero vector -> 0)."""
+        nrm = np.ascontiguousarray(normals, dtype=np.float64)
+        assert nrm.shape == (self.n_sites, 3)
+        out = np.zeros(self.n_sites, dtype=np.float64)
+        self._lib.hlbo_get_wall_shear_stress(self._h, _ptr(nrm), _ptr(out))
+        return out
 
     def get_macroscopic(self):
         rho = np.zeros(self.n_sites, dtype=np.float64)

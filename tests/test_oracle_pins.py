@@ -483,6 +483,37 @@ def test_stress_of_poiseuille_flow_is_linear_and_balances_the_pressure_gradient(
     assert np.max(np.abs(got + got[::-1])) < 1e-12 * np.max(np.abs(got))   # antisymmetric
 
 
+def test_wall_shear_stress_of_channel_flows():
+    """Couette: the traction on a plane with normal y is (rho nu U/H, 0, 0), all of it
+    tangential -> WSS = rho nu U / H at every site, 0 where no normal is given, and the same
+    for any length or sign of the normal. A normal along the flow sees no shear in Couette
+    flow up to the O(shear^2) normal stresses."""
+    H, U, tau = 8, 0.01, 0.8
+    st = np.zeros((1, H + 2, 1), dtype=np.uint8)
+    st[0, 1:H + 1, 0] = 1
+    st[0, H + 1, 0] = 2
+    o = oracle.Oracle(st, 5, tau, [1.0])
+    o.set_iolet_velocity([1], [[U, 0.0, 0.0]])
+    o.step(20000)
+    nu = (tau - 0.5) / 3.0
+    normals = np.zeros((H, 3))
+    normals[0] = (0.0, 1.0, 0.0)
+    normals[-1] = (0.0, -3.0, 0.0)
+    normals[3] = (0.0, 0.5, 0.0)
+    wss = o.get_wall_shear_stress(normals)
+    for i in (0, 3, H - 1):
+        assert wss[i] == pytest.approx(nu * U / H, rel=1e-10)
+    assert np.all(wss[[1, 2, 4, 5, 6]] == 0.0)
+    tilted = np.tile(np.array([1.0, 1.0, 0.0]), (H, 1))      # 45 degrees: t = s (1,1)/sqrt2 + normal parts
+    w45 = o.get_wall_shear_stress(tilted)
+    sg = o.get_stress()
+    n = np.array([1.0, 1.0, 0.0]) / math.sqrt(2.0)
+    for i in range(H):
+        S = np.array([[sg[i, 0], sg[i, 3], sg[i, 4]], [sg[i, 3], sg[i, 1], sg[i, 5]], [sg[i, 4], sg[i, 5], sg[i, 2]]])
+        t = S @ n
+        assert w45[i] == pytest.approx(np.linalg.norm(t - (t @ n) * n), rel=1e-12)
+
+
 def test_stress_vanishes_at_equilibrium():
     st = np.ones((4, 5, 6), dtype=np.uint8)
     o = oracle.Oracle(st, 7, 0.7, [])
