@@ -170,6 +170,14 @@ int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);
 int hlb_get_stress(hlb_geometry* g, double* sigma);
 int hlb_get_stress_device(hlb_geometry* g, double* sigma_dev);
 
+/* Wall shear stress: with t = sigma n the traction on the plane of unit normal n, the size of
+ * its tangential part, |t - (t.n) n|.
+ *   normals: HOST [N][3] canonical order, the wall normal at each site (any length; a zero
+ *            vector marks a site away from the wall and gives 0). The voxel mask carries no
+ *            normals, so they are the caller's (from the surface the mask was made from).
+ *   wss:     HOST [N]. Synchronises the stream. */
+int hlb_get_wall_shear_stress(hlb_geometry* g, const double* normals, double* wss);
+
 /* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][Q], canonical site
  * order, q in the order of hlb_lattice(). For population-level parity checks. The
  * first call of this or of hlb_set_populations allocates a [N][Q] fp64 staging buffer

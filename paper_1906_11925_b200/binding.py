@@ -87,6 +87,7 @@ def _load() -> ctypes.CDLL:
         "hlb_get_populations": (c_int, [vp, vp]),
         "hlb_get_stress": (c_int, [vp, vp]),
         "hlb_get_stress_device": (c_int, [vp, vp]),
+        "hlb_get_wall_shear_stress": (c_int, [vp, vp, vp]),
         "hlb_render_volume": (c_int, [vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                                       ctypes.POINTER(hlb_view), vp, vp, vp]),
         "hlb_render": (c_int, [vp, ctypes.POINTER(hlb_view), vp, vp]),
@@ -121,7 +122,7 @@ _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_set_iolet_velocity", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
-            "hlb_get_stress", "hlb_get_stress_device", "hlb_render_volume", "hlb_render",
+            "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
@@ -304,6 +305,12 @@ class Geometry:
         sg = np.empty((self.n_sites, 6), dtype=np.float64)
         _check(_lib.hlb_get_stress(self._h, _ptr(sg)))
         return sg
+
+    def hlb_get_wall_shear_stress(self, normals):
+        nrm = _host(normals, np.float64, (self.n_sites, 3))
+        out = np.empty(self.n_sites, dtype=np.float64)
+        _check(_lib.hlb_get_wall_shear_stress(self._h, _ptr(nrm), _ptr(out)))
+        return out
 
     def hlb_get_stress_device(self):
         torch = self._torch

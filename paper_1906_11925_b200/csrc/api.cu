@@ -548,6 +548,24 @@ int hlb_get_stress(hlb_geometry* g, double* sigma) {
   return HLB_OK;
 }
 
+int hlb_get_wall_shear_stress(hlb_geometry* g, const double* normals, double* wss) {
+  if (!g || !normals || !wss) return fail(HLB_EINVAL, "NULL argument");
+  int rc = ensure_scratch_pop(g);  // [N][Q >= 15]: sigma [N][6] | normals [N][3] | wss [N]
+  if (rc) return rc;
+  const size_t n = (size_t)g->N;
+  double* d_sigma = g->scratch_pop;
+  double* d_normals = d_sigma + 6 * n;
+  double* d_wss = d_normals + 3 * n;
+  HLB_CUDA(cudaMemcpyAsync(d_normals, normals, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, g->stream));
+  rc = hlb_get_stress_device(g, d_sigma);
+  if (rc) return rc;
+  launch_wall_shear_stress(d_sigma, d_normals, g->N, d_wss, g->stream);
+  HLB_CUDA(cudaGetLastError());
+  HLB_CUDA(cudaMemcpyAsync(wss, d_wss, sizeof(double) * n, cudaMemcpyDeviceToHost, g->stream));
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
 static int check_view(const hlb_view* v, const float* lut, RenderSetup& r) {
   if (!v || !lut) return fail(HLB_EINVAL, "NULL argument");
   if (v->width <= 0 || v->height <= 0) return fail(HLB_EINVAL, "image size must be positive");

@@ -382,6 +382,26 @@ k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
   for (int k = 0; k < 6; ++k) sigma[c * 6 + k] = pref * pi[k];
 }
 
+// Wall shear stress from a stress tensor field and wall normals, both in canonical order:
+// |t - (t.n) n| with t = sigma n and n the normalised normal; 0 where the normal is zero.
+__global__ void __launch_bounds__(BLOCK)
+k_wall_shear_stress(const double* __restrict__ sigma, const double* __restrict__ normals,
+                    long long N, double* __restrict__ wss) {
+  const long long c = (long long)blockIdx.x * BLOCK + threadIdx.x;
+  if (c >= N) return;
+  const double nx = normals[3 * c], ny = normals[3 * c + 1], nz = normals[3 * c + 2];
+  const double len = sqrt(nx * nx + ny * ny + nz * nz);
+  if (!(len > 0.0)) { wss[c] = 0.0; return; }
+  const double n0 = nx / len, n1 = ny / len, n2 = nz / len;
+  const double* s = sigma + 6 * c;  // xx yy zz xy xz yz
+  const double t0 = s[0] * n0 + s[3] * n1 + s[4] * n2;
+  const double t1 = s[3] * n0 + s[1] * n1 + s[5] * n2;
+  const double t2 = s[4] * n0 + s[5] * n1 + s[2] * n2;
+  const double tn = t0 * n0 + t1 * n1 + t2 * n2;
+  const double a = t0 - tn * n0, b = t1 - tn * n1, d = t2 - tn * n2;
+  wss[c] = sqrt(a * a + b * b + d * d);
+}
+
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
@@ -570,6 +590,10 @@ void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode
 void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
                    double* sigma, cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, bfl, sigma, s); });
+}
+void launch_wall_shear_stress(const double* sigma, const double* normals, long long N, double* wss,
+                              cudaStream_t s) {
+  k_wall_shear_stress<<<grid_for(N), BLOCK, 0, s>>>(sigma, normals, N, wss);
 }
 void launch_init(const DeviceGeometry& g, void* buf, GatherMode mode, const double* rho_in,
                  const double* u_in, const double* f_in, cudaStream_t s) {

@@ -59,6 +59,9 @@ void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mod
 // sigma [N][6] deviatoric stress xx, yy, zz, xy, xz, yz (device, canonical order)
 void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
                    double* sigma, cudaStream_t s);
+// wss [N] from sigma [N][6] and normals [N][3] (all device, canonical order)
+void launch_wall_shear_stress(const double* sigma, const double* normals, long long N, double* wss,
+                              cudaStream_t s);
 // f [N][Q] raw populations (device, canonical order)
 void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode,
                             const BflView& bfl, double* f, cudaStream_t s);

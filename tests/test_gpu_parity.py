@@ -377,6 +377,13 @@ def test_stress_matches_oracle(hlb, scheme, lattice):
             assert scale > 1e-7
             assert np.max(np.abs(got - ref)) / scale < STRESS_TOL[store], (store, n)
             assert np.array_equal(g.hlb_get_stress_device().cpu().numpy(), got)
+            # wall shear stress with seeded normals on a third of the sites
+            rng = np.random.default_rng(n)
+            normals = rng.standard_normal((wl.n_sites, 3))
+            normals[rng.random(wl.n_sites) < 0.66] = 0.0
+            w_ref, w_got = o.get_wall_shear_stress(normals), g.hlb_get_wall_shear_stress(normals)
+            assert np.all(w_got[np.all(normals == 0.0, axis=1)] == 0.0)
+            assert np.max(np.abs(w_got - w_ref)) / np.max(w_ref) < STRESS_TOL[store]
         g.close()
 
 
