@@ -13,7 +13,7 @@ LIB_PATH = os.path.join(HERE, "libhlb.so")
 SOURCES = ["api.cu", "kernels.cu", "render.cu", "preprocess.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "--shared", "-Xcompiler", "-fPIC,-O3,-Wall,-pthread", "-cudart", "static",
+    "--threads", "4", "--shared", "-Xcompiler", "-fPIC,-O3,-Wall,-pthread", "-cudart", "static",
 ]
 
 

@@ -1,18 +1,26 @@
-// kernels.cu -- fused D3Q15 LBGK collide-and-stream kernels for sm_100a.
+// kernels.cu -- fused LBGK collide-and-stream kernels for sm_100a (D3Q15 and D3Q19).
 //
-// One thread per fluid site, structure-of-arrays populations buf[slot][site] with plane
-// stride Ns (a multiple of 128, planes 1 KiB aligned), so the own-site loads and all stores
-// of a warp are single fully-coalesced 256-byte (fp64) / 128-byte (fp32) requests; the 14
-// gathers follow the int32 pull-neighbour table. The work is
-// an indirect gather/scatter stream at ~0.9 flop/byte: HBM-bound, no tensor cores, no
-// shared memory (no intra-block reuse: every population is read exactly once per step).
+// One thread per fluid site, 128 threads per block, one-shot grids of Ns / 128 blocks.
+// Populations are structure-of-arrays buf[slot][site] with plane stride Ns (a multiple of
+// 128, planes 1 KiB aligned), so the own-site loads and all stores of a warp are single fully
+// coalesced requests; the Q - 1 gathers follow the pull links.
+// ~0.7 flop/byte: HBM-bound, no tensor cores, no shared memory (every population is read
+// exactly once per step: there is no intra-block reuse to stage; cp.async / TMA staging was
+// measured slower, profiles/r01_tuning.md).
 //
-// Memory-level parallelism: all 14 index loads are issued first, then all 15 population
-// loads, then the arithmetic (Guideline 7 of the Blackwell guide).
+// What the kernels are shaped by (evidence in profiles/):
+//   * links come as 16-byte run-length records per (warp, link) instead of 32 table entries,
+//     decoded with a handful of integer operations; the int32 table is the fallback;
+//   * 32-bit flat offsets, explicit round-to-nearest fp64 intrinsics, pair-symmetric BGK:
+//     few instructions, because long runs sit at the 1 kW power cap;
+//   * 72-80 registers so that 6-7 blocks are resident per SM: all link loads are issued first,
+//     then all population loads, then the arithmetic;
+//   * every thread L2-prefetches what the site 3/4 of a wave ahead will load;
+//   * iolets (constant density, Ladd velocity) and BFL walls are rare paths behind one
+//     per-site bit; the table entries they need are re-read there, not kept in registers.
 //
-// Sites i in [N, Ns) are padding: their table entries are all "wall", their populations
-// are 0 (rest state in shifted form) and stay exactly 0, so no kernel needs a bounds
-// branch inside a warp.
+// Sites i in [N, Ns) are padding: their links are all "wall", their populations are 0 (rest
+// state in shifted form) and stay exactly 0, so no step kernel needs a bounds branch.
 #include "kernels.cuh"
 
 #include "lbgk.cuh"

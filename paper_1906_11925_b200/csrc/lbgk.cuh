@@ -1,6 +1,6 @@
-// lbgk.cuh -- per-site LBGK arithmetic (device), for either lattice of lattice.h, shared by every kernel variant so
-// that the two-lattice and A-A schemes, fp64 and fp32 storage, are bitwise identical in
-// their arithmetic (SURVEY.md §8(c) pin P14).
+// lbgk.cuh -- per-site LBGK arithmetic (device), for either lattice of lattice.h, shared by
+// every kernel variant so that the two-lattice and A-A schemes, fp64 and fp32 storage, are
+// bitwise identical in their arithmetic (SURVEY.md §8(c) pin P14).
 //
 // Rest-state-shifted form (reading R-shift): registers hold h_q = f_q - w_q.
 //   drho = sum_q h_q, rho = 1 + drho, j = sum_q c_q h_q, u = j / rho
