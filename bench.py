@@ -483,7 +483,10 @@ def main():
         "frac_of_nominal_8000": value * 1e6 * step_bytes / 1e9 / world / 8000.0,
         "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak,
                      "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "bytes_per_site": k_bytes[dominant],
+                     "traffic": traffic,
+                     "traffic_gbs": (traffic / (dom_ms * 1e-3) / 1e9) if traffic else None,
+                     "overfetch": (traffic / (k_bytes[dominant] * N)) if traffic else None,
+                     "bytes_per_site": k_bytes[dominant],
                      "sites_per_launch": N, "ms_per_launch": dom_ms,
                      "kernels": {k: {"ms": k_ms[k], "bytes_per_site": k_bytes[k],
                                      "gbs": k_bytes[k] * N / (k_ms[k] * 1e-3) / 1e9} for k in k_ms}},
