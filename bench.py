@@ -46,6 +46,7 @@ METRIC_Q19 = "fluid site updates/sec (MSUPS), D3Q19 LBGK sparse site update"
 UNIT = "MSUPS"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 DEFAULT_SCHEME = {"pipe": "two_lattice", "cube": "two_lattice", "aneurysm": "two_lattice",
+                  "paper_sized": "two_lattice",
                   "tree": "two_lattice", "bigtree": "aa"}
 WORKLOAD_DESC = {
     "pipe": "BASELINE configs[0]: pipe R=8 L=64",
@@ -53,6 +54,7 @@ WORKLOAD_DESC = {
     "aneurysm": "BASELINE configs[2]: sine vessel + sac, 480x160x160",
     "tree": "BASELINE configs[3]: 5-level tree, 1024^3 box, r0=32",
     "bigtree": "BASELINE configs[4]: 5-level tree, 2048x2048x1024 box, r0=64",
+    "paper_sized": "context only: aneurysm recipe scaled to ~297k sites (the paper's Subject 16, Table II)",
 }
 
 
