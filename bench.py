@@ -79,6 +79,7 @@ def parse_args():
                     help="also time the ray-marching renderer (NEXT-4) on the final state: PIXELS x "
                          "PIXELS frames of the speed field, rotating view; adds a \"render\" object")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
+    ap.add_argument("--no-pdl", action="store_true", help="HLB_NO_PDL (ablation)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="scaled-down geometry (debugging only)")
@@ -356,6 +357,7 @@ def main():
             {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
              "records": hlb.HLB_LINKS_RECORDS}[args.links] | \
             (hlb.HLB_NO_PREFETCH if args.no_prefetch else 0) | \
+            (hlb.HLB_NO_PDL if args.no_pdl else 0) | \
             (hlb.HLB_LATTICE_D3Q19 if args.lattice == "d3q19" else hlb.HLB_LATTICE_D3Q15)
     t_create = time.perf_counter()
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
@@ -470,7 +472,7 @@ def main():
             "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
             "n_sites": N, "lattice": args.lattice, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
             "order": args.order, "links": "records" if g.hlb_uses_records() else "table",
-            "l2_prefetch": not args.no_prefetch, "inlet": args.inlet, "walls": args.walls,
+            "l2_prefetch": not args.no_prefetch, "pdl": not args.no_pdl, "inlet": args.inlet, "walls": args.walls,
             "bfl_sites": g.hlb_num_bfl_sites(),
             "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
             "box": list(wl.shape), "seed": wl.info.get("seed"),

@@ -74,6 +74,9 @@ enum {
   HLB_INDEX64 = 0x100,     /* use the 64-bit flat-offset kernels even when Q * stride fits
                               32 bits (they are otherwise only taken above 286 M sites;
                               this flag lets small tests cover them)                       */
+  HLB_NO_PDL = 0x400,      /* launch the step kernels without programmatic dependent launch
+                              (by default step t+1 starts its blocks and fetches its link
+                              records while the last blocks of step t finish)              */
   HLB_LATTICE_D3Q15 = 0x0, /* 15 velocities: rest, 6 axis, 8 cube diagonals (BASELINE.json) */
   HLB_LATTICE_D3Q19 = 0x200 /* 19 velocities: rest, 6 axis, 12 face diagonals -- the lattice
                               the paper names. Everywhere below

@@ -133,7 +133,7 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
   if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
                              HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH | HLB_INDEX64 |
-                             HLB_LATTICE_D3Q19))
+                             HLB_LATTICE_D3Q19 | HLB_NO_PDL))
     return fail(HLB_EINVAL, "unknown flag bits");
   if ((p->flags & HLB_LINKS_TABLE) && (p->flags & HLB_LINKS_RECORDS))
     return fail(HLB_EINVAL, "HLB_LINKS_TABLE and HLB_LINKS_RECORDS are exclusive");
@@ -294,6 +294,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.iolet_bits = (const uint32_t*)d_bits;
   g->dg.rec = d_rec;
   g->dg.use_rec = use_rec;
+  g->dg.pdl = !(p->flags & HLB_NO_PDL);
   g->dg.index64 = (p->flags & HLB_INDEX64) != 0 || (int64_t)Q * t.Ns >= ((int64_t)1 << 32);
   g->dg.canon = (const int32_t*)d_canon;
   g->dg.omega = 1.0 / p->tau;

@@ -176,6 +176,15 @@ __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr
   }
 }
 
+// Programmatic dependent launch (sm_90+): a step kernel lets the next step's grid start as
+// soon as all of its own blocks have started (launch_dependents), and the next grid waits for
+// the full completion and memory flush of this one (wait) only right before it touches
+// populations. What precedes the wait -- thread setup and the link-record loads, which no
+// step kernel writes -- overlaps the tail of the previous step. Without the launch attribute
+// (HLB_NO_PDL, read-out kernels) both instructions are no-ops.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait_for_previous_step() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // L2 prefetch of data that a block scheduled roughly one wave later will load: brings the
 // DRAM fetch forward without holding registers or a scoreboard slot.
 __device__ __forceinline__ void prefetch_l2(const void* p) {
@@ -233,7 +242,9 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
   double h[L::Q];
   {
     IT off[L::Q - 1];
+    pdl_launch_dependents();
     link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
+    pdl_wait_for_previous_step();
     h[0] = to_real(src[i]);
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) h[q] = to_real(src[off[q - 1]]);
@@ -277,6 +288,8 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   ST* p0 = a + i;
   double h[L::Q];
+  pdl_launch_dependents();
+  pdl_wait_for_previous_step();
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
   if (pf > 0 && i + pf < Ns) {
@@ -300,7 +313,9 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
          long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
+  pdl_launch_dependents();
   link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
+  pdl_wait_for_previous_step();
   double h[L::Q];
   h[0] = to_real(a[i]);
 #pragma unroll
@@ -481,18 +496,34 @@ int resident_sites_per_sm_aa(bool d3q19) {
 }
 
 // ------------------------------------------------------------------ launchers
+// Step kernels are launched with the programmatic-stream-serialization attribute when
+// g.pdl is set (see pdl_launch_dependents above).
+template <typename... KArgs, typename... Args>
+static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(g.Ns / SBLOCK));
+  cfg.blockDim = dim3(SBLOCK);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = g.pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
                         cudaStream_t s) {
-  const unsigned grid = (unsigned)(g.Ns / SBLOCK);
   if (bfl.bits)
-    k_pull<L, ST, REC, IT, true><<<grid, SBLOCK, 0, s>>>(
-        (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns,
-        g.omega, g.prefetch_pull, bfl);
+    launch_step(g, k_pull<L, ST, REC, IT, true>, s, (const ST*)src, (ST*)dst, g.nbr,
+                (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
+                (long long)g.prefetch_pull, bfl);
   else
-    k_pull<L, ST, REC, IT, false><<<grid, SBLOCK, 0, s>>>(
-        (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns,
-        g.omega, g.prefetch_pull, bfl);
+    launch_step(g, k_pull<L, ST, REC, IT, false>, s, (const ST*)src, (ST*)dst, g.nbr,
+                (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
+                (long long)g.prefetch_pull, bfl);
 }
 template <typename L, typename ST>
 static void pull_t(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
@@ -508,15 +539,15 @@ static void pull_t(const DeviceGeometry& g, const void* src, void* dst, const Bf
 }
 template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
-  k_aa_odd<L, ST, REC, IT><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
-      (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.Ns, g.omega, g.prefetch_aa);
+  launch_step(g, k_aa_odd<L, ST, REC, IT>, s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
+              g.iolet_par, (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
 }
 template <typename L, typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (!odd) {
-    k_aa_even<L, ST><<<(unsigned)(g.Ns / SBLOCK), SBLOCK, 0, s>>>(
-        (ST*)a, g.nbr, g.iolet_bits, g.iolet_par, g.Ns, g.omega, g.prefetch_aa);
+    launch_step(g, k_aa_even<L, ST>, s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par, (long long)g.Ns,
+                g.omega, (long long)g.prefetch_aa);
   } else if (g.use_rec) {
     if (idx32) aa_odd_launch<L, ST, true, uint32_t>(g, a, s);
     else aa_odd_launch<L, ST, true, long long>(g, a, s);

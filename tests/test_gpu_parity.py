@@ -169,7 +169,8 @@ def test_d3q19_variants_agree_bitwise(hlb, scheme):
     ref = run_gpu(hlb, wl, steps, scheme, "f64", "raster", "table", "d3q19")
     for order, links, extra in (("raster", "records", 0), ("morton", "records", 0),
                                 ("tiled", "table", 0), ("raster", "records", hlb.HLB_INDEX64),
-                                ("raster", "records", hlb.HLB_NO_PREFETCH | hlb.HLB_NO_GRAPH)):
+                                ("raster", "records", hlb.HLB_NO_PREFETCH | hlb.HLB_NO_GRAPH),
+                                ("raster", "records", hlb.HLB_NO_PDL), ("morton", "table", hlb.HLB_NO_PDL)):
         got = run_gpu(hlb, wl, steps, scheme, "f64", order, links, "d3q19", extra)
         assert np.array_equal(ref[0], got[0]) and np.array_equal(ref[1], got[1]), (order, links, extra)
     other = run_gpu(hlb, wl, steps, "aa" if scheme == "two_lattice" else "two_lattice", "f64",
@@ -458,7 +459,7 @@ def test_graph_replay_equals_direct_launches(hlb, scheme):
     wl = W.by_name("aneurysm", small=True)
     f = flags_of(hlb, scheme, "f64", "raster")
     a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f)
-    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | hlb.HLB_NO_GRAPH)
+    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | hlb.HLB_NO_GRAPH | hlb.HLB_NO_PDL)
     for n in (1, 70, 33, 32, 100):
         a.hlb_step(n)
         b.hlb_step(n)
