@@ -91,6 +91,11 @@ def _load():
         lib.rendo_render.restype = ctypes.c_int64
         lib.rendo_render.argtypes = [ctypes.c_void_p] + [ctypes.c_int] * 5 + [ctypes.c_void_p] + \
             [ctypes.c_float] * 5 + [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbo_set_iolet_normal.restype = None
+        lib.hlbo_set_iolet_normal.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbd_run_all.restype = ctypes.c_int
+        lib.hlbd_run_all.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 4 + \
+            lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
         lib.hlbd_run_bfl.restype = ctypes.c_int
         lib.hlbd_run_bfl.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 3 + \
             lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
@@ -173,6 +178,14 @@ class Oracle:
         assert kind.shape == (self.n_iolets,) and u.shape == (self.n_iolets, 3)
         self._lib.hlbo_set_iolet_velocity(self._h, _ptr(kind), _ptr(u))
 
+    def set_iolet_normal(self, normals):
+        """Normals [n_iolets, 3] of the constant-density iolets (any length; zero vector or
+        None: no projection)."""
+        if normals is not None:
+            normals = np.ascontiguousarray(np.asarray(normals, dtype=np.float64).reshape(-1, 3))
+            assert normals.shape == (self.n_iolets, 3)
+        self._lib.hlbo_set_iolet_normal(self._h, _ptr(normals))
+
     def set_populations(self, f):
         f = np.ascontiguousarray(f, dtype=np.float64)
         assert f.shape == (self.n_sites, self.n_q)
@@ -227,6 +240,8 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
         o.set_state(workload.rho0, workload.u0)
     if getattr(workload, "iolet_kind", None) is not None:
         o.set_iolet_velocity(workload.iolet_kind, workload.iolet_u)
+    if getattr(workload, "iolet_normal", None) is not None:
+        o.set_iolet_normal(workload.iolet_normal)
     if getattr(workload, "wall_distance", None) is not None:
         o.set_wall_distance(workload.wall_distance)
     o.step(workload.steps if steps is None else steps)
@@ -236,7 +251,7 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
 
 
 def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None,
-              lattice="d3q15", iolet_kind=None, iolet_u=None, wall_d27_vox=None):
+              lattice="d3q15", iolet_kind=None, iolet_u=None, wall_d27_vox=None, iolet_normal=None):
     """Dense-grid twin: per-VOXEL rho [nz,ny,nx] and u [nz,ny,nx,3]."""
     lib = _load()
     st = np.ascontiguousarray(site_type, dtype=np.uint8)
@@ -253,9 +268,11 @@ def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=
     wd = None if wall_d27_vox is None else np.ascontiguousarray(wall_d27_vox, dtype=np.float64)
     if wd is not None:
         assert wd.shape == (nz * ny * nx, 27)
-    rc = lib.hlbd_run_bfl(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
-                          _ptr(io), _ptr(kind), _ptr(uio), _ptr(wd), _ptr(r0), _ptr(u0), int(steps),
-                          _ptr(rho), _ptr(u), LATTICE_Q[lattice])
+    nio = None if iolet_normal is None else \
+        np.ascontiguousarray(np.asarray(iolet_normal, dtype=np.float64).reshape(-1, 3))
+    rc = lib.hlbd_run_all(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
+                          _ptr(io), _ptr(kind), _ptr(uio), _ptr(wd), _ptr(nio), _ptr(r0), _ptr(u0),
+                          int(steps), _ptr(rho), _ptr(u), LATTICE_Q[lattice])
     if rc != 0:
         raise ValueError("hlbd_run rejected its arguments")
     return rho, u

@@ -20,6 +20,7 @@
 //         wd >= 1/2: f_opp(q)(x, t+1) = f*_q(x,t)/(2 wd) + (1 - 1/(2 wd)) f*_opp(q)(x,t)
 // which is the pull rule of hlb_oracle.cpp read from the other end of the link.
 
+#include <cmath>
 #include <cstdint>
 #include <vector>
 
@@ -69,9 +70,9 @@ extern "C" {
 // Returns 0, or -1 on a bad argument.
 static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
                          int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
-                         const double* iolet_u, const double* wall_d27, const double* rho0,
-                         const double* u0, int64_t steps, double* rho_out, double* u_out,
-                         int lattice_q) {
+                         const double* iolet_u, const double* wall_d27, const double* iolet_n,
+                         const double* rho0, const double* u0, int64_t steps, double* rho_out,
+                         double* u_out, int lattice_q) {
   if (lattice_q != 15 && lattice_q != 19) return -1;
   const Lattice& L = lattice_q == 15 ? L15 : L19;
   const int Q = L.Q;
@@ -153,6 +154,13 @@ static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned p
                 const double cu = CX[q] * iolet_u[k * 3 + 0] + CY[q] * iolet_u[k * 3 + 1] +
                                   CZ[q] * iolet_u[k * 3 + 2];
                 g[v * Q + OPP[q]] = fstar - 6.0 * L.WT[q] * rho * cu;
+              } else if (iolet_n && (iolet_n[k * 3] != 0.0 || iolet_n[k * 3 + 1] != 0.0 || iolet_n[k * 3 + 2] != 0.0)) {
+                // normal-projected pressure iolet: only the velocity along the unit normal
+                const double len = std::sqrt(iolet_n[k * 3] * iolet_n[k * 3] + iolet_n[k * 3 + 1] * iolet_n[k * 3 + 1] +
+                                             iolet_n[k * 3 + 2] * iolet_n[k * 3 + 2]);
+                const double n0 = iolet_n[k * 3] / len, n1 = iolet_n[k * 3 + 1] / len, n2 = iolet_n[k * 3 + 2] / len;
+                const double un = ux * n0 + uy * n1 + uz * n2;
+                g[v * Q + OPP[q]] = feq(L, OPP[q], iolet_rho[k], un * n0, un * n1, un * n2);
               } else {
                 g[v * Q + OPP[q]] = feq(L, OPP[q], iolet_rho[k], ux, uy, uz);
               }
@@ -180,7 +188,7 @@ int hlbd_run_lattice(const uint8_t* type, int nx, int ny, int nz, unsigned perio
                      int n_iolets, const double* iolet_rho, const double* rho0, const double* u0,
                      int64_t steps, double* rho_out, double* u_out, int lattice_q) {
   return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, nullptr, nullptr, nullptr,
-                       rho0, u0, steps, rho_out, u_out, lattice_q);
+                       nullptr, rho0, u0, steps, rho_out, u_out, lattice_q);
 }
 
 // iolet_kind [n_iolets]: 0 constant density, 1 Ladd velocity with iolet_u [n_iolets][3];
@@ -191,14 +199,23 @@ int hlbd_run_ladd(const uint8_t* type, int nx, int ny, int nz, unsigned periodic
                   const double* iolet_u, const double* rho0, const double* u0, int64_t steps,
                   double* rho_out, double* u_out, int lattice_q) {
   return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
-                       nullptr, rho0, u0, steps, rho_out, u_out, lattice_q);
+                       nullptr, nullptr, rho0, u0, steps, rho_out, u_out, lattice_q);
 }
 int hlbd_run_bfl(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
                  int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
                  const double* iolet_u, const double* wall_d27, const double* rho0,
                  const double* u0, int64_t steps, double* rho_out, double* u_out, int lattice_q) {
   return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
-                       wall_d27, rho0, u0, steps, rho_out, u_out, lattice_q);
+                       wall_d27, nullptr, rho0, u0, steps, rho_out, u_out, lattice_q);
+}
+// + iolet_n [n_iolets][3]: normals of the constant-density iolets (zero vector: no projection)
+int hlbd_run_all(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                 int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
+                 const double* iolet_u, const double* wall_d27, const double* iolet_n,
+                 const double* rho0, const double* u0, int64_t steps, double* rho_out,
+                 double* u_out, int lattice_q) {
+  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
+                       wall_d27, iolet_n, rho0, u0, steps, rho_out, u_out, lattice_q);
 }
 
 int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,

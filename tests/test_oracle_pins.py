@@ -358,6 +358,72 @@ def test_ladd_velocity_at_rest_is_plain_bounce_back():
     assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
 
 
+# ------------------------------------------------------------------ normal-projected iolets
+def test_iolet_normal_projection_special_cases():
+    """(a) no normal, or a zero normal: unchanged bit for bit; (b) a flow that is exactly
+    along the normal at the iolet sites (1-D duct): the projection changes nothing but
+    roundoff; (c) a normal perpendicular to everything the iolet sites can do: the ghost is at
+    rest, i.e. the rule becomes f_eq(rho_k, 0); (d) the length of the normal is irrelevant."""
+    wl = W.random_mask((9, 8, 7), p_fluid=0.65, n_iolets=2, p_iolet=0.08, seed=12)
+
+    def run(normals, st=wl.site_type, rho_io=wl.iolet_rho, steps=12):
+        o = oracle.Oracle(st, 0, wl.tau, rho_io)
+        if st is wl.site_type:
+            o.set_state(wl.rho0, wl.u0)
+        if normals is not None:
+            o.set_iolet_normal(normals)
+        o.step(steps)
+        return o.get_populations()
+
+    base = run(None)
+    assert np.array_equal(base, run(np.zeros((2, 3))))
+    proj = run([[1.0, 2.0, -1.0], [0.0, 0.0, 1.0]])
+    assert np.max(np.abs(proj - base)) > 1e-6                       # it does something
+    assert np.max(np.abs(proj - run([[3.0, 6.0, -3.0], [0.0, 0.0, 0.2]]))) < 1e-15   # (d)
+    # (b), (c): a duct along z, periodic sideways
+    L = 10
+    st = np.zeros((L + 2, 1, 1), dtype=np.uint8)
+    st[1:L + 1, 0, 0] = 1
+    st[0, 0, 0], st[L + 1, 0, 0] = 2, 3
+    rho_io = [1.002, 0.998]
+    a = run(None, st, rho_io, 40)
+    b = run([[0, 0, 1], [0, 0, -1]], st, rho_io, 40)
+    assert np.max(np.abs(a - b)) < 1e-16
+    c = run([[1, 0, 0], [0, 1, 0]], st, rho_io, 40)
+    assert np.max(np.abs(a - c)) > 1e-7
+    # ghost at rest: same as a run whose iolet sites see u = 0 in the rule -> compare with the
+    # dense twin, which implements the projection independently
+    rd, ud = oracle.dense_run(st, 3, wl.tau, rho_io, 40, iolet_normal=[[1, 0, 0], [0, 1, 0]])
+    o = oracle.Oracle(st, 3, wl.tau, rho_io, variant=oracle.VARIANT_RAW)
+    o.set_iolet_normal([[1, 0, 0], [0, 1, 0]])
+    o.step(40)
+    r, u = o.get_macroscopic()
+    v = np.flatnonzero(st.reshape(-1) == 1)
+    assert np.max(np.abs(r - rd.reshape(-1)[v])) < 1e-15 and np.max(np.abs(u - ud.reshape(-1, 3)[v])) < 1e-15
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_iolet_normal_projection_dense_twin(seed):
+    wl = W.random_mask((8, 7, 9), p_fluid=0.65, n_iolets=3, p_iolet=0.08, periodic=seed, seed=600 + seed)
+    st, vox = wl.site_type, wl.fluid_voxels()
+    rng = np.random.default_rng(seed)
+    normals = rng.standard_normal((3, 3))
+    normals[1] = 0.0                                                  # one iolet without a normal
+    kind, uio = np.array([0, 0, 1], dtype=np.uint8), 0.02 * (rng.random((3, 3)) - 0.5)
+    rho0v, u0v = np.ones(st.size), np.zeros((st.size, 3))
+    rho0v[vox], u0v[vox] = wl.rho0, wl.u0
+    rd, ud = oracle.dense_run(st, seed, wl.tau, wl.iolet_rho, 9, rho0v, u0v, iolet_kind=kind, iolet_u=uio,
+                              iolet_normal=normals)
+    o = oracle.Oracle(st, seed, wl.tau, wl.iolet_rho, variant=oracle.VARIANT_RAW)
+    o.set_state(wl.rho0, wl.u0)
+    o.set_iolet_velocity(kind, uio)
+    o.set_iolet_normal(normals)
+    o.step(9)
+    r, u = o.get_macroscopic()
+    assert np.max(np.abs(r - rd.reshape(-1)[vox])) < 5e-15
+    assert np.max(np.abs(u - ud.reshape(-1, 3)[vox])) < 5e-15
+
+
 # ------------------------------------------------------------------ BFL interpolated walls
 def _d27_index(dx, dy, dz):
     return (dz + 1) * 9 + (dy + 1) * 3 + (dx + 1)

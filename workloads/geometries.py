@@ -41,6 +41,7 @@ class Workload:
     u0: Optional[np.ndarray] = None    # float64 (N, 3) canonical order, None => 0
     iolet_kind: Optional[np.ndarray] = None  # uint8 (n_iolets,): 0 density, 1 Ladd velocity; None => all 0
     iolet_u: Optional[np.ndarray] = None     # float64 (n_iolets, 3) velocities of the velocity iolets
+    iolet_normal: Optional[np.ndarray] = None  # float64 (n_iolets, 3): normals of density iolets
     wall_distance: Optional[np.ndarray] = None  # float64 (N, 27): BFL wall distances (include/hlb.h)
     scheme: str = "two_lattice"      # "two_lattice" | "aa"  (what the config asks for)
     store: str = "f64"               # "f64" | "f32"
