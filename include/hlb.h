@@ -121,6 +121,13 @@ int hlb_set_state(hlb_geometry* g, const double* rho, const double* u);
  * step; the density of an iolet that is currently a velocity iolet is kept for later. */
 int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho);
 
+/* Normals of the constant-density iolets ("normal-projected" pressure iolets): with a normal
+ * n_k given, the rule f_q(x,t+1) = f_eq_q(rho_k, u(x,t)) uses only the part of u along n_k,
+ * (u.n_k) n_k.  normals: HOST [n_iolets][3], any length (normalised here), a zero vector (or
+ * NULL for all) = no projection, the default. Ignored for velocity iolets. Takes effect from
+ * the next step. */
+int hlb_set_iolet_normal(hlb_geometry* g, const double* normals);
+
 /* Interpolated ("BFL") walls -- the paper's wall option (ref. [16]:
  * Bouzidi, Firdaouss & Lallemand), linear form. d27: HOST [N][27] in canonical site order;
  * entry (dz+1)*9 + (dy+1)*3 + (dx+1) is the fraction d in (0, 1] of the link from the site

@@ -80,6 +80,7 @@ def _load() -> ctypes.CDLL:
         "hlb_set_state": (c_int, [vp, vp, vp]),
         "hlb_set_iolet_density": (c_int, [vp, vp]),
         "hlb_set_iolet_velocity": (c_int, [vp, vp, vp]),
+        "hlb_set_iolet_normal": (c_int, [vp, vp]),
         "hlb_set_wall_distance": (c_int, [vp, vp]),
         "hlb_num_bfl_sites": (i64, [vp]),
         "hlb_step": (c_int, [vp, i64]),
@@ -121,7 +122,7 @@ def _load() -> ctypes.CDLL:
 LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
-            "hlb_set_iolet_velocity", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
+            "hlb_set_iolet_velocity", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
@@ -274,6 +275,10 @@ class Geometry:
         kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8)
         u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64)
         _check(_lib.hlb_set_iolet_velocity(self._h, _ptr(kind), _ptr(u)))
+
+    def hlb_set_iolet_normal(self, normals):
+        n = None if normals is None else _host(np.asarray(normals, dtype=np.float64).reshape(-1, 3), np.float64)
+        _check(_lib.hlb_set_iolet_normal(self._h, _ptr(n)))
 
     def hlb_set_wall_distance(self, d27):
         d27 = None if d27 is None else _host(d27, np.float64, (self.n_sites, 27))

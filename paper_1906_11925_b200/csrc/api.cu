@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -58,6 +59,7 @@ struct hlb_geometry {
   std::vector<double> iolet_rho;
   std::vector<uint8_t> iolet_kind;    // 0 constant density, 1 Ladd velocity
   std::vector<double> iolet_u;        // [n_iolets][3]
+  std::vector<double> iolet_n;        // [n_iolets][3] unit normals of density iolets, 0 = none
   std::vector<double> iolet_par;      // [n_iolets][4] as uploaded: {rho or -1, ux, uy, uz}
   DeviceGeometry dg;
   void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
@@ -174,7 +176,7 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
   return HLB_OK;
 }
 
-// {rho_k, 0, 0, 0} for a constant-density iolet, {-1, ux, uy, uz} for a velocity iolet
+// {rho_k, nx, ny, nz} for a constant-density iolet, {-1, ux, uy, uz} for a velocity iolet
 static int upload_iolets(hlb_geometry* g) {
   const int n = g->p.n_iolets;
   if (n == 0) return HLB_OK;
@@ -186,6 +188,7 @@ static int upload_iolets(hlb_geometry* g) {
       for (int a = 0; a < 3; ++a) g->iolet_par[(size_t)k * 4 + 1 + a] = g->iolet_u[(size_t)k * 3 + a];
     } else {
       g->iolet_par[(size_t)k * 4] = g->iolet_rho[(size_t)k];
+      for (int a = 0; a < 3; ++a) g->iolet_par[(size_t)k * 4 + 1 + a] = g->iolet_n[(size_t)k * 3 + a];
     }
   }
   HLB_CUDA(cudaMemcpyAsync((void*)g->dg.iolet_par, g->iolet_par.data(), sizeof(double) * 4 * (size_t)n,
@@ -235,6 +238,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->iolet_rho.assign(p->iolet_rho, p->iolet_rho + p->n_iolets);
   g->iolet_kind.assign((size_t)p->n_iolets, 0);
   g->iolet_u.assign((size_t)p->n_iolets * 3, 0.0);
+  g->iolet_n.assign((size_t)p->n_iolets * 3, 0.0);
   g->canon_voxels.resize((size_t)t.N);
   for (int64_t i = 0; i < t.N; ++i) g->canon_voxels[(size_t)t.canon_of_site[(size_t)i]] = t.voxel_of_site[(size_t)i];
 
@@ -368,6 +372,21 @@ int hlb_set_iolet_density(hlb_geometry* g, const double* iolet_rho) {
   for (int k = 0; k < g->p.n_iolets; ++k)
     if (!(iolet_rho[k] > 0.0)) return fail(HLB_EINVAL, "iolet densities must be positive");
   g->iolet_rho.assign(iolet_rho, iolet_rho + g->p.n_iolets);
+  return upload_iolets(g);
+}
+
+int hlb_set_iolet_normal(hlb_geometry* g, const double* normals) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  const int n = g->p.n_iolets;
+  for (int k = 0; k < n; ++k) {
+    double v[3] = {0.0, 0.0, 0.0};
+    if (normals) {
+      const double* s = normals + k * 3;
+      const double len = std::sqrt(s[0] * s[0] + s[1] * s[1] + s[2] * s[2]);
+      if (len > 0.0) { v[0] = s[0] / len; v[1] = s[1] / len; v[2] = s[2] / len; }
+    }
+    for (int a = 0; a < 3; ++a) g->iolet_n[(size_t)k * 3 + a] = v[a];
+  }
   return upload_iolets(g);
 }
 

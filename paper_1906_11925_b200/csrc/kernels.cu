@@ -152,6 +152,7 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 // Rare path (sites on an inlet/outlet cap): for every iolet link p of site i replace
 // out[p] -- the value that will be read back as f_p(x, t+1), on entry the bounced h*_opp(p) --
 //   constant-density iolet k: by the equilibrium f_eq_p(rho_k, u(x, t))           (reading A6)
+//                             (u replaced by (u.n_k) n_k when a normal n_k is given)
 //   velocity iolet k (Ladd):  by h*_opp(p) + 6 w_p rho(x, t) c_p.u_k             (reading R-ladd)
 // The table entries are re-read here so that the common path does not keep them in
 // registers; fully unrolled so that out[] stays in registers (no call, no stack).
@@ -167,7 +168,15 @@ __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr
       const double* par = iolet_par + 4 * k;
       const double rk = __ldg(par);
       if (rk > 0.0) {
-        out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+        // par[1..3]: unit normal of the iolet, (0,0,0) = none; with a normal the ghost only
+        // carries the normal part (u.n) n of the site's velocity
+        const double n0 = __ldg(par + 1), n1 = __ldg(par + 2), n2 = __ldg(par + 3);
+        if (n0 != 0.0 || n1 != 0.0 || n2 != 0.0) {
+          const double un = add(add(mul(m.ux, n0), mul(m.uy, n1)), mul(m.uz, n2));
+          out[p] = heq_of<L>(p, rk - 1.0, rk, mul(un, n0), mul(un, n1), mul(un, n2));
+        } else {
+          out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+        }
       } else {
         const double cu = c_dot_u<L>(p, __ldg(par + 1), __ldg(par + 2), __ldg(par + 3));
         out[p] = fma_(mul(6.0 * L::weight(p), m.rho), cu, out[p]);

@@ -29,7 +29,8 @@ struct DeviceGeometry {
   // sites resident on the chip at once, i.e. the blocks scheduled just under a wave later)
   int64_t prefetch_pull = 0, prefetch_aa = 0;
   const int32_t* canon = nullptr;       // [N] internal -> canonical rank
-  const double* iolet_par = nullptr;    // [n_iolets][4]: {rho_k, -, -, -} constant density;
+  const double* iolet_par = nullptr;    // [n_iolets][4]: {rho_k, nx, ny, nz} constant density
+                                        // (unit normal or 0,0,0);
                                         // {-1, ux, uy, uz} Ladd velocity iolet
   double omega = 1.0;                   // 1 / tau
   bool f32 = false;                     // HLB_STORE_F32
