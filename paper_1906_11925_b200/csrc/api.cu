@@ -182,7 +182,11 @@ static int upload_iolets(hlb_geometry* g) {
   if (n == 0) return HLB_OK;
   HLB_CUDA(cudaStreamSynchronize(g->stream));  // the previous upload may still read iolet_par
   g->iolet_par.assign((size_t)n * 4, 0.0);
+  g->dg.iolet_full = false;
   for (int k = 0; k < n; ++k) {
+    if (g->iolet_kind[(size_t)k] == 1 || g->iolet_n[(size_t)k * 3] != 0.0 ||
+        g->iolet_n[(size_t)k * 3 + 1] != 0.0 || g->iolet_n[(size_t)k * 3 + 2] != 0.0)
+      g->dg.iolet_full = true;
     if (g->iolet_kind[(size_t)k] == 1) {
       g->iolet_par[(size_t)k * 4] = -1.0;
       for (int a = 0; a < 3; ++a) g->iolet_par[(size_t)k * 4 + 1 + a] = g->iolet_u[(size_t)k * 3 + a];

@@ -156,7 +156,11 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 //   velocity iolet k (Ladd):  by h*_opp(p) + 6 w_p rho(x, t) c_p.u_k             (reading R-ladd)
 // The table entries are re-read here so that the common path does not keep them in
 // registers; fully unrolled so that out[] stays in registers (no call, no stack).
-template <typename L>
+// FULL = false is the lean instantiation for geometries whose iolets are all plain
+// constant-density ones (every BASELINE config): inlined, the Ladd and normal branches make
+// the compiler park four values in local memory on the COMMON path (measured: -1.5 % on
+// configs[4]; moving the rare path out of line instead cost 4-6 %, profiles/r01_tuning.md).
+template <typename L, bool FULL>
 __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
                                                  long long i, const Moments& m,
                                                  const double* __restrict__ iolet_par,
@@ -167,7 +171,9 @@ __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr
     if (k >= 0) {
       const double* par = iolet_par + 4 * k;
       const double rk = __ldg(par);
-      if (rk > 0.0) {
+      if (!FULL) {
+        out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
+      } else if (rk > 0.0) {
         // par[1..3]: unit normal of the iolet, (0,0,0) = none; with a normal the ghost only
         // carries the normal part (u.n) n of the site's velocity
         const double n0 = __ldg(par + 1), n1 = __ldg(par + 2), n2 = __ldg(par + 3);
@@ -241,7 +247,7 @@ __device__ __forceinline__ void bfl_apply(const BflView& b, const ST* __restrict
 // pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
 // of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
 // padding, so only the one warp-uniform test is needed.
-template <typename L, typename ST, bool REC, typename IT, bool BFL>
+template <typename L, typename ST, bool REC, typename IT, bool BFL, bool FULL>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
@@ -275,7 +281,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L>(nbr, Ns, i, m, iolet_par, back);
+    iolet_substitute<L, FULL>(nbr, Ns, i, m, iolet_par, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
@@ -289,7 +295,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // Odd phase: read f_q from slot opp(q) of x - c_q (slot q of x at a wall), write h*_q to
 // the address f_opp(q) was read from. Read set = write set per site in both phases, so one
 // array and no inter-thread hazards.
-template <typename L, typename ST>
+template <typename L, typename ST, bool FULL>
 __global__ void __launch_bounds__(SBLOCK, aa_even_minb<L>())
 k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
           const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
@@ -310,12 +316,12 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
   double out[L::Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_par, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, FULL>(nbr, Ns, i, m, iolet_par, out);
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
 
-template <typename L, typename ST, bool REC, typename IT>
+template <typename L, typename ST, bool REC, typename IT, bool FULL>
 __global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
@@ -343,7 +349,7 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L>(nbr, Ns, i, m, iolet_par, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, FULL>(nbr, Ns, i, m, iolet_par, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
@@ -525,12 +531,16 @@ static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaS
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
                         cudaStream_t s) {
-  if (bfl.bits)
-    launch_step(g, k_pull<L, ST, REC, IT, true>, s, (const ST*)src, (ST*)dst, g.nbr,
+  if (bfl.bits)  // BFL implies the full iolet rules (fewer instantiations)
+    launch_step(g, k_pull<L, ST, REC, IT, true, true>, s, (const ST*)src, (ST*)dst, g.nbr,
+                (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
+                (long long)g.prefetch_pull, bfl);
+  else if (g.iolet_full)
+    launch_step(g, k_pull<L, ST, REC, IT, false, true>, s, (const ST*)src, (ST*)dst, g.nbr,
                 (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
                 (long long)g.prefetch_pull, bfl);
   else
-    launch_step(g, k_pull<L, ST, REC, IT, false>, s, (const ST*)src, (ST*)dst, g.nbr,
+    launch_step(g, k_pull<L, ST, REC, IT, false, false>, s, (const ST*)src, (ST*)dst, g.nbr,
                 (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
                 (long long)g.prefetch_pull, bfl);
 }
@@ -548,15 +558,23 @@ static void pull_t(const DeviceGeometry& g, const void* src, void* dst, const Bf
 }
 template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
-  launch_step(g, k_aa_odd<L, ST, REC, IT>, s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-              g.iolet_par, (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
+  if (g.iolet_full)
+    launch_step(g, k_aa_odd<L, ST, REC, IT, true>, s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
+                g.iolet_par, (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
+  else
+    launch_step(g, k_aa_odd<L, ST, REC, IT, false>, s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
+                g.iolet_par, (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
 }
 template <typename L, typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (!odd) {
-    launch_step(g, k_aa_even<L, ST>, s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par, (long long)g.Ns,
-                g.omega, (long long)g.prefetch_aa);
+    if (g.iolet_full)
+      launch_step(g, k_aa_even<L, ST, true>, s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par,
+                  (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
+    else
+      launch_step(g, k_aa_even<L, ST, false>, s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par,
+                  (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
   } else if (g.use_rec) {
     if (idx32) aa_odd_launch<L, ST, true, uint32_t>(g, a, s);
     else aa_odd_launch<L, ST, true, long long>(g, a, s);

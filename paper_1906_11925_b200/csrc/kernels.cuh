@@ -23,6 +23,7 @@ struct DeviceGeometry {
   const void* rec = nullptr;            // [Ns/32][Q-1] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
   BflView bfl;                          // as stored; the API passes it to a launch only when due
+  bool iolet_full = false;              // some iolet is a velocity iolet or has a normal
   bool pdl = true;                      // programmatic dependent launch of the step kernels
   bool index64 = false;                 // flat offsets need (or are forced to) 64 bits
   // > 0: every thread L2-prefetches what site i + prefetch_* will load (about 3/4 of the
