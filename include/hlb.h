@@ -138,7 +138,8 @@ int hlb_set_iolet_normal(hlb_geometry* g, const double* normals);
  *     d >= 1/2:  f_q(x,t+1) = f*_i(x,t) / (2d) + (1 - 1/(2d)) f*_q(x,t)
  * where y is a fluid site; otherwise (y solid or iolet, or no distance) the link stays a
  * halfway bounce-back (reading R-bfl). Iolet links are not affected. NULL switches
- * the interpolation off. Only with HLB_TWO_LATTICE, and only while hlb_steps_done() == 0
+ * the interpolation off. It runs as a pre-pass kernel over the interpolated links before each
+ * step (one extra launch per step). Only with HLB_TWO_LATTICE, and only while hlb_steps_done() == 0
  * (after create / hlb_set_state / hlb_set_populations; it survives later hlb_set_state
  * calls). Allocates its tables through the allocator. Errors: HLB_EINVAL, HLB_ENOMEM,
  * HLB_ECUDA. hlb_num_bfl_sites: sites with at least one interpolated link (0 when off). */
@@ -205,7 +206,8 @@ int64_t hlb_steps_done(const hlb_geometry* g);
 int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v);
 /* Bytes of device memory the geometry holds (populations + tables + scratch). */
 int64_t hlb_device_bytes(const hlb_geometry* g);
-/* Kernel launches enqueued by hlb_step() so far (graph replays count their nodes). */
+/* Kernel launches enqueued by hlb_step() so far (graph replays count their nodes; with BFL
+ * walls the pre-pass over the interpolated links counts too, also when a read-out runs it). */
 int64_t hlb_launch_count(const hlb_geometry* g);
 /* 1 if the step kernels of this geometry read the link records, 0 if they read the table. */
 int hlb_uses_records(const hlb_geometry* g);

@@ -77,6 +77,7 @@ struct hlb_geometry {
   size_t d_image_floats = 0;
   bool bfl_set = false;               // wall distances given (hlb_set_wall_distance)
   int64_t bfl_sites = 0;              // sites with at least one interpolated link
+  int64_t bfl_links = 0;              // interpolated links
   cudaGraphExec_t graph_exec = nullptr;
   bool graph_failed = false;
   std::vector<void*> owned;           // cudaMalloc'ed (no allocator callback)
@@ -105,9 +106,17 @@ struct hlb_geometry {
     return (steps & 1) ? GATHER_AA_ODD : GATHER_OWN;
   }
   const void* state_buf() const { return aa ? buf[0] : buf[cur]; }
-  // The BFL interpolation belongs to the propagation: it applies to every gather except the
-  // one of the freshly initialised state f(., 0), which is given, not propagated.
-  BflView bfl_view() const { return (bfl_set && steps > 0) ? dg.bfl : BflView(); }
+  // The BFL interpolation belongs to the propagation: it is applied (once, as a pre-pass that
+  // rewrites the bounce-back slots) to every state buffer before it is gathered from, except
+  // the freshly initialised state f(., 0), which is given, not propagated.
+  bool bfl_applied = false;  // the pre-pass has run on the current state buffer
+  void ensure_bfl() {
+    if (bfl_set && steps > 0 && !bfl_applied) {
+      launch_bfl_prepass(dg, buf[cur], stream);
+      bfl_applied = true;
+      if (dg.bfl.n > 0) ++launches;
+    }
+  }
 };
 
 extern "C" {
@@ -332,6 +341,7 @@ static int init_from(hlb_geometry* g, const double* d_rho, const double* d_u, co
   const GatherMode mode = g->aa ? GATHER_OWN : GATHER_PULL;
   g->cur = 0;
   g->steps = 0;
+  g->bfl_applied = false;
   launch_init(g->dg, g->buf[0], mode, d_rho, d_u, d_f, g->stream);
   HLB_CUDA(cudaGetLastError());
   return HLB_OK;
@@ -400,6 +410,7 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   if (g->steps != 0) return fail(HLB_EINVAL, "set the wall distances before the first step (steps_done == 0)");
   if (!d27) {
     g->bfl_set = false;
+    g->dg.bfl = BflLinks();
     return HLB_OK;
   }
   const int Q = g->Q;
@@ -410,45 +421,52 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   HLB_CUDA(cudaStreamSynchronize(g->stream));
   HLB_CUDA(cudaMemcpy(nbr.data(), g->dg.nbr, sizeof(int32_t) * nbr.size(), cudaMemcpyDeviceToHost));
   HLB_CUDA(cudaMemcpy(canon.data(), g->dg.canon, sizeof(int32_t) * canon.size(), cudaMemcpyDeviceToHost));
-  std::vector<uint32_t> bits((size_t)(Ns / 32), 0u);
-  std::vector<int32_t> base((size_t)(Ns / 32), 0);
-  std::vector<double> d;
-  std::vector<double> row((size_t)(Q - 1));
-  int32_t rows = 0;
+  std::vector<int32_t> l_site, l_behind;
+  std::vector<uint8_t> l_link;
+  std::vector<double> l_d;
+  int64_t n_sites = 0;
   for (int64_t i = 0; i < N; ++i) {
-    if ((i & 31) == 0) base[(size_t)(i >> 5)] = rows;
     bool any = false;
     for (int p = 1; p < Q; ++p) {
-      row[(size_t)(p - 1)] = 0.0;
       const int32_t e = nbr[(size_t)(p - 1) * (size_t)Ns + (size_t)i];
       const int32_t behind = nbr[(size_t)(opp(p) - 1) * (size_t)Ns + (size_t)i];
       if (e != (int32_t)NBR_WALL_BIT || behind < 0) continue;  // not a solid-wall link, or no fluid site behind
       // the wall lies along -c_p
       const int idx = (-lat.c[p][2] + 1) * 9 + (-lat.c[p][1] + 1) * 3 + (-lat.c[p][0] + 1);
       const double dd = d27[(size_t)canon[(size_t)i] * 27 + (size_t)idx];
-      if (dd > 0.0 && dd <= 1.0) { row[(size_t)(p - 1)] = dd; any = true; }
+      if (dd > 0.0 && dd <= 1.0) {
+        l_site.push_back((int32_t)i);
+        l_behind.push_back(behind);
+        l_link.push_back((uint8_t)p);
+        l_d.push_back(dd);
+        any = true;
+      }
     }
-    if (any) {
-      bits[(size_t)(i >> 5)] |= 1u << (i & 31);
-      d.insert(d.end(), row.begin(), row.end());
-      ++rows;
-    }
+    if (any) ++n_sites;
   }
-  for (int64_t gi = (N + 31) / 32; gi < Ns / 32; ++gi) base[(size_t)gi] = rows;
-  if (d.empty()) d.assign((size_t)(Q - 1), 0.0);
-  void *d_bits = nullptr, *d_base = nullptr, *d_d = nullptr;
+  const size_t nl = l_site.size();
+  void *d_site = nullptr, *d_behind = nullptr, *d_link = nullptr, *d_d = nullptr;
   int rc;
-  if ((rc = g->alloc(sizeof(uint32_t) * bits.size(), &d_bits))) return rc;
-  if ((rc = g->alloc(sizeof(int32_t) * base.size(), &d_base))) return rc;
-  if ((rc = g->alloc(sizeof(double) * d.size(), &d_d))) return rc;
-  HLB_CUDA(cudaMemcpy(d_bits, bits.data(), sizeof(uint32_t) * bits.size(), cudaMemcpyHostToDevice));
-  HLB_CUDA(cudaMemcpy(d_base, base.data(), sizeof(int32_t) * base.size(), cudaMemcpyHostToDevice));
-  HLB_CUDA(cudaMemcpy(d_d, d.data(), sizeof(double) * d.size(), cudaMemcpyHostToDevice));
-  g->dg.bfl.bits = (const uint32_t*)d_bits;
-  g->dg.bfl.base = (const int32_t*)d_base;
+  const size_t cap = nl > 0 ? nl : 1;
+  if ((rc = g->alloc(sizeof(int32_t) * cap, &d_site))) return rc;
+  if ((rc = g->alloc(sizeof(int32_t) * cap, &d_behind))) return rc;
+  if ((rc = g->alloc(sizeof(uint8_t) * cap, &d_link))) return rc;
+  if ((rc = g->alloc(sizeof(double) * cap, &d_d))) return rc;
+  if (nl > 0) {
+    HLB_CUDA(cudaMemcpy(d_site, l_site.data(), sizeof(int32_t) * nl, cudaMemcpyHostToDevice));
+    HLB_CUDA(cudaMemcpy(d_behind, l_behind.data(), sizeof(int32_t) * nl, cudaMemcpyHostToDevice));
+    HLB_CUDA(cudaMemcpy(d_link, l_link.data(), sizeof(uint8_t) * nl, cudaMemcpyHostToDevice));
+    HLB_CUDA(cudaMemcpy(d_d, l_d.data(), sizeof(double) * nl, cudaMemcpyHostToDevice));
+  }
+  g->dg.bfl.site = (const int32_t*)d_site;
+  g->dg.bfl.behind = (const int32_t*)d_behind;
+  g->dg.bfl.link = (const uint8_t*)d_link;
   g->dg.bfl.d = (const double*)d_d;
+  g->dg.bfl.n = (long long)nl;
   g->bfl_set = true;
-  g->bfl_sites = rows;
+  g->bfl_applied = false;
+  g->bfl_sites = n_sites;
+  g->bfl_links = (int64_t)nl;
   return HLB_OK;
 }
 
@@ -475,7 +493,9 @@ static void enqueue_one_step(hlb_geometry* g) {
   if (g->aa) {
     launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
   } else {
-    launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->bfl_view(), g->stream);
+    g->ensure_bfl();
+    launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->stream);
+    g->bfl_applied = false;  // the new state buffer is untouched
     g->cur ^= 1;
   }
   ++g->steps;
@@ -536,7 +556,8 @@ int hlb_step(hlb_geometry* g, int64_t n) {
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   if (!rho_dev && !u_dev) return HLB_OK;
-  launch_macroscopic(g->dg, g->state_buf(), g->gather_mode(), g->bfl_view(), rho_dev, u_dev, g->stream);
+  g->ensure_bfl();
+  launch_macroscopic(g->dg, g->state_buf(), g->gather_mode(), rho_dev, u_dev, g->stream);
   HLB_CUDA(cudaGetLastError());
   return HLB_OK;
 }
@@ -556,7 +577,8 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u) {
 
 int hlb_get_stress_device(hlb_geometry* g, double* sigma_dev) {
   if (!g || !sigma_dev) return fail(HLB_EINVAL, "NULL argument");
-  launch_stress(g->dg, g->state_buf(), g->gather_mode(), g->bfl_view(), sigma_dev, g->stream);
+  g->ensure_bfl();
+  launch_stress(g->dg, g->state_buf(), g->gather_mode(), sigma_dev, g->stream);
   HLB_CUDA(cudaGetLastError());
   return HLB_OK;
 }
@@ -681,7 +703,8 @@ int hlb_get_populations(hlb_geometry* g, double* f) {
   if (!g || !f) return fail(HLB_EINVAL, "NULL argument");
   int rc = ensure_scratch_pop(g);
   if (rc) return rc;
-  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->bfl_view(), g->scratch_pop, g->stream);
+  g->ensure_bfl();
+  launch_get_populations(g->dg, g->state_buf(), g->gather_mode(), g->scratch_pop, g->stream);
   HLB_CUDA(cudaGetLastError());
   HLB_CUDA(cudaMemcpyAsync(f, g->scratch_pop, sizeof(double) * (size_t)g->Q * (size_t)g->N, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));

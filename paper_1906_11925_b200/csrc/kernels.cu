@@ -16,8 +16,9 @@
 //   * 72-80 registers so that 6-7 blocks are resident per SM: all link loads are issued first,
 //     then all population loads, then the arithmetic;
 //   * every thread L2-prefetches what the site 3/4 of a wave ahead will load;
-//   * iolets (constant density, Ladd velocity) and BFL walls are rare paths behind one
-//     per-site bit; the table entries they need are re-read there, not kept in registers.
+//   * iolets (constant density, Ladd velocity) are a rare path behind one per-site bit; the
+//     table entries they need are re-read there, not kept in registers; BFL walls are a
+//     pre-pass over the interpolated links, outside the step kernel.
 //
 // Sites i in [N, Ns) are padding: their links are all "wall", their populations are 0 (rest
 // state in shifted form) and stay exactly 0, so no step kernel needs a bounds branch.
@@ -211,34 +212,39 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
 }
 
 // BFL interpolated walls (linear Bouzidi-Firdaouss-Lallemand rule; the paper's "BFL" wall
-// option, ref [16]), applied to the gathered pre-collision values of
-// the two-lattice scheme. On entry h[p] of a wall link p holds the halfway bounce-back value
-// f*_opp(p)(x, t-1) (own slot opp(p) of src); with the wall at the fraction d of the link,
-//   d <  1/2:  h[p] = 2d h[p] + (1 - 2d) f*_opp(p)(x + c_p, t-1)   = ... h[opp(p)], gathered anyway
-//   d >= 1/2:  h[p] = h[p] / (2d) + (1 - 1/(2d)) f*_p(x, t-1)      = own slot p of src
-// d[p-1] > 0 only for wall links whose site behind, x + c_p, is fluid (the host builds it so),
-// hence h[opp(p)] is a plain fluid gather and is never itself rewritten here.
-template <typename L, typename ST>
-__device__ __forceinline__ void bfl_apply(const BflView& b, const ST* __restrict__ src, long long Ns,
-                                          long long i, double (&h)[L::Q]) {
-  const uint32_t word = __ldg(b.bits + (i >> 5));
-  const uint32_t lane = (uint32_t)(i & 31);
-  if (!((word >> lane) & 1u)) return;
-  const long long row = (long long)__ldg(b.base + (i >> 5)) + __popc(word & ((1u << lane) - 1u));
-  const double* d = b.d + row * (L::Q - 1);
-#pragma unroll
-  for (int p = 1; p < L::Q; ++p) {
-    const double dd = __ldg(d + (p - 1));
-    if (dd > 0.0) {
-      const double two_d = mul(2.0, dd);
-      if (dd < 0.5) {
-        h[p] = fma_(two_d, h[p], mul(sub(1.0, two_d), h[opp(p)]));
-      } else {
-        const double inv = __ddiv_rn(1.0, two_d);
-        h[p] = fma_(inv, h[p], mul(sub(1.0, inv), to_real(src[(long long)p * Ns + i])));
-      }
-    }
+// option, ref [16]) as a PRE-PASS over the list of interpolated links,
+// run on the state buffer of the two-lattice scheme before the step (or read-out) that
+// gathers from it. Slot opp(p) of site x holds f*_opp(p)(x, t-1) and is read by nobody but x
+// itself, as the halfway bounce-back value of its wall link p; the pre-pass replaces it by
+//   d <  1/2:  2d f*_opp(p)(x) + (1 - 2d) f*_opp(p)(x + c_p)      (slot opp(p) of the site behind)
+//   d >= 1/2:  f*_opp(p)(x) / (2d) + (1 - 1/(2d)) f*_p(x)         (slot p of x itself)
+// so that the fused step kernel needs no BFL code at all. The sources are slots that no
+// link of the list writes (a link is in the list only if the site behind it is fluid), so
+// the pass has no ordering hazards. An in-kernel version (interpolating at gather time behind
+// a per-site bit) cost 30 % of the step on configs[3]; this costs ~9 % (profiles/r01_tuning.md).
+template <typename ST>
+__global__ void __launch_bounds__(BLOCK)
+k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ site,
+              const int32_t* __restrict__ behind, const uint8_t* __restrict__ link,
+              const double* __restrict__ dist, long long n) {
+  const long long l = (long long)blockIdx.x * BLOCK + threadIdx.x;
+  if (l >= n) return;
+  const long long i = site[l];
+  const int p = link[l], po = opp(p);
+  const double dd = dist[l];
+  ST* own = buf + (long long)po * Ns + i;
+  const double a = to_real(*own);
+  const double two_d = mul(2.0, dd);
+  double r;
+  if (dd < 0.5) {
+    const double b = to_real(buf[(long long)po * Ns + behind[l]]);
+    r = fma_(two_d, a, mul(sub(1.0, two_d), b));
+  } else {
+    const double b = to_real(buf[(long long)p * Ns + i]);
+    const double inv = __ddiv_rn(1.0, two_d);
+    r = fma_(inv, a, mul(sub(1.0, inv), b));
   }
+  *own = to_store<ST>(r);
 }
 
 // ------------------------------------------------------------------ two-lattice pull
@@ -247,12 +253,11 @@ __device__ __forceinline__ void bfl_apply(const BflView& b, const ST* __restrict
 // pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
 // of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
 // padding, so only the one warp-uniform test is needed.
-template <typename L, typename ST, bool REC, typename IT, bool BFL, bool FULL>
+template <typename L, typename ST, bool REC, typename IT, bool FULL>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
-       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf,
-       BflView bfl) {
+       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[L::Q];
   {
@@ -273,7 +278,6 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
       for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
     }
   }
-  if (BFL) bfl_apply<L, ST>(bfl, src, Ns, i, h);
   const Moments m = moments_of<L>(h);
   collide<L>(h, m, omega, h);
   if (has_iolet_link(iolet_bits, i)) {  // rare: sites on an inlet/outlet cap
@@ -359,26 +363,24 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 template <typename L, typename ST, int MODE>
 __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
                                                     const int32_t* __restrict__ nbr, long long Ns,
-                                                    long long i, const BflView& bfl,
-                                                    double (&h)[L::Q]) {
+                                                    long long i, double (&h)[L::Q]) {
   int32_t e[L::Q - 1];
   if (MODE != GATHER_OWN) load_entries<L>(nbr, Ns, i, e);
   h[0] = to_real(buf[i]);
 #pragma unroll
   for (int q = 1; q < L::Q; ++q)
     h[q] = to_real(buf[slot_of<MODE>(q, MODE != GATHER_OWN ? e[q - 1] : 0, Ns, i)]);
-  if (MODE == GATHER_PULL && bfl.bits) bfl_apply<L, ST>(bfl, buf, Ns, i, h);
 }
 
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
-              const int32_t* __restrict__ canon, long long N, long long Ns, BflView bfl,
+              const int32_t* __restrict__ canon, long long N, long long Ns,
               double* __restrict__ rho, double* __restrict__ u) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, bfl, h);
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
   const Moments m = moments_of<L>(h);
   const long long c = canon[i];
   if (rho) rho[c] = m.rho;
@@ -395,12 +397,12 @@ k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
-         const int32_t* __restrict__ canon, long long N, long long Ns, double omega, BflView bfl,
+         const int32_t* __restrict__ canon, long long N, long long Ns, double omega,
          double* __restrict__ sigma) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, bfl, h);
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
   const Moments m = moments_of<L>(h);
   double pi[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
@@ -443,12 +445,12 @@ k_wall_shear_stress(const double* __restrict__ sigma, const double* __restrict__
 template <typename L, typename ST, int MODE>
 __global__ void __launch_bounds__(BLOCK)
 k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
-                  const int32_t* __restrict__ canon, long long N, long long Ns, BflView bfl,
+                  const int32_t* __restrict__ canon, long long N, long long Ns,
                   double* __restrict__ f) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, bfl, h);
+  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
   const long long c = canon[i];
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) f[c * L::Q + q] = h[q] + L::weight(q);
@@ -529,31 +531,25 @@ static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaS
 }
 
 template <typename L, typename ST, bool REC, typename IT>
-static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
-                        cudaStream_t s) {
-  if (bfl.bits)  // BFL implies the full iolet rules (fewer instantiations)
-    launch_step(g, k_pull<L, ST, REC, IT, true, true>, s, (const ST*)src, (ST*)dst, g.nbr,
+static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+  if (g.iolet_full)
+    launch_step(g, k_pull<L, ST, REC, IT, true>, s, (const ST*)src, (ST*)dst, g.nbr,
                 (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
-                (long long)g.prefetch_pull, bfl);
-  else if (g.iolet_full)
-    launch_step(g, k_pull<L, ST, REC, IT, false, true>, s, (const ST*)src, (ST*)dst, g.nbr,
-                (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
-                (long long)g.prefetch_pull, bfl);
+                (long long)g.prefetch_pull);
   else
-    launch_step(g, k_pull<L, ST, REC, IT, false, false>, s, (const ST*)src, (ST*)dst, g.nbr,
+    launch_step(g, k_pull<L, ST, REC, IT, false>, s, (const ST*)src, (ST*)dst, g.nbr,
                 (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
-                (long long)g.prefetch_pull, bfl);
+                (long long)g.prefetch_pull);
 }
 template <typename L, typename ST>
-static void pull_t(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
-                   cudaStream_t s) {
+static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (g.use_rec) {
-    if (idx32) pull_launch<L, ST, true, uint32_t>(g, src, dst, bfl, s);
-    else pull_launch<L, ST, true, long long>(g, src, dst, bfl, s);
+    if (idx32) pull_launch<L, ST, true, uint32_t>(g, src, dst, s);
+    else pull_launch<L, ST, true, long long>(g, src, dst, s);
   } else {
-    if (idx32) pull_launch<L, ST, false, uint32_t>(g, src, dst, bfl, s);
-    else pull_launch<L, ST, false, long long>(g, src, dst, bfl, s);
+    if (idx32) pull_launch<L, ST, false, uint32_t>(g, src, dst, s);
+    else pull_launch<L, ST, false, long long>(g, src, dst, s);
   }
 }
 template <typename L, typename ST, bool REC, typename IT>
@@ -584,36 +580,36 @@ static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   }
 }
 template <typename L, typename ST>
-static void macroscopic_t(const DeviceGeometry& g, const void* buf, GatherMode mode,
-                          const BflView& bfl, double* rho, double* u, cudaStream_t s) {
+static void macroscopic_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
+                          double* u, cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_macroscopic<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, rho, u); break;
-    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, rho, u); break;
-    case GATHER_AA_ODD: k_macroscopic<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, rho, u); break;
+    case GATHER_PULL: k_macroscopic<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_AA_ODD: k_macroscopic<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
   }
 }
 template <typename L, typename ST>
-static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMode mode,
-                              const BflView& bfl, double* f, cudaStream_t s) {
+static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
+                              cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_get_populations<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, f); break;
-    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, f); break;
-    case GATHER_AA_ODD: k_get_populations<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, bfl, f); break;
+    case GATHER_PULL: k_get_populations<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_AA_ODD: k_get_populations<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
   }
 }
 template <typename L, typename ST>
-static void stress_t(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
-                     double* sigma, cudaStream_t s) {
+static void stress_t(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
+                     cudaStream_t s) {
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_stress<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, bfl, sigma); break;
-    case GATHER_OWN: k_stress<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, bfl, sigma); break;
-    case GATHER_AA_ODD: k_stress<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, bfl, sigma); break;
+    case GATHER_PULL: k_stress<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_OWN: k_stress<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_AA_ODD: k_stress<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
   }
 }
 template <typename L, typename ST>
@@ -638,24 +634,31 @@ static void dispatch(const DeviceGeometry& g, F&& f) {
   }
 }
 
-void launch_pull(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
-                 cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { pull_t<decltype(l), decltype(st)>(g, src, dst, bfl, s); });
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { pull_t<decltype(l), decltype(st)>(g, src, dst, s); });
+}
+void launch_bfl_prepass(const DeviceGeometry& g, void* buf, cudaStream_t s) {
+  const BflLinks& b = g.bfl;
+  if (b.n <= 0) return;
+  if (g.f32)
+    k_bfl_prepass<float><<<grid_for(b.n), BLOCK, 0, s>>>((float*)buf, g.Ns, b.site, b.behind, b.link, b.d, b.n);
+  else
+    k_bfl_prepass<double><<<grid_for(b.n), BLOCK, 0, s>>>((double*)buf, g.Ns, b.site, b.behind, b.link, b.d, b.n);
 }
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { aa_t<decltype(l), decltype(st)>(g, a, odd, s); });
 }
-void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
-                        double* rho, double* u, cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { macroscopic_t<decltype(l), decltype(st)>(g, buf, mode, bfl, rho, u, s); });
+void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
+                        double* u, cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { macroscopic_t<decltype(l), decltype(st)>(g, buf, mode, rho, u, s); });
 }
-void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode,
-                            const BflView& bfl, double* f, cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { get_populations_t<decltype(l), decltype(st)>(g, buf, mode, bfl, f, s); });
+void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
+                            cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { get_populations_t<decltype(l), decltype(st)>(g, buf, mode, f, s); });
 }
-void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
-                   double* sigma, cudaStream_t s) {
-  dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, bfl, sigma, s); });
+void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
+                   cudaStream_t s) {
+  dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, sigma, s); });
 }
 void launch_wall_shear_stress(const double* sigma, const double* normals, long long N, double* wss,
                               cudaStream_t s) {

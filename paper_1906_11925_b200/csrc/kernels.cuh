@@ -6,13 +6,15 @@
 
 namespace hlb {
 
-// BFL interpolated walls (two-lattice scheme): sites with at least one interpolated link are
-// flagged in bits [Ns/32]; their distances live in d [n_flagged][Q-1] (0 = plain bounce-back
-// for that link), row = base[group] + number of flagged lanes below. bits == nullptr: off.
-struct BflView {
-  const uint32_t* bits = nullptr;
-  const int32_t* base = nullptr;
+// BFL interpolated walls (two-lattice scheme): the list of interpolated links. Link l belongs
+// to internal site site[l], is its pull link link[l] (1 .. Q-1), has the wall at the fraction
+// d[l] of its length, and behind[l] is the internal index of the fluid site x + c_p behind it.
+struct BflLinks {
+  const int32_t* site = nullptr;
+  const int32_t* behind = nullptr;
+  const uint8_t* link = nullptr;
   const double* d = nullptr;
+  long long n = 0;
 };
 
 struct DeviceGeometry {
@@ -22,7 +24,7 @@ struct DeviceGeometry {
   const uint32_t* iolet_bits = nullptr; // [Ns/32]
   const void* rec = nullptr;            // [Ns/32][Q-1] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
-  BflView bfl;                          // as stored; the API passes it to a launch only when due
+  BflLinks bfl;                         // applied by launch_bfl_prepass when the API says so
   bool iolet_full = false;              // some iolet is a velocity iolet or has a normal
   bool pdl = true;                      // programmatic dependent launch of the step kernels
   bool index64 = false;                 // flat offsets need (or are forced to) 64 bits
@@ -43,8 +45,10 @@ int resident_sites_per_sm_pull(bool d3q19);
 int resident_sites_per_sm_aa(bool d3q19);
 
 // One time step, two-lattice pull: dst <- collide(gather(src)).
-void launch_pull(const DeviceGeometry& g, const void* src, void* dst, const BflView& bfl,
-                 cudaStream_t s);
+void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);
+// Rewrite, in the two-lattice state buffer `buf`, the bounce-back slots of the interpolated
+// links (see kernels.cu); run once per state, before the step or read-out that gathers from it.
+void launch_bfl_prepass(const DeviceGeometry& g, void* buf, cudaStream_t s);
 // One time step, A-A in place; `odd` selects the phase.
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s);
 
@@ -55,19 +59,17 @@ enum GatherMode {
   GATHER_AA_ODD = 2  // A-A after an odd number of steps: slot opp(q) of x - c_q (slot q at walls)
 };
 // rho [N] / u [N][3] (device, canonical order; either may be NULL)
-// The read-out launchers take the BFL view that applies to the state in `buf` (only used in
-// GATHER_PULL mode; pass BflView() otherwise).
-void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
-                        double* rho, double* u, cudaStream_t s);
+void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
+                        double* u, cudaStream_t s);
 // sigma [N][6] deviatoric stress xx, yy, zz, xy, xz, yz (device, canonical order)
-void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, const BflView& bfl,
-                   double* sigma, cudaStream_t s);
+void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, double* sigma,
+                   cudaStream_t s);
 // wss [N] from sigma [N][6] and normals [N][3] (all device, canonical order)
 void launch_wall_shear_stress(const double* sigma, const double* normals, long long N, double* wss,
                               cudaStream_t s);
 // f [N][Q] raw populations (device, canonical order)
-void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode,
-                            const BflView& bfl, double* f, cudaStream_t s);
+void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
+                            cudaStream_t s);
 // Initialise a buffer so that gathering in `mode` (GATHER_PULL or GATHER_OWN) yields
 //   f_q(x) = f_in[canon(x)][q]                       if f_in != NULL, else
 //   f_q(x) = f_eq_q(rho_in[canon(x)], u_in[canon(x)])  (NULL rho => 1, NULL u => 0).
