@@ -240,6 +240,7 @@ def time_renderer(hlb, g, wl, pixels, frames=12):
     import torch
     nx, ny, nz = wl.shape
     lut = np.stack([np.linspace(0, 1, 256)] * 3 + [np.full(256, 0.02)], axis=1).astype(np.float32)
+    lut[0, 3] = 0.0          # value 0 (solid voxels, fluid at rest) is transparent: empty cells are skipped
     rho, u = g.hlb_get_macroscopic()
     umax = float(np.max(np.linalg.norm(u, axis=1))) or 1.0
     zoom = pixels / float(max(nx, ny, nz))
@@ -265,6 +266,7 @@ def time_renderer(hlb, g, wl, pixels, frames=12):
             "volume_voxels": nx * ny * nz, "sample_step": 0.5,
             "ray_samples_per_frame_upper_bound": int(rays * (diag / 0.5 + 1)),
             "includes": "macroscopic read-out + scatter into the voxel volume + ray march, per frame",
+            "empty_space_skipping": not os.environ.get("HLB_RENDER_NO_SKIP", "0").strip("0"),
             "max_alpha": float(img[..., 3].max())}
 
 

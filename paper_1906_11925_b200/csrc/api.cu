@@ -73,6 +73,7 @@ struct hlb_geometry {
   // the per-launch host cost that dominates small geometries (BASELINE configs[0], [2])
   float* volume = nullptr;            // [nz][ny][nx] floats for hlb_render (lazy)
   long long* d_voxels = nullptr;      // [N] canonical voxel index on the device (lazy)
+  unsigned char* occ = nullptr;       // macro-cell emptiness of the volume (solid cells; lazy)
   float* d_image = nullptr;           // staging image for hlb_render
   size_t d_image_floats = 0;
   bool bfl_set = false;               // wall distances given (hlb_set_wall_distance)
@@ -623,6 +624,13 @@ static int check_view(const hlb_view* v, const float* lut, RenderSetup& r) {
   return HLB_OK;
 }
 
+// HLB_RENDER_NO_SKIP=1 in the environment turns the empty-space skipping off (same image; for
+// measurement only)
+static bool render_skip_disabled() {
+  static const bool off = [] { const char* e = getenv("HLB_RENDER_NO_SKIP"); return e && *e && *e != '0'; }();
+  return off;
+}
+
 int hlb_render_volume(const float* volume, int32_t nx, int32_t ny, int32_t nz, const hlb_view* view,
                       const float* lut, float* image, void* stream) {
   if (!volume || !image) return fail(HLB_EINVAL, "NULL argument");
@@ -635,15 +643,18 @@ int hlb_render_volume(const float* volume, int32_t nx, int32_t ny, int32_t nz, c
   const size_t vbytes = sizeof(float) * (size_t)nx * (size_t)ny * (size_t)nz;
   const size_t ibytes = sizeof(float) * 4 * (size_t)view->width * (size_t)view->height;
   float *d_vol = nullptr, *d_img = nullptr;
-  auto done = [&](int code) { cudaFree(d_vol); cudaFree(d_img); return code; };
-  if (cudaMalloc((void**)&d_vol, vbytes) != cudaSuccess || cudaMalloc((void**)&d_img, ibytes) != cudaSuccess) {
+  unsigned char* d_occ = nullptr;
+  auto done = [&](int code) { cudaFree(d_vol); cudaFree(d_img); cudaFree(d_occ); return code; };
+  if (cudaMalloc((void**)&d_vol, vbytes) != cudaSuccess || cudaMalloc((void**)&d_img, ibytes) != cudaSuccess ||
+      cudaMalloc((void**)&d_occ, (size_t)occupancy_cells(nx, ny, nz)) != cudaSuccess) {
     const cudaError_t e = cudaGetLastError();
     return done(e == cudaErrorMemoryAllocation ? fail(HLB_ENOMEM, "cudaMalloc: out of memory")
                                                : cuda_fail(e, "cudaMalloc"));
   }
   cudaError_t e = cudaMemcpyAsync(d_vol, volume, vbytes, cudaMemcpyHostToDevice, s);
   if (e == cudaSuccess) e = render_upload(r, lut, s);
-  if (e == cudaSuccess) { launch_raymarch(r, d_vol, d_img, s); e = cudaGetLastError(); }
+  if (e == cudaSuccess) { launch_occupancy(d_vol, nx, ny, nz, d_occ, s); e = cudaGetLastError(); }
+  if (e == cudaSuccess) { launch_raymarch(r, d_vol, render_skip_disabled() ? nullptr : d_occ, d_img, s); e = cudaGetLastError(); }
   if (e == cudaSuccess) e = cudaMemcpyAsync(image, d_img, ibytes, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return done(cuda_fail(e, "hlb_render_volume"));
@@ -673,10 +684,20 @@ int hlb_render_device(hlb_geometry* g, const hlb_view* view, const float* lut, f
   double* d_u = g->scratch + g->N;
   rc = hlb_get_macroscopic_device(g, d_rho, d_u);
   if (rc) return rc;
+  if (!g->occ && !render_skip_disabled()) {
+    // Only fluid voxels are ever written, so a macro-cell without fluid stays empty for good:
+    // mark every fluid voxel with a non-zero value once and take the occupancy of that.
+    void* ptr = nullptr;
+    if ((rc = g->alloc((size_t)occupancy_cells(r.nx, r.ny, r.nz), &ptr))) return rc;
+    launch_scatter_field(d_rho, d_u, g->d_voxels, g->N, 2, g->volume, g->stream);  // field 2: the constant 1
+    launch_occupancy(g->volume, r.nx, r.ny, r.nz, (unsigned char*)ptr, g->stream);
+    HLB_CUDA(cudaGetLastError());
+    g->occ = (unsigned char*)ptr;
+  }
   launch_scatter_field(d_rho, d_u, g->d_voxels, g->N, view->field, g->volume, g->stream);
   HLB_CUDA(cudaGetLastError());
   HLB_CUDA(render_upload(r, lut, g->stream));
-  launch_raymarch(r, g->volume, image_dev, g->stream);
+  launch_raymarch(r, g->volume, g->occ, image_dev, g->stream);
   HLB_CUDA(cudaGetLastError());
   return HLB_OK;
 }

@@ -57,8 +57,13 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ vol, int nx
 
 constexpr int TILE = 16;
 
+// occ (may be NULL): one byte per 8 x 8 x 8 macro-cell, 1 = every voxel a sample of the cell
+// can touch ([8c, 8c + 8] per axis) is exactly +0. Such a sample has the value +0 exactly; if
+// the transfer function gives value 0 no opacity, it contributes exactly nothing and may be
+// skipped, together with the following samples that provably stay in the same cell. The
+// image is therefore bit-identical with and without occ.
 __global__ void __launch_bounds__(TILE * TILE)
-k_raymarch(const float* __restrict__ vol, float* __restrict__ image) {
+k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ, float* __restrict__ image) {
   const int px = blockIdx.x * TILE + threadIdx.x, py = blockIdx.y * TILE + threadIdx.y;
   const ViewParams& v = c_view;
   if (px >= v.width || py >= v.height) return;
@@ -100,11 +105,45 @@ k_raymarch(const float* __restrict__ vol, float* __restrict__ image) {
       k1 = min(K - 1, (int)ceilf((z1 + T) / v.step) + 2);
     }
   }
+  // does the value 0 have zero opacity? (same operations as for a sample of value 0)
+  bool skip_empty = false;
+  if (occ) {
+    const float t0 = clamp01(__fmaf_rn(0.0f, v.tf_scale, v.tf_offset));
+    const int i0 = (int)__fmaf_rn(t0, 255.0f, 0.5f);
+    skip_empty = clamp01(__fmul_rn(c_lut[4 * i0 + 3], v.opacity)) == 0.0f;
+  }
+  const int mx = (v.nx + 7) >> 3, my = (v.ny + 7) >> 3;
+  const float r2[3] = {v.rot[2], v.rot[5], v.rot[8]};
   float Cr = 0.0f, Cg = 0.0f, Cb = 0.0f, A = 0.0f;
   for (int k = k0; k <= k1; ++k) {
     const float Z = __fmaf_rn((float)k, v.step, -T);
     const float qx = __fmaf_rn(v.rot[2], Z, bx), qy = __fmaf_rn(v.rot[5], Z, by), qz = __fmaf_rn(v.rot[8], Z, bz);
     if (qx < 0.0f || qx > hx || qy < 0.0f || qy > hy || qz < 0.0f || qz > hz) continue;
+    if (skip_empty) {
+      // the cell of the sample's lower corner voxel, as trilinear() clamps it
+      const int ix = max(min((int)floorf(qx), v.nx - 2), 0), iy = max(min((int)floorf(qy), v.ny - 2), 0),
+                iz = max(min((int)floorf(qz), v.nz - 2), 0);
+      const int cxm = ix >> 3, cym = iy >> 3, czm = iz >> 3;
+      if (__ldg(occ + ((long long)czm * my + cym) * mx + cxm)) {
+        // conservative count of further samples whose lower corner stays in this cell: keep a
+        // margin (>= 0.01 voxel, far above the rounding of the sample positions) clear of the
+        // cell faces; an axis the ray hardly moves along must already be clear of them
+        const float q[3] = {qx, qy, qz};
+        const int c8[3] = {cxm << 3, cym << 3, czm << 3};
+        float room = 1e30f;  // distance in Z the ray may still travel
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          const float margin = 0.01f * (1.0f + fabsf(r2[a]));
+          const float hi = (float)(c8[a] + 8) - margin - q[a], lo = q[a] - (float)c8[a] - margin;
+          if (r2[a] > 1e-6f) room = fminf(room, hi / r2[a]);
+          else if (r2[a] < -1e-6f) room = fminf(room, lo / -r2[a]);
+          else if (hi < 0.0f || lo < 0.0f) room = 0.0f;
+        }
+        const int jump = room > 0.0f ? (int)fminf(floorf(room / v.step) - 1.0f, 1.0e6f) : 0;
+        if (jump > 0) k += jump;
+        continue;
+      }
+    }
     const float val = trilinear(vol, v.nx, v.ny, v.nz, qx, qy, qz);
     const float t = clamp01(__fmaf_rn(val, v.tf_scale, v.tf_offset));
     const int i = (int)__fmaf_rn(t, 255.0f, 0.5f);
@@ -127,7 +166,9 @@ k_scatter_field(const double* __restrict__ rho, const double* __restrict__ u,
   const long long c = (long long)blockIdx.x * 256 + threadIdx.x;
   if (c >= N) return;
   double s;
-  if (field == 1) {
+  if (field == 2) {
+    s = 1.0;  // marks the fluid voxels (occupancy of the geometry)
+  } else if (field == 1) {
     s = rho[c] - 1.0;
   } else {
     const double ux = u[3 * c], uy = u[3 * c + 1], uz = u[3 * c + 2];
@@ -150,9 +191,37 @@ cudaError_t render_upload(const RenderSetup& r, const float* lut_host, cudaStrea
   return cudaStreamSynchronize(s);  // v is a stack object; lut_host is the caller's
 }
 
-void launch_raymarch(const RenderSetup& r, const float* vol, float* image, cudaStream_t s) {
+void launch_raymarch(const RenderSetup& r, const float* vol, const unsigned char* occ, float* image,
+                     cudaStream_t s) {
   const dim3 grid((unsigned)((r.width + TILE - 1) / TILE), (unsigned)((r.height + TILE - 1) / TILE));
-  k_raymarch<<<grid, dim3(TILE, TILE), 0, s>>>(vol, image);
+  k_raymarch<<<grid, dim3(TILE, TILE), 0, s>>>(vol, occ, image);
+}
+
+namespace {
+// one warp per macro-cell: 1 if all voxels of [8c, 8c + 8] (clipped to the box) are +0.0f bits
+__global__ void __launch_bounds__(256)
+k_occupancy(const float* __restrict__ vol, int nx, int ny, int nz, unsigned char* __restrict__ occ) {
+  const int mx = (nx + 7) >> 3, my = (ny + 7) >> 3, mz = (nz + 7) >> 3;
+  const long long cell = ((long long)blockIdx.x * 256 + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (cell >= (long long)mx * my * mz) return;
+  const int cx = (int)(cell % mx), cy = (int)((cell / mx) % my), cz = (int)(cell / ((long long)mx * my));
+  unsigned any = 0u;
+  for (int t = lane; t < 9 * 9 * 9; t += 32) {
+    const int x = (cx << 3) + t % 9, y = (cy << 3) + (t / 9) % 9, z = (cz << 3) + t / 81;
+    if (x < nx && y < ny && z < nz) any |= __float_as_uint(__ldg(vol + ((long long)z * ny + y) * nx + x));
+  }
+  any = __reduce_or_sync(0xffffffffu, any);
+  if (lane == 0) occ[cell] = any == 0u ? 1 : 0;
+}
+}  // namespace
+
+long long occupancy_cells(int nx, int ny, int nz) {
+  return (long long)((nx + 7) >> 3) * ((ny + 7) >> 3) * ((nz + 7) >> 3);
+}
+void launch_occupancy(const float* vol, int nx, int ny, int nz, unsigned char* occ, cudaStream_t s) {
+  const long long threads = occupancy_cells(nx, ny, nz) * 32;
+  k_occupancy<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(vol, nx, ny, nz, occ);
 }
 
 void launch_scatter_field(const double* rho, const double* u, const long long* voxel, long long N,

@@ -12,8 +12,13 @@ struct RenderSetup {
 
 // Copies the viewing parameters and the 256 x RGBA look-up table (host) into constant memory.
 cudaError_t render_upload(const RenderSetup& r, const float* lut_host, cudaStream_t s);
-// image [height][width][4] floats (device), vol [nz][ny][nx] floats (device)
-void launch_raymarch(const RenderSetup& r, const float* vol, float* image, cudaStream_t s);
+// image [height][width][4] floats (device), vol [nz][ny][nx] floats (device); occ: macro-cell
+// emptiness bytes from launch_occupancy, or NULL (no empty-space skipping; same image)
+void launch_raymarch(const RenderSetup& r, const float* vol, const unsigned char* occ, float* image,
+                     cudaStream_t s);
+// occ [occupancy_cells()] bytes: 1 where every voxel a sample of the 8^3 macro-cell can touch is +0
+long long occupancy_cells(int nx, int ny, int nz);
+void launch_occupancy(const float* vol, int nx, int ny, int nz, unsigned char* occ, cudaStream_t s);
 // vol[voxel[c]] = |u| (field 0) or rho - 1 (field 1) of canonical site c
 void launch_scatter_field(const double* rho, const double* u, const long long* voxel, long long N,
                           int field, float* vol, cudaStream_t s);

@@ -60,6 +60,66 @@ def test_render_volume_equals_oracle_bitwise(hlb, shape, view):
         assert inside > 0 and np.max(ref[..., 3]) > 0.05           # the comparison is not of black images
 
 
+def clear_lut(first_opaque=1, alpha=0.06):
+    """A look-up table whose entries below `first_opaque` are fully transparent: value 0 then
+    contributes nothing and the renderer may skip empty macro-cells."""
+    lut = rainbow_lut(alpha)
+    lut[:first_opaque, 3] = 0.0
+    return lut
+
+
+SKIP_VIEWS = VIEWS + [
+    dict(rot=rotation((1, 0, 0), 90), zoom=1.3, step=0.25, tf_scale=1.0, tf_offset=0.0, opacity=2.0),
+    dict(rot=rotation((0, 1, 0), 90.0001), zoom=2.0, step=0.11, tf_scale=1.5, tf_offset=0.0, opacity=1.0),
+    dict(rot=rotation((3, 1, -2), 131), zoom=0.9, step=1.9, tf_scale=1.0, tf_offset=0.001, opacity=1.0),
+]
+
+
+def sparse_volume(shape, seed):
+    """Mostly exact zeros with a few blobs, a thin diagonal tube and isolated voxels on cell faces."""
+    rng = np.random.default_rng(seed)
+    vol = np.zeros(shape, dtype=np.float32)
+    nz, ny, nx = shape
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    for _ in range(3):
+        c = rng.random(3) * np.array(shape)
+        r = 2.0 + 5.0 * rng.random()
+        m = (z - c[0]) ** 2 + (y - c[1]) ** 2 + (x - c[2]) ** 2 < r * r
+        vol[m] = rng.random(int(m.sum())).astype(np.float32)
+    t = np.linspace(0, 1, 4 * max(shape))
+    vol[(t * (nz - 1)).astype(int), (t * (ny - 1)).astype(int), (t * (nx - 1)).astype(int)] = 0.8
+    for k in range(0, min(shape), 8):                # single voxels exactly on macro-cell corners
+        vol[k, k, k] = 1.0
+        if k + 7 < min(shape):
+            vol[k + 7, k, k + 7] = 0.6
+    return vol
+
+
+@pytest.mark.parametrize("shape", [(41, 57, 70), (64, 64, 64), (9, 130, 17), (3, 8, 100)])
+@pytest.mark.parametrize("view", range(len(SKIP_VIEWS)))
+def test_empty_space_skipping_keeps_the_image_bitwise(hlb, shape, view):
+    """With a transfer function that is transparent at value 0 the kernel jumps over empty 8^3
+    macro-cells; the image must not change by a single bit (oracle: no skipping at all)."""
+    vol = sparse_volume(shape, 7 * view + shape[2])
+    kw = SKIP_VIEWS[view]
+    for lut in (clear_lut(1), clear_lut(40)):
+        ref, inside = oracle.render(vol, 80, 56, lut=lut, **kw)
+        img = hlb.hlb_render_volume(vol, hlb.make_view(80, 56, **kw), lut)
+        assert np.array_equal(img, ref), float(np.max(np.abs(img - ref)))
+    assert inside > 0
+    if view in (0, 1, 4):
+        assert np.max(ref[..., 3]) > 0.01
+
+
+def test_empty_volume_renders_black(hlb):
+    vol = np.zeros((33, 20, 47), dtype=np.float32)
+    img = hlb.hlb_render_volume(vol, hlb.make_view(40, 40, rot=rotation((1, 1, 0), 50)), clear_lut())
+    assert not img.any()
+    vol[:] = -0.0                                    # not +0: cells are not "empty", result the same
+    img = hlb.hlb_render_volume(vol, hlb.make_view(40, 40, rot=rotation((1, 1, 0), 50)), clear_lut())
+    assert not img.any()
+
+
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
 def test_render_of_a_running_simulation(hlb, scheme):
     """hlb_render: the speed field of the current state scattered into the voxel box and
@@ -71,7 +131,7 @@ def test_render_of_a_running_simulation(hlb, scheme):
     g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
     o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, threads=0)
     o.set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
-    lut = rainbow_lut(0.08)
+    lut = clear_lut(1, 0.08) if scheme == "aa" else rainbow_lut(0.08)   # with / without skipping
     vox = wl.fluid_voxels()
     for n, field in ((80, 0), (35, 1)):
         g.hlb_step(n)
