@@ -138,8 +138,10 @@ int hlb_set_iolet_normal(hlb_geometry* g, const double* normals);
  *     d >= 1/2:  f_q(x,t+1) = f*_i(x,t) / (2d) + (1 - 1/(2d)) f*_q(x,t)
  * where y is a fluid site; otherwise (y solid or iolet, or no distance) the link stays a
  * halfway bounce-back (reading R-bfl). Iolet links are not affected. NULL switches
- * the interpolation off. It runs as a pre-pass kernel over the interpolated links before each
- * step (one extra launch per step). Only with HLB_TWO_LATTICE, and only while hlb_steps_done() == 0
+ * the interpolation off. The step kernels of both schemes apply it in registers (the d >= 1/2
+ * rule to the value a site writes back, the d < 1/2 rule to the values it gathers; no extra
+ * launch per step); a read-out between steps first runs a pre-pass kernel over the d < 1/2
+ * links of the state buffer. Only while hlb_steps_done() == 0
  * (after create / hlb_set_state / hlb_set_populations; it survives later hlb_set_state
  * calls). Allocates its tables through the allocator. Errors: HLB_EINVAL, HLB_ENOMEM,
  * HLB_ECUDA. hlb_num_bfl_sites: sites with at least one interpolated link (0 when off). */

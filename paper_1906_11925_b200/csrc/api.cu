@@ -81,6 +81,15 @@ struct hlb_geometry {
   int64_t bfl_links = 0;              // interpolated links
   cudaGraphExec_t graph_exec = nullptr;
   bool graph_failed = false;
+  // The captured launches fix the kernel instantiation and the by-value arguments: drop the
+  // graph whenever one of them changes (iolet kinds / normals, wall distances).
+  void drop_graph() {
+    if (graph_exec) {
+      cudaStreamSynchronize(stream);
+      cudaGraphExecDestroy(graph_exec);
+      graph_exec = nullptr;
+    }
+  }
   std::vector<void*> owned;           // cudaMalloc'ed (no allocator callback)
 
   int alloc(size_t bytes, void** out) {
@@ -107,13 +116,16 @@ struct hlb_geometry {
     return (steps & 1) ? GATHER_AA_ODD : GATHER_OWN;
   }
   const void* state_buf() const { return aa ? buf[0] : buf[cur]; }
-  // The BFL interpolation belongs to the propagation: it is applied (once, as a pre-pass that
-  // rewrites the bounce-back slots) to every state buffer before it is gathered from, except
-  // the freshly initialised state f(., 0), which is given, not propagated.
+  // The BFL interpolation belongs to the propagation. Its d >= 1/2 part is in what the step
+  // kernels write; its d < 1/2 part is applied to every state when it is gathered from --
+  // by the next step kernel in registers (gather_bfl()), or, before a read-out, once by a
+  // pre-pass that rewrites the bounce-back slots in the state buffer (ensure_bfl()) -- except
+  // to the freshly initialised state f(., 0), which is given, not propagated.
   bool bfl_applied = false;  // the pre-pass has run on the current state buffer
+  bool gather_bfl() const { return bfl_set && steps > 0 && !bfl_applied; }
   void ensure_bfl() {
     if (bfl_set && steps > 0 && !bfl_applied) {
-      launch_bfl_prepass(dg, buf[cur], stream);
+      launch_bfl_prepass(dg, aa ? buf[0] : buf[cur], gather_mode(), stream);
       bfl_applied = true;
       if (dg.bfl.n > 0) ++launches;
     }
@@ -192,6 +204,7 @@ static int upload_iolets(hlb_geometry* g) {
   if (n == 0) return HLB_OK;
   HLB_CUDA(cudaStreamSynchronize(g->stream));  // the previous upload may still read iolet_par
   g->iolet_par.assign((size_t)n * 4, 0.0);
+  const bool was_full = g->dg.iolet_full;
   g->dg.iolet_full = false;
   for (int k = 0; k < n; ++k) {
     if (g->iolet_kind[(size_t)k] == 1 || g->iolet_n[(size_t)k * 3] != 0.0 ||
@@ -205,6 +218,7 @@ static int upload_iolets(hlb_geometry* g) {
       for (int a = 0; a < 3; ++a) g->iolet_par[(size_t)k * 4 + 1 + a] = g->iolet_n[(size_t)k * 3 + a];
     }
   }
+  if (g->dg.iolet_full != was_full) g->drop_graph();  // another instantiation of the step kernels
   HLB_CUDA(cudaMemcpyAsync((void*)g->dg.iolet_par, g->iolet_par.data(), sizeof(double) * 4 * (size_t)n,
                            cudaMemcpyHostToDevice, g->stream));
   return HLB_OK;
@@ -407,11 +421,13 @@ int hlb_set_iolet_normal(hlb_geometry* g, const double* normals) {
 
 int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
-  if (g->aa) return fail(HLB_EINVAL, "interpolated walls need the two-lattice scheme (HLB_TWO_LATTICE)");
   if (g->steps != 0) return fail(HLB_EINVAL, "set the wall distances before the first step (steps_done == 0)");
+  g->drop_graph();
   if (!d27) {
     g->bfl_set = false;
     g->dg.bfl = BflLinks();
+    g->dg.bflf = BflFused();
+    g->dg.bfl_on = false;
     return HLB_OK;
   }
   const int Q = g->Q;
@@ -422,13 +438,14 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   HLB_CUDA(cudaStreamSynchronize(g->stream));
   HLB_CUDA(cudaMemcpy(nbr.data(), g->dg.nbr, sizeof(int32_t) * nbr.size(), cudaMemcpyDeviceToHost));
   HLB_CUDA(cudaMemcpy(canon.data(), g->dg.canon, sizeof(int32_t) * canon.size(), cudaMemcpyDeviceToHost));
-  std::vector<int32_t> l_site, l_behind;
-  std::vector<uint8_t> l_link;
-  std::vector<double> l_d;
-  int64_t n_sites = 0;
-  for (int64_t i = 0; i < N; ++i) {
-    bool any = false;
-    for (int p = 1; p < Q; ++p) {
+  // Every interpolated link, link-major (all links of direction 1, then 2, ...; sites
+  // ascending within each).
+  std::vector<int32_t> a_site, a_behind;
+  std::vector<uint8_t> a_link;
+  std::vector<double> a_d;
+  std::vector<uint32_t> bits((size_t)(Ns / 32), 0u);
+  for (int p = 1; p < Q; ++p)
+    for (int64_t i = 0; i < N; ++i) {
       const int32_t e = nbr[(size_t)(p - 1) * (size_t)Ns + (size_t)i];
       const int32_t behind = nbr[(size_t)(opp(p) - 1) * (size_t)Ns + (size_t)i];
       if (e != (int32_t)NBR_WALL_BIT || behind < 0) continue;  // not a solid-wall link, or no fluid site behind
@@ -436,38 +453,77 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
       const int idx = (-lat.c[p][2] + 1) * 9 + (-lat.c[p][1] + 1) * 3 + (-lat.c[p][0] + 1);
       const double dd = d27[(size_t)canon[(size_t)i] * 27 + (size_t)idx];
       if (dd > 0.0 && dd <= 1.0) {
-        l_site.push_back((int32_t)i);
-        l_behind.push_back(behind);
-        l_link.push_back((uint8_t)p);
-        l_d.push_back(dd);
-        any = true;
+        a_site.push_back((int32_t)i);
+        a_behind.push_back(behind);
+        a_link.push_back((uint8_t)p);
+        a_d.push_back(dd);
+        bits[(size_t)(i >> 5)] |= 1u << (i & 31);
       }
     }
-    if (any) ++n_sites;
+  // site form for the step kernels (BflFused in kernels.cuh)
+  std::vector<int32_t> rank(bits.size());
+  int64_t n_sites = 0;
+  for (size_t w = 0; w < bits.size(); ++w) {
+    rank[w] = (int32_t)n_sites;
+    n_sites += __builtin_popcount(bits[w]);
+  }
+  const size_t nf = (size_t)((n_sites + 31) / 32 * 32 + 32);
+  const size_t row = (size_t)bfl_row_doubles(Q == 19);
+  std::vector<double> coef(row * nf, 0.0);
+  // list form for the read-out pre-pass: the links with d < 1/2 only (the others are already
+  // in what the step kernels write)
+  std::vector<int32_t> l_site, l_behind;
+  std::vector<uint8_t> l_link;
+  std::vector<double> l_d;
+  for (size_t l = 0; l < a_site.size(); ++l) {
+    const int64_t i = a_site[l];
+    const size_t at = (size_t)rank[(size_t)(i >> 5)] +
+                      (size_t)__builtin_popcount(bits[(size_t)(i >> 5)] & ((1u << (i & 31)) - 1u));
+    const double dd = a_d[l];
+    coef[at * row + (size_t)(a_link[l] - 1)] = dd < 0.5 ? 2.0 * dd : -(1.0 / (2.0 * dd));
+    if (dd < 0.5) {
+      l_site.push_back(a_site[l]);
+      l_behind.push_back(a_behind[l]);
+      l_link.push_back(a_link[l]);
+      l_d.push_back(dd);
+    }
   }
   const size_t nl = l_site.size();
   void *d_site = nullptr, *d_behind = nullptr, *d_link = nullptr, *d_d = nullptr;
+  void *d_bits = nullptr, *d_rank = nullptr, *d_coef = nullptr;
   int rc;
   const size_t cap = nl > 0 ? nl : 1;
   if ((rc = g->alloc(sizeof(int32_t) * cap, &d_site))) return rc;
   if ((rc = g->alloc(sizeof(int32_t) * cap, &d_behind))) return rc;
   if ((rc = g->alloc(sizeof(uint8_t) * cap, &d_link))) return rc;
   if ((rc = g->alloc(sizeof(double) * cap, &d_d))) return rc;
+  if ((rc = g->alloc(sizeof(uint32_t) * bits.size(), &d_bits))) return rc;
+  if ((rc = g->alloc(sizeof(int32_t) * rank.size(), &d_rank))) return rc;
+  if ((rc = g->alloc(sizeof(double) * coef.size(), &d_coef))) return rc;
   if (nl > 0) {
     HLB_CUDA(cudaMemcpy(d_site, l_site.data(), sizeof(int32_t) * nl, cudaMemcpyHostToDevice));
     HLB_CUDA(cudaMemcpy(d_behind, l_behind.data(), sizeof(int32_t) * nl, cudaMemcpyHostToDevice));
     HLB_CUDA(cudaMemcpy(d_link, l_link.data(), sizeof(uint8_t) * nl, cudaMemcpyHostToDevice));
     HLB_CUDA(cudaMemcpy(d_d, l_d.data(), sizeof(double) * nl, cudaMemcpyHostToDevice));
   }
+  HLB_CUDA(cudaMemcpy(d_bits, bits.data(), sizeof(uint32_t) * bits.size(), cudaMemcpyHostToDevice));
+  HLB_CUDA(cudaMemcpy(d_rank, rank.data(), sizeof(int32_t) * rank.size(), cudaMemcpyHostToDevice));
+  HLB_CUDA(cudaMemcpy(d_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice));
   g->dg.bfl.site = (const int32_t*)d_site;
   g->dg.bfl.behind = (const int32_t*)d_behind;
   g->dg.bfl.link = (const uint8_t*)d_link;
   g->dg.bfl.d = (const double*)d_d;
   g->dg.bfl.n = (long long)nl;
+  g->dg.bflf.bits = (const uint32_t*)d_bits;
+  g->dg.bflf.rank = (const int32_t*)d_rank;
+  g->dg.bflf.coef = (const double*)d_coef;
+  g->dg.bflf.nf = (long long)nf;
+  g->dg.bflf.gather = 0;
+  g->dg.bfl_on = true;
   g->bfl_set = true;
   g->bfl_applied = false;
   g->bfl_sites = n_sites;
-  g->bfl_links = (int64_t)nl;
+  g->bfl_links = (int64_t)a_site.size();
   return HLB_OK;
 }
 
@@ -491,10 +547,11 @@ int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u
 constexpr int64_t GRAPH_STEPS = 32;  // even: the buffer / phase parity is back where it started
 
 static void enqueue_one_step(hlb_geometry* g) {
+  g->dg.bflf.gather = g->gather_bfl() ? 1 : 0;
   if (g->aa) {
     launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
+    g->bfl_applied = false;  // every slot has been rewritten in place
   } else {
-    g->ensure_bfl();
     launch_pull(g->dg, g->buf[g->cur], g->buf[g->cur ^ 1], g->stream);
     g->bfl_applied = false;  // the new state buffer is untouched
     g->cur ^= 1;
@@ -533,11 +590,14 @@ int hlb_step(hlb_geometry* g, int64_t n) {
   if (n < 0) return fail(HLB_EINVAL, "n < 0");
   // graphs pay off only when a step is short next to the launch cost
   const bool want_graph = !(g->p.flags & HLB_NO_GRAPH) && !g->graph_failed && g->stream != nullptr &&
-                          g->N <= (int64_t)4 << 20 && !g->bfl_set;  // BFL: step 0 differs
+                          g->N <= (int64_t)4 << 20;
   int64_t left = n;
   while (left > 0) {
     const bool even = g->aa ? (g->steps & 1) == 0 : g->cur == 0;
-    if (want_graph && even && left >= GRAPH_STEPS && !g->graph_failed) {
+    // with interpolated walls the captured steps all apply the gather-side rule: not from
+    // the initial state, nor right after a read-out's pre-pass
+    const bool uniform = !g->bfl_set || g->gather_bfl();
+    if (want_graph && even && uniform && left >= GRAPH_STEPS && !g->graph_failed) {
       if (!g->graph_exec) build_step_graph(g);
       if (g->graph_exec) {
         HLB_CUDA(cudaGraphLaunch(g->graph_exec, g->stream));

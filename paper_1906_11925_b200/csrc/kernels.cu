@@ -211,10 +211,75 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
   return (__ldg(iolet_bits + (i >> 5)) >> (threadIdx.x & 31)) & 1u;
 }
 
+// BFL interpolated walls inside the step kernels (V == 2 instantiations; BflFused in
+// kernels.cuh). With i = opp(p) the direction from x to the wall and y = x + c_p behind x:
+//   d <  1/2:  f_p(x,t+1) = 2d f*_i(x,t) + (1 - 2d) f*_i(y,t).  After the gather of step t+1,
+//              h[p] is the bounced f*_i(x,t) and h[opp(p)] is f*_i(y,t), streamed from y: the
+//              rule is applied to the gathered registers.
+//   d >= 1/2:  f_p(x,t+1) = f*_i(x,t) / (2d) + (1 - 1/(2d)) f*_p(x,t).  Both are this site's
+//              own post-collision values of step t: the rule is applied to the value the site
+//              writes back for link p.
+// Neither needs a memory access beyond the coefficients. Two links p and opp(p) of one site
+// are never both interpolated (that needs x + c_p solid and fluid), so updating in place is safe.
+__device__ __forceinline__ long long bfl_site_index(const BflFused& bf, long long i) {
+  const uint32_t w = __ldg(bf.bits + (i >> 5));
+  const unsigned lane = threadIdx.x & 31;
+  if (!((w >> lane) & 1u)) return -1;
+  return (long long)__ldg(bf.rank + (i >> 5)) + __popc(w & ((1u << lane) - 1u));
+}
+// The coefficients are static: fetch them towards the SM before the populations are waited
+// for, so that the dependent chain bits -> rank -> coef does not add a DRAM round trip. A
+// site's coefficients are one row of bfl_row<L>() doubles (128 B for D3Q15, 160 B for D3Q19),
+// read two at a time.
+template <typename L>
+__host__ __device__ constexpr int bfl_row() { return (L::Q - 1 + 3) / 4 * 4; }
+template <typename L>
+__device__ __forceinline__ void bfl_prefetch(const BflFused& bf, long long idx) {
+  const char* row = (const char*)(bf.coef + idx * bfl_row<L>());
+#pragma unroll
+  for (int b = 0; b < bfl_row<L>() * 8; b += 128) asm volatile("prefetch.global.L1 [%0];" ::"l"(row + b));
+}
+template <typename L>
+__device__ __forceinline__ void bfl_gather(const BflFused& bf, long long idx, double (&h)[L::Q]) {
+  const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
+#pragma unroll
+  for (int k = 0; k < (L::Q - 1) / 2; ++k) {
+    const double2 c = __ldg(row + k);
+    const int p = 2 * k + 1;
+    if (c.x > 0.0) h[p] = fma_(c.x, h[p], mul(sub(1.0, c.x), h[opp(p)]));
+    if (c.y > 0.0) h[p + 1] = fma_(c.y, h[p + 1], mul(sub(1.0, c.y), h[opp(p + 1)]));
+  }
+}
+// out[p]: the value written back for link p (the bounced h*_opp(p)); h: post-collision
+template <typename L>
+__device__ __forceinline__ void bfl_write(const BflFused& bf, long long idx, const double (&h)[L::Q],
+                                          double (&out)[L::Q]) {
+  const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
+#pragma unroll
+  for (int k = 0; k < (L::Q - 1) / 2; ++k) {
+    const double2 c = __ldg(row + k);
+    const int p = 2 * k + 1;
+    if (c.x < 0.0) out[p] = fma_(-c.x, out[p], mul(sub(1.0, -c.x), h[p]));
+    if (c.y < 0.0) out[p + 1] = fma_(-c.y, out[p + 1], mul(sub(1.0, -c.y), h[p + 1]));
+  }
+}
+// two-lattice: the value written back for link p is h[opp(p)] itself
+template <typename L>
+__device__ __forceinline__ void bfl_write_pull(const BflFused& bf, long long idx, double (&h)[L::Q]) {
+  const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
+#pragma unroll
+  for (int k = 0; k < (L::Q - 1) / 2; ++k) {
+    const double2 c = __ldg(row + k);
+    const int p = 2 * k + 1;
+    if (c.x < 0.0) h[opp(p)] = fma_(-c.x, h[opp(p)], mul(sub(1.0, -c.x), h[p]));
+    if (c.y < 0.0) h[opp(p + 1)] = fma_(-c.y, h[opp(p + 1)], mul(sub(1.0, -c.y), h[p + 1]));
+  }
+}
+
 // BFL interpolated walls (linear Bouzidi-Firdaouss-Lallemand rule; the paper's "BFL" wall
 // option, ref [16]) as a PRE-PASS over the list of interpolated links,
-// run on the state buffer of the two-lattice scheme before the step (or read-out) that
-// gathers from it. Slot opp(p) of site x holds f*_opp(p)(x, t-1) and is read by nobody but x
+// run on the state buffer before the step (or read-out) that gathers from it. Written out for
+// the two-lattice scheme: slot opp(p) of site x holds f*_opp(p)(x, t-1) and is read by nobody but x
 // itself, as the halfway bounce-back value of its wall link p; the pre-pass replaces it by
 //   d <  1/2:  2d f*_opp(p)(x) + (1 - 2d) f*_opp(p)(x + c_p)      (slot opp(p) of the site behind)
 //   d >= 1/2:  f*_opp(p)(x) / (2d) + (1 - 1/(2d)) f*_p(x)         (slot p of x itself)
@@ -222,29 +287,68 @@ __device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iole
 // link of the list writes (a link is in the list only if the site behind it is fluid), so
 // the pass has no ordering hazards. An in-kernel version (interpolating at gather time behind
 // a per-site bit) cost 30 % of the step on configs[3]; this costs ~9 % (profiles/r01_tuning.md).
+// Where the three values live depends on what the state buffer holds (GatherMode of the state):
+//   GATHER_PULL   (two-lattice, post-collision f*_r(z) in slot r of z):
+//       target f*_i(x): slot i of x;  f*_i(y): slot i of y;  f*_q(x): slot q of x
+//   GATHER_AA_ODD (A-A after the even kernel, f*_r(z) in slot opp(r) of z):
+//       target: slot q of x;          f*_i(y): slot q of y;  f*_q(x): slot i of x
+//   GATHER_OWN    (A-A after the odd kernel, f*_r(z) in slot r of z + c_r, bounced walls in
+//                  slot opp(r) of z):
+//       target: slot q of x;          f*_i(y): slot i of x (= y + c_i);  f*_q(x): slot q of y
+// In every case the target is the slot the step kernel reads as the bounced f_q(x, t+1), no
+// other link reads or writes it, and neither source is the target of another link (that
+// would need y or x to be solid).
+// Each thread takes BFL_UNROLL links (a block: BFL_UNROLL * BLOCK consecutive ones): the
+// link data (static) are fetched before the wait on the previous step, then all population
+// loads are in flight together -- the pass is latency-bound, not bandwidth-bound.
+constexpr int BFL_UNROLL = 4;
 template <typename ST>
 __global__ void __launch_bounds__(BLOCK)
 k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ site,
               const int32_t* __restrict__ behind, const uint8_t* __restrict__ link,
-              const double* __restrict__ dist, long long n) {
-  const long long l = (long long)blockIdx.x * BLOCK + threadIdx.x;
-  if (l >= n) return;
-  const long long i = site[l];
-  const int p = link[l], po = opp(p);
-  const double dd = dist[l];
-  ST* own = buf + (long long)po * Ns + i;
-  const double a = to_real(*own);
-  const double two_d = mul(2.0, dd);
-  double r;
-  if (dd < 0.5) {
-    const double b = to_real(buf[(long long)po * Ns + behind[l]]);
-    r = fma_(two_d, a, mul(sub(1.0, two_d), b));
-  } else {
-    const double b = to_real(buf[(long long)p * Ns + i]);
-    const double inv = __ddiv_rn(1.0, two_d);
-    r = fma_(inv, a, mul(sub(1.0, inv), b));
+              const double* __restrict__ dist, long long n, int mode) {
+  const long long l0 = (long long)blockIdx.x * (BFL_UNROLL * BLOCK) + threadIdx.x;
+  long long tgt[BFL_UNROLL], src[BFL_UNROLL];
+  double dd[BFL_UNROLL];
+  pdl_launch_dependents();
+#pragma unroll
+  for (int k = 0; k < BFL_UNROLL; ++k) {
+    const long long l = l0 + (long long)k * BLOCK;
+    dd[k] = -1.0;
+    if (l < n) {
+      const long long i = __ldg(site + l), y = __ldg(behind + l);
+      const int p = __ldg(link + l), po = opp(p);
+      dd[k] = __ldg(dist + l);
+      tgt[k] = (long long)(mode == GATHER_PULL ? po : p) * Ns + i;
+      if (dd[k] < 0.5)
+        src[k] = mode == GATHER_PULL ? (long long)po * Ns + y
+               : mode == GATHER_AA_ODD ? (long long)p * Ns + y : (long long)po * Ns + i;
+      else
+        src[k] = mode == GATHER_PULL ? (long long)p * Ns + i
+               : mode == GATHER_AA_ODD ? (long long)po * Ns + i : (long long)p * Ns + y;
+    }
   }
-  *own = to_store<ST>(r);
+  pdl_wait_for_previous_step();
+  double a[BFL_UNROLL], b[BFL_UNROLL];
+#pragma unroll
+  for (int k = 0; k < BFL_UNROLL; ++k)
+    if (dd[k] > 0.0) {
+      a[k] = to_real(buf[tgt[k]]);
+      b[k] = to_real(buf[src[k]]);
+    }
+#pragma unroll
+  for (int k = 0; k < BFL_UNROLL; ++k)
+    if (dd[k] > 0.0) {
+      const double two_d = mul(2.0, dd[k]);
+      double r;
+      if (dd[k] < 0.5) {
+        r = fma_(two_d, a[k], mul(sub(1.0, two_d), b[k]));
+      } else {
+        const double inv = __ddiv_rn(1.0, two_d);
+        r = fma_(inv, a[k], mul(sub(1.0, inv), b[k]));
+      }
+      buf[tgt[k]] = to_store<ST>(r);
+    }
 }
 
 // ------------------------------------------------------------------ two-lattice pull
@@ -253,16 +357,21 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
 // pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
 // of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
 // padding, so only the one warp-uniform test is needed.
-template <typename L, typename ST, bool REC, typename IT, bool FULL>
+template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
-       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf) {
+       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[L::Q];
+  long long bidx = -1;
   {
     IT off[L::Q - 1];
     pdl_launch_dependents();
+    if (V == 2) {
+      bidx = bfl_site_index(bf, i);
+      if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+    }
     link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
     pdl_wait_for_previous_step();
     h[0] = to_real(src[i]);
@@ -278,14 +387,16 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
       for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
     }
   }
+  if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
   collide<L>(h, m, omega, h);
+  if (V == 2 && bidx >= 0) bfl_write_pull<L>(bf, bidx, h);
   if (has_iolet_link(iolet_bits, i)) {  // rare: sites on an inlet/outlet cap
     // slot opp(p) of this site is read back by link p next step
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L, FULL>(nbr, Ns, i, m, iolet_par, back);
+    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
@@ -299,15 +410,20 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // Odd phase: read f_q from slot opp(q) of x - c_q (slot q of x at a wall), write h*_q to
 // the address f_opp(q) was read from. Read set = write set per site in both phases, so one
 // array and no inter-thread hazards.
-template <typename L, typename ST, bool FULL>
+template <typename L, typename ST, int V>
 __global__ void __launch_bounds__(SBLOCK, aa_even_minb<L>())
 k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
           const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-          long long Ns, double omega, long long pf) {
+          long long Ns, double omega, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   ST* p0 = a + i;
   double h[L::Q];
+  long long bidx = -1;
   pdl_launch_dependents();
+  if (V == 2) {
+    bidx = bfl_site_index(bf, i);
+    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+  }
   pdl_wait_for_previous_step();
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
@@ -315,24 +431,31 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
 #pragma unroll
     for (int q = 0; q < L::Q; ++q) prefetch_l2(p0 + (long long)q * Ns + pf);
   }
+  if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
   collide<L>(h, m, omega, h);
   double out[L::Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, FULL>(nbr, Ns, i, m, iolet_par, out);
+  if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, out);
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
 
-template <typename L, typename ST, bool REC, typename IT, bool FULL>
+template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-         long long Ns, double omega, long long pf) {
+         long long Ns, double omega, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
+  long long bidx = -1;
   pdl_launch_dependents();
+  if (V == 2) {
+    bidx = bfl_site_index(bf, i);
+    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+  }
   link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
   pdl_wait_for_previous_step();
   double h[L::Q];
@@ -348,12 +471,14 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
   }
+  if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
   collide<L>(h, m, omega, h);
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, FULL>(nbr, Ns, i, m, iolet_par, out);
+  if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
@@ -505,6 +630,7 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + BLOCK - 1) / BLOC
 
 }  // namespace
 
+int bfl_row_doubles(bool d3q19) { return d3q19 ? bfl_row<D3Q19>() : bfl_row<D3Q15>(); }
 int resident_sites_per_sm_pull(bool d3q19) {
   return SBLOCK * (d3q19 ? pull_minb<D3Q19, true>() : pull_minb<D3Q15, true>());
 }
@@ -532,14 +658,12 @@ static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaS
 
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-  if (g.iolet_full)
-    launch_step(g, k_pull<L, ST, REC, IT, true>, s, (const ST*)src, (ST*)dst, g.nbr,
-                (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
-                (long long)g.prefetch_pull);
-  else
-    launch_step(g, k_pull<L, ST, REC, IT, false>, s, (const ST*)src, (ST*)dst, g.nbr,
-                (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega,
-                (long long)g.prefetch_pull);
+#define HLB_PULL_ARGS s, (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, \
+                      (long long)g.Ns, g.omega, (long long)g.prefetch_pull, g.bflf
+  if (g.bfl_on) launch_step(g, k_pull<L, ST, REC, IT, 2>, HLB_PULL_ARGS);
+  else if (g.iolet_full) launch_step(g, k_pull<L, ST, REC, IT, 1>, HLB_PULL_ARGS);
+  else launch_step(g, k_pull<L, ST, REC, IT, 0>, HLB_PULL_ARGS);
+#undef HLB_PULL_ARGS
 }
 template <typename L, typename ST>
 static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
@@ -554,23 +678,23 @@ static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStre
 }
 template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
-  if (g.iolet_full)
-    launch_step(g, k_aa_odd<L, ST, REC, IT, true>, s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-                g.iolet_par, (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
-  else
-    launch_step(g, k_aa_odd<L, ST, REC, IT, false>, s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits,
-                g.iolet_par, (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
+#define HLB_ODD_ARGS s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega, \
+                     (long long)g.prefetch_aa, g.bflf
+  if (g.bfl_on) launch_step(g, k_aa_odd<L, ST, REC, IT, 2>, HLB_ODD_ARGS);
+  else if (g.iolet_full) launch_step(g, k_aa_odd<L, ST, REC, IT, 1>, HLB_ODD_ARGS);
+  else launch_step(g, k_aa_odd<L, ST, REC, IT, 0>, HLB_ODD_ARGS);
+#undef HLB_ODD_ARGS
 }
 template <typename L, typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (!odd) {
-    if (g.iolet_full)
-      launch_step(g, k_aa_even<L, ST, true>, s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par,
-                  (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
-    else
-      launch_step(g, k_aa_even<L, ST, false>, s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par,
-                  (long long)g.Ns, g.omega, (long long)g.prefetch_aa);
+#define HLB_EVEN_ARGS s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega, \
+                      (long long)g.prefetch_aa, g.bflf
+    if (g.bfl_on) launch_step(g, k_aa_even<L, ST, 2>, HLB_EVEN_ARGS);
+    else if (g.iolet_full) launch_step(g, k_aa_even<L, ST, 1>, HLB_EVEN_ARGS);
+    else launch_step(g, k_aa_even<L, ST, 0>, HLB_EVEN_ARGS);
+#undef HLB_EVEN_ARGS
   } else if (g.use_rec) {
     if (idx32) aa_odd_launch<L, ST, true, uint32_t>(g, a, s);
     else aa_odd_launch<L, ST, true, long long>(g, a, s);
@@ -637,13 +761,26 @@ static void dispatch(const DeviceGeometry& g, F&& f) {
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { pull_t<decltype(l), decltype(st)>(g, src, dst, s); });
 }
-void launch_bfl_prepass(const DeviceGeometry& g, void* buf, cudaStream_t s) {
+template <typename ST>
+static void bfl_prepass_t(const DeviceGeometry& g, void* buf, GatherMode mode, cudaStream_t s) {
   const BflLinks& b = g.bfl;
-  if (b.n <= 0) return;
-  if (g.f32)
-    k_bfl_prepass<float><<<grid_for(b.n), BLOCK, 0, s>>>((float*)buf, g.Ns, b.site, b.behind, b.link, b.d, b.n);
-  else
-    k_bfl_prepass<double><<<grid_for(b.n), BLOCK, 0, s>>>((double*)buf, g.Ns, b.site, b.behind, b.link, b.d, b.n);
+  const long long per_block = (long long)BFL_UNROLL * BLOCK;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)((b.n + per_block - 1) / per_block));
+  cfg.blockDim = dim3(BLOCK);
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = g.pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, k_bfl_prepass<ST>, (ST*)buf, (long long)g.Ns, b.site, b.behind, b.link, b.d,
+                     (long long)b.n, (int)mode);
+}
+void launch_bfl_prepass(const DeviceGeometry& g, void* buf, GatherMode mode, cudaStream_t s) {
+  if (g.bfl.n <= 0) return;
+  if (g.f32) bfl_prepass_t<float>(g, buf, mode, s);
+  else bfl_prepass_t<double>(g, buf, mode, s);
 }
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { aa_t<decltype(l), decltype(st)>(g, a, odd, s); });

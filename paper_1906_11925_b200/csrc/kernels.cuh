@@ -6,15 +6,32 @@
 
 namespace hlb {
 
-// BFL interpolated walls (two-lattice scheme): the list of interpolated links. Link l belongs
-// to internal site site[l], is its pull link link[l] (1 .. Q-1), has the wall at the fraction
-// d[l] of its length, and behind[l] is the internal index of the fluid site x + c_p behind it.
+// BFL interpolated walls, list form (used by the pre-pass before a read-out): the interpolated
+// links with d < 1/2. Link l belongs to internal site site[l], is its pull link link[l]
+// (1 .. Q-1), has the wall at the fraction d[l] of its length, and behind[l] is the internal
+// index of the fluid site x + c_p behind it.
 struct BflLinks {
   const int32_t* site = nullptr;
   const int32_t* behind = nullptr;
   const uint8_t* link = nullptr;
   const double* d = nullptr;
   long long n = 0;
+};
+
+// BFL interpolated walls, site form (used inside the step kernels, by value as a kernel
+// argument): bit i of `bits` marks the sites with an interpolated link; such a site has the
+// dense index idx = rank[i / 32] + popcount(bits word below lane i % 32), and coef[idx * row
+// + p - 1] (row = bfl_row_doubles(): Q-1 rounded up to a multiple of 4; 16-byte aligned) is,
+// for its pull link p,  2d  where d < 1/2 (applied while gathering),  -1/(2d)
+// where d >= 1/2 (applied to the value the site writes back for that link),  0 = plain
+// bounce-back. gather = 0 when the d < 1/2 part is already in the state buffer (pre-pass
+// run for a read-out) or does not apply (the initial state).
+struct BflFused {
+  const uint32_t* bits = nullptr;  // [Ns/32]
+  const int32_t* rank = nullptr;   // [Ns/32]
+  const double* coef = nullptr;    // [nf][row]
+  long long nf = 0;
+  int gather = 0;
 };
 
 struct DeviceGeometry {
@@ -25,6 +42,8 @@ struct DeviceGeometry {
   const void* rec = nullptr;            // [Ns/32][Q-1] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
   BflLinks bfl;                         // applied by launch_bfl_prepass when the API says so
+  BflFused bflf;                        // used by the step kernels when bfl_on
+  bool bfl_on = false;                  // interpolated walls are set
   bool iolet_full = false;              // some iolet is a velocity iolet or has a normal
   bool pdl = true;                      // programmatic dependent launch of the step kernels
   bool index64 = false;                 // flat offsets need (or are forced to) 64 bits
@@ -40,15 +59,13 @@ struct DeviceGeometry {
   bool d3q19 = false;                   // HLB_LATTICE_D3Q19 (else D3Q15)
 };
 
+int bfl_row_doubles(bool d3q19);
 // Sites resident on an SM at once (threads per block x resident blocks) per step kernel.
 int resident_sites_per_sm_pull(bool d3q19);
 int resident_sites_per_sm_aa(bool d3q19);
 
 // One time step, two-lattice pull: dst <- collide(gather(src)).
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);
-// Rewrite, in the two-lattice state buffer `buf`, the bounce-back slots of the interpolated
-// links (see kernels.cu); run once per state, before the step or read-out that gathers from it.
-void launch_bfl_prepass(const DeviceGeometry& g, void* buf, cudaStream_t s);
 // One time step, A-A in place; `odd` selects the phase.
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s);
 
@@ -58,6 +75,10 @@ enum GatherMode {
   GATHER_OWN = 1,    // A-A after an even number of steps: slot q of the site itself
   GATHER_AA_ODD = 2  // A-A after an odd number of steps: slot opp(q) of x - c_q (slot q at walls)
 };
+// Rewrite, in the state buffer `buf` (its layout given by `mode`), the bounce-back slots of the
+// interpolated links (see kernels.cu); run once per state, before the step or read-out that
+// gathers from it.
+void launch_bfl_prepass(const DeviceGeometry& g, void* buf, GatherMode mode, cudaStream_t s);
 // rho [N] / u [N][3] (device, canonical order; either may be NULL)
 void launch_macroscopic(const DeviceGeometry& g, const void* buf, GatherMode mode, double* rho,
                         double* u, cudaStream_t s);

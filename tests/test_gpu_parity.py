@@ -304,12 +304,13 @@ def test_normal_projected_pressure_iolets_match_oracle(hlb, scheme, lattice):
 
 
 # ------------------------------------------------------------- BFL interpolated walls (NEXT-2)
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
 @pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
 @pytest.mark.parametrize("name", ["pipe", "aneurysm"])
-def test_bfl_walls_match_oracle(hlb, name, lattice):
+def test_bfl_walls_match_oracle(hlb, name, lattice, scheme):
     """The paper's wall option: sub-voxel wall distances from the
-    analytic surfaces of the pipe and the aneurysm, with a Ladd velocity inlet; two-lattice
-    scheme, both storage types, records and table, even / odd / zero step counts."""
+    analytic surfaces of the pipe and the aneurysm, with a Ladd velocity inlet; both schemes,
+    both storage types, records and table, even / odd / zero step counts."""
     wl = W.with_bfl_walls(W.with_velocity_inlet(W.by_name(name, small=True)))
     plain = W.with_velocity_inlet(W.by_name(name, small=True))
     for steps, store, order, links in ((wl.steps, "f64", "raster", "records"),
@@ -317,9 +318,9 @@ def test_bfl_walls_match_oracle(hlb, name, lattice):
                                        (0, "f64", "raster", "auto"), (1, "f64", "raster", "auto"),
                                        (wl.steps, "f32", "raster", "auto")):
         rho_ref, u_ref = run_oracle(wl, steps, lattice=lattice)
-        rho, u = run_gpu(hlb, wl, steps, "two_lattice", store, order, links, lattice)
+        rho, u = run_gpu(hlb, wl, steps, scheme, store, order, links, lattice)
         e_rho, e_u = errors(rho, u, rho_ref, u_ref)
-        assert e_rho < TOL[store] and e_u < TOL[store], (name, store, steps, e_rho, e_u)
+        assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
     # and the interpolation does change the flow (the test above is not vacuous)
     rho_p, u_p = run_oracle(plain, wl.steps, lattice=lattice)
     rho_b, u_b = run_oracle(wl, wl.steps, lattice=lattice)
@@ -328,7 +329,8 @@ def test_bfl_walls_match_oracle(hlb, name, lattice):
 
 @pytest.mark.parametrize("seed,periodic,shape", [(0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (33, 5, 4)),
                                                  (3, 0, (24, 20, 18)), (4, 5, (40, 9, 23))])
-def test_bfl_random_masks_and_distances_match_oracle(hlb, seed, periodic, shape):
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_bfl_random_masks_and_distances_match_oracle(hlb, seed, periodic, shape, scheme):
     wl = W.random_mask(shape, p_fluid=0.65, n_iolets=3, p_iolet=0.05, periodic=periodic,
                        tau=0.56 + 0.08 * seed, seed=500 + seed)
     rng = np.random.default_rng(seed)
@@ -337,13 +339,13 @@ def test_bfl_random_masks_and_distances_match_oracle(hlb, seed, periodic, shape)
     perm = _match_directions(hlb)
     o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho)
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
-                                flags_of(hlb, "two_lattice", "f64", "raster" if seed % 2 else "morton"))
+                                flags_of(hlb, scheme, "f64", "raster" if seed % 2 else "morton"))
     for x in (o, ):
         x.set_state(wl.rho0, wl.u0)
         x.set_wall_distance(d27)
     g.hlb_set_state(wl.rho0, wl.u0)
     g.hlb_set_wall_distance(d27)
-    for n in (0, 1, 1, 7, 12):
+    for n in (0, 1, 1, 7, 12, 1):                        # read-outs at even and odd step counts
         o.step(n)
         g.hlb_step(n)
         assert np.max(np.abs(g.hlb_get_populations()[:, perm] - o.get_populations())) < 1e-14
@@ -356,16 +358,18 @@ def test_bfl_random_masks_and_distances_match_oracle(hlb, seed, periodic, shape)
     g.close()
 
 
-def test_bfl_at_half_a_link_is_bounce_back_bitwise_and_argument_errors(hlb):
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_bfl_at_half_a_link_is_bounce_back_bitwise_and_argument_errors(hlb, scheme):
     wl = W.by_name("tree", small=True)
-    a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, "two_lattice", "f64", "raster"))
-    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, "two_lattice", "f64", "raster"))
+    a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, scheme, "f64", "raster"))
+    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, scheme, "f64", "raster"))
     b.hlb_set_wall_distance(np.full((wl.n_sites, 27), 0.5))
     assert b.hlb_num_bfl_sites() > 100 and a.hlb_num_bfl_sites() == 0
-    a.hlb_step(40)
-    b.hlb_step(40)
-    (ra, ua), (rb, ub) = a.hlb_get_macroscopic(), b.hlb_get_macroscopic()
-    assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
+    for n in (40, 1):
+        a.hlb_step(n)
+        b.hlb_step(n)
+        (ra, ua), (rb, ub) = a.hlb_get_macroscopic(), b.hlb_get_macroscopic()
+        assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
     with pytest.raises(hlb.HlbError) as e:
         b.hlb_set_wall_distance(None)                    # not after the first step
     assert e.value.code == hlb.HLB_EINVAL
@@ -374,11 +378,28 @@ def test_bfl_at_half_a_link_is_bounce_back_bitwise_and_argument_errors(hlb):
     assert b.hlb_num_bfl_sites() == 0
     a.close()
     b.close()
-    c = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, flags_of(hlb, "aa", "f64"))
-    with pytest.raises(hlb.HlbError) as e:
-        c.hlb_set_wall_distance(np.full((wl.n_sites, 27), 0.3))
-    assert e.value.code == hlb.HLB_EINVAL
-    c.close()
+
+
+def test_bfl_is_the_same_in_both_schemes(hlb):
+    """Two-lattice and A-A apply the same interpolation to the same values: populations after
+    even and odd step counts agree to rounding (the two schemes round alike, see the bitwise
+    variant tests; with interpolated walls the order of operations is the same too)."""
+    wl = W.with_bfl_walls(W.with_velocity_inlet(W.by_name("aneurysm", small=True)))
+    gs = []
+    for scheme in ("two_lattice", "aa"):
+        g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags_of(hlb, scheme, "f64"))
+        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+        g.hlb_set_wall_distance(wl.wall_distance)
+        gs.append(g)
+    assert gs[0].hlb_num_bfl_sites() == gs[1].hlb_num_bfl_sites() > 0
+    for n in (1, 1, 9, 20):
+        fs = []
+        for g in gs:
+            g.hlb_step(n)
+            fs.append(g.hlb_get_populations())
+        assert np.max(np.abs(fs[0] - fs[1])) < 1e-14
+    for g in gs:
+        g.close()
 
 
 # ------------------------------------------------------------- stress read-out (NEXT-3)
@@ -501,6 +522,40 @@ def test_graph_replay_equals_direct_launches(hlb, scheme):
     a.hlb_step(64)
     b.hlb_step(64)
     assert np.array_equal(a.hlb_get_macroscopic()[1], b.hlb_get_macroscopic()[1])
+    a.close()
+    b.close()
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_graph_replay_with_boundary_options(hlb, scheme):
+    """Graph replay with interpolated walls (read-outs in between: the step after a read-out
+    and the first step are launched directly) equals direct launches bitwise; and a graph
+    captured with the lean iolet kernels is dropped when an iolet becomes a velocity iolet."""
+    wl = W.with_bfl_walls(W.with_velocity_inlet(W.by_name("aneurysm", small=True)))
+    f = flags_of(hlb, scheme, "f64", "raster")
+    a = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f)
+    b = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | hlb.HLB_NO_GRAPH)
+    o = oracle.Oracle(wl.site_type, 0, wl.tau, wl.iolet_rho)
+    for x in (a, b):
+        x.hlb_set_wall_distance(wl.wall_distance)
+    o.set_wall_distance(wl.wall_distance)
+    total = 0
+    for n in (70, 33, 1, 64):                            # pressure iolets: lean kernels
+        a.hlb_step(n)
+        b.hlb_step(n)
+        total += n
+        assert np.array_equal(a.hlb_get_populations(), b.hlb_get_populations())
+    for x in (a, b):
+        x.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)   # now the full kernels
+    o.step(total)
+    o.set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+    for n in (66, 35):
+        a.hlb_step(n)
+        b.hlb_step(n)
+        o.step(n)
+        assert np.array_equal(a.hlb_get_populations(), b.hlb_get_populations())
+        e_rho, e_u = errors(*a.hlb_get_macroscopic(), *o.get_macroscopic())
+        assert e_rho < 1e-13 and e_u < 1e-12, (n, e_rho, e_u)
     a.close()
     b.close()
 
