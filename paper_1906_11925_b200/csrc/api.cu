@@ -79,6 +79,8 @@ struct hlb_geometry {
   bool bfl_set = false;               // wall distances given (hlb_set_wall_distance)
   int64_t bfl_sites = 0;              // sites with at least one interpolated link
   int64_t bfl_links = 0;              // interpolated links
+  void* bfl_mem[7] = {};              // device tables of hlb_set_wall_distance, kept for reuse
+  size_t bfl_cap_links = 0, bfl_cap_coef = 0;
   cudaGraphExec_t graph_exec = nullptr;
   bool graph_failed = false;
   // The captured launches fix the kernel instantiation and the by-value arguments: drop the
@@ -493,13 +495,24 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   void *d_bits = nullptr, *d_rank = nullptr, *d_coef = nullptr;
   int rc;
   const size_t cap = nl > 0 ? nl : 1;
-  if ((rc = g->alloc(sizeof(int32_t) * cap, &d_site))) return rc;
-  if ((rc = g->alloc(sizeof(int32_t) * cap, &d_behind))) return rc;
-  if ((rc = g->alloc(sizeof(uint8_t) * cap, &d_link))) return rc;
-  if ((rc = g->alloc(sizeof(double) * cap, &d_d))) return rc;
-  if ((rc = g->alloc(sizeof(uint32_t) * bits.size(), &d_bits))) return rc;
-  if ((rc = g->alloc(sizeof(int32_t) * rank.size(), &d_rank))) return rc;
-  if ((rc = g->alloc(sizeof(double) * coef.size(), &d_coef))) return rc;
+  if (g->bfl_mem[0] && cap <= g->bfl_cap_links && coef.size() <= g->bfl_cap_coef) {
+    // tables of an earlier call are large enough: reuse them (there is no free callback)
+    d_site = g->bfl_mem[0]; d_behind = g->bfl_mem[1]; d_link = g->bfl_mem[2]; d_d = g->bfl_mem[3];
+    d_bits = g->bfl_mem[4]; d_rank = g->bfl_mem[5]; d_coef = g->bfl_mem[6];
+    HLB_CUDA(cudaStreamSynchronize(g->stream));
+  } else {
+    if ((rc = g->alloc(sizeof(int32_t) * cap, &d_site))) return rc;
+    if ((rc = g->alloc(sizeof(int32_t) * cap, &d_behind))) return rc;
+    if ((rc = g->alloc(sizeof(uint8_t) * cap, &d_link))) return rc;
+    if ((rc = g->alloc(sizeof(double) * cap, &d_d))) return rc;
+    if ((rc = g->alloc(sizeof(uint32_t) * bits.size(), &d_bits))) return rc;
+    if ((rc = g->alloc(sizeof(int32_t) * rank.size(), &d_rank))) return rc;
+    if ((rc = g->alloc(sizeof(double) * coef.size(), &d_coef))) return rc;
+    void* mem[7] = {d_site, d_behind, d_link, d_d, d_bits, d_rank, d_coef};
+    for (int k = 0; k < 7; ++k) g->bfl_mem[k] = mem[k];
+    g->bfl_cap_links = cap;
+    g->bfl_cap_coef = coef.size();
+  }
   if (nl > 0) {
     HLB_CUDA(cudaMemcpy(d_site, l_site.data(), sizeof(int32_t) * nl, cudaMemcpyHostToDevice));
     HLB_CUDA(cudaMemcpy(d_behind, l_behind.data(), sizeof(int32_t) * nl, cudaMemcpyHostToDevice));

@@ -57,8 +57,9 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ vol, int nx
 
 constexpr int TILE = 16;
 
-// occ (may be NULL): one byte per 8 x 8 x 8 macro-cell, 1 = every voxel a sample of the cell
-// can touch ([8c, 8c + 8] per axis) is exactly +0. Such a sample has the value +0 exactly; if
+// occ (may be NULL): one byte per 8 x 8 x 8 macro-cell, != 0 = every voxel a sample of the cell
+// can touch ([8c, 8c + 8] per axis) is exactly +0 (2 = the same holds for all macro-cells of
+// the 64^3 super-cell around it, so the jump may span the super-cell). Such a sample has the value +0 exactly; if
 // the transfer function gives value 0 no opacity, it contributes exactly nothing and may be
 // skipped, together with the following samples that provably stay in the same cell. The
 // image is therefore bit-identical with and without occ.
@@ -124,17 +125,20 @@ k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ,
       const int ix = max(min((int)floorf(qx), v.nx - 2), 0), iy = max(min((int)floorf(qy), v.ny - 2), 0),
                 iz = max(min((int)floorf(qz), v.nz - 2), 0);
       const int cxm = ix >> 3, cym = iy >> 3, czm = iz >> 3;
-      if (__ldg(occ + ((long long)czm * my + cym) * mx + cxm)) {
+      const int level = __ldg(occ + ((long long)czm * my + cym) * mx + cxm);
+      if (level) {
+        // level 2: the whole 64^3 super-cell around the macro-cell is empty
+        const int sh = level == 2 ? 6 : 3;
         // conservative count of further samples whose lower corner stays in this cell: keep a
         // margin (>= 0.01 voxel, far above the rounding of the sample positions) clear of the
         // cell faces; an axis the ray hardly moves along must already be clear of them
         const float q[3] = {qx, qy, qz};
-        const int c8[3] = {cxm << 3, cym << 3, czm << 3};
+        const int c8[3] = {(ix >> sh) << sh, (iy >> sh) << sh, (iz >> sh) << sh};
         float room = 1e30f;  // distance in Z the ray may still travel
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
           const float margin = 0.01f * (1.0f + fabsf(r2[a]));
-          const float hi = (float)(c8[a] + 8) - margin - q[a], lo = q[a] - (float)c8[a] - margin;
+          const float hi = (float)(c8[a] + (1 << sh)) - margin - q[a], lo = q[a] - (float)c8[a] - margin;
           if (r2[a] > 1e-6f) room = fminf(room, hi / r2[a]);
           else if (r2[a] < -1e-6f) room = fminf(room, lo / -r2[a]);
           else if (hi < 0.0f || lo < 0.0f) room = 0.0f;
@@ -216,12 +220,37 @@ k_occupancy(const float* __restrict__ vol, int nx, int ny, int nz, unsigned char
 }
 }  // namespace
 
+namespace {
+// one warp per 64^3 super-cell: if all of its macro-cells are empty, mark them 2
+__global__ void __launch_bounds__(256)
+k_occupancy_super(int mx, int my, int mz, unsigned char* __restrict__ occ) {
+  const int sx = (mx + 7) >> 3, sy = (my + 7) >> 3, sz = (mz + 7) >> 3;
+  const long long sc = ((long long)blockIdx.x * 256 + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (sc >= (long long)sx * sy * sz) return;
+  const int bx = (int)(sc % sx) << 3, by = (int)((sc / sx) % sy) << 3, bz = (int)(sc / ((long long)sx * sy)) << 3;
+  bool all = true;
+  for (int t = lane; t < 512; t += 32) {
+    const int x = bx + (t & 7), y = by + ((t >> 3) & 7), z = bz + (t >> 6);
+    if (x < mx && y < my && z < mz && occ[((long long)z * my + y) * mx + x] == 0) all = false;
+  }
+  if (!__all_sync(0xffffffffu, all)) return;
+  for (int t = lane; t < 512; t += 32) {
+    const int x = bx + (t & 7), y = by + ((t >> 3) & 7), z = bz + (t >> 6);
+    if (x < mx && y < my && z < mz) occ[((long long)z * my + y) * mx + x] = 2;
+  }
+}
+}  // namespace
+
 long long occupancy_cells(int nx, int ny, int nz) {
   return (long long)((nx + 7) >> 3) * ((ny + 7) >> 3) * ((nz + 7) >> 3);
 }
 void launch_occupancy(const float* vol, int nx, int ny, int nz, unsigned char* occ, cudaStream_t s) {
   const long long threads = occupancy_cells(nx, ny, nz) * 32;
   k_occupancy<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(vol, nx, ny, nz, occ);
+  const int mx = (nx + 7) >> 3, my = (ny + 7) >> 3, mz = (nz + 7) >> 3;
+  const long long sthreads = (long long)((mx + 7) >> 3) * ((my + 7) >> 3) * ((mz + 7) >> 3) * 32;
+  k_occupancy_super<<<(unsigned)((sthreads + 255) / 256), 256, 0, s>>>(mx, my, mz, occ);
 }
 
 void launch_scatter_field(const double* rho, const double* u, const long long* voxel, long long N,

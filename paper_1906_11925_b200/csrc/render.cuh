@@ -16,7 +16,8 @@ cudaError_t render_upload(const RenderSetup& r, const float* lut_host, cudaStrea
 // emptiness bytes from launch_occupancy, or NULL (no empty-space skipping; same image)
 void launch_raymarch(const RenderSetup& r, const float* vol, const unsigned char* occ, float* image,
                      cudaStream_t s);
-// occ [occupancy_cells()] bytes: 1 where every voxel a sample of the 8^3 macro-cell can touch is +0
+// occ [occupancy_cells()] bytes: != 0 where every voxel a sample of the 8^3 macro-cell can touch
+// is +0 (2: all macro-cells of the enclosing 64^3 super-cell are)
 long long occupancy_cells(int nx, int ny, int nz);
 void launch_occupancy(const float* vol, int nx, int ny, int nz, unsigned char* occ, cudaStream_t s);
 // vol[voxel[c]] = |u| (field 0) or rho - 1 (field 1) of canonical site c

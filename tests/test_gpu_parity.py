@@ -351,6 +351,10 @@ def test_bfl_random_masks_and_distances_match_oracle(hlb, seed, periodic, shape,
         assert np.max(np.abs(g.hlb_get_populations()[:, perm] - o.get_populations())) < 1e-14
     g.hlb_set_state(wl.rho0, wl.u0)                      # distances survive a re-initialisation
     o.set_state(wl.rho0, wl.u0)
+    if seed % 2:                                         # setting them again reuses the tables
+        before = g.hlb_device_bytes()
+        g.hlb_set_wall_distance(d27)
+        assert g.hlb_device_bytes() == before
     o.step(5)
     g.hlb_step(5)
     e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())

@@ -95,7 +95,7 @@ def sparse_volume(shape, seed):
     return vol
 
 
-@pytest.mark.parametrize("shape", [(41, 57, 70), (64, 64, 64), (9, 130, 17), (3, 8, 100)])
+@pytest.mark.parametrize("shape", [(41, 57, 70), (64, 64, 64), (9, 130, 17), (3, 8, 100), (70, 140, 200)])
 @pytest.mark.parametrize("view", range(len(SKIP_VIEWS)))
 def test_empty_space_skipping_keeps_the_image_bitwise(hlb, shape, view):
     """With a transfer function that is transparent at value 0 the kernel jumps over empty 8^3
