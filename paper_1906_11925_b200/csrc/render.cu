@@ -115,6 +115,12 @@ k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ,
   }
   const int mx = (v.nx + 7) >> 3, my = (v.ny + 7) >> 3;
   const float r2[3] = {v.rot[2], v.rot[5], v.rot[8]};
+  // per ray: 1 / (direction component) and 1 / step for the jump lengths (their rounding is
+  // far inside the margin below)
+  float inv[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) inv[a] = fabsf(r2[a]) > 1e-6f ? 1.0f / fabsf(r2[a]) : 0.0f;
+  const float inv_step = 1.0f / v.step;
   float Cr = 0.0f, Cg = 0.0f, Cb = 0.0f, A = 0.0f;
   for (int k = k0; k <= k1; ++k) {
     const float Z = __fmaf_rn((float)k, v.step, -T);
@@ -139,11 +145,12 @@ k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ,
         for (int a = 0; a < 3; ++a) {
           const float margin = 0.01f * (1.0f + fabsf(r2[a]));
           const float hi = (float)(c8[a] + (1 << sh)) - margin - q[a], lo = q[a] - (float)c8[a] - margin;
-          if (r2[a] > 1e-6f) room = fminf(room, hi / r2[a]);
-          else if (r2[a] < -1e-6f) room = fminf(room, lo / -r2[a]);
+          if (r2[a] > 1e-6f) room = fminf(room, hi * inv[a]);
+          else if (r2[a] < -1e-6f) room = fminf(room, lo * inv[a]);
           else if (hi < 0.0f || lo < 0.0f) room = 0.0f;
         }
-        const int jump = room > 0.0f ? (int)fminf(floorf(room / v.step) - 1.0f, 1.0e6f) : 0;
+        // samples k+1 .. k+jump lie within `room` of this one: inside the cell, margin to spare
+        const int jump = room > 0.0f ? (int)fminf(floorf(room * inv_step), 1.0e6f) : 0;
         if (jump > 0) k += jump;
         continue;
       }
