@@ -17,8 +17,9 @@
 //     then all population loads, then the arithmetic;
 //   * every thread L2-prefetches what the site 3/4 of a wave ahead will load;
 //   * iolets (constant density, Ladd velocity) are a rare path behind one per-site bit; the
-//     table entries they need are re-read there, not kept in registers; BFL walls are a
-//     pre-pass over the interpolated links, outside the step kernel.
+//     table entries they need are re-read there, not kept in registers;
+//   * BFL interpolated walls are a third instantiation (V = 2) that applies both rules to
+//     registers; the lean (V = 0) and full (V = 1) instantiations carry none of its code.
 //
 // Sites i in [N, Ns) are padding: their links are all "wall", their populations are 0 (rest
 // state in shifted form) and stay exactly 0, so no step kernel needs a bounds branch.
@@ -277,16 +278,18 @@ __device__ __forceinline__ void bfl_write_pull(const BflFused& bf, long long idx
 }
 
 // BFL interpolated walls (linear Bouzidi-Firdaouss-Lallemand rule; the paper's "BFL" wall
-// option, ref [16]) as a PRE-PASS over the list of interpolated links,
-// run on the state buffer before the step (or read-out) that gathers from it. Written out for
-// the two-lattice scheme: slot opp(p) of site x holds f*_opp(p)(x, t-1) and is read by nobody but x
-// itself, as the halfway bounce-back value of its wall link p; the pre-pass replaces it by
+// option, ref [16]) as a PRE-PASS over a list of interpolated links,
+// run on the state buffer before a READ-OUT that gathers from it (the step kernels apply the
+// rules themselves, see above; the API passes the d < 1/2 links only, the d >= 1/2 rule being
+// already in what the step kernels wrote -- the kernel handles both). Written out for the
+// two-lattice scheme: slot opp(p) of site x holds f*_opp(p)(x, t-1) and is read by nobody but
+// x itself, as the halfway bounce-back value of its wall link p; the pre-pass replaces it by
 //   d <  1/2:  2d f*_opp(p)(x) + (1 - 2d) f*_opp(p)(x + c_p)      (slot opp(p) of the site behind)
 //   d >= 1/2:  f*_opp(p)(x) / (2d) + (1 - 1/(2d)) f*_p(x)         (slot p of x itself)
-// so that the fused step kernel needs no BFL code at all. The sources are slots that no
-// link of the list writes (a link is in the list only if the site behind it is fluid), so
-// the pass has no ordering hazards. An in-kernel version (interpolating at gather time behind
-// a per-site bit) cost 30 % of the step on configs[3]; this costs ~9 % (profiles/r01_tuning.md).
+// The sources are slots that no link of the list writes (a link is in the list only if the
+// site behind it is fluid), so the pass has no ordering hazards. As the way to apply BFL on
+// every step it cost 23-25 % of configs[3] against 12-18 % in registers (profiles/r01_tuning.md
+// section 11).
 // Where the three values live depends on what the state buffer holds (GatherMode of the state):
 //   GATHER_PULL   (two-lattice, post-collision f*_r(z) in slot r of z):
 //       target f*_i(x): slot i of x;  f*_i(y): slot i of y;  f*_q(x): slot q of x
