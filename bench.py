@@ -70,8 +70,11 @@ def parse_args():
     ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
     ap.add_argument("--lattice", default="d3q15", choices=["d3q15", "d3q19"],
                     help="d3q15 = BASELINE.json's metric; d3q19 = the lattice the paper ran (NEXT-1)")
-    ap.add_argument("--inlet", default="pressure", choices=["pressure", "velocity"],
-                    help="velocity: iolet 0 becomes a Ladd velocity inlet (the paper's LADDIOLET)")
+    ap.add_argument("--inlet", default="pressure", choices=["pressure", "velocity", "waveform", "host_waveform"],
+                    help="velocity: iolet 0 becomes a Ladd velocity inlet (the paper's LADDIOLET); "
+                         "waveform: the same, driven by a device-resident pulsatile waveform "
+                         "(hlb_set_iolet_waveform, period 1000 steps); host_waveform: the same "
+                         "waveform handed over by hlb_set_iolet_velocity before every LB step")
     ap.add_argument("--walls", default="bounce_back", choices=["bounce_back", "bfl_random"],
                     help="bfl_random: interpolated (BFL) walls with seeded random distances on every "
                          "wall link -- the kernel work of the paper's BFL option (two_lattice only)")
@@ -369,14 +372,27 @@ def main():
     S = args.inner
     if wl.rho0 is not None or wl.u0 is not None:
         g.hlb_set_state(wl.rho0, wl.u0)
-    if args.inlet == "velocity" and wl.n_iolets > 0:
+    wave = None
+    if args.inlet != "pressure" and wl.n_iolets > 0:
         wl = W.with_velocity_inlet(wl)
         g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+        if args.inlet in ("waveform", "host_waveform"):
+            wave = W.pulsatile_waveform(wl, 1000)
+            if args.inlet == "waveform":
+                g.hlb_set_iolet_waveform(wave)
     if args.walls == "bfl_random":
         d27 = np.random.default_rng(1906).uniform(0.05, 1.0, size=(N, 27))
         g.hlb_set_wall_distance(d27)
         del d27
     stream = torch.cuda.current_stream()
+
+    def advance(n):
+        if args.inlet == "host_waveform" and wave is not None:
+            for _ in range(n):       # the time-varying inlet without the device-resident table
+                g.hlb_set_iolet_velocity(wl.iolet_kind, wave[g.hlb_steps_done() % len(wave)])
+                g.hlb_step(1)
+        else:
+            g.hlb_step(n)
 
     def barrier():
         if world > 1:
@@ -385,7 +401,7 @@ def main():
 
     # ---------------- device-resident timing: K x hlb_step(S)
     for _ in range(args.warmup):
-        g.hlb_step(S)
+        advance(S)
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -396,7 +412,7 @@ def main():
     w0 = time.time()
     ev0.record(stream)
     for _ in range(args.steps):
-        g.hlb_step(S)
+        advance(S)
     ev1.record(stream)
     barrier()
     w1 = time.time()
@@ -443,7 +459,7 @@ def main():
 
         def e2e_step():
             g.hlb_set_state(rin_np, uin_np)             # H2D: rho [N], u [N][3]
-            g.hlb_step(S)
+            advance(S)
             g.hlb_get_macroscopic(rho_np, u_np)        # D2H: rho [N], u [N][3] (synchronises)
 
         e2e_steps = max(2, min(args.steps, 5))

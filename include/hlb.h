@@ -159,6 +159,25 @@ int64_t hlb_num_bfl_sites(const hlb_geometry* g);
  * hlb_step(n) / hlb_set_iolet_velocity(...) in turn. Errors: HLB_EINVAL. */
 int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u);
 
+/* Device-resident velocity waveform for the velocity iolets (the paper drives its inlet from
+ * a velocity file, Table I "inlet velocity" and line 126 Fig. 8): with a
+ * waveform the step that advances the state from time t to t+1 (t = hlb_steps_done() before
+ * it) applies Ladd's rule of hlb_set_iolet_velocity with
+ *     u_k = u[t mod n_t][k]            (periodic in time, one vector per iolet and time level)
+ * for every iolet k of kind 1, so hlb_step(n) covers n time levels with no host work between
+ * the launches (calling hlb_set_iolet_velocity before every step gives the same result and
+ * costs a stream synchronisation per step).
+ *   u: HOST [n_t][n_iolets][3] lattice velocities, copied during the call; rows of iolets of
+ *   kind 0 are ignored. n_t >= 1. u == NULL or n_t == 0 removes the waveform: velocity iolets
+ *   go back to the constant vectors of hlb_set_iolet_velocity.
+ * The kinds (hlb_set_iolet_velocity), densities and normals may be changed afterwards; the
+ * waveform stays. hlb_set_state / hlb_set_populations reset the time to 0. The table
+ * (n_t * n_iolets * 32 bytes) comes from the allocator. While a waveform is set the steps are
+ * launched directly (no CUDA-graph replay: a captured launch fixes its time level).
+ * Errors: HLB_EINVAL (n_t < 0, no iolets but n_t > 0, non-finite velocity), HLB_ENOMEM,
+ * HLB_ECUDA. */
+int hlb_set_iolet_waveform(hlb_geometry* g, const double* u, int64_t n_t);
+
 /* Advance n >= 0 time steps: n launches of ONE fused collide-and-stream kernel (A-A:
  * alternating even/odd kernels), asynchronously on the stream. n == 0 is a no-op. A
  * kernel fault surfaces at the next synchronising call. For geometries of up to 2^22

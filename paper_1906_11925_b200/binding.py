@@ -80,6 +80,7 @@ def _load() -> ctypes.CDLL:
         "hlb_set_state": (c_int, [vp, vp, vp]),
         "hlb_set_iolet_density": (c_int, [vp, vp]),
         "hlb_set_iolet_velocity": (c_int, [vp, vp, vp]),
+        "hlb_set_iolet_waveform": (c_int, [vp, vp, i64]),
         "hlb_set_iolet_normal": (c_int, [vp, vp]),
         "hlb_set_wall_distance": (c_int, [vp, vp]),
         "hlb_num_bfl_sites": (i64, [vp]),
@@ -122,7 +123,7 @@ def _load() -> ctypes.CDLL:
 LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
-            "hlb_set_iolet_velocity", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
+            "hlb_set_iolet_velocity", "hlb_set_iolet_waveform", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
@@ -259,6 +260,7 @@ class Geometry:
             _check(_lib.hlb_geometry_create(_ptr(st), ctypes.byref(p), ctypes.byref(self._h)))
         self.n_sites = int(_lib.hlb_num_sites(self._h))
         self.n_q = int(_lib.hlb_num_q(self._h))
+        self.n_iolets = int(p.n_iolets)
         self.flags = int(flags)
 
     # -- the C-ABI calls, same names -------------------------------------------------
@@ -275,6 +277,18 @@ class Geometry:
         kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8)
         u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64)
         _check(_lib.hlb_set_iolet_velocity(self._h, _ptr(kind), _ptr(u)))
+
+    def hlb_set_iolet_waveform(self, u):
+        """u: [n_t][n_iolets][3] (or None to remove the waveform)."""
+        if u is None:
+            _check(_lib.hlb_set_iolet_waveform(self._h, None, 0))
+            return
+        u = _host(np.asarray(u, dtype=np.float64), np.float64)
+        if u.ndim != 3 or u.shape[2] != 3:
+            raise ValueError("waveform must have shape [n_t][n_iolets][3]")
+        if u.shape[1] != self.n_iolets:
+            raise ValueError(f"waveform has {u.shape[1]} iolets, the geometry {self.n_iolets}")
+        _check(_lib.hlb_set_iolet_waveform(self._h, _ptr(u), int(u.shape[0])))
 
     def hlb_set_iolet_normal(self, normals):
         n = None if normals is None else _host(np.asarray(normals, dtype=np.float64).reshape(-1, 3), np.float64)

@@ -61,6 +61,15 @@ struct hlb_geometry {
   std::vector<double> iolet_u;        // [n_iolets][3]
   std::vector<double> iolet_n;        // [n_iolets][3] unit normals of density iolets, 0 = none
   std::vector<double> iolet_par;      // [n_iolets][4] as uploaded: {rho or -1, ux, uy, uz}
+  double* d_iolet_par = nullptr;      // device copy of iolet_par (dg.iolet_par points here, or
+                                      // into d_wave while a waveform is set)
+  // hlb_set_iolet_waveform: one [n_iolets][4] slice per time level, the rows of velocity
+  // iolets carrying u[t][k]; the step at time t is launched with the slice t mod wave_nt
+  std::vector<double> wave_u;         // [wave_nt][n_iolets][3] as given
+  std::vector<double> wave_par;       // [wave_nt][n_iolets][4] as uploaded
+  int64_t wave_nt = 0;
+  double* d_wave = nullptr;
+  size_t wave_cap = 0;                // doubles d_wave can hold
   DeviceGeometry dg;
   void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
   int cur = 0;                        // two-lattice: buffer the next step reads
@@ -221,8 +230,30 @@ static int upload_iolets(hlb_geometry* g) {
     }
   }
   if (g->dg.iolet_full != was_full) g->drop_graph();  // another instantiation of the step kernels
-  HLB_CUDA(cudaMemcpyAsync((void*)g->dg.iolet_par, g->iolet_par.data(), sizeof(double) * 4 * (size_t)n,
+  HLB_CUDA(cudaMemcpyAsync(g->d_iolet_par, g->iolet_par.data(), sizeof(double) * 4 * (size_t)n,
                            cudaMemcpyHostToDevice, g->stream));
+  if (g->wave_nt > 0) {
+    // every time level is the slice above with the velocity rows replaced by u[t][k]
+    const size_t slice = 4 * (size_t)n, total = slice * (size_t)g->wave_nt;
+    if (total > g->wave_cap) {
+      void* ptr = nullptr;
+      const int rc = g->alloc(sizeof(double) * total, &ptr);  // (there is no free callback)
+      if (rc) return rc;
+      g->d_wave = (double*)ptr;
+      g->wave_cap = total;
+    }
+    g->wave_par.resize(total);
+    for (int64_t t = 0; t < g->wave_nt; ++t) {
+      double* row = g->wave_par.data() + (size_t)t * slice;
+      std::memcpy(row, g->iolet_par.data(), sizeof(double) * slice);
+      for (int k = 0; k < n; ++k)
+        if (g->iolet_kind[(size_t)k] == 1)
+          for (int a = 0; a < 3; ++a)
+            row[(size_t)k * 4 + 1 + a] = g->wave_u[((size_t)t * (size_t)n + (size_t)k) * 3 + (size_t)a];
+    }
+    HLB_CUDA(cudaMemcpyAsync(g->d_wave, g->wave_par.data(), sizeof(double) * total,
+                             cudaMemcpyHostToDevice, g->stream));
+  }
   return HLB_OK;
 }
 
@@ -320,7 +351,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   if (use_rec)
     HLB_CUDA_G(cudaMemcpyAsync(d_rec, t.rec.data(), sizeof(uint32_t) * t.rec.size(), cudaMemcpyHostToDevice, g->stream));
   HLB_CUDA_G(cudaMemcpyAsync(d_canon, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N, cudaMemcpyHostToDevice, g->stream));
-  g->dg.iolet_par = (const double*)d_rho;
+  g->d_iolet_par = (double*)d_rho;
+  g->dg.iolet_par = g->d_iolet_par;
   if ((rc = upload_iolets(g))) return bail(rc);
   g->dg.N = t.N;
   g->dg.Ns = t.Ns;
@@ -557,10 +589,39 @@ int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u
   return upload_iolets(g);
 }
 
+int hlb_set_iolet_waveform(hlb_geometry* g, const double* u, int64_t n_t) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (n_t < 0) return fail(HLB_EINVAL, "n_t < 0");
+  const int n = g->p.n_iolets;
+  if (n_t > 0 && n == 0) return fail(HLB_EINVAL, "a waveform needs at least one iolet");
+  g->drop_graph();
+  if (!u || n_t == 0) {
+    g->wave_nt = 0;
+    g->wave_u.clear();
+    return HLB_OK;
+  }
+  const size_t count = (size_t)n_t * (size_t)n * 3;
+  for (size_t j = 0; j < count; ++j)
+    if (!std::isfinite(u[j])) return fail(HLB_EINVAL, "non-finite waveform velocity");
+  HLB_CUDA(cudaStreamSynchronize(g->stream));  // an earlier upload may still read wave_par
+  g->wave_u.assign(u, u + count);
+  g->wave_nt = n_t;
+  const int rc = upload_iolets(g);
+  if (rc) {
+    g->wave_nt = 0;
+    g->wave_u.clear();
+  }
+  return rc;
+}
+
 constexpr int64_t GRAPH_STEPS = 32;  // even: the buffer / phase parity is back where it started
 
 static void enqueue_one_step(hlb_geometry* g) {
   g->dg.bflf.gather = g->gather_bfl() ? 1 : 0;
+  // the iolet parameters of this time level (hlb_set_iolet_waveform), else the constant ones
+  g->dg.iolet_par = g->wave_nt > 0
+                        ? g->d_wave + (size_t)(g->steps % g->wave_nt) * 4 * (size_t)g->p.n_iolets
+                        : g->d_iolet_par;
   if (g->aa) {
     launch_aa(g->dg, g->buf[0], (g->steps & 1) != 0, g->stream);
     g->bfl_applied = false;  // every slot has been rewritten in place
@@ -602,8 +663,9 @@ int hlb_step(hlb_geometry* g, int64_t n) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
   if (n < 0) return fail(HLB_EINVAL, "n < 0");
   // graphs pay off only when a step is short next to the launch cost
+  // (a captured launch carries its arguments: not with a waveform, whose slice changes per step)
   const bool want_graph = !(g->p.flags & HLB_NO_GRAPH) && !g->graph_failed && g->stream != nullptr &&
-                          g->N <= (int64_t)4 << 20;
+                          g->N <= (int64_t)4 << 20 && g->wave_nt == 0;
   int64_t left = n;
   while (left > 0) {
     const bool even = g->aa ? (g->steps & 1) == 0 : g->cur == 0;

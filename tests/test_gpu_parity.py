@@ -277,6 +277,103 @@ def test_time_varying_velocity_inlet_and_mixed_kinds(hlb, scheme):
     g.close()
 
 
+def _oracle_with_waveform(wl, wave, steps, lattice):
+    """The definition the waveform must reproduce: the oracle stepped one time level at a time,
+    its velocity iolets set to u[t mod n_t] before the step from t to t+1."""
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, lattice=lattice)
+    if wl.rho0 is not None or wl.u0 is not None:
+        o.set_state(wl.rho0, wl.u0)
+    for t in range(steps):
+        o.set_iolet_velocity(wl.iolet_kind, wave[t % len(wave)])
+        o.step(1)
+    out = o.get_macroscopic()
+    o.close()
+    return out
+
+
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_inlet_waveform_matches_per_step_oracle(hlb, scheme, lattice):
+    """Device-resident inlet waveform (the paper's inlet velocity file):
+    hlb_step(n) over several periods, with a read-out in between, against the oracle driven one
+    step at a time. 71 steps on a small geometry would use the 32-step graph replay if the
+    waveform did not switch it off (a captured launch fixes its time level)."""
+    for name, store, n_t, steps in (("pipe", "f64", 7, 71), ("aneurysm", "f64", 5, 18),
+                                    ("tree", "f32", 9, 23)):
+        wl = W.with_velocity_inlet(W.by_name(name, small=True))
+        wave = W.pulsatile_waveform(wl, n_t)
+        rho_ref, u_ref = _oracle_with_waveform(wl, wave, steps, lattice)
+        g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                    flags_of(hlb, scheme, store, "raster", "auto", lattice))
+        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+        g.hlb_set_iolet_waveform(wave)
+        launches0 = g.hlb_launch_count()
+        g.hlb_step(n_t + 1)
+        g.hlb_get_macroscopic()                               # a read-out in mid-period
+        g.hlb_step(steps - n_t - 1)
+        assert g.hlb_steps_done() == steps
+        assert g.hlb_launch_count() - launches0 == steps      # one fused kernel per time level
+        e_rho, e_u = errors(*g.hlb_get_macroscopic(), rho_ref, u_ref)
+        assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, lattice, e_rho, e_u)
+        g.close()
+        assert np.max(np.abs(u_ref)) > 1e-4
+
+
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_inlet_waveform_is_bitwise_the_host_driven_sequence(hlb, scheme):
+    """The waveform is only another way of handing u_k(t) to the same kernels: populations are
+    bitwise those of hlb_set_iolet_velocity before every step. Also: the time restarts with
+    hlb_set_state, later density / kind changes keep the waveform, NULL removes it."""
+    wl = W.random_mask((13, 11, 12), p_fluid=0.7, n_iolets=3, p_iolet=0.08, periodic=1, tau=0.58, seed=17)
+    kind = np.array([1, 0, 1], dtype=np.uint8)
+    rng = np.random.default_rng(5)
+    n_t = 4
+    wave = 0.02 * (rng.random((n_t, 3, 3)) - 0.5)
+    flags = flags_of(hlb, scheme, "f64", "raster", "auto")
+    a = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
+    b = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
+    for x in (a, b):
+        x.hlb_set_state(wl.rho0, wl.u0)
+    a.hlb_set_iolet_velocity(kind, np.zeros((3, 3)))
+    a.hlb_set_iolet_waveform(wave)
+    a.hlb_step(11)
+    for t in range(11):
+        b.hlb_set_iolet_velocity(kind, wave[t % n_t])
+        b.hlb_step(1)
+    assert np.array_equal(a.hlb_get_populations(), b.hlb_get_populations())
+    # densities and kinds change, the waveform stays; time restarts at 0 with hlb_set_state
+    rho2 = [1.004, 0.997, 1.001]
+    kind2 = np.array([0, 1, 1], dtype=np.uint8)
+    for x in (a, b):
+        x.hlb_set_state(wl.rho0, wl.u0)
+        x.hlb_set_iolet_density(rho2)
+    a.hlb_set_iolet_velocity(kind2, np.zeros((3, 3)))
+    a.hlb_step(6)
+    for t in range(6):
+        b.hlb_set_iolet_velocity(kind2, wave[t % n_t])
+        b.hlb_step(1)
+    assert np.array_equal(a.hlb_get_populations(), b.hlb_get_populations())
+    # removed: back to the constant vectors
+    const_u = 0.01 * (rng.random((3, 3)) - 0.5)
+    a.hlb_set_iolet_waveform(None)
+    a.hlb_set_iolet_velocity(kind2, const_u)
+    b.hlb_set_iolet_velocity(kind2, const_u)
+    a.hlb_step(5)
+    b.hlb_step(5)
+    assert np.array_equal(a.hlb_get_populations(), b.hlb_get_populations())
+    with pytest.raises(hlb.HlbError):
+        a.hlb_set_iolet_waveform(np.full((2, 3, 3), np.nan))
+    with pytest.raises(ValueError):
+        a.hlb_set_iolet_waveform(np.zeros((2, 2, 3)))
+    a.close()
+    b.close()
+    cube = W.by_name("cube", small=True)                      # no iolets: nothing to drive
+    c = hlb.hlb_geometry_create(cube.site_type, cube.periodic, cube.tau, cube.iolet_rho, flags)
+    with pytest.raises(hlb.HlbError):
+        c.hlb_set_iolet_waveform(np.zeros((2, 0, 3)))
+    c.close()
+
+
 @pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
 def test_normal_projected_pressure_iolets_match_oracle(hlb, scheme, lattice):

@@ -14,6 +14,7 @@ from .geometries import (  # noqa: F401
     random_mask,
     by_name,
     with_velocity_inlet,
+    pulsatile_waveform,
     with_bfl_walls,
     wall_distance_by_bisection,
     CONFIG_NAMES,

@@ -353,6 +353,27 @@ def with_velocity_inlet(wl: Workload, u_in: float = 0.004) -> Workload:
     return dataclasses.replace(wl, iolet_kind=kind, iolet_u=u, name=wl.name)
 
 
+def pulsatile_waveform(wl: Workload, n_t: int, u_peak: float = 0.006, u_base: float = 0.002,
+                       seed: int = 8) -> np.ndarray:
+    """A periodic inlet-velocity waveform u[n_t][n_iolets][3] standing in for the paper's inlet
+    velocity file (Table I, line 126 Fig. 8 -- the data are not in the paper):
+    a cardiac-cycle-like pulse, baseline u_base plus a systolic bump to u_peak over the first
+    third of the period and a small seeded dicrotic ripple, along the direction of
+    ``wl.iolet_u[0]`` (see with_velocity_inlet) for iolet 0; all other rows are 0 (constant-
+    density outlets ignore them). One period = n_t time steps."""
+    if wl.iolet_u is None:
+        raise ValueError("apply with_velocity_inlet first")
+    rng = np.random.default_rng(seed)
+    phase = np.arange(n_t, dtype=np.float64) / float(n_t)
+    bump = np.where(phase < 1.0 / 3.0, np.sin(3.0 * np.pi * phase) ** 2, 0.0)
+    ripple = 0.08 * float(rng.uniform(0.5, 1.0)) * np.sin(2.0 * np.pi * 3.0 * phase + float(rng.uniform(0, 6.28)))
+    speed = u_base + (u_peak - u_base) * bump + (u_peak - u_base) * ripple * (phase >= 1.0 / 3.0)
+    direction = wl.iolet_u[0] / np.linalg.norm(wl.iolet_u[0])
+    u = np.zeros((n_t, wl.n_iolets, 3), dtype=np.float64)
+    u[:, 0, :] = speed[:, None] * direction[None, :]
+    return u
+
+
 def wall_distance_by_bisection(wl: Workload, inside_fn, iters: int = 48) -> np.ndarray:
     """Sub-voxel wall distances for interpolated (BFL) walls from the analytic surface the
     voxel mask was painted from: for every fluid voxel and each of the 26 lattice vectors whose
