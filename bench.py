@@ -83,6 +83,9 @@ def parse_args():
                          "PIXELS frames of the speed field, rotating view; adds a \"render\" object")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--no-pdl", action="store_true", help="HLB_NO_PDL (ablation)")
+    ap.add_argument("--no-resident", action="store_true",
+                    help="HLB_NO_RESIDENT (ablation: small geometries step by graph replay instead "
+                         "of the resident multi-step kernel)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="scaled-down geometry (debugging only)")
@@ -363,6 +366,7 @@ def main():
              "records": hlb.HLB_LINKS_RECORDS}[args.links] | \
             (hlb.HLB_NO_PREFETCH if args.no_prefetch else 0) | \
             (hlb.HLB_NO_PDL if args.no_pdl else 0) | \
+            (hlb.HLB_NO_RESIDENT if args.no_resident else 0) | \
             (hlb.HLB_LATTICE_D3Q19 if args.lattice == "d3q19" else hlb.HLB_LATTICE_D3Q15)
     t_create = time.perf_counter()
     g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
@@ -442,6 +446,13 @@ def main():
     else:
         k_ms = {"k_pull": float(np.mean(per))}
         k_bytes = {"k_pull": pop_bytes + 4 * (nq - 1)}
+    if launches < S * args.steps:
+        # the timed region ran the resident multi-step kernel (one launch per hlb_step(S)): its
+        # per-launch duration is the timed region's own; bytes per launch = S steps' worth
+        name = "k_aa_resident" if scheme == "aa" else "k_pull_resident"
+        per_site = S * (pop_bytes + (2 if scheme == "aa" else 4) * (nq - 1))
+        k_ms = {name: ms / args.steps}
+        k_bytes = {name: per_site}
     dominant = max(k_ms, key=lambda k: k_ms[k])
 
     # ---------------- end to end through the C-ABI with host buffers
@@ -490,7 +501,8 @@ def main():
             "workload": WORKLOAD_DESC[args.workload] + (" (small)" if args.small else ""),
             "n_sites": N, "lattice": args.lattice, "lb_steps_per_step": S, "scheme": scheme, "store": args.store,
             "order": args.order, "links": "records" if g.hlb_uses_records() else "table",
-            "l2_prefetch": not args.no_prefetch, "pdl": not args.no_pdl, "inlet": args.inlet, "walls": args.walls,
+            "l2_prefetch": not args.no_prefetch, "pdl": not args.no_pdl,
+            "resident_kernel": bool(launches < S * args.steps), "inlet": args.inlet, "walls": args.walls,
             "bfl_sites": g.hlb_num_bfl_sites(),
             "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
             "box": list(wl.shape), "seed": wl.info.get("seed"),

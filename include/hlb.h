@@ -65,7 +65,9 @@ enum {
   HLB_ORDER_TILED = 0xC,   /* Morton over 8x8x8 blocks, x-fastest raster inside a block    */
   HLB_ORDER_MASK = 0xC,
   HLB_NO_GRAPH = 0x10,     /* launch every step directly instead of replaying a captured
-                              CUDA graph of steps (debugging / profiling)                  */
+                              CUDA graph of steps or running the resident multi-step kernel
+                              (debugging / profiling)                                      */
+  HLB_NO_RESIDENT = 0x800, /* never use the resident multi-step kernel (see hlb_step)      */
   HLB_LINKS_AUTO = 0x0,    /* the step kernels read the run-length link records when at
                               least half of them are not sentinels, else the table         */
   HLB_LINKS_TABLE = 0x20,  /* always read the int32 table (ablation / profiling)           */
@@ -182,7 +184,15 @@ int hlb_set_iolet_waveform(hlb_geometry* g, const double* u, int64_t n_t);
  * alternating even/odd kernels), asynchronously on the stream. n == 0 is a no-op. A
  * kernel fault surfaces at the next synchronising call. For geometries of up to 2^22
  * sites on a non-NULL stream the launches are replayed from a captured CUDA graph in
- * chunks of 32 steps (same kernels, same order; HLB_NO_GRAPH switches it off). */
+ * chunks of 32 steps (same kernels, same order; HLB_NO_GRAPH switches it off).
+ * Geometries small enough for all their thread blocks (128 sites each) to be resident on
+ * the chip at once (about 10^5 sites on a B200) run a call of n >= 2 steps as ONE
+ * cooperative launch of a resident kernel instead: every thread keeps its site and its link
+ * offsets in registers for the n steps, with a grid-wide barrier between steps in place of
+ * the kernel boundary (same per-site arithmetic, bitwise the same results; not with
+ * interpolated walls or a waveform; HLB_NO_RESIDENT or HLB_NO_GRAPH switches it off). Such a
+ * launch needs every SM slot it was sized for: it must not share the device with another
+ * long-running kernel of the same process that waits on it. */
 int hlb_step(hlb_geometry* g, int64_t n);
 
 /* rho(x) = sum_q f_q, u(x) = sum_q c_q f_q / rho of the PRE-collision populations after
@@ -227,7 +237,8 @@ int64_t hlb_steps_done(const hlb_geometry* g);
 int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v);
 /* Bytes of device memory the geometry holds (populations + tables + scratch). */
 int64_t hlb_device_bytes(const hlb_geometry* g);
-/* Kernel launches enqueued by hlb_step() so far (graph replays count their nodes; with BFL
+/* Kernel launches enqueued by hlb_step() so far (graph replays count their nodes; a resident
+ * multi-step launch counts once; with BFL
  * walls the pre-pass over the interpolated links counts too, also when a read-out runs it). */
 int64_t hlb_launch_count(const hlb_geometry* g);
 /* 1 if the step kernels of this geometry read the link records, 0 if they read the table. */

@@ -24,6 +24,7 @@ HLB_LINKS_AUTO, HLB_LINKS_TABLE, HLB_LINKS_RECORDS = 0x0, 0x20, 0x40
 HLB_NO_PREFETCH = 0x80
 HLB_INDEX64 = 0x100
 HLB_NO_PDL = 0x400
+HLB_NO_RESIDENT = 0x800
 HLB_LATTICE_D3Q15, HLB_LATTICE_D3Q19 = 0x0, 0x200
 
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)

@@ -92,6 +92,11 @@ struct hlb_geometry {
   size_t bfl_cap_links = 0, bfl_cap_coef = 0;
   cudaGraphExec_t graph_exec = nullptr;
   bool graph_failed = false;
+  // resident multi-step kernel (small geometries; kernels.cuh launch_resident_steps)
+  unsigned long long* d_bar = nullptr;  // grid-barrier arrival counter
+  unsigned long long bar_base = 0;      // its value once everything enqueued so far has run
+  int64_t resident_max_sites = 0;       // Ns up to which the whole grid is resident at once
+  bool resident_failed = false;         // a cooperative launch was refused: do not try again
   // The captured launches fix the kernel instantiation and the by-value arguments: drop the
   // graph whenever one of them changes (iolet kinds / normals, wall distances).
   void drop_graph() {
@@ -168,7 +173,7 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
   if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
                              HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH | HLB_INDEX64 |
-                             HLB_LATTICE_D3Q19 | HLB_NO_PDL))
+                             HLB_LATTICE_D3Q19 | HLB_NO_PDL | HLB_NO_RESIDENT))
     return fail(HLB_EINVAL, "unknown flag bits");
   if ((p->flags & HLB_LINKS_TABLE) && (p->flags & HLB_LINKS_RECORDS))
     return fail(HLB_EINVAL, "HLB_LINKS_TABLE and HLB_LINKS_RECORDS are exclusive");
@@ -340,6 +345,19 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   if (!g->aa && (rc = g->alloc(pop_bytes + pad_bytes, &g->buf[1]))) return bail(rc);
   if ((rc = g->alloc(sizeof(double) * 4 * (size_t)t.N, &d_scratch))) return bail(rc);
   g->scratch = (double*)d_scratch;
+  {
+    int dev = 0, sms = 0, coop = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop) {
+      void* d_bar = nullptr;
+      if ((rc = g->alloc(256, &d_bar))) return bail(rc);
+      g->d_bar = (unsigned long long*)d_bar;
+      g->resident_max_sites = (int64_t)sms * resident_kernel_sites_per_sm();
+    } else {
+      (void)cudaGetLastError();
+    }
+  }
 
 #define HLB_CUDA_G(call)                                                   \
   do {                                                                     \
@@ -350,6 +368,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   HLB_CUDA_G(cudaMemcpyAsync(d_bits, t.iolet_bits.data(), sizeof(uint32_t) * t.iolet_bits.size(), cudaMemcpyHostToDevice, g->stream));
   if (use_rec)
     HLB_CUDA_G(cudaMemcpyAsync(d_rec, t.rec.data(), sizeof(uint32_t) * t.rec.size(), cudaMemcpyHostToDevice, g->stream));
+  if (g->d_bar) HLB_CUDA_G(cudaMemsetAsync(g->d_bar, 0, 256, g->stream));
   HLB_CUDA_G(cudaMemcpyAsync(d_canon, t.canon_of_site.data(), sizeof(int32_t) * (size_t)t.N, cudaMemcpyHostToDevice, g->stream));
   g->d_iolet_par = (double*)d_rho;
   g->dg.iolet_par = g->d_iolet_par;
@@ -666,6 +685,23 @@ int hlb_step(hlb_geometry* g, int64_t n) {
   // (a captured launch carries its arguments: not with a waveform, whose slice changes per step)
   const bool want_graph = !(g->p.flags & HLB_NO_GRAPH) && !g->graph_failed && g->stream != nullptr &&
                           g->N <= (int64_t)4 << 20 && g->wave_nt == 0;
+  // small geometry: all n steps in one cooperative launch of the resident kernel
+  if (n >= 2 && g->d_bar && !(g->p.flags & (HLB_NO_GRAPH | HLB_NO_RESIDENT)) && !g->resident_failed &&
+      !g->bfl_set && g->wave_nt == 0 && g->Ns <= g->resident_max_sites) {
+    g->dg.iolet_par = g->d_iolet_par;
+    const cudaError_t e = launch_resident_steps(
+        g->dg, g->aa, g->aa ? g->buf[0] : g->buf[g->cur], g->aa ? nullptr : g->buf[g->cur ^ 1],
+        (long long)n, (int)(g->steps & 1), g->d_bar, g->bar_base, g->stream);
+    if (e == cudaSuccess) {
+      g->bar_base += (unsigned long long)(n - 1) * (unsigned long long)(g->Ns / 128);
+      g->steps += n;
+      if (!g->aa && (n & 1)) g->cur ^= 1;
+      ++g->launches;
+      return HLB_OK;
+    }
+    (void)cudaGetLastError();  // refused (e.g. too large for this instantiation): step by step
+    g->resident_failed = true;
+  }
   int64_t left = n;
   while (left > 0) {
     const bool even = g->aa ? (g->steps & 1) == 0 : g->cur == 0;

@@ -25,6 +25,8 @@
 // state in shifted form) and stay exactly 0, so no step kernel needs a bounds branch.
 #include "kernels.cuh"
 
+#include <tuple>
+
 #include "lbgk.cuh"
 
 namespace hlb {
@@ -487,6 +489,131 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
 }
 
+// ------------------------------------------------------------------ resident multi-step kernels
+// Small geometries (every block of the grid resident on the chip at once; BASELINE configs[0]
+// is 99 blocks) are bound by the launch-to-launch gap, not by memory: one cooperative launch
+// runs n time steps, a thread keeping its site and its decoded link offsets in registers for
+// the whole run, with a grid-wide barrier between steps in place of the kernel boundary. The
+// per-site arithmetic is the same device code as in the one-shot kernels (bitwise identical
+// results). Populations written by other SMs are read with ld.global.cg (L2; never a stale L1
+// line). The barrier is a monotone arrival counter in global memory: after step s every block
+// adds 1 and waits until the counter reaches base + (s + 1) * gridDim.x (the host advances
+// base by (n - 1) * gridDim.x per launch; 64 bits never wrap).
+__device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned long long target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    // release: this block's stores (ordered before by the bar.sync) are visible before the
+    // arrival; a reduction, so nothing waits for the old value to come back
+    asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(bar) : "memory");
+    unsigned long long v;
+    do {
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(bar) : "memory");
+    } while (v < target);
+  }
+  __syncthreads();
+}
+template <typename ST>
+__device__ __forceinline__ double load_l2(const ST* p) { return to_real(__ldcg(p)); }
+// Occupancy does not matter here (the grid is at most one block per slot and the run is
+// latency-bound): 4 blocks per SM leave 128 registers, enough to keep the link offsets, the
+// populations and the loop state without spills. (A second instantiation for 6 blocks per SM,
+// 80 registers with spills, gained 3-9 % at 96 k sites and lost 10-14 % at 112 k against the
+// one-shot kernels; so did a looping form for L2-sized geometries: profiles/r01_tuning.md
+// section 14.)
+constexpr int RESIDENT_MINB = 4;
+
+// One site update of the resident kernels (the bodies of k_aa_even / k_aa_odd and k_pull).
+template <typename L, typename ST, typename IT, int V>
+__device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
+                                        const double* __restrict__ iolet_par, long long Ns,
+                                        double omega, long long i, const IT (&off)[L::Q - 1],
+                                        bool iolet, bool odd) {
+  double h[L::Q];
+  h[0] = load_l2(a + i);
+  if (odd) {
+#pragma unroll
+    for (int q = 1; q < L::Q; ++q) h[q] = load_l2(a + off[q - 1]);
+  } else {
+#pragma unroll
+    for (int q = 1; q < L::Q; ++q) h[q] = load_l2(a + (long long)q * Ns + i);
+  }
+  const Moments m = moments_of<L>(h);
+  collide<L>(h, m, omega, h);
+  double out[L::Q];
+#pragma unroll
+  for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
+  if (iolet) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, out);
+  a[i] = to_store<ST>(out[0]);
+  if (odd) {
+#pragma unroll
+    for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
+  } else {
+#pragma unroll
+    for (int p = 1; p < L::Q; ++p) a[(long long)p * Ns + i] = to_store<ST>(out[p]);
+  }
+}
+template <typename L, typename ST, typename IT, int V>
+__device__ __forceinline__ void pull_site(const ST* src, ST* dst, const int32_t* __restrict__ nbr,
+                                          const double* __restrict__ iolet_par, long long Ns,
+                                          double omega, long long i, const IT (&off)[L::Q - 1],
+                                          bool iolet) {
+  double h[L::Q];
+  h[0] = load_l2(src + i);
+#pragma unroll
+  for (int q = 1; q < L::Q; ++q) h[q] = load_l2(src + off[q - 1]);
+  const Moments m = moments_of<L>(h);
+  collide<L>(h, m, omega, h);
+  if (iolet) {
+    double back[L::Q];
+#pragma unroll
+    for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
+    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, back);
+#pragma unroll
+    for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
+  }
+#pragma unroll
+  for (int q = 0; q < L::Q; ++q) dst[(long long)q * Ns + i] = to_store<ST>(h[q]);
+}
+
+template <typename L, typename ST, bool REC, typename IT, int V>
+__global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
+k_aa_resident(ST* a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
+              const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
+              long long Ns, double omega, long long n_steps, int odd0, unsigned long long* bar,
+              unsigned long long bar_base) {
+  const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
+  IT off[L::Q - 1];
+  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
+  const bool iolet = has_iolet_link(iolet_bits, i);
+  bool odd = odd0 != 0;
+  for (long long s = 0; s < n_steps; ++s) {
+    aa_site<L, ST, IT, V>(a, nbr, iolet_par, Ns, omega, i, off, iolet, odd);
+    odd = !odd;
+    if (s + 1 < n_steps) grid_barrier(bar, bar_base + (unsigned long long)(s + 1) * gridDim.x);
+  }
+}
+
+template <typename L, typename ST, bool REC, typename IT, int V>
+__global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
+k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
+                const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
+                long long Ns, double omega, long long n_steps, unsigned long long* bar,
+                unsigned long long bar_base) {
+  const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
+  IT off[L::Q - 1];
+  link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
+  const bool iolet = has_iolet_link(iolet_bits, i);
+  const ST* src = b0;
+  ST* dst = b1;
+  for (long long s = 0; s < n_steps; ++s) {
+    pull_site<L, ST, IT, V>(src, dst, nbr, iolet_par, Ns, omega, i, off, iolet);
+    ST* t = const_cast<ST*>(src);
+    src = dst;
+    dst = t;
+    if (s + 1 < n_steps) grid_barrier(bar, bar_base + (unsigned long long)(s + 1) * gridDim.x);
+  }
+}
+
 // ------------------------------------------------------------------ read-out / init
 template <typename L, typename ST, int MODE>
 __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
@@ -637,6 +764,7 @@ int bfl_row_doubles(bool d3q19) { return d3q19 ? bfl_row<D3Q19>() : bfl_row<D3Q1
 int resident_sites_per_sm_pull(bool d3q19) {
   return SBLOCK * (d3q19 ? pull_minb<D3Q19, true>() : pull_minb<D3Q15, true>());
 }
+int resident_kernel_sites_per_sm() { return SBLOCK * RESIDENT_MINB; }
 int resident_sites_per_sm_aa(bool d3q19) {
   return SBLOCK * (d3q19 ? aa_odd_minb<D3Q19, true>() : aa_odd_minb<D3Q15, true>());
 }
@@ -759,6 +887,50 @@ static void dispatch(const DeviceGeometry& g, F&& f) {
     if (g.f32) f(D3Q15{}, float{});
     else f(D3Q15{}, double{});
   }
+}
+
+// Cooperative launch of a resident kernel: fails (without launching) with
+// cudaErrorCooperativeLaunchTooLarge when the grid does not fit on the chip at once.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_resident(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaStream_t s,
+                                   Args... args) {
+  std::tuple<KArgs...> vals{KArgs(args)...};
+  void* ptrs[sizeof...(KArgs)];
+  int k = 0;
+  std::apply([&](auto&... v) { ((ptrs[k++] = (void*)&v), ...); }, vals);
+  return cudaLaunchCooperativeKernel((const void*)kernel, dim3((unsigned)(g.Ns / SBLOCK)), dim3(SBLOCK),
+                                     ptrs, 0, s);
+}
+template <typename L, typename ST, bool REC>
+static cudaError_t resident_launch(const DeviceGeometry& g, bool aa, void* b0, void* b1, long long n,
+                                   int odd0, unsigned long long* bar, unsigned long long base,
+                                   cudaStream_t s) {
+  using IT = uint32_t;
+  if (aa) {
+#define HLB_RES_ARGS s, (ST*)b0, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, \
+                     g.omega, n, odd0, bar, base
+    return g.iolet_full ? launch_resident(g, k_aa_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS)
+                        : launch_resident(g, k_aa_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
+#undef HLB_RES_ARGS
+  }
+#define HLB_RES_ARGS s, (ST*)b0, (ST*)b1, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, \
+                     (long long)g.Ns, g.omega, n, bar, base
+  return g.iolet_full ? launch_resident(g, k_pull_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS)
+                      : launch_resident(g, k_pull_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
+#undef HLB_RES_ARGS
+}
+cudaError_t launch_resident_steps(const DeviceGeometry& g, bool aa, void* b0, void* b1, long long n,
+                                  int odd0, unsigned long long* bar, unsigned long long base,
+                                  cudaStream_t s) {
+  if (g.index64) return cudaErrorCooperativeLaunchTooLarge;  // 32-bit offsets only (small geometries)
+  cudaError_t e = cudaSuccess;
+  dispatch(g, [&](auto l, auto st) {
+    using L = decltype(l);
+    using ST = decltype(st);
+    e = g.use_rec ? resident_launch<L, ST, true>(g, aa, b0, b1, n, odd0, bar, base, s)
+                  : resident_launch<L, ST, false>(g, aa, b0, b1, n, odd0, bar, base, s);
+  });
+  return e;
 }
 
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {

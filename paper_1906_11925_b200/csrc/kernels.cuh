@@ -63,11 +63,23 @@ int bfl_row_doubles(bool d3q19);
 // Sites resident on an SM at once (threads per block x resident blocks) per step kernel.
 int resident_sites_per_sm_pull(bool d3q19);
 int resident_sites_per_sm_aa(bool d3q19);
+// Sites per SM the resident multi-step kernels (launch_resident_steps) are sized for.
+int resident_kernel_sites_per_sm();
 
 // One time step, two-lattice pull: dst <- collide(gather(src)).
 void launch_pull(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s);
 // One time step, A-A in place; `odd` selects the phase.
 void launch_aa(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s);
+
+// n >= 1 time steps in ONE cooperative launch (small geometries: the whole grid of Ns / 128
+// blocks must be resident at once, else cudaErrorCooperativeLaunchTooLarge and nothing is
+// launched). A-A: b0 is the array, odd0 the phase of the first step; two-lattice: the first
+// step reads b0 and writes b1, then they alternate. bar: a zero-initialised device counter owned
+// by the geometry; base: its value before the launch (the launch adds (n - 1) * Ns / 128).
+// Plain iolet rules only (no interpolated walls).
+cudaError_t launch_resident_steps(const DeviceGeometry& g, bool aa, void* b0, void* b1, long long n,
+                                  int odd0, unsigned long long* bar, unsigned long long base,
+                                  cudaStream_t s);
 
 // How the pre-collision populations f(., n) are found in a buffer.
 enum GatherMode {

@@ -27,8 +27,12 @@ def hlb():
     return m
 
 
-def flags_of(hlb, scheme, store, order="morton", links="auto", lattice="d3q15"):
+def flags_of(hlb, scheme, store, order="morton", links="auto", lattice="d3q15", resident=False):
+    """resident=False: the tests' small geometries would otherwise all take the resident
+    multi-step kernel (hlb_step, include/hlb.h) instead of the one-shot step kernels the large
+    configs run; the resident kernel has its own tests below."""
     f = hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE
+    f |= 0 if resident else hlb.HLB_NO_RESIDENT
     f |= hlb.HLB_STORE_F32 if store == "f32" else hlb.HLB_STORE_F64
     f |= {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
           "tiled": hlb.HLB_ORDER_TILED}[order]
@@ -622,6 +626,84 @@ def test_graph_replay_equals_direct_launches(hlb, scheme):
     b.hlb_set_state(None, None)
     a.hlb_step(64)
     b.hlb_step(64)
+    assert np.array_equal(a.hlb_get_macroscopic()[1], b.hlb_get_macroscopic()[1])
+    a.close()
+    b.close()
+
+
+# ------------------------------------------------------------- resident multi-step kernel
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("store", ["f64", "f32"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_resident_kernel_matches_oracle(hlb, scheme, store, lattice):
+    """Small geometries run hlb_step(n >= 2) as one cooperative launch with grid barriers
+    between the steps: BASELINE configs[0] at full size and step count, and the scaled-down
+    other configs, against the oracle (even and odd step counts)."""
+    for name, small in (("pipe", False), ("cube", True), ("aneurysm", True), ("tree", True)):
+        wl = W.by_name(name, small=small)
+        for steps in (wl.steps, 7):
+            rho_ref, u_ref = (run_oracle(wl, steps, lattice=lattice) if not small
+                              else oracle_cached(name, steps, lattice))
+            g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                        flags_of(hlb, scheme, store, "raster", "auto", lattice, resident=True))
+            if wl.rho0 is not None or wl.u0 is not None:
+                g.hlb_set_state(wl.rho0, wl.u0)
+            g.hlb_step(steps)
+            assert g.hlb_steps_done() == steps and g.hlb_launch_count() == 1, (name, g.hlb_launch_count())
+            e_rho, e_u = errors(*g.hlb_get_macroscopic(), rho_ref, u_ref)
+            g.close()
+            assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, lattice, steps, e_rho, e_u)
+
+
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_resident_kernel_equals_direct_launches(hlb, scheme, lattice):
+    """Same per-site arithmetic: populations bitwise equal to the one-shot kernels launched
+    step by step, for any split of the steps into calls (odd starts, single steps in between,
+    which are launched directly), with every boundary kind on the sites (walls, density and
+    velocity iolets, iolet normals), table and record links, 64-bit offsets."""
+    wl = W.random_mask((21, 17, 19), p_fluid=0.7, n_iolets=3, p_iolet=0.06, periodic=4, tau=0.57, seed=33)
+    kind = np.array([1, 0, 0], dtype=np.uint8)
+    u = np.array([[0.004, -0.002, 0.001], [0, 0, 0], [0, 0, 0]], dtype=np.float64)
+    normals = np.array([[0, 0, 0], [0.0, 1.0, 0.0], [0, 0, 0]], dtype=np.float64)
+    for links, extra, full in (("records", 0, False), ("table", 0, True), ("auto", hlb.HLB_INDEX64, True)):
+        f = flags_of(hlb, scheme, "f64", "raster", links, lattice, resident=True) | extra
+        a = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, f)
+        b = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, f | hlb.HLB_NO_GRAPH)
+        for x in (a, b):
+            x.hlb_set_state(wl.rho0, wl.u0)
+            if full:
+                x.hlb_set_iolet_velocity(kind, u)
+                x.hlb_set_iolet_normal(normals)
+        done = 0
+        for n in (3, 1, 64, 2, 33):
+            a.hlb_step(n)
+            b.hlb_step(n)
+            done += n
+            assert a.hlb_steps_done() == b.hlb_steps_done() == done
+            assert np.array_equal(a.hlb_get_populations(), b.hlb_get_populations()), (links, n)
+        # (the resident kernels exist for 32-bit offsets only: HLB_INDEX64 steps one by one)
+        assert a.hlb_launch_count() == (done if extra & hlb.HLB_INDEX64 else 5) and b.hlb_launch_count() == done
+        a.close()
+        b.close()
+
+
+def test_resident_kernel_is_not_used_where_it_does_not_apply(hlb):
+    """Interpolated walls and waveforms keep the one-shot kernels; so does a geometry too large
+    to be resident (one launch per step), and the results stay those of the direct launches."""
+    wl = W.with_bfl_walls(W.with_velocity_inlet(W.by_name("pipe", small=True)))
+    f = flags_of(hlb, "aa", "f64", "raster", resident=True)
+    g = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f)
+    g.hlb_set_wall_distance(wl.wall_distance)
+    g.hlb_step(6)
+    assert g.hlb_launch_count() >= 6
+    g.close()
+    big = W.by_name("aneurysm")                              # 739 k sites: not resident
+    a = hlb.hlb_geometry_create(big.site_type, 0, big.tau, big.iolet_rho, f)
+    b = hlb.hlb_geometry_create(big.site_type, 0, big.tau, big.iolet_rho, f | hlb.HLB_NO_GRAPH)
+    a.hlb_step(40)
+    b.hlb_step(40)
+    assert a.hlb_launch_count() == b.hlb_launch_count() == 40
     assert np.array_equal(a.hlb_get_macroscopic()[1], b.hlb_get_macroscopic()[1])
     a.close()
     b.close()
