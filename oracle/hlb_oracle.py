@@ -96,6 +96,11 @@ def _load():
         lib.hlbd_run_all.restype = ctypes.c_int
         lib.hlbd_run_all.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 4 + \
             lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
+        lib.hlbo_set_iolet_weight.restype = None
+        lib.hlbo_set_iolet_weight.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.hlbd_run_weights.restype = ctypes.c_int
+        lib.hlbd_run_weights.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 5 + \
+            lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
         lib.hlbd_run_bfl.restype = ctypes.c_int
         lib.hlbd_run_bfl.argtypes = lib.hlbd_run.argtypes[:8] + [ctypes.c_void_p] * 3 + \
             lib.hlbd_run.argtypes[8:] + [ctypes.c_int]
@@ -178,6 +183,16 @@ class Oracle:
         assert kind.shape == (self.n_iolets,) and u.shape == (self.n_iolets, 3)
         self._lib.hlbo_set_iolet_velocity(self._h, _ptr(kind), _ptr(u))
 
+    def set_iolet_weight(self, weight):
+        """weight [N] (canonical order): factor of u_k on the velocity-iolet links of each site
+        (a velocity profile across the inlet cap); None removes it."""
+        if weight is None:
+            self._lib.hlbo_set_iolet_weight(self._h, None)
+            return
+        w = np.ascontiguousarray(np.asarray(weight, dtype=np.float64).reshape(-1))
+        assert w.shape == (self.n_sites,)
+        self._lib.hlbo_set_iolet_weight(self._h, _ptr(w))
+
     def set_iolet_normal(self, normals):
         """Normals [n_iolets, 3] of the constant-density iolets (any length; zero vector or
         None: no projection)."""
@@ -242,6 +257,8 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
         o.set_iolet_velocity(workload.iolet_kind, workload.iolet_u)
     if getattr(workload, "iolet_normal", None) is not None:
         o.set_iolet_normal(workload.iolet_normal)
+    if getattr(workload, "iolet_weight", None) is not None:
+        o.set_iolet_weight(workload.iolet_weight)
     if getattr(workload, "wall_distance", None) is not None:
         o.set_wall_distance(workload.wall_distance)
     o.step(workload.steps if steps is None else steps)
@@ -251,7 +268,8 @@ def run(workload, steps=None, variant=VARIANT_SHIFTED, threads=1, lattice="d3q15
 
 
 def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=None,
-              lattice="d3q15", iolet_kind=None, iolet_u=None, wall_d27_vox=None, iolet_normal=None):
+              lattice="d3q15", iolet_kind=None, iolet_u=None, wall_d27_vox=None, iolet_normal=None,
+              site_weight_vox=None):
     """Dense-grid twin: per-VOXEL rho [nz,ny,nx] and u [nz,ny,nx,3]."""
     lib = _load()
     st = np.ascontiguousarray(site_type, dtype=np.uint8)
@@ -270,9 +288,13 @@ def dense_run(site_type, periodic, tau, iolet_rho, steps, rho0_vox=None, u0_vox=
         assert wd.shape == (nz * ny * nx, 27)
     nio = None if iolet_normal is None else \
         np.ascontiguousarray(np.asarray(iolet_normal, dtype=np.float64).reshape(-1, 3))
-    rc = lib.hlbd_run_all(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
-                          _ptr(io), _ptr(kind), _ptr(uio), _ptr(wd), _ptr(nio), _ptr(r0), _ptr(u0),
-                          int(steps), _ptr(rho), _ptr(u), LATTICE_Q[lattice])
+    sw = None if site_weight_vox is None else \
+        np.ascontiguousarray(np.asarray(site_weight_vox, dtype=np.float64).reshape(-1))
+    if sw is not None:
+        assert sw.shape == (nz * ny * nx,)
+    rc = lib.hlbd_run_weights(_ptr(st), nx, ny, nz, int(periodic), float(tau), int(io.shape[0]),
+                              _ptr(io), _ptr(kind), _ptr(uio), _ptr(wd), _ptr(nio), _ptr(sw), _ptr(r0),
+                              _ptr(u0), int(steps), _ptr(rho), _ptr(u), LATTICE_Q[lattice])
     if rc != 0:
         raise ValueError("hlbd_run rejected its arguments")
     return rho, u

@@ -72,7 +72,7 @@ static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned p
                          int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
                          const double* iolet_u, const double* wall_d27, const double* iolet_n,
                          const double* rho0, const double* u0, int64_t steps, double* rho_out,
-                         double* u_out, int lattice_q) {
+                         double* u_out, int lattice_q, const double* site_w = nullptr) {
   if (lattice_q != 15 && lattice_q != 19) return -1;
   const Lattice& L = lattice_q == 15 ? L15 : L19;
   const int Q = L.Q;
@@ -153,7 +153,8 @@ static int hlbd_run_impl(const uint8_t* type, int nx, int ny, int nz, unsigned p
                 // returning direction opp(q) the gain is +6 w rho c_opp(q).u = -6 w rho c_q.u
                 const double cu = CX[q] * iolet_u[k * 3 + 0] + CY[q] * iolet_u[k * 3 + 1] +
                                   CZ[q] * iolet_u[k * 3 + 2];
-                g[v * Q + OPP[q]] = fstar - 6.0 * L.WT[q] * rho * cu;
+                // site_w: per-voxel weight of the prescribed velocity as seen from this voxel
+                g[v * Q + OPP[q]] = fstar - 6.0 * L.WT[q] * rho * ((site_w ? site_w[v] : 1.0) * cu);
               } else if (iolet_n && (iolet_n[k * 3] != 0.0 || iolet_n[k * 3 + 1] != 0.0 || iolet_n[k * 3 + 2] != 0.0)) {
                 // normal-projected pressure iolet: only the velocity along the unit normal
                 const double len = std::sqrt(iolet_n[k * 3] * iolet_n[k * 3] + iolet_n[k * 3 + 1] * iolet_n[k * 3 + 1] +
@@ -216,6 +217,17 @@ int hlbd_run_all(const uint8_t* type, int nx, int ny, int nz, unsigned periodic,
                  double* u_out, int lattice_q) {
   return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
                        wall_d27, iolet_n, rho0, u0, steps, rho_out, u_out, lattice_q);
+}
+
+// + site_w per VOXEL [nvox]: velocity weight omega(x) of the Ladd links of fluid voxel x
+// (NULL: 1 everywhere)
+int hlbd_run_weights(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,
+                     int n_iolets, const double* iolet_rho, const uint8_t* iolet_kind,
+                     const double* iolet_u, const double* wall_d27, const double* iolet_n,
+                     const double* site_w, const double* rho0, const double* u0, int64_t steps,
+                     double* rho_out, double* u_out, int lattice_q) {
+  return hlbd_run_impl(type, nx, ny, nz, periodic, tau, n_iolets, iolet_rho, iolet_kind, iolet_u,
+                       wall_d27, iolet_n, rho0, u0, steps, rho_out, u_out, lattice_q, site_w);
 }
 
 int hlbd_run(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, double tau,

@@ -358,6 +358,100 @@ def test_ladd_velocity_at_rest_is_plain_bounce_back():
     assert np.array_equal(ra, rb) and np.array_equal(ua, ub)
 
 
+# ------------------------------------------------------------------ velocity weights (inlet profile)
+def test_ladd_velocity_weights_special_cases():
+    """Per-site weights omega(x) scale the prescribed velocity seen from site x (PAPER.md line
+    59, USE_VELOCITY_WEIGHTS_FILE; reading R-weights): all ones is no weights, bit
+    for bit; a uniform weight a is the iolet velocity a u_k; weight 0 everywhere is a wall."""
+    wl = W.random_mask((9, 8, 7), p_fluid=0.65, n_iolets=2, p_iolet=0.1, periodic=2, seed=77)
+    kind, u = [1, 0], np.array([[0.011, -0.004, 0.006], [0.0, 0.0, 0.0]])
+    n = int(wl.n_sites)
+
+    def run(weight, uk=u, st=wl.site_type, rho_io=wl.iolet_rho, kinds=kind):
+        o = oracle.Oracle(st, 2, wl.tau, rho_io)
+        o.set_state(wl.rho0, wl.u0)
+        if kinds is not None:
+            o.set_iolet_velocity(kinds, uk)
+        o.set_iolet_weight(weight)
+        o.step(15)
+        return o.get_macroscopic()
+
+    r0, u0 = run(None)
+    r1, u1 = run(np.ones(n))
+    assert np.array_equal(r0, r1) and np.array_equal(u0, u1)
+    ra, ua = run(np.full(n, 0.37))
+    rb, ub = run(None, uk=0.37 * u)
+    assert np.max(np.abs(ra - rb)) < 1e-15 and np.max(np.abs(ua - ub)) < 1e-15
+    assert np.max(np.abs(ua - u0)) > 1e-6                             # and it does matter
+    rz, uz = run(np.zeros(n))                                         # boundary at rest = bounce-back
+    rw, uw = run(None, uk=np.zeros((2, 3)))
+    assert np.array_equal(rz, rw) and np.array_equal(uz, uw)
+
+
+def test_ladd_velocity_weights_inject_the_weighted_mass_per_site(lattice):
+    """One step from rest (rho = 1, u = 0, so f* = w): a site gains exactly
+    sum over its velocity-iolet links q of 6 w_q omega(x) c_q.u_k, and nothing else moves mass.
+    Evaluated voxel by voxel from the site types: pins which site's weight multiplies which
+    link, the factor and the sign."""
+    wl = W.random_mask((10, 9, 8), p_fluid=0.6, n_iolets=2, p_iolet=0.12, seed=5)
+    st = wl.site_type
+    nz, ny, nx = st.shape
+    uk = np.array([[0.013, 0.007, -0.009], [-0.004, 0.01, 0.002]])
+    rng = np.random.default_rng(3)
+    om = rng.uniform(0.0, 2.0, int(wl.n_sites))
+    o = oracle.Oracle(st, 0, 0.9, [1.0, 1.0])
+    o.set_iolet_velocity([1, 1], uk)
+    o.set_iolet_weight(om)
+    o.step(1)
+    rho, _ = o.get_macroscopic()
+    c, w = C, WT                                                      # the lattice under test
+    expect = np.zeros(int(wl.n_sites))
+    for i, (x, y, z) in enumerate(zip(*canon_coords(st))):
+        for q in range(len(w)):
+            sx, sy, sz = x - c[q][0], y - c[q][1], z - c[q][2]
+            if 0 <= sx < nx and 0 <= sy < ny and 0 <= sz < nz and st[sz, sy, sx] >= 2:
+                k = int(st[sz, sy, sx]) - 2
+                expect[i] += 6.0 * w[q] * om[i] * float(np.dot(c[q], uk[k]))
+    assert np.max(np.abs(expect)) > 1e-3
+    assert np.max(np.abs((rho - 1.0) - expect)) < 1e-15
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_ladd_velocity_weights_dense_twin(seed):
+    """The dense push implementation carries the weights per voxel, independently."""
+    wl = W.random_mask((8, 9, 7), p_fluid=0.65, n_iolets=3, p_iolet=0.09, periodic=seed, seed=700 + seed)
+    st, vox = wl.site_type, wl.fluid_voxels()
+    rng = np.random.default_rng(seed)
+    kind, uio = np.array([1, 0, 1], dtype=np.uint8), 0.02 * (rng.random((3, 3)) - 0.5)
+    om = rng.uniform(0.0, 2.0, len(vox))
+    om_vox = np.zeros(st.size)
+    om_vox[vox] = om
+    rho0v, u0v = np.ones(st.size), np.zeros((st.size, 3))
+    rho0v[vox], u0v[vox] = wl.rho0, wl.u0
+    rd, ud = oracle.dense_run(st, seed, wl.tau, wl.iolet_rho, 11, rho0v, u0v, iolet_kind=kind, iolet_u=uio,
+                              site_weight_vox=om_vox)
+    o = oracle.Oracle(st, seed, wl.tau, wl.iolet_rho, variant=oracle.VARIANT_RAW)
+    o.set_state(wl.rho0, wl.u0)
+    o.set_iolet_velocity(kind, uio)
+    o.set_iolet_weight(om)
+    o.step(11)
+    r, u = o.get_macroscopic()
+    assert np.max(np.abs(r - rd.reshape(-1)[vox])) < 5e-15
+    assert np.max(np.abs(u - ud.reshape(-1, 3)[vox])) < 5e-15
+    o.set_iolet_weight(None)                                           # and the weights are not a no-op
+    o.set_state(wl.rho0, wl.u0)
+    o.step(11)
+    assert np.max(np.abs(o.get_macroscopic()[1] - u)) > 1e-7
+
+
+def test_inlet_profile_weights_average_to_one_and_vanish_at_the_rim():
+    wl = W.with_inlet_profile(W.with_velocity_inlet(W.by_name("pipe")))
+    w = wl.iolet_weight
+    first = np.flatnonzero(w != 1.0)
+    assert len(first) == 197                                           # the first slice of the pipe
+    assert abs(w[first].mean() - 1.0) < 1e-12 and 1.7 < w[first].max() < 2.0 and 0.0 < w[first].min() < 0.25
+
+
 # ------------------------------------------------------------------ normal-projected iolets
 def test_iolet_normal_projection_special_cases():
     """(a) no normal, or a zero normal: unchanged bit for bit; (b) a flow that is exactly

@@ -15,6 +15,7 @@ from .geometries import (  # noqa: F401
     by_name,
     with_velocity_inlet,
     pulsatile_waveform,
+    with_inlet_profile,
     with_bfl_walls,
     wall_distance_by_bisection,
     CONFIG_NAMES,

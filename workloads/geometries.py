@@ -42,6 +42,8 @@ class Workload:
     iolet_kind: Optional[np.ndarray] = None  # uint8 (n_iolets,): 0 density, 1 Ladd velocity; None => all 0
     iolet_u: Optional[np.ndarray] = None     # float64 (n_iolets, 3) velocities of the velocity iolets
     iolet_normal: Optional[np.ndarray] = None  # float64 (n_iolets, 3): normals of density iolets
+    iolet_weight: Optional[np.ndarray] = None  # float64 (N,), canonical order: factor of u_k on the
+                                               # velocity-iolet links of each site; None => 1
     wall_distance: Optional[np.ndarray] = None  # float64 (N, 27): BFL wall distances (include/hlb.h)
     scheme: str = "two_lattice"      # "two_lattice" | "aa"  (what the config asks for)
     store: str = "f64"               # "f64" | "f32"
@@ -351,6 +353,37 @@ def with_velocity_inlet(wl: Workload, u_in: float = 0.004) -> Workload:
     kind[0] = 1
     u[0, 2 if wl.name == "pipe" else 0] = u_in
     return dataclasses.replace(wl, iolet_kind=kind, iolet_u=u, name=wl.name)
+
+
+def with_inlet_profile(wl: Workload) -> Workload:
+    """Per-site velocity weights for iolet 0 (the paper's USE_VELOCITY_WEIGHTS_FILE build flag,
+    PAPER.md line 59; the file itself is not in the paper): a parabolic profile across the inlet
+    cap, omega proportional to 1 - r^2 / R^2 and scaled to mean 1 over the cap (so the mean inlet
+    velocity stays u_k), r measured from the centroid of the fluid sites that touch a ghost
+    voxel of iolet 0 and R = their largest distance + 1/2. Sites
+    that do not touch the inlet keep weight 1 (they have no velocity link to weigh)."""
+    st = wl.site_type
+    nz, ny, nx = st.shape
+    v = wl.fluid_voxels()
+    x, y, z = v % nx, (v // nx) % ny, v // (nx * ny)
+    touch = np.zeros(len(v), dtype=bool)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                xs, ys, zs = x + dx, y + dy, z + dz
+                ok = (xs >= 0) & (xs < nx) & (ys >= 0) & (ys < ny) & (zs >= 0) & (zs < nz)
+                hit = np.zeros(len(v), dtype=bool)
+                hit[ok] = st[zs[ok], ys[ok], xs[ok]] == IOLET0
+                touch |= hit
+    w = np.ones(len(v), dtype=np.float64)
+    if touch.any():
+        p = np.stack([x[touch], y[touch], z[touch]], axis=1).astype(np.float64)
+        c = p.mean(axis=0)
+        r = np.linalg.norm(p - c, axis=1)
+        R = r.max() + 0.5
+        prof = 1.0 - (r / R) ** 2
+        w[touch] = prof / prof.mean()
+    return dataclasses.replace(wl, iolet_weight=w)
 
 
 def pulsatile_waveform(wl: Workload, n_t: int, u_peak: float = 0.006, u_base: float = 0.002,
