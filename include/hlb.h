@@ -161,6 +161,18 @@ int64_t hlb_num_bfl_sites(const hlb_geometry* g);
  * hlb_step(n) / hlb_set_iolet_velocity(...) in turn. Errors: HLB_EINVAL. */
 int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u);
 
+/* Per-site velocity weights of the velocity iolets -- a velocity profile across the inlet
+ * cap (the paper's build flag USE_VELOCITY_WEIGHTS_FILE; the file itself is
+ * not in the paper): as seen from site x the boundary of a velocity iolet k moves with
+ * omega(x) u_k,
+ *     f_q(x,t+1) = f*_opp(q)(x,t) + 6 w_q rho(x,t) omega(x) c_q.u_k   (reading R-weights)
+ * for every link q of x whose source voxel is a ghost voxel of a kind-1 iolet (with or without
+ * a waveform). weight: HOST [N] in canonical site order, copied during the call (entries of
+ * sites without such a link are ignored); NULL removes the weights (omega = 1). Takes effect
+ * from the next step. Synchronises the stream. Errors: HLB_EINVAL (non-finite weight),
+ * HLB_ENOMEM, HLB_ECUDA. */
+int hlb_set_iolet_weight(hlb_geometry* g, const double* weight);
+
 /* Device-resident velocity waveform for the velocity iolets (the paper drives its inlet from
  * a velocity file, Table I "inlet velocity" and line 126 Fig. 8): with a
  * waveform the step that advances the state from time t to t+1 (t = hlb_steps_done() before

@@ -82,6 +82,7 @@ def _load() -> ctypes.CDLL:
         "hlb_set_iolet_density": (c_int, [vp, vp]),
         "hlb_set_iolet_velocity": (c_int, [vp, vp, vp]),
         "hlb_set_iolet_waveform": (c_int, [vp, vp, i64]),
+        "hlb_set_iolet_weight": (c_int, [vp, vp]),
         "hlb_set_iolet_normal": (c_int, [vp, vp]),
         "hlb_set_wall_distance": (c_int, [vp, vp]),
         "hlb_num_bfl_sites": (i64, [vp]),
@@ -124,7 +125,7 @@ def _load() -> ctypes.CDLL:
 LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
-            "hlb_set_iolet_velocity", "hlb_set_iolet_waveform", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
+            "hlb_set_iolet_velocity", "hlb_set_iolet_waveform", "hlb_set_iolet_weight", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
@@ -278,6 +279,11 @@ class Geometry:
         kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8)
         u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64)
         _check(_lib.hlb_set_iolet_velocity(self._h, _ptr(kind), _ptr(u)))
+
+    def hlb_set_iolet_weight(self, weight):
+        w = None if weight is None else _host(np.asarray(weight, dtype=np.float64).reshape(-1),
+                                              np.float64, (self.n_sites,))
+        _check(_lib.hlb_set_iolet_weight(self._h, _ptr(w)))
 
     def hlb_set_iolet_waveform(self, u):
         """u: [n_t][n_iolets][3] (or None to remove the waveform)."""

@@ -70,6 +70,7 @@ struct hlb_geometry {
   int64_t wave_nt = 0;
   double* d_wave = nullptr;
   size_t wave_cap = 0;                // doubles d_wave can hold
+  double* d_iolet_w = nullptr;        // [Ns] velocity weights, internal order (hlb_set_iolet_weight)
   DeviceGeometry dg;
   void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
   int cur = 0;                        // two-lattice: buffer the next step reads
@@ -479,7 +480,9 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   if (!d27) {
     g->bfl_set = false;
     g->dg.bfl = BflLinks();
+    const double* keep_w = g->dg.bflf.iolet_w;  // the velocity weights travel in the same argument
     g->dg.bflf = BflFused();
+    g->dg.bflf.iolet_w = keep_w;
     g->dg.bfl_on = false;
     return HLB_OK;
   }
@@ -606,6 +609,34 @@ int hlb_set_iolet_velocity(hlb_geometry* g, const uint8_t* kind, const double* u
     for (int a = 0; a < 3; ++a) g->iolet_u[(size_t)k * 3 + a] = u ? u[k * 3 + a] : 0.0;
   }
   return upload_iolets(g);
+}
+
+int hlb_set_iolet_weight(hlb_geometry* g, const double* weight) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (!weight) {
+    if (g->dg.bflf.iolet_w) g->drop_graph();  // captured launches carry the pointer
+    g->dg.bflf.iolet_w = nullptr;
+    return HLB_OK;
+  }
+  const size_t N = (size_t)g->N, Ns = (size_t)g->Ns;
+  for (size_t c = 0; c < N; ++c)
+    if (!std::isfinite(weight[c])) return fail(HLB_EINVAL, "non-finite velocity weight");
+  if (!g->d_iolet_w) {
+    void* ptr = nullptr;
+    const int rc = g->alloc(sizeof(double) * Ns, &ptr);
+    if (rc) return rc;
+    g->d_iolet_w = (double*)ptr;
+  }
+  // canonical -> internal order (the ranks live on the device only: fetch them)
+  std::vector<int32_t> canon(N);
+  HLB_CUDA(cudaStreamSynchronize(g->stream));
+  HLB_CUDA(cudaMemcpy(canon.data(), g->dg.canon, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
+  std::vector<double> w(Ns, 1.0);
+  for (size_t i = 0; i < N; ++i) w[i] = weight[(size_t)canon[i]];
+  HLB_CUDA(cudaMemcpy(g->d_iolet_w, w.data(), sizeof(double) * Ns, cudaMemcpyHostToDevice));
+  if (g->dg.bflf.iolet_w != g->d_iolet_w) g->drop_graph();
+  g->dg.bflf.iolet_w = g->d_iolet_w;
+  return HLB_OK;
 }
 
 int hlb_set_iolet_waveform(hlb_geometry* g, const double* u, int64_t n_t) {

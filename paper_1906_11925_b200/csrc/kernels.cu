@@ -158,6 +158,8 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 //   constant-density iolet k: by the equilibrium f_eq_p(rho_k, u(x, t))           (reading A6)
 //                             (u replaced by (u.n_k) n_k when a normal n_k is given)
 //   velocity iolet k (Ladd):  by h*_opp(p) + 6 w_p rho(x, t) c_p.u_k             (reading R-ladd)
+//                             (u_k scaled by the site's weight omega(x) when iolet_w is given,
+//                              reading R-weights)
 // The table entries are re-read here so that the common path does not keep them in
 // registers; fully unrolled so that out[] stays in registers (no call, no stack).
 // FULL = false is the lean instantiation for geometries whose iolets are all plain
@@ -168,6 +170,7 @@ template <typename L, bool FULL>
 __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
                                                  long long i, const Moments& m,
                                                  const double* __restrict__ iolet_par,
+                                                 const double* __restrict__ iolet_w,
                                                  double (&out)[L::Q]) {
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) {
@@ -188,7 +191,8 @@ __device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr
           out[p] = heq_of<L>(p, rk - 1.0, rk, m.ux, m.uy, m.uz);
         }
       } else {
-        const double cu = c_dot_u<L>(p, __ldg(par + 1), __ldg(par + 2), __ldg(par + 3));
+        double cu = c_dot_u<L>(p, __ldg(par + 1), __ldg(par + 2), __ldg(par + 3));
+        if (iolet_w) cu = mul(__ldg(iolet_w + i), cu);  // velocity profile across the cap
         out[p] = fma_(mul(6.0 * L::weight(p), m.rho), cu, out[p]);
       }
     }
@@ -401,7 +405,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, back);
+    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, bf.iolet_w, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
@@ -443,7 +447,7 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
   if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, bf.iolet_w, out);
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
@@ -483,7 +487,7 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
   if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, out);
+  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, bf.iolet_w, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
@@ -525,7 +529,8 @@ constexpr int RESIDENT_MINB = 4;
 // One site update of the resident kernels (the bodies of k_aa_even / k_aa_odd and k_pull).
 template <typename L, typename ST, typename IT, int V>
 __device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
-                                        const double* __restrict__ iolet_par, long long Ns,
+                                        const double* __restrict__ iolet_par,
+                                        const double* __restrict__ iolet_w, long long Ns,
                                         double omega, long long i, const IT (&off)[L::Q - 1],
                                         bool iolet, bool odd) {
   double h[L::Q];
@@ -542,7 +547,7 @@ __device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (iolet) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, out);
+  if (iolet) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, iolet_w, out);
   a[i] = to_store<ST>(out[0]);
   if (odd) {
 #pragma unroll
@@ -554,7 +559,8 @@ __device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
 }
 template <typename L, typename ST, typename IT, int V>
 __device__ __forceinline__ void pull_site(const ST* src, ST* dst, const int32_t* __restrict__ nbr,
-                                          const double* __restrict__ iolet_par, long long Ns,
+                                          const double* __restrict__ iolet_par,
+                                          const double* __restrict__ iolet_w, long long Ns,
                                           double omega, long long i, const IT (&off)[L::Q - 1],
                                           bool iolet) {
   double h[L::Q];
@@ -567,7 +573,7 @@ __device__ __forceinline__ void pull_site(const ST* src, ST* dst, const int32_t*
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, back);
+    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, iolet_w, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
@@ -579,7 +585,7 @@ template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
 k_aa_resident(ST* a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
               const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-              long long Ns, double omega, long long n_steps, int odd0, unsigned long long* bar,
+              const double* __restrict__ iolet_w, long long Ns, double omega, long long n_steps, int odd0, unsigned long long* bar,
               unsigned long long bar_base) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
@@ -587,7 +593,7 @@ k_aa_resident(ST* a, const int32_t* __restrict__ nbr, const uint4* __restrict__ 
   const bool iolet = has_iolet_link(iolet_bits, i);
   bool odd = odd0 != 0;
   for (long long s = 0; s < n_steps; ++s) {
-    aa_site<L, ST, IT, V>(a, nbr, iolet_par, Ns, omega, i, off, iolet, odd);
+    aa_site<L, ST, IT, V>(a, nbr, iolet_par, iolet_w, Ns, omega, i, off, iolet, odd);
     odd = !odd;
     if (s + 1 < n_steps) grid_barrier(bar, bar_base + (unsigned long long)(s + 1) * gridDim.x);
   }
@@ -597,7 +603,7 @@ template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
 k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
                 const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-                long long Ns, double omega, long long n_steps, unsigned long long* bar,
+                const double* __restrict__ iolet_w, long long Ns, double omega, long long n_steps, unsigned long long* bar,
                 unsigned long long bar_base) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
@@ -606,7 +612,7 @@ k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __
   const ST* src = b0;
   ST* dst = b1;
   for (long long s = 0; s < n_steps; ++s) {
-    pull_site<L, ST, IT, V>(src, dst, nbr, iolet_par, Ns, omega, i, off, iolet);
+    pull_site<L, ST, IT, V>(src, dst, nbr, iolet_par, iolet_w, Ns, omega, i, off, iolet);
     ST* t = const_cast<ST*>(src);
     src = dst;
     dst = t;
@@ -907,14 +913,14 @@ static cudaError_t resident_launch(const DeviceGeometry& g, bool aa, void* b0, v
                                    cudaStream_t s) {
   using IT = uint32_t;
   if (aa) {
-#define HLB_RES_ARGS s, (ST*)b0, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, \
-                     g.omega, n, odd0, bar, base
+#define HLB_RES_ARGS s, (ST*)b0, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.bflf.iolet_w, \
+                     (long long)g.Ns, g.omega, n, odd0, bar, base
     return g.iolet_full ? launch_resident(g, k_aa_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS)
                         : launch_resident(g, k_aa_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
 #undef HLB_RES_ARGS
   }
 #define HLB_RES_ARGS s, (ST*)b0, (ST*)b1, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, \
-                     (long long)g.Ns, g.omega, n, bar, base
+                     g.bflf.iolet_w, (long long)g.Ns, g.omega, n, bar, base
   return g.iolet_full ? launch_resident(g, k_pull_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS)
                       : launch_resident(g, k_pull_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
 #undef HLB_RES_ARGS

@@ -32,6 +32,10 @@ struct BflFused {
   const double* coef = nullptr;    // [nf][row]
   long long nf = 0;
   int gather = 0;
+  // The other per-site option that travels in this by-value argument: velocity weights of the
+  // Ladd iolets (hlb_set_iolet_weight), [Ns] in internal site order, read on the rare iolet
+  // path only; NULL = no weights.
+  const double* iolet_w = nullptr;
 };
 
 struct DeviceGeometry {

@@ -60,6 +60,8 @@ def run_gpu(hlb, wl, steps, scheme, store, order="morton", links="auto", lattice
         g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
     if wl.iolet_normal is not None:
         g.hlb_set_iolet_normal(wl.iolet_normal)
+    if wl.iolet_weight is not None:
+        g.hlb_set_iolet_weight(wl.iolet_weight)
     if wl.wall_distance is not None:
         g.hlb_set_wall_distance(wl.wall_distance)
         assert g.hlb_num_bfl_sites() > 0
@@ -281,12 +283,69 @@ def test_time_varying_velocity_inlet_and_mixed_kinds(hlb, scheme):
     g.close()
 
 
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_velocity_inlet_with_profile_matches_oracle(hlb, scheme, lattice):
+    """Per-site velocity weights (the paper's USE_VELOCITY_WEIGHTS_FILE flag):
+    a parabolic profile across the inlet cap, in every site order (the weights cross the
+    boundary in canonical order), both storage types, even and odd step counts; also through
+    the resident multi-step kernel, and random weights on random masks with mixed iolet kinds."""
+    for name in ("pipe", "aneurysm", "tree"):
+        wl = W.with_inlet_profile(W.with_velocity_inlet(W.by_name(name, small=True)))
+        for steps, store, order, links in ((wl.steps, "f64", "raster", "records"),
+                                           (wl.steps + 1, "f64", "morton", "table"),
+                                           (wl.steps + 1, "f32", "tiled", "auto")):
+            rho_ref, u_ref = run_oracle(wl, steps, lattice=lattice)
+            rho, u = run_gpu(hlb, wl, steps, scheme, store, order, links, lattice)
+            e_rho, e_u = errors(rho, u, rho_ref, u_ref)
+            assert e_rho < TOL[store] and e_u < TOL[store], (name, scheme, store, steps, e_rho, e_u)
+        plain = run_oracle(W.with_velocity_inlet(W.by_name(name, small=True)), wl.steps, lattice=lattice)
+        assert np.max(np.abs(plain[1] - run_oracle(wl, wl.steps, lattice=lattice)[1])) > 1e-6  # it matters
+        g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                    flags_of(hlb, scheme, "f64", "raster", "auto", lattice, resident=True))
+        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+        g.hlb_set_iolet_weight(wl.iolet_weight)
+        g.hlb_step(wl.steps)
+        assert g.hlb_launch_count() == 1
+        e_rho, e_u = errors(*g.hlb_get_macroscopic(), *run_oracle(wl, wl.steps, lattice=lattice))
+        g.close()
+        assert e_rho < 1e-12 and e_u < 1e-12, (name, "resident", e_rho, e_u)
+    wl = W.random_mask((13, 12, 11), p_fluid=0.65, n_iolets=3, p_iolet=0.08, periodic=1, tau=0.6, seed=123)
+    rng = np.random.default_rng(9)
+    kind, uio = np.array([1, 0, 1], dtype=np.uint8), 0.02 * (rng.random((3, 3)) - 0.5)
+    om = rng.uniform(0.0, 2.0, int(wl.n_sites))
+    o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, lattice=lattice)
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, scheme, "f64", "morton", "auto", lattice))
+    for x in (o, g):
+        (x.set_state if x is o else x.hlb_set_state)(wl.rho0, wl.u0)
+    o.set_iolet_velocity(kind, uio)
+    o.set_iolet_weight(om)
+    g.hlb_set_iolet_velocity(kind, uio)
+    g.hlb_set_iolet_weight(om)
+    o.step(9)
+    g.hlb_step(9)
+    e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())
+    assert e_rho < 1e-13 and e_u < 1e-12
+    g.hlb_set_iolet_weight(None)                             # removed: omega = 1 again
+    o.set_iolet_weight(None)
+    o.step(6)
+    g.hlb_step(6)
+    e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())
+    assert e_rho < 1e-13 and e_u < 1e-12
+    with pytest.raises(hlb.HlbError):
+        g.hlb_set_iolet_weight(np.full(int(wl.n_sites), np.inf))
+    g.close()
+
+
 def _oracle_with_waveform(wl, wave, steps, lattice):
     """The definition the waveform must reproduce: the oracle stepped one time level at a time,
     its velocity iolets set to u[t mod n_t] before the step from t to t+1."""
     o = oracle.Oracle(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, lattice=lattice)
     if wl.rho0 is not None or wl.u0 is not None:
         o.set_state(wl.rho0, wl.u0)
+    if wl.iolet_weight is not None:
+        o.set_iolet_weight(wl.iolet_weight)
     for t in range(steps):
         o.set_iolet_velocity(wl.iolet_kind, wave[t % len(wave)])
         o.step(1)
@@ -305,12 +364,16 @@ def test_inlet_waveform_matches_per_step_oracle(hlb, scheme, lattice):
     for name, store, n_t, steps in (("pipe", "f64", 7, 71), ("aneurysm", "f64", 5, 18),
                                     ("tree", "f32", 9, 23)):
         wl = W.with_velocity_inlet(W.by_name(name, small=True))
+        if name == "aneurysm":                                # waveform x inlet profile
+            wl = W.with_inlet_profile(wl)
         wave = W.pulsatile_waveform(wl, n_t)
         rho_ref, u_ref = _oracle_with_waveform(wl, wave, steps, lattice)
         g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
                                     flags_of(hlb, scheme, store, "raster", "auto", lattice))
         g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
         g.hlb_set_iolet_waveform(wave)
+        if wl.iolet_weight is not None:
+            g.hlb_set_iolet_weight(wl.iolet_weight)
         launches0 = g.hlb_launch_count()
         g.hlb_step(n_t + 1)
         g.hlb_get_macroscopic()                               # a read-out in mid-period
