@@ -88,6 +88,25 @@ __device__ __forceinline__ void load_entries(const int32_t* __restrict__ nbr, lo
 // (include/hlb.h, hlb_preprocess_records): entry = (lane >= second ? off1 : off0) + lane;
 // a sentinel record (warp-uniform) sends the warp to the table for that link. The iolet id
 // is NOT decoded here; the rare iolet path re-reads the table.
+// -DHLB_BOUNDS_CHECK (debug builds only; compute-sanitizer is not available on every box):
+// every flat offset a step kernel is about to gather from / scatter to must lie inside the
+// Q * Ns elements of a population array, else the kernel traps and the next CUDA call fails.
+// (-DHLB_BOUNDS_SELFTEST=1 shrinks the limit by one plane so that legitimate accesses trap:
+// the negative control that shows the check is live.)
+#ifndef HLB_BOUNDS_SELFTEST
+#define HLB_BOUNDS_SELFTEST 0
+#endif
+template <typename L, typename IT>
+__device__ __forceinline__ void check_offsets(const IT (&off)[L::Q - 1], long long Ns) {
+#ifdef HLB_BOUNDS_CHECK
+#pragma unroll
+  for (int q = 1; q < L::Q; ++q)
+    if ((unsigned long long)off[q - 1] >= (unsigned long long)(L::Q - HLB_BOUNDS_SELFTEST) * (unsigned long long)Ns) __trap();
+#else
+  (void)off; (void)Ns;
+#endif
+}
+
 template <typename L, int MODE, bool REC, typename IT>
 __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
                                              const uint4* __restrict__ rec, long long Ns,
@@ -102,6 +121,7 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
       const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
       off[q - 1] = e[q - 1] < 0 ? (IT)qw * n + self : (IT)qf * n + (IT)e[q - 1];
     }
+    check_offsets<L, IT>(off, Ns);
     return;
   }
   const uint32_t lane = threadIdx.x & 31u;
@@ -140,12 +160,16 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
       off[q - 1] = wall ? (IT)qw * n + self : (IT)qf * n + (IT)e;
     }
   }
+  check_offsets<L, IT>(off, Ns);
 }
 
 // Address (element offset) where the pre-collision f_q(x) of link q lives.
 template <int MODE>
 __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, long long i) {
   if (MODE == GATHER_OWN) return (long long)q * Ns + i;
+#ifdef HLB_BOUNDS_CHECK
+  if (e >= Ns) __trap();
+#endif
   const bool wall = e < 0;
   if (MODE == GATHER_PULL)  // post-collision buffer: wall -> own opposite slot
     return wall ? (long long)opp(q) * Ns + i : (long long)q * Ns + e;
