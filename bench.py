@@ -87,6 +87,9 @@ def parse_args():
                     help="HLB_NO_RESIDENT (ablation: small geometries step by graph replay instead "
                          "of the resident multi-step kernel)")
     ap.add_argument("--inner", type=int, default=50, help="LB time steps per bench step (even)")
+    ap.add_argument("--sweep", default="auto", choices=["auto", "on", "off"],
+                    help="after the headline, time the other configs / variants shortly and attach "
+                         "them as \"configs\" (auto: with the default workload and flags at 1 GPU)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="scaled-down geometry (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -107,24 +110,6 @@ def measured_peak():
         return v, "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-
-
-def committed_traffic(workload, scheme, store, kernel):
-    """dram bytes per launch from the committed ncu --set full capture (profiles/traffic.csv:
-    workload,scheme,store,kernel,n_sites,dram_bytes_per_launch,source), or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.csv")
-    if not os.path.exists(path):
-        return None
-    for line in open(path):
-        if line.startswith("#") or not line.strip():
-            continue
-        parts = [p.strip() for p in line.split(",")]
-        if parts[:4] == [workload, scheme, store, kernel]:
-            try:
-                return float(parts[5])
-            except (ValueError, IndexError):
-                return None
-    return None
 
 
 class ClockSampler:
@@ -330,6 +315,241 @@ def run_reference(args, rank, world):
 
 
 # --------------------------------------------------------------------------- our arm
+def variant_flags(hlb, v):
+    return (hlb.HLB_AA if v["scheme"] == "aa" else hlb.HLB_TWO_LATTICE) | \
+        (hlb.HLB_STORE_F32 if v["store"] == "f32" else hlb.HLB_STORE_F64) | \
+        {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
+         "tiled": hlb.HLB_ORDER_TILED}[v["order"]] | \
+        {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
+         "records": hlb.HLB_LINKS_RECORDS}[v["links"]] | \
+        (0 if v["prefetch"] else hlb.HLB_NO_PREFETCH) | (0 if v["pdl"] else hlb.HLB_NO_PDL) | \
+        (0 if v["resident"] else hlb.HLB_NO_RESIDENT) | \
+        (hlb.HLB_LATTICE_D3Q19 if v["lattice"] == "d3q19" else hlb.HLB_LATTICE_D3Q15)
+
+
+def default_variant(**kw):
+    v = {"scheme": "two_lattice", "store": "f64", "lattice": "d3q15", "order": "auto", "links": "auto",
+         "prefetch": True, "pdl": True, "resident": True, "inlet": "pressure", "walls": "bounce_back"}
+    v.update(kw)
+    return v
+
+
+class Run:
+    """One geometry on the device in one variant, with the timing helpers of a bench line."""
+
+    def __init__(self, hlb, W, wl, name, v, world=1, local_rank=0):
+        import torch
+        self.torch, self.hlb, self.W, self.name, self.v = torch, hlb, W, name, v
+        self.world, self.local_rank = world, local_rank
+        t0 = time.perf_counter()
+        self.g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, variant_flags(hlb, v))
+        torch.cuda.synchronize()
+        self.t_create = time.perf_counter() - t0
+        g = self.g
+        self.N, self.nq = g.n_sites, g.hlb_num_q()
+        if wl.rho0 is not None or wl.u0 is not None:
+            g.hlb_set_state(wl.rho0, wl.u0)
+        self.wave = None
+        if v["inlet"] != "pressure" and wl.n_iolets > 0:
+            wl = W.with_velocity_inlet(wl)
+            g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
+            if v["inlet"] in ("waveform", "host_waveform"):
+                self.wave = W.pulsatile_waveform(wl, 1000)
+                if v["inlet"] == "waveform":
+                    g.hlb_set_iolet_waveform(self.wave)
+        if v["walls"] == "bfl_random":
+            d27 = np.random.default_rng(1906).uniform(0.05, 1.0, size=(self.N, 27))
+            g.hlb_set_wall_distance(d27)
+            del d27
+        self.wl = wl
+        self.stream = torch.cuda.current_stream()
+
+    def advance(self, n):
+        g = self.g
+        if self.v["inlet"] == "host_waveform" and self.wave is not None:
+            for _ in range(n):       # the time-varying inlet without the device-resident table
+                g.hlb_set_iolet_velocity(self.wl.iolet_kind, self.wave[g.hlb_steps_done() % len(self.wave)])
+                g.hlb_step(1)
+        else:
+            g.hlb_step(n)
+
+    def barrier(self):
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def timed(self, S, K, warmup):
+        """K x hlb_step(S) between CUDA events on the launching stream, clocks sampled during it.
+        Returns (milliseconds of the K steps, launches inside them, clocks)."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.advance(S)
+        self.barrier()
+        sampler = ClockSampler(self.local_rank)
+        sampler.start()
+        time.sleep(0.25)
+        l0 = self.g.hlb_launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        self.barrier()
+        w0 = time.time()
+        ev0.record(self.stream)
+        for _ in range(K):
+            self.advance(S)
+        ev1.record(self.stream)
+        self.barrier()
+        w1 = time.time()
+        clocks = sampler.stop(w0, w1)
+        return ev0.elapsed_time(ev1), self.g.hlb_launch_count() - l0, clocks
+
+    def kernel_times(self, reps, S, timed_ms, K, launches):
+        """Average duration of every step kernel (events around single launches on the same
+        stream) with its bytes per site in both models; the resident multi-step kernel is one
+        launch per hlb_step(S), so its duration is the timed region's own."""
+        torch, g, v, nq = self.torch, self.g, self.v, self.nq
+        scheme, store = v["scheme"], v["store"]
+        rec, sf = bool(g.hlb_uses_records()), g.hlb_record_sentinel_fraction()
+        moved = lambda phase: self.hlb.moved_bytes_per_site(scheme, store, nq, rec, sf, phase)  # noqa: E731
+        pop_bytes = nq * 2 * (4 if store == "f32" else 8)
+        if launches < S * K:
+            name = "k_aa_resident" if scheme == "aa" else "k_pull_resident"
+            return {name: {"ms": timed_ms / K, "steps_per_launch": S,
+                           "bytes_per_site": S * self.hlb.algorithmic_bytes_per_site(scheme, store, nq),
+                           "moved_bytes_per_site": S * moved("step")}}
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+               for _ in range(2 * reps)]
+        torch.cuda.synchronize()
+        parity0 = g.hlb_steps_done() & 1
+        for a, b in evs:
+            a.record(self.stream)
+            g.hlb_step(1)
+            b.record(self.stream)
+        torch.cuda.synchronize()
+        per = np.array([a.elapsed_time(b) for a, b in evs])
+        if scheme == "aa":
+            phase = (parity0 + np.arange(per.size)) & 1          # 0: even-phase kernel, 1: odd-phase
+            return {"k_aa<even>": {"ms": float(np.mean(per[phase == 0])), "bytes_per_site": pop_bytes,
+                                   "moved_bytes_per_site": moved("even")},
+                    "k_aa<odd>": {"ms": float(np.mean(per[phase == 1])), "bytes_per_site": pop_bytes + 4 * (nq - 1),
+                                  "moved_bytes_per_site": moved("odd")}}
+        return {"k_pull": {"ms": float(np.mean(per)), "bytes_per_site": pop_bytes + 4 * (nq - 1),
+                           "moved_bytes_per_site": moved("step")}}
+
+    def close(self):
+        self.g.close()
+
+
+def traffic_key(name, v, nq):
+    return [name + ("_d3q19" if nq == 19 else ""), v["scheme"], v["store"], v["order"], v["links"],
+            "prefetch" if v["prefetch"] else "no_prefetch", v["inlet"], v["walls"]]
+
+
+def committed_traffic(name, v, nq, kernel):
+    """dram bytes per launch from the committed ncu --set full capture of EXACTLY this
+    configuration (profiles/traffic.csv: workload,scheme,store,order,links,prefetch,inlet,walls,
+    kernel,n_sites,dram_bytes_per_launch,source), else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    key = traffic_key(name, v, nq) + [kernel]
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        parts = [p.strip() for p in line.split(",")]
+        if parts[:9] == key:
+            try:
+                return float(parts[10])
+            except (ValueError, IndexError):
+                return None
+    return None
+
+
+def roofline_of(run, kernels, name):
+    """The roofline object of the dominant kernel. `achieved` is ALGORITHMIC bytes (SURVEY.md
+    section 8(d): Q populations read + written + the int32 table) over the measured launch
+    duration -- with link records the kernels read less than that model charges, so it can
+    exceed the copy peak; `frac_moved_model` uses the bytes the variant really has to move and
+    `frac_traffic` the DRAM bytes ncu counted for exactly this configuration (None if that was
+    not captured)."""
+    peak, peak_src = measured_peak()
+    dom = max(kernels, key=lambda k: kernels[k]["ms"])
+    k = kernels[dom]
+    sec = k["ms"] * 1e-3
+    N = run.N
+    achieved = k["bytes_per_site"] * N / sec / 1e9
+    moved = k["moved_bytes_per_site"] * N / sec / 1e9
+    traffic = committed_traffic(name, run.v, run.nq, dom)
+    return {"bound": "hbm", "kernel": dom, "achieved": achieved, "achieved_is": "algorithmic bytes (SURVEY 8(d) model)",
+            "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
+            "moved_model_gbs": moved, "frac_moved_model": moved / peak,
+            "traffic": traffic, "traffic_gbs": (traffic / sec / 1e9) if traffic else None,
+            "frac_traffic": (traffic / sec / 1e9 / peak) if traffic else None,
+            "overfetch": (traffic / (k["bytes_per_site"] * N)) if traffic else None,
+            "bytes_per_site": k["bytes_per_site"], "moved_bytes_per_site": k["moved_bytes_per_site"],
+            "sites_per_launch": N, "ms_per_launch": k["ms"],
+            "kernels": {n: dict(kk, gbs=kk["bytes_per_site"] * N / (kk["ms"] * 1e-3) / 1e9,
+                                moved_gbs=kk["moved_bytes_per_site"] * N / (kk["ms"] * 1e-3) / 1e9)
+                        for n, kk in kernels.items()}}
+
+
+# The other configurations the driver's single run should observe (north_star: "reported at 1
+# GPU on the synthetic geometries below"; SURVEY.md section 8(d) "per config and variant"):
+# (workload, variant overrides, LB steps per hlb_step call, calls) sized for ~0.5 s each.
+SWEEP = [
+    ("pipe", {}, 2000, 100),
+    ("cube", {}, 200, 30),
+    ("aneurysm", {}, 400, 35),
+    ("paper_sized", {"lattice": "d3q19", "scheme": "auto"}, 500, 50),
+    ("tree", {}, 100, 24),
+    ("tree", {"store": "f32"}, 100, 32),
+    ("bigtree", {"scheme": "two_lattice"}, 50, 7),
+    ("bigtree", {"scheme": "aa", "store": "f32"}, 50, 10),
+    ("bigtree", {"scheme": "aa", "lattice": "d3q19"}, 50, 6),
+]
+
+
+def run_sweep(hlb, W, have):
+    """Short timed runs of SWEEP; `have` maps workload name -> Workload already generated."""
+    out = []
+    cache = dict(have)
+    for name, over, S, K in SWEEP:
+        if name not in cache:
+            for k in list(cache):          # one big voxel array at a time
+                if k != name:
+                    del cache[k]
+            cache[name] = W.by_name(name)
+        wl = cache[name]
+        v = default_variant(scheme=DEFAULT_SCHEME[name])
+        v.update(over)
+        if v["scheme"] == "auto":
+            v["scheme"] = auto_scheme(wl.n_sites)
+        try:
+            run = Run(hlb, W, wl, name, v)
+            ms, launches, clocks = run.timed(S, K, 3)
+            kernels = run.kernel_times(6, S, ms, K, launches)
+            rf = roofline_of(run, kernels, name)
+            value = run.N * S * K / (ms * 1e-3) / 1e6
+            step_bytes = hlb.algorithmic_bytes_per_site(v["scheme"], v["store"], run.nq)
+            out.append({"workload": name, "n_sites": run.N, "scheme": v["scheme"], "store": v["store"],
+                        "lattice": v["lattice"], "links": "records" if run.g.hlb_uses_records() else "table",
+                        "resident_kernel": bool(launches < S * K),
+                        "value": value, "unit": UNIT, "lb_steps": S * K, "ms_per_lb_step": ms / (S * K),
+                        "algorithmic_gbs": value * 1e6 * step_bytes / 1e9,
+                        "roofline": {k: rf[k] for k in ("kernel", "frac", "frac_moved_model", "frac_traffic",
+                                                        "ms_per_launch", "bytes_per_site", "moved_bytes_per_site")},
+                        "hbm_bound": bool(run.g.hlb_device_bytes() > 4 * 126e6),
+                        "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "power_w_max")}})
+            run.close()
+        except Exception as e:   # one failing entry must not take the headline down with it
+            out.append({"workload": name, "variant": over, "error": repr(e)})
+    return out
+
+
+def auto_scheme(n_sites):
+    """The scheme HLB_SCHEME_AUTO picks (include/hlb.h): named here only to label the line."""
+    return "aa"
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -355,105 +575,19 @@ def main():
     import workloads as W
 
     scheme = args.scheme or DEFAULT_SCHEME[args.workload]
+    v = default_variant(scheme=scheme, store=args.store, lattice=args.lattice, order=args.order,
+                        links=args.links, prefetch=not args.no_prefetch, pdl=not args.no_pdl,
+                        resident=not args.no_resident, inlet=args.inlet, walls=args.walls)
     t_gen = time.perf_counter()
     wl = W.by_name(args.workload, small=args.small)
     t_gen = time.perf_counter() - t_gen
-    flags = (hlb.HLB_AA if scheme == "aa" else hlb.HLB_TWO_LATTICE) | \
-            (hlb.HLB_STORE_F32 if args.store == "f32" else hlb.HLB_STORE_F64) | \
-            {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
-             "tiled": hlb.HLB_ORDER_TILED}[args.order] | \
-            {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
-             "records": hlb.HLB_LINKS_RECORDS}[args.links] | \
-            (hlb.HLB_NO_PREFETCH if args.no_prefetch else 0) | \
-            (hlb.HLB_NO_PDL if args.no_pdl else 0) | \
-            (hlb.HLB_NO_RESIDENT if args.no_resident else 0) | \
-            (hlb.HLB_LATTICE_D3Q19 if args.lattice == "d3q19" else hlb.HLB_LATTICE_D3Q15)
-    t_create = time.perf_counter()
-    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags)
-    torch.cuda.synchronize()
-    t_create = time.perf_counter() - t_create
-    N = g.n_sites
-    S = args.inner
-    if wl.rho0 is not None or wl.u0 is not None:
-        g.hlb_set_state(wl.rho0, wl.u0)
-    wave = None
-    if args.inlet != "pressure" and wl.n_iolets > 0:
-        wl = W.with_velocity_inlet(wl)
-        g.hlb_set_iolet_velocity(wl.iolet_kind, wl.iolet_u)
-        if args.inlet in ("waveform", "host_waveform"):
-            wave = W.pulsatile_waveform(wl, 1000)
-            if args.inlet == "waveform":
-                g.hlb_set_iolet_waveform(wave)
-    if args.walls == "bfl_random":
-        d27 = np.random.default_rng(1906).uniform(0.05, 1.0, size=(N, 27))
-        g.hlb_set_wall_distance(d27)
-        del d27
-    stream = torch.cuda.current_stream()
-
-    def advance(n):
-        if args.inlet == "host_waveform" and wave is not None:
-            for _ in range(n):       # the time-varying inlet without the device-resident table
-                g.hlb_set_iolet_velocity(wl.iolet_kind, wave[g.hlb_steps_done() % len(wave)])
-                g.hlb_step(1)
-        else:
-            g.hlb_step(n)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    run = Run(hlb, W, wl, args.workload, v, world, local_rank)
+    g, N, S, nq = run.g, run.N, args.inner, run.nq
 
     # ---------------- device-resident timing: K x hlb_step(S)
-    for _ in range(args.warmup):
-        advance(S)
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    time.sleep(0.25)
-    l0 = g.hlb_launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    w0 = time.time()
-    ev0.record(stream)
-    for _ in range(args.steps):
-        advance(S)
-    ev1.record(stream)
-    barrier()
-    w1 = time.time()
-    clocks = sampler.stop(w0, w1)
-    ms = ev0.elapsed_time(ev1)
-    launches = g.hlb_launch_count() - l0
-
+    ms, launches, clocks = run.timed(S, args.steps, args.warmup)
     # ---------------- per-kernel durations (events around single launches, same stream)
-    reps = max(6, min(40, 2 * args.steps))
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-           for _ in range(2 * reps)]
-    torch.cuda.synchronize()
-    parity0 = g.hlb_steps_done() & 1
-    for a, b in evs:
-        a.record(stream)
-        g.hlb_step(1)
-        b.record(stream)
-    torch.cuda.synchronize()
-    per = np.array([a.elapsed_time(b) for a, b in evs])
-    nq = g.hlb_num_q()
-    pop_bytes = nq * 2 * (4 if args.store == "f32" else 8)
-    if scheme == "aa":
-        phase = (parity0 + np.arange(per.size)) & 1          # 0: even-phase kernel, 1: odd-phase
-        k_ms = {"k_aa<even>": float(np.mean(per[phase == 0])),
-                "k_aa<odd>": float(np.mean(per[phase == 1]))}
-        k_bytes = {"k_aa<even>": pop_bytes, "k_aa<odd>": pop_bytes + 4 * (nq - 1)}
-    else:
-        k_ms = {"k_pull": float(np.mean(per))}
-        k_bytes = {"k_pull": pop_bytes + 4 * (nq - 1)}
-    if launches < S * args.steps:
-        # the timed region ran the resident multi-step kernel (one launch per hlb_step(S)): its
-        # per-launch duration is the timed region's own; bytes per launch = S steps' worth
-        name = "k_aa_resident" if scheme == "aa" else "k_pull_resident"
-        per_site = S * (pop_bytes + (2 if scheme == "aa" else 4) * (nq - 1))
-        k_ms = {name: ms / args.steps}
-        k_bytes = {name: per_site}
-    dominant = max(k_ms, key=lambda k: k_ms[k])
+    kernels = run.kernel_times(max(6, min(40, 2 * args.steps)) // 2, S, ms, args.steps, launches)
 
     # ---------------- end to end through the C-ABI with host buffers
     e2e = None
@@ -470,29 +604,28 @@ def main():
 
         def e2e_step():
             g.hlb_set_state(rin_np, uin_np)             # H2D: rho [N], u [N][3]
-            advance(S)
+            run.advance(S)
             g.hlb_get_macroscopic(rho_np, u_np)        # D2H: rho [N], u [N][3] (synchronises)
 
         e2e_steps = max(2, min(args.steps, 5))
         e2e_step()
-        barrier()
+        run.barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             e2e_step()
-        barrier()
+        run.barrier()
         t_e2e = time.perf_counter() - t0
         e2e = (t_e2e, e2e_steps)
+        del rho_h, u_h, rho_in, u_in
 
     # ---------------- aggregate over ranks (max time; total work)
     ms_all, e2e_all = max_over_ranks([ms, e2e[0] if e2e else 0.0], world, dev)
     value = replicas_value(N, S * args.steps, world, ms_all * 1e-3)
 
     peak, peak_src = measured_peak()
-    dom_ms = k_ms[dominant]
-    achieved = k_bytes[dominant] * N / (dom_ms * 1e-3) / 1e9
-    traffic = committed_traffic(args.workload, scheme, args.store, dominant) if nq == 15 else \
-        committed_traffic(args.workload + "_d3q19", scheme, args.store, dominant)
     step_bytes = hlb.algorithmic_bytes_per_site(scheme, args.store, nq)
+    moved_step = hlb.moved_bytes_per_site(scheme, args.store, nq, bool(g.hlb_uses_records()),
+                                          g.hlb_record_sentinel_fraction())
     out = {
         "metric": METRIC if nq == 15 else METRIC_Q19, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
@@ -510,20 +643,14 @@ def main():
             "l2": "no flush: the populations + table (device_bytes) exceed the 126 MB L2"
                   if g.hlb_device_bytes() > 4 * 126e6 else "working set is L2-sized: not an HBM measurement",
             "parallelism": "replicas" if world > 1 else "single GPU",
-            "geometry_seconds": {"generate": round(t_gen, 2), "create": round(t_create, 2)},
+            "geometry_seconds": {"generate": round(t_gen, 2), "create": round(run.t_create, 2)},
         },
         "algorithmic_gbs": value * 1e6 * step_bytes / 1e9 / world,
         "frac_of_measured_hbm": value * 1e6 * step_bytes / 1e9 / world / peak,
         "frac_of_nominal_8000": value * 1e6 * step_bytes / 1e9 / world / 8000.0,
-        "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak,
-                     "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic,
-                     "traffic_gbs": (traffic / (dom_ms * 1e-3) / 1e9) if traffic else None,
-                     "overfetch": (traffic / (k_bytes[dominant] * N)) if traffic else None,
-                     "bytes_per_site": k_bytes[dominant],
-                     "sites_per_launch": N, "ms_per_launch": dom_ms,
-                     "kernels": {k: {"ms": k_ms[k], "bytes_per_site": k_bytes[k],
-                                     "gbs": k_bytes[k] * N / (k_ms[k] * 1e-3) / 1e9} for k in k_ms}},
+        "moved_model_gbs": value * 1e6 * moved_step / 1e9 / world,
+        "frac_moved_model_of_measured_hbm": value * 1e6 * moved_step / 1e9 / world / peak,
+        "roofline": roofline_of(run, kernels, args.workload),
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
@@ -534,10 +661,18 @@ def main():
                       "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}
     if args.render > 0:
         out["render"] = time_renderer(hlb, g, wl, args.render)
-    g.close()
+    run.close()
+    sweep = args.sweep == "on" or (args.sweep == "auto" and world == 1 and args.workload == "bigtree"
+                                   and not args.small and v == default_variant(scheme="aa"))
+    if sweep and rank == 0:
+        out["configs"] = run_sweep(hlb, W, {args.workload: wl})
+        # the same numbers as scalars (MSUPS, fraction of the measured copy peak in moved bytes)
+        out["config"]["sweep"] = "; ".join(
+            f"{c['workload']}/{c['scheme']}/{c['store']}/{c['lattice']}={c['value']:.0f}"
+            f"@{c['roofline']['frac_moved_model']:.2f}" for c in out["configs"] if "value" in c)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, n, st, dt, what, thr = time_oracle(wl, args.cpu_seconds, threads=1, lattice=args.lattice)
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
+        val, n, st, dt, what, thr = time_oracle(wl, args.cpu_seconds, threads=1, lattice=args.lattice)
+        out["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": thr, "kind": "oracle",
                                "sample": f"{what}: {n} sites x {st} LB steps in {dt:.1f} s",
                                "host_cpu": host_cpu_model(), "host_cores": os.cpu_count()}
     if rank == 0:

@@ -6,4 +6,4 @@ and loads the library and fails loudly if that is impossible -- there is no CPU 
 """
 from .binding import *  # noqa: F401,F403
 from .binding import Geometry, HlbError, LIB_PATH, EXPORTED, hlb_params, hlb_view, make_view  # noqa: F401
-from .metrics import msups, sups, BYTES_PER_SITE, algorithmic_bytes_per_site  # noqa: F401
+from .metrics import msups, sups, BYTES_PER_SITE, algorithmic_bytes_per_site, moved_bytes_per_site  # noqa: F401

@@ -31,3 +31,22 @@ def algorithmic_bytes_per_site(scheme: str, store: str, n_q: int = 15) -> float:
     pop = 8.0 if store == "f64" else 4.0
     table = 4.0 * (n_q - 1)
     return 2.0 * n_q * pop + (table if scheme == "two_lattice" else table / 2.0)
+
+
+def moved_bytes_per_site(scheme: str, store: str, n_q: int = 15, records: bool = True,
+                         sentinel_fraction: float = 0.0, phase: str = "step") -> float:
+    """Bytes one site update of the selected variant really has to move (the model ncu's DRAM
+    counters are compared with): Q populations read + Q written, the links in the form the
+    kernel reads them -- 16-byte run-length records per (warp, link), i.e. (Q - 1) / 2 bytes
+    per site, plus the int32 table rows of the sentinel records; or the whole table -- and one
+    iolet bit per site. ``phase``: "step" (A-A: mean of the even and odd kernels), "even", "odd".
+    """
+    pop = 8.0 if store == "f64" else 4.0
+    links = (16.0 * (n_q - 1) / 32.0 + sentinel_fraction * 4.0 * (n_q - 1)) if records \
+        else 4.0 * (n_q - 1)
+    base = 2.0 * n_q * pop + 4.0 / 32.0
+    if scheme == "two_lattice" or phase == "odd":
+        return base + links
+    if phase == "even":
+        return base
+    return base + links / 2.0

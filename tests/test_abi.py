@@ -87,3 +87,15 @@ def test_bytes_per_site_model():
     assert hlb.algorithmic_bytes_per_site("two_lattice", "f64", 19) == 19 * 8 * 2 + 18 * 4   # 376
     assert hlb.algorithmic_bytes_per_site("aa", "f64", 19) == 19 * 8 * 2 + 18 * 4 / 2
     assert hlb.algorithmic_bytes_per_site("two_lattice", "f32", 19) == 19 * 4 * 2 + 18 * 4
+
+
+def test_moved_bytes_model():
+    """What the selected variant really reads and writes (bench.py roofline.frac_moved_model)."""
+    m = hlb.moved_bytes_per_site
+    assert m("two_lattice", "f64", 15, records=False) == 240 + 56 + 0.125
+    assert m("two_lattice", "f64", 15, records=True, sentinel_fraction=0.0) == 240 + 7 + 0.125
+    assert m("two_lattice", "f64", 15, records=True, sentinel_fraction=0.5) == 240 + 7 + 28 + 0.125
+    assert m("aa", "f64", 15, records=True, phase="even") == 240 + 0.125
+    assert m("aa", "f64", 15, records=True, phase="odd") == 240 + 7 + 0.125
+    assert m("aa", "f64", 15, records=True) == 240 + 3.5 + 0.125
+    assert m("aa", "f32", 19, records=False, phase="odd") == 152 + 72 + 0.125
