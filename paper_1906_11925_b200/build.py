@@ -9,7 +9,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-LIB_PATH = os.path.join(HERE, "libhlb.so")
+# HLB_LIB_PATH (tuning experiments only): build / load another copy of the library, e.g. one made
+# with HLB_EXTRA_NVCC_FLAGS, so that several variants can be compared in one GPU session
+LIB_PATH = os.environ.get("HLB_LIB_PATH") or os.path.join(HERE, "libhlb.so")
 SOURCES = ["api.cu", "kernels.cu", "render.cu", "preprocess.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -310,7 +310,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   for (int64_t i = 0; i < t.N; ++i) g->canon_voxels[(size_t)t.canon_of_site[(size_t)i]] = t.voxel_of_site[(size_t)i];
 
   void *d_nbr = nullptr, *d_bits = nullptr, *d_canon = nullptr, *d_rho = nullptr, *d_scratch = nullptr;
-  void* d_rec = nullptr;
+  void *d_rec = nullptr, *d_iolinks = nullptr;
   g->sentinel_fraction = (double)t.n_rec_fallback / (double)((t.Ns / 32) * (Q - 1));
   const bool use_rec = (p->flags & HLB_LINKS_RECORDS) ? true
                        : (p->flags & HLB_LINKS_TABLE) ? false
@@ -338,7 +338,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   const size_t pop_bytes = (size_t)Q * (size_t)t.Ns * g->store_bytes();
   auto bail = [&](int code) { hlb_geometry_destroy(g); return code; };
   if ((rc = g->alloc(sizeof(int32_t) * t.nbr.size(), &d_nbr))) return bail(rc);
-  if ((rc = g->alloc(sizeof(uint32_t) * t.iolet_bits.size(), &d_bits))) return bail(rc);
+  if ((rc = g->alloc(sizeof(uint32_t) * t.iolet_idx.size(), &d_bits))) return bail(rc);
+  if ((rc = g->alloc(t.iolet_links.size(), &d_iolinks))) return bail(rc);
   if (use_rec && (rc = g->alloc(sizeof(uint32_t) * t.rec.size(), &d_rec))) return bail(rc);
   if ((rc = g->alloc(sizeof(int32_t) * (size_t)t.N, &d_canon))) return bail(rc);
   if ((rc = g->alloc(sizeof(double) * 4 * (size_t)(p->n_iolets > 0 ? p->n_iolets : 1), &d_rho))) return bail(rc);
@@ -366,7 +367,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
     if (e__ != cudaSuccess) { cuda_fail(e__, #call); return bail(HLB_ECUDA); } \
   } while (0)
   HLB_CUDA_G(cudaMemcpyAsync(d_nbr, t.nbr.data(), sizeof(int32_t) * t.nbr.size(), cudaMemcpyHostToDevice, g->stream));
-  HLB_CUDA_G(cudaMemcpyAsync(d_bits, t.iolet_bits.data(), sizeof(uint32_t) * t.iolet_bits.size(), cudaMemcpyHostToDevice, g->stream));
+  HLB_CUDA_G(cudaMemcpyAsync(d_bits, t.iolet_idx.data(), sizeof(uint32_t) * t.iolet_idx.size(), cudaMemcpyHostToDevice, g->stream));
+  HLB_CUDA_G(cudaMemcpyAsync(d_iolinks, t.iolet_links.data(), t.iolet_links.size(), cudaMemcpyHostToDevice, g->stream));
   if (use_rec)
     HLB_CUDA_G(cudaMemcpyAsync(d_rec, t.rec.data(), sizeof(uint32_t) * t.rec.size(), cudaMemcpyHostToDevice, g->stream));
   if (g->d_bar) HLB_CUDA_G(cudaMemsetAsync(g->d_bar, 0, 256, g->stream));
@@ -377,7 +379,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.N = t.N;
   g->dg.Ns = t.Ns;
   g->dg.nbr = (const int32_t*)d_nbr;
-  g->dg.iolet_bits = (const uint32_t*)d_bits;
+  g->dg.iolet_idx = d_bits;
+  g->dg.iolet_links = d_iolinks;
   g->dg.rec = d_rec;
   g->dg.use_rec = use_rec;
   g->dg.pdl = !(p->flags & HLB_NO_PDL);

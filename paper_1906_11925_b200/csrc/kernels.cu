@@ -25,6 +25,8 @@
 // state in shifted form) and stay exactly 0, so no step kernel needs a bounds branch.
 #include "kernels.cuh"
 
+#include <cstdio>
+#include <cstdlib>
 #include <tuple>
 
 #include "lbgk.cuh"
@@ -65,10 +67,6 @@ template <typename L, bool REC> constexpr int aa_odd_minb() {
 }
 template <typename L> constexpr int aa_even_minb() {
   return HLB_AA_EVEN_MINB - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
-}
-
-__device__ __forceinline__ int iolet_of(int32_t e) {  // -1: not an iolet link
-  return e < 0 ? (int)(e & 0x7fffffff) - 1 : -1;
 }
 
 template <typename L>
@@ -163,6 +161,13 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
   check_offsets<L, IT>(off, Ns);
 }
 
+// Make the compiler forget how a value was computed: the A-A odd kernel scatters to the
+// offsets it gathered from, and without this ptxas keeps the 14 64-bit ADDRESSES alive across
+// the collision (28 registers, spills) instead of the 14 32-bit offsets (one IMAD.WIDE each to
+// rebuild).
+__device__ __forceinline__ void opaque(uint32_t& v) { asm volatile("" : "+r"(v)); }
+__device__ __forceinline__ void opaque(long long& v) { asm volatile("" : "+l"(v)); }
+
 // Address (element offset) where the pre-collision f_q(x) of link q lives.
 template <int MODE>
 __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, long long i) {
@@ -177,6 +182,34 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
   return wall ? (long long)q * Ns + i : (long long)opp(q) * Ns + e;
 }
 
+// The iolet index of a group of 32 sites (preprocess.h): {bits, rank}. Loaded at the very top
+// of every step kernel -- ncu showed 12-24 % of a warp's lifetime spent waiting for this word
+// when it was loaded where it is used, after the collision (profiles/r02_ncu_step_kernels.md).
+struct IoletIndex {
+  const uint2* idx = nullptr;    // [Ns/32] {bits, rank}
+  const uint4* links = nullptr;  // [iolet sites][iolet_row<L>() uint4]: byte p - 1 = k + 1 or 0
+};
+__device__ __forceinline__ uint2 load_iolet_word(const IoletIndex& io, long long i) {
+  return __ldg(io.idx + (i >> 5));
+}
+__device__ __forceinline__ bool has_iolet_link(uint2 w) { return (w.x >> (threadIdx.x & 31)) & 1u; }
+// row of this site in IoletIndex::links, -1 if it has no iolet link (one register instead of two)
+__device__ __forceinline__ int iolet_row_of(uint2 w) {
+  const unsigned lane = threadIdx.x & 31;
+  return ((w.x >> lane) & 1u) ? (int)(w.y + __popc(w.x & ((1u << lane) - 1u))) : -1;
+}
+template <typename L>
+__host__ __device__ constexpr int iolet_row() { return (L::Q - 1 + 15) / 16; }
+// iolet id of link p (compile-time p after unrolling) in a row of link bytes; -1: not an iolet link
+template <typename L>
+__device__ __forceinline__ int iolet_of_link(const uint4 (&row)[iolet_row<L>()], int p) {
+  const int b = p - 1;
+  const uint4 v = row[b / 16];
+  const int wi = (b % 16) / 4;
+  const uint32_t word = wi == 0 ? v.x : (wi == 1 ? v.y : (wi == 2 ? v.z : v.w));
+  return (int)((word >> (8 * (b % 4))) & 0xffu) - 1;
+}
+
 // Rare path (sites on an inlet/outlet cap): for every iolet link p of site i replace
 // out[p] -- the value that will be read back as f_p(x, t+1), on entry the bounced h*_opp(p) --
 //   constant-density iolet k: by the equilibrium f_eq_p(rho_k, u(x, t))           (reading A6)
@@ -184,21 +217,25 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 //   velocity iolet k (Ladd):  by h*_opp(p) + 6 w_p rho(x, t) c_p.u_k             (reading R-ladd)
 //                             (u_k scaled by the site's weight omega(x) when iolet_w is given,
 //                              reading R-weights)
-// The table entries are re-read here so that the common path does not keep them in
-// registers; fully unrolled so that out[] stays in registers (no call, no stack).
+// Which links are iolet links comes from ONE row of link bytes per flagged site (one or two
+// 128-bit loads), not from the neighbour table: the table version issued Q - 1 dependent loads
+// one after the other and cost 6-9 % of all warp time although 3 % of the warps take it.
+// Fully unrolled so that out[] stays in registers (no call, no stack).
 // FULL = false is the lean instantiation for geometries whose iolets are all plain
 // constant-density ones (every BASELINE config): inlined, the Ladd and normal branches make
-// the compiler park four values in local memory on the COMMON path (measured: -1.5 % on
-// configs[4]; moving the rare path out of line instead cost 4-6 %, profiles/r01_tuning.md).
+// the compiler park values in local memory on the COMMON path (profiles/r01_tuning.md).
 template <typename L, bool FULL>
-__device__ __forceinline__ void iolet_substitute(const int32_t* __restrict__ nbr, long long Ns,
-                                                 long long i, const Moments& m,
+__device__ __forceinline__ void iolet_substitute(const IoletIndex& io, int irow, long long i,
+                                                 const Moments& m,
                                                  const double* __restrict__ iolet_par,
                                                  const double* __restrict__ iolet_w,
                                                  double (&out)[L::Q]) {
+  uint4 row[iolet_row<L>()];
+#pragma unroll
+  for (int k = 0; k < iolet_row<L>(); ++k) row[k] = __ldg(io.links + (long long)irow * iolet_row<L>() + k);
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) {
-    const int k = iolet_of(__ldg(nbr + (long long)(p - 1) * Ns + i));
+    const int k = iolet_of_link<L>(row, p);
     if (k >= 0) {
       const double* par = iolet_par + 4 * k;
       const double rk = __ldg(par);
@@ -236,10 +273,6 @@ __device__ __forceinline__ void pdl_wait_for_previous_step() { asm volatile("gri
 // DRAM fetch forward without holding registers or a scoreboard slot.
 __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
-
-__device__ __forceinline__ bool has_iolet_link(const uint32_t* __restrict__ iolet_bits, long long i) {
-  return (__ldg(iolet_bits + (i >> 5)) >> (threadIdx.x & 31)) & 1u;
 }
 
 // BFL interpolated walls inside the step kernels (V == 2 instantiations; BflFused in
@@ -393,14 +426,16 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
 template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
-       const uint4* __restrict__ rec, const uint32_t* __restrict__ iolet_bits,
-       const double* __restrict__ iolet_par, long long Ns, double omega, long long pf, BflFused bf) {
+       const uint4* __restrict__ rec, IoletIndex io, const double* __restrict__ iolet_par,
+       long long Ns, Relax rx, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[L::Q];
   long long bidx = -1;
+  uint2 iow;
   {
     IT off[L::Q - 1];
     pdl_launch_dependents();
+    iow = load_iolet_word(io, i);
     if (V == 2) {
       bidx = bfl_site_index(bf, i);
       if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
@@ -420,20 +455,25 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
       for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
     }
   }
+  const int irow = iolet_row_of(iow);
   if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, omega, h);
+  ST* d = dst + i;
+  if (V != 2 && irow < 0) {  // common path: every value is stored as soon as it is known
+    collide_emit<L>(h, m, rx, [&](int q, double v) { d[(long long)q * Ns] = to_store<ST>(v); });
+    return;
+  }
+  collide<L>(h, m, rx, h);
   if (V == 2 && bidx >= 0) bfl_write_pull<L>(bf, bidx, h);
-  if (has_iolet_link(iolet_bits, i)) {  // rare: sites on an inlet/outlet cap
+  if (irow >= 0) {  // rare: sites on an inlet/outlet cap
     // slot opp(p) of this site is read back by link p next step
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, bf.iolet_w, back);
+    iolet_substitute<L, (V >= 1)>(io, irow, i, m, iolet_par, bf.iolet_w, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
-  ST* d = dst + i;
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) d[(long long)q * Ns] = to_store<ST>(h[q]);
 }
@@ -445,14 +485,14 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // array and no inter-thread hazards.
 template <typename L, typename ST, int V>
 __global__ void __launch_bounds__(SBLOCK, aa_even_minb<L>())
-k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
-          const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-          long long Ns, double omega, long long pf, BflFused bf) {
+k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_par,
+          long long Ns, Relax rx, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   ST* p0 = a + i;
   double h[L::Q];
   long long bidx = -1;
   pdl_launch_dependents();
+  const uint2 iow = load_iolet_word(io, i);
   if (V == 2) {
     bidx = bfl_site_index(bf, i);
     if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
@@ -464,14 +504,20 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
 #pragma unroll
     for (int q = 0; q < L::Q; ++q) prefetch_l2(p0 + (long long)q * Ns + pf);
   }
+  opaque(Ns);  // the stores rebuild their addresses (else 15 address pairs stay live: spills)
+  const int irow = iolet_row_of(iow);
   if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, omega, h);
+  if (V != 2 && irow < 0) {  // common path: h*_q goes to slot opp(q) as soon as it is known
+    collide_emit<L>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
+    return;
+  }
+  collide<L>(h, m, rx, h);
   double out[L::Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
   if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, bf.iolet_w, out);
+  if (irow >= 0) iolet_substitute<L, (V >= 1)>(io, irow, i, m, iolet_par, bf.iolet_w, out);
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
@@ -479,12 +525,13 @@ k_aa_even(ST* __restrict__ a, const int32_t* __restrict__ nbr,
 template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
-         const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-         long long Ns, double omega, long long pf, BflFused bf) {
+         IoletIndex io, const double* __restrict__ iolet_par,
+         long long Ns, Relax rx, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
   long long bidx = -1;
   pdl_launch_dependents();
+  const uint2 iow = load_iolet_word(io, i);
   if (V == 2) {
     bidx = bfl_site_index(bf, i);
     if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
@@ -504,14 +551,24 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
   }
+#pragma unroll
+  for (int q = 1; q < L::Q; ++q) opaque(off[q - 1]);
+  const int irow = iolet_row_of(iow);
   if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, omega, h);
+  if (V != 2 && irow < 0) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
+    collide_emit<L>(h, m, rx, [&](int q, double v) {
+      if (q == 0) a[i] = to_store<ST>(v);
+      else a[off[opp(q) - 1]] = to_store<ST>(v);
+    });
+    return;
+  }
+  collide<L>(h, m, rx, h);
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
   if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
-  if (has_iolet_link(iolet_bits, i)) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, bf.iolet_w, out);
+  if (irow >= 0) iolet_substitute<L, (V >= 1)>(io, irow, i, m, iolet_par, bf.iolet_w, out);
   a[i] = to_store<ST>(out[0]);
 #pragma unroll
   for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
@@ -552,10 +609,10 @@ constexpr int RESIDENT_MINB = 4;
 
 // One site update of the resident kernels (the bodies of k_aa_even / k_aa_odd and k_pull).
 template <typename L, typename ST, typename IT, int V>
-__device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
+__device__ __forceinline__ void aa_site(ST* a, const IoletIndex& io, int irow,
                                         const double* __restrict__ iolet_par,
                                         const double* __restrict__ iolet_w, long long Ns,
-                                        double omega, long long i, const IT (&off)[L::Q - 1],
+                                        const Relax& rx, long long i, const IT (&off)[L::Q - 1],
                                         bool iolet, bool odd) {
   double h[L::Q];
   h[0] = load_l2(a + i);
@@ -567,11 +624,11 @@ __device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
     for (int q = 1; q < L::Q; ++q) h[q] = load_l2(a + (long long)q * Ns + i);
   }
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, omega, h);
+  collide<L>(h, m, rx, h);
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
-  if (iolet) iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, iolet_w, out);
+  if (iolet) iolet_substitute<L, (V >= 1)>(io, irow, i, m, iolet_par, iolet_w, out);
   a[i] = to_store<ST>(out[0]);
   if (odd) {
 #pragma unroll
@@ -582,22 +639,22 @@ __device__ __forceinline__ void aa_site(ST* a, const int32_t* __restrict__ nbr,
   }
 }
 template <typename L, typename ST, typename IT, int V>
-__device__ __forceinline__ void pull_site(const ST* src, ST* dst, const int32_t* __restrict__ nbr,
+__device__ __forceinline__ void pull_site(const ST* src, ST* dst, const IoletIndex& io, int irow,
                                           const double* __restrict__ iolet_par,
                                           const double* __restrict__ iolet_w, long long Ns,
-                                          double omega, long long i, const IT (&off)[L::Q - 1],
+                                          const Relax& rx, long long i, const IT (&off)[L::Q - 1],
                                           bool iolet) {
   double h[L::Q];
   h[0] = load_l2(src + i);
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) h[q] = load_l2(src + off[q - 1]);
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, omega, h);
+  collide<L>(h, m, rx, h);
   if (iolet) {
     double back[L::Q];
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) back[p] = h[opp(p)];
-    iolet_substitute<L, (V >= 1)>(nbr, Ns, i, m, iolet_par, iolet_w, back);
+    iolet_substitute<L, (V >= 1)>(io, irow, i, m, iolet_par, iolet_w, back);
 #pragma unroll
     for (int p = 1; p < L::Q; ++p) h[opp(p)] = back[p];
   }
@@ -608,16 +665,17 @@ __device__ __forceinline__ void pull_site(const ST* src, ST* dst, const int32_t*
 template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
 k_aa_resident(ST* a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
-              const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-              const double* __restrict__ iolet_w, long long Ns, double omega, long long n_steps, int odd0, unsigned long long* bar,
+              IoletIndex io, const double* __restrict__ iolet_par,
+              const double* __restrict__ iolet_w, long long Ns, Relax rx, long long n_steps, int odd0, unsigned long long* bar,
               unsigned long long bar_base) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
+  const int irow = iolet_row_of(load_iolet_word(io, i));
   link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
-  const bool iolet = has_iolet_link(iolet_bits, i);
+  const bool iolet = irow >= 0;
   bool odd = odd0 != 0;
   for (long long s = 0; s < n_steps; ++s) {
-    aa_site<L, ST, IT, V>(a, nbr, iolet_par, iolet_w, Ns, omega, i, off, iolet, odd);
+    aa_site<L, ST, IT, V>(a, io, irow, iolet_par, iolet_w, Ns, rx, i, off, iolet, odd);
     odd = !odd;
     if (s + 1 < n_steps) grid_barrier(bar, bar_base + (unsigned long long)(s + 1) * gridDim.x);
   }
@@ -626,17 +684,18 @@ k_aa_resident(ST* a, const int32_t* __restrict__ nbr, const uint4* __restrict__ 
 template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
 k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
-                const uint32_t* __restrict__ iolet_bits, const double* __restrict__ iolet_par,
-                const double* __restrict__ iolet_w, long long Ns, double omega, long long n_steps, unsigned long long* bar,
+                IoletIndex io, const double* __restrict__ iolet_par,
+                const double* __restrict__ iolet_w, long long Ns, Relax rx, long long n_steps, unsigned long long* bar,
                 unsigned long long bar_base) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
+  const int irow = iolet_row_of(load_iolet_word(io, i));
   link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
-  const bool iolet = has_iolet_link(iolet_bits, i);
+  const bool iolet = irow >= 0;
   const ST* src = b0;
   ST* dst = b1;
   for (long long s = 0; s < n_steps; ++s) {
-    pull_site<L, ST, IT, V>(src, dst, nbr, iolet_par, iolet_w, Ns, omega, i, off, iolet);
+    pull_site<L, ST, IT, V>(src, dst, io, irow, iolet_par, iolet_w, Ns, rx, i, off, iolet);
     ST* t = const_cast<ST*>(src);
     src = dst;
     dst = t;
@@ -800,6 +859,12 @@ int resident_sites_per_sm_aa(bool d3q19) {
 }
 
 // ------------------------------------------------------------------ launchers
+static IoletIndex iolet_index(const DeviceGeometry& g) {
+  IoletIndex io;
+  io.idx = (const uint2*)g.iolet_idx;
+  io.links = (const uint4*)g.iolet_links;
+  return io;
+}
 // Step kernels are launched with the programmatic-stream-serialization attribute when
 // g.pdl is set (see pdl_launch_dependents above).
 template <typename... KArgs, typename... Args>
@@ -817,12 +882,20 @@ static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaS
   cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+// -DHLB_TUNE_MIN (tuning builds only): compile just the instantiations the BASELINE configs run
+// (D3Q15, link records, 32-bit offsets, lean iolet path) so that a kernel experiment builds in
+// seconds; everything else aborts.
+#ifdef HLB_TUNE_MIN
+#define HLB_FULL_ONLY(...) do { fprintf(stderr, "HLB_TUNE_MIN build: instantiation not compiled\n"); abort(); } while (0)
+#else
+#define HLB_FULL_ONLY(...) __VA_ARGS__
+#endif
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
-#define HLB_PULL_ARGS s, (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, \
-                      (long long)g.Ns, g.omega, (long long)g.prefetch_pull, g.bflf
-  if (g.bfl_on) launch_step(g, k_pull<L, ST, REC, IT, 2>, HLB_PULL_ARGS);
-  else if (g.iolet_full) launch_step(g, k_pull<L, ST, REC, IT, 1>, HLB_PULL_ARGS);
+#define HLB_PULL_ARGS s, (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, \
+                      (long long)g.Ns, make_relax<L>(g.omega), (long long)g.prefetch_pull, g.bflf
+  if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 2>, HLB_PULL_ARGS));
+  else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 1>, HLB_PULL_ARGS));
   else launch_step(g, k_pull<L, ST, REC, IT, 0>, HLB_PULL_ARGS);
 #undef HLB_PULL_ARGS
 }
@@ -831,18 +904,18 @@ static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStre
   const bool idx32 = !g.index64;
   if (g.use_rec) {
     if (idx32) pull_launch<L, ST, true, uint32_t>(g, src, dst, s);
-    else pull_launch<L, ST, true, long long>(g, src, dst, s);
+    else HLB_FULL_ONLY(pull_launch<L, ST, true, long long>(g, src, dst, s));
   } else {
-    if (idx32) pull_launch<L, ST, false, uint32_t>(g, src, dst, s);
-    else pull_launch<L, ST, false, long long>(g, src, dst, s);
+    if (idx32) HLB_FULL_ONLY(pull_launch<L, ST, false, uint32_t>(g, src, dst, s));
+    else HLB_FULL_ONLY(pull_launch<L, ST, false, long long>(g, src, dst, s));
   }
 }
 template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
-#define HLB_ODD_ARGS s, (ST*)a, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega, \
-                     (long long)g.prefetch_aa, g.bflf
-  if (g.bfl_on) launch_step(g, k_aa_odd<L, ST, REC, IT, 2>, HLB_ODD_ARGS);
-  else if (g.iolet_full) launch_step(g, k_aa_odd<L, ST, REC, IT, 1>, HLB_ODD_ARGS);
+#define HLB_ODD_ARGS s, (ST*)a, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, (long long)g.Ns, \
+                     make_relax<L>(g.omega), (long long)g.prefetch_aa, g.bflf
+  if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 2>, HLB_ODD_ARGS));
+  else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 1>, HLB_ODD_ARGS));
   else launch_step(g, k_aa_odd<L, ST, REC, IT, 0>, HLB_ODD_ARGS);
 #undef HLB_ODD_ARGS
 }
@@ -850,18 +923,18 @@ template <typename L, typename ST>
 static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   const bool idx32 = !g.index64;
   if (!odd) {
-#define HLB_EVEN_ARGS s, (ST*)a, g.nbr, g.iolet_bits, g.iolet_par, (long long)g.Ns, g.omega, \
+#define HLB_EVEN_ARGS s, (ST*)a, iolet_index(g), g.iolet_par, (long long)g.Ns, make_relax<L>(g.omega), \
                       (long long)g.prefetch_aa, g.bflf
-    if (g.bfl_on) launch_step(g, k_aa_even<L, ST, 2>, HLB_EVEN_ARGS);
-    else if (g.iolet_full) launch_step(g, k_aa_even<L, ST, 1>, HLB_EVEN_ARGS);
+    if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_aa_even<L, ST, 2>, HLB_EVEN_ARGS));
+    else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_aa_even<L, ST, 1>, HLB_EVEN_ARGS));
     else launch_step(g, k_aa_even<L, ST, 0>, HLB_EVEN_ARGS);
 #undef HLB_EVEN_ARGS
   } else if (g.use_rec) {
     if (idx32) aa_odd_launch<L, ST, true, uint32_t>(g, a, s);
-    else aa_odd_launch<L, ST, true, long long>(g, a, s);
+    else HLB_FULL_ONLY(aa_odd_launch<L, ST, true, long long>(g, a, s));
   } else {
-    if (idx32) aa_odd_launch<L, ST, false, uint32_t>(g, a, s);
-    else aa_odd_launch<L, ST, false, long long>(g, a, s);
+    if (idx32) HLB_FULL_ONLY(aa_odd_launch<L, ST, false, uint32_t>(g, a, s));
+    else HLB_FULL_ONLY(aa_odd_launch<L, ST, false, long long>(g, a, s));
   }
 }
 template <typename L, typename ST>
@@ -911,8 +984,8 @@ static void init_t(const DeviceGeometry& g, void* buf, GatherMode mode, const do
 template <typename F>
 static void dispatch(const DeviceGeometry& g, F&& f) {
   if (g.d3q19) {
-    if (g.f32) f(D3Q19{}, float{});
-    else f(D3Q19{}, double{});
+    if (g.f32) HLB_FULL_ONLY(f(D3Q19{}, float{}));
+    else HLB_FULL_ONLY(f(D3Q19{}, double{}));
   } else {
     if (g.f32) f(D3Q15{}, float{});
     else f(D3Q15{}, double{});
@@ -937,16 +1010,20 @@ static cudaError_t resident_launch(const DeviceGeometry& g, bool aa, void* b0, v
                                    cudaStream_t s) {
   using IT = uint32_t;
   if (aa) {
-#define HLB_RES_ARGS s, (ST*)b0, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, g.bflf.iolet_w, \
-                     (long long)g.Ns, g.omega, n, odd0, bar, base
-    return g.iolet_full ? launch_resident(g, k_aa_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS)
-                        : launch_resident(g, k_aa_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
+#define HLB_RES_ARGS s, (ST*)b0, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, g.bflf.iolet_w, \
+                     (long long)g.Ns, make_relax<L>(g.omega), n, odd0, bar, base
+#ifndef HLB_TUNE_MIN
+    if (g.iolet_full) return launch_resident(g, k_aa_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS);
+#endif
+    return launch_resident(g, k_aa_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
 #undef HLB_RES_ARGS
   }
-#define HLB_RES_ARGS s, (ST*)b0, (ST*)b1, g.nbr, (const uint4*)g.rec, g.iolet_bits, g.iolet_par, \
-                     g.bflf.iolet_w, (long long)g.Ns, g.omega, n, bar, base
-  return g.iolet_full ? launch_resident(g, k_pull_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS)
-                      : launch_resident(g, k_pull_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
+#define HLB_RES_ARGS s, (ST*)b0, (ST*)b1, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, \
+                     g.bflf.iolet_w, (long long)g.Ns, make_relax<L>(g.omega), n, bar, base
+#ifndef HLB_TUNE_MIN
+  if (g.iolet_full) return launch_resident(g, k_pull_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS);
+#endif
+  return launch_resident(g, k_pull_resident<L, ST, REC, IT, 0>, HLB_RES_ARGS);
 #undef HLB_RES_ARGS
 }
 cudaError_t launch_resident_steps(const DeviceGeometry& g, bool aa, void* b0, void* b1, long long n,
@@ -957,8 +1034,8 @@ cudaError_t launch_resident_steps(const DeviceGeometry& g, bool aa, void* b0, vo
   dispatch(g, [&](auto l, auto st) {
     using L = decltype(l);
     using ST = decltype(st);
-    e = g.use_rec ? resident_launch<L, ST, true>(g, aa, b0, b1, n, odd0, bar, base, s)
-                  : resident_launch<L, ST, false>(g, aa, b0, b1, n, odd0, bar, base, s);
+    if (g.use_rec) e = resident_launch<L, ST, true>(g, aa, b0, b1, n, odd0, bar, base, s);
+    else HLB_FULL_ONLY(e = resident_launch<L, ST, false>(g, aa, b0, b1, n, odd0, bar, base, s));
   });
   return e;
 }

@@ -42,7 +42,8 @@ struct DeviceGeometry {
   int64_t N = 0;                        // fluid sites
   int64_t Ns = 0;                       // plane stride (multiple of 128), arrays are [Q][Ns]
   const int32_t* nbr = nullptr;         // [Q-1][Ns] pull-neighbour table (include/hlb.h)
-  const uint32_t* iolet_bits = nullptr; // [Ns/32]
+  const void* iolet_idx = nullptr;      // [Ns/32] {bits, rank} (preprocess.h: iolet index)
+  const void* iolet_links = nullptr;    // [iolet sites + 1] rows of link -> iolet id bytes
   const void* rec = nullptr;            // [Ns/32][Q-1] 16-byte link records (include/hlb.h)
   bool use_rec = false;                 // step kernels read rec instead of nbr
   BflLinks bfl;                         // applied by launch_bfl_prepass when the API says so

@@ -62,6 +62,25 @@ inline const LatticeDesc& lattice_desc(bool d3q19) {
   return d3q19 ? b : a;
 }
 
+// The relaxation constants of one geometry, computed once on the host (IEEE double products,
+// bit-identical to __dmul_rn): omega = 1 / tau, omc = 1 - omega, and the lattice weights of the
+// rest / axis / diagonal directions times omega (w0, wa, wd) and times 3 omega (a3, d3).
+struct Relax {
+  double omega, omc, w0, wa, wd, a3, d3;
+};
+template <typename L>
+inline Relax make_relax(double omega) {
+  Relax r;
+  r.omega = omega;
+  r.omc = 1.0 - omega;
+  r.w0 = L::weight(0) * omega;
+  r.wa = L::weight(1) * omega;
+  r.wd = L::weight(7) * omega;
+  r.a3 = 3.0 * L::weight(1) * omega;
+  r.d3 = 3.0 * L::weight(7) * omega;
+  return r;
+}
+
 // neighbour-table entry encoding (include/hlb.h, hlb_preprocess_tables)
 constexpr uint32_t NBR_WALL_BIT = 0x80000000u;
 

@@ -311,7 +311,7 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
   // ---- pass D: pull-neighbour table
   const int64_t Ns = out.Ns;
   out.nbr.assign((size_t)(Q - 1) * (size_t)Ns, (int32_t)NBR_WALL_BIT);
-  out.iolet_bits.assign((size_t)(Ns / 32), 0u);
+  std::vector<uint32_t> iolet_bits((size_t)(Ns / 32), 0u);
   std::atomic<int64_t> n_io_sites{0}, n_wall_links{0};
   const bool px = periodic & 1u, py = periodic & 2u, pz = periodic & 4u;
   parallel_for(N, 1 << 14, [&](int64_t b, int64_t e) {  // grain is a multiple of 32
@@ -344,7 +344,7 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
         out.nbr[(size_t)((q - 1) * Ns + i)] = entry;
       }
       if (has_io) {
-        out.iolet_bits[(size_t)(i >> 5)] |= 1u << (i & 31);
+        iolet_bits[(size_t)(i >> 5)] |= 1u << (i & 31);
         ++io_sites;
       }
     }
@@ -353,6 +353,36 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
   });
   out.n_iolet_sites = n_io_sites.load();
   out.n_wall_links = n_wall_links.load();
+
+  // ---- iolet index: {bits, rank} per group and one row of link -> iolet id per flagged site
+  const int64_t G = Ns / 32;
+  out.iolet_idx.assign((size_t)G * 2, 0u);
+  {
+    uint32_t rank = 0;
+    for (int64_t g = 0; g < G; ++g) {
+      out.iolet_idx[(size_t)g * 2] = iolet_bits[(size_t)g];
+      out.iolet_idx[(size_t)g * 2 + 1] = rank;
+      rank += (uint32_t)__builtin_popcount(iolet_bits[(size_t)g]);
+    }
+  }
+  const int row = iolet_row_bytes(Q);
+  out.iolet_links.assign((size_t)(out.n_iolet_sites + 1) * (size_t)row, (uint8_t)0);
+  parallel_for(G, 1 << 12, [&](int64_t gb, int64_t ge) {
+    for (int64_t g = gb; g < ge; ++g) {
+      uint32_t m = iolet_bits[(size_t)g];
+      size_t r = out.iolet_idx[(size_t)g * 2 + 1];
+      while (m) {
+        const int64_t i = g * 32 + __builtin_ctz(m);
+        m &= m - 1;
+        uint8_t* dst = out.iolet_links.data() + r * (size_t)row;
+        for (int q = 1; q < Q; ++q) {
+          const uint32_t e = (uint32_t)out.nbr[(size_t)((q - 1) * Ns + i)];
+          if ((e & NBR_WALL_BIT) && (e & 0x7fffffffu)) dst[q - 1] = (uint8_t)(e & 0x7fffffffu);  // k + 1
+        }
+        ++r;
+      }
+    }
+  });
 
   // ---- pass E: run-length link records
   out.rec.assign((size_t)(Ns / 32) * (Q - 1) * 4, 0u);

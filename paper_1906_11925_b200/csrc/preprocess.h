@@ -17,7 +17,12 @@ struct GeometryTables {
   std::vector<int64_t> voxel_of_site;  // [N]  internal order -> linear voxel index
   std::vector<int32_t> canon_of_site;  // [N]  internal order -> canonical rank
   std::vector<int32_t> nbr;            // [Q-1][Ns], encoding: include/hlb.h
-  std::vector<uint32_t> iolet_bits;    // [Ns/32] bit (i & 31) of word i >> 5: site i has an iolet link
+  // Iolet index (the only thing the step kernels read about iolets): per group of 32 sites
+  // {bits, rank}: bit (i & 31) of bits = site i has an iolet link; rank = number of such sites
+  // in the groups below. Site i's links are row rank + popcount(bits below lane i & 31) of
+  // iolet_links: byte p - 1 of the row = k + 1 if pull link p crosses iolet k, else 0.
+  std::vector<uint32_t> iolet_idx;     // [Ns/32][2]
+  std::vector<uint8_t> iolet_links;    // [n_iolet_sites + 1][iolet_row_bytes(Q)]
   std::vector<uint32_t> rec;           // [Ns/32][Q-1][4] run-length link records (include/hlb.h)
   int64_t n_rec_fallback = 0;          // (group, q) pairs with more than 2 runs (record = sentinel)
   int64_t n_iolet_sites = 0;
@@ -33,6 +38,10 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
 // Run-length link records of a finished table: rec [Ns/32][Q-1][4] (encoding: include/hlb.h,
 // hlb_preprocess_records). Returns the number of (group, q) pairs that got the sentinel.
 int64_t build_link_records(const int32_t* nbr, int n_links, int64_t Ns, uint32_t* rec);
+
+// Bytes of one row of GeometryTables::iolet_links: Q - 1 bytes rounded up to 16 (one or two
+// 128-bit loads).
+inline int iolet_row_bytes(int Q) { return (Q - 1 + 15) / 16 * 16; }
 
 int preprocess_threads();
 
