@@ -330,10 +330,11 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
  *   second  the non-wall lanes split into runs of lanes with consecutive entries (a wall
  *           lane or a jump in the entries ends a run); second = the lane at which run 1
  *           starts, 32 if there is only one run (or none)
- *   off0, off1: (entry of the run's first lane) - (that lane), as int32, for run 0 and 1
- * so that the entry of a non-wall lane l is (l >= second ? off1 : off0) + l. A (g, q) with
- * more than two runs gets the sentinel { 0, 0xffffffff, 0, 0 } and the kernels read nbr for
- * it instead.
+ *   off0, off1: (entry of a lane of the run) - (internal index 32 g + l of that lane's own
+ *           site), modulo 2^32, for run 0 and run 1; off1 = off0 when there is only one run
+ * so that the entry of a non-wall lane l is (l >= second ? off1 : off0) + 32 g + l (mod 2^32):
+ * the step kernels add the same delta to every lane's own index. A (g, q) with more than two
+ * runs gets the sentinel { 0, 0xffffffff, 0, 0 } and the kernels read nbr for it instead.
  *   nbr: HOST [n_links][stride] as filled by hlb_preprocess_tables; stride a multiple of 32;
  *        n_links = Q - 1 = 14 or 18
  *   rec: HOST [stride/32][n_links][4] uint32, filled

@@ -35,8 +35,9 @@ def _deps():
 
 def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(f) for f in _deps())
-    if not force and os.path.exists(LIB_PATH) and os.path.getmtime(LIB_PATH) >= newest:
-        return LIB_PATH
+    if not force and os.path.exists(LIB_PATH) and \
+            (os.path.getmtime(LIB_PATH) >= newest or os.environ.get("HLB_NO_REBUILD") == "1"):
+        return LIB_PATH   # (HLB_NO_REBUILD: tuning runs that compare libraries built from other sources)
     tmp = LIB_PATH + f".tmp{os.getpid()}"
     extra = os.environ.get("HLB_EXTRA_NVCC_FLAGS", "").split()   # tuning experiments only
     cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \

@@ -325,8 +325,12 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
       delete g;
       return HLB_ECUDA;
     }
-    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull(Q == 19) * 3 / 4 / 128 * 128;
-    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa(Q == 19) * 3 / 4 / 128 * 128;
+    // The distance is one in BYTES per plane: with 4-byte populations twice as many sites
+    // (same-box sweep of the fp32-storage kernels: 0.82 / 1.00 ms at this many sites, 0.72 /
+    // 0.97 ms at twice as many; profiles/r02_tuning.md).
+    const int64_t per8 = g->f32 ? 2 : 1;
+    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull(Q == 19) * 3 / 4 / 128 * 128 * per8;
+    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa(Q == 19) * 3 / 4 / 128 * 128 * per8;
     if (const char* e = std::getenv("HLB_PREFETCH_SITES")) {
       const long long v = std::atoll(e);
       g->dg.prefetch_pull = g->dg.prefetch_aa = v > 0 ? (v < (1ll << 24) ? v : (1ll << 24)) : 0;

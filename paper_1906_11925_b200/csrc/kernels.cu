@@ -65,8 +65,11 @@ template <typename L, bool REC> constexpr int pull_minb() {
 template <typename L, bool REC> constexpr int aa_odd_minb() {
   return HLB_AA_ODD_MINB - (REC ? 0 : 1) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
 }
-template <typename L> constexpr int aa_even_minb() {
-  return HLB_AA_EVEN_MINB - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
+// The even kernel keeps no offsets: with 4-byte populations it fits 72 registers without
+// spills, and the seventh block is worth 2.5 % there (0.704 vs 0.723 ms on configs[4]; nothing
+// in fp64, where it sits at the copy rate already).
+template <typename L, typename ST> constexpr int aa_even_minb() {
+  return HLB_AA_EVEN_MINB + (sizeof(ST) == 4 && L::Q == 15 ? 1 : 0) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
 }
 
 template <typename L>
@@ -105,10 +108,16 @@ __device__ __forceinline__ void check_offsets(const IT (&off)[L::Q - 1], long lo
 #endif
 }
 
+// q * Ns for q = 0 .. Q-1 as 32-bit values in the kernel's parameter space (constant bank):
+// the decode adds them as an instruction operand instead of computing q * Ns per thread.
+// Meaningful when Q * Ns < 2^32 (the 32-bit offset instantiations); the others ignore it.
+struct Planes {
+  uint32_t p[MAXQ];
+};
 template <typename L, int MODE, bool REC, typename IT>
 __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
                                              const uint4* __restrict__ rec, long long Ns,
-                                             long long i, IT (&off)[L::Q - 1]) {
+                                             long long i, const Planes& pl, IT (&off)[L::Q - 1]) {
   const IT n = (IT)Ns, self = (IT)i;
   if (!REC) {
     int32_t e[L::Q - 1];
@@ -134,12 +143,21 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) any |= v[q - 1].y;
   if ((int32_t)any >= 0) {
+    // offset = own index + delta + plane: delta is the run's (source - own index), or, at a
+    // wall lane, the step from plane qf to plane qw at the site itself -- five integer
+    // instructions per link (compare, select, mask test, select, 3-input add)
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) {
       const int qf = MODE == GATHER_PULL ? q : opp(q), qw = MODE == GATHER_PULL ? opp(q) : q;
       const uint4 t = v[q - 1];
-      const IT e = (IT)((lane >= t.y ? t.w : t.z) + lane);
-      off[q - 1] = (t.x & lane_bit) ? (IT)qw * n + self : (IT)qf * n + e;
+      uint32_t d = lane >= t.y ? t.w : t.z;
+      if (sizeof(IT) == 4) {
+        d = (t.x & lane_bit) ? (uint32_t)(qw - qf) * (uint32_t)n : d;
+        off[q - 1] = (IT)((uint32_t)self + d + pl.p[qf]);
+      } else {
+        const long long dd = (t.x & lane_bit) ? (long long)(qw - qf) * (long long)n : (long long)(int32_t)d;
+        off[q - 1] = (IT)((long long)self + dd + (long long)qf * (long long)n);
+      }
     }
   } else {
 #pragma unroll
@@ -152,7 +170,7 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
         e = __ldg(nbr + (long long)(q - 1) * Ns + i);
         wall = e < 0;
       } else {
-        e = (int32_t)((lane >= t.y ? t.w : t.z) + lane);
+        e = (int32_t)((lane >= t.y ? t.w : t.z) + (uint32_t)i);
         wall = (t.x & lane_bit) != 0u;
       }
       off[q - 1] = wall ? (IT)qw * n + self : (IT)qf * n + (IT)e;
@@ -167,6 +185,13 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
 // rebuild).
 __device__ __forceinline__ void opaque(uint32_t& v) { asm volatile("" : "+r"(v)); }
 __device__ __forceinline__ void opaque(long long& v) { asm volatile("" : "+l"(v)); }
+// The same for a pointer: loads through it are not merged with earlier loads of the same
+// address (the rare paths of the step kernels read their populations AGAIN on purpose).
+template <typename T>
+__device__ __forceinline__ T* relaunder(T* p) {
+  asm volatile("" : "+l"(p));
+  return p;
+}
 
 // Address (element offset) where the pre-collision f_q(x) of link q lives.
 template <int MODE>
@@ -273,6 +298,17 @@ __device__ __forceinline__ void pdl_wait_for_previous_step() { asm volatile("gri
 // DRAM fetch forward without holding registers or a scoreboard slot.
 __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// The even A-A kernel reads Q planes at the block's own 128 sites: the block pf sites ahead
+// will read Q x (128 sizeof(ST) / 128) lines, one per thread -- one prefetch instruction per
+// warp instead of Q per thread (and none of their 64-bit address arithmetic).
+template <typename L, typename ST>
+__device__ __forceinline__ void prefetch_block_planes(const ST* a, long long Ns, long long pf) {
+  constexpr int LPP = SBLOCK * (int)sizeof(ST) / 128;  // lines per plane per block
+  const ST* first = a + (long long)blockIdx.x * SBLOCK + pf;
+  for (int l = threadIdx.x; l < L::Q * LPP; l += SBLOCK)
+    prefetch_l2((const char*)(first + (long long)(l / LPP) * Ns) + (l % LPP) * 128);
 }
 
 // BFL interpolated walls inside the step kernels (V == 2 instantiations; BflFused in
@@ -423,29 +459,36 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
 // pf > 0: also L2-prefetch what site i + pf will gather; to first order its links are those
 // of site i shifted by pf (x-fastest order). The population buffers carry pf elements of
 // padding, so only the one warp-uniform test is needed.
+// Shape shared by the three step kernels. Common path (no iolet link at this site, no
+// interpolated walls): gather, moments, and every post-collision value stored the moment it
+// is known. Rare path (2-3 % of the warps): the populations are READ AGAIN (L1 / L2 hits) and
+// the moments recomputed, so that nothing has to be kept for it across the common path -- the
+// compiler otherwise parks copies of the gathered values in local memory on every thread
+// (profiles/r02_tuning.md). Safe in the in-place kernels too: a site's read set is its own
+// write set, so nobody else has written these slots, and this thread has not stored yet.
 template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, IoletIndex io, const double* __restrict__ iolet_par,
-       long long Ns, Relax rx, long long pf, BflFused bf) {
+       long long Ns, Relax rx, Planes pl, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   double h[L::Q];
   long long bidx = -1;
-  uint2 iow;
+  pdl_launch_dependents();
+  if (V == 2) {
+    bidx = bfl_site_index(bf, i);
+    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+  }
+  const bool ahead_ok = pf > 0 && i + pf < Ns;  // warp-uniform (pf, Ns: multiples of 128)
+  const uint2 iow = load_iolet_word(io, i);
   {
     IT off[L::Q - 1];
-    pdl_launch_dependents();
-    iow = load_iolet_word(io, i);
-    if (V == 2) {
-      bidx = bfl_site_index(bf, i);
-      if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
-    }
-    link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
+    link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, pl, off);
     pdl_wait_for_previous_step();
     h[0] = to_real(src[i]);
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) h[q] = to_real(src[off[q - 1]]);
-    if (pf > 0 && i + pf < Ns) {
+    if (ahead_ok) {  // every thread prefetches its own gathers shifted by pf (exact inside a run)
       const ST* ahead = src + pf;
       asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
       if (REC && (threadIdx.x & 31) < ((L::Q - 1) * 16 + 31) / 32)
@@ -459,13 +502,15 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
   if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
   ST* d = dst + i;
+  // (no second gather here, unlike the A-A kernels: the offsets are dead by now, and keeping
+  // the gathered values for the rare path costs this kernel nothing measurable)
   if (V != 2 && irow < 0) {  // common path: every value is stored as soon as it is known
-    collide_emit<L>(h, m, rx, [&](int q, double v) { d[(long long)q * Ns] = to_store<ST>(v); });
+    collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { d[(long long)q * Ns] = to_store<ST>(v); });
     return;
   }
-  collide<L>(h, m, rx, h);
+  collide<L, sizeof(ST) == 4>(h, m, rx, h);
   if (V == 2 && bidx >= 0) bfl_write_pull<L>(bf, bidx, h);
-  if (irow >= 0) {  // rare: sites on an inlet/outlet cap
+  if (irow >= 0) {  // sites on an inlet/outlet cap
     // slot opp(p) of this site is read back by link p next step
     double back[L::Q];
 #pragma unroll
@@ -482,9 +527,9 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
 // Even phase: read slot q of the site, write h*_q to slot opp(q) of the site (no table).
 // Odd phase: read f_q from slot opp(q) of x - c_q (slot q of x at a wall), write h*_q to
 // the address f_opp(q) was read from. Read set = write set per site in both phases, so one
-// array and no inter-thread hazards.
+// array and no inter-thread hazards (tests/test_aa_model.py).
 template <typename L, typename ST, int V>
-__global__ void __launch_bounds__(SBLOCK, aa_even_minb<L>())
+__global__ void __launch_bounds__(SBLOCK, aa_even_minb<L, ST>())
 k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_par,
           long long Ns, Relax rx, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
@@ -500,19 +545,22 @@ k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_pa
   pdl_wait_for_previous_step();
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
-  if (pf > 0 && i + pf < Ns) {
-#pragma unroll
-    for (int q = 0; q < L::Q; ++q) prefetch_l2(p0 + (long long)q * Ns + pf);
-  }
+  if (pf > 0 && i + pf < Ns) prefetch_block_planes<L, ST>(a, Ns, pf);  // block-uniform test
   opaque(Ns);  // the stores rebuild their addresses (else 15 address pairs stay live: spills)
   const int irow = iolet_row_of(iow);
+  if (V != 2) {
+    if (irow < 0) {  // common path: h*_q goes to slot opp(q) as soon as it is known
+      const Moments m = moments_of<L>(h);
+      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
+      return;
+    }
+    const ST* again = relaunder(p0);  // rare path: read again
+#pragma unroll
+    for (int q = 0; q < L::Q; ++q) h[q] = to_real(again[(long long)q * Ns]);
+  }
   if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
-  if (V != 2 && irow < 0) {  // common path: h*_q goes to slot opp(q) as soon as it is known
-    collide_emit<L>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
-    return;
-  }
-  collide<L>(h, m, rx, h);
+  collide<L, sizeof(ST) == 4>(h, m, rx, h);
   double out[L::Q];  // out[p] is written where f_p was read: the bounced h*_opp(p)
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
@@ -526,23 +574,24 @@ template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          IoletIndex io, const double* __restrict__ iolet_par,
-         long long Ns, Relax rx, long long pf, BflFused bf) {
+         long long Ns, Relax rx, Planes pl, long long pf, BflFused bf) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
   long long bidx = -1;
   pdl_launch_dependents();
-  const uint2 iow = load_iolet_word(io, i);
   if (V == 2) {
     bidx = bfl_site_index(bf, i);
     if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
   }
-  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
+  const bool ahead_ok = pf > 0 && i + pf < Ns;  // warp-uniform (pf, Ns: multiples of 128)
+  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, pl, off);
+  const uint2 iow = load_iolet_word(io, i);  // (not before the decode: its registers are the scarce ones)
   pdl_wait_for_previous_step();
   double h[L::Q];
   h[0] = to_real(a[i]);
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) h[q] = to_real(a[off[q - 1]]);
-  if (pf > 0 && i + pf < Ns) {
+  if (ahead_ok) {  // every thread prefetches its own gathers shifted by pf (exact inside a run)
     const ST* ahead = a + pf;
     asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
     if (REC && (threadIdx.x & 31) < ((L::Q - 1) * 16 + 31) / 32)
@@ -554,16 +603,23 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) opaque(off[q - 1]);
   const int irow = iolet_row_of(iow);
+  if (V != 2) {
+    if (irow < 0) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
+      const Moments m = moments_of<L>(h);
+      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) {
+        if (q == 0) a[i] = to_store<ST>(v);
+        else a[off[opp(q) - 1]] = to_store<ST>(v);
+      });
+      return;
+    }
+    const ST* again = relaunder(a);  // rare path: read again
+    h[0] = to_real(again[i]);
+#pragma unroll
+    for (int q = 1; q < L::Q; ++q) h[q] = to_real(again[off[q - 1]]);
+  }
   if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
   const Moments m = moments_of<L>(h);
-  if (V != 2 && irow < 0) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
-    collide_emit<L>(h, m, rx, [&](int q, double v) {
-      if (q == 0) a[i] = to_store<ST>(v);
-      else a[off[opp(q) - 1]] = to_store<ST>(v);
-    });
-    return;
-  }
-  collide<L>(h, m, rx, h);
+  collide<L, sizeof(ST) == 4>(h, m, rx, h);
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
@@ -624,7 +680,7 @@ __device__ __forceinline__ void aa_site(ST* a, const IoletIndex& io, int irow,
     for (int q = 1; q < L::Q; ++q) h[q] = load_l2(a + (long long)q * Ns + i);
   }
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, rx, h);
+  collide<L, sizeof(ST) == 4>(h, m, rx, h);
   double out[L::Q];
 #pragma unroll
   for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
@@ -649,7 +705,7 @@ __device__ __forceinline__ void pull_site(const ST* src, ST* dst, const IoletInd
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) h[q] = load_l2(src + off[q - 1]);
   const Moments m = moments_of<L>(h);
-  collide<L>(h, m, rx, h);
+  collide<L, sizeof(ST) == 4>(h, m, rx, h);
   if (iolet) {
     double back[L::Q];
 #pragma unroll
@@ -666,12 +722,12 @@ template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
 k_aa_resident(ST* a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
               IoletIndex io, const double* __restrict__ iolet_par,
-              const double* __restrict__ iolet_w, long long Ns, Relax rx, long long n_steps, int odd0, unsigned long long* bar,
+              const double* __restrict__ iolet_w, long long Ns, Relax rx, Planes pl, long long n_steps, int odd0, unsigned long long* bar,
               unsigned long long bar_base) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
   const int irow = iolet_row_of(load_iolet_word(io, i));
-  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, off);
+  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, pl, off);
   const bool iolet = irow >= 0;
   bool odd = odd0 != 0;
   for (long long s = 0; s < n_steps; ++s) {
@@ -685,12 +741,12 @@ template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, RESIDENT_MINB)
 k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
                 IoletIndex io, const double* __restrict__ iolet_par,
-                const double* __restrict__ iolet_w, long long Ns, Relax rx, long long n_steps, unsigned long long* bar,
+                const double* __restrict__ iolet_w, long long Ns, Relax rx, Planes pl, long long n_steps, unsigned long long* bar,
                 unsigned long long bar_base) {
   const long long i = (long long)blockIdx.x * SBLOCK + threadIdx.x;
   IT off[L::Q - 1];
   const int irow = iolet_row_of(load_iolet_word(io, i));
-  link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, off);
+  link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, pl, off);
   const bool iolet = irow >= 0;
   const ST* src = b0;
   ST* dst = b1;
@@ -859,6 +915,11 @@ int resident_sites_per_sm_aa(bool d3q19) {
 }
 
 // ------------------------------------------------------------------ launchers
+static Planes planes_of(const DeviceGeometry& g) {
+  Planes pl;
+  for (int q = 0; q < MAXQ; ++q) pl.p[q] = (uint32_t)((uint64_t)q * (uint64_t)g.Ns);
+  return pl;
+}
 static IoletIndex iolet_index(const DeviceGeometry& g) {
   IoletIndex io;
   io.idx = (const uint2*)g.iolet_idx;
@@ -893,7 +954,7 @@ static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaS
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
 #define HLB_PULL_ARGS s, (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, \
-                      (long long)g.Ns, make_relax<L>(g.omega), (long long)g.prefetch_pull, g.bflf
+                      (long long)g.Ns, make_relax<L>(g.omega), planes_of(g), (long long)g.prefetch_pull, g.bflf
   if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 2>, HLB_PULL_ARGS));
   else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 1>, HLB_PULL_ARGS));
   else launch_step(g, k_pull<L, ST, REC, IT, 0>, HLB_PULL_ARGS);
@@ -913,7 +974,7 @@ static void pull_t(const DeviceGeometry& g, const void* src, void* dst, cudaStre
 template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
 #define HLB_ODD_ARGS s, (ST*)a, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, (long long)g.Ns, \
-                     make_relax<L>(g.omega), (long long)g.prefetch_aa, g.bflf
+                     make_relax<L>(g.omega), planes_of(g), (long long)g.prefetch_aa, g.bflf
   if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 2>, HLB_ODD_ARGS));
   else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 1>, HLB_ODD_ARGS));
   else launch_step(g, k_aa_odd<L, ST, REC, IT, 0>, HLB_ODD_ARGS);
@@ -1011,7 +1072,7 @@ static cudaError_t resident_launch(const DeviceGeometry& g, bool aa, void* b0, v
   using IT = uint32_t;
   if (aa) {
 #define HLB_RES_ARGS s, (ST*)b0, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, g.bflf.iolet_w, \
-                     (long long)g.Ns, make_relax<L>(g.omega), n, odd0, bar, base
+                     (long long)g.Ns, make_relax<L>(g.omega), planes_of(g), n, odd0, bar, base
 #ifndef HLB_TUNE_MIN
     if (g.iolet_full) return launch_resident(g, k_aa_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS);
 #endif
@@ -1019,7 +1080,7 @@ static cudaError_t resident_launch(const DeviceGeometry& g, bool aa, void* b0, v
 #undef HLB_RES_ARGS
   }
 #define HLB_RES_ARGS s, (ST*)b0, (ST*)b1, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, \
-                     g.bflf.iolet_w, (long long)g.Ns, make_relax<L>(g.omega), n, bar, base
+                     g.bflf.iolet_w, (long long)g.Ns, make_relax<L>(g.omega), planes_of(g), n, bar, base
 #ifndef HLB_TUNE_MIN
   if (g.iolet_full) return launch_resident(g, k_pull_resident<L, ST, REC, IT, 1>, HLB_RES_ARGS);
 #endif

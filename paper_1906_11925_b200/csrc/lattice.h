@@ -62,9 +62,10 @@ inline const LatticeDesc& lattice_desc(bool d3q19) {
   return d3q19 ? b : a;
 }
 
-// The relaxation constants of one geometry, computed once on the host (IEEE double products,
-// bit-identical to __dmul_rn): omega = 1 / tau, omc = 1 - omega, and the lattice weights of the
-// rest / axis / diagonal directions times omega (w0, wa, wd) and times 3 omega (a3, d3).
+// The relaxation constants of one geometry as the step kernels take them (by value), computed
+// on the host (IEEE double products, bit-identical to __dmul_rn): omega = 1 / tau for the
+// difference form of the relaxation; omc = 1 - omega and the rest / axis / diagonal weights
+// times omega (w0, wa, wd) and times 3 omega (a3, d3) for the folded form (lbgk.cuh).
 struct Relax {
   double omega, omc, w0, wa, wd, a3, d3;
 };

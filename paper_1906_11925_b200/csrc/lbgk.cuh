@@ -102,38 +102,61 @@ __device__ __forceinline__ double heq_of(int q, double drho, double rho, double 
   return mul(L::weight(q), fma_(rho, poly, drho));
 }
 
-// hs_q = h_q + omega (heq_q(m) - h_q) = (1 - omega) h_q + omega heq_q, evaluated per opposite
-// pair (a, b = opp(a)), c = c_a:
-//   omega heq_a = S + A, omega heq_b = S - A,
-//   S = omega w (drho + rho (4.5 (c.u)^2 - 1.5 u.u)),  A = 3 omega w rho (c.u)
-// -- the same equilibrium as heq_of(), with the part even in c computed once per pair and
-// omega folded into the weights: two fp64 operations per direction after S and A (the
-// kernels' power draw and issue slots are what this buys).
+// hs_q = h_q + omega (heq_q(m) - h_q), evaluated per opposite pair (a, b = opp(a)), c = c_a:
+//   heq_a = S + A, heq_b = S - A,  S = w (drho + rho (4.5 (c.u)^2 - 1.5 u.u)),  A = 3 w rho (c.u)
+// -- the same equilibrium as heq_of(), with the part even in c computed once per pair (a
+// third fewer fp64 operations; the kernels run into the 1 kW power cap otherwise).
+//
+// Two forms of the relaxation, chosen by the storage type (profiles/r02_tuning.md):
+//   FOLDED = false (fp64 storage): applied to the DIFFERENCE, h + omega ((S +- A) - h). heq - h
+//     is small and nearly exact, so this is the accurate form: E_u ~ 4e-15 on configs[2] after
+//     2000 steps against the oracle.
+//   FOLDED = true (fp32 storage): (1 - omega) h + (omega S +- omega A) with omega folded into
+//     the weights on the host -- one operation and one dependent step less per direction,
+//     1-4 % faster on the fp32-storage kernels (which are latency-, not HBM-bound), and 30x
+//     less accurate in fp64 terms (E_u 1.2e-13), which is six orders below the rounding of the
+//     stored binary32 values themselves (E_u ~ 1e-7, bar 1e-5).
 // emit(q, hs_q) is called as soon as a post-collision value is known, so that a kernel can
 // store it at once and free its registers (and those of its address): with all stores after
 // the whole collision the A-A odd kernel kept 7 of its 14 offsets in local memory.
-template <typename L, typename F>
+template <typename L, bool FOLDED, typename F>
 __device__ __forceinline__ void collide_emit(const double (&h)[L::Q], const Moments& m, const Relax& rx,
                                              F&& emit) {
   const double uu15 = mul(1.5, u_dot_u(m.ux, m.uy, m.uz));
-  emit(0, fma_(rx.omc, h[0], mul(rx.w0, fma_(-m.rho, uu15, m.drho))));
-  // two weight classes: axis (q = 1..6) and diagonal (q >= 7)
-  const double r3_axis = mul(rx.a3, m.rho), r3_diag = mul(rx.d3, m.rho);
+  if (FOLDED) {
+    emit(0, fma_(rx.omc, h[0], mul(rx.w0, fma_(-m.rho, uu15, m.drho))));
+    const double r3_axis = mul(rx.a3, m.rho), r3_diag = mul(rx.d3, m.rho);
 #pragma unroll
-  for (int a = 1; a < L::Q; a += 2) {
-    const int b = a + 1;  // opp(a)
-    const double cu = c_dot_u<L>(a, m.ux, m.uy, m.uz);
-    const double S = mul(a <= 6 ? rx.wa : rx.wd, fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
-    const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
-    const double ha = h[a], hb = h[b];
-    emit(a, fma_(rx.omc, ha, add(S, A)));
-    emit(b, fma_(rx.omc, hb, sub(S, A)));
+    for (int a = 1; a < L::Q; a += 2) {
+      const int b = a + 1;  // opp(a)
+      const double cu = c_dot_u<L>(a, m.ux, m.uy, m.uz);
+      const double S = mul(a <= 6 ? rx.wa : rx.wd, fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
+      const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
+      emit(a, fma_(rx.omc, h[a], add(S, A)));
+      emit(b, fma_(rx.omc, h[b], sub(S, A)));
+    }
+  } else {
+    const double omega = rx.omega;
+    const double heq0 = mul(L::weight(0), fma_(-m.rho, uu15, m.drho));
+    emit(0, fma_(omega, sub(heq0, h[0]), h[0]));
+    // two weight classes: axis (q = 1..6) and diagonal (q >= 7)
+    const double r3_axis = mul(3.0 * L::weight(1), m.rho), r3_diag = mul(3.0 * L::weight(7), m.rho);
+#pragma unroll
+    for (int a = 1; a < L::Q; a += 2) {
+      const int b = a + 1;  // opp(a)
+      const double cu = c_dot_u<L>(a, m.ux, m.uy, m.uz);
+      const double S = mul(L::weight(a), fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
+      const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
+      const double ha = h[a], hb = h[b];
+      emit(a, fma_(omega, sub(add(S, A), ha), ha));
+      emit(b, fma_(omega, sub(sub(S, A), hb), hb));
+    }
   }
 }
-template <typename L>
+template <typename L, bool FOLDED>
 __device__ __forceinline__ void collide(const double (&h)[L::Q], const Moments& m, const Relax& rx,
                                         double (&hs)[L::Q]) {
-  collide_emit<L>(h, m, rx, [&](int q, double v) { hs[q] = v; });
+  collide_emit<L, FOLDED>(h, m, rx, [&](int q, double v) { hs[q] = v; });
 }
 
 // storage <-> arithmetic conversions (HLB_STORE_F64 / HLB_STORE_F32; include/hlb.h)

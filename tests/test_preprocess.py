@@ -157,11 +157,13 @@ def decode_records(rec, nbr):
                 sentinel[g, k] = True
                 continue
             assert 1 <= second <= 32
+            if second == 32:
+                assert o1 == o0
             for l in range(32):
                 if (wall >> l) & 1:
                     continue
                 off = o1 if l >= second else o0
-                out[k, g * 32 + l] = int(np.int32(np.uint32(off))) + l
+                out[k, g * 32 + l] = (off + g * 32 + l) % 2 ** 32
     return out, sentinel
 
 
