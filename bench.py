@@ -64,7 +64,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="bigtree", choices=list(WORKLOAD_DESC))
-    ap.add_argument("--scheme", default=None, choices=["aa", "two_lattice"])
+    ap.add_argument("--scheme", default=None, choices=["aa", "two_lattice", "auto"])
     ap.add_argument("--store", default="f64", choices=["f64", "f32"])
     ap.add_argument("--order", default="auto", choices=["auto", "morton", "raster", "tiled"])
     ap.add_argument("--links", default="auto", choices=["auto", "table", "records"])
@@ -316,7 +316,7 @@ def run_reference(args, rank, world):
 
 # --------------------------------------------------------------------------- our arm
 def variant_flags(hlb, v):
-    return (hlb.HLB_AA if v["scheme"] == "aa" else hlb.HLB_TWO_LATTICE) | \
+    return {"aa": hlb.HLB_AA, "two_lattice": hlb.HLB_TWO_LATTICE, "auto": hlb.HLB_SCHEME_AUTO}[v["scheme"]] | \
         (hlb.HLB_STORE_F32 if v["store"] == "f32" else hlb.HLB_STORE_F64) | \
         {"auto": hlb.HLB_ORDER_AUTO, "morton": hlb.HLB_ORDER_MORTON, "raster": hlb.HLB_ORDER_RASTER,
          "tiled": hlb.HLB_ORDER_TILED}[v["order"]] | \
@@ -347,6 +347,8 @@ class Run:
         self.t_create = time.perf_counter() - t0
         g = self.g
         self.N, self.nq = g.n_sites, g.hlb_num_q()
+        if v["scheme"] == "auto":          # report what HLB_SCHEME_AUTO took
+            self.v = v = dict(v, scheme="aa" if g.hlb_uses_aa() else "two_lattice", scheme_auto=True)
         if wl.rho0 is not None or wl.u0 is not None:
             g.hlb_set_state(wl.rho0, wl.u0)
         self.wave = None
@@ -521,10 +523,9 @@ def run_sweep(hlb, W, have):
         wl = cache[name]
         v = default_variant(scheme=DEFAULT_SCHEME[name])
         v.update(over)
-        if v["scheme"] == "auto":
-            v["scheme"] = auto_scheme(wl.n_sites)
         try:
             run = Run(hlb, W, wl, name, v)
+            v = run.v
             ms, launches, clocks = run.timed(S, K, 3)
             kernels = run.kernel_times(6, S, ms, K, launches)
             rf = roofline_of(run, kernels, name)
@@ -543,11 +544,6 @@ def run_sweep(hlb, W, have):
         except Exception as e:   # one failing entry must not take the headline down with it
             out.append({"workload": name, "variant": over, "error": repr(e)})
     return out
-
-
-def auto_scheme(n_sites):
-    """The scheme HLB_SCHEME_AUTO picks (include/hlb.h): named here only to label the line."""
-    return "aa"
 
 
 def main():
@@ -583,6 +579,7 @@ def main():
     t_gen = time.perf_counter() - t_gen
     run = Run(hlb, W, wl, args.workload, v, world, local_rank)
     g, N, S, nq = run.g, run.N, args.inner, run.nq
+    scheme = run.v["scheme"]          # what HLB_SCHEME_AUTO took, if that was asked for
 
     # ---------------- device-resident timing: K x hlb_step(S)
     ms, launches, clocks = run.timed(S, args.steps, args.warmup)
@@ -663,7 +660,7 @@ def main():
         out["render"] = time_renderer(hlb, g, wl, args.render)
     run.close()
     sweep = args.sweep == "on" or (args.sweep == "auto" and world == 1 and args.workload == "bigtree"
-                                   and not args.small and v == default_variant(scheme="aa"))
+                                   and not args.small and run.v == default_variant(scheme="aa"))
     if sweep and rank == 0:
         out["configs"] = run_sweep(hlb, W, {args.workload: wl})
         # the same numbers as scalars (MSUPS, fraction of the measured copy peak in moved bytes)

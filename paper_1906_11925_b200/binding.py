@@ -25,6 +25,7 @@ HLB_NO_PREFETCH = 0x80
 HLB_INDEX64 = 0x100
 HLB_NO_PDL = 0x400
 HLB_NO_RESIDENT = 0x800
+HLB_SCHEME_AUTO = 0x1000
 HLB_LATTICE_D3Q15, HLB_LATTICE_D3Q19 = 0x0, 0x200
 
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
@@ -106,6 +107,7 @@ def _load() -> ctypes.CDLL:
         "hlb_device_bytes": (i64, [vp]),
         "hlb_launch_count": (i64, [vp]),
         "hlb_uses_records": (c_int, [vp]),
+        "hlb_uses_aa": (c_int, [vp]),
         "hlb_record_sentinel_fraction": (ctypes.c_double, [vp]),
         "hlb_preprocess_records": (c_int, [vp, ctypes.c_int32, i64, vp, ctypes.POINTER(i64)]),
         "hlb_geometry_destroy": (None, [vp]),
@@ -130,7 +132,7 @@ EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
-            "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records",
+            "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records", "hlb_uses_aa",
             "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
             "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables",
             "hlb_preprocess_records")
@@ -387,6 +389,9 @@ class Geometry:
 
     def hlb_launch_count(self) -> int:
         return int(_lib.hlb_launch_count(self._h))
+
+    def hlb_uses_aa(self) -> bool:
+        return bool(_lib.hlb_uses_aa(self._h))
 
     def hlb_uses_records(self) -> bool:
         return bool(_lib.hlb_uses_records(self._h))

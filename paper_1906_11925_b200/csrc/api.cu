@@ -174,7 +174,7 @@ static int check_params(const uint8_t* site_type, const hlb_params* p, SiteOrder
   if (p->periodic & ~7u) return fail(HLB_EINVAL, "unknown periodic bits");
   if (p->flags & ~(uint32_t)(HLB_STORE_F32 | HLB_AA | HLB_ORDER_MASK | HLB_NO_GRAPH |
                              HLB_LINKS_TABLE | HLB_LINKS_RECORDS | HLB_NO_PREFETCH | HLB_INDEX64 |
-                             HLB_LATTICE_D3Q19 | HLB_NO_PDL | HLB_NO_RESIDENT))
+                             HLB_LATTICE_D3Q19 | HLB_NO_PDL | HLB_NO_RESIDENT | HLB_SCHEME_AUTO))
     return fail(HLB_EINVAL, "unknown flag bits");
   if ((p->flags & HLB_LINKS_TABLE) && (p->flags & HLB_LINKS_RECORDS))
     return fail(HLB_EINVAL, "HLB_LINKS_TABLE and HLB_LINKS_RECORDS are exclusive");
@@ -297,6 +297,16 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->p.iolet_rho = nullptr;
   g->stream = (cudaStream_t)p->stream;
   g->aa = (p->flags & HLB_AA) != 0;
+  if (p->flags & HLB_SCHEME_AUTO) {
+    // A-A everywhere except where the resident multi-step kernel applies (there two-lattice
+    // is faster: 5.4 k vs 5.0 k MSUPS on configs[0]; profiles/r02_tuning.md)
+    int dev = 0, sms = 0;
+    const bool resident = !(p->flags & (HLB_NO_GRAPH | HLB_NO_RESIDENT)) &&
+                          cudaGetDevice(&dev) == cudaSuccess &&
+                          cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+                          t.Ns <= (int64_t)sms * resident_kernel_sites_per_sm();
+    g->aa = !resident;
+  }
   g->f32 = (p->flags & HLB_STORE_F32) != 0;
   g->Q = (p->flags & HLB_LATTICE_D3Q19) ? 19 : 15;
   const int Q = g->Q;
@@ -946,6 +956,7 @@ int64_t hlb_num_sites(const hlb_geometry* g) { return g ? g->N : (int64_t)HLB_EI
 int64_t hlb_steps_done(const hlb_geometry* g) { return g ? g->steps : (int64_t)HLB_EINVAL; }
 int64_t hlb_device_bytes(const hlb_geometry* g) { return g ? g->device_bytes : (int64_t)HLB_EINVAL; }
 int64_t hlb_launch_count(const hlb_geometry* g) { return g ? g->launches : (int64_t)HLB_EINVAL; }
+int hlb_uses_aa(const hlb_geometry* g) { return g ? (g->aa ? 1 : 0) : (int)HLB_EINVAL; }
 int hlb_uses_records(const hlb_geometry* g) { return g ? (g->dg.use_rec ? 1 : 0) : (int)HLB_EINVAL; }
 double hlb_record_sentinel_fraction(const hlb_geometry* g) { return g ? g->sentinel_fraction : -1.0; }
 int hlb_get_site_voxels(const hlb_geometry* g, int64_t* v) {

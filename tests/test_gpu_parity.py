@@ -1031,6 +1031,25 @@ def test_configs_3_4_full_size_sampled_against_oracle(hlb, name, scheme, store, 
     assert checked > 20000
 
 
+def test_scheme_auto_picks_and_matches_the_explicit_scheme(hlb):
+    """HLB_SCHEME_AUTO: two-lattice where the resident multi-step kernel applies (small
+    geometries), A-A in place otherwise; either way bitwise the explicitly chosen scheme."""
+    wl = W.by_name("aneurysm", small=True)
+    for extra, want_aa in ((0, False), (hlb.HLB_NO_RESIDENT, True)):
+        g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                    hlb.HLB_SCHEME_AUTO | extra)
+        assert g.hlb_uses_aa() == want_aa
+        g.hlb_step(31)
+        got = g.hlb_get_macroscopic()
+        g.close()
+        ref = run_gpu(hlb, wl, 31, "aa" if want_aa else "two_lattice", "f64", "auto")
+        assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1])
+    big = W.by_name("paper_sized")                       # 296 k sites: beyond the resident kernel
+    g = hlb.hlb_geometry_create(big.site_type, big.periodic, big.tau, big.iolet_rho, hlb.HLB_SCHEME_AUTO)
+    assert g.hlb_uses_aa()
+    g.close()
+
+
 # ------------------------------------------------------------- north_star's acceptance runs
 # "GPU results must match the oracle on the same seeded inputs ... after the configured steps
 # ... on all five configs" (BASELINE.json north_star; SURVEY.md §8(d) config table): full size

@@ -136,7 +136,7 @@ def test_argument_errors():
     assert e.value.code == hlb.HLB_EINVAL
     st[0, 0, 0] = 0
     with pytest.raises(hlb.HlbError) as e:
-        hlb.hlb_preprocess(st, 0, 0, 0x1000)                           # unknown flag bit
+        hlb.hlb_preprocess(st, 0, 0, 0x4000)                           # unknown flag bit
     assert e.value.code == hlb.HLB_EINVAL
     t = hlb.hlb_preprocess(st, 0, 0, 0)                                # isolated site: all walls
     assert t["N"] == 1 and np.all(t["nbr"] == WALL)
