@@ -47,7 +47,7 @@ UNIT = "MSUPS"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 DEFAULT_SCHEME = {"pipe": "two_lattice", "cube": "two_lattice", "aneurysm": "two_lattice",
                   "paper_sized": "two_lattice",
-                  "tree": "two_lattice", "bigtree": "aa"}
+                  "tree": "two_lattice", "bigtree": "aa", "cube672": "aa", "bigtree_x": "aa"}
 WORKLOAD_DESC = {
     "pipe": "BASELINE configs[0]: pipe R=8 L=64",
     "cube": "BASELINE configs[1]: periodic 128^3 Taylor-Green",
@@ -55,6 +55,9 @@ WORKLOAD_DESC = {
     "tree": "BASELINE configs[3]: 5-level tree, 1024^3 box, r0=32",
     "bigtree": "BASELINE configs[4]: 5-level tree, 2048x2048x1024 box, r0=64",
     "paper_sized": "context only: aneurysm recipe scaled to ~297k sites (the paper's Subject 16, Table II)",
+    "cube672": "context only: periodic 672^3 cube, 303.5 M sites (64-bit flat offsets: Q N > 2^32)",
+    "bigtree_x": "context only: configs[4] generator at 77 um voxels (box and r0 x 1.3), 85.5 M sites "
+                 "(BASELINE's nominal 80-100 M)",
 }
 
 
@@ -588,6 +591,8 @@ def main():
 
     # ---------------- end to end through the C-ABI with host buffers
     e2e = None
+    if not args.no_e2e and 128 * N > 16e9:
+        args.no_e2e = True          # four pinned host arrays of 32 N bytes: not at this size
     if not args.no_e2e:
         rho_h = torch.empty(N, dtype=torch.float64).pin_memory()
         u_h = torch.empty((N, 3), dtype=torch.float64).pin_memory()
@@ -636,7 +641,7 @@ def main():
             "bfl_sites": g.hlb_num_bfl_sites(),
             "record_sentinel_fraction": round(g.hlb_record_sentinel_fraction(), 4), "tau": wl.tau, "n_iolets": wl.n_iolets,
             "box": list(wl.shape), "seed": wl.info.get("seed"),
-            "device_bytes": g.hlb_device_bytes(),
+            "device_bytes": g.hlb_device_bytes(), "offset_bits": g.hlb_offset_bits(),
             "l2": "no flush: the populations + table (device_bytes) exceed the 126 MB L2"
                   if g.hlb_device_bytes() > 4 * 126e6 else "working set is L2-sized: not an HBM measurement",
             "parallelism": "replicas" if world > 1 else "single GPU",

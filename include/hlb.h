@@ -258,6 +258,9 @@ int64_t hlb_device_bytes(const hlb_geometry* g);
  * multi-step launch counts once; with BFL
  * walls the pre-pass over the interpolated links counts too, also when a read-out runs it). */
 int64_t hlb_launch_count(const hlb_geometry* g);
+/* Width of the flat population offsets the step kernels compute: 32, or 64 when Q * stride
+ * >= 2^32 (above 286 M sites for D3Q15) or HLB_INDEX64 was given. */
+int hlb_offset_bits(const hlb_geometry* g);
 /* 1 if the geometry steps in place (A-A), 0 if it uses two arrays (see HLB_SCHEME_AUTO). */
 int hlb_uses_aa(const hlb_geometry* g);
 /* 1 if the step kernels of this geometry read the link records, 0 if they read the table. */

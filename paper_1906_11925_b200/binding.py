@@ -108,6 +108,7 @@ def _load() -> ctypes.CDLL:
         "hlb_launch_count": (i64, [vp]),
         "hlb_uses_records": (c_int, [vp]),
         "hlb_uses_aa": (c_int, [vp]),
+        "hlb_offset_bits": (c_int, [vp]),
         "hlb_record_sentinel_fraction": (ctypes.c_double, [vp]),
         "hlb_preprocess_records": (c_int, [vp, ctypes.c_int32, i64, vp, ctypes.POINTER(i64)]),
         "hlb_geometry_destroy": (None, [vp]),
@@ -132,7 +133,7 @@ EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
-            "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records", "hlb_uses_aa",
+            "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records", "hlb_uses_aa", "hlb_offset_bits",
             "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
             "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables",
             "hlb_preprocess_records")
@@ -389,6 +390,9 @@ class Geometry:
 
     def hlb_launch_count(self) -> int:
         return int(_lib.hlb_launch_count(self._h))
+
+    def hlb_offset_bits(self) -> int:
+        return int(_lib.hlb_offset_bits(self._h))
 
     def hlb_uses_aa(self) -> bool:
         return bool(_lib.hlb_uses_aa(self._h))

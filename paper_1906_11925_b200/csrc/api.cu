@@ -956,6 +956,7 @@ int64_t hlb_num_sites(const hlb_geometry* g) { return g ? g->N : (int64_t)HLB_EI
 int64_t hlb_steps_done(const hlb_geometry* g) { return g ? g->steps : (int64_t)HLB_EINVAL; }
 int64_t hlb_device_bytes(const hlb_geometry* g) { return g ? g->device_bytes : (int64_t)HLB_EINVAL; }
 int64_t hlb_launch_count(const hlb_geometry* g) { return g ? g->launches : (int64_t)HLB_EINVAL; }
+int hlb_offset_bits(const hlb_geometry* g) { return g ? (g->dg.index64 ? 64 : 32) : (int)HLB_EINVAL; }
 int hlb_uses_aa(const hlb_geometry* g) { return g ? (g->aa ? 1 : 0) : (int)HLB_EINVAL; }
 int hlb_uses_records(const hlb_geometry* g) { return g ? (g->dg.use_rec ? 1 : 0) : (int)HLB_EINVAL; }
 double hlb_record_sentinel_fraction(const hlb_geometry* g) { return g ? g->sentinel_fraction : -1.0; }

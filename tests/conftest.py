@@ -15,17 +15,6 @@ RECORD_LINES = []
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
     config.addinivalue_line("markers", "slow: the longest GPU cases (minutes; part of the default -m gpu run)")
-    config.addinivalue_line("markers", "huge: needs > 64 GB of host memory and > 40 GB of HBM; "
-                                       "opt-in via HLB_RUN_HUGE=1")
-
-
-def pytest_collection_modifyitems(config, items):
-    if os.environ.get("HLB_RUN_HUGE") == "1":
-        return
-    skip = pytest.mark.skip(reason="needs a large-memory box; set HLB_RUN_HUGE=1")
-    for item in items:
-        if "huge" in item.keywords:
-            item.add_marker(skip)
 
 
 @pytest.fixture

@@ -1069,6 +1069,86 @@ def test_full_configs_full_steps_record(hlb, name, record):
         assert e_rho < TOL[store] and e_u < TOL[store]
 
 
+# ------------------------------------------------------------- the sizes the library claims
+def _needs(host_gb, device_gb):
+    """These two cases need a large box (the B200 boxes of this pool have 196 GB of host memory
+    and 180 GB of HBM); elsewhere they skip rather than drive a small machine out of memory."""
+    import psutil
+    import torch
+    if psutil.virtual_memory().available < host_gb * 2 ** 30:
+        pytest.skip(f"needs {host_gb} GB of free host memory")
+    if torch.cuda.mem_get_info()[0] < device_gb * 2 ** 30:
+        pytest.skip(f"needs {device_gb} GB of free device memory")
+
+
+@pytest.mark.slow
+def test_cube672_runs_the_64_bit_offset_kernels_for_real(hlb, record):
+    """303.5 M sites: Q * N = 4.55e9 > 2^32, so the `long long` offset instantiations are the ones
+    launched (without HLB_INDEX64), the int32 table holds entries up to 3.0e8, the link-record
+    deltas wrap, and 17 GB of table + 36 GB of populations are uploaded. Checked by exact mass
+    conservation (periodic box) and by the oracle on interior sub-boxes of the same field,
+    chosen so that the compared sites sit in the first, a middle and the last plane rows."""
+    _needs(70, 80)
+    wl = W.by_name("cube672")
+    n = wl.info["n"]
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, "aa", "f64", "auto", "auto"))
+    assert g.hlb_offset_bits() == 64 and g.hlb_uses_records() and g.n_sites == n ** 3
+    ax = np.arange(n, dtype=np.float64)
+    rho = (1.0 + 0.01 * np.sin(0.07 * ax[None, None, :] + 0.05 * ax[None, :, None])
+           * np.cos(0.06 * ax[:, None, None])).reshape(-1)
+    u = np.empty((n ** 3, 3), dtype=np.float64)
+    z, y, x = ax[:, None, None], ax[None, :, None], ax[None, None, :]
+    u[:, 0] = (0.02 * np.sin(0.05 * y + 0.03 * z) + 0.0 * x).reshape(-1)
+    u[:, 1] = (0.02 * np.cos(0.04 * x - 0.06 * z) + 0.0 * y).reshape(-1)
+    u[:, 2] = (0.02 * np.sin(0.03 * x + 0.07 * y) + 0.0 * z).reshape(-1)
+    g.hlb_set_state(rho, u)
+    mass0 = float(np.sum(rho, dtype=np.float64))
+    del rho, u
+    steps = 25
+    g.hlb_step(steps)
+    rho, u = g.hlb_get_macroscopic()
+    dev_gb = g.hlb_device_bytes() / 2 ** 30
+    g.close()
+    assert np.all(np.isfinite(rho)) and np.all(np.isfinite(u))
+    drift = abs(float(np.sum(rho, dtype=np.float64)) - mass0) / n ** 3
+    assert drift < 1e-14, drift                     # shifted populations: mass is conserved to roundoff
+    checked = 0
+    for centre in ((60, 60, 60), (336, 300, 340), (600, 610, 611)):
+        k, un = _crop_check(hlb, wl, rho, u, steps, centre, 56, TOL["f64"])
+        assert un > 1e-3
+        checked += k
+    record(f"HUGE cube672 N={n ** 3} steps={steps} aa/f64 offsets=64-bit device={dev_gb:.1f} GiB "
+           f"mass drift/site={drift:.1e} sites compared with the oracle={checked}")
+
+
+@pytest.mark.slow
+def test_bigtree_at_baselines_nominal_size(hlb, record):
+    """configs[4]'s generator at BASELINE's nominal 80-100 M sites (workloads 'bigtree_x':
+    85.5 M), A-A fp64 in the bench's launch configuration, 25 steps from a smooth field, sampled
+    sub-boxes against the oracle."""
+    _needs(40, 30)
+    wl = W.by_name("bigtree_x")
+    steps = 25
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, "aa", "f64", "auto", "auto"))
+    assert g.hlb_uses_records() and g.hlb_offset_bits() == 32
+    nz, ny, nx = wl.site_type.shape
+    v = wl.fluid_voxels()
+    g.hlb_set_state(*_smooth_state(v % nx, (v // nx) % ny, v // (nx * ny)))
+    g.hlb_step(steps)
+    rho, u = g.hlb_get_macroscopic()
+    g.close()
+    assert np.all(np.isfinite(rho)) and np.all(np.isfinite(u))
+    checked = 0
+    for centre in _sample_centres(wl, 5):
+        k, un = _crop_check(hlb, wl, rho, u, steps, centre, 56, TOL["f64"])
+        assert un > 1e-3
+        checked += k
+    assert checked > 20000
+    record(f"HUGE bigtree_x N={wl.n_sites} steps={steps} aa/f64 sites compared with the oracle={checked}")
+
+
 # ------------------------------------------------------------- long horizon, every variant
 @pytest.mark.parametrize("store", ["f64", "f32"])
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])

@@ -89,7 +89,7 @@ def pipe(radius: int = 8, length: int = 64, tau: float = 0.8, rho_in: float = 1.
 
 # --------------------------------------------------------------------------- config 1
 def periodic_cube(n: int = 128, tau: float = 0.6, u0: float = 0.01, steps: int = 1000,
-                  nz: Optional[int] = None) -> Workload:
+                  nz: Optional[int] = None, with_state: bool = True) -> Workload:
     """Fully periodic all-fluid box with a z-invariant Taylor-Green vortex
     (BASELINE configs[1]; field: SURVEY.md §8(c) A12).
 
@@ -98,6 +98,9 @@ def periodic_cube(n: int = 128, tau: float = 0.6, u0: float = 0.01, steps: int =
     nz = n if nz is None else nz
     st = np.full((nz, n, n), FLUID, dtype=np.uint8)
     k = 2.0 * math.pi / n
+    if not with_state:   # geometry only (rest state): the huge cube of the 64-bit-offset runs
+        return Workload("cube", st, PERIODIC_X | PERIODIC_Y | PERIODIC_Z, tau,
+                        np.zeros(0, dtype=np.float64), steps, info={"n": n, "u0": 0.0, "k": k})
     xs = np.arange(n, dtype=np.float64)
     sx, cx = np.sin(k * xs), np.cos(k * xs)
     ux2d = u0 * np.outer(cx, sx)          # [y, x] -> u0 sin(kx) cos(ky)
@@ -485,6 +488,24 @@ def by_name(name: str, small: bool = False) -> Workload:
         if small:
             return tree(box=(160, 160, 160), r0=5.0, levels=3, steps=60)
         return tree()
+    if name == "cube672":
+        # not a BASELINE config: the smallest periodic cube whose Q * N exceeds 2^32 (303.5 M
+        # sites), so that the 64-bit flat-offset kernels are the ones that run (include/hlb.h
+        # HLB_INDEX64); A-A in place, rest state unless the caller sets one
+        w = periodic_cube(n=40 if small else 672, steps=25, with_state=False)
+        return dataclasses.replace(w, name="cube672", scheme="aa")
+    if name == "bigtree_x":
+        # not a BASELINE config: configs[4] at BASELINE's nominal 80-100 M sites. Its generator
+        # cannot get there inside the 2048 x 2048 x 1024 box (SURVEY.md section 8(d) caveat: with
+        # r0, the radius law and the angles fixed, L / r = 8 is what fits -- the root-to-leaf
+        # path is 1862 voxels -- and three sacs on the largest bifurcations would add 34 M at
+        # most), so the third knob is turned: the voxel size. Box and r0 scaled by 1.3
+        # (77 um voxels instead of 100 um), same seed search, everything else as configs[4].
+        if small:
+            return tree(box=(248, 248, 124), r0=6.5, levels=3, planar_deg=30.0, tau=0.52,
+                        steps=60, scheme="aa", name="bigtree_x")
+        return tree(box=(2662, 2662, 1331), r0=83.2, planar_deg=30.0, tau=0.52, steps=200,
+                    scheme="aa", name="bigtree_x")
     if name == "bigtree":
         if small:
             return tree(box=(192, 192, 96), r0=5.0, levels=3, planar_deg=30.0, tau=0.52,
