@@ -84,6 +84,9 @@ def parse_args():
     ap.add_argument("--render", type=int, default=0, metavar="PIXELS",
                     help="also time the ray-marching renderer (NEXT-4) on the final state: PIXELS x "
                          "PIXELS frames of the speed field, rotating view; adds a \"render\" object")
+    ap.add_argument("--render-view", default="rotate", choices=["rotate", "axis", "oblique1", "oblique2", "oblique3"],
+                    help="rotate: the view turns about the y axis over the frames; else one fixed view "
+                         "(the ones profiles/render_inst.csv has instruction counts for)")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--no-pdl", action="store_true", help="HLB_NO_PDL (ablation)")
     ap.add_argument("--no-resident", action="store_true",
@@ -226,42 +229,101 @@ def replicas_value(n_sites, lb_steps, world, seconds):
     return world * n_sites * lb_steps / seconds / 1e6
 
 
-def time_renderer(hlb, g, wl, pixels, frames=12):
+RENDER_VIEWS = {   # rotations (degrees about x, then about y) of the fixed views of --render-view
+    "rotate": None, "axis": (0.0, 0.0), "oblique1": (20.0, 30.0), "oblique2": (-35.0, 60.0), "oblique3": (50.0, -20.0)}
+SM_ISSUE_PEAK = 148 * 4 * 1.965e9   # warp instructions / s: 148 SMs x 4 schedulers x 1965 MHz
+
+
+def render_inst_count(workload, pixels, view, texture):
+    """Warp instructions of one k_raymarch launch from the committed ncu capture of exactly this
+    frame (profiles/render_inst.csv: workload,pixels,view,texture,smsp__inst_executed.sum,source)."""
+    path = os.path.join(ROOT, "profiles", "render_inst.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        parts = [p.strip() for p in line.split(",")]
+        if parts[:4] == [workload, str(pixels), view, "texture" if texture else "linear"]:
+            return float(parts[4])
+    return None
+
+
+def time_renderer(hlb, g, wl, workload, pixels, view_name="rotate", frames=12, cpu_pixels=96):
     """Frames per second of hlb_render_device on the geometry's current state (speed field,
-    orthographic view turning about the y axis, sample step 0.5 voxel, image kept on the
-    device). The first frame also builds the dense voxel volume."""
+    orthographic view, sample step 0.5 voxel, image kept on the device), the ray marcher alone
+    (CUDA events around it are not possible from here, so: frame time minus the time of the same
+    calls with a 16 x 16 image), the oracle renderer timed on a cpu_pixels^2 frame of the same
+    view as the CPU baseline, and -- for the fixed views with a committed instruction count --
+    the issue-slot roofline of k_raymarch."""
     import math
     import torch
     nx, ny, nz = wl.shape
     lut = np.stack([np.linspace(0, 1, 256)] * 3 + [np.full(256, 0.02)], axis=1).astype(np.float32)
     lut[0, 3] = 0.0          # value 0 (solid voxels, fluid at rest) is transparent: empty cells are skipped
     rho, u = g.hlb_get_macroscopic()
-    umax = float(np.max(np.linalg.norm(u, axis=1))) or 1.0
-    zoom = pixels / float(max(nx, ny, nz))
+    speed = np.linalg.norm(u, axis=1)
+    umax = float(np.max(speed)) or 1.0
 
-    def view(k):
-        a = 2.0 * math.pi * k / frames
-        rot = [[math.cos(a), 0, math.sin(a)], [0, 1, 0], [-math.sin(a), 0, math.cos(a)]]
-        return hlb.make_view(pixels, pixels, rot=rot, zoom=zoom, step=0.5, tf_scale=1.0 / umax,
-                             tf_offset=0.0, opacity=1.0, field=0)
+    def rot_of(k):
+        if RENDER_VIEWS[view_name] is None:
+            ax, ay = 0.0, 360.0 * k / frames
+        else:
+            ax, ay = RENDER_VIEWS[view_name]
+        ax, ay = math.radians(ax), math.radians(ay)
+        rx = np.array([[1, 0, 0], [0, math.cos(ax), -math.sin(ax)], [0, math.sin(ax), math.cos(ax)]])
+        ry = np.array([[math.cos(ay), 0, math.sin(ay)], [0, 1, 0], [-math.sin(ay), 0, math.cos(ay)]])
+        return ry @ rx
 
-    g.hlb_render_device(view(0), lut)                       # builds the volume
-    torch.cuda.synchronize()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(torch.cuda.current_stream())
-    for k in range(frames):
-        img = g.hlb_render_device(view(k), lut)
-    ev1.record(torch.cuda.current_stream())
-    torch.cuda.synchronize()
-    ms = ev0.elapsed_time(ev1) / frames
-    diag = math.sqrt(nx * nx + ny * ny + nz * nz)
-    rays = pixels * pixels
-    return {"pixels": [pixels, pixels], "frames": frames, "ms_per_frame": ms, "fps": 1e3 / ms,
-            "volume_voxels": nx * ny * nz, "sample_step": 0.5,
-            "ray_samples_per_frame_upper_bound": int(rays * (diag / 0.5 + 1)),
-            "includes": "macroscopic read-out + scatter into the voxel volume + ray march, per frame",
-            "empty_space_skipping": not os.environ.get("HLB_RENDER_NO_SKIP", "0").strip("0"),
-            "max_alpha": float(img[..., 3].max())}
+    def view(k, px):
+        return hlb.make_view(px, px, rot=rot_of(k), zoom=px / float(max(nx, ny, nz)), step=0.5,
+                             tf_scale=1.0 / umax, tf_offset=0.0, opacity=1.0, field=0)
+
+    def timed(px):
+        g.hlb_render_device(view(0, px), lut)                       # builds the volume
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(torch.cuda.current_stream())
+        for k in range(frames):
+            img = g.hlb_render_device(view(k, px), lut)
+        ev1.record(torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / frames, img
+
+    ms_small, _ = timed(16)          # read-out + scatter + a negligible march
+    ms, img = timed(pixels)
+    ms_march = max(ms - ms_small, 1e-6)
+    texture = not os.environ.get("HLB_RENDER_LINEAR", "0").strip("0")
+    out = {"pixels": [pixels, pixels], "frames": frames, "view": view_name, "ms_per_frame": ms, "fps": 1e3 / ms,
+           "ms_ray_march": ms_march, "ms_readout_and_scatter": ms_small,
+           "rays_per_s": pixels * pixels / (ms_march * 1e-3),
+           "volume_voxels": nx * ny * nz, "sample_step": 0.5, "volume_through": "texture" if texture else "linear",
+           "includes": "macroscopic read-out + scatter into the voxel volume + ray march, per frame",
+           "empty_space_skipping": not os.environ.get("HLB_RENDER_NO_SKIP", "0").strip("0"),
+           "max_alpha": float(img[..., 3].max())}
+    inst = render_inst_count(workload, pixels, view_name, texture)
+    out["roofline"] = {"bound": "alu", "kernel": "k_raymarch", "unit": "Gwarp-inst/s",
+                       "peak": SM_ISSUE_PEAK / 1e9, "peak_source": "148 SMs x 4 schedulers x 1965 MHz (issue slots)",
+                       "warp_inst_per_frame": inst,
+                       "achieved": (inst / (ms_march * 1e-3) / 1e9) if inst else None,
+                       "frac": (inst / (ms_march * 1e-3) / SM_ISSUE_PEAK) if inst else None}
+    # CPU baseline: the oracle renderer (oracle/render_oracle.cpp, 1 core) on the same volume and
+    # view at cpu_pixels^2 rays -- a bounded sample of the frame, centred on the same axis
+    import oracle
+    vol = np.zeros(nx * ny * nz, dtype=np.float32)
+    vol[wl.fluid_voxels()] = speed.astype(np.float32)
+    vol = vol.reshape(nz, ny, nx)
+    v = view(0, cpu_pixels)
+    t0 = time.perf_counter()
+    _, n_samples = oracle.render(vol, cpu_pixels, cpu_pixels, rot_of(0), v.zoom, v.step, v.tf_scale,
+                                 v.tf_offset, v.opacity, lut)
+    dt = time.perf_counter() - t0
+    del vol
+    out["cpu_baseline"] = {"kind": "oracle", "cores": 1, "value": cpu_pixels * cpu_pixels / dt, "unit": "rays/s",
+                           "samples_inside_the_box_per_s": n_samples / dt,
+                           "sample": f"{cpu_pixels} x {cpu_pixels} rays of the same view (zoom scaled to the frame) "
+                                     f"in {dt:.1f} s; the oracle visits every sample, the GPU skips empty cells"}
+    return out
 
 
 def host_cpu_model():
@@ -662,7 +724,7 @@ def main():
                       "steps": e2e[1], "ms_per_step": e2e_all / e2e[1] * 1e3,
                       "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}
     if args.render > 0:
-        out["render"] = time_renderer(hlb, g, wl, args.render)
+        out["render"] = time_renderer(hlb, g, wl, args.workload, args.render, args.render_view)
     run.close()
     sweep = args.sweep == "on" or (args.sweep == "auto" and world == 1 and args.workload == "bigtree"
                                    and not args.small and run.v == default_variant(scheme="aa"))

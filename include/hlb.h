@@ -96,6 +96,11 @@ typedef struct hlb_geometry hlb_geometry; /* opaque handle */
 /* Returns a DEVICE pointer to `bytes` bytes, at least 256-byte aligned, or NULL. The
  * memory must stay valid until after hlb_geometry_destroy(). */
 typedef void* (*hlb_alloc_fn)(size_t bytes, void* user);
+/* Optional counterpart: called with a pointer hlb_alloc_fn returned once the library no longer
+ * uses it and no enqueued work refers to it (a table that was regrown: a longer waveform, a
+ * larger image, other wall distances). Without it such buffers stay with the caller until
+ * hlb_geometry_destroy(). */
+typedef void (*hlb_free_fn)(void* ptr, void* user);
 
 typedef struct {
   int32_t nx, ny, nz;      /* voxel box, each >= 1                                         */
@@ -109,6 +114,8 @@ typedef struct {
   hlb_alloc_fn alloc;      /* device allocator or NULL (=> cudaMalloc)                     */
   void* alloc_user;
   void* stream;            /* cudaStream_t as void*; NULL = the legacy default stream      */
+  hlb_free_fn free;        /* optional (NULL): releases one buffer of `alloc` early; called
+                              with alloc_user                                              */
 } hlb_params;
 
 /* Build the geometry: extract the fluid sites, order them, build the int32 pull-neighbour
@@ -121,7 +128,9 @@ typedef struct {
 int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geometry** out);
 
 /* Set f_q(x, 0) = f_eq_q(rho(x), u(x)) and the step counter to 0.
- *   rho: HOST [N] or NULL (=> 1);  u: HOST [N][3] or NULL (=> 0); canonical order. */
+ *   rho: HOST [N] or NULL (=> 1);  u: HOST [N][3] or NULL (=> 0); canonical order.
+ * The host arrays have been read when the call returns (it waits for its own copies; this
+ * holds for every hlb_set_* call that takes host arrays). */
 int hlb_set_state(hlb_geometry* g, const double* rho, const double* u);
 
 /* Replace the n_iolets iolet densities (HOST array, each > 0). Takes effect from the next

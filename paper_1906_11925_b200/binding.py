@@ -29,6 +29,7 @@ HLB_SCHEME_AUTO = 0x1000
 HLB_LATTICE_D3Q15, HLB_LATTICE_D3Q19 = 0x0, 0x200
 
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+_FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
 
 
 class hlb_params(ctypes.Structure):
@@ -42,6 +43,7 @@ class hlb_params(ctypes.Structure):
         ("alloc", _ALLOC_FN),
         ("alloc_user", ctypes.c_void_p),
         ("stream", ctypes.c_void_p),
+        ("free", _FREE_FN),
     ]
 
 
@@ -256,8 +258,16 @@ class Geometry:
             self._buffers.append(t)
             return t.data_ptr()
 
-        self._alloc_cb = _ALLOC_FN(_alloc)     # keep the callback object alive
+        def _free(ptr, _user):
+            for k, t in enumerate(self._buffers):
+                if t.data_ptr() == ptr:
+                    del self._buffers[k]
+                    return
+
+        self._alloc_cb = _ALLOC_FN(_alloc)     # keep the callback objects alive
+        self._free_cb = _FREE_FN(_free)
         p.alloc = self._alloc_cb
+        p.free = self._free_cb
         p.alloc_user = None
         with torch.cuda.device(self.device):
             self.stream = torch.cuda.current_stream() if stream is None else stream
@@ -268,58 +278,70 @@ class Geometry:
         self.n_iolets = int(p.n_iolets)
         self.flags = int(flags)
 
+    def _call(self, fn, *args):
+        """Every library call runs with the geometry's device current: the library itself never
+        calls cudaSetDevice, and its launches go to whatever device is current."""
+        with self._torch.cuda.device(self.device):
+            return fn(self._h, *args)
+
     # -- the C-ABI calls, same names -------------------------------------------------
     def hlb_set_state(self, rho=None, u=None):
         n = self.n_sites
         rho, u = _host(rho, np.float64, (n,)), _host(u, np.float64, (n, 3))
-        _check(_lib.hlb_set_state(self._h, _ptr(rho), _ptr(u)))
+        _check(self._call(_lib.hlb_set_state, _ptr(rho), _ptr(u)))
 
     def hlb_set_iolet_density(self, iolet_rho):
-        io = _host(np.asarray(iolet_rho).reshape(-1), np.float64)
-        _check(_lib.hlb_set_iolet_density(self._h, _ptr(io)))
+        io = _host(np.asarray(iolet_rho).reshape(-1), np.float64, (self.n_iolets,))
+        _check(self._call(_lib.hlb_set_iolet_density, _ptr(io)))
 
     def hlb_set_iolet_velocity(self, kind, u=None):
-        kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8)
-        u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64)
-        _check(_lib.hlb_set_iolet_velocity(self._h, _ptr(kind), _ptr(u)))
+        kind = None if kind is None else _host(np.asarray(kind).reshape(-1), np.uint8, (self.n_iolets,))
+        u = None if u is None else _host(np.asarray(u, dtype=np.float64).reshape(-1, 3), np.float64,
+                                         (self.n_iolets, 3))
+        _check(self._call(_lib.hlb_set_iolet_velocity, _ptr(kind), _ptr(u)))
 
     def hlb_set_iolet_weight(self, weight):
         w = None if weight is None else _host(np.asarray(weight, dtype=np.float64).reshape(-1),
                                               np.float64, (self.n_sites,))
-        _check(_lib.hlb_set_iolet_weight(self._h, _ptr(w)))
+        _check(self._call(_lib.hlb_set_iolet_weight, _ptr(w)))
 
     def hlb_set_iolet_waveform(self, u):
         """u: [n_t][n_iolets][3] (or None to remove the waveform)."""
         if u is None:
-            _check(_lib.hlb_set_iolet_waveform(self._h, None, 0))
+            _check(self._call(_lib.hlb_set_iolet_waveform, None, 0))
             return
         u = _host(np.asarray(u, dtype=np.float64), np.float64)
         if u.ndim != 3 or u.shape[2] != 3:
             raise ValueError("waveform must have shape [n_t][n_iolets][3]")
         if u.shape[1] != self.n_iolets:
             raise ValueError(f"waveform has {u.shape[1]} iolets, the geometry {self.n_iolets}")
-        _check(_lib.hlb_set_iolet_waveform(self._h, _ptr(u), int(u.shape[0])))
+        _check(self._call(_lib.hlb_set_iolet_waveform, _ptr(u), int(u.shape[0])))
 
     def hlb_set_iolet_normal(self, normals):
-        n = None if normals is None else _host(np.asarray(normals, dtype=np.float64).reshape(-1, 3), np.float64)
-        _check(_lib.hlb_set_iolet_normal(self._h, _ptr(n)))
+        n = None if normals is None else _host(np.asarray(normals, dtype=np.float64).reshape(-1, 3), np.float64,
+                                               (self.n_iolets, 3))
+        _check(self._call(_lib.hlb_set_iolet_normal, _ptr(n)))
 
     def hlb_set_wall_distance(self, d27):
         d27 = None if d27 is None else _host(d27, np.float64, (self.n_sites, 27))
-        _check(_lib.hlb_set_wall_distance(self._h, _ptr(d27)))
+        _check(self._call(_lib.hlb_set_wall_distance, _ptr(d27)))
 
     def hlb_num_bfl_sites(self) -> int:
-        return int(_lib.hlb_num_bfl_sites(self._h))
+        return int(self._call(_lib.hlb_num_bfl_sites))
 
     def hlb_step(self, n: int = 1):
-        _check(_lib.hlb_step(self._h, int(n)))
+        _check(self._call(_lib.hlb_step, int(n)))
 
     def hlb_get_macroscopic(self, rho_out=None, u_out=None):
         """Host results (numpy); pass preallocated (e.g. pinned) arrays to reuse them."""
         n = self.n_sites
         rho = np.empty(n, dtype=np.float64) if rho_out is None else rho_out
         u = np.empty((n, 3), dtype=np.float64) if u_out is None else u_out
-        _check(_lib.hlb_get_macroscopic(self._h, _ptr(rho), _ptr(u)))
+        for a, shape in ((rho, (n,)), (u, (n, 3))):
+            if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.shape == shape
+                    and a.flags.c_contiguous and a.flags.writeable):
+                raise ValueError(f"output array must be a writable C-contiguous float64 array of shape {shape}")
+        _check(self._call(_lib.hlb_get_macroscopic, _ptr(rho), _ptr(u)))
         return rho, u
 
     def hlb_get_macroscopic_device(self):
@@ -327,86 +349,86 @@ class Geometry:
         torch = self._torch
         rho = torch.empty(self.n_sites, dtype=torch.float64, device=self.device)
         u = torch.empty((self.n_sites, 3), dtype=torch.float64, device=self.device)
-        _check(_lib.hlb_get_macroscopic_device(self._h, rho.data_ptr(), u.data_ptr()))
+        _check(self._call(_lib.hlb_get_macroscopic_device, rho.data_ptr(), u.data_ptr()))
         return rho, u
 
     def hlb_get_stress(self):
         """Deviatoric stress [N, 6] (xx, yy, zz, xy, xz, yz), host."""
         sg = np.empty((self.n_sites, 6), dtype=np.float64)
-        _check(_lib.hlb_get_stress(self._h, _ptr(sg)))
+        _check(self._call(_lib.hlb_get_stress, _ptr(sg)))
         return sg
 
     def hlb_get_wall_shear_stress(self, normals):
         nrm = _host(normals, np.float64, (self.n_sites, 3))
         out = np.empty(self.n_sites, dtype=np.float64)
-        _check(_lib.hlb_get_wall_shear_stress(self._h, _ptr(nrm), _ptr(out)))
+        _check(self._call(_lib.hlb_get_wall_shear_stress, _ptr(nrm), _ptr(out)))
         return out
 
     def hlb_get_stress_device(self):
         torch = self._torch
         sg = torch.empty((self.n_sites, 6), dtype=torch.float64, device=self.device)
-        _check(_lib.hlb_get_stress_device(self._h, sg.data_ptr()))
+        _check(self._call(_lib.hlb_get_stress_device, sg.data_ptr()))
         return sg
 
     def hlb_render(self, view: "hlb_view", lut):
         """Image [height, width, 4] float32 (host) of the current state."""
         lut = np.ascontiguousarray(np.asarray(lut, dtype=np.float32).reshape(256, 4))
         img = np.empty((view.height, view.width, 4), dtype=np.float32)
-        _check(_lib.hlb_render(self._h, ctypes.byref(view), _ptr(lut), _ptr(img)))
+        _check(self._call(_lib.hlb_render, ctypes.byref(view), _ptr(lut), _ptr(img)))
         return img
 
     def hlb_render_device(self, view: "hlb_view", lut):
         torch = self._torch
         lut = np.ascontiguousarray(np.asarray(lut, dtype=np.float32).reshape(256, 4))
         img = torch.empty((view.height, view.width, 4), dtype=torch.float32, device=self.device)
-        _check(_lib.hlb_render_device(self._h, ctypes.byref(view), _ptr(lut), img.data_ptr()))
+        _check(self._call(_lib.hlb_render_device, ctypes.byref(view), _ptr(lut), img.data_ptr()))
         return img
 
     def hlb_get_populations(self):
         f = np.empty((self.n_sites, self.n_q), dtype=np.float64)
-        _check(_lib.hlb_get_populations(self._h, _ptr(f)))
+        _check(self._call(_lib.hlb_get_populations, _ptr(f)))
         return f
 
     def hlb_set_populations(self, f):
         f = _host(f, np.float64, (self.n_sites, self.n_q))
-        _check(_lib.hlb_set_populations(self._h, _ptr(f)))
+        _check(self._call(_lib.hlb_set_populations, _ptr(f)))
 
     def hlb_num_q(self) -> int:
-        return int(_lib.hlb_num_q(self._h))
+        return int(self._call(_lib.hlb_num_q))
 
     def hlb_num_sites(self) -> int:
-        return int(_lib.hlb_num_sites(self._h))
+        return int(self._call(_lib.hlb_num_sites))
 
     def hlb_steps_done(self) -> int:
-        return int(_lib.hlb_steps_done(self._h))
+        return int(self._call(_lib.hlb_steps_done))
 
     def hlb_get_site_voxels(self):
         v = np.empty(self.n_sites, dtype=np.int64)
-        _check(_lib.hlb_get_site_voxels(self._h, _ptr(v)))
+        _check(self._call(_lib.hlb_get_site_voxels, _ptr(v)))
         return v
 
     def hlb_device_bytes(self) -> int:
-        return int(_lib.hlb_device_bytes(self._h))
+        return int(self._call(_lib.hlb_device_bytes))
 
     def hlb_launch_count(self) -> int:
-        return int(_lib.hlb_launch_count(self._h))
+        return int(self._call(_lib.hlb_launch_count))
 
     def hlb_offset_bits(self) -> int:
-        return int(_lib.hlb_offset_bits(self._h))
+        return int(self._call(_lib.hlb_offset_bits))
 
     def hlb_uses_aa(self) -> bool:
-        return bool(_lib.hlb_uses_aa(self._h))
+        return bool(self._call(_lib.hlb_uses_aa))
 
     def hlb_uses_records(self) -> bool:
-        return bool(_lib.hlb_uses_records(self._h))
+        return bool(self._call(_lib.hlb_uses_records))
 
     def hlb_record_sentinel_fraction(self) -> float:
-        return float(_lib.hlb_record_sentinel_fraction(self._h))
+        return float(self._call(_lib.hlb_record_sentinel_fraction))
 
     def hlb_geometry_destroy(self):
         if self._h:
             self._torch.cuda.synchronize(self.device)
-            _lib.hlb_geometry_destroy(self._h)
+            self._call(_lib.hlb_geometry_destroy)
             self._h = ctypes.c_void_p(None)
             self._buffers.clear()
 

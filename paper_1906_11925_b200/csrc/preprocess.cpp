@@ -102,6 +102,9 @@ struct BlockIndex {
 }  // namespace
 
 int preprocess_threads() { return thread_count(); }
+void host_parallel_for(int64_t n, int64_t grain, const std::function<void(int64_t, int64_t)>& fn) {
+  parallel_for(n, grain, [&](int64_t b, int64_t e) { fn(b, e); });
+}
 
 // A group is 32 consecutive sites (one warp). For link q of a group, the lanes whose pull
 // source is a fluid site split into runs of lanes with consecutive source indices; with an

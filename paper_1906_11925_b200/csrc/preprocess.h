@@ -2,6 +2,7 @@
 // pull-neighbour table. Subsystem (b) of BASELINE.json north_star; SURVEY.md §8(a) row S0.
 #pragma once
 #include <cstdint>
+#include <functional>
 #include <string>
 #include <vector>
 
@@ -44,5 +45,10 @@ int64_t build_link_records(const int32_t* nbr, int n_links, int64_t Ns, uint32_t
 inline int iolet_row_bytes(int Q) { return (Q - 1 + 15) / 16 * 16; }
 
 int preprocess_threads();
+
+// fn(begin, end) over [0, n) in chunks of `grain`, dynamically scheduled on the preprocessor's
+// host threads (HLB_THREADS, else the hardware concurrency); also used by the set-up calls of
+// the API that loop over all sites.
+void host_parallel_for(int64_t n, int64_t grain, const std::function<void(int64_t, int64_t)>& fn);
 
 }  // namespace hlb

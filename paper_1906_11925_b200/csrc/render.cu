@@ -29,9 +29,14 @@ struct ViewParams {
   float zoom, step, tf_scale, tf_offset, opacity;
 };
 
-// "GPU constant memory buffers" for the look-up table and the viewing parameters
-__constant__ float c_lut[256 * 4];
-__constant__ ViewParams c_view;
+// "GPU constant memory buffers" for the look-up table and the viewing parameters: both
+// travel as ONE by-value kernel argument, which the hardware serves from the constant bank of
+// that launch -- not from module-global __constant__ arrays, which two geometries (or two host
+// threads) rendering on different streams would overwrite under each other's running kernels.
+struct RenderParams {
+  ViewParams v;
+  float lut[256 * 4];
+};
 
 __device__ __forceinline__ float clamp01(float x) { return x < 0.0f ? 0.0f : (x > 1.0f ? 1.0f : x); }
 
@@ -39,19 +44,29 @@ __device__ __forceinline__ float lerp_rn(float f, float a, float b) {  // a + f 
   return __fmaf_rn(f, __fsub_rn(b, a), a);
 }
 
-__device__ __forceinline__ float trilinear(const float* __restrict__ vol, int nx, int ny, int nz,
-                                           float px, float py, float pz) {
+// The volume: a plain float array read through the read-only cache (TEX = false), or a 3-D
+// CUDA array behind a POINT-sampled texture object (TEX = true; the paper keeps its volume "in
+// a 3D texture unit"). Either way the eight corner values are fetched exactly and the
+// interpolation below is the same arithmetic, so the two give bit-identical images; the
+// texture's own (8-bit-weight) filtering is not used.
+template <bool TEX>
+__device__ __forceinline__ float voxel_at(const float* __restrict__ vol, cudaTextureObject_t tex,
+                                          int nx, int ny, int x, int y, int z) {
+  if (TEX) return tex3D<float>(tex, (float)x + 0.5f, (float)y + 0.5f, (float)z + 0.5f);
+  return __ldg(vol + ((long long)z * ny + y) * nx + x);
+}
+template <bool TEX>
+__device__ __forceinline__ float trilinear(const float* __restrict__ vol, cudaTextureObject_t tex,
+                                           int nx, int ny, int nz, float px, float py, float pz) {
   int ix = (int)floorf(px), iy = (int)floorf(py), iz = (int)floorf(pz);
   ix = min(ix, nx - 2); iy = min(iy, ny - 2); iz = min(iz, nz - 2);
   ix = max(ix, 0); iy = max(iy, 0); iz = max(iz, 0);
   const float fx = __fsub_rn(px, (float)ix), fy = __fsub_rn(py, (float)iy), fz = __fsub_rn(pz, (float)iz);
   const int x1 = ix + 1 < nx ? ix + 1 : ix, y1 = iy + 1 < ny ? iy + 1 : iy, z1 = iz + 1 < nz ? iz + 1 : iz;
-  const long long r00 = ((long long)iz * ny + iy) * nx, r10 = ((long long)iz * ny + y1) * nx,
-                  r01 = ((long long)z1 * ny + iy) * nx, r11 = ((long long)z1 * ny + y1) * nx;
-  const float c00 = lerp_rn(fx, __ldg(vol + r00 + ix), __ldg(vol + r00 + x1));
-  const float c10 = lerp_rn(fx, __ldg(vol + r10 + ix), __ldg(vol + r10 + x1));
-  const float c01 = lerp_rn(fx, __ldg(vol + r01 + ix), __ldg(vol + r01 + x1));
-  const float c11 = lerp_rn(fx, __ldg(vol + r11 + ix), __ldg(vol + r11 + x1));
+  const float c00 = lerp_rn(fx, voxel_at<TEX>(vol, tex, nx, ny, ix, iy, iz), voxel_at<TEX>(vol, tex, nx, ny, x1, iy, iz));
+  const float c10 = lerp_rn(fx, voxel_at<TEX>(vol, tex, nx, ny, ix, y1, iz), voxel_at<TEX>(vol, tex, nx, ny, x1, y1, iz));
+  const float c01 = lerp_rn(fx, voxel_at<TEX>(vol, tex, nx, ny, ix, iy, z1), voxel_at<TEX>(vol, tex, nx, ny, x1, iy, z1));
+  const float c11 = lerp_rn(fx, voxel_at<TEX>(vol, tex, nx, ny, ix, y1, z1), voxel_at<TEX>(vol, tex, nx, ny, x1, y1, z1));
   return lerp_rn(fz, lerp_rn(fy, c00, c10), lerp_rn(fy, c01, c11));
 }
 
@@ -63,10 +78,13 @@ constexpr int TILE = 16;
 // the transfer function gives value 0 no opacity, it contributes exactly nothing and may be
 // skipped, together with the following samples that provably stay in the same cell. The
 // image is therefore bit-identical with and without occ.
+template <bool TEX>
 __global__ void __launch_bounds__(TILE * TILE)
-k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ, float* __restrict__ image) {
+k_raymarch(const __grid_constant__ RenderParams par, const float* __restrict__ vol, cudaTextureObject_t tex,
+           const unsigned char* __restrict__ occ, float* __restrict__ image) {
   const int px = blockIdx.x * TILE + threadIdx.x, py = blockIdx.y * TILE + threadIdx.y;
-  const ViewParams& v = c_view;
+  const ViewParams& v = par.v;
+  const float* c_lut = par.lut;
   if (px >= v.width || py >= v.height) return;
   const float fnx = (float)v.nx, fny = (float)v.ny, fnz = (float)v.nz;
   const float cx = __fmul_rn(0.5f, (float)(v.nx - 1)), cy = __fmul_rn(0.5f, (float)(v.ny - 1)),
@@ -155,7 +173,7 @@ k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ,
         continue;
       }
     }
-    const float val = trilinear(vol, v.nx, v.ny, v.nz, qx, qy, qz);
+    const float val = trilinear<TEX>(vol, tex, v.nx, v.ny, v.nz, qx, qy, qz);
     const float t = clamp01(__fmaf_rn(val, v.tf_scale, v.tf_offset));
     const int i = (int)__fmaf_rn(t, 255.0f, 0.5f);
     const float* e = c_lut + 4 * i;
@@ -173,7 +191,8 @@ k_raymarch(const float* __restrict__ vol, const unsigned char* __restrict__ occ,
 // volume[voxel of site c] = scalar field of site c (canonical order); the rest stays 0
 __global__ void __launch_bounds__(256)
 k_scatter_field(const double* __restrict__ rho, const double* __restrict__ u,
-                const long long* __restrict__ voxel, long long N, int field, float* __restrict__ vol) {
+                const long long* __restrict__ voxel, long long N, int field, float* __restrict__ vol,
+                cudaSurfaceObject_t surf, int nx, int ny) {
   const long long c = (long long)blockIdx.x * 256 + threadIdx.x;
   if (c >= N) return;
   double s;
@@ -185,27 +204,27 @@ k_scatter_field(const double* __restrict__ rho, const double* __restrict__ u,
     const double ux = u[3 * c], uy = u[3 * c + 1], uz = u[3 * c + 2];
     s = sqrt(ux * ux + uy * uy + uz * uz);
   }
-  vol[voxel[c]] = (float)s;
+  const long long v = voxel[c];
+  vol[v] = (float)s;
+  if (surf) {  // the same value into the 3-D array behind the texture object
+    const long long row = v / nx;
+    surf3Dwrite((float)s, surf, (int)(v - row * nx) * (int)sizeof(float), (int)(row % ny), (int)(row / ny));
+  }
 }
 
 }  // namespace
 
-cudaError_t render_upload(const RenderSetup& r, const float* lut_host, cudaStream_t s) {
-  ViewParams v;
+void launch_raymarch(const RenderSetup& r, const float* lut_host, const float* vol, cudaTextureObject_t tex,
+                     const unsigned char* occ, float* image, cudaStream_t s) {
+  RenderParams par;
+  ViewParams& v = par.v;
   v.nx = r.nx; v.ny = r.ny; v.nz = r.nz; v.width = r.width; v.height = r.height;
   for (int k = 0; k < 9; ++k) v.rot[k] = r.rot[k];
   v.zoom = r.zoom; v.step = r.step; v.tf_scale = r.tf_scale; v.tf_offset = r.tf_offset; v.opacity = r.opacity;
-  cudaError_t e = cudaMemcpyToSymbolAsync(c_view, &v, sizeof(v), 0, cudaMemcpyHostToDevice, s);
-  if (e != cudaSuccess) return e;
-  e = cudaMemcpyToSymbolAsync(c_lut, lut_host, sizeof(float) * 1024, 0, cudaMemcpyHostToDevice, s);
-  if (e != cudaSuccess) return e;
-  return cudaStreamSynchronize(s);  // v is a stack object; lut_host is the caller's
-}
-
-void launch_raymarch(const RenderSetup& r, const float* vol, const unsigned char* occ, float* image,
-                     cudaStream_t s) {
+  for (int k = 0; k < 1024; ++k) par.lut[k] = lut_host[k];
   const dim3 grid((unsigned)((r.width + TILE - 1) / TILE), (unsigned)((r.height + TILE - 1) / TILE));
-  k_raymarch<<<grid, dim3(TILE, TILE), 0, s>>>(vol, occ, image);
+  if (tex) k_raymarch<true><<<grid, dim3(TILE, TILE), 0, s>>>(par, vol, tex, occ, image);
+  else k_raymarch<false><<<grid, dim3(TILE, TILE), 0, s>>>(par, vol, tex, occ, image);
 }
 
 namespace {
@@ -261,8 +280,8 @@ void launch_occupancy(const float* vol, int nx, int ny, int nz, unsigned char* o
 }
 
 void launch_scatter_field(const double* rho, const double* u, const long long* voxel, long long N,
-                          int field, float* vol, cudaStream_t s) {
-  k_scatter_field<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(rho, u, voxel, N, field, vol);
+                          int field, float* vol, cudaSurfaceObject_t surf, int nx, int ny, cudaStream_t s) {
+  k_scatter_field<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(rho, u, voxel, N, field, vol, surf, nx, ny);
 }
 
 }  // namespace hlb
