@@ -339,6 +339,10 @@ __device__ __forceinline__ void bfl_prefetch(const BflFused& bf, long long idx) 
 #pragma unroll
   for (int b = 0; b < bfl_row<L>() * 8; b += 128) asm volatile("prefetch.global.L1 [%0];" ::"l"(row + b));
 }
+// a x + (1 - a) y, in the three-term form: at a = 1 (wall half a link away, d = 1/2) it returns x
+// exactly, so that BFL with d = 1/2 IS halfway bounce-back bit for bit (the two-operation form
+// y + a (x - y) is not, and gained 1 % where tried)
+__device__ __forceinline__ double lerp2(double a, double x, double y) { return fma_(a, x, mul(sub(1.0, a), y)); }
 template <typename L>
 __device__ __forceinline__ void bfl_gather(const BflFused& bf, long long idx, double (&h)[L::Q]) {
   const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
@@ -346,8 +350,8 @@ __device__ __forceinline__ void bfl_gather(const BflFused& bf, long long idx, do
   for (int k = 0; k < (L::Q - 1) / 2; ++k) {
     const double2 c = __ldg(row + k);
     const int p = 2 * k + 1;
-    if (c.x > 0.0) h[p] = fma_(c.x, h[p], mul(sub(1.0, c.x), h[opp(p)]));
-    if (c.y > 0.0) h[p + 1] = fma_(c.y, h[p + 1], mul(sub(1.0, c.y), h[opp(p + 1)]));
+    if (c.x > 0.0) h[p] = lerp2(c.x, h[p], h[opp(p)]);
+    if (c.y > 0.0) h[p + 1] = lerp2(c.y, h[p + 1], h[opp(p + 1)]);
   }
 }
 // out[p]: the value written back for link p (the bounced h*_opp(p)); h: post-collision
@@ -359,8 +363,8 @@ __device__ __forceinline__ void bfl_write(const BflFused& bf, long long idx, con
   for (int k = 0; k < (L::Q - 1) / 2; ++k) {
     const double2 c = __ldg(row + k);
     const int p = 2 * k + 1;
-    if (c.x < 0.0) out[p] = fma_(-c.x, out[p], mul(sub(1.0, -c.x), h[p]));
-    if (c.y < 0.0) out[p + 1] = fma_(-c.y, out[p + 1], mul(sub(1.0, -c.y), h[p + 1]));
+    if (c.x < 0.0) out[p] = lerp2(-c.x, out[p], h[p]);
+    if (c.y < 0.0) out[p + 1] = lerp2(-c.y, out[p + 1], h[p + 1]);
   }
 }
 // two-lattice: the value written back for link p is h[opp(p)] itself
@@ -371,8 +375,8 @@ __device__ __forceinline__ void bfl_write_pull(const BflFused& bf, long long idx
   for (int k = 0; k < (L::Q - 1) / 2; ++k) {
     const double2 c = __ldg(row + k);
     const int p = 2 * k + 1;
-    if (c.x < 0.0) h[opp(p)] = fma_(-c.x, h[opp(p)], mul(sub(1.0, -c.x), h[p]));
-    if (c.y < 0.0) h[opp(p + 1)] = fma_(-c.y, h[opp(p + 1)], mul(sub(1.0, -c.y), h[p + 1]));
+    if (c.x < 0.0) h[opp(p)] = lerp2(-c.x, h[opp(p)], h[p]);
+    if (c.y < 0.0) h[opp(p + 1)] = lerp2(-c.y, h[opp(p + 1)], h[p + 1]);
   }
 }
 
@@ -444,10 +448,10 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
       const double two_d = mul(2.0, dd[k]);
       double r;
       if (dd[k] < 0.5) {
-        r = fma_(two_d, a[k], mul(sub(1.0, two_d), b[k]));
+        r = lerp2(two_d, a[k], b[k]);
       } else {
         const double inv = __ddiv_rn(1.0, two_d);
-        r = fma_(inv, a[k], mul(sub(1.0, inv), b[k]));
+        r = lerp2(inv, a[k], b[k]);
       }
       buf[tgt[k]] = to_store<ST>(r);
     }
@@ -951,11 +955,16 @@ static void launch_step(const DeviceGeometry& g, void (*kernel)(KArgs...), cudaS
 #else
 #define HLB_FULL_ONLY(...) __VA_ARGS__
 #endif
+#if defined(HLB_TUNE_MIN) && !defined(HLB_TUNE_BFL)
+#define HLB_BFL_ONLY(...) HLB_FULL_ONLY(__VA_ARGS__)
+#else
+#define HLB_BFL_ONLY(...) __VA_ARGS__   // (-DHLB_TUNE_BFL: a tuning build that keeps the V = 2 kernels)
+#endif
 template <typename L, typename ST, bool REC, typename IT>
 static void pull_launch(const DeviceGeometry& g, const void* src, void* dst, cudaStream_t s) {
 #define HLB_PULL_ARGS s, (const ST*)src, (ST*)dst, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, \
                       (long long)g.Ns, make_relax<L>(g.omega), planes_of(g), (long long)g.prefetch_pull, g.bflf
-  if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 2>, HLB_PULL_ARGS));
+  if (g.bfl_on) HLB_BFL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 2>, HLB_PULL_ARGS));
   else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_pull<L, ST, REC, IT, 1>, HLB_PULL_ARGS));
   else launch_step(g, k_pull<L, ST, REC, IT, 0>, HLB_PULL_ARGS);
 #undef HLB_PULL_ARGS
@@ -975,7 +984,7 @@ template <typename L, typename ST, bool REC, typename IT>
 static void aa_odd_launch(const DeviceGeometry& g, void* a, cudaStream_t s) {
 #define HLB_ODD_ARGS s, (ST*)a, g.nbr, (const uint4*)g.rec, iolet_index(g), g.iolet_par, (long long)g.Ns, \
                      make_relax<L>(g.omega), planes_of(g), (long long)g.prefetch_aa, g.bflf
-  if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 2>, HLB_ODD_ARGS));
+  if (g.bfl_on) HLB_BFL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 2>, HLB_ODD_ARGS));
   else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_aa_odd<L, ST, REC, IT, 1>, HLB_ODD_ARGS));
   else launch_step(g, k_aa_odd<L, ST, REC, IT, 0>, HLB_ODD_ARGS);
 #undef HLB_ODD_ARGS
@@ -986,7 +995,7 @@ static void aa_t(const DeviceGeometry& g, void* a, bool odd, cudaStream_t s) {
   if (!odd) {
 #define HLB_EVEN_ARGS s, (ST*)a, iolet_index(g), g.iolet_par, (long long)g.Ns, make_relax<L>(g.omega), \
                       (long long)g.prefetch_aa, g.bflf
-    if (g.bfl_on) HLB_FULL_ONLY(launch_step(g, k_aa_even<L, ST, 2>, HLB_EVEN_ARGS));
+    if (g.bfl_on) HLB_BFL_ONLY(launch_step(g, k_aa_even<L, ST, 2>, HLB_EVEN_ARGS));
     else if (g.iolet_full) HLB_FULL_ONLY(launch_step(g, k_aa_even<L, ST, 1>, HLB_EVEN_ARGS));
     else launch_step(g, k_aa_even<L, ST, 0>, HLB_EVEN_ARGS);
 #undef HLB_EVEN_ARGS
