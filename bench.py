@@ -402,12 +402,13 @@ def default_variant(**kw):
 class Run:
     """One geometry on the device in one variant, with the timing helpers of a bench line."""
 
-    def __init__(self, hlb, W, wl, name, v, world=1, local_rank=0):
+    def __init__(self, hlb, W, wl, name, v, world=1, local_rank=0, copy_stream=False):
         import torch
         self.torch, self.hlb, self.W, self.name, self.v = torch, hlb, W, name, v
         self.world, self.local_rank = world, local_rank
         t0 = time.perf_counter()
-        self.g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, variant_flags(hlb, v))
+        self.g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, variant_flags(hlb, v),
+                                         copy_stream=torch.cuda.Stream() if copy_stream else None)
         torch.cuda.synchronize()
         self.t_create = time.perf_counter() - t0
         g = self.g
@@ -642,7 +643,7 @@ def main():
     t_gen = time.perf_counter()
     wl = W.by_name(args.workload, small=args.small)
     t_gen = time.perf_counter() - t_gen
-    run = Run(hlb, W, wl, args.workload, v, world, local_rank)
+    run = Run(hlb, W, wl, args.workload, v, world, local_rank, copy_stream=not args.no_e2e)
     g, N, S, nq = run.g, run.N, args.inner, run.nq
     scheme = run.v["scheme"]          # what HLB_SCHEME_AUTO took, if that was asked for
 
@@ -656,31 +657,37 @@ def main():
     if not args.no_e2e and 128 * N > 16e9:
         args.no_e2e = True          # four pinned host arrays of 32 N bytes: not at this size
     if not args.no_e2e:
-        rho_h = torch.empty(N, dtype=torch.float64).pin_memory()
-        u_h = torch.empty((N, 3), dtype=torch.float64).pin_memory()
+        # pinned host buffers: the inputs of every step, and two sets of outputs (the read-out of
+        # step k is copied back on the copy stream while step k + 1 uploads and runs)
         rho_in = torch.ones(N, dtype=torch.float64).pin_memory()
         u_in = torch.zeros((N, 3), dtype=torch.float64).pin_memory()
         if wl.rho0 is not None:
             rho_in.numpy()[:] = wl.rho0
         if wl.u0 is not None:
             u_in.numpy()[:] = wl.u0
-        rho_np, u_np, rin_np, uin_np = rho_h.numpy(), u_h.numpy(), rho_in.numpy(), u_in.numpy()
+        outs = [(torch.empty(N, dtype=torch.float64).pin_memory(), torch.empty((N, 3), dtype=torch.float64).pin_memory())
+                for _ in range(2)]
+        outs_np = [(r.numpy(), uu.numpy()) for r, uu in outs]
+        rin_np, uin_np = rho_in.numpy(), u_in.numpy()
 
-        def e2e_step():
-            g.hlb_set_state(rin_np, uin_np)             # H2D: rho [N], u [N][3]
+        def e2e_step(k):
+            g.hlb_set_state(rin_np, uin_np)                   # H2D: rho [N], u [N][3]
             run.advance(S)
-            g.hlb_get_macroscopic(rho_np, u_np)        # D2H: rho [N], u [N][3] (synchronises)
+            g.hlb_get_macroscopic_async(*outs_np[k & 1])      # D2H: rho [N], u [N][3], on the copy stream
 
         e2e_steps = max(2, min(args.steps, 5))
-        e2e_step()
+        e2e_step(0)
+        g.hlb_wait_copies()
         run.barrier()
         t0 = time.perf_counter()
-        for _ in range(e2e_steps):
-            e2e_step()
+        for k in range(e2e_steps):
+            e2e_step(k)
+        g.hlb_wait_copies()                                   # every step's result is on the host
         run.barrier()
         t_e2e = time.perf_counter() - t0
         e2e = (t_e2e, e2e_steps)
-        del rho_h, u_h, rho_in, u_in
+        assert np.all(np.isfinite(outs_np[(e2e_steps - 1) & 1][0][:1000]))
+        del rho_in, u_in, outs, outs_np
 
     # ---------------- aggregate over ranks (max time; total work)
     ms_all, e2e_all = max_over_ranks([ms, e2e[0] if e2e else 0.0], world, dev)
@@ -722,7 +729,10 @@ def main():
         out["e2e"] = {"value": replicas_value(N, S * e2e[1], world, e2e_all), "unit": UNIT,
                       "h2d_bytes_per_step": 32 * N, "d2h_bytes_per_step": 32 * N,
                       "steps": e2e[1], "ms_per_step": e2e_all / e2e[1] * 1e3,
-                      "what": "hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic(host rho,u), pinned buffers"}
+                      "what": "per step: hlb_set_state(host rho,u) + hlb_step(S) + hlb_get_macroscopic_async(host "
+                              "rho,u) from / to pinned buffers through the C-ABI; the device-to-host copy of "
+                              "step k runs on a second stream under the upload and the LB steps of step k+1; "
+                              "hlb_wait_copies() before the clock stops"}
     if args.render > 0:
         out["render"] = time_renderer(hlb, g, wl, args.workload, args.render, args.render_view)
     run.close()

@@ -116,6 +116,9 @@ typedef struct {
   void* stream;            /* cudaStream_t as void*; NULL = the legacy default stream      */
   hlb_free_fn free;        /* optional (NULL): releases one buffer of `alloc` early; called
                               with alloc_user                                              */
+  void* copy_stream;       /* optional (NULL): a second cudaStream_t of the caller, used only by
+                              hlb_get_macroscopic_async for its device-to-host copies, so that
+                              they overlap the next upload / steps on `stream`             */
 } hlb_params;
 
 /* Build the geometry: extract the fluid sites, order them, build the int32 pull-neighbour
@@ -157,7 +160,12 @@ int hlb_set_iolet_normal(hlb_geometry* g, const double* normals);
  * the interpolation off. The step kernels of both schemes apply it in registers (the d >= 1/2
  * rule to the value a site writes back, the d < 1/2 rule to the values it gathers; no extra
  * launch per step); a read-out between steps first runs a pre-pass kernel over the d < 1/2
- * links of the state buffer. Only while hlb_steps_done() == 0
+ * links of the state buffer. With HLB_STORE_F64 the pre-pass writes exactly what the next step
+ * would have computed in registers, so reading out does not change the run. With HLB_STORE_F32
+ * it rounds those interpolated values to binary32 one step earlier than a run without the
+ * read-out would: a read-out (hlb_get_macroscopic, _stress, _populations, hlb_render) then
+ * perturbs the trajectory at the level of the storage rounding itself (~1e-8 relative, inside
+ * the 1e-5 bar; tests/test_gpu_parity.py). Only while hlb_steps_done() == 0
  * (after create / hlb_set_state / hlb_set_populations; it survives later hlb_set_state
  * calls). Allocates its tables through the allocator. Errors: HLB_EINVAL, HLB_ENOMEM,
  * HLB_ECUDA. hlb_num_bfl_sites: sites with at least one interpolated link (0 when off). */
@@ -225,6 +233,14 @@ int hlb_step(hlb_geometry* g, int64_t n);
  * hlb_steps_done() steps (reading R-readout), canonical order.
  *   rho: HOST [N];  u: HOST [N][3]. Either may be NULL. Synchronises the stream. */
 int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u);
+/* The same, without waiting: the read-out kernel runs on `stream`, the copies to the HOST
+ * arrays (pinned memory, or they are not asynchronous) on params.copy_stream once it is
+ * done, and the call returns at once; work enqueued on `stream` afterwards (hlb_set_state,
+ * hlb_step) overlaps the copies. The arrays are valid after hlb_wait_copies(), which also any
+ * later hlb_get_macroscopic_async waits for before it reuses the staging buffer. Needs
+ * params.copy_stream (else HLB_EINVAL). */
+int hlb_get_macroscopic_async(hlb_geometry* g, double* rho, double* u);
+int hlb_wait_copies(hlb_geometry* g);
 
 /* Same, into DEVICE buffers (rho [N], u [N][3]); enqueued on the stream, no sync. */
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);

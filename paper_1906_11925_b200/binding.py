@@ -44,6 +44,7 @@ class hlb_params(ctypes.Structure):
         ("alloc_user", ctypes.c_void_p),
         ("stream", ctypes.c_void_p),
         ("free", _FREE_FN),
+        ("copy_stream", ctypes.c_void_p),
     ]
 
 
@@ -92,6 +93,8 @@ def _load() -> ctypes.CDLL:
         "hlb_step": (c_int, [vp, i64]),
         "hlb_get_macroscopic": (c_int, [vp, vp, vp]),
         "hlb_get_macroscopic_device": (c_int, [vp, vp, vp]),
+        "hlb_get_macroscopic_async": (c_int, [vp, vp, vp]),
+        "hlb_wait_copies": (c_int, [vp]),
         "hlb_get_populations": (c_int, [vp, vp]),
         "hlb_get_stress": (c_int, [vp, vp]),
         "hlb_get_stress_device": (c_int, [vp, vp]),
@@ -131,7 +134,8 @@ LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_set_iolet_velocity", "hlb_set_iolet_waveform", "hlb_set_iolet_weight", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
-            "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_populations",
+            "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_macroscopic_async", "hlb_wait_copies",
+            "hlb_get_populations",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
@@ -239,7 +243,7 @@ class Geometry:
     """Owner of one hlb_geometry handle and of the torch buffers behind it."""
 
     def __init__(self, site_type, periodic=0, tau=1.0, iolet_rho=(), flags=0, device=None,
-                 stream=None):
+                 stream=None, copy_stream=None):
         import torch
         if not torch.cuda.is_available():
             raise HlbError(HLB_ECUDA, "no CUDA device: the site update has no CPU fallback")
@@ -272,6 +276,8 @@ class Geometry:
         with torch.cuda.device(self.device):
             self.stream = torch.cuda.current_stream() if stream is None else stream
             p.stream = self.stream.cuda_stream
+            self.copy_stream = copy_stream     # a torch.cuda.Stream for hlb_get_macroscopic_async
+            p.copy_stream = copy_stream.cuda_stream if copy_stream is not None else None
             _check(_lib.hlb_geometry_create(_ptr(st), ctypes.byref(p), ctypes.byref(self._h)))
         self.n_sites = int(_lib.hlb_num_sites(self._h))
         self.n_q = int(_lib.hlb_num_q(self._h))
@@ -343,6 +349,19 @@ class Geometry:
                 raise ValueError(f"output array must be a writable C-contiguous float64 array of shape {shape}")
         _check(self._call(_lib.hlb_get_macroscopic, _ptr(rho), _ptr(u)))
         return rho, u
+
+    def hlb_get_macroscopic_async(self, rho_out, u_out):
+        """Read-out into caller-owned PINNED host arrays without waiting (needs copy_stream);
+        valid after hlb_wait_copies()."""
+        n = self.n_sites
+        for a, shape in ((rho_out, (n,)), (u_out, (n, 3))):
+            if a is not None and not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.shape == shape
+                                      and a.flags.c_contiguous and a.flags.writeable):
+                raise ValueError(f"output array must be a writable C-contiguous float64 array of shape {shape}")
+        _check(self._call(_lib.hlb_get_macroscopic_async, _ptr(rho_out), _ptr(u_out)))
+
+    def hlb_wait_copies(self):
+        _check(self._call(_lib.hlb_wait_copies))
 
     def hlb_get_macroscopic_device(self):
         """rho [N], u [N,3] as torch cuda tensors (canonical order), stream-ordered."""

@@ -75,6 +75,10 @@ struct hlb_geometry {
   void* buf[2] = {nullptr, nullptr};  // population arrays [15][Ns]; A-A uses buf[0] only
   int cur = 0;                        // two-lattice: buffer the next step reads
   double* scratch = nullptr;          // [4 N] doubles: staging of rho [N], u [N][3] transfers
+  cudaStream_t copy_stream = nullptr; // params.copy_stream (hlb_get_macroscopic_async)
+  double* scratch_out = nullptr;      // [4 N] doubles: its own staging buffer (lazy), so that an
+                                      // upload through `scratch` may overlap the copies
+  cudaEvent_t ev_ready = nullptr, ev_copied = nullptr;  // read-out done / copies done
   double* scratch_pop = nullptr;      // [N][15] doubles, allocated by the first
                                       // hlb_get_populations / hlb_set_populations call
   int64_t steps = 0, launches = 0, device_bytes = 0;
@@ -314,6 +318,7 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->p = *p;
   g->p.iolet_rho = nullptr;
   g->stream = (cudaStream_t)p->stream;
+  g->copy_stream = (cudaStream_t)p->copy_stream;
   g->aa = (p->flags & HLB_AA) != 0;
   if (p->flags & HLB_SCHEME_AUTO) {
     // A-A everywhere except where the resident multi-step kernel applies (there two-lattice
@@ -434,6 +439,11 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
 void hlb_geometry_destroy(hlb_geometry* g) {
   if (!g) return;
   if (g->graph_exec) cudaGraphExecDestroy(g->graph_exec);
+  if (g->ev_ready) {
+    cudaStreamSynchronize(g->copy_stream);
+    cudaEventDestroy(g->ev_ready);
+    cudaEventDestroy(g->ev_copied);
+  }
   if (g->vol_array) {
     cudaStreamSynchronize(g->stream);
     if (g->vol_tex) cudaDestroyTextureObject(g->vol_tex);
@@ -852,6 +862,40 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u) {
   if (rho) HLB_CUDA(cudaMemcpyAsync(rho, d_rho, sizeof(double) * n, cudaMemcpyDeviceToHost, g->stream));
   if (u) HLB_CUDA(cudaMemcpyAsync(u, d_u, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
+int hlb_get_macroscopic_async(hlb_geometry* g, double* rho, double* u) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (!g->copy_stream) return fail(HLB_EINVAL, "hlb_get_macroscopic_async needs params.copy_stream");
+  if (!rho && !u) return HLB_OK;
+  const size_t n = (size_t)g->N;
+  if (!g->scratch_out) {
+    void* ptr = nullptr;
+    const int rc = g->alloc(sizeof(double) * 4 * n, &ptr);
+    if (rc) return rc;
+    g->scratch_out = (double*)ptr;
+    HLB_CUDA(cudaEventCreateWithFlags(&g->ev_ready, cudaEventDisableTiming));
+    HLB_CUDA(cudaEventCreateWithFlags(&g->ev_copied, cudaEventDisableTiming));
+    HLB_CUDA(cudaEventRecord(g->ev_copied, g->copy_stream));
+  }
+  // the previous copies out of the staging buffer must be done before it is rewritten
+  HLB_CUDA(cudaStreamWaitEvent(g->stream, g->ev_copied, 0));
+  double* d_rho = g->scratch_out;
+  double* d_u = g->scratch_out + n;
+  int rc = hlb_get_macroscopic_device(g, rho ? d_rho : nullptr, u ? d_u : nullptr);
+  if (rc) return rc;
+  HLB_CUDA(cudaEventRecord(g->ev_ready, g->stream));
+  HLB_CUDA(cudaStreamWaitEvent(g->copy_stream, g->ev_ready, 0));
+  if (rho) HLB_CUDA(cudaMemcpyAsync(rho, d_rho, sizeof(double) * n, cudaMemcpyDeviceToHost, g->copy_stream));
+  if (u) HLB_CUDA(cudaMemcpyAsync(u, d_u, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, g->copy_stream));
+  HLB_CUDA(cudaEventRecord(g->ev_copied, g->copy_stream));
+  return HLB_OK;
+}
+
+int hlb_wait_copies(hlb_geometry* g) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (g->copy_stream && g->ev_ready) HLB_CUDA(cudaStreamSynchronize(g->copy_stream));
   return HLB_OK;
 }
 

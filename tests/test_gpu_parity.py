@@ -548,6 +548,33 @@ def test_bfl_at_half_a_link_is_bounce_back_bitwise_and_argument_errors(hlb, sche
     b.close()
 
 
+@pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
+def test_bfl_read_outs_between_steps(hlb, scheme):
+    """include/hlb.h, hlb_set_wall_distance: a read-out between steps runs the d < 1/2 pre-pass
+    on the state buffer. In fp64 storage that changes nothing (bitwise); in fp32 storage it
+    rounds the interpolated values one step early -- a perturbation of the size of the storage
+    rounding, which must stay inside the fp32 bar against the oracle."""
+    wl = W.with_bfl_walls(W.by_name("aneurysm", small=True))
+    steps = 40
+    rho_ref, u_ref = run_oracle(wl, steps, threads=1)
+    for store in ("f64", "f32"):
+        plain = run_gpu(hlb, wl, steps, scheme, store, "auto")
+        g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                    flags_of(hlb, scheme, store, "auto"))
+        g.hlb_set_wall_distance(wl.wall_distance)
+        for _ in range(steps // 4):
+            g.hlb_step(3)
+            g.hlb_get_macroscopic()          # odd and even step counts
+            g.hlb_step(1)
+            g.hlb_get_populations()
+        monitored = g.hlb_get_macroscopic()
+        g.close()
+        if store == "f64":
+            assert np.array_equal(plain[0], monitored[0]) and np.array_equal(plain[1], monitored[1])
+        e_rho, e_u = errors(*monitored, rho_ref, u_ref)
+        assert e_rho < TOL[store] and e_u < TOL[store], (store, e_rho, e_u)
+
+
 def test_bfl_is_the_same_in_both_schemes(hlb):
     """Two-lattice and A-A apply the same interpolation to the same values: populations after
     even and odd step counts agree to rounding (the two schemes round alike, see the bitwise
@@ -875,6 +902,34 @@ def test_state_round_trip_and_iolet_update(hlb):
         e_rho, e_u = errors(*g.hlb_get_macroscopic(), *o.get_macroscopic())
         assert e_rho < 1e-12 and e_u < 1e-12
         g.close()
+
+
+def test_asynchronous_read_out_on_a_copy_stream(hlb):
+    """hlb_get_macroscopic_async + hlb_wait_copies (include/hlb.h): the same numbers as the
+    synchronous read-out, also when the next upload and steps are enqueued before the copies
+    are waited for; without a copy stream the call is refused."""
+    import torch
+    wl = W.by_name("tree", small=True)
+    n = wl.n_sites
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, "aa", "f64", "auto"), copy_stream=torch.cuda.Stream())
+    outs = [(torch.empty(n, dtype=torch.float64).pin_memory().numpy(),
+             torch.empty((n, 3), dtype=torch.float64).pin_memory().numpy()) for _ in range(2)]
+    want = []
+    for k, steps in enumerate((7, 12)):
+        g.hlb_set_state(None, None)
+        g.hlb_step(steps)
+        g.hlb_get_macroscopic_async(*outs[k])      # not waited for: the next round is enqueued behind it
+        want.append(run_gpu(hlb, wl, steps, "aa", "f64", "auto"))
+    g.hlb_wait_copies()
+    for k in range(2):
+        assert np.array_equal(outs[k][0], want[k][0]) and np.array_equal(outs[k][1], want[k][1])
+    g.close()
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags_of(hlb, "aa", "f64", "auto"))
+    with pytest.raises(hlb.HlbError) as e:
+        g.hlb_get_macroscopic_async(*outs[0])
+    assert e.value.code == hlb.HLB_EINVAL
+    g.close()
 
 
 def test_degenerate_geometries(hlb):
