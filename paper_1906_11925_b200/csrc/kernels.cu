@@ -209,7 +209,7 @@ __device__ __forceinline__ long long slot_of(int q, int32_t e, long long Ns, lon
 
 // The iolet index of a group of 32 sites (preprocess.h): {bits, rank}. Loaded at the very top
 // of every step kernel -- ncu showed 12-24 % of a warp's lifetime spent waiting for this word
-// when it was loaded where it is used, after the collision (profiles/r02_ncu_step_kernels.md).
+// when it was loaded where it is used, after the collision (profiles/r02_tuning.md section 1).
 struct IoletIndex {
   const uint2* idx = nullptr;    // [Ns/32] {bits, rank}
   const uint4* links = nullptr;  // [iolet sites][iolet_row<L>() uint4]: byte p - 1 = k + 1 or 0
