@@ -262,6 +262,26 @@ int hlb_get_stress_device(hlb_geometry* g, double* sigma_dev);
  *   wss:     HOST [N]. Synchronises the stream. */
 int hlb_get_wall_shear_stress(hlb_geometry* g, const double* normals, double* wss);
 
+/* The same wall shear stress for callers that must not allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): this call allocates NOTHING
+ * -- no cudaMalloc / cudaFree, no allocator callback, no allocating library routine -- and does
+ * not synchronise. Its only scratch, the stress tensor sigma [N][6] between the two kernels, lives
+ * in a file-scope static __device__ array of HLB_NOALLOC_MAX_SITES x 6 doubles (12 MiB) that
+ * every GPU which loads the library holds until the process exits; its device address is taken
+ * once per device when a geometry is created on it.
+ *   normals: DEVICE [N][3] canonical order (as hlb_get_wall_shear_stress);  wss: DEVICE [N].
+ * Both are the caller's; the two kernels are enqueued on the geometry's stream.
+ * Limits: N <= HLB_NOALLOC_MAX_SITES (= hlb_noalloc_max_sites()), else HLB_ETOOLARGE and nothing
+ * is launched. ALL geometries of a process share the one array on a device: two such calls that
+ * overlap on the GPU (different streams, or graphs replayed concurrently) race on it -- order
+ * them. The array keeps the last call's contents; every element a call reads it has written
+ * itself first, so nothing needs clearing between calls.
+ * Errors: HLB_EINVAL (NULL argument), HLB_ETOOLARGE, HLB_ECUDA (launch error, or the address of
+ * the array could not be taken when the geometry was created: hlb_last_error says which). */
+#define HLB_NOALLOC_MAX_SITES 262144
+int hlb_get_wall_shear_stress_noalloc(hlb_geometry* g, const double* normals_dev, double* wss_dev);
+int64_t hlb_noalloc_max_sites(void);
+
 /* Pre-collision populations f_q(x) (not shifted) as fp64, HOST [N][Q], canonical site
  * order, q in the order of hlb_lattice(). For population-level parity checks. The
  * first call of this or of hlb_set_populations allocates a [N][Q] fp64 staging buffer

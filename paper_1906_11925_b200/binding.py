@@ -99,6 +99,8 @@ def _load() -> ctypes.CDLL:
         "hlb_get_stress": (c_int, [vp, vp]),
         "hlb_get_stress_device": (c_int, [vp, vp]),
         "hlb_get_wall_shear_stress": (c_int, [vp, vp, vp]),
+        "hlb_get_wall_shear_stress_noalloc": (c_int, [vp, vp, vp]),
+        "hlb_noalloc_max_sites": (i64, []),
         "hlb_render_volume": (c_int, [vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                                       ctypes.POINTER(hlb_view), vp, vp, vp]),
         "hlb_render": (c_int, [vp, ctypes.POINTER(hlb_view), vp, vp]),
@@ -136,7 +138,7 @@ EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_set_iolet_velocity", "hlb_set_iolet_waveform", "hlb_set_iolet_weight", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
             "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_macroscopic_async", "hlb_wait_copies",
             "hlb_get_populations",
-            "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_render_volume", "hlb_render",
+            "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_get_wall_shear_stress_noalloc", "hlb_noalloc_max_sites", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
             "hlb_set_populations", "hlb_num_sites", "hlb_num_q", "hlb_lattice", "hlb_steps_done", "hlb_get_site_voxels",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records", "hlb_uses_aa", "hlb_offset_bits",
@@ -187,6 +189,10 @@ def hlb_render_volume(volume, view: "hlb_view", lut):
     stream = torch.cuda.current_stream().cuda_stream
     _check(_lib.hlb_render_volume(_ptr(vol), nx, ny, nz, ctypes.byref(view), _ptr(lut), _ptr(img), stream))
     return img
+
+
+def hlb_noalloc_max_sites() -> int:
+    return int(_lib.hlb_noalloc_max_sites())
 
 
 def hlb_lattice(flags=0):
@@ -382,6 +388,17 @@ class Geometry:
         out = np.empty(self.n_sites, dtype=np.float64)
         _check(self._call(_lib.hlb_get_wall_shear_stress, _ptr(nrm), _ptr(out)))
         return out
+
+    def hlb_get_wall_shear_stress_noalloc(self, normals_dev, wss_dev):
+        """No-allocation variant (include/hlb.h): normals_dev [N, 3] and wss_dev [N] are the
+        caller's float64 CUDA tensors on this geometry's device; nothing is allocated, nothing
+        synchronised; N <= hlb_noalloc_max_sites()."""
+        torch = self._torch
+        for t, shape in ((normals_dev, (self.n_sites, 3)), (wss_dev, (self.n_sites,))):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.device == self.device and
+                    t.dtype == torch.float64 and tuple(t.shape) == shape and t.is_contiguous()):
+                raise ValueError(f"expected a contiguous float64 CUDA tensor of shape {shape} on {self.device}")
+        _check(self._call(_lib.hlb_get_wall_shear_stress_noalloc, normals_dev.data_ptr(), wss_dev.data_ptr()))
 
     def hlb_get_stress_device(self):
         torch = self._torch

@@ -93,6 +93,7 @@ struct hlb_geometry {
   cudaSurfaceObject_t vol_surf = 0;   // not the caller's allocator: CUDA arrays are opaque)
   float* d_image = nullptr;           // staging image for hlb_render
   size_t d_image_floats = 0;
+  cudaError_t noalloc_setup = cudaSuccess;  // result of noalloc_scratch_setup() at create
   bool bfl_set = false;               // wall distances given (hlb_set_wall_distance)
   int64_t bfl_sites = 0;              // sites with at least one interpolated link
   int64_t bfl_links = 0;              // interpolated links
@@ -426,6 +427,10 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->dg.omega = 1.0 / p->tau;
   g->dg.f32 = g->f32;
   g->dg.d3q19 = Q == 19;
+  // set-up of the static scratch of hlb_get_wall_shear_stress_noalloc: its device address, once
+  // per device, with this geometry's device current (kept, not fatal: only that call needs it)
+  g->noalloc_setup = noalloc_scratch_setup();
+  if (g->noalloc_setup != cudaSuccess) (void)cudaGetLastError();
   // the host tables die at the end of this call: finish the uploads first
   HLB_CUDA_G(cudaStreamSynchronize(g->stream));
   rc = hlb_set_state(g, nullptr, nullptr);
@@ -933,6 +938,31 @@ int hlb_get_wall_shear_stress(hlb_geometry* g, const double* normals, double* ws
   HLB_CUDA(cudaGetLastError());
   HLB_CUDA(cudaMemcpyAsync(wss, d_wss, sizeof(double) * n, cudaMemcpyDeviceToHost, g->stream));
   HLB_CUDA(cudaStreamSynchronize(g->stream));
+  return HLB_OK;
+}
+
+int64_t hlb_noalloc_max_sites(void) { return (int64_t)NOALLOC_MAX_SITES; }
+static_assert(NOALLOC_MAX_SITES == HLB_NOALLOC_MAX_SITES, "include/hlb.h and kernels.cuh disagree");
+
+int hlb_get_wall_shear_stress_noalloc(hlb_geometry* g, const double* normals_dev, double* wss_dev) {
+  if (!g || !normals_dev || !wss_dev) return fail(HLB_EINVAL, "NULL argument");
+  if (g->N > (int64_t)NOALLOC_MAX_SITES)
+    return fail(HLB_ETOOLARGE, "hlb_get_wall_shear_stress_noalloc: " + std::to_string((long long)g->N) +
+                               " sites exceed the static scratch of HLB_NOALLOC_MAX_SITES = " +
+                               std::to_string((long long)NOALLOC_MAX_SITES) +
+                               " sites; use hlb_get_wall_shear_stress");
+  if (g->noalloc_setup != cudaSuccess)
+    return cuda_fail(g->noalloc_setup, "cudaGetSymbolAddress(static scratch) at hlb_geometry_create");
+  double* d_sigma = noalloc_scratch();  // the DEVICE address taken at set-up, not the symbol's name
+  if (!d_sigma) return fail(HLB_ECUDA, "static scratch not set up on the current device "
+                                       "(the geometry was created on another one)");
+  // k_stress writes sigma[c][0..5] for every c < N, k_wall_shear_stress reads exactly those:
+  // nothing of an earlier call is read, nothing needs clearing. No allocation on this path
+  // (the BFL pre-pass, if due, is a plain launch).
+  const int rc = hlb_get_stress_device(g, d_sigma);
+  if (rc) return rc;
+  launch_wall_shear_stress(d_sigma, normals_dev, g->N, wss_dev, g->stream);
+  HLB_CUDA(cudaGetLastError());
   return HLB_OK;
 }
 

@@ -27,6 +27,7 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <tuple>
 
 #include "lbgk.cuh"
@@ -1149,6 +1150,39 @@ void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, do
                    cudaStream_t s) {
   dispatch(g, [&](auto l, auto st) { stress_t<decltype(l), decltype(st)>(g, buf, mode, sigma, s); });
 }
+// ------------------------------------------------------------------ static scratch (no-allocation entry point)
+// sigma [NOALLOC_MAX_SITES][6] of hlb_get_wall_shear_stress_noalloc. Uninitialised device
+// memory of the module (12 MiB per GPU that loads the library, until exit; not in the file).
+// Host code must NOT pass `g_noalloc_sigma` itself to a kernel -- in host code the name is a
+// host-side shadow of the symbol -- but the address cudaGetSymbolAddress returns for the device
+// that is current.
+static __device__ __align__(256) double g_noalloc_sigma[NOALLOC_MAX_SITES * 6];
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+double* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+std::mutex g_noalloc_mutex;
+}  // namespace
+cudaError_t noalloc_scratch_setup() {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (g_noalloc_ptr[dev]) return cudaSuccess;  // once per device
+  double* ptr = nullptr;
+  e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_sigma);
+  if (e != cudaSuccess) return e;
+  if (!ptr) return cudaErrorInvalidSymbol;
+  g_noalloc_ptr[dev] = ptr;
+  return cudaSuccess;
+}
+double* noalloc_scratch() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NOALLOC_MAX_DEVICES) return nullptr;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  return g_noalloc_ptr[dev];
+}
+
 void launch_wall_shear_stress(const double* sigma, const double* normals, long long N, double* wss,
                               cudaStream_t s) {
   k_wall_shear_stress<<<grid_for(N), BLOCK, 0, s>>>(sigma, normals, N, wss);

@@ -105,6 +105,14 @@ void launch_stress(const DeviceGeometry& g, const void* buf, GatherMode mode, do
 // wss [N] from sigma [N][6] and normals [N][3] (all device, canonical order)
 void launch_wall_shear_stress(const double* sigma, const double* normals, long long N, double* wss,
                               cudaStream_t s);
+// The static device scratch of hlb_get_wall_shear_stress_noalloc (include/hlb.h): `max_sites`
+// x 6 doubles in a file-scope __device__ array of kernels.cu. noalloc_scratch_setup() takes its
+// DEVICE address for the CURRENT device (cudaGetSymbolAddress; the array's name in host code is
+// only a host-side stand-in) and remembers it per device; call it at set-up, with the device
+// current. noalloc_scratch() returns the remembered address for the current device, or NULL.
+constexpr long long NOALLOC_MAX_SITES = 262144;
+cudaError_t noalloc_scratch_setup();
+double* noalloc_scratch();
 // f [N][Q] raw populations (device, canonical order)
 void launch_get_populations(const DeviceGeometry& g, const void* buf, GatherMode mode, double* f,
                             cudaStream_t s);
