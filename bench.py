@@ -46,7 +46,7 @@ METRIC_Q19 = "fluid site updates/sec (MSUPS), D3Q19 LBGK sparse site update"
 UNIT = "MSUPS"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 DEFAULT_SCHEME = {"pipe": "two_lattice", "cube": "two_lattice", "aneurysm": "two_lattice",
-                  "paper_sized": "two_lattice",
+                  "paper_sized": "two_lattice", "paper_sized_23": "two_lattice",
                   "tree": "two_lattice", "bigtree": "aa", "cube672": "aa", "bigtree_x": "aa"}
 WORKLOAD_DESC = {
     "pipe": "BASELINE configs[0]: pipe R=8 L=64",
@@ -55,6 +55,7 @@ WORKLOAD_DESC = {
     "tree": "BASELINE configs[3]: 5-level tree, 1024^3 box, r0=32",
     "bigtree": "BASELINE configs[4]: 5-level tree, 2048x2048x1024 box, r0=64",
     "paper_sized": "context only: aneurysm recipe scaled to ~297k sites (the paper's Subject 16, Table II)",
+    "paper_sized_23": "context only: aneurysm recipe scaled to ~133k sites (the paper's Subject 23, Table II)",
     "cube672": "context only: periodic 672^3 cube, 303.5 M sites (64-bit flat offsets: Q N > 2^32)",
     "bigtree_x": "context only: configs[4] generator at 77 um voxels (box and r0 x 1.3), 85.5 M sites "
                  "(BASELINE's nominal 80-100 M)",
@@ -568,6 +569,7 @@ SWEEP = [
     ("cube", {}, 200, 30),
     ("aneurysm", {}, 400, 35),
     ("paper_sized", {"lattice": "d3q19", "scheme": "auto"}, 500, 50),
+    ("paper_sized_23", {"lattice": "d3q19", "scheme": "auto"}, 1000, 60),
     ("tree", {}, 100, 24),
     ("tree", {"store": "f32"}, 100, 32),
     ("bigtree", {"scheme": "two_lattice"}, 50, 7),

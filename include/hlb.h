@@ -58,10 +58,11 @@ enum {
                               is h_q = f_q - w_q (reading R-shift)               */
   HLB_TWO_LATTICE = 0x0,   /* two population arrays, pull (gather) form                    */
   HLB_AA = 0x2,            /* one array updated in place, A-A pattern (even/odd steps)     */
-  HLB_SCHEME_AUTO = 0x1000,/* the library picks: A-A in place (one array; measured 2-25 %
-                              faster than two-lattice from 0.3 M sites up)
-                              unless the geometry is small enough for the resident multi-step
-                              kernel, where two-lattice is the faster one; overrides HLB_AA.
+  HLB_SCHEME_AUTO = 0x1000,/* the library picks: A-A in place (one array; measured 1-25 %
+                              faster than two-lattice above ~150 k sites), except where the
+                              resident multi-step kernel applies and where the grid is one
+                              wave of the two-lattice kernel but more than one of the A-A
+                              kernels (DESIGN.md section 6 item 17); overrides HLB_AA.
                               hlb_uses_aa() tells which was taken                          */
   HLB_ORDER_AUTO = 0x0,    /* internal site order: the library's choice -- currently raster,
                               the fastest measured on B200       */

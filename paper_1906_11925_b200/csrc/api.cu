@@ -322,14 +322,24 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
   g->copy_stream = (cudaStream_t)p->copy_stream;
   g->aa = (p->flags & HLB_AA) != 0;
   if (p->flags & HLB_SCHEME_AUTO) {
-    // A-A everywhere except where the resident multi-step kernel applies (there two-lattice
-    // is faster: 5.4 k vs 5.0 k MSUPS on configs[0]; profiles/r02_tuning.md)
+    // A-A in place (half the launches read no links; one array in L2 for the mid sizes) except
+    //  * where the resident multi-step kernel applies: two-lattice is the faster one there
+    //    (5.4 k vs 5.0 k MSUPS on configs[0]);
+    //  * where the whole grid is ONE wave of the two-lattice kernel (7 resident blocks per SM,
+    //    5 % slack) but more than one wave of the A-A kernels (6 per SM): the second, nearly
+    //    empty wave costs A-A 13 % at the paper's Subject-23 size (133 k sites).
+    // profiles/r02_tuning.md section 7.
     int dev = 0, sms = 0;
-    const bool resident = !(p->flags & (HLB_NO_GRAPH | HLB_NO_RESIDENT)) &&
-                          cudaGetDevice(&dev) == cudaSuccess &&
-                          cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+    const bool have = cudaGetDevice(&dev) == cudaSuccess &&
+                      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess;
+    const bool q19 = (p->flags & HLB_LATTICE_D3Q19) != 0;
+    const int64_t blocks = t.Ns / 128;
+    const int64_t slots_pull = (int64_t)sms * resident_sites_per_sm_pull(q19) / 128;
+    const int64_t slots_aa = (int64_t)sms * resident_sites_per_sm_aa(q19) / 128;
+    const bool resident = have && !(p->flags & (HLB_NO_GRAPH | HLB_NO_RESIDENT)) &&
                           t.Ns <= (int64_t)sms * resident_kernel_sites_per_sm();
-    g->aa = !resident;
+    const bool one_pull_wave = have && blocks > slots_aa && blocks * 100 <= slots_pull * 105;
+    g->aa = !(resident || one_pull_wave);
   }
   g->f32 = (p->flags & HLB_STORE_F32) != 0;
   g->Q = (p->flags & HLB_LATTICE_D3Q19) ? 19 : 15;

@@ -300,6 +300,20 @@ __device__ __forceinline__ void pdl_wait_for_previous_step() { asm volatile("gri
 __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
+// The gather kernels' prefetches: a warp's 32 addresses of one link cover two to four 128-byte
+// lines (one or two runs of consecutive sites), so only the lanes at which a line or a run can
+// begin need to ask. HLB_PF_LANES: 0 = every lane (round 1), 1 = lanes 0, 15, 16, 31 (8-byte
+// populations: line starts and ends of an aligned run, and both ends of the warp).
+// Table links (REC = false: Morton / tiled orders) gather anywhere: every lane asks.
+#ifndef HLB_PF_LANES
+#define HLB_PF_LANES 1   // +0.5 % on the two-lattice kernel, neutral elsewhere (profiles/r02_tuning.md section 11)
+#endif
+template <bool REC>
+__device__ __forceinline__ bool prefetch_lane() {
+  if (!REC || !HLB_PF_LANES) return true;
+  const unsigned l = threadIdx.x & 15u;
+  return l == 0u || l == 15u;
+}
 
 // The even A-A kernel reads Q planes at the block's own 128 sites: the block pf sites ahead
 // will read Q x (128 sizeof(ST) / 128) lines, one per thread -- one prefetch instruction per
@@ -498,9 +512,11 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
       asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
       if (REC && (threadIdx.x & 31) < ((L::Q - 1) * 16 + 31) / 32)
         prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (L::Q - 1)) + 32 * (threadIdx.x & 31));
-      prefetch_l2(ahead + i);
+      if (prefetch_lane<REC>()) {
+        prefetch_l2(ahead + i);
 #pragma unroll
-      for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
+        for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
+      }
     }
   }
   const int irow = iolet_row_of(iow);
@@ -601,9 +617,11 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
     asm volatile("" : "+l"(ahead));  // keep base + offset * size: one IMAD.WIDE per prefetch
     if (REC && (threadIdx.x & 31) < ((L::Q - 1) * 16 + 31) / 32)
       prefetch_l2((const char*)(rec + ((i + pf) >> 5) * (L::Q - 1)) + 32 * (threadIdx.x & 31));
-    prefetch_l2(ahead + i);
+    if (prefetch_lane<REC>()) {
+      prefetch_l2(ahead + i);
 #pragma unroll
-    for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
+      for (int q = 1; q < L::Q; ++q) prefetch_l2(ahead + off[q - 1]);
+    }
   }
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) opaque(off[q - 1]);

@@ -1099,10 +1099,20 @@ def test_scheme_auto_picks_and_matches_the_explicit_scheme(hlb):
         g.close()
         ref = run_gpu(hlb, wl, 31, "aa" if want_aa else "two_lattice", "f64", "auto")
         assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1])
-    big = W.by_name("paper_sized")                       # 296 k sites: beyond the resident kernel
-    g = hlb.hlb_geometry_create(big.site_type, big.periodic, big.tau, big.iolet_rho, hlb.HLB_SCHEME_AUTO)
-    assert g.hlb_uses_aa()
-    g.close()
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    for name, lattice in (("paper_sized", "d3q15"), ("paper_sized", "d3q19"), ("paper_sized_23", "d3q15"),
+                          ("paper_sized_23", "d3q19")):
+        big = W.by_name(name)
+        g = hlb.hlb_geometry_create(big.site_type, big.periodic, big.tau, big.iolet_rho,
+                                    hlb.HLB_SCHEME_AUTO | flags_of(hlb, "two_lattice", "f64", "auto", "auto", lattice, True))
+        # beyond the resident kernel: two-lattice only if the grid is one wave of the two-lattice
+        # kernel (7 blocks per SM for D3Q15, 5 for D3Q19; 5 % slack) and more than one of A-A (6 / 4)
+        blocks = -(-big.n_sites // 128)
+        per_sm_pull, per_sm_aa = (7, 6) if lattice == "d3q15" else (5, 4)
+        want_aa = not (blocks > sms * per_sm_aa and blocks * 100 <= sms * per_sm_pull * 105)
+        assert g.hlb_uses_aa() == want_aa, (name, lattice, blocks)
+        g.close()
 
 
 # ------------------------------------------------------------- north_star's acceptance runs

@@ -484,6 +484,10 @@ def by_name(name: str, small: bool = False) -> Workload:
         # not a BASELINE config: the aneurysm recipe scaled to the site count of the paper's
         # larger subject (296,814 sites, Table II) -- context for its Table III
         return aneurysm(scale=0.2 if small else 0.7375, steps=100 if small else 2000)
+    if name == "paper_sized_23":
+        # not a BASELINE config: the same recipe at the site count of the paper's smaller subject
+        # (132,910 sites, Table II)
+        return aneurysm(scale=0.2 if small else 0.5645, steps=100 if small else 2000)
     if name == "tree":
         if small:
             return tree(box=(160, 160, 160), r0=5.0, levels=3, steps=60)
