@@ -651,15 +651,14 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
     if ((rc = g->alloc(sizeof(int32_t) * cap, &d_behind))) return rc;
     if ((rc = g->alloc(sizeof(uint8_t) * cap, &d_link))) return rc;
     if ((rc = g->alloc(sizeof(double) * cap, &d_d))) return rc;
-    if ((rc = g->alloc(sizeof(uint32_t) * bits.size(), &d_bits))) return rc;
-    if ((rc = g->alloc(sizeof(int32_t) * rank.size(), &d_rank))) return rc;
+    if ((rc = g->alloc(sizeof(uint32_t) * 2 * bits.size(), &d_bits))) return rc;  // {bits, rank} words
     if ((rc = g->alloc(sizeof(double) * coef.size(), &d_coef))) return rc;
     void* mem[7] = {d_site, d_behind, d_link, d_d, d_bits, d_rank, d_coef};
     if (g->bfl_mem[0]) {  // smaller tables of an earlier call
       HLB_CUDA(cudaStreamSynchronize(g->stream));
       const size_t old_bytes[7] = {sizeof(int32_t) * g->bfl_cap_links, sizeof(int32_t) * g->bfl_cap_links,
                                    sizeof(uint8_t) * g->bfl_cap_links, sizeof(double) * g->bfl_cap_links,
-                                   sizeof(uint32_t) * bits.size(), sizeof(int32_t) * rank.size(),
+                                   sizeof(uint32_t) * 2 * bits.size(), 0,
                                    sizeof(double) * g->bfl_cap_coef};
       for (int k = 0; k < 7; ++k) g->release(g->bfl_mem[k], old_bytes[k]);
     }
@@ -673,16 +672,18 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
     HLB_CUDA(cudaMemcpy(d_link, l_link.data(), sizeof(uint8_t) * nl, cudaMemcpyHostToDevice));
     HLB_CUDA(cudaMemcpy(d_d, l_d.data(), sizeof(double) * nl, cudaMemcpyHostToDevice));
   }
-  HLB_CUDA(cudaMemcpy(d_bits, bits.data(), sizeof(uint32_t) * bits.size(), cudaMemcpyHostToDevice));
-  HLB_CUDA(cudaMemcpy(d_rank, rank.data(), sizeof(int32_t) * rank.size(), cudaMemcpyHostToDevice));
+  {
+    std::vector<uint32_t> words(2 * bits.size());
+    for (size_t w = 0; w < bits.size(); ++w) { words[2 * w] = bits[w]; words[2 * w + 1] = (uint32_t)rank[w]; }
+    HLB_CUDA(cudaMemcpy(d_bits, words.data(), sizeof(uint32_t) * words.size(), cudaMemcpyHostToDevice));
+  }
   HLB_CUDA(cudaMemcpy(d_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice));
   g->dg.bfl.site = (const int32_t*)d_site;
   g->dg.bfl.behind = (const int32_t*)d_behind;
   g->dg.bfl.link = (const uint8_t*)d_link;
   g->dg.bfl.d = (const double*)d_d;
   g->dg.bfl.n = (long long)nl;
-  g->dg.bflf.bits = (const uint32_t*)d_bits;
-  g->dg.bflf.rank = (const int32_t*)d_rank;
+  g->dg.bflf.idx = (const uint2*)d_bits;
   g->dg.bflf.coef = (const double*)d_coef;
   g->dg.bflf.nf = (long long)nf;
   g->dg.bflf.gather = 0;

@@ -336,11 +336,22 @@ __device__ __forceinline__ void prefetch_block_planes(const ST* a, long long Ns,
 //              writes back for link p.
 // Neither needs a memory access beyond the coefficients. Two links p and opp(p) of one site
 // are never both interpolated (that needs x + c_p solid and fluid), so updating in place is safe.
-__device__ __forceinline__ long long bfl_site_index(const BflFused& bf, long long i) {
-  const uint32_t w = __ldg(bf.bits + (i >> 5));
+// Who takes the common path (values stored as they become known, then return). Without
+// interpolated walls: every thread that is not a cap site (cap sites are few and clustered).
+// With them (V == 2) the choice is made per WARP, from the group's words: flagged sites are 16 %
+// of all and sit in two thirds of the warps; letting their lanes alone take the long path makes
+// those warps run both paths one after the other (measured +4...11 %), so a warp with any
+// flagged lane takes the long path with all its lanes, the rules predicated per lane.
+template <int V>
+__device__ __forceinline__ bool lean_path(int irow, uint32_t iolet_bits, uint32_t bfl_bits) {
+  if (V != 2) return irow < 0;
+  return (iolet_bits | bfl_bits) == 0u;  // the same for all lanes of the warp
+}
+__device__ __forceinline__ uint2 load_bfl_word(const BflFused& bf, long long i) { return __ldg(bf.idx + (i >> 5)); }
+__device__ __forceinline__ long long bfl_index_of(uint2 w) {
   const unsigned lane = threadIdx.x & 31;
-  if (!((w >> lane) & 1u)) return -1;
-  return (long long)__ldg(bf.rank + (i >> 5)) + __popc(w & ((1u << lane) - 1u));
+  if (!((w.x >> lane) & 1u)) return -1;
+  return (long long)w.y + __popc(w.x & ((1u << lane) - 1u));
 }
 // The coefficients are static: fetch them towards the SM before the populations are waited
 // for, so that the dependent chain bits -> rank -> coef does not add a DRAM round trip. A
@@ -494,15 +505,17 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
   double h[L::Q];
   long long bidx = -1;
   pdl_launch_dependents();
-  if (V == 2) {
-    bidx = bfl_site_index(bf, i);
-    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
-  }
   const bool ahead_ok = pf > 0 && i + pf < Ns;  // warp-uniform (pf, Ns: multiples of 128)
   const uint2 iow = load_iolet_word(io, i);
+  uint2 bw = make_uint2(0u, 0u);
+  if (V == 2) bw = load_bfl_word(bf, i);  // in flight together with the link records
   {
     IT off[L::Q - 1];
     link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, pl, off);
+    if (V == 2) {  // the row request goes out before the gathers and travels with them
+      bidx = bfl_index_of(bw);
+      if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+    }
     pdl_wait_for_previous_step();
     h[0] = to_real(src[i]);
 #pragma unroll
@@ -525,7 +538,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
   ST* d = dst + i;
   // (no second gather here, unlike the A-A kernels: the offsets are dead by now, and keeping
   // the gathered values for the rare path costs this kernel nothing measurable)
-  if (V != 2 && irow < 0) {  // common path: every value is stored as soon as it is known
+  if (lean_path<V>(irow, iow.x, bw.x)) {  // common path: every value is stored as soon as it is known
     collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { d[(long long)q * Ns] = to_store<ST>(v); });
     return;
   }
@@ -559,23 +572,25 @@ k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_pa
   long long bidx = -1;
   pdl_launch_dependents();
   const uint2 iow = load_iolet_word(io, i);
-  if (V == 2) {
-    bidx = bfl_site_index(bf, i);
-    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
-  }
+  uint2 bw = make_uint2(0u, 0u);
+  if (V == 2) bw = load_bfl_word(bf, i);
   pdl_wait_for_previous_step();
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
+  if (V == 2) {  // after the population loads are issued: waiting for the word must not delay them
+    bidx = bfl_index_of(bw);
+    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+  }
   if (pf > 0 && i + pf < Ns) prefetch_block_planes<L, ST>(a, Ns, pf);  // block-uniform test
   opaque(Ns);  // the stores rebuild their addresses (else 15 address pairs stay live: spills)
   const int irow = iolet_row_of(iow);
-  if (V != 2) {
-    if (irow < 0) {  // common path: h*_q goes to slot opp(q) as soon as it is known
-      const Moments m = moments_of<L>(h);
-      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
-      return;
-    }
-    const ST* again = relaunder(p0);  // rare path: read again
+  if (lean_path<V>(irow, iow.x, bw.x)) {  // common path: h*_q goes to slot opp(q) as soon as it is known
+    const Moments m = moments_of<L>(h);
+    collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
+    return;
+  }
+  if (V != 2) {  // rare path (cap sites): read again; with interpolated walls two thirds of the warps are here
+    const ST* again = relaunder(p0);
 #pragma unroll
     for (int q = 0; q < L::Q; ++q) h[q] = to_real(again[(long long)q * Ns]);
   }
@@ -600,12 +615,14 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   IT off[L::Q - 1];
   long long bidx = -1;
   pdl_launch_dependents();
-  if (V == 2) {
-    bidx = bfl_site_index(bf, i);
-    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
-  }
+  uint2 bw = make_uint2(0u, 0u);
+  if (V == 2) bw = load_bfl_word(bf, i);  // in flight together with the link records
   const bool ahead_ok = pf > 0 && i + pf < Ns;  // warp-uniform (pf, Ns: multiples of 128)
   link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, pl, off);
+  if (V == 2) {  // the row request goes out before the gathers and travels with them
+    bidx = bfl_index_of(bw);
+    if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
+  }
   const uint2 iow = load_iolet_word(io, i);  // (not before the decode: its registers are the scarce ones)
   pdl_wait_for_previous_step();
   double h[L::Q];
@@ -626,16 +643,16 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) opaque(off[q - 1]);
   const int irow = iolet_row_of(iow);
-  if (V != 2) {
-    if (irow < 0) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
-      const Moments m = moments_of<L>(h);
-      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) {
-        if (q == 0) a[i] = to_store<ST>(v);
-        else a[off[opp(q) - 1]] = to_store<ST>(v);
-      });
-      return;
-    }
-    const ST* again = relaunder(a);  // rare path: read again
+  if (lean_path<V>(irow, iow.x, bw.x)) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
+    const Moments m = moments_of<L>(h);
+    collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) {
+      if (q == 0) a[i] = to_store<ST>(v);
+      else a[off[opp(q) - 1]] = to_store<ST>(v);
+    });
+    return;
+  }
+  if (V != 2) {  // rare path (cap sites): read again; with interpolated walls two thirds of the warps are here
+    const ST* again = relaunder(a);
     h[0] = to_real(again[i]);
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) h[q] = to_real(again[off[q - 1]]);

@@ -19,16 +19,18 @@ struct BflLinks {
 };
 
 // BFL interpolated walls, site form (used inside the step kernels, by value as a kernel
-// argument): bit i of `bits` marks the sites with an interpolated link; such a site has the
-// dense index idx = rank[i / 32] + popcount(bits word below lane i % 32), and coef[idx * row
+// argument): idx[i / 32] = {bits, rank}: bit i % 32 of bits marks the sites with an interpolated
+// link; such a site has the dense index rank + popcount(bits below lane i % 32). ONE 8-byte word
+// per group, loaded with the kernel's first loads: as two arrays read one after the other (bits,
+// then rank only where flagged) they put two dependent memory round trips in front of the link
+// records (profiles/r02_tuning.md section 12). coef[idx * row
 // + p - 1] (row = bfl_row_doubles(): Q-1 rounded up to a multiple of 4; 16-byte aligned) is,
 // for its pull link p,  2d  where d < 1/2 (applied while gathering),  -1/(2d)
 // where d >= 1/2 (applied to the value the site writes back for that link),  0 = plain
 // bounce-back. gather = 0 when the d < 1/2 part is already in the state buffer (pre-pass
 // run for a read-out) or does not apply (the initial state).
 struct BflFused {
-  const uint32_t* bits = nullptr;  // [Ns/32]
-  const int32_t* rank = nullptr;   // [Ns/32]
+  const uint2* idx = nullptr;      // [Ns/32] {bits, rank}
   const double* coef = nullptr;    // [nf][row]
   long long nf = 0;
   int gather = 0;
