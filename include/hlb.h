@@ -118,8 +118,8 @@ typedef struct {
   hlb_free_fn free;        /* optional (NULL): releases one buffer of `alloc` early; called
                               with alloc_user                                              */
   void* copy_stream;       /* optional (NULL): a second cudaStream_t of the caller, used only by
-                              hlb_get_macroscopic_async for its device-to-host copies, so that
-                              they overlap the next upload / steps on `stream`             */
+                              hlb_get_macroscopic_async and hlb_stage_state for their copies
+                              from / to the host, so that they overlap the steps on `stream` */
 } hlb_params;
 
 /* Build the geometry: extract the fluid sites, order them, build the int32 pull-neighbour
@@ -242,6 +242,18 @@ int hlb_get_macroscopic(hlb_geometry* g, double* rho, double* u);
  * params.copy_stream (else HLB_EINVAL). */
 int hlb_get_macroscopic_async(hlb_geometry* g, double* rho, double* u);
 int hlb_wait_copies(hlb_geometry* g);
+
+/* The counterpart for the way in: hlb_stage_state uploads an initial state (HOST, pinned, as
+ * hlb_set_state: rho [N] or NULL => 1, u [N][3] or NULL => 0) into a staging buffer on
+ * params.copy_stream WITHOUT touching the simulation -- it may run under hlb_step calls still
+ * in flight on `stream` -- and returns at once; the arrays must stay valid until the next
+ * hlb_wait_copies(). hlb_set_state_staged then does what hlb_set_state does, from the staged
+ * copy: `stream` waits for the upload, f = f_eq(rho, u), step counter 0. One staged state at
+ * a time: a second hlb_stage_state waits (on the device) until the first has been consumed.
+ * Errors: HLB_EINVAL (no copy stream; hlb_set_state_staged without a staged state),
+ * HLB_ENOMEM (the first call allocates the staging buffer), HLB_ECUDA. */
+int hlb_stage_state(hlb_geometry* g, const double* rho, const double* u);
+int hlb_set_state_staged(hlb_geometry* g);
 
 /* Same, into DEVICE buffers (rho [N], u [N][3]); enqueued on the stream, no sync. */
 int hlb_get_macroscopic_device(hlb_geometry* g, double* rho_dev, double* u_dev);

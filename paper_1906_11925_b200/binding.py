@@ -95,6 +95,8 @@ def _load() -> ctypes.CDLL:
         "hlb_get_macroscopic_device": (c_int, [vp, vp, vp]),
         "hlb_get_macroscopic_async": (c_int, [vp, vp, vp]),
         "hlb_wait_copies": (c_int, [vp]),
+        "hlb_stage_state": (c_int, [vp, vp, vp]),
+        "hlb_set_state_staged": (c_int, [vp]),
         "hlb_get_populations": (c_int, [vp, vp]),
         "hlb_get_stress": (c_int, [vp, vp]),
         "hlb_get_stress_device": (c_int, [vp, vp]),
@@ -136,7 +138,7 @@ LIB_PATH = _build.LIB_PATH
 _lib = _load()
 EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_set_iolet_velocity", "hlb_set_iolet_waveform", "hlb_set_iolet_weight", "hlb_set_iolet_normal", "hlb_set_wall_distance", "hlb_num_bfl_sites", "hlb_step",
-            "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_macroscopic_async", "hlb_wait_copies",
+            "hlb_get_macroscopic", "hlb_get_macroscopic_device", "hlb_get_macroscopic_async", "hlb_wait_copies", "hlb_stage_state", "hlb_set_state_staged",
             "hlb_get_populations",
             "hlb_get_stress", "hlb_get_stress_device", "hlb_get_wall_shear_stress", "hlb_get_wall_shear_stress_noalloc", "hlb_noalloc_max_sites", "hlb_render_volume", "hlb_render",
             "hlb_render_device",
@@ -365,6 +367,20 @@ class Geometry:
                                       and a.flags.c_contiguous and a.flags.writeable):
                 raise ValueError(f"output array must be a writable C-contiguous float64 array of shape {shape}")
         _check(self._call(_lib.hlb_get_macroscopic_async, _ptr(rho_out), _ptr(u_out)))
+
+    def hlb_stage_state(self, rho=None, u=None):
+        """Upload rho [N] / u [N, 3] (PINNED float64 numpy arrays, kept alive and unchanged by the
+        caller until hlb_wait_copies()) into the staging buffer on the copy stream; no effect on
+        the simulation until hlb_set_state_staged()."""
+        n = self.n_sites
+        for a, shape in ((rho, (n,)), (u, (n, 3))):
+            if a is not None and not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.shape == shape
+                                      and a.flags.c_contiguous):
+                raise ValueError(f"expected a C-contiguous float64 array of shape {shape}")
+        _check(self._call(_lib.hlb_stage_state, _ptr(rho), _ptr(u)))
+
+    def hlb_set_state_staged(self):
+        _check(self._call(_lib.hlb_set_state_staged))
 
     def hlb_wait_copies(self):
         _check(self._call(_lib.hlb_wait_copies))

@@ -79,6 +79,9 @@ struct hlb_geometry {
   double* scratch_out = nullptr;      // [4 N] doubles: its own staging buffer (lazy), so that an
                                       // upload through `scratch` may overlap the copies
   cudaEvent_t ev_ready = nullptr, ev_copied = nullptr;  // read-out done / copies done
+  double* scratch_in = nullptr;       // [4 N] doubles: staging buffer of hlb_stage_state (lazy)
+  cudaEvent_t ev_staged = nullptr, ev_consumed = nullptr;  // upload done / init kernel has read it
+  bool staged = false, staged_rho = false, staged_u = false;
   double* scratch_pop = nullptr;      // [N][15] doubles, allocated by the first
                                       // hlb_get_populations / hlb_set_populations call
   int64_t steps = 0, launches = 0, device_bytes = 0;
@@ -454,10 +457,14 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
 void hlb_geometry_destroy(hlb_geometry* g) {
   if (!g) return;
   if (g->graph_exec) cudaGraphExecDestroy(g->graph_exec);
+  if (g->ev_ready || g->ev_staged) cudaStreamSynchronize(g->copy_stream);
   if (g->ev_ready) {
-    cudaStreamSynchronize(g->copy_stream);
     cudaEventDestroy(g->ev_ready);
     cudaEventDestroy(g->ev_copied);
+  }
+  if (g->ev_staged) {
+    cudaEventDestroy(g->ev_staged);
+    cudaEventDestroy(g->ev_consumed);
   }
   if (g->vol_array) {
     cudaStreamSynchronize(g->stream);
@@ -911,7 +918,43 @@ int hlb_get_macroscopic_async(hlb_geometry* g, double* rho, double* u) {
 
 int hlb_wait_copies(hlb_geometry* g) {
   if (!g) return fail(HLB_EINVAL, "NULL geometry");
-  if (g->copy_stream && g->ev_ready) HLB_CUDA(cudaStreamSynchronize(g->copy_stream));
+  if (g->copy_stream && (g->ev_ready || g->ev_staged)) HLB_CUDA(cudaStreamSynchronize(g->copy_stream));
+  return HLB_OK;
+}
+
+int hlb_stage_state(hlb_geometry* g, const double* rho, const double* u) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (!g->copy_stream) return fail(HLB_EINVAL, "hlb_stage_state needs params.copy_stream");
+  const size_t n = (size_t)g->N;
+  if (!g->scratch_in) {
+    void* ptr = nullptr;
+    const int rc = g->alloc(sizeof(double) * 4 * n, &ptr);
+    if (rc) return rc;
+    g->scratch_in = (double*)ptr;
+    HLB_CUDA(cudaEventCreateWithFlags(&g->ev_staged, cudaEventDisableTiming));
+    HLB_CUDA(cudaEventCreateWithFlags(&g->ev_consumed, cudaEventDisableTiming));
+    HLB_CUDA(cudaEventRecord(g->ev_consumed, g->stream));
+  }
+  // the init kernel of the previous hlb_set_state_staged must have read the buffer
+  HLB_CUDA(cudaStreamWaitEvent(g->copy_stream, g->ev_consumed, 0));
+  if (rho) HLB_CUDA(cudaMemcpyAsync(g->scratch_in, rho, sizeof(double) * n, cudaMemcpyHostToDevice, g->copy_stream));
+  if (u) HLB_CUDA(cudaMemcpyAsync(g->scratch_in + n, u, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, g->copy_stream));
+  HLB_CUDA(cudaEventRecord(g->ev_staged, g->copy_stream));
+  g->staged = true;
+  g->staged_rho = rho != nullptr;
+  g->staged_u = u != nullptr;
+  return HLB_OK;
+}
+
+int hlb_set_state_staged(hlb_geometry* g) {
+  if (!g) return fail(HLB_EINVAL, "NULL geometry");
+  if (!g->staged) return fail(HLB_EINVAL, "hlb_set_state_staged without a staged state (hlb_stage_state)");
+  HLB_CUDA(cudaStreamWaitEvent(g->stream, g->ev_staged, 0));
+  const int rc = init_from(g, g->staged_rho ? g->scratch_in : nullptr,
+                           g->staged_u ? g->scratch_in + (size_t)g->N : nullptr, nullptr);
+  if (rc) return rc;
+  HLB_CUDA(cudaEventRecord(g->ev_consumed, g->stream));
+  g->staged = false;
   return HLB_OK;
 }
 

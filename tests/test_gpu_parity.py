@@ -932,6 +932,41 @@ def test_asynchronous_read_out_on_a_copy_stream(hlb):
     g.close()
 
 
+def test_staged_upload_on_a_copy_stream(hlb):
+    """hlb_stage_state + hlb_set_state_staged (include/hlb.h): the same run as hlb_set_state, also
+    when the upload of the next state is enqueued while the steps of the current one are in
+    flight; refused without a copy stream or without a staged state."""
+    import torch
+    wl = W.by_name("cube", small=True)
+    n = wl.n_sites
+    rng = np.random.default_rng(3)
+    states = [(1.0 + 0.01 * rng.random(n), 0.02 * (rng.random((n, 3)) - 0.5)) for _ in range(3)]
+    pinned = [(torch.from_numpy(r).pin_memory().numpy(), torch.from_numpy(u).pin_memory().numpy()) for r, u in states]
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho,
+                                flags_of(hlb, "aa", "f64", "auto"), copy_stream=torch.cuda.Stream())
+    with pytest.raises(hlb.HlbError):
+        g.hlb_set_state_staged()                       # nothing staged
+    got = []
+    g.hlb_stage_state(*pinned[0])
+    for k in range(3):
+        g.hlb_set_state_staged()
+        g.hlb_step(9 + k)
+        if k + 1 < 3:
+            g.hlb_stage_state(*pinned[k + 1])          # uploads under the steps just enqueued
+        got.append(g.hlb_get_macroscopic())
+    g.hlb_wait_copies()
+    g.close()
+    for k in range(3):
+        wl_k = W.Workload("cube", wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, 0, rho0=states[k][0], u0=states[k][1])
+        want = run_gpu(hlb, wl_k, 9 + k, "aa", "f64", "auto")
+        assert np.array_equal(got[k][0], want[0]) and np.array_equal(got[k][1], want[1])
+    g = hlb.hlb_geometry_create(wl.site_type, wl.periodic, wl.tau, wl.iolet_rho, flags_of(hlb, "aa", "f64", "auto"))
+    with pytest.raises(hlb.HlbError) as e:
+        g.hlb_stage_state(*pinned[0])
+    assert e.value.code == hlb.HLB_EINVAL
+    g.close()
+
+
 def test_degenerate_geometries(hlb):
     st = np.zeros((3, 3, 3), dtype=np.uint8)
     st[1, 1, 1] = 1                                   # one site, every link bounces back
