@@ -69,6 +69,11 @@ template <typename L, bool REC> constexpr int aa_odd_minb() {
 // The even kernel keeps no offsets: with 4-byte populations it fits 72 registers without
 // spills, and the seventh block is worth 2.5 % there (0.704 vs 0.723 ms on configs[4]; nothing
 // in fp64, where it sits at the copy rate already).
+// (see link_offsets: shared-memory records in the 4-byte-storage A-A odd kernel)
+template <typename ST, bool REC> constexpr bool odd_rec_smem() { return sizeof(ST) == 4 && REC; }
+template <typename L, typename ST, bool REC, typename IT, int V> constexpr int odd_smem_minb_add() {
+  return odd_rec_smem<ST, REC>() && L::Q == 15 && sizeof(IT) == 4 && V != 2 ? 1 : 0;  // (64-bit offsets: spills)
+}
 template <typename L, typename ST> constexpr int aa_even_minb() {
   return HLB_AA_EVEN_MINB + (sizeof(ST) == 4 && L::Q == 15 ? 1 : 0) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
 }
@@ -115,7 +120,15 @@ __device__ __forceinline__ void check_offsets(const IT (&off)[L::Q - 1], long lo
 struct Planes {
   uint32_t p[MAXQ];
 };
-template <typename L, int MODE, bool REC, typename IT>
+// SMEM (with REC): the Q - 1 records of a warp are the same for its 32 lanes; held in registers
+// by every lane they are the register peak of a gather kernel (14 x 4 = 56). With SMEM lane
+// l < Q - 1 loads record l (ONE load instruction per warp), the warp's slice of shared memory
+// holds them, and each link reads its record back by broadcast right before it is decoded.
+// Used where the freed registers buy a resident block that pays: the A-A odd kernel with 4-byte
+// storage (0.942 -> 0.902 ms on configs[4] at 7 blocks per SM). The fp64 kernels and the
+// two-lattice kernel lose 1-5 % with it, with or without the extra block
+// (profiles/r02_tuning.md section 13).
+template <typename L, int MODE, bool REC, typename IT, bool SMEM = false>
 __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
                                              const uint4* __restrict__ rec, long long Ns,
                                              long long i, const Planes& pl, IT (&off)[L::Q - 1]) {
@@ -135,15 +148,30 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t lane_bit = 1u << lane;
   const uint4* r = rec + (i >> 5) * (L::Q - 1);
-  uint4 v[L::Q - 1];
-#pragma unroll
-  for (int q = 1; q < L::Q; ++q) v[q - 1] = __ldg(r + (q - 1));
   // second <= 32 in a real record, 0xffffffff in a sentinel: one warp-uniform test decides
   // whether this warp needs the table at all, so the common path carries no sentinel code
-  uint32_t any = 0u;
+  __shared__ uint4 s_rec[SMEM ? SBLOCK / 32 : 1][SMEM ? L::Q - 1 : 1];
+  uint4 v_reg[SMEM ? 1 : L::Q - 1];
+  uint4* v = SMEM ? s_rec[threadIdx.x >> 5] : v_reg;
+  bool no_sentinel;
+  if (SMEM) {
+    bool sentinel_here = false;
+    if (lane < L::Q - 1) {
+      const uint4 mine = __ldg(r + lane);
+      v[lane] = mine;
+      sentinel_here = mine.y == 0xffffffffu;
+    }
+    no_sentinel = !__any_sync(0xffffffffu, sentinel_here);
+    __syncwarp();
+  } else {
 #pragma unroll
-  for (int q = 1; q < L::Q; ++q) any |= v[q - 1].y;
-  if ((int32_t)any >= 0) {
+    for (int q = 1; q < L::Q; ++q) v[q - 1] = __ldg(r + (q - 1));
+    uint32_t any = 0u;
+#pragma unroll
+    for (int q = 1; q < L::Q; ++q) any |= v[q - 1].y;
+    no_sentinel = (int32_t)any >= 0;
+  }
+  if (no_sentinel) {
     // offset = own index + delta + plane: delta is the run's (source - own index), or, at a
     // wall lane, the step from plane qf to plane qw at the site itself -- five integer
     // instructions per link (compare, select, mask test, select, 3-input add)
@@ -607,7 +635,7 @@ k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_pa
 }
 
 template <typename L, typename ST, bool REC, typename IT, int V>
-__global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>())
+__global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>() + odd_smem_minb_add<L, ST, REC, IT, V>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
          IoletIndex io, const double* __restrict__ iolet_par,
          long long Ns, Relax rx, Planes pl, long long pf, BflFused bf) {
@@ -618,7 +646,8 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   uint2 bw = make_uint2(0u, 0u);
   if (V == 2) bw = load_bfl_word(bf, i);  // in flight together with the link records
   const bool ahead_ok = pf > 0 && i + pf < Ns;  // warp-uniform (pf, Ns: multiples of 128)
-  link_offsets<L, GATHER_AA_ODD, REC, IT>(nbr, rec, Ns, i, pl, off);
+  constexpr bool REC_SMEM = sizeof(ST) == 4 && REC;  // = odd_rec_smem<ST, REC>()
+  link_offsets<L, GATHER_AA_ODD, REC, IT, REC_SMEM>(nbr, rec, Ns, i, pl, off);
   if (V == 2) {  // the row request goes out before the gathers and travels with them
     bidx = bfl_index_of(bw);
     if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
