@@ -572,6 +572,7 @@ SWEEP = [
     ("paper_sized_23", {"lattice": "d3q19", "scheme": "auto"}, 1000, 60),
     ("tree", {}, 100, 24),
     ("tree", {"store": "f32"}, 100, 32),
+    ("tree", {"store": "f32", "scheme": "auto"}, 100, 36),
     ("bigtree", {"scheme": "two_lattice"}, 50, 7),
     ("bigtree", {"scheme": "aa", "store": "f32"}, 50, 10),
     ("bigtree", {"scheme": "aa", "lattice": "d3q19"}, 50, 6),

@@ -839,14 +839,15 @@ def test_64_bit_offset_kernels_equal_32_bit(hlb, scheme, links):
     """Above 2^32 / 15 sites the kernels index with 64-bit offsets; HLB_INDEX64 forces that
     instantiation on a small geometry: bitwise the same as the 32-bit one."""
     wl = W.by_name("bigtree", small=True)
-    f = flags_of(hlb, scheme, "f64", "raster", links)
-    out = []
-    for extra in (0, hlb.HLB_INDEX64):
-        g = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | extra)
-        g.hlb_step(23)
-        out.append(g.hlb_get_macroscopic())
-        g.close()
-    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    for store in ("f64", "f32"):      # (f32 + A-A + records: the shared-memory record path of k_aa_odd)
+        f = flags_of(hlb, scheme, store, "raster", links)
+        out = []
+        for extra in (0, hlb.HLB_INDEX64):
+            g = hlb.hlb_geometry_create(wl.site_type, 0, wl.tau, wl.iolet_rho, f | extra)
+            g.hlb_step(23)
+            out.append(g.hlb_get_macroscopic())
+            g.close()
+        assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]), store
 
 
 @pytest.mark.parametrize("scheme", ["two_lattice", "aa"])
