@@ -1168,6 +1168,15 @@ def test_full_configs_full_steps_record(hlb, name, record):
         record(f"RECORD {name} N={wl.n_sites} steps={wl.steps} {wl.scheme}/{store} "
                f"E_rho={e_rho:.3e} E_u={e_u:.3e} (bar {TOL[store]:.0e})")
         assert e_rho < TOL[store] and e_u < TOL[store]
+    if name == "tree":   # the scheme HLB_SCHEME_AUTO picks at this size, with 4-byte storage
+        e_rho, e_u = errors(*run_gpu(hlb, wl, wl.steps, "aa", "f32", "auto"), rho_ref, u_ref)
+        record(f"RECORD {name} N={wl.n_sites} steps={wl.steps} aa/f32 E_rho={e_rho:.3e} E_u={e_u:.3e} (bar 1e-05)")
+        assert e_rho < TOL["f32"] and e_u < TOL["f32"]
+    if name == "aneurysm":   # the lattice the paper ran, in place
+        rho19, u19 = run_oracle(wl, wl.steps, lattice="d3q19")
+        e_rho, e_u = errors(*run_gpu(hlb, wl, wl.steps, "aa", "f64", "auto", "auto", "d3q19"), rho19, u19)
+        record(f"RECORD {name} N={wl.n_sites} steps={wl.steps} D3Q19 aa/f64 E_rho={e_rho:.3e} E_u={e_u:.3e} (bar 1e-12)")
+        assert e_rho < TOL["f64"] and e_u < TOL["f64"]
 
 
 # ------------------------------------------------------------- the sizes the library claims
