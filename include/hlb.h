@@ -393,16 +393,19 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
 
 /* Run-length link records of a table (host only): the compressed form of nbr that the step
  * kernels read. A group is 32 consecutive internal sites (one warp). For group g and link q
- * the record rec[(g*n_links + (q-1))*4 .. +4] = { wall, second, off0, off1 }:
+ * the record rec[(g*n_links + (q-1))*4 .. +4] = { wall, runs, off0, off1 }:
  *   wall    bit l set: the entry of lane l is negative (solid or iolet: bounce-back target)
- *   second  the non-wall lanes split into runs of lanes with consecutive entries (a wall
- *           lane or a jump in the entries ends a run); second = the lane at which run 1
- *           starts, 32 if there is only one run (or none)
+ *   runs    the non-wall lanes split into runs of lanes with consecutive entries (a wall
+ *           lane or a jump in the entries ends a run). Bits 0..5: second = the lane at which
+ *           run 1 starts, 32 if there is only one run (or none). Bit 6: there is a third run;
+ *           then bits 7..11: third = the lane at which run 2 starts, and bits 12..31: the
+ *           signed difference off2 - off1. All higher bits 0 without a third run.
  *   off0, off1: (entry of a lane of the run) - (internal index 32 g + l of that lane's own
  *           site), modulo 2^32, for run 0 and run 1; off1 = off0 when there is only one run
- * so that the entry of a non-wall lane l is (l >= second ? off1 : off0) + 32 g + l (mod 2^32):
- * the step kernels add the same delta to every lane's own index. A (g, q) with more than two
- * runs gets the sentinel { 0, 0xffffffff, 0, 0 } and the kernels read nbr for it instead.
+ * so that the entry of a non-wall lane l is 32 g + l + (l >= third ? off2 : l >= second ? off1 :
+ * off0) (mod 2^32): the step kernels add the same delta to every lane's own index. A (g, q)
+ * with more than three runs, or with a third run whose off2 - off1 does not fit 20 signed
+ * bits, gets the sentinel { 0, 0xffffffff, 0, 0 } and the kernels read nbr for it instead.
  *   nbr: HOST [n_links][stride] as filled by hlb_preprocess_tables; stride a multiple of 32;
  *        n_links = Q - 1 = 14 or 18
  *   rec: HOST [stride/32][n_links][4] uint32, filled

@@ -328,17 +328,18 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
     // A-A in place (half the launches read no links; one array in L2 for the mid sizes) except
     //  * where the resident multi-step kernel applies: two-lattice is the faster one there
     //    (5.4 k vs 5.0 k MSUPS on configs[0]);
-    //  * where the whole grid is ONE wave of the two-lattice kernel (7 resident blocks per SM,
-    //    5 % slack) but more than one wave of the A-A kernels (6 per SM): the second, nearly
-    //    empty wave costs A-A 13 % at the paper's Subject-23 size (133 k sites).
+    //  * where the whole grid is ONE wave of the two-lattice kernel (5 % slack) but more than
+    //    one wave of the A-A kernels, i.e. where the two-lattice kernel has the larger register
+    //    budget in blocks per SM (D3Q19: 5 against 4): the second, nearly empty wave costs A-A
+    //    8-20 % there.
     // profiles/r02_tuning.md section 7.
     int dev = 0, sms = 0;
     const bool have = cudaGetDevice(&dev) == cudaSuccess &&
                       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess;
     const bool q19 = (p->flags & HLB_LATTICE_D3Q19) != 0;
     const int64_t blocks = t.Ns / 128;
-    const int64_t slots_pull = (int64_t)sms * resident_sites_per_sm_pull(q19) / 128;
-    const int64_t slots_aa = (int64_t)sms * resident_sites_per_sm_aa(q19) / 128;
+    const int64_t slots_pull = (int64_t)sms * resident_sites_per_sm_pull(q19, (p->flags & HLB_STORE_F32) != 0) / 128;
+    const int64_t slots_aa = (int64_t)sms * resident_sites_per_sm_aa(q19, (p->flags & HLB_STORE_F32) != 0) / 128;
     const bool resident = have && !(p->flags & (HLB_NO_GRAPH | HLB_NO_RESIDENT)) &&
                           t.Ns <= (int64_t)sms * resident_kernel_sites_per_sm();
     const bool one_pull_wave = have && blocks > slots_aa && blocks * 100 <= slots_pull * 105;
@@ -376,8 +377,8 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
     // (same-box sweep of the fp32-storage kernels: 0.82 / 1.00 ms at this many sites, 0.72 /
     // 0.97 ms at twice as many; profiles/r02_tuning.md).
     const int64_t per8 = g->f32 ? 2 : 1;
-    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull(Q == 19) * 3 / 4 / 128 * 128 * per8;
-    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa(Q == 19) * 3 / 4 / 128 * 128 * per8;
+    g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull(Q == 19, g->f32) * 3 / 4 / 128 * 128 * per8;
+    g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa(Q == 19, g->f32) * 3 / 4 / 128 * 128 * per8;
     if (const char* e = std::getenv("HLB_PREFETCH_SITES")) {
       const long long v = std::atoll(e);
       g->dg.prefetch_pull = g->dg.prefetch_aa = v > 0 ? (v < (1ll << 24) ? v : (1ll << 24)) : 0;

@@ -69,6 +69,16 @@ template <typename L, bool REC> constexpr int aa_odd_minb() {
 // The even kernel keeps no offsets: with 4-byte populations it fits 72 registers without
 // spills, and the seventh block is worth 2.5 % there (0.704 vs 0.723 ms on configs[4]; nothing
 // in fp64, where it sits at the copy rate already).
+// k_pull with 8-byte storage and link records gets 80 registers (6 blocks): with the three-run
+// decode on its general path ptxas' tighter 72-register allocation cost it 2.7 % on configs[4]
+// (1.478 -> 1.515 ms; at 6 blocks 1.491, configs[3] 0.199 either way); 4-byte storage stays at 7
+// (0.870 vs 0.890 ms). profiles/r02_tuning.md section 14.
+#ifndef HLB_PULL_F64_DROP
+#define HLB_PULL_F64_DROP 1
+#endif
+template <typename L, typename ST, bool REC> constexpr int pull_f64_drop() {
+  return sizeof(ST) == 8 && REC && L::Q == 15 ? HLB_PULL_F64_DROP : 0;
+}
 // (see link_offsets: shared-memory records in the 4-byte-storage A-A odd kernel)
 template <typename ST, bool REC> constexpr bool odd_rec_smem() { return sizeof(ST) == 4 && REC; }
 template <typename L, typename ST, bool REC, typename IT, int V> constexpr int odd_smem_minb_add() {
@@ -153,15 +163,18 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
   __shared__ uint4 s_rec[SMEM ? SBLOCK / 32 : 1][SMEM ? L::Q - 1 : 1];
   uint4 v_reg[SMEM ? 1 : L::Q - 1];
   uint4* v = SMEM ? s_rec[threadIdx.x >> 5] : v_reg;
-  bool no_sentinel;
+  // word y of a record: second (<= 32) alone when the link has one or two runs; bit 6 set with a
+  // third run (include/hlb.h); 0xffffffff = sentinel. "simple" = all Q - 1 records of the warp
+  // have at most two runs: the path nearly every warp takes.
+  bool simple;
   if (SMEM) {
-    bool sentinel_here = false;
+    bool plain_here = true;
     if (lane < L::Q - 1) {
       const uint4 mine = __ldg(r + lane);
       v[lane] = mine;
-      sentinel_here = mine.y == 0xffffffffu;
+      plain_here = (mine.y & 0x80000040u) == 0u;
     }
-    no_sentinel = !__any_sync(0xffffffffu, sentinel_here);
+    simple = __all_sync(0xffffffffu, plain_here);
     __syncwarp();
   } else {
 #pragma unroll
@@ -169,9 +182,9 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
     uint32_t any = 0u;
 #pragma unroll
     for (int q = 1; q < L::Q; ++q) any |= v[q - 1].y;
-    no_sentinel = (int32_t)any >= 0;
+    simple = (any & 0x80000040u) == 0u;
   }
-  if (no_sentinel) {
+  if (simple) {
     // offset = own index + delta + plane: delta is the run's (source - own index), or, at a
     // wall lane, the step from plane qf to plane qw at the site itself -- five integer
     // instructions per link (compare, select, mask test, select, 3-input add)
@@ -195,11 +208,13 @@ __device__ __forceinline__ void link_offsets(const int32_t* __restrict__ nbr,
       const uint4 t = v[q - 1];
       int32_t e;
       bool wall;
-      if (t.y == 0xffffffffu) {  // sentinel: more than two runs
+      if (t.y == 0xffffffffu) {  // sentinel: more than three runs (or a third delta out of range)
         e = __ldg(nbr + (long long)(q - 1) * Ns + i);
         wall = e < 0;
-      } else {
-        e = (int32_t)((lane >= t.y ? t.w : t.z) + (uint32_t)i);
+      } else {  // one, two or three runs, all from the record: no dependent load
+        uint32_t d = lane >= (t.y & 63u) ? t.w : t.z;
+        if ((t.y & 0x40u) && lane >= ((t.y >> 7) & 31u)) d = t.w + (uint32_t)((int32_t)t.y >> 12);
+        e = (int32_t)(d + (uint32_t)i);
         wall = (t.x & lane_bit) != 0u;
       }
       off[q - 1] = wall ? (IT)qw * n + self : (IT)qf * n + (IT)e;
@@ -525,7 +540,7 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
 // (profiles/r02_tuning.md). Safe in the in-place kernels too: a site's read set is its own
 // write set, so nobody else has written these slots, and this thread has not stored yet.
 template <typename L, typename ST, bool REC, typename IT, int V>
-__global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>())
+__global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>() - pull_f64_drop<L, ST, REC>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, IoletIndex io, const double* __restrict__ iolet_par,
        long long Ns, Relax rx, Planes pl, long long pf, BflFused bf) {
@@ -975,12 +990,16 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + BLOCK - 1) / BLOC
 }  // namespace
 
 int bfl_row_doubles(bool d3q19) { return d3q19 ? bfl_row<D3Q19>() : bfl_row<D3Q15>(); }
-int resident_sites_per_sm_pull(bool d3q19) {
-  return SBLOCK * (d3q19 ? pull_minb<D3Q19, true>() : pull_minb<D3Q15, true>());
+int resident_sites_per_sm_pull(bool d3q19, bool f32) {
+  if (d3q19) return SBLOCK * pull_minb<D3Q19, true>();
+  return SBLOCK * (f32 ? pull_minb<D3Q15, true>() - pull_f64_drop<D3Q15, float, true>()
+                       : pull_minb<D3Q15, true>() - pull_f64_drop<D3Q15, double, true>());
 }
 int resident_kernel_sites_per_sm() { return SBLOCK * RESIDENT_MINB; }
-int resident_sites_per_sm_aa(bool d3q19) {
-  return SBLOCK * (d3q19 ? aa_odd_minb<D3Q19, true>() : aa_odd_minb<D3Q15, true>());
+int resident_sites_per_sm_aa(bool d3q19, bool f32) {  // of the odd (gather) kernel, the tighter of the two
+  if (d3q19) return SBLOCK * aa_odd_minb<D3Q19, true>();
+  return SBLOCK * (aa_odd_minb<D3Q15, true>() +
+                   (f32 ? odd_smem_minb_add<D3Q15, float, true, uint32_t, 0>() : 0));
 }
 
 // ------------------------------------------------------------------ launchers

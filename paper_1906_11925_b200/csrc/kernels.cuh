@@ -68,8 +68,8 @@ struct DeviceGeometry {
 
 int bfl_row_doubles(bool d3q19);
 // Sites resident on an SM at once (threads per block x resident blocks) per step kernel.
-int resident_sites_per_sm_pull(bool d3q19);
-int resident_sites_per_sm_aa(bool d3q19);
+int resident_sites_per_sm_pull(bool d3q19, bool f32);
+int resident_sites_per_sm_aa(bool d3q19, bool f32);
 // Sites per SM the resident multi-step kernels (launch_resident_steps) are sized for.
 int resident_kernel_sites_per_sm();
 

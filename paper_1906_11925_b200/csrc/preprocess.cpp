@@ -119,25 +119,33 @@ int64_t build_link_records(const int32_t* nbr, int n_links, int64_t Ns, uint32_t
     for (int64_t g = gb; g < ge; ++g) {
       for (int q = 1; q < Q; ++q) {
         const int32_t* e = nbr + (int64_t)(q - 1) * Ns + g * 32;
-        uint32_t wall = 0, second = 32;   // second: lane at which run 1 starts
-        uint32_t delta[2] = {0u, 0u};      // source index minus own index (mod 2^32) within a run
+        uint32_t wall = 0, second = 32, third = 0;  // second / third: lane at which run 1 / run 2 starts
+        uint32_t delta[3] = {0u, 0u, 0u};  // source index minus own index (mod 2^32) within a run
         int runs = 0;
         for (int l = 0; l < 32; ++l) {
           if (e[l] < 0) { wall |= 1u << l; continue; }
           const bool cont = l > 0 && e[l - 1] >= 0 && e[l] == e[l - 1] + 1;
           if (!cont) {
-            if (runs < 2) delta[runs] = (uint32_t)e[l] - (uint32_t)(g * 32 + l);
+            if (runs < 3) delta[runs] = (uint32_t)e[l] - (uint32_t)(g * 32 + l);
             if (runs == 1) second = (uint32_t)l;
+            if (runs == 2) third = (uint32_t)l;
             ++runs;
           }
         }
         if (runs < 2) delta[1] = delta[0];
         uint32_t* r = rec + ((size_t)g * (Q - 1) + (size_t)(q - 1)) * 4;
-        if (runs > 2) {
+        // a third run: its delta as a 20-bit signed difference to the second run's (consecutive
+        // runs of a warp come from neighbouring rows; if it does not fit, the pair is a sentinel)
+        const int64_t dd2 = (int64_t)(int32_t)(delta[2] - delta[1]);
+        const bool three = runs == 3 && dd2 >= -(1 << 19) && dd2 < (1 << 19);
+        if (runs > 3 || (runs == 3 && !three)) {
           r[0] = 0u; r[1] = 0xffffffffu; r[2] = r[3] = 0u;  // sentinel: read the table itself
           ++fb;
         } else {
-          r[0] = wall; r[1] = second; r[2] = delta[0]; r[3] = delta[1];
+          r[0] = wall;
+          r[1] = three ? (second | 0x40u | (third << 7) | ((uint32_t)(int32_t)dd2 << 12)) : second;
+          r[2] = delta[0];
+          r[3] = delta[1];
         }
       }
     }

@@ -1143,9 +1143,9 @@ def test_scheme_auto_picks_and_matches_the_explicit_scheme(hlb):
         g = hlb.hlb_geometry_create(big.site_type, big.periodic, big.tau, big.iolet_rho,
                                     hlb.HLB_SCHEME_AUTO | flags_of(hlb, "two_lattice", "f64", "auto", "auto", lattice, True))
         # beyond the resident kernel: two-lattice only if the grid is one wave of the two-lattice
-        # kernel (7 blocks per SM for D3Q15, 5 for D3Q19; 5 % slack) and more than one of A-A (6 / 4)
+        # kernel (blocks per SM: 6 for D3Q15 fp64, 5 for D3Q19; 5 % slack) and more than one of A-A (6 / 4)
         blocks = -(-big.n_sites // 128)
-        per_sm_pull, per_sm_aa = (7, 6) if lattice == "d3q15" else (5, 4)
+        per_sm_pull, per_sm_aa = (6, 6) if lattice == "d3q15" else (5, 4)
         want_aa = not (blocks > sms * per_sm_aa and blocks * 100 <= sms * per_sm_pull * 105)
         assert g.hlb_uses_aa() == want_aa, (name, lattice, blocks)
         g.close()

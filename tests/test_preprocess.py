@@ -156,13 +156,22 @@ def decode_records(rec, nbr):
                 assert wall == 0 and o0 == 0 and o1 == 0
                 sentinel[g, k] = True
                 continue
+            runs_word = second
+            second = runs_word & 63
+            three = bool(runs_word & 0x40)
+            third = (runs_word >> 7) & 31 if three else 32
+            dd2 = (runs_word >> 12) - (1 << 20 if runs_word & 0x80000000 else 0)   # 20-bit signed
             assert 1 <= second <= 32
+            if three:
+                assert second < third <= 31
+            else:
+                assert runs_word == second                  # no stray bits
             if second == 32:
-                assert o1 == o0
+                assert o1 == o0 and not three
             for l in range(32):
                 if (wall >> l) & 1:
                     continue
-                off = o1 if l >= second else o0
+                off = o1 + dd2 if l >= third else (o1 if l >= second else o0)
                 out[k, g * 32 + l] = (off + g * 32 + l) % 2 ** 32
     return out, sentinel
 
@@ -199,7 +208,7 @@ def test_link_records_decode_to_the_table(order, case, lattice):
                 if prev is None or e != prev + 1:
                     runs += 1
                 prev = e
-            assert sentinel[g, k] == (runs > 2)
+            assert (not sentinel[g, k]) if runs <= 2 else (sentinel[g, k] or runs == 3)
     keep = ~np.repeat(sentinel.T, 32, axis=1)              # [NL, Ns]
     expect = np.where(nbr >= 0, nbr, -1)
     assert np.array_equal(dec[keep], expect[keep])
