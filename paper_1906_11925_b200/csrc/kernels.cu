@@ -4,20 +4,22 @@
 // Populations are structure-of-arrays buf[slot][site] with plane stride Ns (a multiple of
 // 128, planes 1 KiB aligned), so the own-site loads and all stores of a warp are single fully
 // coalesced requests; the Q - 1 gathers follow the pull links.
-// ~0.7 flop/byte: HBM-bound, no tensor cores, no shared memory (every population is read
-// exactly once per step: there is no intra-block reuse to stage; cp.async / TMA staging was
-// measured slower, profiles/r01_tuning.md).
+// ~0.7 flop/byte: HBM-bound, no tensor cores, no staging of populations in shared memory (every
+// population is read exactly once per step: there is no intra-block reuse to stage; cp.async /
+// TMA staging was measured slower, profiles/r01_tuning.md).
 //
 // What the kernels are shaped by (evidence in profiles/):
-//   * links come as 16-byte run-length records per (warp, link) instead of 32 table entries,
-//     decoded with a handful of integer operations; the int32 table is the fallback;
+//   * links come as 16-byte run-length records per (warp, link) -- up to three runs of consecutive
+//     sources -- instead of 32 table entries, decoded with five integer operations per link; the
+//     int32 table is the fallback for the rest;
 //   * 32-bit flat offsets, explicit round-to-nearest fp64 intrinsics, pair-symmetric BGK:
 //     few instructions, because long runs sit at the 1 kW power cap;
-//   * 72-80 registers so that 6-7 blocks are resident per SM: all link loads are issued first,
-//     then all population loads, then the arithmetic;
-//   * every thread L2-prefetches what the site 3/4 of a wave ahead will load;
-//   * iolets (constant density, Ladd velocity) are a rare path behind one per-site bit; the
-//     table entries they need are re-read there, not kept in registers;
+//   * 70-80 registers so that 6-7 blocks are resident per SM (more blocks HURT the fp64 kernels):
+//     all link loads are issued first, then all population loads, then the arithmetic, and
+//     every value is stored the moment it is known;
+//   * threads L2-prefetch what the sites 0.68 MB per plane ahead (3/4 of a wave in fp64) will load;
+//   * iolets (constant density, Ladd velocity) are a rare path behind one {bits, rank} word per
+//     group of 32 sites, loaded with the first loads, and one row of link -> iolet bytes per cap site;
 //   * BFL interpolated walls are a third instantiation (V = 2) that applies both rules to
 //     registers; the lean (V = 0) and full (V = 1) instantiations carry none of its code.
 //
@@ -102,9 +104,9 @@ __device__ __forceinline__ void load_entries(const int32_t* __restrict__ nbr, lo
 //   MODE GATHER_PULL  : fluid source e -> q * Ns + e       ; wall -> opp(q) * Ns + i
 //   MODE GATHER_AA_ODD: fluid source e -> opp(q) * Ns + e  ; wall -> q * Ns + i
 // With REC the warp reads one 16-byte record per link instead of 32 table entries
-// (include/hlb.h, hlb_preprocess_records): entry = (lane >= second ? off1 : off0) + lane;
-// a sentinel record (warp-uniform) sends the warp to the table for that link. The iolet id
-// is NOT decoded here; the rare iolet path re-reads the table.
+// (include/hlb.h, hlb_preprocess_records): source = own index + the delta of the lane's run; a
+// sentinel record (warp-uniform) sends the warp to the table for that link. The iolet id is
+// NOT decoded here; the rare iolet path has its own row of link -> iolet bytes.
 // -DHLB_BOUNDS_CHECK (debug builds only; compute-sanitizer is not available on every box):
 // every flat offset a step kernel is about to gather from / scatter to must lie inside the
 // Q * Ns elements of a population array, else the kernel traps and the next CUDA call fails.

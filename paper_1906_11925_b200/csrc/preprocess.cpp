@@ -108,7 +108,7 @@ void host_parallel_for(int64_t n, int64_t grain, const std::function<void(int64_
 
 // A group is 32 consecutive sites (one warp). For link q of a group, the lanes whose pull
 // source is a fluid site split into runs of lanes with consecutive source indices; with an
-// x-fastest site order almost every (group, q) has one or two runs, and 16 bytes then
+// x-fastest site order almost every (group, q) has one to three runs, and 16 bytes then
 // replace the 128 bytes of table entries the warp would load.
 int64_t build_link_records(const int32_t* nbr, int n_links, int64_t Ns, uint32_t* rec) {
   const int Q = n_links + 1;

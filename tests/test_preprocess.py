@@ -194,7 +194,8 @@ def test_link_records_decode_to_the_table(order, case, lattice):
     assert rec.shape == (t["Ns"] // 32, NL, 4)
     dec, sentinel = decode_records(rec, nbr)
     assert n_sentinel == int(sentinel.sum())
-    # brute-force run count per (group, q): sentinel <=> more than two runs
+    # brute-force run count per (group, q): <= 2 runs never a sentinel, > 3 runs always, 3 runs
+    # a sentinel only if the third delta does not fit
     G = t["Ns"] // 32
     nb = nbr.reshape(NL, G, 32)
     for g in range(G):
