@@ -626,6 +626,7 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   const size_t nf = (size_t)((n_sites + 31) / 32 * 32 + 32);
   const size_t row = (size_t)bfl_row_doubles(Q == 19);
   std::vector<double> coef(row * nf, 0.0);
+  std::vector<uint32_t> member(nf, 0u);
   // list form for the read-out pre-pass: the links with d < 1/2 only (the others are already
   // in what the step kernels write)
   std::vector<int32_t> l_site, l_behind;
@@ -636,13 +637,21 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
     const size_t at = (size_t)rank[(size_t)(i >> 5)] +
                       (size_t)__builtin_popcount(bits[(size_t)(i >> 5)] & ((1u << (i & 31)) - 1u));
     const double dd = a_d[l];
-    coef[at * row + (size_t)(a_link[l] - 1)] = dd < 0.5 ? 2.0 * dd : -(1.0 / (2.0 * dd));
+    // one coefficient per opposite pair (2k + 1, 2k + 2) -- its two links are never both
+    // interpolated: each needs the site on the other side to be fluid -- and the member word
+    const size_t k = (size_t)(a_link[l] - 1) / 2;
+    coef[at * row + k] = dd < 0.5 ? 1.0 - 2.0 * dd : -(1.0 - 1.0 / (2.0 * dd));  // +-(1 - a), kernels.cu
+    if ((a_link[l] - 1) & 1) member[at] |= 1u << k;
     if (dd < 0.5) {
       l_site.push_back(a_site[l]);
       l_behind.push_back(a_behind[l]);
       l_link.push_back(a_link[l]);
       l_d.push_back(dd);
     }
+  }
+  for (size_t at = 0; at < nf; ++at) {  // the member word sits behind the (Q-1)/2 coefficients of the row
+    const uint64_t word = member[at];
+    std::memcpy(&coef[at * row + (size_t)(Q - 1) / 2], &word, sizeof(double));
   }
   const size_t nl = l_site.size();
   void *d_site = nullptr, *d_behind = nullptr, *d_link = nullptr, *d_d = nullptr;

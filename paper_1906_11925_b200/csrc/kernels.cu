@@ -83,11 +83,25 @@ template <typename L, typename ST, bool REC> constexpr int pull_f64_drop() {
 }
 // (see link_offsets: shared-memory records in the 4-byte-storage A-A odd kernel)
 template <typename ST, bool REC> constexpr bool odd_rec_smem() { return sizeof(ST) == 4 && REC; }
+// Interpolated walls (V = 2) with 8-byte storage: the gather kernels take one block MORE (7, 72
+// registers, 8-20 offsets and coefficients in local memory) -- their flagged warps wait for a
+// coefficient row on top of everything else, and more warps hide that better than registers
+// do: k_aa_odd 0.233 -> 0.226 ms, k_pull 0.212 -> 0.2095 on configs[3] with every wall link
+// interpolated; 5 blocks 0.245, 8 blocks 0.255 / 0.225; the even kernel 0.194 either way. With
+// 4-byte storage the odd kernel keeps its seventh block with V = 2 as well (0.185 -> 0.179 ms).
+// (profiles/r02_tuning.md section 15)
+#ifndef HLB_BFL_GATHER_ADD
+#define HLB_BFL_GATHER_ADD 1
+#endif
 template <typename L, typename ST, bool REC, typename IT, int V> constexpr int odd_smem_minb_add() {
-  return odd_rec_smem<ST, REC>() && L::Q == 15 && sizeof(IT) == 4 && V != 2 ? 1 : 0;  // (64-bit offsets: spills)
+  if (V == 2 && sizeof(ST) == 8 && L::Q == 15) return sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
+  return odd_rec_smem<ST, REC>() && L::Q == 15 && sizeof(IT) == 4 ? 1 : 0;  // (64-bit offsets: spills)
 }
 template <typename L, typename ST> constexpr int aa_even_minb() {
   return HLB_AA_EVEN_MINB + (sizeof(ST) == 4 && L::Q == 15 ? 1 : 0) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
+}
+template <typename L, typename ST, typename IT, int V> constexpr int bfl_pull_add() {
+  return V == 2 && sizeof(ST) == 8 && L::Q == 15 && sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
 }
 
 template <typename L>
@@ -381,73 +395,116 @@ __device__ __forceinline__ void prefetch_block_planes(const ST* a, long long Ns,
 //              writes back for link p.
 // Neither needs a memory access beyond the coefficients. Two links p and opp(p) of one site
 // are never both interpolated (that needs x + c_p solid and fluid), so updating in place is safe.
-// Who takes the common path (values stored as they become known, then return). Without
-// interpolated walls: every thread that is not a cap site (cap sites are few and clustered).
-// With them (V == 2) the choice is made per WARP, from the group's words: flagged sites are 16 %
-// of all and sit in two thirds of the warps; letting their lanes alone take the long path makes
-// those warps run both paths one after the other (measured +4...11 %), so a warp with any
-// flagged lane takes the long path with all its lanes, the rules predicated per lane.
-template <int V>
-__device__ __forceinline__ bool lean_path(int irow, uint32_t iolet_bits, uint32_t bfl_bits) {
-  if (V != 2) return irow < 0;
-  return (iolet_bits | bfl_bits) == 0u;  // the same for all lanes of the warp
-}
+// Both rules mix the two members of ONE opposite pair (p, opp(p)) only, and the two links of a
+// pair are never both interpolated (an interpolated link needs the site behind x to be fluid,
+// include/hlb.h), so a site's coefficients are one double per PAIR plus a word that says which
+// member is the link: BflFused in kernels.cuh. And so the rule for the written value fits into
+// the store-as-you-go shape of the common path: the pair-symmetric collision hands over both
+// post-collision values of a pair at once (collide_emit_pairs), the rule is applied to them
+// (branch-free: a coefficient of 0 selects the plain value) and both are stored. Every thread
+// that is not a cap site takes that path; the long path is for cap sites alone, as without
+// interpolated walls. (Round 2 first sent every warp with a flagged lane down a long path
+// that stored nothing early: 17-19 % below the plain kernels; profiles/r02_tuning.md 12, 15.)
 __device__ __forceinline__ uint2 load_bfl_word(const BflFused& bf, long long i) { return __ldg(bf.idx + (i >> 5)); }
+// warp-uniform: does any site of this group of 32 carry an interpolated link? A warp without
+// one runs the plain common path (a third of the warps when every wall link is interpolated).
+__device__ __forceinline__ bool bfl_warp(uint2 w) {
+  return w.x != 0u;
+}
 __device__ __forceinline__ long long bfl_index_of(uint2 w) {
   const unsigned lane = threadIdx.x & 31;
   if (!((w.x >> lane) & 1u)) return -1;
   return (long long)w.y + __popc(w.x & ((1u << lane) - 1u));
 }
-// The coefficients are static: fetch them towards the SM before the populations are waited
-// for, so that the dependent chain bits -> rank -> coef does not add a DRAM round trip. A
-// site's coefficients are one row of bfl_row<L>() doubles (128 B for D3Q15, 160 B for D3Q19),
-// read two at a time.
+// A site's row: P = (Q-1)/2 coefficients, then the member word (bit k set: the interpolated
+// link of pair k is 2k + 2, else 2k + 1), padded to an even count: 64 B for D3Q15, 80 B for
+// D3Q19, 16-byte aligned.
 template <typename L>
-__host__ __device__ constexpr int bfl_row() { return (L::Q - 1 + 3) / 4 * 4; }
+__host__ __device__ constexpr int bfl_row() { return ((L::Q - 1) / 2 + 2) / 2 * 2; }
+// The coefficients are static: fetch them towards the SM before the populations are waited
+// for, so that the dependent chain bits -> rank -> coef does not add a DRAM round trip.
 template <typename L>
 __device__ __forceinline__ void bfl_prefetch(const BflFused& bf, long long idx) {
   const char* row = (const char*)(bf.coef + idx * bfl_row<L>());
-#pragma unroll
-  for (int b = 0; b < bfl_row<L>() * 8; b += 128) asm volatile("prefetch.global.L1 [%0];" ::"l"(row + b));
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(row));
+  if ((bfl_row<L>() * 8) % 128 != 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(row + bfl_row<L>() * 8 - 16));
 }
-// a x + (1 - a) y, in the three-term form: at a = 1 (wall half a link away, d = 1/2) it returns x
-// exactly, so that BFL with d = 1/2 IS halfway bounce-back bit for bit (the two-operation form
-// y + a (x - y) is not, and gained 1 % where tried)
-__device__ __forceinline__ double lerp2(double a, double x, double y) { return fma_(a, x, mul(sub(1.0, a), y)); }
+// Interpolation a x + (1 - a) y in the form x + b (y - x), b = 1 - a computed once on the host:
+// two operations with no data-dependent control flow, b = 0 (no interpolated link in this pair,
+// or the wall exactly half a link away, d = 1/2) returns x exactly -- so plain links need no
+// select, and BFL with d = 1/2 IS halfway bounce-back bit for bit. The stored coefficient is
+// +b for a d < 1/2 link (b = 1 - 2d), -b for a d >= 1/2 link (b = 1 - 1/(2d)).
+// d < 1/2, on the gathered values: h[p] += b (h[opp(p)] - h[p])
 template <typename L>
 __device__ __forceinline__ void bfl_gather(const BflFused& bf, long long idx, double (&h)[L::Q]) {
-  const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
+  constexpr int P = (L::Q - 1) / 2, R = bfl_row<L>();
+  const double* row = bf.coef + idx * R;
+  const unsigned member = (unsigned)__double_as_longlong(__ldg(row + P));
 #pragma unroll
-  for (int k = 0; k < (L::Q - 1) / 2; ++k) {
-    const double2 c = __ldg(row + k);
-    const int p = 2 * k + 1;
-    if (c.x > 0.0) h[p] = lerp2(c.x, h[p], h[opp(p)]);
-    if (c.y > 0.0) h[p + 1] = lerp2(c.y, h[p + 1], h[opp(p + 1)]);
+  for (int k = 0; k < P; k += 2) {  // two pairs per 16-byte load
+    const double2 v = __ldg((const double2*)row + k / 2);
+#pragma unroll
+    for (int j = k; j < k + 2 && j < P; ++j) {
+      const int a = 2 * j + 1, b = a + 1;
+      const bool s = (member >> j) & 1u;
+      const double cj = j == k ? v.x : v.y;
+      const double cp = cj > 0.0 ? cj : 0.0;
+      const double D = sub(h[a], h[b]);
+      h[a] = fma_(s ? 0.0 : -cp, D, h[a]);
+      h[b] = fma_(s ? cp : 0.0, D, h[b]);
+    }
   }
 }
-// out[p]: the value written back for link p (the bounced h*_opp(p)); h: post-collision
+// d >= 1/2 (coefficient < 0), on the values a site writes back: out[p], the value written for
+// link p, is the bounced h*_opp(p) without interpolation, h*_opp(p) + b (h*_p - h*_opp(p)) with
+// it. BflWrite: what a thread needs for that, read before the collision; the coefficients
+// themselves are read pair by pair (L1 hits after bfl_gather / the prefetch), not kept in
+// 14-18 registers.
+struct BflWrite {
+  const double* row;  // NULL: no interpolated link at this site
+  unsigned member;
+};
+template <typename L>
+__device__ __forceinline__ BflWrite bfl_write_begin(const BflFused& bf, long long idx) {
+  BflWrite w;
+  w.row = nullptr;
+  w.member = 0u;
+  if (idx >= 0) {
+    w.row = bf.coef + idx * bfl_row<L>();
+    asm volatile("" : "+l"(w.row));  // read again below, do not keep bfl_gather's copies alive
+    w.member = (unsigned)__double_as_longlong(__ldg(w.row + (L::Q - 1) / 2));
+  }
+  return w;
+}
+// pair (a, a + 1) with post-collision values va, vb: oa = out[a], ob = out[a + 1]
+__device__ __forceinline__ void bfl_pair(const BflWrite& w, int a, double va, double vb, double& oa, double& ob) {
+  const int k = (a - 1) / 2;
+  double c = 0.0;
+  if (w.row) c = __ldg(w.row + k);
+  const bool s = (w.member >> k) & 1u;
+  const double cn = c < 0.0 ? c : 0.0;  // -b
+  const double D = sub(va, vb);
+  oa = fma_(s ? 0.0 : -cn, D, vb);
+  ob = fma_(s ? cn : 0.0, D, va);
+}
+// the same on whole arrays, for the cap-site path. h: post-collision; out[p] as above
 template <typename L>
 __device__ __forceinline__ void bfl_write(const BflFused& bf, long long idx, const double (&h)[L::Q],
                                           double (&out)[L::Q]) {
-  const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
+  const BflWrite w = bfl_write_begin<L>(bf, idx);
 #pragma unroll
-  for (int k = 0; k < (L::Q - 1) / 2; ++k) {
-    const double2 c = __ldg(row + k);
-    const int p = 2 * k + 1;
-    if (c.x < 0.0) out[p] = lerp2(-c.x, out[p], h[p]);
-    if (c.y < 0.0) out[p + 1] = lerp2(-c.y, out[p + 1], h[p + 1]);
-  }
+  for (int a = 1; a < L::Q; a += 2) bfl_pair(w, a, h[a], h[a + 1], out[a], out[a + 1]);
 }
-// two-lattice: the value written back for link p is h[opp(p)] itself
+// two-lattice: the value written back for link p is slot opp(p) of the site
 template <typename L>
 __device__ __forceinline__ void bfl_write_pull(const BflFused& bf, long long idx, double (&h)[L::Q]) {
-  const double2* row = (const double2*)(bf.coef + idx * bfl_row<L>());
+  const BflWrite w = bfl_write_begin<L>(bf, idx);
 #pragma unroll
-  for (int k = 0; k < (L::Q - 1) / 2; ++k) {
-    const double2 c = __ldg(row + k);
-    const int p = 2 * k + 1;
-    if (c.x < 0.0) h[opp(p)] = lerp2(-c.x, h[opp(p)], h[p]);
-    if (c.y < 0.0) h[opp(p + 1)] = lerp2(-c.y, h[opp(p + 1)], h[p + 1]);
+  for (int a = 1; a < L::Q; a += 2) {
+    double oa, ob;
+    bfl_pair(w, a, h[a], h[a + 1], oa, ob);
+    h[a + 1] = oa;
+    h[a] = ob;
   }
 }
 
@@ -460,6 +517,7 @@ __device__ __forceinline__ void bfl_write_pull(const BflFused& bf, long long idx
 // x itself, as the halfway bounce-back value of its wall link p; the pre-pass replaces it by
 //   d <  1/2:  2d f*_opp(p)(x) + (1 - 2d) f*_opp(p)(x + c_p)      (slot opp(p) of the site behind)
 //   d >= 1/2:  f*_opp(p)(x) / (2d) + (1 - 1/(2d)) f*_p(x)         (slot p of x itself)
+// (evaluated as x + (1 - a) (y - x), like the step kernels)
 // The sources are slots that no link of the list writes (a link is in the list only if the
 // site behind it is fluid), so the pass has no ordering hazards. As the way to apply BFL on
 // every step it cost 23-25 % of configs[3] against 12-18 % in registers (profiles/r01_tuning.md
@@ -516,15 +574,11 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
 #pragma unroll
   for (int k = 0; k < BFL_UNROLL; ++k)
     if (dd[k] > 0.0) {
+      // the step kernels' form and operation order (bitwise the same: a read-out between two
+      // steps does not change an fp64 run): x + (1 - a) (y - x), 1 - a as the host computes it
       const double two_d = mul(2.0, dd[k]);
-      double r;
-      if (dd[k] < 0.5) {
-        r = lerp2(two_d, a[k], b[k]);
-      } else {
-        const double inv = __ddiv_rn(1.0, two_d);
-        r = lerp2(inv, a[k], b[k]);
-      }
-      buf[tgt[k]] = to_store<ST>(r);
+      const double w = dd[k] < 0.5 ? sub(1.0, two_d) : sub(1.0, __ddiv_rn(1.0, two_d));
+      buf[tgt[k]] = to_store<ST>(fma_(w, sub(b[k], a[k]), a[k]));
     }
 }
 
@@ -542,7 +596,7 @@ k_bfl_prepass(ST* __restrict__ buf, long long Ns, const int32_t* __restrict__ si
 // (profiles/r02_tuning.md). Safe in the in-place kernels too: a site's read set is its own
 // write set, so nobody else has written these slots, and this thread has not stored yet.
 template <typename L, typename ST, bool REC, typename IT, int V>
-__global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>() - pull_f64_drop<L, ST, REC>())
+__global__ void __launch_bounds__(SBLOCK, pull_minb<L, REC>() - pull_f64_drop<L, ST, REC>() + bfl_pull_add<L, ST, IT, V>())
 k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restrict__ nbr,
        const uint4* __restrict__ rec, IoletIndex io, const double* __restrict__ iolet_par,
        long long Ns, Relax rx, Planes pl, long long pf, BflFused bf) {
@@ -583,8 +637,19 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
   ST* d = dst + i;
   // (no second gather here, unlike the A-A kernels: the offsets are dead by now, and keeping
   // the gathered values for the rare path costs this kernel nothing measurable)
-  if (lean_path<V>(irow, iow.x, bw.x)) {  // common path: every value is stored as soon as it is known
-    collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { d[(long long)q * Ns] = to_store<ST>(v); });
+  if (irow < 0) {  // common path: every value is stored as soon as it is known
+    if (V == 2 && bfl_warp(bw)) {  // slot opp(p) holds what link p reads next step
+      const BflWrite w = bfl_write_begin<L>(bf, bidx);
+      collide_emit_pairs<L, sizeof(ST) == 4>(h, m, rx, [&](double v) { d[0] = to_store<ST>(v); },
+        [&](int a, double va, double vb) {
+          double oa, ob;
+          bfl_pair(w, a, va, vb, oa, ob);
+          d[(long long)a * Ns] = to_store<ST>(ob);
+          d[(long long)(a + 1) * Ns] = to_store<ST>(oa);
+        });
+    } else {
+      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { d[(long long)q * Ns] = to_store<ST>(v); });
+    }
     return;
   }
   collide<L, sizeof(ST) == 4>(h, m, rx, h);
@@ -629,12 +694,24 @@ k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_pa
   if (pf > 0 && i + pf < Ns) prefetch_block_planes<L, ST>(a, Ns, pf);  // block-uniform test
   opaque(Ns);  // the stores rebuild their addresses (else 15 address pairs stay live: spills)
   const int irow = iolet_row_of(iow);
-  if (lean_path<V>(irow, iow.x, bw.x)) {  // common path: h*_q goes to slot opp(q) as soon as it is known
+  if (irow < 0) {  // common path: h*_q goes to slot opp(q) as soon as it is known
+    if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
     const Moments m = moments_of<L>(h);
-    collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
+    if (V == 2 && bfl_warp(bw)) {
+      const BflWrite w = bfl_write_begin<L>(bf, bidx);
+      collide_emit_pairs<L, sizeof(ST) == 4>(h, m, rx, [&](double v) { p0[0] = to_store<ST>(v); },
+        [&](int a, double va, double vb) {
+          double oa, ob;
+          bfl_pair(w, a, va, vb, oa, ob);
+          p0[(long long)a * Ns] = to_store<ST>(oa);
+          p0[(long long)(a + 1) * Ns] = to_store<ST>(ob);
+        });
+    } else {
+      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) { p0[(long long)opp(q) * Ns] = to_store<ST>(v); });
+    }
     return;
   }
-  if (V != 2) {  // rare path (cap sites): read again; with interpolated walls two thirds of the warps are here
+  {  // rare path (cap sites): read again
     const ST* again = relaunder(p0);
 #pragma unroll
     for (int q = 0; q < L::Q; ++q) h[q] = to_real(again[(long long)q * Ns]);
@@ -689,15 +766,27 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
 #pragma unroll
   for (int q = 1; q < L::Q; ++q) opaque(off[q - 1]);
   const int irow = iolet_row_of(iow);
-  if (lean_path<V>(irow, iow.x, bw.x)) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
+  if (irow < 0) {  // common path: h*_q goes where f_opp(q) was read, as soon as it is known
+    if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
     const Moments m = moments_of<L>(h);
-    collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) {
-      if (q == 0) a[i] = to_store<ST>(v);
-      else a[off[opp(q) - 1]] = to_store<ST>(v);
-    });
+    if (V == 2 && bfl_warp(bw)) {
+      const BflWrite w = bfl_write_begin<L>(bf, bidx);
+      collide_emit_pairs<L, sizeof(ST) == 4>(h, m, rx, [&](double v) { a[i] = to_store<ST>(v); },
+        [&](int p, double va, double vb) {
+          double oa, ob;
+          bfl_pair(w, p, va, vb, oa, ob);
+          a[off[p - 1]] = to_store<ST>(oa);
+          a[off[p]] = to_store<ST>(ob);
+        });
+    } else {
+      collide_emit<L, sizeof(ST) == 4>(h, m, rx, [&](int q, double v) {
+        if (q == 0) a[i] = to_store<ST>(v);
+        else a[off[opp(q) - 1]] = to_store<ST>(v);
+      });
+    }
     return;
   }
-  if (V != 2) {  // rare path (cap sites): read again; with interpolated walls two thirds of the warps are here
+  {  // rare path (cap sites): read again
     const ST* again = relaunder(a);
     h[0] = to_real(again[i]);
 #pragma unroll

@@ -23,10 +23,12 @@ struct BflLinks {
 // link; such a site has the dense index rank + popcount(bits below lane i % 32). ONE 8-byte word
 // per group, loaded with the kernel's first loads: as two arrays read one after the other (bits,
 // then rank only where flagged) they put two dependent memory round trips in front of the link
-// records (profiles/r02_tuning.md section 12). coef[idx * row
-// + p - 1] (row = bfl_row_doubles(): Q-1 rounded up to a multiple of 4; 16-byte aligned) is,
-// for its pull link p,  2d  where d < 1/2 (applied while gathering),  -1/(2d)
-// where d >= 1/2 (applied to the value the site writes back for that link),  0 = plain
+// records (profiles/r02_tuning.md section 12). A site's row coef[idx * row ...] (row =
+// bfl_row_doubles() doubles, 16-byte aligned) holds ONE coefficient per opposite pair of links
+// (2k + 1, 2k + 2), k = 0 .. (Q-1)/2 - 1 -- the two are never both interpolated --, then a
+// 64-bit word whose bit k says which member is the interpolated link (1: 2k + 2). The
+// coefficient is, for that pull link,  1 - 2d  where d < 1/2 (applied while gathering),
+// -(1 - 1/(2d))  where d >= 1/2 (applied to the value the site writes back for that link),  0 = plain
 // bounce-back. gather = 0 when the d < 1/2 part is already in the state buffer (pre-pass
 // run for a read-out) or does not apply (the initial state).
 struct BflFused {

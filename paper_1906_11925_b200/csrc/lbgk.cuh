@@ -119,12 +119,14 @@ __device__ __forceinline__ double heq_of(int q, double drho, double rho, double 
 // emit(q, hs_q) is called as soon as a post-collision value is known, so that a kernel can
 // store it at once and free its registers (and those of its address): with all stores after
 // the whole collision the A-A odd kernel kept 7 of its 14 offsets in local memory.
-template <typename L, bool FOLDED, typename F>
-__device__ __forceinline__ void collide_emit(const double (&h)[L::Q], const Moments& m, const Relax& rx,
-                                             F&& emit) {
+// emit0(hs_0) and emit2(a, hs_a, hs_b) for each opposite pair (a, b = a + 1): the form the kernels
+// with interpolated walls use -- both BFL rules mix the two members of one pair only.
+template <typename L, bool FOLDED, typename F0, typename F2>
+__device__ __forceinline__ void collide_emit_pairs(const double (&h)[L::Q], const Moments& m, const Relax& rx,
+                                                   F0&& emit0, F2&& emit2) {
   const double uu15 = mul(1.5, u_dot_u(m.ux, m.uy, m.uz));
   if (FOLDED) {
-    emit(0, fma_(rx.omc, h[0], mul(rx.w0, fma_(-m.rho, uu15, m.drho))));
+    emit0(fma_(rx.omc, h[0], mul(rx.w0, fma_(-m.rho, uu15, m.drho))));
     const double r3_axis = mul(rx.a3, m.rho), r3_diag = mul(rx.d3, m.rho);
 #pragma unroll
     for (int a = 1; a < L::Q; a += 2) {
@@ -132,13 +134,12 @@ __device__ __forceinline__ void collide_emit(const double (&h)[L::Q], const Mome
       const double cu = c_dot_u<L>(a, m.ux, m.uy, m.uz);
       const double S = mul(a <= 6 ? rx.wa : rx.wd, fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
       const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
-      emit(a, fma_(rx.omc, h[a], add(S, A)));
-      emit(b, fma_(rx.omc, h[b], sub(S, A)));
+      emit2(a, fma_(rx.omc, h[a], add(S, A)), fma_(rx.omc, h[b], sub(S, A)));
     }
   } else {
     const double omega = rx.omega;
     const double heq0 = mul(L::weight(0), fma_(-m.rho, uu15, m.drho));
-    emit(0, fma_(omega, sub(heq0, h[0]), h[0]));
+    emit0(fma_(omega, sub(heq0, h[0]), h[0]));
     // two weight classes: axis (q = 1..6) and diagonal (q >= 7)
     const double r3_axis = mul(3.0 * L::weight(1), m.rho), r3_diag = mul(3.0 * L::weight(7), m.rho);
 #pragma unroll
@@ -148,10 +149,15 @@ __device__ __forceinline__ void collide_emit(const double (&h)[L::Q], const Mome
       const double S = mul(L::weight(a), fma_(m.rho, fma_(mul(4.5, cu), cu, -uu15), m.drho));
       const double A = mul(a <= 6 ? r3_axis : r3_diag, cu);
       const double ha = h[a], hb = h[b];
-      emit(a, fma_(omega, sub(add(S, A), ha), ha));
-      emit(b, fma_(omega, sub(sub(S, A), hb), hb));
+      emit2(a, fma_(omega, sub(add(S, A), ha), ha), fma_(omega, sub(sub(S, A), hb), hb));
     }
   }
+}
+template <typename L, bool FOLDED, typename F>
+__device__ __forceinline__ void collide_emit(const double (&h)[L::Q], const Moments& m, const Relax& rx,
+                                             F&& emit) {
+  collide_emit_pairs<L, FOLDED>(h, m, rx, [&](double v) { emit(0, v); },
+                                [&](int a, double va, double vb) { emit(a, va); emit(a + 1, vb); });
 }
 template <typename L, bool FOLDED>
 __device__ __forceinline__ void collide(const double (&h)[L::Q], const Moments& m, const Relax& rx,
