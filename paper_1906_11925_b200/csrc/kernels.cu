@@ -416,6 +416,16 @@ __device__ __forceinline__ long long bfl_index_of(uint2 w) {
   if (!((w.x >> lane) & 1u)) return -1;
   return (long long)w.y + __popc(w.x & ((1u << lane) - 1u));
 }
+// (-DHLB_BOUNDS_CHECK: the row index must lie inside the nf rows of the table)
+__device__ __forceinline__ long long bfl_index_of(const BflFused& bf, uint2 w) {
+  const long long idx = bfl_index_of(w);
+#ifdef HLB_BOUNDS_CHECK
+  if (idx >= bf.nf) __trap();
+#else
+  (void)bf;
+#endif
+  return idx;
+}
 // A site's row: P = (Q-1)/2 coefficients, then the member word (bit k set: the interpolated
 // link of pair k is 2k + 2, else 2k + 1), padded to an even count: 64 B for D3Q15, 80 B for
 // D3Q19, 16-byte aligned.
@@ -612,7 +622,7 @@ k_pull(const ST* __restrict__ src, ST* __restrict__ dst, const int32_t* __restri
     IT off[L::Q - 1];
     link_offsets<L, GATHER_PULL, REC, IT>(nbr, rec, Ns, i, pl, off);
     if (V == 2) {  // the row request goes out before the gathers and travels with them
-      bidx = bfl_index_of(bw);
+      bidx = bfl_index_of(bf, bw);
       if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
     }
     pdl_wait_for_previous_step();
@@ -688,7 +698,7 @@ k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_pa
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) h[q] = to_real(p0[(long long)q * Ns]);
   if (V == 2) {  // after the population loads are issued: waiting for the word must not delay them
-    bidx = bfl_index_of(bw);
+    bidx = bfl_index_of(bf, bw);
     if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
   }
   if (pf > 0 && i + pf < Ns) prefetch_block_planes<L, ST>(a, Ns, pf);  // block-uniform test
@@ -743,7 +753,7 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
   constexpr bool REC_SMEM = sizeof(ST) == 4 && REC;  // = odd_rec_smem<ST, REC>()
   link_offsets<L, GATHER_AA_ODD, REC, IT, REC_SMEM>(nbr, rec, Ns, i, pl, off);
   if (V == 2) {  // the row request goes out before the gathers and travels with them
-    bidx = bfl_index_of(bw);
+    bidx = bfl_index_of(bf, bw);
     if (bidx >= 0) bfl_prefetch<L>(bf, bidx);
   }
   const uint2 iow = load_iolet_word(io, i);  // (not before the decode: its registers are the scarce ones)
