@@ -89,12 +89,13 @@ template <typename ST, bool REC> constexpr bool odd_rec_smem() { return sizeof(S
 // do: k_aa_odd 0.233 -> 0.226 ms, k_pull 0.212 -> 0.2095 on configs[3] with every wall link
 // interpolated; 5 blocks 0.245, 8 blocks 0.255 / 0.225; the even kernel 0.194 either way. With
 // 4-byte storage the odd kernel keeps its seventh block with V = 2 as well (0.185 -> 0.179 ms).
+// D3Q19: k_aa_odd 4 -> 5 blocks 0.3145 -> 0.2944 ms (6: 0.3276); k_pull stays at 5 (6: 0.272 -> 0.283).
 // (profiles/r02_tuning.md section 15)
 #ifndef HLB_BFL_GATHER_ADD
 #define HLB_BFL_GATHER_ADD 1
 #endif
 template <typename L, typename ST, bool REC, typename IT, int V> constexpr int odd_smem_minb_add() {
-  if (V == 2 && sizeof(ST) == 8 && L::Q == 15) return sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
+  if (V == 2 && sizeof(ST) == 8) return sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
   return odd_rec_smem<ST, REC>() && L::Q == 15 && sizeof(IT) == 4 ? 1 : 0;  // (64-bit offsets: spills)
 }
 template <typename L, typename ST> constexpr int aa_even_minb() {

@@ -5,6 +5,7 @@ Bar (BASELINE.json north_star): fp64 rho and u within 1e-12 relative max error, 
 fp32-storage variant within 1e-5. Norm (reading R-norm):
 E_rho = max|rho - rho_ref| / max|rho_ref|,  E_u = max_{x,a}|u_a - u_ref,a| / max_x |u_ref|_2.
 """
+import dataclasses
 import math
 import os
 
@@ -1177,6 +1178,24 @@ def test_full_configs_full_steps_record(hlb, name, record):
         e_rho, e_u = errors(*run_gpu(hlb, wl, wl.steps, "aa", "f64", "auto", "auto", "d3q19"), rho19, u19)
         record(f"RECORD {name} N={wl.n_sites} steps={wl.steps} D3Q19 aa/f64 E_rho={e_rho:.3e} E_u={e_u:.3e} (bar 1e-12)")
         assert e_rho < TOL["f64"] and e_u < TOL["f64"]
+
+
+@pytest.mark.slow
+def test_config3_full_size_with_every_wall_link_interpolated_record(hlb, record):
+    """NEXT-2 at the size bench.py times it (--workload tree --inlet velocity --walls bfl_random):
+    all 4.9 M sites of configs[3], a Ladd velocity inlet and a seeded random wall distance on
+    every wall link (0.8 M sites carry one; row ranks far beyond 16 bits), every site against
+    the oracle, both schemes, both storage types; odd step count for the in-place scheme."""
+    wl = W.with_velocity_inlet(W.by_name("tree"))
+    d27 = np.random.default_rng(1906).uniform(0.05, 1.0, size=(wl.n_sites, 27))
+    wl = dataclasses.replace(wl, wall_distance=d27)
+    refs = {steps: run_oracle(wl, steps) for steps in (100, 101)}
+    for scheme, store, steps in (("two_lattice", "f64", 100), ("aa", "f64", 101), ("aa", "f32", 101),
+                                 ("two_lattice", "f32", 100)):
+        e_rho, e_u = errors(*run_gpu(hlb, wl, steps, scheme, store, "auto"), *refs[steps])
+        record(f"RECORD tree + velocity inlet + BFL on every wall link N={wl.n_sites} steps={steps} "
+               f"{scheme}/{store} E_rho={e_rho:.3e} E_u={e_u:.3e} (bar {TOL[store]:.0e})")
+        assert e_rho < TOL[store] and e_u < TOL[store]
 
 
 # ------------------------------------------------------------- the sizes the library claims
