@@ -946,27 +946,45 @@ k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __
 }
 
 // ------------------------------------------------------------------ read-out / init
-template <typename L, typename ST, int MODE>
+// REC: the sources come from the 16-byte link records (7 B per site) instead of the int32 table
+// (56 / 72 B per site) wherever the geometry has records -- the read-outs are HBM-bound like the
+// step kernels, and the table was a quarter of what they moved. READOUT_MINB: the decode holds
+// Q - 1 records of four words for a moment; without a bound ptxas takes 70-92 registers (two or
+// three blocks of 256 per SM) and the two dependent round trips (records, then populations) are
+// not covered (profiles/r02_tuning.md section 16).
+#ifndef HLB_READOUT_MINB
+#define HLB_READOUT_MINB 4
+#endif
+constexpr int READOUT_MINB = HLB_READOUT_MINB;
+template <typename L, typename ST, int MODE, bool REC, typename IT>
 __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
-                                                    const int32_t* __restrict__ nbr, long long Ns,
-                                                    long long i, double (&h)[L::Q]) {
+                                                    const int32_t* __restrict__ nbr,
+                                                    const uint4* __restrict__ rec, long long Ns,
+                                                    const Planes& pl, long long i, double (&h)[L::Q]) {
+  h[0] = to_real(buf[i]);
+  if (REC && MODE != GATHER_OWN) {
+    IT off[L::Q - 1];
+    link_offsets<L, MODE, true, IT>(nbr, rec, Ns, i, pl, off);
+#pragma unroll
+    for (int q = 1; q < L::Q; ++q) h[q] = to_real(buf[off[q - 1]]);
+    return;
+  }
   int32_t e[L::Q - 1];
   if (MODE != GATHER_OWN) load_entries<L>(nbr, Ns, i, e);
-  h[0] = to_real(buf[i]);
 #pragma unroll
   for (int q = 1; q < L::Q; ++q)
     h[q] = to_real(buf[slot_of<MODE>(q, MODE != GATHER_OWN ? e[q - 1] : 0, Ns, i)]);
 }
 
-template <typename L, typename ST, int MODE>
-__global__ void __launch_bounds__(BLOCK)
-k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
+template <typename L, typename ST, int MODE, bool REC, typename IT>
+__global__ void __launch_bounds__(BLOCK, READOUT_MINB)
+k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec, Planes pl,
               const int32_t* __restrict__ canon, long long N, long long Ns,
               double* __restrict__ rho, double* __restrict__ u) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  gather_precollision<L, ST, MODE, REC, IT>(buf, nbr, rec, Ns, pl, i, h);
   const Moments m = moments_of<L>(h);
   const long long c = canon[i];
   if (rho) rho[c] = m.rho;
@@ -980,15 +998,15 @@ k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
 // Deviatoric (viscous) stress of the pre-collision state, canonical order, [N][6] in the
 // order xx, yy, zz, xy, xz, yz:  sigma_ab = -(1 - omega / 2) sum_q c_qa c_qb (h_q - heq_q)
 // (the shift w_q cancels in h - heq).
-template <typename L, typename ST, int MODE>
-__global__ void __launch_bounds__(BLOCK)
-k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
+template <typename L, typename ST, int MODE, bool REC, typename IT>
+__global__ void __launch_bounds__(BLOCK, READOUT_MINB)
+k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec, Planes pl,
          const int32_t* __restrict__ canon, long long N, long long Ns, double omega,
          double* __restrict__ sigma) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  gather_precollision<L, ST, MODE, REC, IT>(buf, nbr, rec, Ns, pl, i, h);
   const Moments m = moments_of<L>(h);
   double pi[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
@@ -1028,15 +1046,15 @@ k_wall_shear_stress(const double* __restrict__ sigma, const double* __restrict__
   wss[c] = sqrt(a * a + b * b + d * d);
 }
 
-template <typename L, typename ST, int MODE>
-__global__ void __launch_bounds__(BLOCK)
-k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr,
+template <typename L, typename ST, int MODE, bool REC, typename IT>
+__global__ void __launch_bounds__(BLOCK, READOUT_MINB)
+k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec, Planes pl,
                   const int32_t* __restrict__ canon, long long N, long long Ns,
                   double* __restrict__ f) {
   const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
   if (i >= N) return;
   double h[L::Q];
-  gather_precollision<L, ST, MODE>(buf, nbr, Ns, i, h);
+  gather_precollision<L, ST, MODE, REC, IT>(buf, nbr, rec, Ns, pl, i, h);
   const long long c = canon[i];
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) f[c * L::Q + q] = h[q] + L::weight(q);
@@ -1199,9 +1217,17 @@ static void macroscopic_t(const DeviceGeometry& g, const void* buf, GatherMode m
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_macroscopic<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
-    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
-    case GATHER_AA_ODD: k_macroscopic<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_PULL:
+      if (g.use_rec && !g.index64) k_macroscopic<L, ST, GATHER_PULL, true, uint32_t><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, rho, u);
+      else if (g.use_rec) HLB_FULL_ONLY((k_macroscopic<L, ST, GATHER_PULL, true, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, rho, u)));
+      else HLB_FULL_ONLY((k_macroscopic<L, ST, GATHER_PULL, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, rho, u)));
+      break;
+    case GATHER_OWN: k_macroscopic<L, ST, GATHER_OWN, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, rho, u); break;
+    case GATHER_AA_ODD:
+      if (g.use_rec && !g.index64) k_macroscopic<L, ST, GATHER_AA_ODD, true, uint32_t><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, rho, u);
+      else if (g.use_rec) HLB_FULL_ONLY((k_macroscopic<L, ST, GATHER_AA_ODD, true, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, rho, u)));
+      else HLB_FULL_ONLY((k_macroscopic<L, ST, GATHER_AA_ODD, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, rho, u)));
+      break;
   }
 }
 template <typename L, typename ST>
@@ -1210,9 +1236,17 @@ static void get_populations_t(const DeviceGeometry& g, const void* buf, GatherMo
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_get_populations<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
-    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
-    case GATHER_AA_ODD: k_get_populations<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, f); break;
+    case GATHER_PULL:
+      if (g.use_rec && !g.index64) k_get_populations<L, ST, GATHER_PULL, true, uint32_t><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, f);
+      else if (g.use_rec) HLB_FULL_ONLY((k_get_populations<L, ST, GATHER_PULL, true, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, f)));
+      else HLB_FULL_ONLY((k_get_populations<L, ST, GATHER_PULL, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, f)));
+      break;
+    case GATHER_OWN: k_get_populations<L, ST, GATHER_OWN, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, f); break;
+    case GATHER_AA_ODD:
+      if (g.use_rec && !g.index64) k_get_populations<L, ST, GATHER_AA_ODD, true, uint32_t><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, f);
+      else if (g.use_rec) HLB_FULL_ONLY((k_get_populations<L, ST, GATHER_AA_ODD, true, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, f)));
+      else HLB_FULL_ONLY((k_get_populations<L, ST, GATHER_AA_ODD, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, f)));
+      break;
   }
 }
 template <typename L, typename ST>
@@ -1221,9 +1255,17 @@ static void stress_t(const DeviceGeometry& g, const void* buf, GatherMode mode, 
   const unsigned grid = grid_for(g.N);
   const ST* b = (const ST*)buf;
   switch (mode) {
-    case GATHER_PULL: k_stress<L, ST, GATHER_PULL><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
-    case GATHER_OWN: k_stress<L, ST, GATHER_OWN><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
-    case GATHER_AA_ODD: k_stress<L, ST, GATHER_AA_ODD><<<grid, BLOCK, 0, s>>>(b, g.nbr, g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_PULL:
+      if (g.use_rec && !g.index64) k_stress<L, ST, GATHER_PULL, true, uint32_t><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma);
+      else if (g.use_rec) HLB_FULL_ONLY((k_stress<L, ST, GATHER_PULL, true, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma)));
+      else HLB_FULL_ONLY((k_stress<L, ST, GATHER_PULL, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma)));
+      break;
+    case GATHER_OWN: k_stress<L, ST, GATHER_OWN, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma); break;
+    case GATHER_AA_ODD:
+      if (g.use_rec && !g.index64) k_stress<L, ST, GATHER_AA_ODD, true, uint32_t><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma);
+      else if (g.use_rec) HLB_FULL_ONLY((k_stress<L, ST, GATHER_AA_ODD, true, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, (const uint4*)g.rec, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma)));
+      else HLB_FULL_ONLY((k_stress<L, ST, GATHER_AA_ODD, false, long long><<<grid, BLOCK, 0, s>>>(b, g.nbr, nullptr, planes_of(g), g.canon, g.N, g.Ns, g.omega, sigma)));
+      break;
   }
 }
 template <typename L, typename ST>
