@@ -575,6 +575,7 @@ SWEEP = [
     ("tree", {"store": "f32", "scheme": "auto"}, 100, 36),
     ("bigtree", {"scheme": "two_lattice"}, 50, 7),
     ("bigtree", {"scheme": "aa", "store": "f32"}, 50, 10),
+    ("bigtree", {"scheme": "two_lattice", "store": "f32"}, 50, 9),
     ("bigtree", {"scheme": "aa", "lattice": "d3q19"}, 50, 6),
 ]
 
