@@ -78,7 +78,9 @@ enum {
                               least half of them are not sentinels, else the table         */
   HLB_LINKS_TABLE = 0x20,  /* always read the int32 table (ablation / profiling)           */
   HLB_LINKS_RECORDS = 0x40,/* always read the records                                     */
-  HLB_NO_PREFETCH = 0x80,  /* step kernels issue no L2 prefetches (ablation / profiling)   */
+  HLB_NO_PREFETCH = 0x80,  /* step kernels issue no L2 prefetches (ablation / profiling;
+                              the library issues none by itself where the populations fit
+                              half of the L2 cache)                                        */
   HLB_INDEX64 = 0x100,     /* use the 64-bit flat-offset kernels even when Q * stride fits
                               32 bits (they are otherwise only taken above 286 M sites;
                               this flag lets small tests cover them)                       */

@@ -379,6 +379,19 @@ int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geome
     const int64_t per8 = g->f32 ? 2 : 1;
     g->dg.prefetch_pull = (int64_t)sms * resident_sites_per_sm_pull(Q == 19, g->f32) * 3 / 4 / 128 * 128 * per8;
     g->dg.prefetch_aa = (int64_t)sms * resident_sites_per_sm_aa(Q == 19, g->f32) * 3 / 4 / 128 * 128 * per8;
+    // A state that fits half of the L2 stays there from step to step: the prefetches are then
+    // only instructions (296 k sites, A-A: 10.54 -> 10.05 us per step without them, D3Q19 13.18 ->
+    // 12.61; at 89 MB of state, configs[2] in place, no difference; beyond, they pay:
+    // profiles/r02_tuning.md section 18).
+    {
+      int l2 = 0;
+      const size_t state_bytes = (size_t)Q * (size_t)t.Ns * g->store_bytes() * (g->aa ? 1 : 2);
+      if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) == cudaSuccess && l2 > 0 &&
+          state_bytes <= (size_t)l2 / 2)
+        g->dg.prefetch_pull = g->dg.prefetch_aa = 0;
+      else
+        (void)cudaGetLastError();
+    }
     if (const char* e = std::getenv("HLB_PREFETCH_SITES")) {
       const long long v = std::atoll(e);
       g->dg.prefetch_pull = g->dg.prefetch_aa = v > 0 ? (v < (1ll << 24) ? v : (1ll << 24)) : 0;
