@@ -81,7 +81,7 @@ def parse_args():
                          "waveform handed over by hlb_set_iolet_velocity before every LB step")
     ap.add_argument("--walls", default="bounce_back", choices=["bounce_back", "bfl_random"],
                     help="bfl_random: interpolated (BFL) walls with seeded random distances on every "
-                         "wall link -- the kernel work of the paper's BFL option (two_lattice only)")
+                         "wall link -- the kernel work of the paper's BFL option")
     ap.add_argument("--render", type=int, default=0, metavar="PIXELS",
                     help="also time the ray-marching renderer (NEXT-4) on the final state: PIXELS x "
                          "PIXELS frames of the speed field, rotating view; adds a \"render\" object")
@@ -478,7 +478,8 @@ class Run:
         torch, g, v, nq = self.torch, self.g, self.v, self.nq
         scheme, store = v["scheme"], v["store"]
         rec, sf = bool(g.hlb_uses_records()), g.hlb_record_sentinel_fraction()
-        moved = lambda phase: self.hlb.moved_bytes_per_site(scheme, store, nq, rec, sf, phase)  # noqa: E731
+        bfl = self.g.hlb_num_bfl_sites() / float(self.N)
+        moved = lambda phase: self.hlb.moved_bytes_per_site(scheme, store, nq, rec, sf, phase, bfl)  # noqa: E731
         pop_bytes = nq * 2 * (4 if store == "f32" else 8)
         if launches < S * K:
             name = "k_aa_resident" if scheme == "aa" else "k_pull_resident"
@@ -702,7 +703,8 @@ def main():
     peak, peak_src = measured_peak()
     step_bytes = hlb.algorithmic_bytes_per_site(scheme, args.store, nq)
     moved_step = hlb.moved_bytes_per_site(scheme, args.store, nq, bool(g.hlb_uses_records()),
-                                          g.hlb_record_sentinel_fraction())
+                                          g.hlb_record_sentinel_fraction(), "step",
+                                          g.hlb_num_bfl_sites() / float(N))
     out = {
         "metric": METRIC if nq == 15 else METRIC_Q19, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,

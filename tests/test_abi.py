@@ -99,3 +99,6 @@ def test_moved_bytes_model():
     assert m("aa", "f64", 15, records=True, phase="odd") == 240 + 7 + 0.125
     assert m("aa", "f64", 15, records=True) == 240 + 3.5 + 0.125
     assert m("aa", "f32", 19, records=False, phase="odd") == 152 + 72 + 0.125
+    # interpolated walls: one index word per 32 sites, one 64-byte (D3Q19: 80-byte) row per flagged site
+    assert m("aa", "f64", 15, phase="even", bfl_site_fraction=0.25) == 240 + 0.125 + 0.25 + 16
+    assert m("two_lattice", "f64", 19, bfl_site_fraction=0.5) == 304 + 9 + 0.125 + 0.25 + 40
