@@ -739,6 +739,39 @@ k_aa_even(ST* __restrict__ a, IoletIndex io, const double* __restrict__ iolet_pa
   for (int p = 0; p < L::Q; ++p) p0[(long long)p * Ns] = to_store<ST>(out[p]);
 }
 
+// The cap-site path of k_aa_odd for the instantiations with the full iolet rules (V >= 1), as a
+// function of its own that starts from the site index again (decode, read, update, scatter).
+// Inlined, its register needs made ptxas spill 7 of the 14 offsets where they are DEFINED -- in
+// the decode every thread runs: 7 STL + 14 LDL per thread on the common path of the V = 1 kernel
+// (ncu, profiles/r02_ncu_bfl_readout.md). A call keeps the two allocations apart; nothing is
+// live across it. Used where it was measured to pay: V = 1, D3Q15 (configs[4] with a velocity
+// inlet: odd kernel 1.525 -> 1.515 ms in fp64, 0.926 -> 0.907 with 4-byte storage; configs[3]
+// unchanged). With interpolated walls (V = 2) and on D3Q19 the inlined form is 1-2 % faster.
+template <typename L, typename ST, bool REC, typename IT, int V>
+__device__ __noinline__ void aa_odd_cap_site(ST* __restrict__ a, const int32_t* __restrict__ nbr,
+                                             const uint4* __restrict__ rec, IoletIndex io,
+                                             int irow, const double* __restrict__ iolet_par, long long Ns,
+                                             Relax rx, Planes pl, BflFused bf,  // by value: copied at the call, not in the kernel's prologue
+                                             long long bidx, long long i) {
+  IT off[L::Q - 1];
+  link_offsets<L, GATHER_AA_ODD, REC, IT, false>(nbr, rec, Ns, i, pl, off);
+  double h[L::Q];
+  h[0] = to_real(a[i]);
+#pragma unroll
+  for (int q = 1; q < L::Q; ++q) h[q] = to_real(a[off[q - 1]]);
+  if (V == 2 && bidx >= 0 && bf.gather) bfl_gather<L>(bf, bidx, h);
+  const Moments m = moments_of<L>(h);
+  collide<L, sizeof(ST) == 4>(h, m, rx, h);
+  double out[L::Q];
+#pragma unroll
+  for (int p = 0; p < L::Q; ++p) out[p] = h[opp(p)];
+  if (V == 2 && bidx >= 0) bfl_write<L>(bf, bidx, h, out);
+  iolet_substitute<L, (V >= 1)>(io, irow, i, m, iolet_par, bf.iolet_w, out);
+  a[i] = to_store<ST>(out[0]);
+#pragma unroll
+  for (int p = 1; p < L::Q; ++p) a[off[p - 1]] = to_store<ST>(out[p]);
+}
+
 template <typename L, typename ST, bool REC, typename IT, int V>
 __global__ void __launch_bounds__(SBLOCK, aa_odd_minb<L, REC>() + odd_smem_minb_add<L, ST, REC, IT, V>())
 k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec,
@@ -795,6 +828,10 @@ k_aa_odd(ST* __restrict__ a, const int32_t* __restrict__ nbr, const uint4* __res
         else a[off[opp(q) - 1]] = to_store<ST>(v);
       });
     }
+    return;
+  }
+  if (V == 1 && L::Q == 15) {  // cap sites, full iolet rules: a call (see aa_odd_cap_site)
+    aa_odd_cap_site<L, ST, REC, IT, V>(a, nbr, rec, io, irow, iolet_par, Ns, rx, pl, bf, bidx, i);
     return;
   }
   {  // rare path (cap sites): read again
