@@ -681,7 +681,7 @@ def main():
             g.hlb_stage_state(rin_np, uin_np)                 # H2D of the NEXT step: rho [N], u [N][3]
             g.hlb_get_macroscopic_async(*outs_np[k & 1])      # D2H: rho [N], u [N][3], on the copy stream
 
-        e2e_steps = max(2, min(args.steps, 5))
+        e2e_steps = max(2, min(args.steps, 20))    # the last read-out copy has nothing to hide under: amortised over the steps
         g.hlb_stage_state(rin_np, uin_np)
         e2e_step(0)
         g.hlb_wait_copies()
