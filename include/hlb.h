@@ -415,6 +415,26 @@ int hlb_preprocess_tables(const uint8_t* site_type, const hlb_params* p, int64_t
 int hlb_preprocess_records(const int32_t* nbr, int32_t n_links, int64_t stride, uint32_t* rec,
                            int64_t* n_sentinel);
 
+/* Interpolated-wall (BFL) tables of a geometry (host only): the site form hlb_set_wall_distance
+ * builds for the step kernels, exposed so that it can be checked without a GPU. A link p
+ * (1 .. n_links) of internal site i is interpolated when nbr[p-1][i] is a solid wall, the pull
+ * source of opp(p) -- the site behind i -- is fluid, and 0 < d <= 1 is given for it, d =
+ * d27[canon_of_site[i]][(1 - c_pz) * 9 + (1 - c_py) * 3 + (1 - c_px)] (the wall lies along -c_p).
+ * opp(p) = ((p - 1) ^ 1) + 1, so links 2k + 1 and 2k + 2 form opposite pair k; the two links of a
+ * pair are never both interpolated.
+ *   index: HOST [stride/32][2] uint32 {bits, rank}: bit l of bits marks site 32 g + l as carrying
+ *          an interpolated link; its row is rank + popcount(bits below l). May be NULL.
+ *   coef:  HOST [coef_rows][row] doubles, row = ((n_links / 2 + 2) / 2) * 2 (8 for D3Q15, 10 for
+ *          D3Q19): entries 0 .. n_links/2 - 1 are one coefficient per pair -- +(1 - 2d) for a
+ *          d < 1/2 link (applied to the gathered value), -(1 - 1/(2d)) for a d >= 1/2 link (applied
+ *          to the value written back), 0 without an interpolated link --, entry n_links/2 holds a
+ *          64-bit word whose bit k is set when the link of pair k is 2k + 2 (else 2k + 1). May be
+ *          NULL; else coef_rows must be at least the number of flagged sites (HLB_EINVAL).
+ *   n_flagged, n_interpolated: sites with a row / interpolated links (may be NULL) */
+int hlb_preprocess_bfl(const int32_t* nbr, const int32_t* canon_of_site, int32_t n_links, int64_t n_sites,
+                       int64_t stride, const double* d27, uint32_t* index, double* coef, int64_t coef_rows,
+                       int64_t* n_flagged, int64_t* n_interpolated);
+
 #ifdef __cplusplus
 }
 #endif

@@ -120,6 +120,8 @@ def _load() -> ctypes.CDLL:
         "hlb_offset_bits": (c_int, [vp]),
         "hlb_record_sentinel_fraction": (ctypes.c_double, [vp]),
         "hlb_preprocess_records": (c_int, [vp, ctypes.c_int32, i64, vp, ctypes.POINTER(i64)]),
+        "hlb_preprocess_bfl": (c_int, [vp, vp, ctypes.c_int32, i64, i64, vp, vp, vp, i64,
+                                      ctypes.POINTER(i64), ctypes.POINTER(i64)]),
         "hlb_geometry_destroy": (None, [vp]),
         "hlb_last_error": (ctypes.c_char_p, []),
         "hlb_velocity_set": (None, [vp, vp, vp]),
@@ -146,7 +148,7 @@ EXPORTED = ("hlb_geometry_create", "hlb_set_state", "hlb_set_iolet_density",
             "hlb_device_bytes", "hlb_launch_count", "hlb_uses_records", "hlb_uses_aa", "hlb_offset_bits",
             "hlb_record_sentinel_fraction", "hlb_geometry_destroy", "hlb_last_error",
             "hlb_velocity_set", "hlb_preprocess_count", "hlb_preprocess_tables",
-            "hlb_preprocess_records")
+            "hlb_preprocess_records", "hlb_preprocess_bfl")
 
 
 def hlb_last_error() -> str:
@@ -245,6 +247,29 @@ def hlb_preprocess_records(nbr):
     n = ctypes.c_int64(0)
     _check(_lib.hlb_preprocess_records(_ptr(nbr), nl, ns, _ptr(rec), ctypes.byref(n)))
     return rec, n.value
+
+
+def hlb_preprocess_bfl(nbr, canon_of_site, d27):
+    """Site form of the interpolated-wall tables (host only): dict(index [Ns/32, 2] uint32,
+    coef [n_flagged, row] float64, n_flagged, n_interpolated); see include/hlb.h."""
+    nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+    canon = np.ascontiguousarray(canon_of_site, dtype=np.int32)
+    d27 = np.ascontiguousarray(d27, dtype=np.float64)
+    if nbr.ndim != 2 or nbr.shape[0] not in (14, 18):
+        raise ValueError("nbr must be [14, Ns] or [18, Ns]")
+    nl, ns = nbr.shape
+    n = canon.shape[0]
+    if d27.shape != (n, 27):
+        raise ValueError("d27 must be [N, 27]")
+    nf, ni = ctypes.c_int64(0), ctypes.c_int64(0)
+    index = np.zeros((ns // 32, 2), dtype=np.uint32)
+    _check(_lib.hlb_preprocess_bfl(_ptr(nbr), _ptr(canon), nl, n, ns, _ptr(d27), _ptr(index), None, 0,
+                                   ctypes.byref(nf), ctypes.byref(ni)))
+    row = ((nl // 2 + 2) // 2) * 2
+    coef = np.zeros((max(nf.value, 1), row), dtype=np.float64)
+    _check(_lib.hlb_preprocess_bfl(_ptr(nbr), _ptr(canon), nl, n, ns, _ptr(d27), None, _ptr(coef), coef.shape[0],
+                                   None, None))
+    return {"index": index, "coef": coef[:nf.value], "n_flagged": nf.value, "n_interpolated": ni.value}
 
 
 class Geometry:

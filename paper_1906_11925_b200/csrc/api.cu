@@ -299,6 +299,25 @@ int hlb_preprocess_records(const int32_t* nbr, int32_t n_links, int64_t stride, 
   return HLB_OK;
 }
 
+int hlb_preprocess_bfl(const int32_t* nbr, const int32_t* canon_of_site, int32_t n_links, int64_t n_sites,
+                       int64_t stride, const double* d27, uint32_t* index, double* coef, int64_t coef_rows,
+                       int64_t* n_flagged, int64_t* n_interpolated) {
+  if (!nbr || !canon_of_site || !d27) return fail(HLB_EINVAL, "NULL argument");
+  if (n_links != 14 && n_links != 18) return fail(HLB_EINVAL, "n_links must be 14 (D3Q15) or 18 (D3Q19)");
+  if (stride <= 0 || stride % 32 || n_sites < 0 || n_sites > stride)
+    return fail(HLB_EINVAL, "stride must be a positive multiple of 32 and at least n_sites");
+  BflTables bt;
+  build_bfl_tables(nbr, canon_of_site, n_links + 1, n_sites, stride, d27, bt);
+  if (n_flagged) *n_flagged = bt.n_sites;
+  if (n_interpolated) *n_interpolated = (int64_t)bt.site.size();
+  if (index) std::memcpy(index, bt.index.data(), sizeof(uint32_t) * bt.index.size());
+  if (coef) {
+    if (coef_rows < bt.n_sites) return fail(HLB_EINVAL, "coef_rows is smaller than the number of flagged sites");
+    std::memcpy(coef, bt.coef.data(), sizeof(double) * bt.row * (size_t)bt.n_sites);
+  }
+  return HLB_OK;
+}
+
 int hlb_geometry_create(const uint8_t* site_type, const hlb_params* p, hlb_geometry** out) {
   if (out) *out = nullptr;
   if (!out) return fail(HLB_EINVAL, "out is NULL");
@@ -581,91 +600,30 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
   }
   const int Q = g->Q;
   const int64_t N = g->N, Ns = g->Ns;
-  const LatticeDesc& lat = lattice_desc(Q == 19);
   // the link table and the canonical ranks live on the device only: fetch them
   std::vector<int32_t> nbr((size_t)(Q - 1) * (size_t)Ns), canon((size_t)N);
   HLB_CUDA(cudaStreamSynchronize(g->stream));
   HLB_CUDA(cudaMemcpy(nbr.data(), g->dg.nbr, sizeof(int32_t) * nbr.size(), cudaMemcpyDeviceToHost));
   HLB_CUDA(cudaMemcpy(canon.data(), g->dg.canon, sizeof(int32_t) * canon.size(), cudaMemcpyDeviceToHost));
-  // Every interpolated link, link-major (all links of direction 1, then 2, ...; sites
-  // ascending within each).
-  std::vector<int32_t> a_site, a_behind;
-  std::vector<uint8_t> a_link;
-  std::vector<double> a_d;
-  std::vector<uint32_t> bits((size_t)(Ns / 32), 0u);
-  {
-    // threaded over chunks of sites (multiples of 32: a word of `bits` has one writer); the
-    // chunks' finds are concatenated in order, so the list is the same for any thread count
-    struct Found { std::vector<int32_t> site, behind; std::vector<uint8_t> link; std::vector<double> d; };
-    const int64_t grain = 1 << 16;
-    const int64_t nchunks = (N + grain - 1) / grain;
-    std::vector<Found> found((size_t)nchunks);
-    for (int p = 1; p < Q; ++p) {
-      // the wall lies along -c_p
-      const int idx = (-lat.c[p][2] + 1) * 9 + (-lat.c[p][1] + 1) * 3 + (-lat.c[p][0] + 1);
-      const int32_t* e_row = nbr.data() + (size_t)(p - 1) * (size_t)Ns;
-      const int32_t* b_row = nbr.data() + (size_t)(opp(p) - 1) * (size_t)Ns;
-      host_parallel_for(N, grain, [&](int64_t b, int64_t e) {
-        Found& f = found[(size_t)(b / grain)];
-        f.site.clear(); f.behind.clear(); f.link.clear(); f.d.clear();
-        for (int64_t i = b; i < e; ++i) {
-          // a solid-wall link with a fluid site behind the site
-          if (e_row[i] != (int32_t)NBR_WALL_BIT || b_row[i] < 0) continue;
-          const double dd = d27[(size_t)canon[(size_t)i] * 27 + (size_t)idx];
-          if (dd > 0.0 && dd <= 1.0) {
-            f.site.push_back((int32_t)i);
-            f.behind.push_back(b_row[i]);
-            f.link.push_back((uint8_t)p);
-            f.d.push_back(dd);
-            bits[(size_t)(i >> 5)] |= 1u << (i & 31);
-          }
-        }
-      });
-      for (const Found& f : found) {
-        a_site.insert(a_site.end(), f.site.begin(), f.site.end());
-        a_behind.insert(a_behind.end(), f.behind.begin(), f.behind.end());
-        a_link.insert(a_link.end(), f.link.begin(), f.link.end());
-        a_d.insert(a_d.end(), f.d.begin(), f.d.end());
-      }
-    }
-  }
-  // site form for the step kernels (BflFused in kernels.cuh)
-  std::vector<int32_t> rank(bits.size());
-  int64_t n_sites = 0;
-  for (size_t w = 0; w < bits.size(); ++w) {
-    rank[w] = (int32_t)n_sites;
-    n_sites += __builtin_popcount(bits[w]);
-  }
-  const size_t nf = (size_t)((n_sites + 31) / 32 * 32 + 32);
-  const size_t row = (size_t)bfl_row_doubles(Q == 19);
-  std::vector<double> coef(row * nf, 0.0);
-  std::vector<uint32_t> member(nf, 0u);
+  BflTables bt;
+  build_bfl_tables(nbr.data(), canon.data(), Q, N, Ns, d27, bt);
+  if (bt.row != (size_t)bfl_row_doubles(Q == 19)) return fail(HLB_EINVAL, "internal: BFL row size mismatch");
+  const int64_t n_sites = bt.n_sites;
+  const size_t nf = bt.nf;
+  const std::vector<double>& coef = bt.coef;
+  const std::vector<int32_t>& a_site = bt.site;
   // list form for the read-out pre-pass: the links with d < 1/2 only (the others are already
   // in what the step kernels write)
   std::vector<int32_t> l_site, l_behind;
   std::vector<uint8_t> l_link;
   std::vector<double> l_d;
-  for (size_t l = 0; l < a_site.size(); ++l) {
-    const int64_t i = a_site[l];
-    const size_t at = (size_t)rank[(size_t)(i >> 5)] +
-                      (size_t)__builtin_popcount(bits[(size_t)(i >> 5)] & ((1u << (i & 31)) - 1u));
-    const double dd = a_d[l];
-    // one coefficient per opposite pair (2k + 1, 2k + 2) -- its two links are never both
-    // interpolated: each needs the site on the other side to be fluid -- and the member word
-    const size_t k = (size_t)(a_link[l] - 1) / 2;
-    coef[at * row + k] = dd < 0.5 ? 1.0 - 2.0 * dd : -(1.0 - 1.0 / (2.0 * dd));  // +-(1 - a), kernels.cu
-    if ((a_link[l] - 1) & 1) member[at] |= 1u << k;
-    if (dd < 0.5) {
-      l_site.push_back(a_site[l]);
-      l_behind.push_back(a_behind[l]);
-      l_link.push_back(a_link[l]);
-      l_d.push_back(dd);
+  for (size_t l = 0; l < bt.site.size(); ++l)
+    if (bt.d[l] < 0.5) {
+      l_site.push_back(bt.site[l]);
+      l_behind.push_back(bt.behind[l]);
+      l_link.push_back(bt.link[l]);
+      l_d.push_back(bt.d[l]);
     }
-  }
-  for (size_t at = 0; at < nf; ++at) {  // the member word sits behind the (Q-1)/2 coefficients of the row
-    const uint64_t word = member[at];
-    std::memcpy(&coef[at * row + (size_t)(Q - 1) / 2], &word, sizeof(double));
-  }
   const size_t nl = l_site.size();
   void *d_site = nullptr, *d_behind = nullptr, *d_link = nullptr, *d_d = nullptr;
   void *d_bits = nullptr, *d_rank = nullptr, *d_coef = nullptr;
@@ -681,14 +639,14 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
     if ((rc = g->alloc(sizeof(int32_t) * cap, &d_behind))) return rc;
     if ((rc = g->alloc(sizeof(uint8_t) * cap, &d_link))) return rc;
     if ((rc = g->alloc(sizeof(double) * cap, &d_d))) return rc;
-    if ((rc = g->alloc(sizeof(uint32_t) * 2 * bits.size(), &d_bits))) return rc;  // {bits, rank} words
+    if ((rc = g->alloc(sizeof(uint32_t) * bt.index.size(), &d_bits))) return rc;  // {bits, rank} words
     if ((rc = g->alloc(sizeof(double) * coef.size(), &d_coef))) return rc;
     void* mem[7] = {d_site, d_behind, d_link, d_d, d_bits, d_rank, d_coef};
     if (g->bfl_mem[0]) {  // smaller tables of an earlier call
       HLB_CUDA(cudaStreamSynchronize(g->stream));
       const size_t old_bytes[7] = {sizeof(int32_t) * g->bfl_cap_links, sizeof(int32_t) * g->bfl_cap_links,
                                    sizeof(uint8_t) * g->bfl_cap_links, sizeof(double) * g->bfl_cap_links,
-                                   sizeof(uint32_t) * 2 * bits.size(), 0,
+                                   sizeof(uint32_t) * bt.index.size(), 0,
                                    sizeof(double) * g->bfl_cap_coef};
       for (int k = 0; k < 7; ++k) g->release(g->bfl_mem[k], old_bytes[k]);
     }
@@ -702,11 +660,7 @@ int hlb_set_wall_distance(hlb_geometry* g, const double* d27) {
     HLB_CUDA(cudaMemcpy(d_link, l_link.data(), sizeof(uint8_t) * nl, cudaMemcpyHostToDevice));
     HLB_CUDA(cudaMemcpy(d_d, l_d.data(), sizeof(double) * nl, cudaMemcpyHostToDevice));
   }
-  {
-    std::vector<uint32_t> words(2 * bits.size());
-    for (size_t w = 0; w < bits.size(); ++w) { words[2 * w] = bits[w]; words[2 * w + 1] = (uint32_t)rank[w]; }
-    HLB_CUDA(cudaMemcpy(d_bits, words.data(), sizeof(uint32_t) * words.size(), cudaMemcpyHostToDevice));
-  }
+  HLB_CUDA(cudaMemcpy(d_bits, bt.index.data(), sizeof(uint32_t) * bt.index.size(), cudaMemcpyHostToDevice));
   HLB_CUDA(cudaMemcpy(d_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice));
   g->dg.bfl.site = (const int32_t*)d_site;
   g->dg.bfl.behind = (const int32_t*)d_behind;

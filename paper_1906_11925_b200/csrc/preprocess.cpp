@@ -402,4 +402,76 @@ int preprocess(const uint8_t* type, int nx, int ny, int nz, unsigned periodic, i
   return HLB_OK;
 }
 
+void build_bfl_tables(const int32_t* nbr, const int32_t* canon, int Q, int64_t N, int64_t Ns,
+                      const double* d27, BflTables& out) {
+  const LatticeDesc& lat = lattice_desc(Q == 19);
+  out = BflTables();
+  std::vector<uint32_t> bits((size_t)(Ns / 32), 0u);
+  {
+    // threaded over chunks of sites (multiples of 32: a word of `bits` has one writer); the
+    // chunks' finds are concatenated in order, so the list is the same for any thread count
+    struct Found { std::vector<int32_t> site, behind; std::vector<uint8_t> link; std::vector<double> d; };
+    const int64_t grain = 1 << 16;
+    const int64_t nchunks = (N + grain - 1) / grain;
+    std::vector<Found> found((size_t)nchunks);
+    for (int p = 1; p < Q; ++p) {
+      // the wall lies along -c_p
+      const int idx = (-lat.c[p][2] + 1) * 9 + (-lat.c[p][1] + 1) * 3 + (-lat.c[p][0] + 1);
+      const int32_t* e_row = nbr + (size_t)(p - 1) * (size_t)Ns;
+      const int32_t* b_row = nbr + (size_t)(opp(p) - 1) * (size_t)Ns;
+      host_parallel_for(N, grain, [&](int64_t b, int64_t e) {
+        Found& f = found[(size_t)(b / grain)];
+        f.site.clear(); f.behind.clear(); f.link.clear(); f.d.clear();
+        for (int64_t i = b; i < e; ++i) {
+          // a solid-wall link with a fluid site behind the site
+          if (e_row[i] != (int32_t)NBR_WALL_BIT || b_row[i] < 0) continue;
+          const double dd = d27[(size_t)canon[(size_t)i] * 27 + (size_t)idx];
+          if (dd > 0.0 && dd <= 1.0) {
+            f.site.push_back((int32_t)i);
+            f.behind.push_back(b_row[i]);
+            f.link.push_back((uint8_t)p);
+            f.d.push_back(dd);
+            bits[(size_t)(i >> 5)] |= 1u << (i & 31);
+          }
+        }
+      });
+      for (const Found& f : found) {
+        out.site.insert(out.site.end(), f.site.begin(), f.site.end());
+        out.behind.insert(out.behind.end(), f.behind.begin(), f.behind.end());
+        out.link.insert(out.link.end(), f.link.begin(), f.link.end());
+        out.d.insert(out.d.end(), f.d.begin(), f.d.end());
+      }
+    }
+  }
+  std::vector<int32_t> rank(bits.size());
+  for (size_t w = 0; w < bits.size(); ++w) {
+    rank[w] = (int32_t)out.n_sites;
+    out.n_sites += __builtin_popcount(bits[w]);
+  }
+  out.nf = (size_t)((out.n_sites + 31) / 32 * 32 + 32);
+  out.row = bfl_row_of(Q);
+  out.coef.assign(out.row * out.nf, 0.0);
+  std::vector<uint32_t> member(out.nf, 0u);
+  for (size_t l = 0; l < out.site.size(); ++l) {
+    const int64_t i = out.site[l];
+    const size_t at = (size_t)rank[(size_t)(i >> 5)] +
+                      (size_t)__builtin_popcount(bits[(size_t)(i >> 5)] & ((1u << (i & 31)) - 1u));
+    const double dd = out.d[l];
+    // one coefficient per opposite pair (2k + 1, 2k + 2) -- its two links are never both
+    // interpolated: each needs the site on the other side to be fluid -- and the member word
+    const size_t k = (size_t)(out.link[l] - 1) / 2;
+    out.coef[at * out.row + k] = dd < 0.5 ? 1.0 - 2.0 * dd : -(1.0 - 1.0 / (2.0 * dd));  // +-(1 - a), kernels.cu
+    if ((out.link[l] - 1) & 1) member[at] |= 1u << k;
+  }
+  for (size_t at = 0; at < out.nf; ++at) {  // the member word sits behind the (Q-1)/2 coefficients of the row
+    const uint64_t word = member[at];
+    std::memcpy(&out.coef[at * out.row + (size_t)(Q - 1) / 2], &word, sizeof(double));
+  }
+  out.index.resize(2 * bits.size());
+  for (size_t w = 0; w < bits.size(); ++w) {
+    out.index[2 * w] = bits[w];
+    out.index[2 * w + 1] = (uint32_t)rank[w];
+  }
+}
+
 }  // namespace hlb

@@ -49,6 +49,25 @@ int preprocess_threads();
 // fn(begin, end) over [0, n) in chunks of `grain`, dynamically scheduled on the preprocessor's
 // host threads (HLB_THREADS, else the hardware concurrency); also used by the set-up calls of
 // the API that loop over all sites.
+// Interpolated-wall (BFL) tables, built from the pull table and the wall distances
+// (hlb_set_wall_distance; include/hlb.h, hlb_preprocess_bfl). A link p of site i is
+// interpolated when its table entry is a solid wall, the site behind (the pull source of
+// opp(p)) is fluid, and 0 < d <= 1 is given for it.
+struct BflTables {
+  // every interpolated link, link-major (all of direction 1, then 2, ...; sites ascending)
+  std::vector<int32_t> site, behind;
+  std::vector<uint8_t> link;
+  std::vector<double> d;
+  // site form for the step kernels (BflFused in kernels.cuh)
+  std::vector<uint32_t> index;  // [Ns/32][2] {bits, rank}
+  std::vector<double> coef;     // [nf][row]
+  int64_t n_sites = 0;          // sites with at least one interpolated link
+  size_t row = 0, nf = 0;       // doubles per row; rows allocated (n_sites rounded up + 32)
+};
+inline size_t bfl_row_of(int Q) { return (size_t)(((Q - 1) / 2 + 2) / 2 * 2); }
+void build_bfl_tables(const int32_t* nbr, const int32_t* canon, int Q, int64_t N, int64_t Ns,
+                      const double* d27, BflTables& out);
+
 void host_parallel_for(int64_t n, int64_t grain, const std::function<void(int64_t, int64_t)>& fn);
 
 }  // namespace hlb

@@ -222,3 +222,67 @@ def test_link_records_argument_errors():
         hlb.hlb_preprocess_records(np.zeros((14, 33), dtype=np.int32))
     with pytest.raises(ValueError):
         hlb.hlb_preprocess_records(np.zeros((13, 32), dtype=np.int32))
+
+
+# ------------------------------------------------------------- interpolated-wall (BFL) tables
+@pytest.mark.parametrize("lattice", ["d3q15", "d3q19"])
+@pytest.mark.parametrize("seed,periodic,shape", [(0, 0, (7, 6, 5)), (1, 7, (9, 8, 10)), (2, 1, (40, 5, 4)),
+                                                 (3, 0, (1, 1, 3)), (4, 5, (37, 9, 6))])
+def test_bfl_tables_against_brute_force(seed, periodic, shape, lattice):
+    """include/hlb.h, hlb_preprocess_bfl: the per-site rows the step kernels read (one coefficient
+    per opposite pair + the member word) decoded back into (site, link) -> coefficient and compared
+    with the rule written out link by link from the table, the voxel types and the distances --
+    including distances outside (0, 1] (ignored), one-voxel channels (both links of a pair at a
+    wall: neither has a fluid site behind, plain bounce-back) and d = 1/2 (coefficient -0.0)."""
+    flags = {"d3q15": hlb.HLB_LATTICE_D3Q15, "d3q19": hlb.HLB_LATTICE_D3Q19}[lattice]
+    wl = W.random_mask(shape, p_fluid=0.6, n_iolets=2, p_iolet=0.06, periodic=periodic, seed=300 + seed)
+    t = hlb.hlb_preprocess(wl.site_type, wl.periodic, wl.n_iolets, flags | hlb.HLB_ORDER_MORTON)
+    c, w, opp = hlb.hlb_lattice(flags)
+    nq, n, nbr, canon = len(w), t["N"], t["nbr"], t["canon_of_site"]
+    rng = np.random.default_rng(seed)
+    d27 = rng.uniform(-0.3, 1.3, size=(n, 27))
+    d27[rng.random((n, 27)) < 0.1] = 0.5
+    got = hlb.hlb_preprocess_bfl(nbr, canon, d27)
+    # brute force: link p of site i is interpolated iff its entry is the solid-wall code, the pull
+    # source of opp(p) is a fluid site, and 0 < d <= 1
+    want = {}
+    for i in range(n):
+        for p in range(1, nq):
+            e, behind = int(nbr[p - 1, i]), int(nbr[opp[p] - 1, i])
+            if e >= 0 or (e & 0x7fffffff) != 0 or behind < 0:
+                continue
+            idx = (1 - c[p][2]) * 9 + (1 - c[p][1]) * 3 + (1 - c[p][0])
+            d = d27[canon[i], idx]
+            if 0.0 < d <= 1.0:
+                want[(i, p)] = 1.0 - 2.0 * d if d < 0.5 else -(1.0 - 1.0 / (2.0 * d))
+    assert got["n_interpolated"] == len(want)
+    flagged = sorted({i for i, _ in want})
+    assert got["n_flagged"] == len(flagged)
+    row, pairs = got["coef"].shape[1], (nq - 1) // 2
+    assert row == {15: 8, 19: 10}[nq]
+    bits, rank = got["index"][:, 0], got["index"][:, 1]
+    seen = {}
+    for r, i in enumerate(flagged):                      # rows in ascending site order
+        g, l = i >> 5, i & 31
+        assert (int(bits[g]) >> l) & 1
+        assert int(rank[g]) + bin(int(bits[g]) & ((1 << l) - 1)).count("1") == r
+        member = int(got["coef"][r, pairs:pairs + 1].view(np.uint64)[0])
+        assert member >> pairs == 0
+        for k in range(pairs):
+            p = 2 * k + 1 + ((member >> k) & 1)
+            other = 2 * k + 2 - ((member >> k) & 1)
+            assert (i, other) not in want                # never both links of a pair
+            cf = got["coef"][r, k]
+            if (i, p) in want:
+                seen[(i, p)] = cf
+            else:
+                assert cf == 0.0 and ((member >> k) & 1) == 0
+    assert seen.keys() == want.keys()
+    for key, cf in want.items():
+        assert seen[key] == cf and np.signbit(seen[key]) == np.signbit(cf), key
+    # unflagged sites have their bit clear
+    mask = np.zeros(t["Ns"], dtype=bool)
+    mask[flagged] = True
+    unpacked = ((bits[:, None] >> np.arange(32, dtype=np.uint32)[None, :]) & 1).astype(bool).ravel()
+    assert np.array_equal(unpacked, mask)
+
