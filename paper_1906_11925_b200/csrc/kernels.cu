@@ -992,7 +992,10 @@ k_pull_resident(ST* b0, ST* b1, const int32_t* __restrict__ nbr, const uint4* __
 #ifndef HLB_READOUT_MINB
 #define HLB_READOUT_MINB 4
 #endif
-constexpr int READOUT_MINB = HLB_READOUT_MINB;
+#ifndef HLB_READOUT_MINB_Q19
+#define HLB_READOUT_MINB_Q19 3
+#endif
+template <typename L> constexpr int readout_minb() { return L::Q > 15 ? HLB_READOUT_MINB_Q19 : HLB_READOUT_MINB; }
 template <typename L, typename ST, int MODE, bool REC, typename IT>
 __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
                                                     const int32_t* __restrict__ nbr,
@@ -1014,7 +1017,7 @@ __device__ __forceinline__ void gather_precollision(const ST* __restrict__ buf,
 }
 
 template <typename L, typename ST, int MODE, bool REC, typename IT>
-__global__ void __launch_bounds__(BLOCK, READOUT_MINB)
+__global__ void __launch_bounds__(BLOCK, readout_minb<L>())
 k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec, Planes pl,
               const int32_t* __restrict__ canon, long long N, long long Ns,
               double* __restrict__ rho, double* __restrict__ u) {
@@ -1036,7 +1039,7 @@ k_macroscopic(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const
 // order xx, yy, zz, xy, xz, yz:  sigma_ab = -(1 - omega / 2) sum_q c_qa c_qb (h_q - heq_q)
 // (the shift w_q cancels in h - heq).
 template <typename L, typename ST, int MODE, bool REC, typename IT>
-__global__ void __launch_bounds__(BLOCK, READOUT_MINB)
+__global__ void __launch_bounds__(BLOCK, readout_minb<L>())
 k_stress(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec, Planes pl,
          const int32_t* __restrict__ canon, long long N, long long Ns, double omega,
          double* __restrict__ sigma) {
@@ -1084,7 +1087,7 @@ k_wall_shear_stress(const double* __restrict__ sigma, const double* __restrict__
 }
 
 template <typename L, typename ST, int MODE, bool REC, typename IT>
-__global__ void __launch_bounds__(BLOCK, READOUT_MINB)
+__global__ void __launch_bounds__(BLOCK, readout_minb<L>())
 k_get_populations(const ST* __restrict__ buf, const int32_t* __restrict__ nbr, const uint4* __restrict__ rec, Planes pl,
                   const int32_t* __restrict__ canon, long long N, long long Ns,
                   double* __restrict__ f) {
