@@ -94,14 +94,32 @@ template <typename ST, bool REC> constexpr bool odd_rec_smem() { return sizeof(S
 #ifndef HLB_BFL_GATHER_ADD
 #define HLB_BFL_GATHER_ADD 1
 #endif
+// D3Q19 with 4-byte storage (V != 2, 32-bit offsets): the populations wait in 19 registers, not
+// 38, and these kernels are latency-bound like their D3Q15 twins, so the A-A kernels take two
+// blocks more than with 8-byte storage (6; ms per launch on configs[4] / configs[3], same call:
+// even 4 blocks 1.016 / 0.139, 5: 0.918 / 0.128, 6: 0.906 / 0.128, 7: 0.919 / 0.126; odd 4: 1.280 /
+// 0.203, 5: 1.234 / 0.191, 6: 1.225 / 0.187, 7: 1.259 / 0.190). k_pull stays at 5 (6: 1.190 ->
+// 1.233, 7: 1.401). profiles/r02_tuning.md section 21.
+#ifndef HLB_Q19F_EVEN_ADD
+#define HLB_Q19F_EVEN_ADD 2
+#endif
+#ifndef HLB_Q19F_ODD_ADD
+#define HLB_Q19F_ODD_ADD 2
+#endif
+#ifndef HLB_Q19F_PULL_ADD
+#define HLB_Q19F_PULL_ADD 0
+#endif
 template <typename L, typename ST, bool REC, typename IT, int V> constexpr int odd_smem_minb_add() {
   if (V == 2 && sizeof(ST) == 8) return sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
+  if (V != 2 && sizeof(ST) == 4 && L::Q == 19 && sizeof(IT) == 4 && REC) return HLB_Q19F_ODD_ADD;
   return odd_rec_smem<ST, REC>() && L::Q == 15 && sizeof(IT) == 4 ? 1 : 0;  // (64-bit offsets: spills)
 }
 template <typename L, typename ST> constexpr int aa_even_minb() {
-  return HLB_AA_EVEN_MINB + (sizeof(ST) == 4 && L::Q == 15 ? 1 : 0) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0);
+  return HLB_AA_EVEN_MINB + (sizeof(ST) == 4 && L::Q == 15 ? 1 : 0) - (L::Q > 15 ? HLB_Q19_MINB_DROP : 0) +
+         (sizeof(ST) == 4 && L::Q == 19 ? HLB_Q19F_EVEN_ADD : 0);
 }
 template <typename L, typename ST, typename IT, int V> constexpr int bfl_pull_add() {
+  if (V != 2 && sizeof(ST) == 4 && L::Q == 19 && sizeof(IT) == 4) return HLB_Q19F_PULL_ADD;
   return V == 2 && sizeof(ST) == 8 && L::Q == 15 && sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
 }
 
@@ -1157,7 +1175,8 @@ int resident_sites_per_sm_pull(bool d3q19, bool f32) {
 }
 int resident_kernel_sites_per_sm() { return SBLOCK * RESIDENT_MINB; }
 int resident_sites_per_sm_aa(bool d3q19, bool f32) {  // of the odd (gather) kernel, the tighter of the two
-  if (d3q19) return SBLOCK * aa_odd_minb<D3Q19, true>();
+  if (d3q19) return SBLOCK * (aa_odd_minb<D3Q19, true>() +
+                              (f32 ? odd_smem_minb_add<D3Q19, float, true, uint32_t, 0>() : 0));
   return SBLOCK * (aa_odd_minb<D3Q15, true>() +
                    (f32 ? odd_smem_minb_add<D3Q15, float, true, uint32_t, 0>() : 0));
 }
