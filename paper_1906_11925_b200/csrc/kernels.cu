@@ -109,7 +109,15 @@ template <typename ST, bool REC> constexpr bool odd_rec_smem() { return sizeof(S
 #ifndef HLB_Q19F_PULL_ADD
 #define HLB_Q19F_PULL_ADD 0
 #endif
+// 64-bit offsets (above 286 M sites, or HLB_INDEX64): 14 offsets are 28 registers; at 80 the odd
+// kernel kept them in local memory (120 B of stack). One block less (96 registers): configs[4]
+// forced onto the 64-bit kernels 1.553 -> 1.442 ms per A-A step in fp64, 0.923 -> 0.862 with 4-byte
+// storage; two blocks less 1.449 / 0.909 (profiles/r02_tuning.md section 22).
+#ifndef HLB_IDX64_ODD_DROP
+#define HLB_IDX64_ODD_DROP 1
+#endif
 template <typename L, typename ST, bool REC, typename IT, int V> constexpr int odd_smem_minb_add() {
+  if (V != 2 && sizeof(IT) == 8 && L::Q == 15) return -HLB_IDX64_ODD_DROP;
   if (V == 2 && sizeof(ST) == 8) return sizeof(IT) == 4 ? HLB_BFL_GATHER_ADD : 0;
   if (V != 2 && sizeof(ST) == 4 && L::Q == 19 && sizeof(IT) == 4 && REC) return HLB_Q19F_ODD_ADD;
   return odd_rec_smem<ST, REC>() && L::Q == 15 && sizeof(IT) == 4 ? 1 : 0;  // (64-bit offsets: spills)
