@@ -90,6 +90,11 @@ def parse_args():
                          "(the ones profiles/render_inst.csv has instruction counts for)")
     ap.add_argument("--no-prefetch", action="store_true", help="HLB_NO_PREFETCH (ablation)")
     ap.add_argument("--no-pdl", action="store_true", help="HLB_NO_PDL (ablation)")
+    ap.add_argument("--index64", action="store_true",
+                    help="HLB_INDEX64: run the 64-bit-offset kernels at any size (tuning)")
+    ap.add_argument("--readouts", action="store_true",
+                    help="also time the read-out kernels (hlb_get_macroscopic_device, hlb_get_stress_device) "
+                         "after an even and after an odd step count: 'readouts' in the JSON line")
     ap.add_argument("--no-resident", action="store_true",
                     help="HLB_NO_RESIDENT (ablation: small geometries step by graph replay instead "
                          "of the resident multi-step kernel)")
@@ -380,6 +385,34 @@ def run_reference(args, rank, world):
     return 0
 
 
+def time_readouts(g, N, nq, store):
+    """Device time of the read-out kernels on the state as it stands and one LB
+    step later (A-A: own slots after an even step count, gathered after an odd one; two-lattice:
+    always gathered): CUDA events around the C-ABI call with device outputs, best of 5, and the
+    rate in the bytes the read-out has to move at least (populations + outputs)."""
+    import torch
+    pop = nq * (4 if store == "f32" else 8)
+    res = []
+    for _ in range(2):
+        for name, fn, out_bytes in (("hlb_get_macroscopic_device", g.hlb_get_macroscopic_device, 32),
+                                    ("hlb_get_stress_device", g.hlb_get_stress_device, 48)):
+            fn()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            best = 1e30
+            for _ in range(5):
+                e0.record()
+                fn()
+                e1.record()
+                torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1))
+            res.append({"call": name, "steps_done": g.hlb_steps_done(), "ms": best,
+                        "min_bytes_per_site": pop + out_bytes, "gbs": N * (pop + out_bytes) / best / 1e6})
+        g.hlb_step(1)
+    g.hlb_step(1)      # back to an even step count
+    return res
+
+
 # --------------------------------------------------------------------------- our arm
 def variant_flags(hlb, v):
     return {"aa": hlb.HLB_AA, "two_lattice": hlb.HLB_TWO_LATTICE, "auto": hlb.HLB_SCHEME_AUTO}[v["scheme"]] | \
@@ -389,7 +422,7 @@ def variant_flags(hlb, v):
         {"auto": hlb.HLB_LINKS_AUTO, "table": hlb.HLB_LINKS_TABLE,
          "records": hlb.HLB_LINKS_RECORDS}[v["links"]] | \
         (0 if v["prefetch"] else hlb.HLB_NO_PREFETCH) | (0 if v["pdl"] else hlb.HLB_NO_PDL) | \
-        (0 if v["resident"] else hlb.HLB_NO_RESIDENT) | \
+        (0 if v["resident"] else hlb.HLB_NO_RESIDENT) | (hlb.HLB_INDEX64 if v.get("index64") else 0) | \
         (hlb.HLB_LATTICE_D3Q19 if v["lattice"] == "d3q19" else hlb.HLB_LATTICE_D3Q15)
 
 
@@ -521,6 +554,8 @@ def committed_traffic(name, v, nq, kernel):
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(path):
         return None
+    if v.get("index64"):
+        return None         # other kernels (64-bit offsets) than the captured ones
     key = traffic_key(name, v, nq) + [kernel]
     for line in open(path):
         if line.startswith("#") or not line.strip():
@@ -645,6 +680,8 @@ def main():
     v = default_variant(scheme=scheme, store=args.store, lattice=args.lattice, order=args.order,
                         links=args.links, prefetch=not args.no_prefetch, pdl=not args.no_pdl,
                         resident=not args.no_resident, inlet=args.inlet, walls=args.walls)
+    if args.index64:
+        v["index64"] = True
     t_gen = time.perf_counter()
     wl = W.by_name(args.workload, small=args.small)
     t_gen = time.perf_counter() - t_gen
@@ -743,6 +780,8 @@ def main():
                               "the LB steps; hlb_wait_copies() before the clock stops"}
     if args.render > 0:
         out["render"] = time_renderer(hlb, g, wl, args.workload, args.render, args.render_view)
+    if args.readouts:
+        out["readouts"] = time_readouts(g, N, nq, args.store)
     run.close()
     sweep = args.sweep == "on" or (args.sweep == "auto" and world == 1 and args.workload == "bigtree"
                                    and not args.small and run.v == default_variant(scheme="aa"))
