@@ -79,9 +79,12 @@ def parse_args():
                          "waveform: the same, driven by a device-resident pulsatile waveform "
                          "(hlb_set_iolet_waveform, period 1000 steps); host_waveform: the same "
                          "waveform handed over by hlb_set_iolet_velocity before every LB step")
-    ap.add_argument("--walls", default="bounce_back", choices=["bounce_back", "bfl_random"],
+    ap.add_argument("--walls", default="bounce_back",
+                    choices=["bounce_back", "bfl_random", "bfl_none", "bfl_one_direction"],
                     help="bfl_random: interpolated (BFL) walls with seeded random distances on every "
-                         "wall link -- the kernel work of the paper's BFL option")
+                         "wall link -- the kernel work of the paper's BFL option; bfl_none: the kernels with "
+                         "interpolated walls but no link flagged; bfl_one_direction: d = 0.3 on the links of one "
+                         "lattice direction (the cost split of profiles/r02_tuning.md sections 12 and 15)")
     ap.add_argument("--render", type=int, default=0, metavar="PIXELS",
                     help="also time the ray-marching renderer (NEXT-4) on the final state: PIXELS x "
                          "PIXELS frames of the speed field, rotating view; adds a \"render\" object")
@@ -461,6 +464,12 @@ class Run:
                     g.hlb_set_iolet_waveform(self.wave)
         if v["walls"] == "bfl_random":
             d27 = np.random.default_rng(1906).uniform(0.05, 1.0, size=(self.N, 27))
+            g.hlb_set_wall_distance(d27)
+            del d27
+        elif v["walls"] in ("bfl_none", "bfl_one_direction"):
+            d27 = np.full((self.N, 27), -1.0)
+            if v["walls"] == "bfl_one_direction":
+                d27[:, 14] = 0.3                 # lattice vector (+1, 0, 0)
             g.hlb_set_wall_distance(d27)
             del d27
         self.wl = wl
